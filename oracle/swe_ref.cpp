@@ -1,0 +1,445 @@
+// oracle/swe_ref.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT. See oracle/swe_ref.h for scope, citations and pins.
+//
+// Plain, single-threaded, fp64. Compile with -O2 -ffp-contract=off (no FMA contraction) so that the
+// parenthesisation written here IS the arithmetic (R-14). No blocking, no fusion, no
+// reordering beyond what SURVEY.md 8(c) S0-S4 states; loops run over edges and cells in index order.
+#include "swe_ref.h"
+
+#include <cmath>
+#include <cstdio>
+#include <limits>
+#include <map>
+#include <string>
+#include <vector>
+
+namespace {
+
+struct BString {
+  int type = 0;
+  std::vector<double> params;
+  std::vector<int32_t> edges;  // members in ascending (caller) edge id = "string order"
+  // values fixed at t^n by eval_strings():
+  double Q = 0.0, sumK = 0.0, sumL = 0.0;
+};
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct swe_ref_ctx {
+  int64_t nc = 0, ne = 0;
+  double g = 9.81, h_dry = 1e-3, dt_max = std::numeric_limits<double>::infinity();
+  std::vector<double> area, invA, gn2, zb, kst;
+  std::vector<int32_t> eL, eR, ce;      // ce[3*i+k]
+  std::vector<double> nx, ny, len;      // per edge, normal from L to R  [PAPER.md:228]
+  std::vector<double> h, qx, qy;
+  std::vector<double> F1, F3, GL, GR;   // per edge, most recent step (after the limiter)
+  std::vector<double> theta;            // per cell, most recent step
+  std::map<int, BString> strings;
+  double t = 0.0, dt_last = 0.0, vol_clipped = 0.0, vol_in = 0.0, vol_out = 0.0;
+  int64_t steps_done = 0;
+  int flags = 0;
+  std::string err;
+};
+
+// ------------------------------------------------------------------------------------------------
+// S1, interior edge. PAPER.md:252 (HLLC, "Chapter 10 of [18]"), PAPER.md:254 (modified-state bed
+// slope of ref [69]); arithmetic exactly as SURVEY.md 8(c) S1 / DESIGN.md R-1, R-2, R-3.
+// ------------------------------------------------------------------------------------------------
+static void riemann_nt(double g, double heL, double unL, double utL, double zL,
+                       double heR, double unR, double utR, double zR,
+                       double *F1o, double *F3o, double *GLo, double *GRo) {
+  const double dz = zR - zL;
+  const double hsL = std::fmax(0.0, heL - std::fmax(0.0, dz));    // face depths over z* = max(zL, zR)
+  const double hsR = std::fmax(0.0, heR - std::fmax(0.0, -dz));
+  if (hsL == 0.0 && hsR == 0.0) {
+    *F1o = 0.0; *F3o = 0.0; *GLo = 0.0; *GRo = 0.0;
+    return;
+  }
+  const double cL = std::sqrt(g * hsL), cR = std::sqrt(g * hsR);
+  double SL, SR;
+  if (hsL > 0.0 && hsR > 0.0) {                  // two-rarefaction estimates
+    const double us = 0.5 * (unL + unR) + (cL - cR);
+    const double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
+    SL = std::fmin(unL - cL, us - cs);
+    SR = std::fmax(unR + cR, us + cs);
+  } else if (hsR == 0.0) {                       // dry bed on the right
+    SL = unL - cL;
+    SR = unL + 2.0 * cL;
+  } else {                                       // dry bed on the left
+    SL = unR - 2.0 * cR;
+    SR = unR + cR;
+  }
+  const double qsL = hsL * unL, qsR = hsR * unR;
+  const double pL = (0.5 * g) * (hsL * hsL), pR = (0.5 * g) * (hsR * hsR);
+  const double FL1 = qsL, FL2 = qsL * unL + pL;
+  const double FR1 = qsR, FR2 = qsR * unR + pR;
+  double F1, F2;
+  if (SL >= 0.0) {
+    F1 = FL1; F2 = FL2;
+  } else if (SR <= 0.0) {
+    F1 = FR1; F2 = FR2;
+  } else {                                       // HLL written as F_L + increment
+    const double inv = 1.0 / (SR - SL);
+    F1 = FL1 + (SL * (SR * (hsR - hsL) - (FR1 - FL1))) * inv;
+    F2 = FL2 + (SL * (SR * (qsR - qsL) - (FR2 - FL2))) * inv;
+  }
+  const double F3 = F1 * (F1 >= 0.0 ? utL : utR);  // contact wave: upwind tangential velocity
+  *F1o = F1;
+  *F3o = F3;
+  *GLo = F2 - pL;                                  // per-side hydrostatic (bed-slope) correction
+  *GRo = F2 - pR;
+}
+
+extern "C" void swe_ref_edge_flux(double g, double heL, double uL, double vL, double zL,
+                                  double heR, double uR, double vR, double zR, double nx, double ny,
+                                  double *F1o, double *F3o, double *GLo, double *GRo) {
+  const double unL = uL * nx + vL * ny, utL = vL * nx - uL * ny;
+  const double unR = uR * nx + vR * ny, utR = vR * nx - uR * ny;
+  riemann_nt(g, heL, unL, utL, zL, heR, unR, utR, zR, F1o, F3o, GLo, GRo);
+}
+
+// wall evaluated through the solver with a mirror ghost (u_n -> -u_n): used only by the pin that
+// checks the closed form in boundary_flux() against it.
+extern "C" void swe_ref_wall_flux_via_ghost(double g, double he, double un, double ut,
+                                            double *F1o, double *F3o, double *Go) {
+  double GR;
+  riemann_nt(g, he, un, ut, 0.0, he, -un, ut, 0.0, F1o, F3o, Go, &GR);
+}
+
+namespace {
+
+// fixed-shape pairwise tree in string order (R-11): pad to a power of two with zeros,
+// then add neighbours at stride 1, 2, 4, ...
+double tree_sum(std::vector<double> v) {
+  if (v.empty()) return 0.0;
+  size_t P = 1;
+  while (P < v.size()) P <<= 1;
+  v.resize(P, 0.0);
+  for (size_t s = 1; s < P; s <<= 1)
+    for (size_t i = 0; i + s < P; i += 2 * s) v[i] = v[i] + v[i + s];
+  return v[0];
+}
+
+inline double pow53(double he) {       // he^(5/3)
+  const double c3 = std::cbrt(he);
+  return (he * c3) * c3;
+}
+
+inline double kweight(double k) { return std::isfinite(k) ? k : 1.0; }
+
+double hydrograph(const std::vector<double> &p, double t) {  // piecewise linear, clamped
+  const size_t m = p.size() / 2;
+  if (m == 0) return 0.0;
+  if (t <= p[0]) return p[1];
+  if (t >= p[2 * (m - 1)]) return p[2 * (m - 1) + 1];
+  size_t k = 0;
+  while (!(p[2 * k] <= t && t < p[2 * (k + 1)])) ++k;
+  const double tk = p[2 * k], Qk = p[2 * k + 1], tk1 = p[2 * k + 2], Qk1 = p[2 * k + 3];
+  return Qk + (Qk1 - Qk) * ((t - tk) / (tk1 - tk));
+}
+
+// R-8: a cell with h <= h_dry (a thin film) keeps its water and still takes part in the hydrostatic
+// reconstruction with its depth, but carries no momentum: its velocity is 0 and it is left out of Eq. 21.
+inline bool is_wet(const swe_ref_ctx *c, int64_t i) { return c->h[i] > c->h_dry; }
+
+// S0 -- Eq. 21: rho_ij = 2 * dist(centroid, edge j) = 4|Omega_i| / (3 l_ij)
+double max_rate(const swe_ref_ctx *c) {
+  double r = 0.0;
+  for (int64_t i = 0; i < c->nc; ++i) {
+    if (!(c->h[i] > c->h_dry)) continue;
+    const double u = c->qx[i] / c->h[i], v = c->qy[i] / c->h[i];
+    const double cel = std::sqrt(c->g * c->h[i]);
+    for (int k = 0; k < 3; ++k) {
+      const int32_t e = c->ce[3 * i + k];
+      const double lam = std::fabs(u * c->nx[e] + v * c->ny[e]) + cel;
+      const double val = lam * ((0.75 * c->len[e]) * c->invA[i]);
+      if (val > r) r = val;
+    }
+  }
+  return r;
+}
+
+struct DtChoice { double dt, t_new; bool unbounded; };
+
+DtChoice choose_dt(const swe_ref_ctx *c, double cfl, double t_end) {
+  const double r = max_rate(c);
+  double dt = (r > 0.0) ? cfl / r : c->dt_max;
+  dt = std::fmin(dt, c->dt_max);
+  const double rem = t_end - c->t;
+  DtChoice o;
+  if (dt >= rem) { o.dt = rem; o.t_new = t_end; }
+  else           { o.dt = dt;  o.t_new = c->t + dt; }
+  o.unbounded = !std::isfinite(o.dt);
+  return o;
+}
+
+// boundary strings at t^n (R-11, R-12; types named at PAPER.md:342)
+void eval_strings(swe_ref_ctx *c) {
+  for (auto &kv : c->strings) {
+    BString &s = kv.second;
+    s.Q = s.sumK = s.sumL = 0.0;
+    std::vector<double> a, b;
+    if (s.type == SWE_REF_BC_INFLOW_Q) {
+      s.Q = hydrograph(s.params, c->t);
+      for (int32_t e : s.edges) {
+        const int64_t L = c->eL[e];
+        a.push_back((c->len[e] * kweight(c->kst[L])) * pow53(c->h[L]));
+        b.push_back(c->len[e]);
+      }
+      s.sumK = tree_sum(a);
+      s.sumL = tree_sum(b);
+    }
+  }
+}
+
+void boundary_flux(swe_ref_ctx *c, int64_t e) {
+  const int64_t L = c->eL[e];
+  const int code = c->eR[e];
+  const double nx = c->nx[e], ny = c->ny[e];
+  const double he = c->h[L];
+  double u = 0.0, v = 0.0;
+  if (is_wet(c, L)) { u = c->qx[L] / c->h[L]; v = c->qy[L] / c->h[L]; }
+  double F1 = 0.0, F3 = 0.0, GL = 0.0, GR = 0.0;
+  const BString *s = nullptr;
+  if (code <= -3) {
+    auto it = c->strings.find(-3 - code);
+    if (it != c->strings.end() && it->second.type != 0) s = &it->second;
+  }
+  if (code == -2) {
+    // transmissive: ghost = copy of the interior state (R-10)
+    swe_ref_edge_flux(c->g, he, u, v, c->zb[L], he, u, v, c->zb[L], nx, ny, &F1, &F3, &GL, &GR);
+  } else if (s && s->type == SWE_REF_BC_INFLOW_Q) {
+    double qe;
+    if (s->sumK > 0.0) {
+      const double Ke = (c->len[e] * kweight(c->kst[L])) * pow53(he);
+      qe = ((s->Q * Ke) / s->sumK) / c->len[e];
+    } else {
+      qe = s->Q / s->sumL;
+    }
+    F1 = -qe;
+    GL = (he > 0.0) ? (qe * qe) / he : 0.0;
+    F3 = 0.0;
+  } else if (s && s->type == SWE_REF_BC_OUTFLOW_UNIFORM) {
+    if (he > 0.0) {
+      const double sqrtS0 = std::sqrt(s->params.empty() ? 0.0 : s->params[0]);
+      const double qn = (kweight(c->kst[L]) * pow53(he)) * sqrtS0;
+      const double ut = v * nx - u * ny;
+      F1 = qn;
+      GL = (qn * qn) / he;
+      F3 = qn * ut;
+    }
+  } else {
+    // wall (default): reflective; closed form of the mirror-ghost Riemann problem (R-9):
+    // F1 = 0, F3 = 0, G = h u_n (u_n + S), S = max(c - u_n, c + u_n/2)
+    if (he > 0.0) {
+      const double un = u * nx + v * ny;
+      const double cel = std::sqrt(c->g * he);
+      const double S = std::fmax(cel - un, cel + 0.5 * un);
+      GL = (he * un) * (un + S);
+    }
+  }
+  c->F1[e] = F1; c->F3[e] = F3; c->GL[e] = GL; c->GR[e] = 0.0;
+  (void)GR;
+}
+
+void one_step(swe_ref_ctx *c, double dt, double t_new) {
+  const double g = c->g;
+  eval_strings(c);
+  // ---- S1 / S1b
+  for (int64_t e = 0; e < c->ne; ++e) {
+    const int64_t L = c->eL[e], R = c->eR[e];
+    if (R < 0) { boundary_flux(c, e); continue; }
+    const double heL = c->h[L], heR = c->h[R];
+    double uL = 0, vL = 0, uR = 0, vR = 0;
+    if (is_wet(c, L)) { uL = c->qx[L] / c->h[L]; vL = c->qy[L] / c->h[L]; }
+    if (is_wet(c, R)) { uR = c->qx[R] / c->h[R]; vR = c->qy[R] / c->h[R]; }
+    swe_ref_edge_flux(g, heL, uL, vL, c->zb[L], heR, uR, vR, c->zb[R], c->nx[e], c->ny[e],
+                      &c->F1[e], &c->F3[e], &c->GL[e], &c->GR[e]);
+  }
+  // ---- S1c draining-time limiter (R-8b): a cell may not lose more water than it holds.
+  //      theta_i = min(1, h_i |Omega_i| / (dt * sum of its outgoing l F1)); every flux component of
+  //      an edge is scaled by theta of the edge's donor cell (the cell the mass flux leaves).
+  for (int64_t i = 0; i < c->nc; ++i) {
+    double o[3];
+    for (int k = 0; k < 3; ++k) {
+      const int32_t e = c->ce[3 * i + k];
+      const double sM = (c->eL[e] == i ? 1.0 : -1.0) * (c->len[e] * c->F1[e]);
+      o[k] = std::fmax(0.0, sM);
+    }
+    const double out = ((o[0] + o[1]) + o[2]);
+    const double avail = c->h[i] * c->area[i];
+    c->theta[i] = (dt * out > avail) ? avail / (dt * out) : 1.0;
+  }
+  for (int64_t e = 0; e < c->ne; ++e) {
+    const int64_t L = c->eL[e], R = c->eR[e];
+    double th = 1.0;
+    if (c->F1[e] > 0.0) th = c->theta[L];
+    else if (c->F1[e] < 0.0 && R >= 0) th = c->theta[R];
+    if (th < 1.0) { c->F1[e] = th * c->F1[e]; c->F3[e] = th * c->F3[e]; c->GL[e] = th * c->GL[e]; c->GR[e] = th * c->GR[e]; }
+  }
+  // ---- S2 + S3 (in place: the fluxes of step n are already stored per edge)
+  for (int64_t i = 0; i < c->nc; ++i) {
+    double M[3], X[3], Y[3], s[3];
+    for (int k = 0; k < 3; ++k) {
+      const int32_t e = c->ce[3 * i + k];
+      const bool isL = (c->eL[e] == i);
+      const double G = isL ? c->GL[e] : c->GR[e];
+      const double l = c->len[e], nx = c->nx[e], ny = c->ny[e];
+      s[k] = isL ? 1.0 : -1.0;
+      M[k] = l * c->F1[e];
+      X[k] = l * (G * nx - c->F3[e] * ny);
+      Y[k] = l * (G * ny + c->F3[e] * nx);
+    }
+    const double dH = ((s[0] * M[0] + s[1] * M[1]) + s[2] * M[2]);
+    const double dX = ((s[0] * X[0] + s[1] * X[1]) + s[2] * X[2]);
+    const double dY = ((s[0] * Y[0] + s[1] * Y[1]) + s[2] * Y[2]);
+    const double a = dt * c->invA[i];
+    double hn = c->h[i] - a * dH;
+    if (hn < 0.0) { c->vol_clipped += -hn * c->area[i]; hn = 0.0; }
+    double qxn = 0.0, qyn = 0.0;
+    if (hn > c->h_dry) {
+      qxn = c->qx[i] - a * dX;
+      qyn = c->qy[i] - a * dY;
+      if (c->gn2[i] > 0.0) {   // split friction, exact integral of dq/dt = -gamma |q| q (R-5, R-6)
+        const double D = 1.0 + ((dt * c->gn2[i]) * std::sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * std::cbrt(hn));
+        qxn = qxn / D;
+        qyn = qyn / D;
+      }
+    }
+    c->h[i] = hn; c->qx[i] = qxn; c->qy[i] = qyn;
+  }
+  for (auto &kv : c->strings) {      // bookkeeping from the (limited) fluxes actually applied
+    BString &s = kv.second;
+    if (s.type == SWE_REF_BC_INFLOW_Q) c->vol_in += dt * s.Q;
+    if (s.type == SWE_REF_BC_OUTFLOW_UNIFORM) {
+      std::vector<double> a;
+      for (int32_t e : s.edges) a.push_back(c->len[e] * c->F1[e]);
+      c->vol_out += dt * tree_sum(a);
+    }
+  }
+  // ---- S4
+  c->t = t_new;
+  c->dt_last = dt;
+  c->steps_done += 1;
+}
+
+void fill_info(swe_ref_ctx *c, swe_ref_info *info) {
+  if (!info) return;
+  double vol = 0.0;
+  int64_t nwet = 0;
+  bool bad = false;
+  for (int64_t i = 0; i < c->nc; ++i) {
+    vol += c->h[i] * c->area[i];
+    if (c->h[i] > c->h_dry) ++nwet;
+    if (!std::isfinite(c->h[i]) || !std::isfinite(c->qx[i]) || !std::isfinite(c->qy[i])) bad = true;
+  }
+  if (bad) c->flags |= 1;
+  info->t = c->t; info->dt_last = c->dt_last; info->steps_done = c->steps_done; info->n_wet = nwet;
+  info->vol = vol; info->vol_clipped = c->vol_clipped; info->vol_in = c->vol_in; info->vol_out = c->vol_out;
+  info->flags = c->flags;
+}
+
+}  // namespace
+
+extern "C" int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, swe_ref_ctx **out) {
+  if (!m || !out || !m->node_xy || !m->tri || !m->edge_cell || !m->cell_edge || !m->zb || !m->kst) {
+    g_create_error = "null argument";
+    return -1;
+  }
+  swe_ref_ctx *c = new swe_ref_ctx;
+  c->nc = m->n_cells; c->ne = m->n_edges;
+  if (p) { c->g = p->g; c->h_dry = p->h_dry; c->dt_max = p->dt_max; }
+  const int64_t nc = c->nc, ne = c->ne;
+  c->area.resize(nc); c->invA.resize(nc); c->gn2.resize(nc);
+  c->zb.assign(m->zb, m->zb + nc); c->kst.assign(m->kst, m->kst + nc);
+  c->ce.assign(m->cell_edge, m->cell_edge + 3 * nc);
+  c->eL.resize(ne); c->eR.resize(ne); c->nx.resize(ne); c->ny.resize(ne); c->len.resize(ne);
+  c->h.assign(nc, 0.0); c->qx.assign(nc, 0.0); c->qy.assign(nc, 0.0);
+  c->theta.assign(nc, 1.0);
+  c->F1.assign(ne, 0.0); c->F3.assign(ne, 0.0); c->GL.assign(ne, 0.0); c->GR.assign(ne, 0.0);
+  for (int64_t e = 0; e < ne; ++e) { c->eL[e] = m->edge_cell[2 * e]; c->eR[e] = m->edge_cell[2 * e + 1]; }
+  // geometry, PAPER.md:226-228 (section 4.1, Fig. 2)
+  for (int64_t i = 0; i < nc; ++i) {
+    const int32_t *t = m->tri + 3 * i;
+    const double x0 = m->node_xy[2 * t[0]], y0 = m->node_xy[2 * t[0] + 1];
+    const double x1 = m->node_xy[2 * t[1]], y1 = m->node_xy[2 * t[1] + 1];
+    const double x2 = m->node_xy[2 * t[2]], y2 = m->node_xy[2 * t[2] + 1];
+    const double A = 0.5 * ((x1 - x0) * (y2 - y0) - (x2 - x0) * (y1 - y0));
+    if (!(A > 0.0)) { g_create_error = "cell " + std::to_string(i) + " is not counter-clockwise / has no area"; delete c; return -2; }
+    c->area[i] = A;
+    c->invA[i] = 1.0 / A;
+    const double k = m->kst[i];
+    c->gn2[i] = std::isfinite(k) ? c->g / (k * k) : 0.0;
+    for (int s = 0; s < 3; ++s) {
+      const int32_t e = c->ce[3 * i + s];
+      if (e < 0 || e >= ne) { g_create_error = "cell_edge out of range"; delete c; return -2; }
+      if (c->eL[e] == i) {               // the edge's stored normal and length come from its L cell's slot
+        const int32_t a = t[s], b = t[(s + 1) % 3];
+        const double dx = m->node_xy[2 * b] - m->node_xy[2 * a], dy = m->node_xy[2 * b + 1] - m->node_xy[2 * a + 1];
+        const double l = std::sqrt(dx * dx + dy * dy);
+        c->len[e] = l; c->nx[e] = dy / l; c->ny[e] = -dx / l;
+      } else if (c->eR[e] != i) {
+        g_create_error = "edge_cell / cell_edge tables are inconsistent at cell " + std::to_string(i);
+        delete c; return -2;
+      }
+    }
+  }
+  for (int64_t e = 0; e < ne; ++e)
+    if (c->eR[e] <= -3) c->strings[-3 - c->eR[e]].edges.push_back((int32_t)e);
+  *out = c;
+  return 0;
+}
+
+extern "C" int swe_ref_set_boundary(swe_ref_ctx *c, int string_id, int type, const double *params, int n_params) {
+  if (!c || string_id < 0) return -1;
+  BString &s = c->strings[string_id];
+  s.type = type;
+  s.params.assign(params, params + n_params);
+  return 0;
+}
+
+extern "C" int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *hu, const double *hv, double t0) {
+  if (!c || !h || !hu || !hv) return -1;
+  c->h.assign(h, h + c->nc); c->qx.assign(hu, hu + c->nc); c->qy.assign(hv, hv + c->nc);
+  c->t = t0; c->dt_last = 0.0; c->steps_done = 0; c->vol_clipped = c->vol_in = c->vol_out = 0.0; c->flags = 0;
+  return 0;
+}
+
+extern "C" int swe_ref_step(swe_ref_ctx *c, int64_t n_steps, double t_end, double cfl, swe_ref_info *info) {
+  if (!c || !(cfl > 0.0)) return -1;
+  int64_t done = 0;
+  while ((n_steps < 0 || done < n_steps) && c->t < t_end) {
+    const DtChoice d = choose_dt(c, cfl, t_end);
+    if (d.unbounded) { c->flags |= 2; break; }
+    one_step(c, d.dt, d.t_new);
+    ++done;
+  }
+  fill_info(c, info);
+  return 0;
+}
+
+extern "C" int swe_ref_get_state(swe_ref_ctx *c, double *h, double *hu, double *hv) {
+  if (!c) return -1;
+  for (int64_t i = 0; i < c->nc; ++i) { h[i] = c->h[i]; hu[i] = c->qx[i]; hv[i] = c->qy[i]; }
+  return 0;
+}
+
+extern "C" void swe_ref_destroy(swe_ref_ctx *c) { delete c; }
+
+extern "C" const char *swe_ref_last_error(const swe_ref_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+extern "C" int swe_ref_get_geometry(swe_ref_ctx *c, double *area, double *nx, double *ny, double *len) {
+  if (!c) return -1;
+  for (int64_t i = 0; i < c->nc; ++i) area[i] = c->area[i];
+  for (int64_t e = 0; e < c->ne; ++e) { nx[e] = c->nx[e]; ny[e] = c->ny[e]; len[e] = c->len[e]; }
+  return 0;
+}
+
+extern "C" int swe_ref_get_edge_flux(swe_ref_ctx *c, double *F1, double *F3, double *GL, double *GR) {
+  if (!c) return -1;
+  for (int64_t e = 0; e < c->ne; ++e) { F1[e] = c->F1[e]; F3[e] = c->F3[e]; GL[e] = c->GL[e]; GR[e] = c->GR[e]; }
+  return 0;
+}
+
+extern "C" double swe_ref_peek_dt(swe_ref_ctx *c, double cfl, double t_end) { return choose_dt(c, cfl, t_end).dt; }

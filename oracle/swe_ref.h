@@ -1,0 +1,83 @@
+/* oracle/swe_ref.h -- TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain single-threaded fp64 C++ oracle of the explicit finite-volume shallow-water step of
+ * BASEMENT v3 (arxiv 2102.12862), written from the paper and SURVEY.md section 8(c) only.
+ * It shares no code, header, table or helper with the CUDA path under paper_2102_12862_b200/.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * load this library.
+ *
+ * What is computed, per time step n (PAPER.md line / equation in brackets):
+ *   S0  dt  = min(CFL / max_i max_j (lambda_ij / rho_ij), t_end - t, dt_max)      [Eq. 21, PAPER.md:306-312]
+ *   S1  per edge: hydrostatic "modified-state" reconstruction [PAPER.md:254, ref 69]
+ *       + HLLC flux (HLL mass/normal momentum + upwinded tangential momentum)     [PAPER.md:252, ref 18 ch.10]
+ *   S2  per cell: sum over j=1..3 of l_ij F_ij                                    [Eq. 12, PAPER.md:244-250]
+ *   S3  explicit Euler update of (h, q_x, q_y) + split friction source            [Eq. 12; Eq. 2, Table 1
+ *       Strickler row PAPER.md:106-123; splitting PAPER.md:254]
+ *   S4  t += dt
+ * Readings of every point the paper leaves open are listed in DESIGN.md (R-1 ... R-18).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): hand-computed fluxes, literal Eq. 10/11 H-form
+ * identity, geometry closed forms, Ritter and Stoker dam breaks, lake at rest, mass conservation,
+ * uniform-flow normal depth, permutation invariance, restart, T6 rest level 0.364 m.
+ * "parity unpinned" items: none of the functions; but the *choice* of readings R-2 (HLLC form) and
+ * R-11 (inflow distribution) cannot be pinned against BASEMENT itself (closed source).
+ */
+#ifndef SWE_REF_H
+#define SWE_REF_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swe_ref_ctx swe_ref_ctx;
+
+typedef struct {
+  int64_t n_nodes, n_cells, n_edges;
+  const double *node_xy;      /* [n_nodes][2] */
+  const int32_t *tri;         /* [n_cells][3] CCW */
+  const int32_t *edge_cell;   /* [n_edges][2] L, R (R<0: -1 wall, -2 transmissive, -3-s string s) */
+  const int32_t *cell_edge;   /* [n_cells][3] slot k = edge (tri[k], tri[(k+1)%3]) */
+  const double *zb;           /* [n_cells] */
+  const double *kst;          /* [n_cells] Strickler k, +inf = frictionless */
+} swe_ref_mesh;
+
+typedef struct { double g, h_dry, dt_max; } swe_ref_params;
+
+typedef struct {
+  double t, dt_last;
+  int64_t steps_done, n_wet;
+  double vol, vol_clipped, vol_in, vol_out;
+  int flags;
+} swe_ref_info;
+
+enum { SWE_REF_BC_INFLOW_Q = 1, SWE_REF_BC_OUTFLOW_UNIFORM = 2 };
+
+int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, swe_ref_ctx **out);
+int swe_ref_set_boundary(swe_ref_ctx *c, int string_id, int type, const double *params, int n_params);
+int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *hu, const double *hv, double t0);
+int swe_ref_step(swe_ref_ctx *c, int64_t n_steps, double t_end, double cfl, swe_ref_info *info);
+int swe_ref_get_state(swe_ref_ctx *c, double *h, double *hu, double *hv);
+void swe_ref_destroy(swe_ref_ctx *c);
+const char *swe_ref_last_error(const swe_ref_ctx *c);
+
+/* --- inspection entry points used by the pins (not part of the 5-call boundary) --------------- */
+/* One interior-edge evaluation of S1: in = effective depths/velocities/bed of both sides and the
+ * unit normal (L -> R); out = F1 (mass), F3 (tangential momentum), GL, GR (normal momentum minus
+ * each side's hydrostatic pressure). */
+void swe_ref_edge_flux(double g, double heL, double uL, double vL, double zL,
+                       double heR, double uR, double vR, double zR, double nx, double ny,
+                       double *F1, double *F3, double *GL, double *GR);
+/* wall flux evaluated through the interior solver with a mirror ghost state (pin for the closed form) */
+void swe_ref_wall_flux_via_ghost(double g, double he, double un, double ut, double *F1, double *F3, double *G);
+/* geometry of the context: area [n_cells]; nx, ny, len [n_edges] (normal from L to R) */
+int swe_ref_get_geometry(swe_ref_ctx *c, double *area, double *nx, double *ny, double *len);
+/* per-edge outputs of the most recent step: F1, F3, GL, GR [n_edges] each */
+int swe_ref_get_edge_flux(swe_ref_ctx *c, double *F1, double *F3, double *GL, double *GR);
+/* dt that S0 would choose now for (cfl, t_end) without advancing */
+double swe_ref_peek_dt(swe_ref_ctx *c, double cfl, double t_end);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
