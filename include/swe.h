@@ -1,0 +1,146 @@
+/* include/swe.h -- C-ABI of the B200-native shallow-water hot path (libswe_b200.so).
+ *
+ * One thing is exported: the explicit finite-volume time step of the 2-D depth-averaged
+ * shallow-water equations on an unstructured triangular mesh, as BASEMENT v3 (arxiv 2102.12862)
+ * states it.  "P:n" below is line n of the paper text; "R-k" are the readings of points
+ * the paper leaves open, listed in DESIGN.md section 2.
+ *
+ *   per time step n (state U^n = (h, q_x, q_y) per cell, fp64):
+ *     S0  dt = min(CFL / max_i max_j(lambda_ij / rho_ij), t_end - t, dt_max)         Eq. 21
+ *     S1  per edge: hydrostatic ("modified-state") face depths + HLLC flux
+ *     S1c per cell: draining-time factor theta_i; edge flux x theta of its donor     R-8b
+ *     S2  per cell: sum_j l_ij F_ij in slot order                                    Eq. 12
+ *     S3  explicit Euler update + split Strickler friction                           Eq. 12; Eq. 2 P:106-111;
+ *                                                                                    Table 1
+ *     S4  t += dt
+ *
+ * Every step of the path runs in CUDA kernels compiled for sm_100a; there is no CPU fallback.  All
+ * functions return SWE_OK (0) or a negative error code; nothing throws or exits across this boundary.
+ * One context must be used by one host thread at a time.
+ */
+#ifndef SWE_B200_H
+#define SWE_B200_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swe_ctx swe_ctx; /* opaque; created by swe_create, freed by swe_destroy */
+
+enum {
+  SWE_OK = 0,
+  SWE_EINVAL = -1,     /* null / out-of-range argument                                             */
+  SWE_EMESH = -2,      /* non-CCW or zero-area cell, non-conforming mesh, inconsistent tables       */
+  SWE_ENOMEM = -3,     /* host allocation failed, or the lent workspace is too small                */
+  SWE_ECUDA = -4,      /* a CUDA call failed (no device, launch error, ...); see swe_last_error     */
+  SWE_ENONFINITE = -5  /* swe_step found a non-finite state value at the end of the call            */
+};
+
+/* Boundary codes in edge_cell[e][1] (P:332 wall is the default of every external edge) */
+enum { SWE_EDGE_WALL = -1, SWE_EDGE_TRANSMISSIVE = -2 /* , -3 - s = member of boundary string s */ };
+/* Boundary-string types for swe_set_boundary (types named at P:342; formulas are readings R-11, R-12) */
+enum { SWE_BC_NONE = 0 /* string behaves as wall */, SWE_BC_INFLOW_Q = 1, SWE_BC_OUTFLOW_UNIFORM = 2 };
+/* Cell / edge renumbering applied inside the library (invisible at this boundary) */
+enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1 };
+/* swe_step_info.flags */
+enum { SWE_FLAG_NONFINITE = 1, SWE_FLAG_DT_UNBOUNDED = 2 };
+
+/* The mesh (section 4.1, Fig. 2): conforming triangulation, cell i with neighbours j = 1..3
+ * across edges Gamma_ij.  All pointers are HOST pointers; everything is copied during swe_create and
+ * the caller may free the arrays as soon as it returns. */
+typedef struct {
+  int64_t n_nodes, n_cells, n_edges;
+  const double *node_xy;    /* [n_nodes][2]  metres                                                  */
+  const int32_t *tri;       /* [n_cells][3]  counter-clockwise node ids                              */
+  const int32_t *edge_cell; /* [n_edges][2]  [0] = L >= 0; [1] = R >= 0, or a boundary code < 0.
+                               The stored unit normal of an edge points from L to R.  May be NULL
+                               together with cell_edge: both tables are then built by the library,
+                               every boundary edge a wall, and n_edges is ignored.                   */
+  const int32_t *cell_edge; /* [n_cells][3]  slot k = edge between tri[k] and tri[(k+1)%3]           */
+  const double *zb;         /* [n_cells]     cell-mean bed elevation z_B (R-13)                      */
+  const double *kst;        /* [n_cells]     Strickler k_str (Table 1); +inf = frictionless   */
+} swe_mesh;
+
+typedef struct {
+  double g;             /* gravity; default 9.81                                                     */
+  double h_dry;         /* wet/dry threshold (R-8): cells with h <= h_dry carry no momentum; 1e-3    */
+  double dt_max;        /* upper bound of dt, used when the whole domain is dry; default +inf        */
+  int renumber;         /* SWE_RENUMBER_*; default MORTON                                            */
+  int state_on_device;  /* 0: swe_set_state/swe_get_state take HOST pointers (default);
+                           1: they take DEVICE pointers (e.g. torch tensors), read/written on stream  */
+  int steps_per_graph;  /* time steps captured per CUDA graph launch; default 32; 0 = no graph       */
+  void *cuda_stream;    /* cudaStream_t all work is enqueued on; NULL = the legacy default stream    */
+  void *workspace;      /* DEVICE memory lent by the caller for the context's lifetime (e.g. a torch
+                           uint8 tensor), 256-byte aligned, or NULL: the library then cudaMallocs   */
+  size_t workspace_bytes; /* size of workspace; must be >= swe_workspace_bytes(n_cells, n_edges)     */
+} swe_params;
+
+typedef struct {
+  double t, dt_last;           /* simulation time; dt of the most recent step                        */
+  int64_t steps_done, n_wet;   /* steps since swe_set_state; cells with h > h_dry                    */
+  double vol;                  /* sum_i h_i |Omega_i|                                                 */
+  double vol_clipped;          /* volume created by clipping residual negative depths (R-8b)         */
+  double vol_in, vol_out;      /* volume through INFLOW_Q / OUTFLOW_UNIFORM strings since set_state  */
+  int flags;                   /* SWE_FLAG_*                                                          */
+} swe_step_info;
+
+/* Fills *p with the defaults named above. */
+void swe_params_default(swe_params *p);
+
+/* Device bytes a context for a mesh of this size needs (an upper bound that also covers tables the
+ * library builds itself).  n_edges <= 0: assume the worst case 3 * n_cells. */
+size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges);
+
+/* Validates the mesh (CCW, positive area, both tables consistent and conforming), computes the geometry
+ * of section 4.1 (areas, edge lengths, unit normals L->R), renumbers cells and edges (Morton order of the
+ * centroids; slot order and L/R orientation are kept, R-15), uploads everything and captures the step graph.
+ * params == NULL: defaults.  On failure *out is NULL and swe_last_error(NULL) describes the reason. */
+int swe_create(const swe_mesh *mesh, const swe_params *params, swe_ctx **out);
+
+/* Sets type and parameters of boundary string s (the edges whose code is -3 - s).
+ *   SWE_BC_INFLOW_Q (R-11):        params = hydrograph table (t_0, Q_0, t_1, Q_1, ...), n_params even, t ascending;
+ *                                  Q(t) piecewise linear, clamped at both ends; Q in m^3/s over the whole string.
+ *   SWE_BC_OUTFLOW_UNIFORM (R-12): params = (S_0), the bed slope of the normal-depth condition.
+ * The parameters are copied. */
+int swe_set_boundary(swe_ctx *ctx, int string_id, int type, const double *params, int n_params);
+
+/* Sets the state (h, hu, hv) [n_cells] in the CALLER's cell numbering and the time t0; resets steps_done and
+ * the volume counters.  Host or device pointers according to swe_params.state_on_device. */
+int swe_set_state(swe_ctx *ctx, const double *h, const double *hu, const double *hv, double t0);
+
+/* Advances until n_steps steps are done (n_steps < 0: no limit) or t reaches t_end (+inf: no limit),
+ * whichever comes first; the last step is shortened to land on t_end exactly.  cfl in (0, 1] (default
+ * 0.9 in the paper).  All steps run on the device without host synchronisation per step; the call synchronises
+ * the stream once per chunk of steps when t_end is finite, and once at the end if info != NULL.
+ * info may be NULL.  Returns SWE_ENONFINITE if info was requested and the state holds NaN/inf. */
+int swe_step(swe_ctx *ctx, int64_t n_steps, double t_end, double cfl, swe_step_info *info);
+
+/* Reads the state in the caller's cell numbering (host or device pointers as for swe_set_state). */
+int swe_get_state(swe_ctx *ctx, double *h, double *hu, double *hv);
+
+void swe_destroy(swe_ctx *ctx);
+
+/* Message of the most recent error of ctx, or of the most recent failed swe_create if ctx == NULL.
+ * The pointer stays valid until the next failing call on the same context / thread. */
+const char *swe_last_error(const swe_ctx *ctx);
+
+/* ---- inspection entry points (used by the parity tests; HOST pointers, caller numbering, they synchronise) */
+/* area [n_cells]; nx, ny, len [n_edges]: geometry of section 4.1 as the kernels use it */
+int swe_get_geometry(swe_ctx *ctx, double *area, double *nx, double *ny, double *len);
+/* per-edge results of the most recent step, after the limiter: F1 (mass), F3 (tangential momentum),
+ * GL, GR (normal momentum minus each side's hydrostatic pressure) [n_edges]; theta [n_cells] (may be NULL) */
+int swe_get_edge_flux(swe_ctx *ctx, double *F1, double *F3, double *GL, double *GR, double *theta);
+/* dt that S0 would choose now for (cfl, t_end), without advancing */
+int swe_peek_dt(swe_ctx *ctx, double cfl, double t_end, double *dt);
+/* internal numbering: cell_perm[new] = caller cell id [n_cells]; edge_perm[new] = caller edge id [n_edges] */
+int swe_get_permutation(swe_ctx *ctx, int32_t *cell_perm, int32_t *edge_perm);
+/* edge tables as used (identical to the caller's when those were given): for meshes passed without tables */
+int swe_get_tables(swe_ctx *ctx, int64_t *n_edges, int32_t *edge_cell, int32_t *cell_edge);
+/* number of kernel launches enqueued by this context since swe_create (graph nodes count individually) */
+int64_t swe_kernel_launches(const swe_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

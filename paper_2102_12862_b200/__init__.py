@@ -1,0 +1,252 @@
+"""Thin Python binding of the C-ABI in include/swe.h (libswe_b200.so, CUDA sm_100a).
+
+Argument marshalling only: every step of the shallow-water path runs in the library's kernels.  PyTorch is
+used for device memory (the workspace tensor lent to the library, optional device-resident state tensors)
+and for the stream.  There is no CPU fallback: a missing library or a missing GPU raises.
+
+    from paper_2102_12862_b200 import Solver
+    s = Solver(node_xy, tri, edge_cell, cell_edge, zb, kst)      # swe_create
+    s.set_boundary(0, BC_INFLOW_Q, [0, 100, 3600, 2000])         # swe_set_boundary
+    s.set_state(h, hu, hv)                                       # swe_set_state
+    info = s.step(n_steps=100, cfl=0.9)                          # swe_step
+    h, hu, hv = s.get_state()                                    # swe_get_state
+    s.close()                                                    # swe_destroy
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libswe_b200.so")
+
+OK, EINVAL, EMESH, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4, -5
+EDGE_WALL, EDGE_TRANSMISSIVE = -1, -2
+BC_NONE, BC_INFLOW_Q, BC_OUTFLOW_UNIFORM = 0, 1, 2
+RENUMBER_NONE, RENUMBER_MORTON = 0, 1
+FLAG_NONFINITE, FLAG_DT_UNBOUNDED = 1, 2
+
+_f64p = C.POINTER(C.c_double)
+_i32p = C.POINTER(C.c_int32)
+
+EXPORTS = (
+    "swe_params_default", "swe_workspace_bytes", "swe_create", "swe_set_boundary", "swe_set_state", "swe_step",
+    "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
+    "swe_get_permutation", "swe_get_tables", "swe_kernel_launches",
+)
+
+
+class SweMesh(C.Structure):
+    _fields_ = [("n_nodes", C.c_int64), ("n_cells", C.c_int64), ("n_edges", C.c_int64),
+                ("node_xy", _f64p), ("tri", _i32p), ("edge_cell", _i32p), ("cell_edge", _i32p),
+                ("zb", _f64p), ("kst", _f64p)]
+
+
+class SweParams(C.Structure):
+    _fields_ = [("g", C.c_double), ("h_dry", C.c_double), ("dt_max", C.c_double), ("renumber", C.c_int),
+                ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("cuda_stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class SweStepInfo(C.Structure):
+    _fields_ = [("t", C.c_double), ("dt_last", C.c_double), ("steps_done", C.c_int64), ("n_wet", C.c_int64),
+                ("vol", C.c_double), ("vol_clipped", C.c_double), ("vol_in", C.c_double), ("vol_out", C.c_double),
+                ("flags", C.c_int)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class SweError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"swe error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Loads libswe_b200.so (built by `python -m paper_2102_12862_b200.build`); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2102_12862_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.swe_params_default.argtypes = [C.POINTER(SweParams)]
+        L.swe_params_default.restype = None
+        L.swe_workspace_bytes.argtypes = [C.c_int64, C.c_int64]
+        L.swe_workspace_bytes.restype = C.c_size_t
+        L.swe_create.argtypes = [C.POINTER(SweMesh), C.POINTER(SweParams), C.POINTER(C.c_void_p)]
+        L.swe_set_boundary.argtypes = [C.c_void_p, C.c_int, C.c_int, _f64p, C.c_int]
+        L.swe_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
+        L.swe_step.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.POINTER(SweStepInfo)]
+        L.swe_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.swe_destroy.argtypes = [C.c_void_p]
+        L.swe_destroy.restype = None
+        L.swe_last_error.argtypes = [C.c_void_p]
+        L.swe_last_error.restype = C.c_char_p
+        L.swe_get_geometry.argtypes = [C.c_void_p, _f64p, _f64p, _f64p, _f64p]
+        L.swe_get_edge_flux.argtypes = [C.c_void_p, _f64p, _f64p, _f64p, _f64p, _f64p]
+        L.swe_peek_dt.argtypes = [C.c_void_p, C.c_double, C.c_double, _f64p]
+        L.swe_get_permutation.argtypes = [C.c_void_p, _i32p, _i32p]
+        L.swe_get_tables.argtypes = [C.c_void_p, C.POINTER(C.c_int64), _i32p, _i32p]
+        L.swe_kernel_launches.argtypes = [C.c_void_p]
+        L.swe_kernel_launches.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _p(a, typ):
+    return a.ctypes.data_as(typ) if a is not None else None
+
+
+class Solver:
+    """One swe_ctx.  Mesh arrays are numpy (host); state arrays are numpy (host pointers) or, with
+    state_on_device=True, torch CUDA float64 tensors (device pointers)."""
+
+    def __init__(self, node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, *, g=9.81, h_dry=1e-3,
+                 dt_max=float("inf"), renumber=RENUMBER_MORTON, state_on_device=False, steps_per_graph=32,
+                 device="cuda:0", own_workspace=False):
+        import torch  # device memory + stream only
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2102_12862_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        L = lib()
+        self._torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        node_xy = np.ascontiguousarray(node_xy, np.float64)
+        tri = np.ascontiguousarray(tri, np.int32)
+        ec = None if edge_cell is None else np.ascontiguousarray(edge_cell, np.int32)
+        ce = None if cell_edge is None else np.ascontiguousarray(cell_edge, np.int32)
+        self.n_cells = int(tri.shape[0])
+        zb = np.ascontiguousarray(zb if zb is not None else np.zeros(self.n_cells), np.float64)
+        kst = np.ascontiguousarray(kst if kst is not None else np.full(self.n_cells, np.inf), np.float64)
+        assert zb.shape == (self.n_cells,) and kst.shape == (self.n_cells,)
+        n_edges = 0 if ec is None else int(ec.shape[0])
+        mesh = SweMesh(int(node_xy.shape[0]), self.n_cells, n_edges, _p(node_xy, _f64p), _p(tri, _i32p),
+                       _p(ec, _i32p), _p(ce, _i32p), _p(zb, _f64p), _p(kst, _f64p))
+        prm = SweParams()
+        L.swe_params_default(C.byref(prm))
+        prm.g, prm.h_dry, prm.dt_max = float(g), float(h_dry), float(dt_max)
+        prm.renumber, prm.state_on_device, prm.steps_per_graph = int(renumber), int(bool(state_on_device)), int(steps_per_graph)
+        self.stream = torch.cuda.current_stream(self.device)
+        prm.cuda_stream = self.stream.cuda_stream
+        self.workspace = None
+        if not own_workspace:
+            nbytes = int(L.swe_workspace_bytes(self.n_cells, n_edges))
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            prm.workspace, prm.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.state_on_device = bool(state_on_device)
+        h = C.c_void_p()
+        rc = L.swe_create(C.byref(mesh), C.byref(prm), C.byref(h))
+        if rc != OK:
+            raise SweError(rc, L.swe_last_error(None).decode())
+        self._h = h
+        ne = C.c_int64()
+        L.swe_get_tables(self._h, C.byref(ne), None, None)
+        self.n_edges = int(ne.value)
+
+    # ---- the five calls + boundary strings
+    def _check(self, rc):
+        if rc != OK:
+            raise SweError(rc, lib().swe_last_error(self._h).decode())
+
+    def set_boundary(self, string_id, typ, params):
+        a = np.ascontiguousarray(params, np.float64)
+        self._check(lib().swe_set_boundary(self._h, int(string_id), int(typ), _p(a, _f64p), int(a.size)))
+
+    def _ptrs(self, arrs):
+        if self.state_on_device:
+            for x in arrs:
+                assert x.is_cuda and x.dtype == self._torch.float64 and x.is_contiguous() and x.numel() == self.n_cells
+            return [C.c_void_p(x.data_ptr()) for x in arrs]
+        for x in arrs:
+            assert x.dtype == np.float64 and x.flags.c_contiguous and x.shape == (self.n_cells,)
+        return [C.c_void_p(x.ctypes.data) for x in arrs]
+
+    def set_state(self, h, hu, hv, t0=0.0):
+        if not self.state_on_device:
+            h, hu, hv = (np.ascontiguousarray(x, np.float64) for x in (h, hu, hv))
+        self._check(lib().swe_set_state(self._h, *self._ptrs((h, hu, hv)), float(t0)))
+
+    def step(self, n_steps=-1, t_end=float("inf"), cfl=0.9, info=True):
+        inf = SweStepInfo() if info else None
+        rc = lib().swe_step(self._h, int(n_steps), float(t_end), float(cfl), C.byref(inf) if info else None)
+        self._check(rc)
+        return inf.as_dict() if info else None
+
+    def get_state(self, out=None):
+        if out is None:
+            if self.state_on_device:
+                out = tuple(self._torch.empty(self.n_cells, dtype=self._torch.float64, device=self.device) for _ in range(3))
+            else:
+                out = tuple(np.empty(self.n_cells) for _ in range(3))
+        self._check(lib().swe_get_state(self._h, *self._ptrs(out)))
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().swe_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- inspection
+    def geometry(self):
+        area = np.empty(self.n_cells)
+        nx, ny, ln = (np.empty(self.n_edges) for _ in range(3))
+        self._check(lib().swe_get_geometry(self._h, _p(area, _f64p), _p(nx, _f64p), _p(ny, _f64p), _p(ln, _f64p)))
+        return area, nx, ny, ln
+
+    def edge_fluxes(self):
+        out = [np.empty(self.n_edges) for _ in range(4)]
+        theta = np.empty(self.n_cells)
+        self._check(lib().swe_get_edge_flux(self._h, *[_p(x, _f64p) for x in out], _p(theta, _f64p)))
+        return tuple(out) + (theta,)
+
+    def peek_dt(self, cfl=0.9, t_end=float("inf")):
+        dt = C.c_double()
+        self._check(lib().swe_peek_dt(self._h, float(cfl), float(t_end), C.byref(dt)))
+        return dt.value
+
+    def permutation(self):
+        cp = np.empty(self.n_cells, np.int32)
+        ep = np.empty(self.n_edges, np.int32)
+        self._check(lib().swe_get_permutation(self._h, _p(cp, _i32p), _p(ep, _i32p)))
+        return cp, ep
+
+    def tables(self):
+        ec = np.empty((self.n_edges, 2), np.int32)
+        ce = np.empty((self.n_cells, 3), np.int32)
+        self._check(lib().swe_get_tables(self._h, None, _p(ec, _i32p), _p(ce, _i32p)))
+        return ec, ce
+
+    @property
+    def kernel_launches(self):
+        return int(lib().swe_kernel_launches(self._h))
+
+
+def from_workload(w, **kw):
+    """Solver for a workloads.configs.Workload (mesh, parameters, boundary strings, initial state)."""
+    kw.setdefault("g", w.g)
+    kw.setdefault("h_dry", w.h_dry)
+    kw.setdefault("dt_max", w.dt_max)
+    s = Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst, **kw)
+    for sid, typ, params in getattr(w, "strings", []):
+        s.set_boundary(sid, typ, params)
+    if s.state_on_device:
+        import torch
+        s.set_state(*(torch.from_numpy(np.ascontiguousarray(x)).to(s.device) for x in (w.h, w.hu, w.hv)), 0.0)
+    else:
+        s.set_state(w.h, w.hu, w.hv, 0.0)
+    return s

@@ -1,0 +1,532 @@
+// C-ABI of include/swe.h: context, workspace carving, upload, CUDA-graph step loop.  Host logic only;
+// every step of the numerical path runs in the kernels of swe_kernels.cuh.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/swe.h"
+#include "mesh_prep.hpp"
+#include "swe_kernels.cuh"
+#include "swe_types.h"
+
+using namespace swe;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+// Sizes of the O(N) device arrays carved out of the workspace, in carving order.
+struct Layout {
+  size_t rec, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, total;
+  Layout(int64_t nc, int64_t ne) {
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+    rec = take(sizeof(CellRec) * nc);
+    geom = take(sizeof(EdgeGeom) * ne);
+    flux = take(sizeof(EdgeFlux) * ne);
+    cell_edge = take(sizeof(int4) * nc);
+    area = take(8 * nc); inv_area = take(8 * nc); gn2 = take(8 * nc); kst = take(8 * nc); theta = take(8 * nc);
+    cell_perm = take(4 * nc); edge_perm = take(4 * ne);
+    stage = take(24 * nc);
+    total = o;
+  }
+};
+
+inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
+
+}  // namespace
+
+struct swe_ctx {
+  int64_t nc = 0, ne = 0;
+  swe_params prm{};
+  HostMesh hm;
+  cudaStream_t stream = nullptr;
+  char *ws = nullptr;
+  bool own_ws = false;
+  // device arrays (inside ws)
+  CellRec *rec = nullptr; EdgeGeom *geom = nullptr; EdgeFlux *flux = nullptr; int4 *cell_edge = nullptr;
+  double *area = nullptr, *inv_area = nullptr, *gn2 = nullptr, *kst = nullptr, *theta = nullptr;
+  int *cell_perm = nullptr, *edge_perm = nullptr;
+  double *stage = nullptr;
+  // small device allocations owned by the library
+  Control *d_ctl = nullptr;
+  Control *h_ctl = nullptr;          // pinned
+  BoundaryString *d_strings = nullptr;
+  int *d_string_edges = nullptr;
+  double *d_scratch = nullptr;
+  std::vector<BoundaryString> strings;
+  std::vector<double *> d_params;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t graph_exec = nullptr;
+  int steps_per_graph = 0;
+  int64_t launches = 0;
+  double t_host = 0.0;               // t as of the last synchronisation
+  std::string err;
+};
+
+namespace {
+
+#define SWE_CUDA(ctx, call)                                                                       \
+  do {                                                                                            \
+    cudaError_t e_ = (call);                                                                      \
+    if (e_ != cudaSuccess) {                                                                      \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                            \
+      return SWE_ECUDA;                                                                           \
+    }                                                                                             \
+  } while (0)
+
+// the four kernels of one time step, in stream order
+void enqueue_step(swe_ctx *c, cudaStream_t s) {
+  k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
+                                           c->theta, c->rec, c->kst, 0);
+  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne);
+  k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
+                                             (int)c->nc);
+  k_cell_update<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
+                                                   c->inv_area, c->gn2, c->rec, (int)c->nc);
+}
+constexpr int kKernelsPerStep = 4;
+
+int capture_graph(swe_ctx *c) {
+  if (c->steps_per_graph <= 0) return SWE_OK;
+  cudaStream_t cap;
+  SWE_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+  SWE_CUDA(c, cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
+  for (int k = 0; k < c->steps_per_graph; ++k) enqueue_step(c, cap);
+  SWE_CUDA(c, cudaStreamEndCapture(cap, &c->graph));
+  SWE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+  SWE_CUDA(c, cudaStreamDestroy(cap));
+  return SWE_OK;
+}
+
+int read_control(swe_ctx *c) {   // device -> pinned host, synchronises the stream
+  SWE_CUDA(c, cudaMemcpyAsync(c->h_ctl, c->d_ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->t_host = c->h_ctl->t;
+  return SWE_OK;
+}
+
+void release(swe_ctx *c) {
+  if (!c) return;
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  if (c->graph) cudaGraphDestroy(c->graph);
+  for (double *p : c->d_params) if (p) cudaFree(p);
+  if (c->d_ctl) cudaFree(c->d_ctl);
+  if (c->h_ctl) cudaFreeHost(c->h_ctl);
+  if (c->d_strings) cudaFree(c->d_strings);
+  if (c->d_string_edges) cudaFree(c->d_string_edges);
+  if (c->d_scratch) cudaFree(c->d_scratch);
+  if (c->own_ws && c->ws) cudaFree(c->ws);
+  delete c;
+}
+
+int upload_strings(swe_ctx *c) {
+  if (c->strings.empty()) return SWE_OK;
+  SWE_CUDA(c, cudaMemcpyAsync(c->d_strings, c->strings.data(), sizeof(BoundaryString) * c->strings.size(),
+                              cudaMemcpyHostToDevice, c->stream));
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  return SWE_OK;
+}
+
+// sum of the member lengths of every string, by the same pairwise tree as the per-step sums
+__global__ void __launch_bounds__(kCtlThreads)
+k_string_lengths(BoundaryString *strings, int n_strings, const int *__restrict__ string_edges, double *scratch,
+                 const EdgeGeom *__restrict__ geom) {
+  for (int s = 0; s < n_strings; ++s) {
+    BoundaryString &bs = strings[s];
+    if (bs.n_edges == 0) continue;
+    double *v = scratch + bs.scratch;
+    for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) v[j] = j < bs.n_edges ? geom[string_edges[bs.first + j]].len : 0.0;
+    const double sum = block_tree_sum(v, bs.pow2);
+    if (threadIdx.x == 0) bs.sumL = sum;
+    __syncthreads();
+  }
+}
+
+int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
+  const int64_t nc = mesh->n_cells, nn = mesh->n_nodes;
+  c->nc = nc;
+  if (params) c->prm = *params; else swe_params_default(&c->prm);
+  const swe_params &p = c->prm;
+  if (!(p.g > 0.0) || !(p.h_dry >= 0.0) || !(p.dt_max > 0.0)) { c->err = "g, h_dry, dt_max out of range"; return SWE_EINVAL; }
+  c->stream = (cudaStream_t)p.cuda_stream;
+  c->steps_per_graph = p.steps_per_graph;
+
+  // ---- tables, validation, geometry, numbering (host)
+  HostMesh &hm = c->hm;
+  hm.nc = nc; hm.nn = nn;
+  if (mesh->edge_cell && mesh->cell_edge) {
+    if (mesh->n_edges <= 0 || mesh->n_edges > 3 * nc) { c->err = "n_edges out of range"; return SWE_EINVAL; }
+    hm.ne = mesh->n_edges;
+    hm.edge_cell.assign(mesh->edge_cell, mesh->edge_cell + 2 * hm.ne);
+    hm.cell_edge.assign(mesh->cell_edge, mesh->cell_edge + 3 * nc);
+  } else if (!mesh->edge_cell && !mesh->cell_edge) {
+    if (!build_tables(nc, nn, mesh->tri, hm, c->err)) return SWE_EMESH;
+  } else {
+    c->err = "edge_cell and cell_edge must be given together or both be NULL";
+    return SWE_EINVAL;
+  }
+  if (!validate_and_measure(nc, nn, mesh->node_xy, mesh->tri, hm, c->err)) return SWE_EMESH;
+  for (int64_t i = 0; i < nc; ++i) {
+    const double k = mesh->kst[i];
+    if (!(k > 0.0) || !std::isfinite(mesh->zb[i])) { c->err = "cell " + std::to_string(i) + ": kst must be > 0 (or +inf), zb finite"; return SWE_EINVAL; }
+  }
+  renumber(p.renumber, nc, mesh->node_xy, mesh->tri, hm);
+  const int64_t ne = c->ne = hm.ne;
+
+  // ---- workspace
+  const Layout lay(nc, ne);
+  if (p.workspace) {
+    if (p.workspace_bytes < lay.total) { c->err = "workspace too small: need " + std::to_string(lay.total) + " bytes"; return SWE_ENOMEM; }
+    if (((uintptr_t)p.workspace) % kAlign != 0) { c->err = "workspace must be 256-byte aligned"; return SWE_EINVAL; }
+    c->ws = (char *)p.workspace;
+  } else {
+    SWE_CUDA(c, cudaMalloc((void **)&c->ws, lay.total));
+    c->own_ws = true;
+  }
+  c->rec = (CellRec *)(c->ws + lay.rec); c->geom = (EdgeGeom *)(c->ws + lay.geom); c->flux = (EdgeFlux *)(c->ws + lay.flux);
+  c->cell_edge = (int4 *)(c->ws + lay.cell_edge);
+  c->area = (double *)(c->ws + lay.area); c->inv_area = (double *)(c->ws + lay.inv_area);
+  c->gn2 = (double *)(c->ws + lay.gn2); c->kst = (double *)(c->ws + lay.kst); c->theta = (double *)(c->ws + lay.theta);
+  c->cell_perm = (int *)(c->ws + lay.cell_perm); c->edge_perm = (int *)(c->ws + lay.edge_perm);
+  c->stage = (double *)(c->ws + lay.stage);
+
+  // ---- arrays in internal numbering
+  {
+    std::vector<CellRec> rec(nc);
+    std::vector<int4> ce(nc);
+    std::vector<double> area(nc), inv_area(nc), gn2(nc), kst(nc), theta(nc, 1.0);
+    for (int64_t i = 0; i < nc; ++i) {
+      const int32_t o = hm.cell_perm[i];
+      rec[i] = {0.0, 0.0, 0.0, mesh->zb[o]};
+      ce[i] = make_int4(hm.edge_new[hm.cell_edge[3 * o]], hm.edge_new[hm.cell_edge[3 * o + 1]],
+                        hm.edge_new[hm.cell_edge[3 * o + 2]], 0);
+      const double A = hm.area[o], k = mesh->kst[o];
+      area[i] = A;
+      inv_area[i] = 1.0 / A;
+      gn2[i] = std::isfinite(k) ? p.g / (k * k) : 0.0;    // g / k_str^2 (Eq. 2 P:106-111 with Table 1, R-6)
+      kst[i] = k;
+    }
+    std::vector<EdgeGeom> geom(ne);
+    for (int64_t e = 0; e < ne; ++e) {
+      const int32_t o = hm.edge_perm[e];
+      const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
+      geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
+    }
+    auto up = [&](void *dst, const void *src, size_t bytes) { return cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice); };
+    SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
+    SWE_CUDA(c, up(c->cell_edge, ce.data(), sizeof(int4) * nc));
+    SWE_CUDA(c, up(c->area, area.data(), 8 * nc));
+    SWE_CUDA(c, up(c->inv_area, inv_area.data(), 8 * nc));
+    SWE_CUDA(c, up(c->gn2, gn2.data(), 8 * nc));
+    SWE_CUDA(c, up(c->kst, kst.data(), 8 * nc));
+    SWE_CUDA(c, up(c->theta, theta.data(), 8 * nc));
+    SWE_CUDA(c, up(c->geom, geom.data(), sizeof(EdgeGeom) * ne));
+    SWE_CUDA(c, up(c->cell_perm, hm.cell_perm.data(), 4 * nc));
+    SWE_CUDA(c, up(c->edge_perm, hm.edge_perm.data(), 4 * ne));
+    SWE_CUDA(c, cudaMemset(c->flux, 0, sizeof(EdgeFlux) * ne));
+  }
+
+  // ---- boundary strings: members in ascending caller edge id ("string order", R-11)
+  int max_id = -1;
+  for (int64_t e = 0; e < ne; ++e) {
+    const int32_t R = hm.edge_cell[2 * e + 1];
+    if (R <= -3) max_id = std::max(max_id, -3 - R);
+  }
+  if (max_id > 65535) { c->err = "boundary string id too large"; return SWE_EINVAL; }
+  c->strings.assign(max_id + 1, BoundaryString{});
+  c->d_params.assign(max_id + 1, nullptr);
+  std::vector<std::vector<int32_t>> members(max_id + 1);
+  for (int64_t e = 0; e < ne; ++e) {
+    const int32_t R = hm.edge_cell[2 * e + 1];
+    if (R <= -3) members[-3 - R].push_back(hm.edge_new[e]);
+  }
+  std::vector<int32_t> flat;
+  size_t scratch = 0;
+  for (int s = 0; s <= max_id; ++s) {
+    BoundaryString &bs = c->strings[s];
+    bs.n_edges = (int32_t)members[s].size();
+    bs.first = (int32_t)flat.size();
+    int32_t P = 1;
+    while (P < bs.n_edges) P <<= 1;
+    bs.pow2 = P;
+    bs.scratch = (int32_t)scratch;
+    scratch += P;
+    flat.insert(flat.end(), members[s].begin(), members[s].end());
+  }
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_ctl, sizeof(Control)));
+  SWE_CUDA(c, cudaMallocHost((void **)&c->h_ctl, sizeof(Control)));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_strings, sizeof(BoundaryString) * std::max<size_t>(1, c->strings.size())));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_string_edges, 4 * std::max<size_t>(1, flat.size())));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_scratch, 8 * std::max<size_t>(1, scratch)));
+  if (!flat.empty()) SWE_CUDA(c, cudaMemcpy(c->d_string_edges, flat.data(), 4 * flat.size(), cudaMemcpyHostToDevice));
+  if (!c->strings.empty()) {
+    SWE_CUDA(c, cudaMemcpy(c->d_strings, c->strings.data(), sizeof(BoundaryString) * c->strings.size(), cudaMemcpyHostToDevice));
+    k_string_lengths<<<1, kCtlThreads, 0, c->stream>>>(c->d_strings, (int)c->strings.size(), c->d_string_edges, c->d_scratch, c->geom);
+    SWE_CUDA(c, cudaGetLastError());
+    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+    SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
+  }
+
+  // ---- control block
+  Control h{};
+  h.g = p.g; h.h_dry = p.h_dry; h.dt_max = p.dt_max;
+  h.t_end = std::numeric_limits<double>::infinity(); h.cfl = 0.9;
+  h.n_strings = (int32_t)c->strings.size();
+  SWE_CUDA(c, cudaMemcpy(c->d_ctl, &h, sizeof(Control), cudaMemcpyHostToDevice));
+  *c->h_ctl = h;
+  return capture_graph(c);
+}
+
+}  // namespace
+
+// =========================================================================================================
+extern "C" {
+
+void swe_params_default(swe_params *p) {
+  if (!p) return;
+  std::memset(p, 0, sizeof(*p));
+  p->g = 9.81;
+  p->h_dry = 1e-3;
+  p->dt_max = std::numeric_limits<double>::infinity();
+  p->renumber = SWE_RENUMBER_MORTON;
+  p->state_on_device = 0;
+  p->steps_per_graph = 32;
+}
+
+size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges) {
+  if (n_cells < 0) return 0;
+  if (n_edges <= 0) n_edges = 3 * n_cells;
+  return Layout(n_cells, n_edges).total;
+}
+
+int swe_create(const swe_mesh *mesh, const swe_params *params, swe_ctx **out) {
+  if (out) *out = nullptr;
+  if (!mesh || !out || !mesh->node_xy || !mesh->tri || !mesh->zb || !mesh->kst) { g_create_error = "null argument"; return SWE_EINVAL; }
+  if (mesh->n_cells <= 0 || mesh->n_nodes <= 0 || mesh->n_cells > (int64_t)0x7fffffff / 3) { g_create_error = "n_cells / n_nodes out of range"; return SWE_EINVAL; }
+  swe_ctx *c = new (std::nothrow) swe_ctx;
+  if (!c) { g_create_error = "out of host memory"; return SWE_ENOMEM; }
+  int rc;
+  try {
+    rc = create_impl(mesh, params, c);
+  } catch (const std::bad_alloc &) {
+    c->err = "out of host memory";
+    rc = SWE_ENOMEM;
+  }
+  if (rc != SWE_OK) {
+    g_create_error = c->err;
+    release(c);
+    return rc;
+  }
+  *out = c;
+  return SWE_OK;
+}
+
+int swe_set_boundary(swe_ctx *c, int string_id, int type, const double *params, int n_params) {
+  if (!c) return SWE_EINVAL;
+  if (string_id < 0 || string_id >= (int)c->strings.size() || c->strings[string_id].n_edges == 0) { c->err = "no edge of the mesh belongs to this boundary string"; return SWE_EINVAL; }
+  if (n_params < 0 || (n_params > 0 && !params)) { c->err = "bad params"; return SWE_EINVAL; }
+  if (type == SWE_BC_INFLOW_Q) {
+    if (n_params < 2 || n_params % 2) { c->err = "INFLOW_Q needs a (t, Q) table"; return SWE_EINVAL; }
+    for (int k = 2; k < n_params; k += 2) if (!(params[k] > params[k - 2])) { c->err = "hydrograph times must ascend"; return SWE_EINVAL; }
+  } else if (type == SWE_BC_OUTFLOW_UNIFORM) {
+    if (n_params < 1 || !(params[0] >= 0.0)) { c->err = "OUTFLOW_UNIFORM needs S0 >= 0"; return SWE_EINVAL; }
+  } else if (type != SWE_BC_NONE) {
+    c->err = "unknown boundary type";
+    return SWE_EINVAL;
+  }
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  BoundaryString &bs = c->strings[string_id];
+  if (c->d_params[string_id]) { cudaFree(c->d_params[string_id]); c->d_params[string_id] = nullptr; }
+  bs.type = type; bs.n_params = n_params; bs.params = nullptr; bs.Q = 0.0; bs.sumK = 0.0;
+  bs.S0 = (type == SWE_BC_OUTFLOW_UNIFORM) ? params[0] : 0.0;
+  if (n_params > 0) {
+    SWE_CUDA(c, cudaMalloc((void **)&c->d_params[string_id], 8 * (size_t)n_params));
+    SWE_CUDA(c, cudaMemcpy(c->d_params[string_id], params, 8 * (size_t)n_params, cudaMemcpyHostToDevice));
+    bs.params = c->d_params[string_id];
+  }
+  return upload_strings(c);
+}
+
+int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *hv, double t0) {
+  if (!c) return SWE_EINVAL;
+  if (!h || !hu || !hv || !std::isfinite(t0)) { c->err = "null state pointer / non-finite t0"; return SWE_EINVAL; }
+  const int64_t nc = c->nc;
+  const double *dh = h, *dhu = hu, *dhv = hv;
+  if (!c->prm.state_on_device) {
+    SWE_CUDA(c, cudaMemcpyAsync(c->stage, h, 8 * nc, cudaMemcpyHostToDevice, c->stream));
+    SWE_CUDA(c, cudaMemcpyAsync(c->stage + nc, hu, 8 * nc, cudaMemcpyHostToDevice, c->stream));
+    SWE_CUDA(c, cudaMemcpyAsync(c->stage + 2 * nc, hv, 8 * nc, cudaMemcpyHostToDevice, c->stream));
+    dh = c->stage; dhu = c->stage + nc; dhv = c->stage + 2 * nc;
+  }
+  k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, dh, dhu, dhv, c->rec, (int)nc);
+  k_reset<<<1, 1, 0, c->stream>>>(c->d_ctl, t0);
+  k_rate<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, (int)nc);
+  c->launches += 3;
+  SWE_CUDA(c, cudaGetLastError());
+  c->t_host = t0;
+  return SWE_OK;
+}
+
+int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_info *info) {
+  if (!c) return SWE_EINVAL;
+  if (!(cfl > 0.0) || std::isnan(t_end)) { c->err = "cfl must be > 0 and t_end a number"; return SWE_EINVAL; }
+  const bool finite_end = std::isfinite(t_end);
+  if (n_steps < 0 && !finite_end) { c->err = "either n_steps >= 0 or a finite t_end is needed"; return SWE_EINVAL; }
+  k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, (long long)n_steps, t_end, cfl);
+  c->launches += 1;
+  const int K = c->steps_per_graph;
+  int64_t remaining = n_steps < 0 ? std::numeric_limits<int64_t>::max() : n_steps;
+  int64_t poll_every = 4;            // graph launches between two reads of t (only when t_end is finite)
+  bool done = !(c->t_host < t_end);  // t_end already reached: nothing to do
+  while (!done && remaining > 0) {
+    int64_t batch_steps = 0;
+    if (K > 0 && remaining >= K) {
+      int64_t n_graphs = remaining / K;
+      if (finite_end) n_graphs = std::min(n_graphs, poll_every);
+      for (int64_t j = 0; j < n_graphs; ++j) SWE_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+      batch_steps = n_graphs * K;
+    } else {
+      batch_steps = std::min<int64_t>(remaining, 64);   // tail shorter than a graph, or graphs switched off
+      for (int64_t j = 0; j < batch_steps; ++j) enqueue_step(c, c->stream);
+      SWE_CUDA(c, cudaGetLastError());
+    }
+    c->launches += batch_steps * kKernelsPerStep;
+    remaining -= batch_steps;
+    if (finite_end) {                // the only host synchronisation inside the loop: once per batch
+      int rc = read_control(c);
+      if (rc != SWE_OK) return rc;
+      if (!(c->h_ctl->t < t_end) || (c->h_ctl->flags & SWE_FLAG_DT_UNBOUNDED)) done = true;
+      poll_every = std::min<int64_t>(poll_every * 2, 64);
+    }
+  }
+  // volume bookkeeping of the last step; then the reductions of swe_step_info
+  k_step_control<<<1, kCtlThreads, 0, c->stream>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom,
+                                                   c->flux, c->theta, c->rec, c->kst, 1);
+  c->launches += 1;
+  SWE_CUDA(c, cudaGetLastError());
+  if (info) {
+    k_info<<<std::min(grid_for(c->nc), 148 * 8), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->area, (int)c->nc);
+    c->launches += 1;
+    int rc = read_control(c);
+    if (rc != SWE_OK) return rc;
+    const Control &h = *c->h_ctl;
+    info->t = h.t; info->dt_last = h.dt_last; info->steps_done = h.steps_done; info->n_wet = h.n_wet;
+    info->vol = h.vol; info->vol_clipped = h.vol_clipped; info->vol_in = h.vol_in; info->vol_out = h.vol_out;
+    info->flags = h.flags | (h.nonfinite ? SWE_FLAG_NONFINITE : 0);
+    if (h.nonfinite) { c->err = "non-finite state value"; return SWE_ENONFINITE; }
+  } else if (!finite_end) {
+    c->t_host = -std::numeric_limits<double>::infinity();   // unknown until the next read; never blocks stepping
+  }
+  return SWE_OK;
+}
+
+int swe_get_state(swe_ctx *c, double *h, double *hu, double *hv) {
+  if (!c) return SWE_EINVAL;
+  if (!h || !hu || !hv) { c->err = "null state pointer"; return SWE_EINVAL; }
+  const int64_t nc = c->nc;
+  if (c->prm.state_on_device) {
+    k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, c->rec, h, hu, hv, (int)nc);
+    c->launches += 1;
+    SWE_CUDA(c, cudaGetLastError());
+    return SWE_OK;
+  }
+  k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, c->rec, c->stage, c->stage + nc, c->stage + 2 * nc, (int)nc);
+  c->launches += 1;
+  SWE_CUDA(c, cudaMemcpyAsync(h, c->stage, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
+  SWE_CUDA(c, cudaMemcpyAsync(hu, c->stage + nc, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
+  SWE_CUDA(c, cudaMemcpyAsync(hv, c->stage + 2 * nc, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  return SWE_OK;
+}
+
+void swe_destroy(swe_ctx *c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  release(c);
+}
+
+const char *swe_last_error(const swe_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+// ---- inspection ---------------------------------------------------------------------------------------
+int swe_get_geometry(swe_ctx *c, double *area, double *nx, double *ny, double *len) {
+  if (!c || !area || !nx || !ny || !len) return SWE_EINVAL;
+  // read back what the kernels use (device arrays, internal numbering) and undo the renumbering
+  std::vector<double> a(c->nc);
+  std::vector<EdgeGeom> g(c->ne);
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  SWE_CUDA(c, cudaMemcpy(a.data(), c->area, 8 * c->nc, cudaMemcpyDeviceToHost));
+  SWE_CUDA(c, cudaMemcpy(g.data(), c->geom, sizeof(EdgeGeom) * c->ne, cudaMemcpyDeviceToHost));
+  for (int64_t i = 0; i < c->nc; ++i) area[c->hm.cell_perm[i]] = a[i];
+  for (int64_t e = 0; e < c->ne; ++e) {
+    const int32_t o = c->hm.edge_perm[e];
+    nx[o] = g[e].nx; ny[o] = g[e].ny; len[o] = g[e].len;
+  }
+  return SWE_OK;
+}
+
+int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR, double *theta) {
+  if (!c || !F1 || !F3 || !GL || !GR) return SWE_EINVAL;
+  const int64_t ne = c->ne, nc = c->nc;
+  double *d = nullptr;
+  SWE_CUDA(c, cudaMalloc((void **)&d, 8 * 4 * ne));
+  k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, c->theta, d, d + ne, d + 2 * ne,
+                                                        d + 3 * ne, (int)ne);
+  c->launches += 1;
+  cudaError_t e1 = cudaStreamSynchronize(c->stream);
+  if (e1 == cudaSuccess) e1 = cudaMemcpy(F1, d, 8 * ne, cudaMemcpyDeviceToHost);
+  if (e1 == cudaSuccess) e1 = cudaMemcpy(F3, d + ne, 8 * ne, cudaMemcpyDeviceToHost);
+  if (e1 == cudaSuccess) e1 = cudaMemcpy(GL, d + 2 * ne, 8 * ne, cudaMemcpyDeviceToHost);
+  if (e1 == cudaSuccess) e1 = cudaMemcpy(GR, d + 3 * ne, 8 * ne, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  SWE_CUDA(c, e1);
+  if (theta) {
+    std::vector<double> th(nc);
+    SWE_CUDA(c, cudaMemcpy(th.data(), c->theta, 8 * nc, cudaMemcpyDeviceToHost));
+    for (int64_t i = 0; i < nc; ++i) theta[c->hm.cell_perm[i]] = th[i];
+  }
+  return SWE_OK;
+}
+
+int swe_peek_dt(swe_ctx *c, double cfl, double t_end, double *dt_out) {
+  if (!c || !dt_out || !(cfl > 0.0)) return SWE_EINVAL;
+  int rc = read_control(c);
+  if (rc != SWE_OK) return rc;
+  const Control &h = *c->h_ctl;
+  double r;
+  std::memcpy(&r, &h.rate_bits, 8);
+  double dt = (r > 0.0) ? cfl / r : h.dt_max;
+  dt = std::fmin(dt, h.dt_max);
+  const double rem = t_end - h.t;
+  *dt_out = (dt >= rem) ? rem : dt;
+  return SWE_OK;
+}
+
+int swe_get_permutation(swe_ctx *c, int32_t *cell_perm, int32_t *edge_perm) {
+  if (!c) return SWE_EINVAL;
+  if (cell_perm) std::memcpy(cell_perm, c->hm.cell_perm.data(), 4 * c->nc);
+  if (edge_perm) std::memcpy(edge_perm, c->hm.edge_perm.data(), 4 * c->ne);
+  return SWE_OK;
+}
+
+int swe_get_tables(swe_ctx *c, int64_t *n_edges, int32_t *edge_cell, int32_t *cell_edge) {
+  if (!c) return SWE_EINVAL;
+  if (n_edges) *n_edges = c->ne;
+  if (edge_cell) std::memcpy(edge_cell, c->hm.edge_cell.data(), 8 * c->ne);
+  if (cell_edge) std::memcpy(cell_edge, c->hm.cell_edge.data(), 12 * c->nc);
+  return SWE_OK;
+}
+
+int64_t swe_kernel_launches(const swe_ctx *c) { return c ? c->launches : 0; }
+
+}  // extern "C"

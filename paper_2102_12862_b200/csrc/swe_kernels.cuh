@@ -1,0 +1,507 @@
+// CUDA kernels (sm_100a) of the explicit finite-volume shallow-water step.  fp64 throughout; compiled with
+// -fmad=false so that the parenthesisation written here IS the arithmetic (R-14).
+//
+//   k_step_control  S0/S4: dt from the max rate of U^n, t += dt, boundary-string values at t^n, volume bookkeeping
+//   k_edge_flux     S1/S1b: hydrostatic reconstruction + HLLC per edge; boundary edges
+//   k_theta         S1c: draining-time factor per cell
+//   k_cell_update   S2+S3 (+S0 of the next step): gather in slot order, Euler update, friction, wet/dry,
+//                   local wave speed -> warp-shuffle + block max -> one atomicMax per block
+//
+// "P:n" = PAPER.md line n; R-k = DESIGN.md section 2.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "swe_types.h"
+
+namespace swe {
+
+constexpr int kBlock = 256;           // threads per block of the mesh kernels
+constexpr int kCtlThreads = 1024;     // the single block of k_step_control
+
+// boundary codes / string types (values of include/swe.h, restated so that device code needs no host header)
+constexpr int kEdgeTransmissive = -2;
+constexpr int kBcInflowQ = 1, kBcOutflowUniform = 2;
+constexpr int kFlagUnbounded = 2;
+
+// ---------------------------------------------------------------------------------------------------------
+// S1, one edge in the (normal, tangential) frame.  P:252 HLLC ("Chapter 10 of [18]"): HLL for mass and normal
+// momentum with two-rarefaction wave speeds and dry-bed limits (R-2, R-3), contact wave = upwinded tangential
+// momentum; P:254 bed slope by the modified-state approach of ref [69] (R-1): face bed z* = max(zL, zR), face
+// depths hs_K = max(0, h_K + z_K - z*), per-side pressure correction G_K = F2 - 1/2 g hs_K^2.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ EdgeFlux riemann_nt(double g, double hL, double unL, double utL, double zL,
+                                               double hR, double unR, double utR, double zR) {
+  EdgeFlux o;
+  const double dz = zR - zL;
+  const double hsL = fmax(0.0, hL - fmax(0.0, dz));
+  const double hsR = fmax(0.0, hR - fmax(0.0, -dz));
+  if (hsL == 0.0 && hsR == 0.0) {
+    o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
+    return o;
+  }
+  const double cL = sqrt(g * hsL), cR = sqrt(g * hsR);
+  double SL, SR;
+  if (hsL > 0.0 && hsR > 0.0) {
+    const double us = 0.5 * (unL + unR) + (cL - cR);
+    const double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
+    SL = fmin(unL - cL, us - cs);
+    SR = fmax(unR + cR, us + cs);
+  } else if (hsR == 0.0) {
+    SL = unL - cL;
+    SR = unL + 2.0 * cL;
+  } else {
+    SL = unR - 2.0 * cR;
+    SR = unR + cR;
+  }
+  const double qsL = hsL * unL, qsR = hsR * unR;
+  const double pL = (0.5 * g) * (hsL * hsL), pR = (0.5 * g) * (hsR * hsR);
+  const double FL2 = qsL * unL + pL, FR2 = qsR * unR + pR;
+  double F1, F2;
+  if (SL >= 0.0) {
+    F1 = qsL; F2 = FL2;
+  } else if (SR <= 0.0) {
+    F1 = qsR; F2 = FR2;
+  } else {
+    const double inv = 1.0 / (SR - SL);
+    F1 = qsL + (SL * (SR * (hsR - hsL) - (qsR - qsL))) * inv;
+    F2 = FL2 + (SL * (SR * (qsR - qsL) - (FR2 - FL2))) * inv;
+  }
+  o.F1 = F1;
+  o.F3 = F1 * (F1 >= 0.0 ? utL : utR);
+  o.GL = F2 - pL;
+  o.GR = F2 - pR;
+  return o;
+}
+
+__device__ __forceinline__ double pow53(double h) {  // h^(5/3), Strickler conveyance (Table 1)
+  const double c3 = cbrt(h);
+  return (h * c3) * c3;
+}
+
+__device__ __forceinline__ double k_weight(double k) { return isfinite(k) ? k : 1.0; }
+
+// S1b, boundary edge (only the L side exists).  P:332 wall; P:342 zero-gradient, inflow hydrograph, uniform outflow.
+__device__ __forceinline__ EdgeFlux boundary_flux(const Control &c, const BoundaryString *__restrict__ strings,
+                                                  const double *__restrict__ kst, const EdgeGeom &eg,
+                                                  const CellRec &a, double u, double v) {
+  EdgeFlux o;
+  o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
+  const double he = a.h;
+  const int code = eg.R;
+  int type = 0;
+  const BoundaryString *s = nullptr;
+  if (code <= -3 && (-3 - code) < c.n_strings) {
+    s = strings + (-3 - code);
+    type = s->type;
+  }
+  if (code == kEdgeTransmissive) {            // R-10: ghost = copy of the interior state
+    const double un = u * eg.nx + v * eg.ny, ut = v * eg.nx - u * eg.ny;
+    o = riemann_nt(c.g, he, un, ut, a.z, he, un, ut, a.z);
+    o.GR = 0.0;
+  } else if (type == kBcInflowQ) {            // R-11: Q(t) distributed by conveyance l k h^(5/3)
+    double qe;
+    if (s->sumK > 0.0) {
+      const double Ke = (eg.len * k_weight(kst[eg.L])) * pow53(he);
+      qe = ((s->Q * Ke) / s->sumK) / eg.len;
+    } else {
+      qe = s->Q / s->sumL;
+    }
+    o.F1 = -qe;
+    o.GL = (he > 0.0) ? (qe * qe) / he : 0.0;
+  } else if (type == kBcOutflowUniform) {     // R-12: normal depth, q_n = k h^(5/3) sqrt(S0)
+    if (he > 0.0) {
+      const double qn = (k_weight(kst[eg.L]) * pow53(he)) * sqrt(s->S0);
+      const double ut = v * eg.nx - u * eg.ny;
+      o.F1 = qn;
+      o.GL = (qn * qn) / he;
+      o.F3 = qn * ut;
+    }
+  } else {                                    // R-9: reflective wall, closed form of the mirror-ghost problem
+    if (he > 0.0) {
+      const double un = u * eg.nx + v * eg.ny;
+      const double cel = sqrt(c.g * he);
+      const double S = fmax(cel - un, cel + 0.5 * un);
+      o.GL = (he * un) * (un + S);
+    }
+  }
+  return o;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1: one thread per edge.  Reads one EdgeGeom record (coalesced 256-bit), gathers the two CellRec records
+// (one sector each), writes one EdgeFlux record (coalesced 256-bit).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock)
+k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
+            const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
+            EdgeFlux *__restrict__ flux, int n_edges) {
+  if (!ctl->active) return;
+  const int e = blockIdx.x * kBlock + threadIdx.x;
+  if (e >= n_edges) return;
+  const double g = ctl->g, h_dry = ctl->h_dry;
+  const EdgeGeom eg = geom[e];
+  const CellRec a = rec[eg.L];
+  double uL = 0.0, vL = 0.0;
+  if (a.h > h_dry) { uL = a.qx / a.h; vL = a.qy / a.h; }   // R-8: thin films carry no momentum
+  EdgeFlux o;
+  if (eg.R >= 0) {
+    const CellRec b = rec[eg.R];
+    double uR = 0.0, vR = 0.0;
+    if (b.h > h_dry) { uR = b.qx / b.h; vR = b.qy / b.h; }
+    const double unL = uL * eg.nx + vL * eg.ny, utL = vL * eg.nx - uL * eg.ny;
+    const double unR = uR * eg.nx + vR * eg.ny, utR = vR * eg.nx - uR * eg.ny;
+    o = riemann_nt(g, a.h, unL, utL, a.z, b.h, unR, utR, b.z);
+  } else {
+    o = boundary_flux(*ctl, strings, kst, eg, a, uL, vL);
+  }
+  flux[e] = o;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1c (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1 of cell i)), slots in order.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock)
+k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
+        const EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
+        double *__restrict__ theta, int n_cells) {
+  if (!ctl->active) return;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  const double dt = ctl->dt;
+  const int4 ce = cell_edge[i];
+  const int es[3] = {ce.x, ce.y, ce.z};
+  double o[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const EdgeGeom eg = geom[es[k]];
+    const double F1 = flux[es[k]].F1;
+    const double sM = (eg.L == i ? 1.0 : -1.0) * (eg.len * F1);
+    o[k] = fmax(0.0, sM);
+  }
+  const double out = ((o[0] + o[1]) + o[2]);
+  const double avail = rec[i].h * area[i];
+  theta[i] = (dt * out > avail) ? avail / (dt * out) : 1.0;
+}
+
+// block-wide max of non-negative doubles -> one atomicMax on the bit pattern (order-preserving for x >= 0)
+__device__ __forceinline__ void block_max_to_global(double r, unsigned long long *dst) {
+  __shared__ double warp_max[kBlock / 32];
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const double other = __shfl_xor_sync(0xffffffffu, r, off);
+    r = (other > r) ? other : r;
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) warp_max[wid] = r;
+  __syncthreads();
+  if (wid == 0) {
+    r = (lane < kBlock / 32) ? warp_max[lane] : 0.0;
+#pragma unroll
+    for (int off = (kBlock / 32) / 2; off > 0; off >>= 1) {
+      const double other = __shfl_xor_sync(0xffffffffu, r, off);
+      r = (other > r) ? other : r;
+    }
+    if (lane == 0 && r > 0.0) atomicMax(dst, (unsigned long long)__double_as_longlong(r));
+  }
+}
+
+// Eq. 21 (R-7) for one cell: max_j lambda_ij / rho_ij with rho_ij = 4|Omega_i| / (3 l_ij)
+__device__ __forceinline__ double cell_rate(double g, double h, double qx, double qy, double invA,
+                                            const double nx[3], const double ny[3], const double len[3]) {
+  const double u = qx / h, v = qy / h;
+  const double cel = sqrt(g * h);
+  double r = 0.0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double lam = fabs(u * nx[k] + v * ny[k]) + cel;
+    const double val = lam * ((0.75 * len[k]) * invA);
+    if (val > r) r = val;
+  }
+  return r;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S2 + S3, and S0 of the NEXT step fused in: one thread per cell.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock)
+k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
+              const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
+              const double *__restrict__ area, const double *__restrict__ inv_area,
+              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells) {
+  if (!ctl->active) return;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  double rate = 0.0;
+  if (i < n_cells) {
+    const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+    const int4 ce = cell_edge[i];
+    const int es[3] = {ce.x, ce.y, ce.z};
+    double nx[3], ny[3], len[3];
+    double dHk[3], dXk[3], dYk[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const EdgeGeom eg = geom[es[k]];
+      EdgeFlux f = flux[es[k]];
+      const bool isL = (eg.L == i);
+      // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
+      double th = 1.0;
+      if (f.F1 > 0.0) th = theta[eg.L];
+      else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
+      double G = isL ? f.GL : f.GR;
+      if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
+      const double s = isL ? 1.0 : -1.0;
+      nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
+      dHk[k] = s * (eg.len * f.F1);
+      dXk[k] = s * (eg.len * (G * eg.nx - f.F3 * eg.ny));
+      dYk[k] = s * (eg.len * (G * eg.ny + f.F3 * eg.nx));
+    }
+    const double dH = ((dHk[0] + dHk[1]) + dHk[2]);
+    const double dX = ((dXk[0] + dXk[1]) + dXk[2]);
+    const double dY = ((dYk[0] + dYk[1]) + dYk[2]);
+    CellRec c = rec[i];
+    const double invA = inv_area[i];
+    const double a = dt * invA;
+    double hn = c.h - a * dH;
+    if (hn < 0.0) {                                  // residual negatives (R-8b): clip and count
+      atomicAdd(&ctl->vol_clipped, -hn * area[i]);
+      hn = 0.0;
+    }
+    double qxn = 0.0, qyn = 0.0;
+    if (hn > h_dry) {
+      qxn = c.qx - a * dX;
+      qyn = c.qy - a * dY;
+      const double f2 = gn2[i];
+      if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
+        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt(hn));
+        qxn = qxn / D;
+        qyn = qyn / D;
+      }
+      rate = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
+    }
+    c.h = hn; c.qx = qxn; c.qy = qyn;
+    rec[i] = c;
+  }
+  block_max_to_global(rate, &ctl->rate_bits);
+}
+
+// Eq. 21 on the current state (after swe_set_state): same arithmetic as the fused part of k_cell_update
+__global__ void __launch_bounds__(kBlock)
+k_rate(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
+       const double *__restrict__ inv_area, const CellRec *__restrict__ rec, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  double rate = 0.0;
+  if (i < n_cells) {
+    const CellRec c = rec[i];
+    if (c.h > ctl->h_dry) {
+      const int4 ce = cell_edge[i];
+      const int es[3] = {ce.x, ce.y, ce.z};
+      double nx[3], ny[3], len[3];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        const EdgeGeom eg = geom[es[k]];
+        nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
+      }
+      rate = cell_rate(ctl->g, c.h, c.qx, c.qy, inv_area[i], nx, ny, len);
+    }
+  }
+  block_max_to_global(rate, &ctl->rate_bits);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Step control: one block.  Fixed-shape pairwise tree in string order (R-11): pad to a power of two with zeros,
+// add neighbours at stride 1, 2, 4, ... -- the same pairs whatever the thread count, hence bit-reproducible.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_tree_sum(double *v, int pow2) {
+  for (int s = 1; s < pow2; s <<= 1) {
+    __syncthreads();
+    for (int j = threadIdx.x; 2 * s * j + s < pow2; j += blockDim.x) v[2 * s * j] = v[2 * s * j] + v[2 * s * j + s];
+  }
+  __syncthreads();
+  return v[0];
+}
+
+__device__ __forceinline__ double hydrograph(const double *p, int n_params, double t) {  // piecewise linear, clamped
+  const int m = n_params / 2;
+  if (m == 0) return 0.0;
+  if (t <= p[0]) return p[1];
+  if (t >= p[2 * (m - 1)]) return p[2 * (m - 1) + 1];
+  int k = 0;
+  while (!(p[2 * k] <= t && t < p[2 * (k + 1)])) ++k;
+  const double tk = p[2 * k], Qk = p[2 * k + 1], tk1 = p[2 * k + 2], Qk1 = p[2 * k + 3];
+  return Qk + (Qk1 - Qk) * ((t - tk) / (tk1 - tk));
+}
+
+// mode 0: start of a step.  mode 1: end of an swe_step call (bookkeeping of the last step only; zeroes the
+// accumulators of k_info).
+__global__ void __launch_bounds__(kCtlThreads)
+k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ string_edges, double *scratch,
+               const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
+               const double *__restrict__ theta, const CellRec *__restrict__ rec,
+               const double *__restrict__ kst, int mode) {
+  const int ns = ctl->n_strings;
+  // ---- volume bookkeeping of the previous step, from the (limited) fluxes actually applied
+  if (ctl->pending) {
+    const double dt_prev = ctl->dt_last;
+    for (int s = 0; s < ns; ++s) {
+      BoundaryString &bs = strings[s];
+      if (bs.type == kBcInflowQ) {
+        if (threadIdx.x == 0) ctl->vol_in += dt_prev * bs.Q;
+      } else if (bs.type == kBcOutflowUniform) {
+        double *v = scratch + bs.scratch;
+        for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
+          double a = 0.0;
+          if (j < bs.n_edges) {
+            const int e = string_edges[bs.first + j];
+            const EdgeGeom eg = geom[e];
+            double F1 = flux[e].F1;
+            if (F1 > 0.0) {
+              const double th = theta[eg.L];
+              if (th < 1.0) F1 = th * F1;
+            }
+            a = eg.len * F1;
+          }
+          v[j] = a;
+        }
+        const double sum = block_tree_sum(v, bs.pow2);
+        if (threadIdx.x == 0) ctl->vol_out += dt_prev * sum;
+      }
+    }
+  }
+  __syncthreads();
+  if (mode == 1) {
+    if (threadIdx.x == 0) { ctl->pending = 0; ctl->vol = 0.0; ctl->n_wet = 0; ctl->nonfinite = 0; }
+    return;
+  }
+  // ---- S0: dt from the rate of U^n; S4: t += dt (t_end is hit exactly)
+  __shared__ int s_active;
+  __shared__ double s_t_old;
+  if (threadIdx.x == 0) {
+    int active = 0;
+    ctl->pending = 0;
+    const double t = ctl->t, t_end = ctl->t_end;
+    if (ctl->steps_left != 0 && t < t_end && !(ctl->flags & kFlagUnbounded)) {
+      const double r = __longlong_as_double((long long)ctl->rate_bits);
+      double dt = (r > 0.0) ? ctl->cfl / r : ctl->dt_max;
+      dt = fmin(dt, ctl->dt_max);
+      const double rem = t_end - t;
+      double t_new;
+      if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = t + dt; }
+      if (!isfinite(dt)) {
+        ctl->flags |= kFlagUnbounded;
+      } else {
+        active = 1;
+        ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
+        ctl->rate_bits = 0ull;
+        ctl->steps_done += 1;
+        if (ctl->steps_left > 0) ctl->steps_left -= 1;
+        ctl->pending = 1;
+      }
+    }
+    ctl->active = active;
+    s_active = active;
+    s_t_old = t;
+  }
+  __syncthreads();
+  if (!s_active) return;
+  // ---- boundary strings at t^n (R-11): Q(t^n) and the conveyance sum over the string
+  for (int s = 0; s < ns; ++s) {
+    BoundaryString &bs = strings[s];
+    if (bs.type != kBcInflowQ) continue;
+    double *v = scratch + bs.scratch;
+    for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
+      double a = 0.0;
+      if (j < bs.n_edges) {
+        const int e = string_edges[bs.first + j];
+        const EdgeGeom eg = geom[e];
+        a = (eg.len * k_weight(kst[eg.L])) * pow53(rec[eg.L].h);
+      }
+      v[j] = a;
+    }
+    const double sum = block_tree_sum(v, bs.pow2);
+    if (threadIdx.x == 0) {
+      bs.sumK = sum;
+      bs.Q = hydrograph(bs.params, bs.n_params, s_t_old);
+    }
+  }
+}
+
+// start of an swe_step call: the stop conditions of this call
+__global__ void k_call_begin(Control *ctl, long long n_steps, double t_end, double cfl) {
+  ctl->steps_left = n_steps;
+  ctl->t_end = t_end;
+  ctl->cfl = cfl;
+  ctl->flags &= ~kFlagUnbounded;
+}
+
+__global__ void k_reset(Control *ctl, double t0) {
+  ctl->t = t0; ctl->dt = 0.0; ctl->dt_last = 0.0;
+  ctl->vol_in = 0.0; ctl->vol_out = 0.0; ctl->vol_clipped = 0.0;
+  ctl->rate_bits = 0ull; ctl->steps_left = 0; ctl->steps_done = 0;
+  ctl->active = 0; ctl->pending = 0; ctl->flags = 0;
+}
+
+// swe_step_info reductions: volume, wet count, non-finite check
+__global__ void __launch_bounds__(kBlock)
+k_info(Control *__restrict__ ctl, const CellRec *__restrict__ rec, const double *__restrict__ area, int n_cells) {
+  double vol = 0.0;
+  long long wet = 0;
+  int bad = 0;
+  const double h_dry = ctl->h_dry;
+  for (int i = blockIdx.x * kBlock + threadIdx.x; i < n_cells; i += gridDim.x * kBlock) {
+    const CellRec c = rec[i];
+    vol += c.h * area[i];
+    wet += (c.h > h_dry);
+    bad |= !(isfinite(c.h) && isfinite(c.qx) && isfinite(c.qy));
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    vol += __shfl_xor_sync(0xffffffffu, vol, off);
+    wet += __shfl_xor_sync(0xffffffffu, wet, off);
+    bad |= __shfl_xor_sync(0xffffffffu, bad, off);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&ctl->vol, vol);
+    atomicAdd((unsigned long long *)&ctl->n_wet, (unsigned long long)wet);
+    if (bad) atomicOr(&ctl->nonfinite, 1);
+  }
+}
+
+// caller numbering <-> internal numbering (cell_perm[new] = caller id)
+__global__ void __launch_bounds__(kBlock)
+k_pack_state(const int *__restrict__ cell_perm, const double *__restrict__ h, const double *__restrict__ hu,
+             const double *__restrict__ hv, CellRec *__restrict__ rec, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  const int o = cell_perm[i];
+  CellRec c = rec[i];
+  c.h = h[o]; c.qx = hu[o]; c.qy = hv[o];
+  rec[i] = c;
+}
+
+__global__ void __launch_bounds__(kBlock)
+k_unpack_state(const int *__restrict__ cell_perm, const CellRec *__restrict__ rec, double *__restrict__ h,
+               double *__restrict__ hu, double *__restrict__ hv, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  const int o = cell_perm[i];
+  const CellRec c = rec[i];
+  h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
+}
+
+// inspection (swe_get_edge_flux): per-edge records after the limiter, in caller edge numbering
+__global__ void __launch_bounds__(kBlock)
+k_export_flux(const int *__restrict__ edge_perm, const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
+              const double *__restrict__ theta, double *__restrict__ F1, double *__restrict__ F3,
+              double *__restrict__ GL, double *__restrict__ GR, int n_edges) {
+  const int e = blockIdx.x * kBlock + threadIdx.x;
+  if (e >= n_edges) return;
+  const EdgeGeom eg = geom[e];
+  EdgeFlux f = flux[e];
+  double th = 1.0;
+  if (f.F1 > 0.0) th = theta[eg.L];
+  else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
+  if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR; }
+  const int o = edge_perm[e];
+  F1[o] = f.F1; F3[o] = f.F3; GL[o] = f.GL; GR[o] = f.GR;
+}
+
+}  // namespace swe

@@ -1,0 +1,326 @@
+"""GPU parity: the CUDA path (through the C-ABI of include/swe.h) against the oracle, element by element,
+on the same seeded inputs.  Run on the B200 box with `-m gpu`.
+
+Bar (BASELINE.json north_star, R-14): after 100 steps per-cell relative error of h, hu, hv <= 1e-10,
+dt agrees to <= 1e-12 relative, wet/dry masks identical.  Geometry, fluxes before any cbrt, theta and the dt of
+the first step are expected bit-identical (only + - * / sqrt min max on both sides, no FMA contraction).
+"""
+import numpy as np
+import pytest
+
+from workloads import configs as C
+
+pytestmark = pytest.mark.gpu
+
+RTOL, ATOL_SCALE, DT_RTOL = 1e-10, 1e-14, 1e-12
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box")
+    import paper_2102_12862_b200 as P
+    P.lib()
+    return P
+
+
+def assert_state_close(got, want, what=""):
+    """abs(d) <= 1e-10 abs(ref) + 1e-14 max abs(ref) per field (R-14), and report the strict relative error
+    on cells that are not pure round-off."""
+    for name, a, b in zip(("h", "hu", "hv"), got, want):
+        scale = np.max(np.abs(b)) if b.size else 0.0
+        err = np.abs(a - b)
+        tol = RTOL * np.abs(b) + ATOL_SCALE * scale
+        bad = np.nonzero(~(err <= tol))[0]
+        assert bad.size == 0, (f"{what} {name}: {bad.size} cells out of tolerance, worst at {bad[:5]}: "
+                               f"got {a[bad[:5]]}, want {b[bad[:5]]}")
+        sig = np.abs(b) > 1e-8 * scale
+        if np.any(sig):
+            assert np.max(err[sig] / np.abs(b[sig])) <= RTOL, f"{what} {name}: strict relative error too large"
+
+
+def run_both(gpu, ref, w, n_steps, t_end=float("inf"), chunks=(None,), **kw):
+    """Steps oracle and GPU side by side in the given chunks; returns the two solvers and info dicts."""
+    o = ref.RefSolver(w)
+    s = gpu.from_workload(w, **kw)
+    io = o.step(n_steps, t_end, w.cfl)
+    ig = s.step(n_steps, t_end, w.cfl)
+    return o, s, io, ig
+
+
+def check_info(ig, io):
+    assert ig["steps_done"] == io["steps_done"]
+    assert ig["n_wet"] == io["n_wet"]
+    assert ig["flags"] == io["flags"]
+    assert abs(ig["t"] - io["t"]) <= DT_RTOL * abs(io["t"])
+    assert abs(ig["dt_last"] - io["dt_last"]) <= DT_RTOL * abs(io["dt_last"])
+    assert abs(ig["vol"] - io["vol"]) <= 1e-12 * abs(io["vol"])
+    for k in ("vol_in", "vol_out"):
+        assert abs(ig[k] - io[k]) <= 1e-11 * max(abs(io[k]), 1e-300) + 0.0, (k, ig[k], io[k])
+    assert abs(ig["vol_clipped"] - io["vol_clipped"]) <= 1e-9 * abs(io["vol_clipped"]) + 1e-13 * abs(io["vol"])
+
+
+CASES = {
+    "config1-ritter": lambda: C.config1(),
+    "config1-stoker": lambda: C.dam_break_channel(h_right=0.1),
+    "config2-lake-small": lambda: C.by_id(2, 0.1),
+    "config3-small": lambda: C.by_id(3, 0.02),
+    "config4-small": lambda: C.by_id(4, 0.01),
+    "uniform-flow": lambda: C.uniform_flow_channel(nx=60, ny=3, lx=300.0, ly=15.0),
+    "t5-rarefactions": lambda: C.dam_break_channel(nx=681, ny=1, ly=0.1, h_left=1.0, h_right=1.0, cfl=0.95,
+                                                   transmissive_ends=True, q_left=-3.0, q_right=3.0, t_end=2.5),
+}
+
+
+@pytest.mark.parametrize("name", ["config2-lake-small", "config3-small", "config4-small"])
+def test_geometry_bit_identical(gpu, ref, name):
+    """Section 4.1 geometry: areas, lengths, normals as the kernels use them == the oracle's."""
+    w = CASES[name]()
+    o = ref.RefSolver(w)
+    s = gpu.from_workload(w)
+    for a, b in zip(s.geometry(), o.geometry()):
+        assert np.array_equal(a, b)
+    s.close()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_first_step_edge_by_edge(gpu, ref, name):
+    """S0 + S1 + S1c of the first step, per edge: fluxes after the limiter, theta, dt."""
+    w = CASES[name]()
+    o = ref.RefSolver(w)
+    s = gpu.from_workload(w)
+    assert s.peek_dt(w.cfl) == o.peek_dt(w.cfl)                      # Eq. 21: exact max, one division
+    io = o.step(1, float("inf"), w.cfl)
+    ig = s.step(1, float("inf"), w.cfl)
+    assert ig["dt_last"] == io["dt_last"]
+    F = s.edge_fluxes()
+    Fo = o.edge_fluxes()
+    inflow = np.zeros(w.n_edges, bool)
+    for sid, typ, _ in w.strings:
+        if typ == C.BC_INFLOW_Q:
+            inflow |= w.edge_cell[:, 1] == -3 - sid
+    for nm, a, b in zip(("F1", "F3", "GL", "GR"), F[:4], Fo):
+        # bit-identical except where cbrt enters (conveyance-weighted inflow / normal-depth outflow edges)
+        plain = np.ones(w.n_edges, bool)
+        for sid, typ, _ in w.strings:
+            plain &= w.edge_cell[:, 1] != -3 - sid
+        assert np.array_equal(a[plain], b[plain]), nm
+        assert np.allclose(a[~plain], b[~plain], rtol=1e-14, atol=0), nm
+    assert_state_close(s.get_state(), o.get_state(), name)
+    check_info(ig, io)
+    s.close()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_parity_100_steps(gpu, ref, name):
+    """The north_star bar: 100 steps, state <= 1e-10 relative, dt <= 1e-12 relative, identical wet/dry masks.
+    Stepped in chunks of 1, 9 and 90 so that graph launches, tails and repeated calls are all exercised."""
+    w = CASES[name]()
+    o = ref.RefSolver(w)
+    s = gpu.from_workload(w)
+    for n in (1, 9, 90):
+        io = o.step(n, float("inf"), w.cfl)
+        ig = s.step(n, float("inf"), w.cfl)
+        so, sg = o.get_state(), s.get_state()
+        assert np.array_equal(sg[0] > w.h_dry, so[0] > w.h_dry), "wet/dry masks differ"
+        assert_state_close(sg, so, f"{name} after {io['steps_done']} steps")
+        check_info(ig, io)
+        assert abs(s.peek_dt(w.cfl) - o.peek_dt(w.cfl)) <= DT_RTOL * o.peek_dt(w.cfl)
+    assert io["steps_done"] == 100
+    s.close()
+
+
+def test_config1_to_t_end(gpu, ref):
+    """BASELINE.json configs[0] in full: Ritter dam break to t = 4 s; the last step lands on t_end exactly."""
+    w = C.config1()
+    o, s, io, ig = run_both(gpu, ref, w, -1, w.t_end)
+    assert ig["t"] == 4.0 and io["t"] == 4.0
+    check_info(ig, io)
+    assert_state_close(s.get_state(), o.get_state(), "config1 t=4")
+    # calling again does nothing
+    ig2 = s.step(-1, w.t_end, w.cfl)
+    assert ig2["steps_done"] == ig["steps_done"] and ig2["t"] == 4.0
+    s.close()
+
+
+def test_config2_lake_at_rest_1000_steps(gpu, ref):
+    """BASELINE.json configs[1] in full (80k cells, 1000 steps): |u|,|v| <= 1e-12, mass to round-off, and parity."""
+    w = C.config2()
+    s = gpu.from_workload(w)
+    ig = s.step(1000, float("inf"), w.cfl)
+    h, hu, hv = s.get_state()
+    wet = h > w.h_dry
+    assert np.array_equal(wet, w.h > w.h_dry)
+    assert np.max(np.abs(hu[wet] / h[wet])) <= 1e-12 and np.max(np.abs(hv[wet] / h[wet])) <= 1e-12
+    area = s.geometry()[0]
+    assert abs(np.sum(h * area) - np.sum(w.h * area)) <= 1e-13 * np.sum(w.h * area)
+    assert ig["vol_clipped"] == 0.0
+    o = ref.RefSolver(w)
+    io = o.step(1000, float("inf"), w.cfl)
+    check_info(ig, io)
+    assert_state_close((h, hu, hv), o.get_state(), "config2 1000 steps")
+    s.close()
+
+
+@pytest.mark.parametrize("name", ["config3-small", "config4-small"])
+def test_renumbering_does_not_change_results(gpu, name):
+    """R-15: Morton numbering vs caller numbering vs a randomly permuted input: bit-identical states."""
+    w = CASES[name]()
+    a = gpu.from_workload(w, renumber=gpu.RENUMBER_NONE)
+    b = gpu.from_workload(w, renumber=gpu.RENUMBER_MORTON)
+    wp, cp = w.permuted(7)
+    c = gpu.from_workload(wp, renumber=gpu.RENUMBER_MORTON)
+    for s in (a, b, c):
+        s.step(60, float("inf"), w.cfl)
+    sa, sb, sc = a.get_state(), b.get_state(), c.get_state()
+    for x, y, z in zip(sa, sb, sc):
+        assert np.array_equal(x, y)
+        assert np.array_equal(x[cp], z)
+    perm = b.permutation()[0]
+    assert np.array_equal(np.sort(perm), np.arange(w.n_cells)) and not np.array_equal(perm, np.arange(w.n_cells))
+    for s in (a, b, c):
+        s.close()
+
+
+def test_graph_and_plain_launches_agree(gpu):
+    """The CUDA-graph step loop and plain kernel launches give bit-identical states; launch counts add up."""
+    w = CASES["config4-small"]()
+    a = gpu.from_workload(w, steps_per_graph=0)
+    b = gpu.from_workload(w, steps_per_graph=8)
+    c = gpu.from_workload(w, steps_per_graph=32)
+    infos = [s.step(75, float("inf"), w.cfl) for s in (a, b, c)]
+    for s in (b, c):
+        for x, y in zip(a.get_state(), s.get_state()):
+            assert np.array_equal(x, y)
+    assert infos[0] == infos[1] == infos[2]
+    assert a.kernel_launches >= 75 * 4
+    for s in (a, b, c):
+        s.close()
+
+
+def test_restart_round_trip(gpu):
+    """S9 / O-10: get_state at step 50 -> new context -> set_state -> 50 more == 100 straight steps, bitwise."""
+    w = CASES["config3-small"]()
+    a = gpu.from_workload(w)
+    a.step(100, float("inf"), w.cfl)
+    b = gpu.from_workload(w)
+    i50 = b.step(50, float("inf"), w.cfl)
+    st = b.get_state()
+    c = gpu.from_workload(w)
+    c.set_state(*st, t0=i50["t"])
+    ic = c.step(50, float("inf"), w.cfl)
+    for x, y in zip(a.get_state(), c.get_state()):
+        assert np.array_equal(x, y)
+    assert ic["steps_done"] == 50
+    for s in (a, b, c):
+        s.close()
+
+
+def test_state_on_device_and_own_workspace(gpu):
+    """Device-pointer state (torch tensors) and a library-owned workspace give the same results as host pointers."""
+    import torch
+    w = CASES["config3-small"]()
+    a = gpu.from_workload(w)
+    b = gpu.from_workload(w, state_on_device=True)
+    c = gpu.from_workload(w, own_workspace=True)
+    for s in (a, b, c):
+        s.step(40, float("inf"), w.cfl, info=False)
+    ref_state = a.get_state()
+    dev = b.get_state()
+    torch.cuda.synchronize()
+    for x, y, z in zip(ref_state, dev, c.get_state()):
+        assert np.array_equal(x, y.cpu().numpy())
+        assert np.array_equal(x, z)
+    for s in (a, b, c):
+        s.close()
+
+
+def test_tables_built_by_the_library(gpu):
+    """edge_cell / cell_edge = NULL: the library builds both; all boundary edges are walls; same result as the
+    harness tables up to the edge numbering."""
+    w = CASES["config2-lake-small"]()
+    a = gpu.from_workload(w)
+    b = gpu.Solver(w.node_xy, w.tri, None, None, w.zb, w.kst, h_dry=w.h_dry)
+    b.set_state(w.h, w.hu, w.hv)
+    ec, ce = b.tables()
+    assert b.n_edges == w.n_edges
+    # slot k of cell i is the edge between tri[k] and tri[(k+1)%3], L/R consistent
+    for k in range(3):
+        e = ce[:, k]
+        assert np.all((ec[e, 0] == np.arange(w.n_cells)) | (ec[e, 1] == np.arange(w.n_cells)))
+    a.step(30, float("inf"), 0.9)
+    b.step(30, float("inf"), 0.9)
+    for x, y in zip(a.get_state(), b.get_state()):
+        assert np.array_equal(x, y)
+    a.close()
+    b.close()
+
+
+def test_degenerate_and_error_cases(gpu):
+    w = C.tiny_mesh("two-cells")
+    # all dry, dt_max = inf: dt unbounded -> flag, no step, no hang
+    s = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s.set_state(np.zeros(2), np.zeros(2), np.zeros(2))
+    info = s.step(5, float("inf"), 0.9)
+    assert info["steps_done"] == 0 and info["flags"] & gpu.FLAG_DT_UNBOUNDED
+    # all dry with a finite dt_max: steps of dt_max that change nothing
+    s2 = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst, dt_max=2.0)
+    s2.set_state(np.zeros(2), np.zeros(2), np.zeros(2))
+    info = s2.step(3, float("inf"), 0.9)
+    assert info["steps_done"] == 3 and info["t"] == 6.0 and info["vol"] == 0.0
+    # n_steps = 0 is a no-op; unlimited steps without t_end is refused
+    assert s2.step(0, float("inf"), 0.9)["steps_done"] == 3
+    with pytest.raises(gpu.SweError) as ei:
+        s2.step(-1, float("inf"), 0.9)
+    assert ei.value.code == gpu.EINVAL
+    # clockwise triangle -> SWE_EMESH
+    bad = w.tri.copy()
+    bad[0] = bad[0][::-1]
+    with pytest.raises(gpu.SweError) as ei:
+        gpu.Solver(w.node_xy, bad, None, None, w.zb, w.kst)
+    assert ei.value.code == gpu.EMESH
+    # inconsistent tables -> SWE_EMESH
+    ec = w.edge_cell.copy()
+    ec[:, 0] = ec[::-1, 0]
+    with pytest.raises(gpu.SweError) as ei:
+        gpu.Solver(w.node_xy, w.tri, ec, w.cell_edge, w.zb, w.kst)
+    assert ei.value.code == gpu.EMESH
+    # non-finite state is reported
+    s3 = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s3.set_state(np.array([1.0, np.nan]), np.zeros(2), np.zeros(2))
+    with pytest.raises(gpu.SweError) as ei:
+        s3.step(1, float("inf"), 0.9)
+    assert ei.value.code == gpu.ENONFINITE
+    # boundary string that no edge belongs to
+    with pytest.raises(gpu.SweError):
+        s.set_boundary(3, gpu.BC_INFLOW_Q, [0.0, 1.0])
+    for x in (s, s2, s3):
+        x.close()
+
+
+def test_hand_values_through_the_abi(gpu):
+    """The worked interior-edge values of tests/golden/hand_fluxes.txt through the CUDA path:
+    two cells sharing the edge x = 1 with normal (1, 0)."""
+    import os
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "hand_fluxes.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                case, q, v = line.split()
+                gold[(case, q)] = float(v)
+    w = C.tiny_mesh("two-cells-x")
+    w.zb = np.array([0.0, 0.5])
+    s = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s.set_state(np.array([2.0, 1.0]), np.array([2.0, 0.0]), np.array([1.0, 0.0]))
+    s.step(1, float("inf"), 1e-6)          # tiny CFL: theta = 1
+    F1, F3, GL, GR, theta = s.edge_fluxes()
+    e = int(np.nonzero(w.edge_cell[:, 1] >= 0)[0][0])
+    sign = 1.0 if w.edge_cell[e, 0] == 0 else -1.0   # normal stored from L to R; the hand values are for L = cell 0
+    assert sign == 1.0
+    assert abs(F1[e] - gold[("interior", "F1")]) < 5e-13
+    assert abs(F3[e] - gold[("interior", "F3")]) < 5e-13
+    assert abs(GL[e] - gold[("interior", "GL")]) < 5e-12
+    assert abs(GR[e] - gold[("interior", "GR")]) < 5e-12
+    assert np.all(theta == 1.0)
+    s.close()
