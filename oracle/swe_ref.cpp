@@ -6,6 +6,7 @@
 #include "swe_ref.h"
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <limits>
 #include <map>
@@ -107,6 +108,65 @@ extern "C" void swe_ref_wall_flux_via_ghost(double g, double he, double un, doub
   riemann_nt(g, he, un, ut, 0.0, he, -un, ut, 0.0, F1o, F3o, Go, &GR);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Cube root, CORRECTLY ROUNDED (round to nearest) -- DESIGN.md R-14.  The friction term needs
+// h^(7/3) (Eq. 2 with the Strickler row of Table 1) and the conveyance weights
+// h^(5/3); a library cbrt is only good to 1 ulp and differs between libraries, which a 100-step
+// run amplifies.  "The nearest double to the real cube root" is a definition, not an algorithm,
+// so both sides can meet it independently.  Here it is found the slow, checkable way:
+//   x = M * 2^E (M a 53-bit integer).  Pick s in {107,108,109} with (E - s) divisible by 3 and let
+//   X = M * 2^s, an integer in [2^159, 2^162).  T = floor(X^(1/3)) is a 54-bit integer in
+//   [2^53, 2^54): one bit more than a double holds.  T is found from a library estimate and then
+//   corrected with exact 192-bit integer cubes until T^3 <= X < (T+1)^3.  X^(1/3) is never a
+//   half-way point (an odd T has an odd cube, X is even), so rounding T's last bit is exact:
+//   mantissa K = (T + 1) >> 1, result K * 2^((E - s)/3 + 1).
+// ------------------------------------------------------------------------------------------------
+struct U192 { uint64_t w[3]; };   // little-endian limbs
+
+static U192 cube_u64(uint64_t t) {   // t < 2^55: t^3 < 2^165
+  typedef unsigned __int128 u128;
+  const u128 sq = (u128)t * t;                         // < 2^110
+  const uint64_t sq_lo = (uint64_t)sq, sq_hi = (uint64_t)(sq >> 64);
+  const u128 a = (u128)sq_lo * t;                      // contributes at limb 0
+  const u128 b = (u128)sq_hi * t;                      // contributes at limb 1
+  U192 r;
+  r.w[0] = (uint64_t)a;
+  const u128 mid = (a >> 64) + (u128)(uint64_t)b;
+  r.w[1] = (uint64_t)mid;
+  r.w[2] = (uint64_t)(b >> 64) + (uint64_t)(mid >> 64);
+  return r;
+}
+
+static bool less_equal(const U192 &a, const U192 &b) {  // a <= b
+  for (int k = 2; k >= 0; --k) {
+    if (a.w[k] < b.w[k]) return true;
+    if (a.w[k] > b.w[k]) return false;
+  }
+  return true;
+}
+
+extern "C" double swe_ref_cbrt(double x) {
+  if (x == 0.0 || !std::isfinite(x)) return x;
+  if (x < 0.0) return -swe_ref_cbrt(-x);
+  int ex;
+  const double fr = std::frexp(x, &ex);                  // x = fr * 2^ex, fr in [0.5, 1); exact, also for subnormals
+  const uint64_t M = (uint64_t)std::ldexp(fr, 53);       // 53-bit integer, x = M * 2^E
+  const int E = ex - 53;
+  int s = 107;
+  while (((E - s) % 3) != 0) ++s;                        // s in {107, 108, 109}
+  const int q = (E - s) / 3;                             // x^(1/3) = X^(1/3) * 2^q
+  U192 X;                                                // X = M << s
+  X.w[0] = 0;
+  X.w[1] = M << (s - 64);
+  X.w[2] = M >> (128 - s);
+  // estimate of T from the library cube root of X / 2^159 in [1, 8)
+  uint64_t T = (uint64_t)std::ldexp(std::cbrt(std::ldexp((double)M, s - 159)), 53);
+  while (!less_equal(cube_u64(T), X)) --T;               // now T^3 <= X
+  while (less_equal(cube_u64(T + 1), X)) ++T;            // now X < (T+1)^3
+  const uint64_t K = (T + 1) >> 1;                       // round to 53 bits; never a tie
+  return std::ldexp((double)K, q + 1);
+}
+
 namespace {
 
 // fixed-shape pairwise tree in string order (R-11): pad to a power of two with zeros,
@@ -122,7 +182,7 @@ double tree_sum(std::vector<double> v) {
 }
 
 inline double pow53(double he) {       // he^(5/3)
-  const double c3 = std::cbrt(he);
+  const double c3 = swe_ref_cbrt(he);
   return (he * c3) * c3;
 }
 
@@ -302,7 +362,7 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
       qxn = c->qx[i] - a * dX;
       qyn = c->qy[i] - a * dY;
       if (c->gn2[i] > 0.0) {   // split friction, exact integral of dq/dt = -gamma |q| q (R-5, R-6)
-        const double D = 1.0 + ((dt * c->gn2[i]) * std::sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * std::cbrt(hn));
+        const double D = 1.0 + ((dt * c->gn2[i]) * std::sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * swe_ref_cbrt(hn));
         qxn = qxn / D;
         qyn = qyn / D;
       }

@@ -74,6 +74,8 @@ void swe_ref_wall_flux_via_ghost(double g, double he, double un, double ut, doub
 int swe_ref_get_geometry(swe_ref_ctx *c, double *area, double *nx, double *ny, double *len);
 /* per-edge outputs of the most recent step: F1, F3, GL, GR [n_edges] each */
 int swe_ref_get_edge_flux(swe_ref_ctx *c, double *F1, double *F3, double *GL, double *GR);
+/* cube root rounded to nearest (R-14): the only non-IEEE-basic operation of the scheme */
+double swe_ref_cbrt(double x);
 /* dt that S0 would choose now for (cfl, t_end) without advancing */
 double swe_ref_peek_dt(swe_ref_ctx *c, double cfl, double t_end);
 

@@ -61,6 +61,8 @@ def lib():
         L.swe_ref_get_edge_flux.argtypes = [C.c_void_p, _f64p, _f64p, _f64p, _f64p]
         L.swe_ref_peek_dt.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.swe_ref_peek_dt.restype = C.c_double
+        L.swe_ref_cbrt.argtypes = [C.c_double]
+        L.swe_ref_cbrt.restype = C.c_double
         _lib = L
     return _lib
 
@@ -74,6 +76,11 @@ def edge_flux(g, heL, uL, vL, zL, heR, uR, vR, zR, nx, ny):
     o = [C.c_double() for _ in range(4)]
     lib().swe_ref_edge_flux(g, heL, uL, vL, zL, heR, uR, vR, zR, nx, ny, *[C.byref(x) for x in o])
     return tuple(x.value for x in o)
+
+
+def cbrt(x):
+    """Cube root rounded to nearest (R-14)."""
+    return lib().swe_ref_cbrt(float(x))
 
 
 def wall_flux_via_ghost(g, he, un, ut):

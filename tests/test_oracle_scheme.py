@@ -239,3 +239,62 @@ def test_hydrograph_inflow_bookkeeping(ref):
         assert abs(info["vol_in"] - vin) < 1e-11 * max(1.0, vin)
         assert abs(info["vol"] - v0 - info["vol_in"]) < 1e-10 * v0
         assert info["vol_clipped"] < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# R-14: the oracle's cube root is the correctly rounded one.  Pin: exact integer arithmetic in Python
+# (fractions of big integers), which shares nothing with the C++ limbs.
+# ------------------------------------------------------------------------------------------------
+def _cbrt_rn_exact(x: float) -> float:
+    """Nearest double to x^(1/3), by exact comparison of cubes of big integers."""
+    import math
+    from fractions import Fraction
+    if x == 0.0:
+        return x
+    if x < 0:
+        return -_cbrt_rn_exact(-x)
+    fx = Fraction(x)
+    k = max(0, 70 - math.frexp(x)[1] // 3)    # estimate: integer cube root of floor(x * 8^k) (>= 64 bits), as a double
+    n = int(fx * 8 ** k)
+    t = 1 << (n.bit_length() // 3 + 1)
+    while True:                               # integer Newton from above
+        u = (2 * t + n // (t * t)) // 3
+        if u >= t:
+            break
+        t = u
+    y = float(Fraction(t, 2 ** k))
+    for _ in range(8):                        # walk to the double whose rounding interval holds the root
+        lo = Fraction(y) - (Fraction(y) - Fraction(math.nextafter(y, 0.0))) / 2
+        hi = Fraction(y) + (Fraction(math.nextafter(y, math.inf)) - Fraction(y)) / 2
+        if lo ** 3 > fx:
+            y = math.nextafter(y, 0.0)
+        elif hi ** 3 < fx:
+            y = math.nextafter(y, math.inf)
+        else:
+            assert lo ** 3 != fx and hi ** 3 != fx     # no ties exist
+            return y
+    raise AssertionError("estimate too far off")
+
+
+def test_cbrt_is_correctly_rounded(ref):
+    import math
+    rng = np.random.default_rng(128620)
+    xs = [1.0, 8.0, 27.0, 0.125, 1e-3, 2.0, 3.0, 7.999999999999999, 1.0000000000000002, 5e-324, 2.2250738585072014e-308,
+          1.7976931348623157e308, 0.001 + 1e-18, 10.0, 1e-300, 3.0 ** 30, -8.0, -2.5]
+    xs += list(np.exp(rng.uniform(np.log(1e-6), np.log(1e4), 20000)))      # depths in metres
+    xs += list(np.ldexp(rng.uniform(0.5, 1.0, 3000), rng.integers(-1070, 1023, 3000)))
+    # hard cases: doubles right next to the cube of a half-way point m * 2^-53, m odd (54 bits)
+    for _ in range(3000):
+        m = int(rng.integers(2 ** 53, 2 ** 54)) | 1
+        c = (m ** 3) >> (159 - 52)            # 53-56 significant bits of m^3, as an integer
+        k = int(rng.integers(-30, 30))
+        for d in (0, 1):
+            xs.append(math.ldexp(float(c + d), 3 * k - 52) if c + d < 2 ** 53 else math.ldexp(float((c >> 3) + d), 3 * k - 49))
+    n_hard = 0
+    for x in xs:
+        got = ref.cbrt(x)
+        want = _cbrt_rn_exact(x)
+        assert got == want, (x, got, want)
+        n_hard += got != math.copysign(abs(x) ** (1.0 / 3.0), x)
+    assert n_hard > 100                        # the pin does separate a 1-ulp cbrt from the rounded one
+    assert ref.cbrt(0.0) == 0.0 and math.isinf(ref.cbrt(math.inf))
