@@ -137,6 +137,9 @@ int swe_peek_dt(swe_ctx *ctx, double cfl, double t_end, double *dt);
 int swe_get_permutation(swe_ctx *ctx, int32_t *cell_perm, int32_t *edge_perm);
 /* edge tables as used (identical to the caller's when those were given): for meshes passed without tables */
 int swe_get_tables(swe_ctx *ctx, int64_t *n_edges, int32_t *edge_cell, int32_t *cell_edge);
+/* y[i] = cube root of x[i] rounded to nearest, evaluated on the device by the function the kernels use (R-14);
+ * x, y: HOST pointers [n]; uses the current device and the legacy default stream; needs no context */
+int swe_device_cbrt(const double *x, double *y, int64_t n);
 /* number of kernel launches enqueued by this context since swe_create (graph nodes count individually) */
 int64_t swe_kernel_launches(const swe_ctx *ctx);
 

@@ -34,7 +34,7 @@ _i32p = C.POINTER(C.c_int32)
 EXPORTS = (
     "swe_params_default", "swe_workspace_bytes", "swe_create", "swe_set_boundary", "swe_set_state", "swe_step",
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
-    "swe_get_permutation", "swe_get_tables", "swe_kernel_launches",
+    "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches",
 )
 
 
@@ -94,6 +94,7 @@ def lib():
         L.swe_peek_dt.argtypes = [C.c_void_p, C.c_double, C.c_double, _f64p]
         L.swe_get_permutation.argtypes = [C.c_void_p, _i32p, _i32p]
         L.swe_get_tables.argtypes = [C.c_void_p, C.POINTER(C.c_int64), _i32p, _i32p]
+        L.swe_device_cbrt.argtypes = [_f64p, _f64p, C.c_int64]
         L.swe_kernel_launches.argtypes = [C.c_void_p]
         L.swe_kernel_launches.restype = C.c_int64
         _lib = L
@@ -234,6 +235,16 @@ class Solver:
     @property
     def kernel_launches(self):
         return int(lib().swe_kernel_launches(self._h))
+
+
+def device_cbrt(x):
+    """Cube root rounded to nearest as the kernels evaluate it (swe_device_cbrt; R-14)."""
+    x = np.ascontiguousarray(x, np.float64)
+    y = np.empty_like(x)
+    rc = lib().swe_device_cbrt(_p(x, _f64p), _p(y, _f64p), int(x.size))
+    if rc != OK:
+        raise SweError(rc, lib().swe_last_error(None).decode())
+    return y
 
 
 def from_workload(w, **kw):

@@ -527,6 +527,22 @@ int swe_get_tables(swe_ctx *c, int64_t *n_edges, int32_t *edge_cell, int32_t *ce
   return SWE_OK;
 }
 
+int swe_device_cbrt(const double *x, double *y, int64_t n) {
+  if (n < 0 || (n > 0 && (!x || !y))) return SWE_EINVAL;
+  if (n == 0) return SWE_OK;
+  double *d = nullptr;
+  if (cudaMalloc((void **)&d, 16 * (size_t)n) != cudaSuccess) return SWE_ECUDA;
+  cudaError_t e = cudaMemcpy(d, x, 8 * (size_t)n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    k_cbrt<<<(unsigned)((n + kBlock - 1) / kBlock), kBlock>>>(d, d + n, (long long)n);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(y, d + n, 8 * (size_t)n, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) { g_create_error = std::string("swe_device_cbrt: ") + cudaGetErrorString(e); return SWE_ECUDA; }
+  return SWE_OK;
+}
+
 int64_t swe_kernel_launches(const swe_ctx *c) { return c ? c->launches : 0; }
 
 }  // extern "C"

@@ -11,6 +11,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "swe_cbrt.cuh"
 #include "swe_types.h"
 
 namespace swe {
@@ -74,7 +75,7 @@ __device__ __forceinline__ EdgeFlux riemann_nt(double g, double hL, double unL, 
 }
 
 __device__ __forceinline__ double pow53(double h) {  // h^(5/3), Strickler conveyance (Table 1)
-  const double c3 = cbrt(h);
+  const double c3 = cbrt_rn(h);
   return (h * c3) * c3;
 }
 
@@ -271,7 +272,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       qyn = c.qy - a * dY;
       const double f2 = gn2[i];
       if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
-        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt(hn));
+        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_rn(hn));
         qxn = qxn / D;
         qyn = qyn / D;
       }
@@ -485,6 +486,13 @@ k_unpack_state(const int *__restrict__ cell_perm, const CellRec *__restrict__ re
   const int o = cell_perm[i];
   const CellRec c = rec[i];
   h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
+}
+
+// inspection (swe_device_cbrt): the cube root of R-14 as the kernels evaluate it
+__global__ void __launch_bounds__(kBlock)
+k_cbrt(const double *__restrict__ x, double *__restrict__ y, long long n) {
+  const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+  if (i < n) y[i] = cbrt_rn(x[i]);
 }
 
 // inspection (swe_get_edge_flux): per-edge records after the limiter, in caller edge numbering

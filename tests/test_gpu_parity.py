@@ -324,3 +324,22 @@ def test_hand_values_through_the_abi(gpu):
     assert abs(GR[e] - gold[("interior", "GR")]) < 5e-12
     assert np.all(theta == 1.0)
     s.close()
+
+
+def test_device_cbrt_matches(gpu, ref):
+    """R-14: the kernels' cube root is the correctly rounded one, like the oracle's (pinned against exact integer
+    arithmetic in test_oracle_scheme.py): random mantissas over 600 binades, neighbours of exact cubes and of
+    powers of two, subnormals, the ends of the range."""
+    rng = np.random.default_rng(128620)
+    x = np.ldexp(1.0 + rng.random(400000), rng.integers(-300, 300, 400000))
+    i = np.arange(1.0, 20001.0)
+    cubes = i * i * i
+    pw = np.ldexp(1.0, np.arange(-1070, 1020))
+    near = np.concatenate([np.nextafter(c, d) for c in (cubes, pw) for d in (0.0, np.inf)] +
+                          [np.nextafter(np.nextafter(pw, 0.0), 0.0), np.nextafter(np.nextafter(pw, np.inf), np.inf)])
+    x = np.concatenate([x, cubes, pw, near, [5e-324, 1e-310, 1.7e308, 0.0, 1e-3, 1.0]])
+    x = x[np.isfinite(x) & (x >= 0)]
+    got = gpu.device_cbrt(x)
+    want = np.array([ref.cbrt(float(v)) for v in x])
+    assert np.array_equal(got, want)
+    assert np.array_equal(gpu.device_cbrt(-x[:1000]), -want[:1000])
