@@ -1,0 +1,334 @@
+"""bench.py -- cell-updates/s (fp64) of the shallow-water step loop on B200, with its HBM roofline fraction.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--scale 1.0]
+
+One bench "step" = `--time-steps` (default 100) consecutive time steps of the whole hot path (S0..S4 of
+include/swe.h: dt, edge fluxes, limiter, gather, update + friction, CFL reduction) over the whole mesh, enqueued by
+ONE swe_step call (CUDA-graph launches, no host synchronisation inside).  Workload: BASELINE.json configs[3], the
+~4M-cell river-reach flood wave with wetting/drying (the workload the north_star's target is quoted on), seeded
+synthetic (workloads/configs.py).  metric = cell-updates/s = cells x time steps / device time.
+
+N > 1 (torchrun): the path is single-GPU by design ("replicas only"): every rank steps its
+own replica of the same workload, no data-path collective; value = all ranks' cell-updates / max-over-ranks time.
+
+--impl reference: the oracle (oracle/, plain single-threaded C++) timed on the host cores on the same workload;
+one step = ONE time step of the whole mesh (a bounded sample of the 100-time-step step above).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures under
+# profiles/ (kernel name, n_cells) -> bytes; absent -> "traffic": null
+NCU_TRAFFIC_BYTES = {}
+
+METRIC = "cell_updates_per_s"
+UNIT = "cell-updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[id-1]")
+    ap.add_argument("--scale", type=float, default=1.0, help="cell-count scale of the workload (1.0 = as named)")
+    ap.add_argument("--time-steps", type=int, default=100, help="time steps per bench step (our arm)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--profile-steps", type=int, default=64, help="event-bracketed steps for the roofline object")
+    return ap.parse_args()
+
+
+def peaks():
+    """HBM GB/s denominator: MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_workload(config_id, scale, rank=0, world=1, barrier=None):
+    """Seeded synthetic workload; rank 0 generates, the others read its cache file (generation is ~50 s at 4M)."""
+    from workloads import configs as C
+    if world == 1:
+        return C.by_id(config_id, scale)
+    import pickle
+    path = f"/tmp/swe_b200_workload_c{config_id}_s{scale:g}_{os.environ.get('MASTER_PORT', '0')}.pkl"
+    if rank == 0:
+        w = C.by_id(config_id, scale)
+        meta, w.meta = w.meta, {}
+        with open(path + ".tmp", "wb") as f:
+            pickle.dump(w, f, protocol=4)
+        os.replace(path + ".tmp", path)
+        w.meta = meta
+        barrier()
+    else:
+        barrier()
+        with open(path, "rb") as f:
+            w = pickle.load(f)
+    barrier()
+    if rank == 0:
+        try:
+            os.remove(path)
+        except OSError:
+            pass
+    return w
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+            getattr(nv, "nvmlClocksEventReasonApplicationsClocksSetting", 0x2): "applications_clocks_setting",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def oracle_time(w, n_warm, max_steps, min_seconds, cfl):
+    """The oracle as it stands on this box's host cores (single thread): (cell-updates/s, time steps timed, s)."""
+    from oracle import swe_ref
+    o = swe_ref.RefSolver(w)
+    if n_warm:
+        o.step(n_warm, float("inf"), cfl)
+    done, t0 = 0, time.perf_counter()
+    while done < max_steps:
+        o.step(1, float("inf"), cfl)
+        done += 1
+        if time.perf_counter() - t0 >= min_seconds:
+            break
+    dt = time.perf_counter() - t0
+    o.close()
+    return w.n_cells * done / dt, done, dt
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle on the host cores; one step = one time step of the whole mesh."""
+    if rank != 0:
+        return
+    from oracle import swe_ref
+    w = load_workload(args.config, args.scale)
+    o = swe_ref.RefSolver(w)
+    for _ in range(args.warmup):
+        o.step(1, float("inf"), w.cfl)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(1, float("inf"), w.cfl)
+    dt = time.perf_counter() - t0
+    o.close()
+    value = w.n_cells * args.steps / dt
+    sample = f"all {w.n_cells} cells x 1 time step per step (the GPU arm's step is {args.time_steps} time steps)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "baseline_config": args.config, "n_cells": w.n_cells, "n_edges": w.n_edges,
+                   "time_steps_per_step": 1, "cfl": w.cfl},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    import paper_2102_12862_b200 as P
+    P.lib()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    w = load_workload(args.config, args.scale, rank, world, barrier)
+    N, E, T = w.n_cells, w.n_edges, args.time_steps
+    t_create = time.perf_counter()
+    s = P.from_workload(w, device=f"cuda:{local_rank}")
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t_create
+    stream = torch.cuda.current_stream(dev)
+
+    # ---- device-resident arm: W warm-up steps, then exactly K steps between barrier + synchronize on both sides
+    for _ in range(args.warmup):
+        s.step(T, float("inf"), w.cfl, info=False)
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    launches0 = s.kernel_launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        s.step(T, float("inf"), w.cfl, info=False)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = s.kernel_launches - launches0
+    info = s.step(0, float("inf"), w.cfl, info=True)       # state check after the timed region: finite, mass balance
+    if world > 1:
+        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * N * T * args.steps / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel: event-bracketed kernels inside the library (rank 0)
+    roofline = None
+    kernel_ms = None
+    if rank == 0:
+        kernel_ms = s.profile_step(args.profile_steps, w.cfl)
+        alg = P.algorithmic_bytes(N, E)
+        top = max(kernel_ms, key=kernel_ms.get)
+        peak, how = peaks()
+        achieved = alg[top] / (kernel_ms[top] * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((top, N)), "peak_source": how,
+                    "algorithmic_bytes_per_launch": alg[top], "kernel_ms": kernel_ms[top],
+                    "step_algorithmic_bytes": sum(alg.values()),
+                    "step_achieved": sum(alg.values()) / (ms * 1e-3 / (T * args.steps)) / 1e9,
+                    "share_of_step": kernel_ms[top] / sum(kernel_ms.values())}
+
+    # ---- end-to-end arm: the same K steps through the C-ABI with HOST (pinned) buffers, copies inside the region
+    e2e = None
+    if not args.no_e2e:
+        host = [torch.empty(N, dtype=torch.float64, pin_memory=True).numpy() for _ in range(3)]
+        s.get_state(tuple(host))
+        t_now = info["t"]
+        for _ in range(min(2, args.warmup)):
+            s.set_state(*host, t0=t_now)
+            t_now = s.step(T, float("inf"), w.cfl, info=True)["t"]
+            s.get_state(tuple(host))
+        torch.cuda.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            s.set_state(*host, t0=t_now)                               # H2D: 3 x 8 x N bytes
+            t_now = s.step(T, float("inf"), w.cfl, info=True)["t"]    # info: the step's result scalars come back
+            s.get_state(tuple(host))                                   # D2H: 3 x 8 x N bytes
+        torch.cuda.synchronize()
+        dt_e2e = time.perf_counter() - t0
+        if world > 1:
+            tt = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt_e2e = float(tt.item())
+        e2e = {"value": world * N * T * args.steps / dt_e2e, "unit": UNIT, "h2d_bytes_per_step": 24 * N,
+               "d2h_bytes_per_step": 24 * N + 72}
+    s.close()
+
+    # ---- CPU baseline: the oracle, single thread, bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"all {N} cells x {n_done} time steps from the initial state ({secs:.1f} s, 1 thread)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
+                       "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
+                       "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
+                       "create_s": round(t_create, 2)},
+            "ms_per_time_step": ms / (args.steps * T),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu,
+            "state_check": {"t": info["t"], "steps_done": info["steps_done"], "n_wet": info["n_wet"],
+                            "vol_clipped": info["vol_clipped"], "flags": info["flags"]},
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -142,6 +142,14 @@ int swe_get_tables(swe_ctx *ctx, int64_t *n_edges, int32_t *edge_cell, int32_t *
 int swe_device_cbrt(const double *x, double *y, int64_t n);
 /* number of kernel launches enqueued by this context since swe_create (graph nodes count individually) */
 int64_t swe_kernel_launches(const swe_ctx *ctx);
+/* Measurement (bench.py roofline): advances n_steps >= 1 time steps with plain launches, every kernel of the step
+ * bracketed by CUDA events on the context's stream; ms[k] = mean device time of kernel k per step, in
+ * milliseconds, for k < min(n_ms, swe_step_kernel_count()).  Results are those of swe_step(n_steps, +inf, cfl).
+ * It synchronises. */
+int swe_profile_step(swe_ctx *ctx, int64_t n_steps, double cfl, double *ms, int n_ms);
+/* kernels per time step, and the name of kernel k of the step (NULL if k is out of range) */
+int swe_step_kernel_count(void);
+const char *swe_step_kernel_name(int k);
 
 #ifdef __cplusplus
 }

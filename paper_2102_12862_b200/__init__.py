@@ -34,7 +34,8 @@ _i32p = C.POINTER(C.c_int32)
 EXPORTS = (
     "swe_params_default", "swe_workspace_bytes", "swe_create", "swe_set_boundary", "swe_set_state", "swe_step",
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
-    "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches",
+    "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
+    "swe_step_kernel_count", "swe_step_kernel_name",
 )
 
 
@@ -97,6 +98,10 @@ def lib():
         L.swe_device_cbrt.argtypes = [_f64p, _f64p, C.c_int64]
         L.swe_kernel_launches.argtypes = [C.c_void_p]
         L.swe_kernel_launches.restype = C.c_int64
+        L.swe_profile_step.argtypes = [C.c_void_p, C.c_int64, C.c_double, _f64p, C.c_int]
+        L.swe_step_kernel_count.argtypes = []
+        L.swe_step_kernel_name.argtypes = [C.c_int]
+        L.swe_step_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -232,9 +237,37 @@ class Solver:
         self._check(lib().swe_get_tables(self._h, None, _p(ec, _i32p), _p(ce, _i32p)))
         return ec, ce
 
+    def profile_step(self, n_steps, cfl=0.9):
+        """{kernel name: mean device ms per step} over n_steps event-bracketed plain-launch steps (swe_profile_step)."""
+        n = int(lib().swe_step_kernel_count())
+        ms = np.zeros(n)
+        self._check(lib().swe_profile_step(self._h, int(n_steps), float(cfl), _p(ms, _f64p), n))
+        return {lib().swe_step_kernel_name(k).decode(): float(ms[k]) for k in range(n)}
+
     @property
     def kernel_launches(self):
         return int(lib().swe_kernel_launches(self._h))
+
+
+def workspace_bytes(n_cells, n_edges=0):
+    """swe_workspace_bytes: device bytes of a context of this size."""
+    return int(lib().swe_workspace_bytes(int(n_cells), int(n_edges)))
+
+
+def algorithmic_bytes(n_cells, n_edges):
+    """Algorithmic DRAM bytes per launch of every kernel of the step: every datum a kernel
+    needs counted once (perfect reuse of gathered records in L2), at the sizes of the records it moves."""
+    N, E = int(n_cells), int(n_edges)
+    return {
+        "k_step_control": 0,
+        # EdgeGeom read + EdgeFlux written per edge; every CellRec gathered once
+        "k_edge_flux": 64 * E + 32 * N,
+        # cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
+        "k_theta": (16 + 32 + 8 + 8) * N + 64 * E,
+        # cell_edge, 1/area, g/k^2, theta (own + gathered = once) read, CellRec read + written per cell;
+        # every EdgeGeom and EdgeFlux gathered once
+        "k_cell_update": (16 + 8 + 8 + 8 + 64) * N + 64 * E,
+    }
 
 
 def device_cbrt(x):

@@ -85,17 +85,24 @@ namespace {
     }                                                                                             \
   } while (0)
 
-// the four kernels of one time step, in stream order
-void enqueue_step(swe_ctx *c, cudaStream_t s) {
+// the four kernels of one time step, in stream order; ev (nullable) = kKernelsPerStep + 1 events recorded around them
+constexpr int kKernelsPerStep = 4;
+const char *const kStepKernelNames[kKernelsPerStep] = {"k_step_control", "k_edge_flux", "k_theta", "k_cell_update"};
+
+void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
+  if (ev) cudaEventRecord(ev[0], s);
   k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
                                            c->theta, c->rec, c->kst, 0);
+  if (ev) cudaEventRecord(ev[1], s);
   k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne);
+  if (ev) cudaEventRecord(ev[2], s);
   k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                              (int)c->nc);
+  if (ev) cudaEventRecord(ev[3], s);
   k_cell_update<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
                                                    c->inv_area, c->gn2, c->rec, (int)c->nc);
+  if (ev) cudaEventRecord(ev[4], s);
 }
-constexpr int kKernelsPerStep = 4;
 
 int capture_graph(swe_ctx *c) {
   if (c->steps_per_graph <= 0) return SWE_OK;
@@ -544,5 +551,43 @@ int swe_device_cbrt(const double *x, double *y, int64_t n) {
 }
 
 int64_t swe_kernel_launches(const swe_ctx *c) { return c ? c->launches : 0; }
+
+int swe_step_kernel_count(void) { return kKernelsPerStep; }
+
+const char *swe_step_kernel_name(int k) { return (k >= 0 && k < kKernelsPerStep) ? kStepKernelNames[k] : nullptr; }
+
+int swe_profile_step(swe_ctx *c, int64_t n_steps, double cfl, double *ms, int n_ms) {
+  if (!c) return SWE_EINVAL;
+  if (n_steps < 1 || !(cfl > 0.0) || !ms || n_ms < 1) { c->err = "swe_profile_step: bad argument"; return SWE_EINVAL; }
+  constexpr int kBatch = 32;                       // steps between two synchronisations
+  constexpr int kEv = kKernelsPerStep + 1;
+  std::vector<cudaEvent_t> ev((size_t)kBatch * kEv, nullptr);
+  for (auto &e : ev) SWE_CUDA(c, cudaEventCreate(&e));
+  double sum[kKernelsPerStep] = {0.0};
+  k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, (long long)n_steps, std::numeric_limits<double>::infinity(), cfl);
+  c->launches += 1;
+  cudaError_t rc = cudaSuccess;
+  for (int64_t done = 0; done < n_steps && rc == cudaSuccess; done += kBatch) {
+    const int nb = (int)std::min<int64_t>(kBatch, n_steps - done);
+    for (int j = 0; j < nb; ++j) enqueue_step(c, c->stream, ev.data() + (size_t)j * kEv);
+    c->launches += (int64_t)nb * kKernelsPerStep;
+    rc = cudaStreamSynchronize(c->stream);
+    for (int j = 0; j < nb && rc == cudaSuccess; ++j)
+      for (int k = 0; k < kKernelsPerStep && rc == cudaSuccess; ++k) {
+        float t = 0.f;
+        rc = cudaEventElapsedTime(&t, ev[(size_t)j * kEv + k], ev[(size_t)j * kEv + k + 1]);
+        sum[k] += t;
+      }
+  }
+  for (auto &e : ev) cudaEventDestroy(e);
+  SWE_CUDA(c, rc);
+  k_step_control<<<1, kCtlThreads, 0, c->stream>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom,
+                                                   c->flux, c->theta, c->rec, c->kst, 1);
+  c->launches += 1;
+  SWE_CUDA(c, cudaGetLastError());
+  for (int k = 0; k < n_ms; ++k) ms[k] = k < kKernelsPerStep ? sum[k] / (double)n_steps : 0.0;
+  c->t_host = -std::numeric_limits<double>::infinity();
+  return SWE_OK;
+}
 
 }  // extern "C"
