@@ -31,7 +31,8 @@ if ROOT not in sys.path:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures under
 # profiles/ (kernel name, n_cells) -> bytes; absent -> "traffic": null
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {("k_cell_update", 3964806): 737.0e6, ("k_theta", 3964806): 633.2e6,
+                     ("k_edge_flux", 3964806): 476.5e6}   # profiles/r1a_ncu_full_three_pass.md
 
 METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
@@ -146,6 +147,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def max_over_ranks(x, world, device):
+    """Max of a host float over all ranks (the N > 1 timing rule); identity when world == 1."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def aggregate_value(n_cells, time_steps, steps, world, seconds):
+    """Whole-job cell-updates/s: every rank advances its own replica (weak scaling, no data-path collective)."""
+    return world * n_cells * time_steps * steps / seconds
+
+
 def physical_gpu_index(local_rank):
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -254,11 +271,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     launches = s.kernel_launches - launches0
     info = s.step(0, float("inf"), w.cfl, info=True)       # state check after the timed region: finite, mass balance
-    if world > 1:
-        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    value = world * N * T * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = aggregate_value(N, T, args.steps, world, ms * 1e-3)
 
     # ---- roofline of the dominant kernel: event-bracketed kernels inside the library (rank 0)
     roofline = None
@@ -295,11 +309,8 @@ def main():
             s.get_state(tuple(host))                                   # D2H: 3 x 8 x N bytes
         torch.cuda.synchronize()
         dt_e2e = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt_e2e = float(tt.item())
-        e2e = {"value": world * N * T * args.steps / dt_e2e, "unit": UNIT, "h2d_bytes_per_step": 24 * N,
+        dt_e2e = max_over_ranks(dt_e2e, world, dev)
+        e2e = {"value": aggregate_value(N, T, args.steps, world, dt_e2e), "unit": UNIT, "h2d_bytes_per_step": 24 * N,
                "d2h_bytes_per_step": 24 * N + 72}
     s.close()
 

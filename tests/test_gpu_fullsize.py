@@ -1,0 +1,74 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default renumbering,
+default CUDA-graph step loop, one swe_step call per window): configs[3] (river reach, ~4M cells, wetting/drying,
+hydrograph inflow, normal-depth outflow) and configs[2] (circular dam break, ~1M cells).  The oracle steps the
+whole mesh too (about 1 s per step at 4M cells), so the windows are short: one from the initial state and one
+re-started from the GPU's own state deep into the run (get_state -> oracle set_state), where the flood wave has
+wetted part of the floodplain.  All cells are compared; mass balance and wet counts are checked as well."""
+import numpy as np
+import pytest
+
+from workloads import configs as C
+
+from test_gpu_parity import assert_state_close, check_info, DT_RTOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box")
+    import paper_2102_12862_b200 as P
+    P.lib()
+    return P
+
+
+def window(s, o, w, n, what):
+    ig = s.step(n, float("inf"), w.cfl)
+    io = o.step(n, float("inf"), w.cfl)
+    sg, so = s.get_state(), o.get_state()
+    assert np.array_equal(sg[0] > w.h_dry, so[0] > w.h_dry), f"{what}: wet/dry masks differ"
+    assert_state_close(sg, so, what)
+    assert ig["n_wet"] == io["n_wet"] and ig["steps_done"] == io["steps_done"]
+    assert abs(ig["dt_last"] - io["dt_last"]) <= DT_RTOL * io["dt_last"]
+    assert abs(ig["t"] - io["t"]) <= DT_RTOL * abs(io["t"])
+    assert abs(ig["vol"] - io["vol"]) <= 1e-12 * io["vol"]
+    return ig, io, sg
+
+
+def test_config4_full_size_windows(gpu, ref):
+    w = C.config4()
+    assert 3.8e6 < w.n_cells < 4.2e6
+    s = gpu.from_workload(w)
+    o = ref.RefSolver(w)
+    area = s.geometry()[0]
+    vol0 = float(np.sum(w.h * area))
+    ig, io, _ = window(s, o, w, 20, "config4 full size, steps 0-20")
+    check_info(ig, io)
+    # deep into the run: 1500 more steps on the GPU only, then both sides continue from the GPU's state
+    ig = s.step(1500, float("inf"), w.cfl)
+    assert ig["flags"] == 0
+    # mass balance over the whole run so far (property that holds at any size)
+    bal = ig["vol"] - vol0 - ig["vol_in"] + ig["vol_out"] - ig["vol_clipped"]
+    assert abs(bal) <= 1e-11 * vol0, bal
+    assert ig["vol_in"] > 0.0 and ig["vol_out"] > 0.0
+    st = s.get_state()
+    assert ig["n_wet"] == int(np.sum(st[0] > w.h_dry)) and ig["n_wet"] != int(np.sum(w.h > w.h_dry))
+    o.set_state(*st, t0=ig["t"])
+    s.set_state(*st, t0=ig["t"])
+    window(s, o, w, 20, "config4 full size, 20 steps from the GPU state at step 1520")
+    s.close()
+    o.close()
+
+
+def test_config3_full_size_window(gpu, ref):
+    w = C.config3()
+    assert 0.95e6 < w.n_cells < 1.05e6
+    s = gpu.from_workload(w)
+    o = ref.RefSolver(w)
+    ig, io, _ = window(s, o, w, 40, "config3 full size, steps 0-40")
+    check_info(ig, io)
+    assert ig["vol_clipped"] == 0.0
+    s.close()
+    o.close()

@@ -180,9 +180,11 @@ def test_mass_closed_box_with_friction(ref):
     assert h.min() >= 0.0 and np.isfinite(hu).all()
 
 
-def test_permutation_invariance(ref):
-    """SURVEY O-9 / R-15: renumbering cells and edges (slot order and L/R kept) leaves the result bit-identical."""
-    w = C.config3(target_cells=3000, lx=110.0)
+@pytest.mark.parametrize("case", ["config3", "config4-strings"])
+def test_permutation_invariance(ref, case):
+    """SURVEY O-9 / R-15: renumbering cells and edges (slot order, L/R and the order of boundary-string members
+    kept) leaves the result bit-identical."""
+    w = C.config3(target_cells=3000, lx=110.0) if case == "config3" else C.by_id(4, 0.002)
     wp, cp = w.permuted(seed=3)
     a, b = ref.RefSolver(w), ref.RefSolver(wp)
     ia, ib = a.step(n_steps=40), b.step(n_steps=40)

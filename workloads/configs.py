@@ -59,6 +59,10 @@ class Workload:
         rng = np.random.default_rng(seed)
         cp = rng.permutation(self.n_cells)
         ep = rng.permutation(self.n_edges)
+        # members of a boundary string keep their relative order: "string order" = ascending caller edge id
+        # is part of the definition of the string sums (R-11), so it is not a renumbering freedom
+        is_member = self.edge_cell[ep, 1] <= -3
+        ep[is_member] = np.sort(ep[is_member])
         tri, ec, ce = M.permute_mesh(self.tri, self.edge_cell, self.cell_edge, cp, ep)
         w = Workload(self.name + "-perm", self.node_xy, tri, ec, ce, self.zb[cp].copy(),
                      self.kst[cp].copy(), self.h[cp].copy(), self.hu[cp].copy(), self.hv[cp].copy(),
