@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[id-1]")
     ap.add_argument("--scale", type=float, default=1.0, help="cell-count scale of the workload (1.0 = as named)")
     ap.add_argument("--time-steps", type=int, default=100, help="time steps per bench step (our arm)")
+    ap.add_argument("--variant", type=int, default=0, help="include/swe.h SWE_VARIANT_* (0 = library default)")
+    ap.add_argument("--patch-cells", type=int, default=0, help="cells per patch of the fused step (0 = default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--profile-steps", type=int, default=64, help="event-bracketed steps for the roofline object")
@@ -246,10 +248,11 @@ def main():
     w = load_workload(args.config, args.scale, rank, world, barrier)
     N, E, T = w.n_cells, w.n_edges, args.time_steps
     t_create = time.perf_counter()
-    s = P.from_workload(w, device=f"cuda:{local_rank}")
+    s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     stream = torch.cuda.current_stream(dev)
+    s_kernels, patch_stats = s.step_kernels(), s.patch_stats()
 
     # ---- device-resident arm: W warm-up steps, then exactly K steps between barrier + synchronize on both sides
     for _ in range(args.warmup):
@@ -279,7 +282,7 @@ def main():
     kernel_ms = None
     if rank == 0:
         kernel_ms = s.profile_step(args.profile_steps, w.cfl)
-        alg = P.algorithmic_bytes(N, E)
+        alg = s.algorithmic_bytes()
         top = max(kernel_ms, key=kernel_ms.get)
         peak, how = peaks()
         achieved = alg[top] / (kernel_ms[top] * 1e-3) / 1e9
@@ -329,7 +332,7 @@ def main():
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
-                       "create_s": round(t_create, 2)},
+                       "create_s": round(t_create, 2), "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu,

@@ -43,6 +43,9 @@ enum { SWE_EDGE_WALL = -1, SWE_EDGE_TRANSMISSIVE = -2 /* , -3 - s = member of bo
 enum { SWE_BC_NONE = 0 /* string behaves as wall */, SWE_BC_INFLOW_Q = 1, SWE_BC_OUTFLOW_UNIFORM = 2 };
 /* Cell / edge renumbering applied inside the library (invisible at this boundary) */
 enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1 };
+/* Step variant: both compute bit-identical states; AUTO = the one that measured fastest */
+enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta -> CSR gather + update */,
+       SWE_VARIANT_PATCH = 2 /* one fused kernel per step over shared-memory mesh patches */ };
 /* swe_step_info.flags */
 enum { SWE_FLAG_NONFINITE = 1, SWE_FLAG_DT_UNBOUNDED = 2 };
 
@@ -70,9 +73,13 @@ typedef struct {
   int state_on_device;  /* 0: swe_set_state/swe_get_state take HOST pointers (default);
                            1: they take DEVICE pointers (e.g. torch tensors), read/written on stream  */
   int steps_per_graph;  /* time steps captured per CUDA graph launch; default 32; 0 = no graph       */
+  int variant;          /* SWE_VARIANT_*; default AUTO                                               */
+  int patch_cells;      /* cells per patch of the fused step; 0 = default (512)                      */
   void *cuda_stream;    /* cudaStream_t all work is enqueued on; NULL = the legacy default stream    */
   void *workspace;      /* DEVICE memory lent by the caller for the context's lifetime (e.g. a torch
-                           uint8 tensor), 256-byte aligned, or NULL: the library then cudaMallocs   */
+                           uint8 tensor), 256-byte aligned, or NULL: the library then cudaMallocs.
+                           (The patch tables of the fused step, whose size is known only once they are
+                           built, are always allocated by the library.)                             */
   size_t workspace_bytes; /* size of workspace; must be >= swe_workspace_bytes(n_cells, n_edges)     */
 } swe_params;
 
@@ -147,9 +154,16 @@ int64_t swe_kernel_launches(const swe_ctx *ctx);
  * milliseconds, for k < min(n_ms, swe_step_kernel_count()).  Results are those of swe_step(n_steps, +inf, cfl).
  * It synchronises. */
 int swe_profile_step(swe_ctx *ctx, int64_t n_steps, double cfl, double *ms, int n_ms);
-/* kernels per time step, and the name of kernel k of the step (NULL if k is out of range) */
-int swe_step_kernel_count(void);
-const char *swe_step_kernel_name(int k);
+/* kernels per time step of this context's variant, and the name of kernel k of the step (NULL if out of range) */
+int swe_step_kernel_count(const swe_ctx *ctx);
+const char *swe_step_kernel_name(const swe_ctx *ctx, int k);
+/* algorithmic DRAM bytes per launch of kernel k of the step: every datum the kernel needs counted once at the size
+ * of the record that carries it; re-reads of halo cells / duplicated records are NOT counted */
+int64_t swe_algorithmic_bytes(const swe_ctx *ctx, int k);
+/* out[0..8] = variant, patches, cells per patch, dynamic shared memory per block [bytes], sum over patches of local
+ * cells, sum over patches of local edges, largest local cell count, largest local edge count, and the number of
+ * patch-steps since swe_create in which a block found its whole patch dry and skipped the flux work.  It synchronises. */
+int swe_get_patch_stats(swe_ctx *ctx, int64_t *out, int n_out);
 
 #ifdef __cplusplus
 }

@@ -27,6 +27,7 @@ EDGE_WALL, EDGE_TRANSMISSIVE = -1, -2
 BC_NONE, BC_INFLOW_Q, BC_OUTFLOW_UNIFORM = 0, 1, 2
 RENUMBER_NONE, RENUMBER_MORTON = 0, 1
 FLAG_NONFINITE, FLAG_DT_UNBOUNDED = 1, 2
+VARIANT_AUTO, VARIANT_THREE_PASS, VARIANT_PATCH = 0, 1, 2
 
 _f64p = C.POINTER(C.c_double)
 _i32p = C.POINTER(C.c_int32)
@@ -35,7 +36,7 @@ EXPORTS = (
     "swe_params_default", "swe_workspace_bytes", "swe_create", "swe_set_boundary", "swe_set_state", "swe_step",
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
-    "swe_step_kernel_count", "swe_step_kernel_name",
+    "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_get_patch_stats",
 )
 
 
@@ -47,7 +48,8 @@ class SweMesh(C.Structure):
 
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("h_dry", C.c_double), ("dt_max", C.c_double), ("renumber", C.c_int),
-                ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("cuda_stream", C.c_void_p),
+                ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("variant", C.c_int), ("patch_cells", C.c_int),
+                ("cuda_stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -99,9 +101,12 @@ def lib():
         L.swe_kernel_launches.argtypes = [C.c_void_p]
         L.swe_kernel_launches.restype = C.c_int64
         L.swe_profile_step.argtypes = [C.c_void_p, C.c_int64, C.c_double, _f64p, C.c_int]
-        L.swe_step_kernel_count.argtypes = []
-        L.swe_step_kernel_name.argtypes = [C.c_int]
+        L.swe_step_kernel_count.argtypes = [C.c_void_p]
+        L.swe_step_kernel_name.argtypes = [C.c_void_p, C.c_int]
         L.swe_step_kernel_name.restype = C.c_char_p
+        L.swe_algorithmic_bytes.argtypes = [C.c_void_p, C.c_int]
+        L.swe_algorithmic_bytes.restype = C.c_int64
+        L.swe_get_patch_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int]
         _lib = L
     return _lib
 
@@ -116,7 +121,7 @@ class Solver:
 
     def __init__(self, node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, *, g=9.81, h_dry=1e-3,
                  dt_max=float("inf"), renumber=RENUMBER_MORTON, state_on_device=False, steps_per_graph=32,
-                 device="cuda:0", own_workspace=False):
+                 device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -140,6 +145,7 @@ class Solver:
         L.swe_params_default(C.byref(prm))
         prm.g, prm.h_dry, prm.dt_max = float(g), float(h_dry), float(dt_max)
         prm.renumber, prm.state_on_device, prm.steps_per_graph = int(renumber), int(bool(state_on_device)), int(steps_per_graph)
+        prm.variant, prm.patch_cells = int(variant), int(patch_cells)
         self.stream = torch.cuda.current_stream(self.device)
         prm.cuda_stream = self.stream.cuda_stream
         self.workspace = None
@@ -237,12 +243,28 @@ class Solver:
         self._check(lib().swe_get_tables(self._h, None, _p(ec, _i32p), _p(ce, _i32p)))
         return ec, ce
 
+    def step_kernels(self):
+        """Names of the kernels of one time step of this context's variant, in launch order."""
+        n = int(lib().swe_step_kernel_count(self._h))
+        return [lib().swe_step_kernel_name(self._h, k).decode() for k in range(n)]
+
     def profile_step(self, n_steps, cfl=0.9):
         """{kernel name: mean device ms per step} over n_steps event-bracketed plain-launch steps (swe_profile_step)."""
-        n = int(lib().swe_step_kernel_count())
-        ms = np.zeros(n)
-        self._check(lib().swe_profile_step(self._h, int(n_steps), float(cfl), _p(ms, _f64p), n))
-        return {lib().swe_step_kernel_name(k).decode(): float(ms[k]) for k in range(n)}
+        names = self.step_kernels()
+        ms = np.zeros(len(names))
+        self._check(lib().swe_profile_step(self._h, int(n_steps), float(cfl), _p(ms, _f64p), len(names)))
+        return {nm: float(ms[k]) for k, nm in enumerate(names)}
+
+    def algorithmic_bytes(self):
+        """{kernel name: algorithmic DRAM bytes per launch} (swe_algorithmic_bytes)."""
+        return {nm: int(lib().swe_algorithmic_bytes(self._h, k)) for k, nm in enumerate(self.step_kernels())}
+
+    def patch_stats(self):
+        out = (C.c_int64 * 9)()
+        self._check(lib().swe_get_patch_stats(self._h, out, 9))
+        keys = ("variant", "patches", "patch_cells", "smem_bytes", "sum_local_cells", "sum_local_edges",
+                "max_local_cells", "max_local_edges", "patch_steps_skipped")
+        return dict(zip(keys, (int(v) for v in out)))
 
     @property
     def kernel_launches(self):
@@ -252,22 +274,6 @@ class Solver:
 def workspace_bytes(n_cells, n_edges=0):
     """swe_workspace_bytes: device bytes of a context of this size."""
     return int(lib().swe_workspace_bytes(int(n_cells), int(n_edges)))
-
-
-def algorithmic_bytes(n_cells, n_edges):
-    """Algorithmic DRAM bytes per launch of every kernel of the step: every datum a kernel
-    needs counted once (perfect reuse of gathered records in L2), at the sizes of the records it moves."""
-    N, E = int(n_cells), int(n_edges)
-    return {
-        "k_step_control": 0,
-        # EdgeGeom read + EdgeFlux written per edge; every CellRec gathered once
-        "k_edge_flux": 64 * E + 32 * N,
-        # cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
-        "k_theta": (16 + 32 + 8 + 8) * N + 64 * E,
-        # cell_edge, 1/area, g/k^2, theta (own + gathered = once) read, CellRec read + written per cell;
-        # every EdgeGeom and EdgeFlux gathered once
-        "k_cell_update": (16 + 8 + 8 + 8 + 64) * N + 64 * E,
-    }
 
 
 def device_cbrt(x):

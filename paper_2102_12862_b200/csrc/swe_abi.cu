@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <map>
@@ -13,7 +14,9 @@
 
 #include "../../include/swe.h"
 #include "mesh_prep.hpp"
+#include "patch_prep.hpp"
 #include "swe_kernels.cuh"
+#include "swe_patch_kernel.cuh"
 #include "swe_types.h"
 
 using namespace swe;
@@ -27,11 +30,12 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 // Sizes of the O(N) device arrays carved out of the workspace, in carving order.
 struct Layout {
-  size_t rec, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, total;
+  size_t rec, rec_b, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, total;
   Layout(int64_t nc, int64_t ne) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
     rec = take(sizeof(CellRec) * nc);
+    rec_b = take(sizeof(CellRec) * nc);     // second state buffer of the fused patch step
     geom = take(sizeof(EdgeGeom) * ne);
     flux = take(sizeof(EdgeFlux) * ne);
     cell_edge = take(sizeof(int4) * nc);
@@ -54,7 +58,7 @@ struct swe_ctx {
   char *ws = nullptr;
   bool own_ws = false;
   // device arrays (inside ws)
-  CellRec *rec = nullptr; EdgeGeom *geom = nullptr; EdgeFlux *flux = nullptr; int4 *cell_edge = nullptr;
+  CellRec *rec = nullptr, *rec_b = nullptr; EdgeGeom *geom = nullptr; EdgeFlux *flux = nullptr; int4 *cell_edge = nullptr;
   double *area = nullptr, *inv_area = nullptr, *gn2 = nullptr, *kst = nullptr, *theta = nullptr;
   int *cell_perm = nullptr, *edge_perm = nullptr;
   double *stage = nullptr;
@@ -66,6 +70,15 @@ struct swe_ctx {
   double *d_scratch = nullptr;
   std::vector<BoundaryString> strings;
   std::vector<double *> d_params;
+  // fused patch step (variant SWE_VARIANT_PATCH): tables built by patch_prep.hpp, allocated by the library
+  int variant = 0;
+  PatchTables pt;                    // host copy (headers kept for statistics; the big vectors are released)
+  PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
+  PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
+  int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
+  int n_patches = 0; size_t patch_smem = 0;
+  void (*patch_kernel)(Control *, PatchArgs) = nullptr;
+  int64_t alg_bytes[4] = {0, 0, 0, 0};   // algorithmic DRAM bytes per launch of the kernels of one step
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
   int steps_per_graph = 0;
@@ -85,19 +98,43 @@ namespace {
     }                                                                                             \
   } while (0)
 
-// the four kernels of one time step, in stream order; ev (nullable) = kKernelsPerStep + 1 events recorded around them
-constexpr int kKernelsPerStep = 4;
-const char *const kStepKernelNames[kKernelsPerStep] = {"k_step_control", "k_edge_flux", "k_theta", "k_cell_update"};
+// the kernels of one time step, in stream order; ev (nullable) = n_step_kernels + 1 events recorded around them
+constexpr int kMaxStepKernels = 4;
+constexpr int kPatchThreads = 256;
+const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta", "k_cell_update"};
+const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
+
+inline int n_step_kernels(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH ? 2 : 4; }
+
+PatchArgs patch_args(const swe_ctx *c) {
+  PatchArgs a;
+  a.hdr = c->d_hdr; a.halo_ids = c->d_halo_ids; a.halo_area = c->d_halo_area; a.pedge = c->d_pedge; a.pce = c->d_pce;
+  a.rec_a = c->rec; a.rec_b = c->rec_b; a.area = c->area; a.inv_area = c->inv_area; a.gn2 = c->gn2; a.kst = c->kst;
+  a.strings = c->d_strings; a.slot_string = c->d_slot_string; a.string_M = c->d_string_M;
+  a.patch_nbr = c->d_patch_nbr; a.dry_a = c->d_dry; a.dry_b = c->d_dry + c->n_patches;
+  a.max_loc = c->pt.max_loc; a.max_c1 = c->pt.max_c1; a.max_e = c->pt.max_e; a.max_eown = c->pt.max_eown;
+  return a;
+}
+
+void launch_control(swe_ctx *c, cudaStream_t s, int mode) {
+  k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
+                                           c->theta, c->rec, c->rec_b, c->kst,
+                                           c->variant == SWE_VARIANT_PATCH ? c->d_string_M : nullptr, mode);
+}
 
 void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
   if (ev) cudaEventRecord(ev[0], s);
-  k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
-                                           c->theta, c->rec, c->kst, 0);
+  launch_control(c, s, 0);
   if (ev) cudaEventRecord(ev[1], s);
-  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne);
+  if (c->variant == SWE_VARIANT_PATCH) {
+    c->patch_kernel<<<c->n_patches, kPatchThreads, c->patch_smem, s>>>(c->d_ctl, patch_args(c));
+    if (ev) cudaEventRecord(ev[2], s);
+    return;
+  }
+  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0);
   if (ev) cudaEventRecord(ev[2], s);
   k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
-                                             (int)c->nc);
+                                             (int)c->nc, 0);
   if (ev) cudaEventRecord(ev[3], s);
   k_cell_update<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
                                                    c->inv_area, c->gn2, c->rec, (int)c->nc);
@@ -133,6 +170,15 @@ void release(swe_ctx *c) {
   if (c->d_strings) cudaFree(c->d_strings);
   if (c->d_string_edges) cudaFree(c->d_string_edges);
   if (c->d_scratch) cudaFree(c->d_scratch);
+  if (c->d_hdr) cudaFree(c->d_hdr);
+  if (c->d_halo_ids) cudaFree(c->d_halo_ids);
+  if (c->d_halo_area) cudaFree(c->d_halo_area);
+  if (c->d_pedge) cudaFree(c->d_pedge);
+  if (c->d_pce) cudaFree(c->d_pce);
+  if (c->d_slot_string) cudaFree(c->d_slot_string);
+  if (c->d_string_M) cudaFree(c->d_string_M);
+  if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
+  if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
 }
@@ -201,7 +247,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMalloc((void **)&c->ws, lay.total));
     c->own_ws = true;
   }
-  c->rec = (CellRec *)(c->ws + lay.rec); c->geom = (EdgeGeom *)(c->ws + lay.geom); c->flux = (EdgeFlux *)(c->ws + lay.flux);
+  c->rec = (CellRec *)(c->ws + lay.rec); c->rec_b = (CellRec *)(c->ws + lay.rec_b); c->geom = (EdgeGeom *)(c->ws + lay.geom); c->flux = (EdgeFlux *)(c->ws + lay.flux);
   c->cell_edge = (int4 *)(c->ws + lay.cell_edge);
   c->area = (double *)(c->ws + lay.area); c->inv_area = (double *)(c->ws + lay.inv_area);
   c->gn2 = (double *)(c->ws + lay.gn2); c->kst = (double *)(c->ws + lay.kst); c->theta = (double *)(c->ws + lay.theta);
@@ -209,10 +255,12 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   c->stage = (double *)(c->ws + lay.stage);
 
   // ---- arrays in internal numbering
+  std::vector<int4> ce(nc);
+  std::vector<double> area(nc);
+  std::vector<EdgeGeom> geom(ne);
   {
     std::vector<CellRec> rec(nc);
-    std::vector<int4> ce(nc);
-    std::vector<double> area(nc), inv_area(nc), gn2(nc), kst(nc), theta(nc, 1.0);
+    std::vector<double> inv_area(nc), gn2(nc), kst(nc), theta(nc, 1.0);
     for (int64_t i = 0; i < nc; ++i) {
       const int32_t o = hm.cell_perm[i];
       rec[i] = {0.0, 0.0, 0.0, mesh->zb[o]};
@@ -224,7 +272,6 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       gn2[i] = std::isfinite(k) ? p.g / (k * k) : 0.0;    // g / k_str^2 (Eq. 2 P:106-111 with Table 1, R-6)
       kst[i] = k;
     }
-    std::vector<EdgeGeom> geom(ne);
     for (int64_t e = 0; e < ne; ++e) {
       const int32_t o = hm.edge_perm[e];
       const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
@@ -232,6 +279,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     }
     auto up = [&](void *dst, const void *src, size_t bytes) { return cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice); };
     SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
+    SWE_CUDA(c, up(c->rec_b, rec.data(), sizeof(CellRec) * nc));     // z_B must be valid in both state buffers
     SWE_CUDA(c, up(c->cell_edge, ce.data(), sizeof(int4) * nc));
     SWE_CUDA(c, up(c->area, area.data(), 8 * nc));
     SWE_CUDA(c, up(c->inv_area, inv_area.data(), 8 * nc));
@@ -285,11 +333,77 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
   }
 
+  // ---- fused patch step: patch tables (host build, upload), shared-memory size
+  c->variant = (p.variant == SWE_VARIANT_THREE_PASS) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+  if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) {
+    c->err = "unknown variant"; return SWE_EINVAL;
+  }
+  if (c->variant == SWE_VARIANT_PATCH) {
+    const int pc = p.patch_cells > 0 ? p.patch_cells : 384;   // 384 cells, 3 blocks/SM: fastest in the round-1 sweep
+    if (pc < 32 || pc > 8192) { c->err = "patch_cells must be in [32, 8192]"; return SWE_EINVAL; }
+    std::vector<int32_t> string_pos(ne, -1);
+    for (size_t j = 0; j < flat.size(); ++j) string_pos[flat[j]] = (int32_t)j;
+    std::vector<int32_t> ce4((size_t)4 * nc);
+    for (int64_t i = 0; i < nc; ++i) { ce4[4 * i] = ce[i].x; ce4[4 * i + 1] = ce[i].y; ce4[4 * i + 2] = ce[i].z; ce4[4 * i + 3] = 0; }
+    PatchTables &pt = c->pt;
+    if (!build_patches(nc, ne, geom, ce4, area, string_pos, pc, pt, c->err)) return SWE_EINVAL;
+    c->n_patches = (int)pt.hdr.size();
+    c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown).total;
+    // 3 blocks per SM need <= 75 KB each; a numbering that is not spatially compact (renumber = NONE on a
+    // scattered input order) blows the halos up: AUTO then falls back to the three-pass step
+    if (c->patch_smem > 227 * 1024 || (p.variant == SWE_VARIANT_AUTO && c->patch_smem > 75 * 1024)) {
+      if (p.variant == SWE_VARIANT_AUTO) { c->variant = SWE_VARIANT_THREE_PASS; c->pt = PatchTables{}; c->n_patches = 0; c->patch_smem = 0; }
+      else { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
+    }
+  }
+  if (c->variant == SWE_VARIANT_PATCH) {
+    PatchTables &pt = c->pt;
+    std::vector<int32_t> slot_string(std::max<size_t>(1, flat.size()), 0);
+    for (int s = 0; s <= max_id; ++s)
+      for (int32_t j = 0; j < c->strings[s].n_edges; ++j) slot_string[c->strings[s].first + j] = s;
+    int min_blocks = 3;
+    if (const char *e = std::getenv("SWE_PATCH_MINBLOCKS")) min_blocks = std::atoi(e);   // tuning experiments only
+    c->patch_kernel = min_blocks <= 2 ? k_patch_step<kPatchThreads, 2> : min_blocks == 3 ? k_patch_step<kPatchThreads, 3>
+                    : min_blocks == 4 ? k_patch_step<kPatchThreads, 4> : k_patch_step<kPatchThreads, 5>;
+    SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->patch_smem));
+    auto dup = [&](void **dst, const void *src, size_t bytes) {
+      cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+      if (e == cudaSuccess && bytes) e = cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
+      return e;
+    };
+    SWE_CUDA(c, dup((void **)&c->d_hdr, pt.hdr.data(), sizeof(PatchHeader) * pt.hdr.size()));
+    SWE_CUDA(c, dup((void **)&c->d_halo_ids, pt.halo_ids.data(), 4 * pt.halo_ids.size()));
+    SWE_CUDA(c, dup((void **)&c->d_halo_area, pt.halo_area.data(), 8 * pt.halo_area.size()));
+    SWE_CUDA(c, dup((void **)&c->d_pedge, pt.pedge.data(), sizeof(PatchEdge) * pt.pedge.size()));
+    SWE_CUDA(c, dup((void **)&c->d_pce, pt.pce.data(), 4 * pt.pce.size()));
+    SWE_CUDA(c, dup((void **)&c->d_slot_string, slot_string.data(), 4 * slot_string.size()));
+    SWE_CUDA(c, dup((void **)&c->d_patch_nbr, pt.patch_nbr.data(), 4 * pt.patch_nbr.size()));
+    SWE_CUDA(c, cudaMalloc((void **)&c->d_dry, 2 * (size_t)c->n_patches));
+    SWE_CUDA(c, cudaMemset(c->d_dry, 0, 2 * (size_t)c->n_patches));
+    SWE_CUDA(c, cudaMalloc((void **)&c->d_string_M, 8 * std::max<size_t>(1, flat.size())));
+    SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 8 * std::max<size_t>(1, flat.size())));
+    // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
+    // state in 32 + state out 32 + pce 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
+    c->alg_bytes[0] = 0;
+    c->alg_bytes[1] = 104 * nc + 32 * ne;
+    pt.halo_ids = {}; pt.halo_area = {}; pt.pedge = {}; pt.pce = {}; pt.patch_nbr = {};   // host copies no longer needed
+  }
+  if (c->variant != SWE_VARIANT_PATCH) {
+    // EdgeGeom read + EdgeFlux written per edge, every CellRec gathered once
+    c->alg_bytes[0] = 0;
+    c->alg_bytes[1] = 64 * ne + 32 * nc;
+    // cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
+    c->alg_bytes[2] = (16 + 32 + 8 + 8) * nc + 64 * ne;
+    // cell_edge, 1/area, g/k^2, theta read, CellRec read + written per cell; every EdgeGeom and EdgeFlux gathered once
+    c->alg_bytes[3] = (16 + 8 + 8 + 8 + 64) * nc + 64 * ne;
+  }
+
   // ---- control block
   Control h{};
   h.g = p.g; h.h_dry = p.h_dry; h.dt_max = p.dt_max;
   h.t_end = std::numeric_limits<double>::infinity(); h.cfl = 0.9;
   h.n_strings = (int32_t)c->strings.size();
+  h.ping_pong = (c->variant == SWE_VARIANT_PATCH) ? 1 : 0;
   SWE_CUDA(c, cudaMemcpy(c->d_ctl, &h, sizeof(Control), cudaMemcpyHostToDevice));
   *c->h_ctl = h;
   return capture_graph(c);
@@ -309,6 +423,8 @@ void swe_params_default(swe_params *p) {
   p->renumber = SWE_RENUMBER_MORTON;
   p->state_on_device = 0;
   p->steps_per_graph = 32;
+  p->variant = SWE_VARIANT_AUTO;
+  p->patch_cells = 0;
 }
 
 size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges) {
@@ -376,9 +492,14 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     SWE_CUDA(c, cudaMemcpyAsync(c->stage + 2 * nc, hv, 8 * nc, cudaMemcpyHostToDevice, c->stream));
     dh = c->stage; dhu = c->stage + nc; dhv = c->stage + 2 * nc;
   }
-  k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, dh, dhu, dhv, c->rec, (int)nc);
+  k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
+  if (c->variant == SWE_VARIANT_PATCH) {
+    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
+                                                                             c->d_dry + c->n_patches);
+    c->launches += 1;
+  }
   k_reset<<<1, 1, 0, c->stream>>>(c->d_ctl, t0);
-  k_rate<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, (int)nc);
+  k_rate<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, c->rec_b, (int)nc);
   c->launches += 3;
   SWE_CUDA(c, cudaGetLastError());
   c->t_host = t0;
@@ -408,7 +529,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
       for (int64_t j = 0; j < batch_steps; ++j) enqueue_step(c, c->stream);
       SWE_CUDA(c, cudaGetLastError());
     }
-    c->launches += batch_steps * kKernelsPerStep;
+    c->launches += batch_steps * n_step_kernels(c);
     remaining -= batch_steps;
     if (finite_end) {                // the only host synchronisation inside the loop: once per batch
       int rc = read_control(c);
@@ -418,12 +539,11 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     }
   }
   // volume bookkeeping of the last step; then the reductions of swe_step_info
-  k_step_control<<<1, kCtlThreads, 0, c->stream>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom,
-                                                   c->flux, c->theta, c->rec, c->kst, 1);
+  launch_control(c, c->stream, 1);
   c->launches += 1;
   SWE_CUDA(c, cudaGetLastError());
   if (info) {
-    k_info<<<std::min(grid_for(c->nc), 148 * 8), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->area, (int)c->nc);
+    k_info<<<std::min(grid_for(c->nc), 148 * 8), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, c->area, (int)c->nc);
     c->launches += 1;
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
@@ -443,12 +563,13 @@ int swe_get_state(swe_ctx *c, double *h, double *hu, double *hv) {
   if (!h || !hu || !hv) { c->err = "null state pointer"; return SWE_EINVAL; }
   const int64_t nc = c->nc;
   if (c->prm.state_on_device) {
-    k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, c->rec, h, hu, hv, (int)nc);
+    k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, h, hu, hv, (int)nc);
     c->launches += 1;
     SWE_CUDA(c, cudaGetLastError());
     return SWE_OK;
   }
-  k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->cell_perm, c->rec, c->stage, c->stage + nc, c->stage + 2 * nc, (int)nc);
+  k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, c->stage, c->stage + nc,
+                                                         c->stage + 2 * nc, (int)nc);
   c->launches += 1;
   SWE_CUDA(c, cudaMemcpyAsync(h, c->stage, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
   SWE_CUDA(c, cudaMemcpyAsync(hu, c->stage + nc, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
@@ -485,6 +606,16 @@ int swe_get_geometry(swe_ctx *c, double *area, double *nx, double *ny, double *l
 int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR, double *theta) {
   if (!c || !F1 || !F3 || !GL || !GR) return SWE_EINVAL;
   const int64_t ne = c->ne, nc = c->nc;
+  if (c->variant == SWE_VARIANT_PATCH) {
+    // the fused step keeps edge fluxes in shared memory: re-evaluate S1 and S1c of the most recent step with the
+    // stand-alone kernels, from the state that step read (still intact in the other buffer) and its dt
+    int rc = read_control(c);
+    if (rc != SWE_OK) return rc;
+    const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
+    k_edge_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1);
+    k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
+    c->launches += 2;
+  }
   double *d = nullptr;
   SWE_CUDA(c, cudaMalloc((void **)&d, 8 * 4 * ne));
   k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, c->theta, d, d + ne, d + 2 * ne,
@@ -552,28 +683,44 @@ int swe_device_cbrt(const double *x, double *y, int64_t n) {
 
 int64_t swe_kernel_launches(const swe_ctx *c) { return c ? c->launches : 0; }
 
-int swe_step_kernel_count(void) { return kKernelsPerStep; }
+int swe_step_kernel_count(const swe_ctx *c) { return c ? n_step_kernels(c) : 0; }
 
-const char *swe_step_kernel_name(int k) { return (k >= 0 && k < kKernelsPerStep) ? kStepKernelNames[k] : nullptr; }
+const char *swe_step_kernel_name(const swe_ctx *c, int k) {
+  if (!c || k < 0 || k >= n_step_kernels(c)) return nullptr;
+  return c->variant == SWE_VARIANT_PATCH ? kPatchNames[k] : kThreePassNames[k];
+}
+
+int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes[k] : 0; }
+
+int swe_get_patch_stats(swe_ctx *c, int64_t *out, int n_out) {
+  if (!c || !out || n_out < 1) return SWE_EINVAL;
+  int rc = read_control(c);
+  if (rc != SWE_OK) return rc;
+  const int64_t v[9] = {c->variant, c->n_patches, c->pt.patch_cells, (int64_t)c->patch_smem, c->pt.sum_loc, c->pt.sum_e,
+                        c->pt.max_loc, c->pt.max_e, (int64_t)c->h_ctl->patches_skipped};
+  for (int k = 0; k < n_out && k < 9; ++k) out[k] = v[k];
+  return SWE_OK;
+}
 
 int swe_profile_step(swe_ctx *c, int64_t n_steps, double cfl, double *ms, int n_ms) {
   if (!c) return SWE_EINVAL;
   if (n_steps < 1 || !(cfl > 0.0) || !ms || n_ms < 1) { c->err = "swe_profile_step: bad argument"; return SWE_EINVAL; }
   constexpr int kBatch = 32;                       // steps between two synchronisations
-  constexpr int kEv = kKernelsPerStep + 1;
+  constexpr int kEv = kMaxStepKernels + 1;
+  const int nk = n_step_kernels(c);
   std::vector<cudaEvent_t> ev((size_t)kBatch * kEv, nullptr);
   for (auto &e : ev) SWE_CUDA(c, cudaEventCreate(&e));
-  double sum[kKernelsPerStep] = {0.0};
+  double sum[kMaxStepKernels] = {0.0};
   k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, (long long)n_steps, std::numeric_limits<double>::infinity(), cfl);
   c->launches += 1;
   cudaError_t rc = cudaSuccess;
   for (int64_t done = 0; done < n_steps && rc == cudaSuccess; done += kBatch) {
     const int nb = (int)std::min<int64_t>(kBatch, n_steps - done);
     for (int j = 0; j < nb; ++j) enqueue_step(c, c->stream, ev.data() + (size_t)j * kEv);
-    c->launches += (int64_t)nb * kKernelsPerStep;
+    c->launches += (int64_t)nb * nk;
     rc = cudaStreamSynchronize(c->stream);
     for (int j = 0; j < nb && rc == cudaSuccess; ++j)
-      for (int k = 0; k < kKernelsPerStep && rc == cudaSuccess; ++k) {
+      for (int k = 0; k < nk && rc == cudaSuccess; ++k) {
         float t = 0.f;
         rc = cudaEventElapsedTime(&t, ev[(size_t)j * kEv + k], ev[(size_t)j * kEv + k + 1]);
         sum[k] += t;
@@ -581,11 +728,10 @@ int swe_profile_step(swe_ctx *c, int64_t n_steps, double cfl, double *ms, int n_
   }
   for (auto &e : ev) cudaEventDestroy(e);
   SWE_CUDA(c, rc);
-  k_step_control<<<1, kCtlThreads, 0, c->stream>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom,
-                                                   c->flux, c->theta, c->rec, c->kst, 1);
+  launch_control(c, c->stream, 1);
   c->launches += 1;
   SWE_CUDA(c, cudaGetLastError());
-  for (int k = 0; k < n_ms; ++k) ms[k] = k < kKernelsPerStep ? sum[k] / (double)n_steps : 0.0;
+  for (int k = 0; k < n_ms; ++k) ms[k] = k < nk ? sum[k] / (double)n_steps : 0.0;
   c->t_host = -std::numeric_limits<double>::infinity();
   return SWE_OK;
 }

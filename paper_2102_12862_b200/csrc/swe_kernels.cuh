@@ -82,28 +82,23 @@ __device__ __forceinline__ double pow53(double h) {  // h^(5/3), Strickler conve
 __device__ __forceinline__ double k_weight(double k) { return isfinite(k) ? k : 1.0; }
 
 // S1b, boundary edge (only the L side exists).  P:332 wall; P:342 zero-gradient, inflow hydrograph, uniform outflow.
-__device__ __forceinline__ EdgeFlux boundary_flux(const Control &c, const BoundaryString *__restrict__ strings,
-                                                  const double *__restrict__ kst, const EdgeGeom &eg,
-                                                  const CellRec &a, double u, double v) {
+// code: -1 wall, -2 transmissive; s: the boundary string the edge belongs to (nullptr if none); kL = k_str of cell L
+// is read only for string edges.
+__device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const BoundaryString *__restrict__ s,
+                                                  const double *__restrict__ kst, int L, double nx, double ny,
+                                                  double len, double he, double z, double u, double v) {
   EdgeFlux o;
   o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
-  const double he = a.h;
-  const int code = eg.R;
-  int type = 0;
-  const BoundaryString *s = nullptr;
-  if (code <= -3 && (-3 - code) < c.n_strings) {
-    s = strings + (-3 - code);
-    type = s->type;
-  }
+  const int type = s ? s->type : 0;
   if (code == kEdgeTransmissive) {            // R-10: ghost = copy of the interior state
-    const double un = u * eg.nx + v * eg.ny, ut = v * eg.nx - u * eg.ny;
-    o = riemann_nt(c.g, he, un, ut, a.z, he, un, ut, a.z);
+    const double un = u * nx + v * ny, ut = v * nx - u * ny;
+    o = riemann_nt(g, he, un, ut, z, he, un, ut, z);
     o.GR = 0.0;
   } else if (type == kBcInflowQ) {            // R-11: Q(t) distributed by conveyance l k h^(5/3)
     double qe;
     if (s->sumK > 0.0) {
-      const double Ke = (eg.len * k_weight(kst[eg.L])) * pow53(he);
-      qe = ((s->Q * Ke) / s->sumK) / eg.len;
+      const double Ke = (len * k_weight(kst[L])) * pow53(he);
+      qe = ((s->Q * Ke) / s->sumK) / len;
     } else {
       qe = s->Q / s->sumL;
     }
@@ -111,16 +106,16 @@ __device__ __forceinline__ EdgeFlux boundary_flux(const Control &c, const Bounda
     o.GL = (he > 0.0) ? (qe * qe) / he : 0.0;
   } else if (type == kBcOutflowUniform) {     // R-12: normal depth, q_n = k h^(5/3) sqrt(S0)
     if (he > 0.0) {
-      const double qn = (k_weight(kst[eg.L]) * pow53(he)) * sqrt(s->S0);
-      const double ut = v * eg.nx - u * eg.ny;
+      const double qn = (k_weight(kst[L]) * pow53(he)) * sqrt(s->S0);
+      const double ut = v * nx - u * ny;
       o.F1 = qn;
       o.GL = (qn * qn) / he;
       o.F3 = qn * ut;
     }
   } else {                                    // R-9: reflective wall, closed form of the mirror-ghost problem
     if (he > 0.0) {
-      const double un = u * eg.nx + v * eg.ny;
-      const double cel = sqrt(c.g * he);
+      const double un = u * nx + v * ny;
+      const double cel = sqrt(g * he);
       const double S = fmax(cel - un, cel + 0.5 * un);
       o.GL = (he * un) * (un + S);
     }
@@ -135,8 +130,8 @@ __device__ __forceinline__ EdgeFlux boundary_flux(const Control &c, const Bounda
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
-            EdgeFlux *__restrict__ flux, int n_edges) {
-  if (!ctl->active) return;
+            EdgeFlux *__restrict__ flux, int n_edges, int force) {
+  if (!ctl->active && !force) return;
   const int e = blockIdx.x * kBlock + threadIdx.x;
   if (e >= n_edges) return;
   const double g = ctl->g, h_dry = ctl->h_dry;
@@ -153,7 +148,8 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     const double unR = uR * eg.nx + vR * eg.ny, utR = vR * eg.nx - uR * eg.ny;
     o = riemann_nt(g, a.h, unL, utL, a.z, b.h, unR, utR, b.z);
   } else {
-    o = boundary_flux(*ctl, strings, kst, eg, a, uL, vL);
+    const BoundaryString *bs = (eg.R <= -3 && (-3 - eg.R) < ctl->n_strings) ? strings + (-3 - eg.R) : nullptr;
+    o = boundary_flux(g, eg.R, bs, kst, eg.L, eg.nx, eg.ny, eg.len, a.h, a.z, uL, vL);
   }
   flux[e] = o;
 }
@@ -164,8 +160,8 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
 __global__ void __launch_bounds__(kBlock)
 k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
         const EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
-        double *__restrict__ theta, int n_cells) {
-  if (!ctl->active) return;
+        double *__restrict__ theta, int n_cells, int force) {
+  if (!ctl->active && !force) return;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
   const double dt = ctl->dt;
@@ -185,8 +181,9 @@ k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
 }
 
 // block-wide max of non-negative doubles -> one atomicMax on the bit pattern (order-preserving for x >= 0)
+template <int kThreads = kBlock>
 __device__ __forceinline__ void block_max_to_global(double r, unsigned long long *dst) {
-  __shared__ double warp_max[kBlock / 32];
+  __shared__ double warp_max[kThreads / 32];
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
     const double other = __shfl_xor_sync(0xffffffffu, r, off);
@@ -196,9 +193,9 @@ __device__ __forceinline__ void block_max_to_global(double r, unsigned long long
   if (lane == 0) warp_max[wid] = r;
   __syncthreads();
   if (wid == 0) {
-    r = (lane < kBlock / 32) ? warp_max[lane] : 0.0;
+    r = (lane < kThreads / 32) ? warp_max[lane] : 0.0;
 #pragma unroll
-    for (int off = (kBlock / 32) / 2; off > 0; off >>= 1) {
+    for (int off = (kThreads / 32) / 2; off > 0; off >>= 1) {
       const double other = __shfl_xor_sync(0xffffffffu, r, off);
       r = (other > r) ? other : r;
     }
@@ -287,7 +284,8 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
 // Eq. 21 on the current state (after swe_set_state): same arithmetic as the fused part of k_cell_update
 __global__ void __launch_bounds__(kBlock)
 k_rate(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
-       const double *__restrict__ inv_area, const CellRec *__restrict__ rec, int n_cells) {
+       const double *__restrict__ inv_area, const CellRec *rec_a, const CellRec *rec_b, int n_cells) {
+  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   double rate = 0.0;
   if (i < n_cells) {
@@ -336,8 +334,8 @@ __device__ __forceinline__ double hydrograph(const double *p, int n_params, doub
 __global__ void __launch_bounds__(kCtlThreads)
 k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ string_edges, double *scratch,
                const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
-               const double *__restrict__ theta, const CellRec *__restrict__ rec,
-               const double *__restrict__ kst, int mode) {
+               const double *__restrict__ theta, const CellRec *rec_a, const CellRec *rec_b,
+               const double *__restrict__ kst, const double *__restrict__ string_M, int mode) {
   const int ns = ctl->n_strings;
   // ---- volume bookkeeping of the previous step, from the (limited) fluxes actually applied
   if (ctl->pending) {
@@ -351,14 +349,18 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
         for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
           double a = 0.0;
           if (j < bs.n_edges) {
-            const int e = string_edges[bs.first + j];
-            const EdgeGeom eg = geom[e];
-            double F1 = flux[e].F1;
-            if (F1 > 0.0) {
-              const double th = theta[eg.L];
-              if (th < 1.0) F1 = th * F1;
+            if (string_M) {                      // fused patch step: l * (limited F1), written by the owning patch
+              a = string_M[bs.first + j];
+            } else {
+              const int e = string_edges[bs.first + j];
+              const EdgeGeom eg = geom[e];
+              double F1 = flux[e].F1;
+              if (F1 > 0.0) {
+                const double th = theta[eg.L];
+                if (th < 1.0) F1 = th * F1;
+              }
+              a = eg.len * F1;
             }
-            a = eg.len * F1;
           }
           v[j] = a;
         }
@@ -392,6 +394,8 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
         active = 1;
         ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
         ctl->rate_bits = 0ull;
+        ctl->src = ctl->cur;                 // the step reads the newest state ...
+        ctl->cur ^= ctl->ping_pong;          // ... and, when it ping-pongs, writes the other buffer
         ctl->steps_done += 1;
         if (ctl->steps_left > 0) ctl->steps_left -= 1;
         ctl->pending = 1;
@@ -404,6 +408,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   __syncthreads();
   if (!s_active) return;
   // ---- boundary strings at t^n (R-11): Q(t^n) and the conveyance sum over the string
+  const CellRec *__restrict__ rec = ctl->src ? rec_b : rec_a;
   for (int s = 0; s < ns; ++s) {
     BoundaryString &bs = strings[s];
     if (bs.type != kBcInflowQ) continue;
@@ -438,11 +443,14 @@ __global__ void k_reset(Control *ctl, double t0) {
   ctl->vol_in = 0.0; ctl->vol_out = 0.0; ctl->vol_clipped = 0.0;
   ctl->rate_bits = 0ull; ctl->steps_left = 0; ctl->steps_done = 0;
   ctl->active = 0; ctl->pending = 0; ctl->flags = 0;
+  ctl->src = ctl->cur;
 }
 
 // swe_step_info reductions: volume, wet count, non-finite check
 __global__ void __launch_bounds__(kBlock)
-k_info(Control *__restrict__ ctl, const CellRec *__restrict__ rec, const double *__restrict__ area, int n_cells) {
+k_info(Control *__restrict__ ctl, const CellRec *rec_a, const CellRec *rec_b, const double *__restrict__ area,
+       int n_cells) {
+  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   double vol = 0.0;
   long long wet = 0;
   int bad = 0;
@@ -468,8 +476,9 @@ k_info(Control *__restrict__ ctl, const CellRec *__restrict__ rec, const double 
 
 // caller numbering <-> internal numbering (cell_perm[new] = caller id)
 __global__ void __launch_bounds__(kBlock)
-k_pack_state(const int *__restrict__ cell_perm, const double *__restrict__ h, const double *__restrict__ hu,
-             const double *__restrict__ hv, CellRec *__restrict__ rec, int n_cells) {
+k_pack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *__restrict__ h,
+             const double *__restrict__ hu, const double *__restrict__ hv, CellRec *rec_a, CellRec *rec_b, int n_cells) {
+  CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
   const int o = cell_perm[i];
@@ -479,8 +488,10 @@ k_pack_state(const int *__restrict__ cell_perm, const double *__restrict__ h, co
 }
 
 __global__ void __launch_bounds__(kBlock)
-k_unpack_state(const int *__restrict__ cell_perm, const CellRec *__restrict__ rec, double *__restrict__ h,
-               double *__restrict__ hu, double *__restrict__ hv, int n_cells) {
+k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const CellRec *rec_a,
+               const CellRec *rec_b, double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv,
+               int n_cells) {
+  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
   const int o = cell_perm[i];

@@ -21,6 +21,31 @@ struct __align__(32) EdgeFlux {  // S1 outputs: F1 mass, F3 tangential momentum,
   double F1, F3, GL, GR;
 };
 
+// ---- fused patch step: the mesh is cut into patches of consecutive (Morton-ordered) cells;
+// one thread block advances one patch by a whole time step out of shared memory.
+//   local cells : [0, n_own) the patch's own cells, then ring 1 (cells sharing an edge with an own cell), then
+//                 ring 2 (cells sharing an edge with a ring-1 cell; needed because the limiter factor theta of a
+//                 ring-1 cell depends on all three of its edges)
+//   local edges : [0, n_eown) every edge of an own cell, then [n_eown, n_eown + n_er1) the other edges of ring 1
+struct __align__(16) PatchHeader {
+  int32_t cell0, n_own, n_r1, n_r2;
+  int32_t n_eown, n_er1;
+  int32_t halo_off;              // first entry of this patch in halo_ids[] / halo_area[]  (n_r1 + n_r2 entries)
+  int32_t edge_off;              // first record of this patch in pedge[]
+  int32_t pce_off;               // first record of this patch in pce[]  (n_own + n_r1 records)
+  int32_t n_string_edges;        // boundary-string edges among the local edges (such a patch is never skipped)
+  int32_t nbr_off, n_nbr;        // the patches that own this patch's ring-1 / ring-2 cells: entries of patch_nbr[]
+};
+
+struct __align__(32) PatchEdge { // geometry of section 4.1 + the two cells in patch-local numbering
+  double nx, ny, len;
+  uint16_t L, R;                 // R == 0xFFFF: boundary edge
+  int32_t aux;                   // boundary: -1 wall, -2 transmissive, <= -3: -3 - (position in string_edges[])
+};
+
+// pce[] record = uint4 {slot0, slot1, slot2, unused}; slot = edge (bits 0-14) | isL (bit 15) | neighbour cell (bits 16-31)
+constexpr uint32_t kPceNoNeighbour = 0xFFFFu;
+
 struct BoundaryString {          // one boundary string (R-11, R-12); lives in device memory
   int32_t type;                  // SWE_BC_*
   int32_t n_edges;               // members
@@ -44,6 +69,12 @@ struct Control {                 // device-side step-loop state: nothing of it i
   int32_t pending;               // 1: volume bookkeeping of the previous step not yet done
   int32_t flags;                 // SWE_FLAG_*
   int32_t n_strings;
+  int32_t cur;                   // index of the state buffer that holds (or will hold, once the enqueued steps have
+                                 // run) the newest state; the fused patch step ping-pongs, the three-pass step stays 0
+  int32_t src;                   // state buffer the step in flight reads (it writes src ^ ping_pong)
+  int32_t ping_pong;             // 1: fused patch step (two state buffers); 0: in-place three-pass step
+  int32_t pad2_;
+  unsigned long long patches_skipped;   // fused patch step: blocks that found their whole patch dry, since swe_create
   // swe_step_info reductions (k_info)
   double vol;
   long long n_wet;

@@ -11,6 +11,10 @@ from workloads import configs as C
 
 from test_gpu_parity import assert_state_close, check_info, DT_RTOL
 
+
+def make(gpu, w, **kw):
+    return gpu.from_workload(w, **kw)     # defaults = the launch configuration bench.py times
+
 pytestmark = pytest.mark.gpu
 
 
@@ -40,7 +44,7 @@ def window(s, o, w, n, what):
 def test_config4_full_size_windows(gpu, ref):
     w = C.config4()
     assert 3.8e6 < w.n_cells < 4.2e6
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     o = ref.RefSolver(w)
     area = s.geometry()[0]
     vol0 = float(np.sum(w.h * area))
@@ -65,7 +69,7 @@ def test_config4_full_size_windows(gpu, ref):
 def test_config3_full_size_window(gpu, ref):
     w = C.config3()
     assert 0.95e6 < w.n_cells < 1.05e6
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     o = ref.RefSolver(w)
     ig, io, _ = window(s, o, w, 40, "config3 full size, steps 0-40")
     check_info(ig, io)

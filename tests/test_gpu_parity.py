@@ -25,6 +25,29 @@ def gpu():
     return P
 
 
+_VARIANT = {"v": 0}
+
+
+@pytest.fixture(autouse=True, params=[1, 2], ids=["three-pass", "patch"])
+def variant(request):
+    """Every test of this module runs with both step variants (include/swe.h SWE_VARIANT_*): the edge-flux ->
+    theta -> gather/update three-pass step and the fused shared-memory patch step."""
+    _VARIANT["v"] = request.param
+    yield request.param
+
+
+def make(gpu, w, **kw):
+    kw.setdefault("variant", _VARIANT["v"])
+    if kw["variant"] == 2:
+        kw.setdefault("patch_cells", 192)      # small patches: the small test meshes still span many patches
+    return gpu.from_workload(w, **kw)
+
+
+def mk(gpu, *a, **kw):
+    kw.setdefault("variant", _VARIANT["v"])
+    return gpu.Solver(*a, **kw)
+
+
 def assert_state_close(got, want, what=""):
     """abs(d) <= 1e-10 abs(ref) + 1e-14 max abs(ref) per field (R-14), and report the strict relative error
     on cells that are not pure round-off."""
@@ -43,7 +66,7 @@ def assert_state_close(got, want, what=""):
 def run_both(gpu, ref, w, n_steps, t_end=float("inf"), chunks=(None,), **kw):
     """Steps oracle and GPU side by side in the given chunks; returns the two solvers and info dicts."""
     o = ref.RefSolver(w)
-    s = gpu.from_workload(w, **kw)
+    s = make(gpu, w, **kw)
     io = o.step(n_steps, t_end, w.cfl)
     ig = s.step(n_steps, t_end, w.cfl)
     return o, s, io, ig
@@ -78,7 +101,7 @@ def test_geometry_bit_identical(gpu, ref, name):
     """Section 4.1 geometry: areas, lengths, normals as the kernels use them == the oracle's."""
     w = CASES[name]()
     o = ref.RefSolver(w)
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     for a, b in zip(s.geometry(), o.geometry()):
         assert np.array_equal(a, b)
     s.close()
@@ -89,7 +112,7 @@ def test_first_step_edge_by_edge(gpu, ref, name):
     """S0 + S1 + S1c of the first step, per edge: fluxes after the limiter, theta, dt."""
     w = CASES[name]()
     o = ref.RefSolver(w)
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     assert s.peek_dt(w.cfl) == o.peek_dt(w.cfl)                      # Eq. 21: exact max, one division
     io = o.step(1, float("inf"), w.cfl)
     ig = s.step(1, float("inf"), w.cfl)
@@ -118,7 +141,7 @@ def test_parity_100_steps(gpu, ref, name):
     Stepped in chunks of 1, 9 and 90 so that graph launches, tails and repeated calls are all exercised."""
     w = CASES[name]()
     o = ref.RefSolver(w)
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     for n in (1, 9, 90):
         io = o.step(n, float("inf"), w.cfl)
         ig = s.step(n, float("inf"), w.cfl)
@@ -147,7 +170,7 @@ def test_config1_to_t_end(gpu, ref):
 def test_config2_lake_at_rest_1000_steps(gpu, ref):
     """BASELINE.json configs[1] in full (80k cells, 1000 steps): |u|,|v| <= 1e-12, mass to round-off, and parity."""
     w = C.config2()
-    s = gpu.from_workload(w)
+    s = make(gpu, w)
     ig = s.step(1000, float("inf"), w.cfl)
     h, hu, hv = s.get_state()
     wet = h > w.h_dry
@@ -167,10 +190,11 @@ def test_config2_lake_at_rest_1000_steps(gpu, ref):
 def test_renumbering_does_not_change_results(gpu, name):
     """R-15: Morton numbering vs caller numbering vs a randomly permuted input: bit-identical states."""
     w = CASES[name]()
-    a = gpu.from_workload(w, renumber=gpu.RENUMBER_NONE)
-    b = gpu.from_workload(w, renumber=gpu.RENUMBER_MORTON)
+    # caller numbering is Qhull's (not spatially compact): AUTO must fall back to the three-pass step for it
+    a = make(gpu, w, renumber=gpu.RENUMBER_NONE, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    b = make(gpu, w, renumber=gpu.RENUMBER_MORTON)
     wp, cp = w.permuted(7)
-    c = gpu.from_workload(wp, renumber=gpu.RENUMBER_MORTON)
+    c = make(gpu, wp, renumber=gpu.RENUMBER_MORTON)
     for s in (a, b, c):
         s.step(60, float("inf"), w.cfl)
     sa, sb, sc = a.get_state(), b.get_state(), c.get_state()
@@ -186,15 +210,15 @@ def test_renumbering_does_not_change_results(gpu, name):
 def test_graph_and_plain_launches_agree(gpu):
     """The CUDA-graph step loop and plain kernel launches give bit-identical states; launch counts add up."""
     w = CASES["config4-small"]()
-    a = gpu.from_workload(w, steps_per_graph=0)
-    b = gpu.from_workload(w, steps_per_graph=8)
-    c = gpu.from_workload(w, steps_per_graph=32)
+    a = make(gpu, w, steps_per_graph=0)
+    b = make(gpu, w, steps_per_graph=8)
+    c = make(gpu, w, steps_per_graph=32)
     infos = [s.step(75, float("inf"), w.cfl) for s in (a, b, c)]
     for s in (b, c):
         for x, y in zip(a.get_state(), s.get_state()):
             assert np.array_equal(x, y)
     assert infos[0] == infos[1] == infos[2]
-    assert a.kernel_launches >= 75 * 4
+    assert a.kernel_launches >= 75 * len(a.step_kernels())
     for s in (a, b, c):
         s.close()
 
@@ -202,12 +226,12 @@ def test_graph_and_plain_launches_agree(gpu):
 def test_restart_round_trip(gpu):
     """S9 / O-10: get_state at step 50 -> new context -> set_state -> 50 more == 100 straight steps, bitwise."""
     w = CASES["config3-small"]()
-    a = gpu.from_workload(w)
+    a = make(gpu, w)
     a.step(100, float("inf"), w.cfl)
-    b = gpu.from_workload(w)
+    b = make(gpu, w)
     i50 = b.step(50, float("inf"), w.cfl)
     st = b.get_state()
-    c = gpu.from_workload(w)
+    c = make(gpu, w)
     c.set_state(*st, t0=i50["t"])
     ic = c.step(50, float("inf"), w.cfl)
     for x, y in zip(a.get_state(), c.get_state()):
@@ -221,9 +245,9 @@ def test_state_on_device_and_own_workspace(gpu):
     """Device-pointer state (torch tensors) and a library-owned workspace give the same results as host pointers."""
     import torch
     w = CASES["config3-small"]()
-    a = gpu.from_workload(w)
-    b = gpu.from_workload(w, state_on_device=True)
-    c = gpu.from_workload(w, own_workspace=True)
+    a = make(gpu, w)
+    b = make(gpu, w, state_on_device=True)
+    c = make(gpu, w, own_workspace=True)
     for s in (a, b, c):
         s.step(40, float("inf"), w.cfl, info=False)
     ref_state = a.get_state()
@@ -240,8 +264,8 @@ def test_tables_built_by_the_library(gpu):
     """edge_cell / cell_edge = NULL: the library builds both; all boundary edges are walls; same result as the
     harness tables up to the edge numbering."""
     w = CASES["config2-lake-small"]()
-    a = gpu.from_workload(w)
-    b = gpu.Solver(w.node_xy, w.tri, None, None, w.zb, w.kst, h_dry=w.h_dry)
+    a = make(gpu, w)
+    b = mk(gpu, w.node_xy, w.tri, None, None, w.zb, w.kst, h_dry=w.h_dry)
     b.set_state(w.h, w.hu, w.hv)
     ec, ce = b.tables()
     assert b.n_edges == w.n_edges
@@ -260,12 +284,12 @@ def test_tables_built_by_the_library(gpu):
 def test_degenerate_and_error_cases(gpu):
     w = C.tiny_mesh("two-cells")
     # all dry, dt_max = inf: dt unbounded -> flag, no step, no hang
-    s = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s = mk(gpu, w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
     s.set_state(np.zeros(2), np.zeros(2), np.zeros(2))
     info = s.step(5, float("inf"), 0.9)
     assert info["steps_done"] == 0 and info["flags"] & gpu.FLAG_DT_UNBOUNDED
     # all dry with a finite dt_max: steps of dt_max that change nothing
-    s2 = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst, dt_max=2.0)
+    s2 = mk(gpu, w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst, dt_max=2.0)
     s2.set_state(np.zeros(2), np.zeros(2), np.zeros(2))
     info = s2.step(3, float("inf"), 0.9)
     assert info["steps_done"] == 3 and info["t"] == 6.0 and info["vol"] == 0.0
@@ -278,16 +302,16 @@ def test_degenerate_and_error_cases(gpu):
     bad = w.tri.copy()
     bad[0] = bad[0][::-1]
     with pytest.raises(gpu.SweError) as ei:
-        gpu.Solver(w.node_xy, bad, None, None, w.zb, w.kst)
+        mk(gpu, w.node_xy, bad, None, None, w.zb, w.kst)
     assert ei.value.code == gpu.EMESH
     # inconsistent tables -> SWE_EMESH
     ec = w.edge_cell.copy()
     ec[:, 0] = ec[::-1, 0]
     with pytest.raises(gpu.SweError) as ei:
-        gpu.Solver(w.node_xy, w.tri, ec, w.cell_edge, w.zb, w.kst)
+        mk(gpu, w.node_xy, w.tri, ec, w.cell_edge, w.zb, w.kst)
     assert ei.value.code == gpu.EMESH
     # non-finite state is reported
-    s3 = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s3 = mk(gpu, w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
     s3.set_state(np.array([1.0, np.nan]), np.zeros(2), np.zeros(2))
     with pytest.raises(gpu.SweError) as ei:
         s3.step(1, float("inf"), 0.9)
@@ -311,7 +335,7 @@ def test_hand_values_through_the_abi(gpu):
                 gold[(case, q)] = float(v)
     w = C.tiny_mesh("two-cells-x")
     w.zb = np.array([0.0, 0.5])
-    s = gpu.Solver(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    s = mk(gpu, w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
     s.set_state(np.array([2.0, 1.0]), np.array([2.0, 0.0]), np.array([1.0, 0.0]))
     s.step(1, float("inf"), 1e-6)          # tiny CFL: theta = 1
     F1, F3, GL, GR, theta = s.edge_fluxes()
@@ -343,3 +367,48 @@ def test_device_cbrt_matches(gpu, ref):
     want = np.array([ref.cbrt(float(v)) for v in x])
     assert np.array_equal(got, want)
     assert np.array_equal(gpu.device_cbrt(-x[:1000]), -want[:1000])
+
+
+@pytest.mark.parametrize("name", ["config3-small", "config4-small", "uniform-flow", "config1-ritter"])
+def test_variants_and_patch_sizes_bit_identical(gpu, name):
+    """The fused patch step (any patch size, ragged last patch, patches larger than the mesh) and the three-pass
+    step evaluate the same arithmetic: bit-identical states, dt and volume counters."""
+    w = CASES[name]()
+    ref_s = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    i0 = ref_s.step(70, float("inf"), w.cfl)
+    s0 = ref_s.get_state()
+    for pc in (32, 100, 512, 1024):                  # 512 / 1024 exceed the cell count of the smallest case
+        s = gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=pc)
+        st = s.patch_stats()
+        assert st["variant"] == gpu.VARIANT_PATCH and st["patches"] == -(-w.n_cells // pc)
+        i1 = s.step(70, float("inf"), w.cfl)
+        for x, y in zip(s0, s.get_state()):
+            assert np.array_equal(x, y), (name, pc)
+        assert i1 == i0, (name, pc)
+        s.close()
+    ref_s.close()
+
+
+def test_dry_patches_are_skipped_and_rewetted(gpu, ref):
+    """Fused patch step: blocks whose whole patch (own cells + both halo rings) is dry skip the flux work; the
+    Ritter front then runs into such patches.  States stay equal to the oracle's; all-wet meshes skip nothing."""
+    w = C.config1()
+    s = gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=64)
+    o = ref.RefSolver(w)
+    skipped = []
+    for n in (5, 60, 200):
+        ig, io = s.step(n, float("inf"), w.cfl), o.step(n, float("inf"), w.cfl)
+        assert_state_close(s.get_state(), o.get_state(), f"ritter after {io['steps_done']} steps")
+        check_info(ig, io)
+        skipped.append(s.patch_stats()["patch_steps_skipped"])
+    st = s.patch_stats()
+    assert skipped[0] > 0                                           # the dry half of the channel is skipped at first
+    per_step = np.diff([0] + skipped) / np.array([5, 60, 200])
+    assert per_step[2] < per_step[0]                                # ... and less and less as the front wets it
+    assert ig["n_wet"] > int(np.sum(w.h > w.h_dry))
+    s.close()
+    w3 = CASES["config3-small"]()
+    s3 = gpu.from_workload(w3, variant=gpu.VARIANT_PATCH, patch_cells=128)
+    s3.step(20, float("inf"), w3.cfl)
+    assert s3.patch_stats()["patch_steps_skipped"] == 0
+    s3.close()
