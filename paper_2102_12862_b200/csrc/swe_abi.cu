@@ -75,6 +75,7 @@ struct swe_ctx {
   PatchTables pt;                    // host copy (headers kept for statistics; the big vectors are released)
   PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
   PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
+  InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
   int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
   int n_patches = 0; size_t patch_smem = 0;
   void (*patch_kernel)(Control *, PatchArgs) = nullptr;
@@ -177,6 +178,8 @@ void release(swe_ctx *c) {
   if (c->d_pce) cudaFree(c->d_pce);
   if (c->d_slot_string) cudaFree(c->d_slot_string);
   if (c->d_string_M) cudaFree(c->d_string_M);
+  if (c->d_info_part) cudaFree(c->d_info_part);
+  if (c->d_info_ticket) cudaFree(c->d_info_ticket);
   if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
   if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -320,6 +323,9 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     flat.insert(flat.end(), members[s].begin(), members[s].end());
   }
   SWE_CUDA(c, cudaMalloc((void **)&c->d_ctl, sizeof(Control)));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_info_part, sizeof(InfoPartial) * kInfoMaxBlocks));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_info_ticket, sizeof(unsigned int)));
+  SWE_CUDA(c, cudaMemset(c->d_info_ticket, 0, sizeof(unsigned int)));
   SWE_CUDA(c, cudaMallocHost((void **)&c->h_ctl, sizeof(Control)));
   SWE_CUDA(c, cudaMalloc((void **)&c->d_strings, sizeof(BoundaryString) * std::max<size_t>(1, c->strings.size())));
   SWE_CUDA(c, cudaMalloc((void **)&c->d_string_edges, 4 * std::max<size_t>(1, flat.size())));
@@ -543,7 +549,8 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
   c->launches += 1;
   SWE_CUDA(c, cudaGetLastError());
   if (info) {
-    k_info<<<std::min(grid_for(c->nc), 148 * 8), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, c->area, (int)c->nc);
+    k_info<<<std::min(grid_for(c->nc), kInfoMaxBlocks), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, c->area, (int)c->nc,
+                                                                               c->d_info_part, c->d_info_ticket);
     c->launches += 1;
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;

@@ -446,10 +446,15 @@ __global__ void k_reset(Control *ctl, double t0) {
   ctl->src = ctl->cur;
 }
 
-// swe_step_info reductions: volume, wet count, non-finite check
+// swe_step_info reductions: volume, wet count, non-finite check.  Deterministic (the same sum order every call):
+// fixed cell -> thread assignment, xor-shuffle tree per warp, warps in order per block, one partial per block, and the
+// block that finishes last adds the partials in block order.
+constexpr int kInfoMaxBlocks = 148 * 8;
+struct InfoPartial { double vol; long long wet; int bad; int pad_; };
+
 __global__ void __launch_bounds__(kBlock)
 k_info(Control *__restrict__ ctl, const CellRec *rec_a, const CellRec *rec_b, const double *__restrict__ area,
-       int n_cells) {
+       int n_cells, InfoPartial *__restrict__ part, unsigned int *__restrict__ ticket) {
   const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   double vol = 0.0;
   long long wet = 0;
@@ -467,10 +472,27 @@ k_info(Control *__restrict__ ctl, const CellRec *rec_a, const CellRec *rec_b, co
     wet += __shfl_xor_sync(0xffffffffu, wet, off);
     bad |= __shfl_xor_sync(0xffffffffu, bad, off);
   }
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&ctl->vol, vol);
-    atomicAdd((unsigned long long *)&ctl->n_wet, (unsigned long long)wet);
-    if (bad) atomicOr(&ctl->nonfinite, 1);
+  __shared__ double s_vol[kBlock / 32];
+  __shared__ long long s_wet[kBlock / 32];
+  __shared__ int s_bad[kBlock / 32];
+  __shared__ bool s_last;
+  if ((threadIdx.x & 31) == 0) { s_vol[threadIdx.x >> 5] = vol; s_wet[threadIdx.x >> 5] = wet; s_bad[threadIdx.x >> 5] = bad; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    InfoPartial p; p.vol = 0.0; p.wet = 0; p.bad = 0; p.pad_ = 0;
+    for (int k = 0; k < kBlock / 32; ++k) { p.vol += s_vol[k]; p.wet += s_wet[k]; p.bad |= s_bad[k]; }
+    part[blockIdx.x] = p;
+    __threadfence();
+    s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x == 0) {
+    double v = 0.0; long long w = 0; int b = 0;
+    for (unsigned k = 0; k < gridDim.x; ++k) { const InfoPartial p = part[k]; v += p.vol; w += p.wet; b |= p.bad; }
+    ctl->vol = v; ctl->n_wet = w; ctl->nonfinite = b;
+    *ticket = 0u;
   }
 }
 
