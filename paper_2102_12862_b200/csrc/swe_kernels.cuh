@@ -30,12 +30,18 @@ constexpr int kFlagUnbounded = 2;
 // momentum; P:254 bed slope by the modified-state approach of ref [69] (R-1): face bed z* = max(zL, zR), face
 // depths hs_K = max(0, h_K + z_K - z*), per-side pressure correction G_K = F2 - 1/2 g hs_K^2.
 // ---------------------------------------------------------------------------------------------------------
+// min / max of finite doubles as one compare + select (fmin / fmax also order NaNs and signed zeros, which costs
+// several more instructions; here a zero of either sign leads to the same branch and the same values)
+__device__ __forceinline__ double dmax0(double x) { return x > 0.0 ? x : 0.0; }
+__device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
+
 __device__ __forceinline__ EdgeFlux riemann_nt(double g, double hL, double unL, double utL, double zL,
                                                double hR, double unR, double utR, double zR) {
   EdgeFlux o;
   const double dz = zR - zL;
-  const double hsL = fmax(0.0, hL - fmax(0.0, dz));
-  const double hsR = fmax(0.0, hR - fmax(0.0, -dz));
+  const double hsL = dmax0(hL - dmax0(dz));
+  const double hsR = dmax0(hR - dmax0(-dz));
   if (hsL == 0.0 && hsR == 0.0) {
     o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
     return o;
@@ -45,8 +51,8 @@ __device__ __forceinline__ EdgeFlux riemann_nt(double g, double hL, double unL, 
   if (hsL > 0.0 && hsR > 0.0) {
     const double us = 0.5 * (unL + unR) + (cL - cR);
     const double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
-    SL = fmin(unL - cL, us - cs);
-    SR = fmax(unR + cR, us + cs);
+    SL = dmin2(unL - cL, us - cs);
+    SR = dmax2(unR + cR, us + cs);
   } else if (hsR == 0.0) {
     SL = unL - cL;
     SR = unL + 2.0 * cL;
@@ -116,7 +122,7 @@ __device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const Boun
     if (he > 0.0) {
       const double un = u * nx + v * ny;
       const double cel = sqrt(g * he);
-      const double S = fmax(cel - un, cel + 0.5 * un);
+      const double S = dmax2(cel - un, cel + 0.5 * un);
       o.GL = (he * un) * (un + S);
     }
   }
@@ -173,7 +179,7 @@ k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
     const EdgeGeom eg = geom[es[k]];
     const double F1 = flux[es[k]].F1;
     const double sM = (eg.L == i ? 1.0 : -1.0) * (eg.len * F1);
-    o[k] = fmax(0.0, sM);
+    o[k] = dmax0(sM);
   }
   const double out = ((o[0] + o[1]) + o[2]);
   const double avail = rec[i].h * area[i];

@@ -170,7 +170,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     for (int k = 0; k < 3; ++k) {
       const int e = w[k] & 0x7FFFu;
       const double sM = ((w[k] & 0x8000u) ? 1.0 : -1.0) * (sh_len[e] * sh_F1[e]);
-      o[k] = fmax(0.0, sM);
+      o[k] = dmax0(sM);
     }
     const double outflow = ((o[0] + o[1]) + o[2]);
     const double avail = sh_h[l] * Ai;
