@@ -32,7 +32,9 @@ if ROOT not in sys.path:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures under
 # profiles/ (kernel name, n_cells) -> bytes; absent -> "traffic": null
 NCU_TRAFFIC_BYTES = {("k_cell_update", 3964806): 737.0e6, ("k_theta", 3964806): 633.2e6,
-                     ("k_edge_flux", 3964806): 476.5e6}   # profiles/r1a_ncu_full_three_pass.md
+                     ("k_edge_flux", 3964806): 476.5e6,   # profiles/r1a_ncu_full_three_pass.md
+                     ("k_patch_step", 3964806): 407.8e6,  # profiles/r1c_ncu_full_patch_river.md (52 % of patches dry)
+                     ("k_patch_step", 3964136): 678.6e6}  # profiles/r1c_ncu_full_patch_allwet.md
 
 METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
