@@ -367,10 +367,19 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     std::vector<int32_t> slot_string(std::max<size_t>(1, flat.size()), 0);
     for (int s = 0; s <= max_id; ++s)
       for (int32_t j = 0; j < c->strings[s].n_edges; ++j) slot_string[c->strings[s].first + j] = s;
-    int min_blocks = 3;
-    if (const char *e = std::getenv("SWE_PATCH_MINBLOCKS")) min_blocks = std::atoi(e);   // tuning experiments only
-    c->patch_kernel = min_blocks <= 2 ? k_patch_step<kPatchThreads, 2> : min_blocks == 3 ? k_patch_step<kPatchThreads, 3>
-                    : min_blocks == 4 ? k_patch_step<kPatchThreads, 4> : k_patch_step<kPatchThreads, 5>;
+    // default patch size on a compact numbering: shared-memory arrays with compile-time capacities; anything else
+    // (other patch sizes, fatter halos) runs the same kernel with run-time capacities
+    constexpr int kCapLoc = 640, kCapC1 = 544, kCapE = 864, kCapEown = 704;
+    if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown &&
+        !std::getenv("SWE_PATCH_DYNAMIC")) {
+      c->patch_kernel = k_patch_step<kPatchThreads, 3, kCapLoc, kCapC1, kCapE, kCapEown>;
+      c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown).total;
+    } else {
+      int min_blocks = 3;
+      if (const char *e = std::getenv("SWE_PATCH_MINBLOCKS")) min_blocks = std::atoi(e);   // tuning experiments only
+      c->patch_kernel = min_blocks <= 2 ? k_patch_step<kPatchThreads, 2, 0, 0, 0, 0> : min_blocks == 3 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0>
+                      : k_patch_step<kPatchThreads, 4, 0, 0, 0, 0>;
+    }
     SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->patch_smem));
     auto dup = [&](void **dst, const void *src, size_t bytes) {
       cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));

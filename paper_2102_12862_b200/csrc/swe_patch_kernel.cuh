@@ -48,12 +48,15 @@ struct PatchArgs {
 
 // Loads are software-pipelined: the record an iteration needs is loaded one iteration (or one phase) ahead, so that
 // the global-memory latency overlaps the arithmetic of the current item instead of stalling its first use.
-template <int kThreads, int kMinBlocks>
+// kCap* != 0: the shared-memory arrays have these compile-time capacities (every offset becomes an immediate of the
+// LDS / STS instructions); kCap* == 0: capacities come from PatchArgs at run time (any patch size).
+template <int kThreads, int kMinBlocks, int kCapLoc, int kCapC1, int kCapE, int kCapEown>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
   if (!ctl->active) return;
   extern __shared__ double sm[];
-  const PatchSmem S = patch_smem_layout(A.max_loc, A.max_c1, A.max_e, A.max_eown);
+  const PatchSmem S = kCapLoc ? patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown)
+                              : patch_smem_layout(A.max_loc, A.max_c1, A.max_e, A.max_eown);
   double *sh_h = sm + S.h, *sh_u = sm + S.u, *sh_v = sm + S.v, *sh_z = sm + S.z, *sh_th = sm + S.theta;
   double *sh_F1 = sm + S.F1, *sh_len = sm + S.len, *sh_F3 = sm + S.F3, *sh_GL = sm + S.GL, *sh_GR = sm + S.GR;
   double *sh_nx = sm + S.nx, *sh_ny = sm + S.ny;
@@ -96,22 +99,49 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     }
   }
 
-  // ---- phase 1: local cell states; velocities once per cell (R-8: thin films carry no momentum)
+  // ---- the patch's streamed tables are contiguous: pull them into L2 now (no registers held), so that the loads of
+  // phases 2-4 pay L2 latency instead of DRAM latency
+  {
+    auto prefetch_range = [&](const void *base, int bytes) {
+      const char *p = (const char *)base;
+      for (int off = tid * 128; off < bytes; off += kThreads * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(p + off));
+    };
+    prefetch_range(pedge, n_e * (int)sizeof(PatchEdge));
+    prefetch_range(pce, n_c1 * (int)sizeof(uint4));
+    prefetch_range(A.area + H.cell0, H.n_own * 8);
+    prefetch_range(A.inv_area + H.cell0, H.n_own * 8);
+    prefetch_range(A.gn2 + H.cell0, H.n_own * 8);
+    prefetch_range(halo_area + H.n_own, H.n_r1 * 8);
+  }
+
+  // ---- phase 1: local cell states; velocities once per cell (R-8: thin films carry no momentum).  Three records per
+  // thread are in flight at a time (the halo part is a dependent id -> record gather).
   PatchEdge pe_next;
   if (tid < n_e) pe_next = pedge[tid];                 // first record of phase 2, in flight during phase 1
   {
-    int l = tid;
     int water = 0;
-    CellRec c_next;
-    if (l < n_loc) c_next = in[l < H.n_own ? H.cell0 + l : halo_ids[l]];
-    for (; l < n_loc; l += kThreads) {
-      const CellRec c = c_next;
-      const int ln = l + kThreads;
-      if (ln < n_loc) c_next = in[ln < H.n_own ? H.cell0 + ln : halo_ids[ln]];
-      double u = 0.0, v = 0.0;
-      if (c.h > h_dry) { u = c.qx / c.h; v = c.qy / c.h; }
-      sh_h[l] = c.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c.z;
-      water |= (c.h != 0.0);
+    int l;
+    for (int base = tid; base < n_loc; base += 3 * kThreads) {
+      int gid[3];
+      CellRec c[3];
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        l = base + j * kThreads;
+        gid[j] = l < H.n_own ? H.cell0 + l : (l < n_loc ? halo_ids[l] : -1);
+      }
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+        if (gid[j] >= 0) c[j] = in[gid[j]];
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        l = base + j * kThreads;
+        if (gid[j] >= 0) {
+          double u = 0.0, v = 0.0;
+          if (c[j].h > h_dry) { u = c[j].qx / c[j].h; v = c[j].qy / c[j].h; }
+          sh_h[l] = c[j].h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c[j].z;
+          water |= (c[j].h != 0.0);
+        }
+      }
     }
     // second, exact test on the local cells themselves (the flags above are per whole patch): no water in any
     // local cell and no boundary string -> same result (+0, 0, 0)
