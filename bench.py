@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--time-steps", type=int, default=100, help="time steps per bench step (our arm)")
     ap.add_argument("--variant", type=int, default=0, help="include/swe.h SWE_VARIANT_* (0 = library default)")
     ap.add_argument("--patch-cells", type=int, default=0, help="cells per patch of the fused step (0 = default)")
+    ap.add_argument("--renumber", type=int, default=1, help="SWE_RENUMBER_*: 0 input order, 1 Morton, 2 RCM")
+    ap.add_argument("--shuffle-input", action="store_true", help="randomly renumber the input mesh first (A/B runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-wet", action="store_true", help="skip the second (all-wet mesh) line")
@@ -249,9 +251,12 @@ def main():
             dist.barrier()
 
     w = load_workload(args.config, args.scale, rank, world, barrier)
+    if args.shuffle_input:
+        w = w.permuted(12862)[0]
     N, E, T = w.n_cells, w.n_edges, args.time_steps
     t_create = time.perf_counter()
-    s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
+    s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells,
+                        renumber=args.renumber)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     stream = torch.cuda.current_stream(dev)
@@ -368,7 +373,7 @@ def main():
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
-                       "create_s": round(t_create, 2), "step_kernels": s_kernels, "patch": patch_stats},
+                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet,

@@ -42,7 +42,7 @@ enum { SWE_EDGE_WALL = -1, SWE_EDGE_TRANSMISSIVE = -2 /* , -3 - s = member of bo
 /* Boundary-string types for swe_set_boundary (types named at P:342; formulas are readings R-11, R-12) */
 enum { SWE_BC_NONE = 0 /* string behaves as wall */, SWE_BC_INFLOW_Q = 1, SWE_BC_OUTFLOW_UNIFORM = 2 };
 /* Cell / edge renumbering applied inside the library (invisible at this boundary) */
-enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1 };
+enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1, SWE_RENUMBER_RCM = 2 /* reverse Cuthill-McKee */ };
 /* Step variant: both compute bit-identical states; AUTO = the one that measured fastest */
 enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta -> CSR gather + update */,
        SWE_VARIANT_PATCH = 2 /* one fused kernel per step over shared-memory mesh patches */ };

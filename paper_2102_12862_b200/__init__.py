@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(HERE, "libswe_b200.so")
 OK, EINVAL, EMESH, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4, -5
 EDGE_WALL, EDGE_TRANSMISSIVE = -1, -2
 BC_NONE, BC_INFLOW_Q, BC_OUTFLOW_UNIFORM = 0, 1, 2
-RENUMBER_NONE, RENUMBER_MORTON = 0, 1
+RENUMBER_NONE, RENUMBER_MORTON, RENUMBER_RCM = 0, 1, 2
 FLAG_NONFINITE, FLAG_DT_UNBOUNDED = 1, 2
 VARIANT_AUTO, VARIANT_THREE_PASS, VARIANT_PATCH = 0, 1, 2
 

@@ -119,8 +119,8 @@ inline uint64_t spread_bits_21(uint64_t v) {   // 21 bits -> every third... here
   return v;
 }
 
-// Cells along the Morton (Z-order) curve of their centroids; edges in the order of the lower new cell id they
-// touch (ties: the other cell).  Slot order inside a cell and L/R of an edge are untouched (R-15).
+// mode 1: cells along the Morton (Z-order) curve of their centroids; mode 2: reverse Cuthill-McKee (below); edges in
+// the order of the lower new cell id they touch (ties: the other cell).  Slot order inside a cell and L/R of an edge are untouched (R-15).
 inline void renumber(int mode, int64_t nc, const double *xy, const int32_t *tri, HostMesh &m) {
   const int64_t ne = m.ne;
   m.cell_perm.resize(nc); m.cell_new.resize(nc); m.edge_perm.resize(ne); m.edge_new.resize(ne);
@@ -145,6 +145,42 @@ inline void renumber(int mode, int64_t nc, const double *xy, const int32_t *tri,
     }
     std::sort(keyed.begin(), keyed.end());
     for (int64_t i = 0; i < nc; ++i) m.cell_perm[i] = keyed[i].second;
+  }
+  if (mode == 2 && nc > 0) {
+    // Reverse Cuthill-McKee on the cell adjacency graph (degree <= 3): breadth-first levels from the cell with the
+    // lowest Morton key, neighbours visited in ascending (degree, Morton rank), the whole order reversed.
+    std::vector<int32_t> rank(nc);                       // Morton rank of every caller cell (computed above)
+    for (int64_t i = 0; i < nc; ++i) rank[m.cell_perm[i]] = (int32_t)i;
+    std::vector<int32_t> morton = m.cell_perm, order;
+    order.reserve(nc);
+    std::vector<uint8_t> seen(nc, 0);
+    auto degree = [&](int32_t c) {
+      int d = 0;
+      for (int k = 0; k < 3; ++k) d += m.edge_cell[2 * m.cell_edge[3 * c + k] + 1] >= 0;
+      return d;
+    };
+    size_t next_seed = 0;
+    while ((int64_t)order.size() < nc) {
+      while (seen[morton[next_seed]]) ++next_seed;
+      size_t head = order.size();
+      order.push_back(morton[next_seed]); seen[morton[next_seed]] = 1;
+      while (head < order.size()) {
+        const int32_t c = order[head++];
+        int32_t nb[3]; int n = 0;
+        for (int k = 0; k < 3; ++k) {
+          const int32_t e = m.cell_edge[3 * c + k];
+          const int32_t L = m.edge_cell[2 * e], R = m.edge_cell[2 * e + 1];
+          const int32_t o = (L == c) ? R : L;
+          if (o >= 0 && !seen[o]) { seen[o] = 1; nb[n++] = o; }
+        }
+        std::sort(nb, nb + n, [&](int32_t a, int32_t b) {
+          const int da = degree(a), db = degree(b);
+          return da != db ? da < db : rank[a] < rank[b];
+        });
+        for (int k = 0; k < n; ++k) order.push_back(nb[k]);
+      }
+    }
+    for (int64_t i = 0; i < nc; ++i) m.cell_perm[i] = order[nc - 1 - i];
   }
   for (int64_t i = 0; i < nc; ++i) m.cell_new[m.cell_perm[i]] = (int32_t)i;
   if (mode != 0 && ne > 0) {

@@ -18,6 +18,7 @@ namespace swe {
 
 constexpr int kBlock = 256;           // threads per block of the mesh kernels
 constexpr int kCtlThreads = 1024;     // the single block of k_step_control
+constexpr int kTreeCap = 4096;        // boundary-string members whose pairwise tree fits the block's shared memory
 
 // boundary codes / string types (values of include/swe.h, restated so that device code needs no host header)
 constexpr int kEdgeTransmissive = -2;
@@ -321,7 +322,9 @@ __device__ __forceinline__ double block_tree_sum(double *v, int pow2) {
     for (int j = threadIdx.x; 2 * s * j + s < pow2; j += blockDim.x) v[2 * s * j] = v[2 * s * j] + v[2 * s * j + s];
   }
   __syncthreads();
-  return v[0];
+  const double sum = v[0];
+  __syncthreads();                    // v may be refilled by the caller right away
+  return sum;
 }
 
 __device__ __forceinline__ double hydrograph(const double *p, int n_params, double t) {  // piecewise linear, clamped
@@ -342,6 +345,8 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
                const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
                const double *__restrict__ theta, const CellRec *rec_a, const CellRec *rec_b,
                const double *__restrict__ kst, const double *__restrict__ string_M, int mode) {
+  // the pairwise trees run in shared memory when the string fits (same pairs, same order as in global scratch)
+  __shared__ double s_tree[kTreeCap];
   const int ns = ctl->n_strings;
   // ---- volume bookkeeping of the previous step, from the (limited) fluxes actually applied
   if (ctl->pending) {
@@ -351,7 +356,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
       if (bs.type == kBcInflowQ) {
         if (threadIdx.x == 0) ctl->vol_in += dt_prev * bs.Q;
       } else if (bs.type == kBcOutflowUniform) {
-        double *v = scratch + bs.scratch;
+        double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
         for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
           double a = 0.0;
           if (j < bs.n_edges) {
@@ -418,7 +423,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   for (int s = 0; s < ns; ++s) {
     BoundaryString &bs = strings[s];
     if (bs.type != kBcInflowQ) continue;
-    double *v = scratch + bs.scratch;
+    double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
     for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
       double a = 0.0;
       if (j < bs.n_edges) {

@@ -76,3 +76,26 @@ def test_config3_full_size_window(gpu, ref):
     assert ig["vol_clipped"] == 0.0
     s.close()
     o.close()
+
+
+def test_config5_8m_window_and_variants(gpu, ref):
+    """BASELINE.json configs[4] at 8M cells: a 10-step window against the oracle on all cells, then a property that
+    holds at any size -- the two step variants (three-pass and fused patch, which share no kernel on the flux /
+    update path) stay bit-identical over 300 steps -- and the volume balance of the transmissive domain."""
+    w = C.config5()
+    assert 7.8e6 < w.n_cells < 8.2e6
+    s = gpu.from_workload(w)                                           # default variant, as bench.py runs it
+    assert s.patch_stats()["variant"] == gpu.VARIANT_PATCH
+    o = ref.RefSolver(w)
+    ig, io, _ = window(s, o, w, 10, "config5 8M, steps 0-10")
+    check_info(ig, io)
+    o.close()
+    t = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    t.step(10, float("inf"), w.cfl, info=False)
+    i1, i2 = s.step(300, float("inf"), w.cfl), t.step(300, float("inf"), w.cfl)
+    assert i1 == i2 and i1["flags"] == 0 and i1["steps_done"] == 310
+    for x, y in zip(s.get_state(), t.get_state()):
+        assert np.array_equal(x, y)
+    assert i1["n_wet"] == w.n_cells and i1["vol_clipped"] == 0.0
+    s.close()
+    t.close()

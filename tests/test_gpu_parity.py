@@ -195,12 +195,17 @@ def test_renumbering_does_not_change_results(gpu, name):
     b = make(gpu, w, renumber=gpu.RENUMBER_MORTON)
     wp, cp = w.permuted(7)
     c = make(gpu, wp, renumber=gpu.RENUMBER_MORTON)
-    for s in (a, b, c):
+    d = make(gpu, w, renumber=gpu.RENUMBER_RCM, variant=gpu.VARIANT_AUTO, patch_cells=0)   # reverse Cuthill-McKee
+    for s in (a, b, c, d):
         s.step(60, float("inf"), w.cfl)
-    sa, sb, sc = a.get_state(), b.get_state(), c.get_state()
-    for x, y, z in zip(sa, sb, sc):
+    sa, sb, sc, sd = a.get_state(), b.get_state(), c.get_state(), d.get_state()
+    for x, y, z, r in zip(sa, sb, sc, sd):
         assert np.array_equal(x, y)
         assert np.array_equal(x[cp], z)
+        assert np.array_equal(x, r)
+    rp = d.permutation()[0]
+    assert np.array_equal(np.sort(rp), np.arange(w.n_cells)) and not np.array_equal(rp, b.permutation()[0])
+    d.close()
     perm = b.permutation()[0]
     assert np.array_equal(np.sort(perm), np.arange(w.n_cells)) and not np.array_equal(perm, np.arange(w.n_cells))
     for s in (a, b, c):
