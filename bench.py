@@ -56,6 +56,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-wet", action="store_true", help="skip the second (all-wet mesh) line")
+    ap.add_argument("--no-other-variant", action="store_true", help="skip the other step variant's line")
     ap.add_argument("--profile-steps", type=int, default=64, help="event-bracketed steps for the roofline object")
     return ap.parse_args()
 
@@ -331,6 +332,33 @@ def main():
                "d2h_bytes_per_step": 24 * N + 72}
     s.close()
 
+    # ---- the other step variant on the same workload (rank 0, N = 1): the default is the fused patch step, which
+    # moves a third of the bytes; the three-pass step (edge flux -> theta -> CSR gather/update, the design the
+    # north_star names) is the bandwidth-bound one, so its per-kernel HBM fractions are reported beside the default's
+    other = None
+    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0:
+        ov = P.VARIANT_THREE_PASS if s_kernels[-1] == "k_patch_step" else P.VARIANT_PATCH
+        s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber)
+        for _ in range(2):
+            s3.step(T, float("inf"), w.cfl, info=False)
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for _ in range(5):
+            s3.step(T, float("inf"), w.cfl, info=False)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        ms3 = ev0.elapsed_time(ev1)
+        km3 = s3.profile_step(16, w.cfl)
+        alg3 = s3.algorithmic_bytes()
+        pk = peaks()[0]
+        other = {"step_kernels": s3.step_kernels(), "value": N * T * 5 / (ms3 * 1e-3), "unit": UNIT,
+                 "ms_per_time_step": ms3 / (5 * T), "kernel_ms": km3,
+                 "kernel_hbm_frac": {k: (alg3[k] / (km3[k] * 1e-3) / 1e9 / pk if km3[k] > 0 else 0.0) for k in km3},
+                 "step_algorithmic_bytes": sum(alg3.values()),
+                 "step_achieved_gbs": sum(alg3.values()) / (ms3 * 1e-3 / (5 * T)) / 1e9,
+                 "step_hbm_frac": sum(alg3.values()) / (ms3 * 1e-3 / (5 * T)) / 1e9 / pk}
+        s3.close()
+
     # ---- second line (rank 0, N = 1): an ALL-WET mesh of the same size, where no patch can be skipped -- the
     # BASELINE.json configs[4] construction (circular dam break, every cell wet, friction everywhere) at 4M cells
     all_wet = None
@@ -376,7 +404,7 @@ def main():
                        "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet,
+            "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet, "other_variant": other,
             "state_check": {"t": info["t"], "steps_done": info["steps_done"], "n_wet": info["n_wet"],
                             "vol_clipped": info["vol_clipped"], "flags": info["flags"]},
         }
