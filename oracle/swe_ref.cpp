@@ -19,6 +19,7 @@ struct BString {
   int type = 0;
   std::vector<double> params;
   std::vector<int32_t> edges;  // members in ascending (caller) edge id = "string order"
+  std::vector<double> phi_in;  // scalar concentrations carried by an INFLOW_Q string, one per species (default 0)
   // values fixed at t^n by eval_strings():
   double Q = 0.0, sumK = 0.0, sumL = 0.0;
 };
@@ -36,6 +37,10 @@ struct swe_ref_ctx {
   std::vector<double> h, qx, qy;
   std::vector<double> F1, F3, GL, GR;   // per edge, most recent step (after the limiter)
   std::vector<double> theta;            // per cell, most recent step
+  // passive scalars (section 3.3, Eq. 8 advective part; Eq. 20 with A_ij only): specific mass q_c = h phi_c
+  int n_species = 0;
+  std::vector<std::vector<double>> qc;  // [species][cell]
+  std::vector<std::vector<double>> Ac;  // [species][edge] advective scalar flux of the most recent step
   std::map<int, BString> strings;
   double t = 0.0, dt_last = 0.0, vol_clipped = 0.0, vol_in = 0.0, vol_out = 0.0;
   int64_t steps_done = 0;
@@ -338,6 +343,27 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
     else if (c->F1[e] < 0.0 && R >= 0) th = c->theta[R];
     if (th < 1.0) { c->F1[e] = th * c->F1[e]; c->F3[e] = th * c->F3[e]; c->GL[e] = th * c->GL[e]; c->GR[e] = th * c->GR[e]; }
   }
+  // ---- scalar advection, PAPER.md:204-208 (Eq. 8), PAPER.md:298-304 (Eq. 20, advective part A_ij): "the HLLC solver
+  //      ... provides the advective component of the scalar fluxes" = the mass flux times the concentration on the
+  //      upwind side of the contact wave, sign(S*) = sign(F1) (R-19, same upwinding as F3 in R-2).
+  //      phi_i = q_c,i / h_i where h_i > 0, else 0; F1 is the limited mass flux, so a cell never loses more scalar
+  //      mass than it holds.  Ghost concentrations: transmissive, wall, outflow = phi of the interior cell; an
+  //      INFLOW_Q string carries the concentrations set with swe_ref_set_boundary_scalar.
+  for (int sp = 0; sp < c->n_species; ++sp) {
+    const std::vector<double> &q = c->qc[sp];
+    for (int64_t e = 0; e < c->ne; ++e) {
+      const int64_t L = c->eL[e], R = c->eR[e];
+      const double phiL = c->h[L] > 0.0 ? q[L] / c->h[L] : 0.0;
+      double phiR = phiL;
+      if (R >= 0) phiR = c->h[R] > 0.0 ? q[R] / c->h[R] : 0.0;
+      else if (R <= -3) {
+        auto it = c->strings.find(-3 - (int)R);
+        if (it != c->strings.end() && it->second.type == SWE_REF_BC_INFLOW_Q)
+          phiR = sp < (int)it->second.phi_in.size() ? it->second.phi_in[sp] : 0.0;
+      }
+      c->Ac[sp][e] = c->F1[e] * (c->F1[e] >= 0.0 ? phiL : phiR);
+    }
+  }
   // ---- S2 + S3 (in place: the fluxes of step n are already stored per edge)
   for (int64_t i = 0; i < c->nc; ++i) {
     double M[3], X[3], Y[3], s[3];
@@ -368,6 +394,12 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
       }
     }
     c->h[i] = hn; c->qx[i] = qxn; c->qy[i] = qyn;
+    for (int sp = 0; sp < c->n_species; ++sp) {     // Eq. 20, advective part: same gather, same slot order
+      double C[3];
+      for (int k = 0; k < 3; ++k) { const int32_t e = c->ce[3 * i + k]; C[k] = c->len[e] * c->Ac[sp][e]; }
+      const double dC = ((s[0] * C[0] + s[1] * C[1]) + s[2] * C[2]);
+      c->qc[sp][i] = c->qc[sp][i] - a * dC;
+    }
   }
   for (auto &kv : c->strings) {      // bookkeeping from the (limited) fluxes actually applied
     BString &s = kv.second;
@@ -463,6 +495,28 @@ extern "C" int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *
   if (!c || !h || !hu || !hv) return -1;
   c->h.assign(h, h + c->nc); c->qx.assign(hu, hu + c->nc); c->qy.assign(hv, hv + c->nc);
   c->t = t0; c->dt_last = 0.0; c->steps_done = 0; c->vol_clipped = c->vol_in = c->vol_out = 0.0; c->flags = 0;
+  return 0;
+}
+
+extern "C" int swe_ref_set_scalars(swe_ref_ctx *c, int n_species, const double *qc) {
+  if (!c || n_species < 0 || n_species > 5 || (n_species > 0 && !qc)) return -1;   // "up to a maximum of 5"
+  c->n_species = n_species;
+  c->qc.assign(n_species, std::vector<double>(c->nc, 0.0));
+  c->Ac.assign(n_species, std::vector<double>(c->ne, 0.0));
+  for (int sp = 0; sp < n_species; ++sp) c->qc[sp].assign(qc + (size_t)sp * c->nc, qc + (size_t)(sp + 1) * c->nc);
+  return 0;
+}
+
+extern "C" int swe_ref_get_scalars(swe_ref_ctx *c, double *qc) {
+  if (!c || !qc) return -1;
+  for (int sp = 0; sp < c->n_species; ++sp)
+    for (int64_t i = 0; i < c->nc; ++i) qc[(size_t)sp * c->nc + i] = c->qc[sp][i];
+  return 0;
+}
+
+extern "C" int swe_ref_set_boundary_scalar(swe_ref_ctx *c, int string_id, const double *phi, int n) {
+  if (!c || string_id < 0 || n < 0 || (n > 0 && !phi)) return -1;
+  c->strings[string_id].phi_in.assign(phi, phi + n);
   return 0;
 }
 

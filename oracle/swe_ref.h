@@ -56,6 +56,12 @@ enum { SWE_REF_BC_INFLOW_Q = 1, SWE_REF_BC_OUTFLOW_UNIFORM = 2 };
 int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, swe_ref_ctx **out);
 int swe_ref_set_boundary(swe_ref_ctx *c, int string_id, int type, const double *params, int n_params);
 int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *hu, const double *hv, double t0);
+/* Passive scalars (Eq. 8, advective part only; update Eq. 20 PAPER.md:298-304 with A_ij = F1 * phi of
+ * the upwind side; R-19).  qc = [n_species][n_cells] specific masses q_c = h * phi_c, n_species <= 5. */
+int swe_ref_set_scalars(swe_ref_ctx *c, int n_species, const double *qc);
+int swe_ref_get_scalars(swe_ref_ctx *c, double *qc);
+/* concentrations phi[0..n) carried by the water that enters through INFLOW_Q string string_id (default 0) */
+int swe_ref_set_boundary_scalar(swe_ref_ctx *c, int string_id, const double *phi, int n);
 int swe_ref_step(swe_ref_ctx *c, int64_t n_steps, double t_end, double cfl, swe_ref_info *info);
 int swe_ref_get_state(swe_ref_ctx *c, double *h, double *hu, double *hv);
 void swe_ref_destroy(swe_ref_ctx *c);

@@ -49,6 +49,9 @@ def lib():
         L.swe_ref_set_state.argtypes = [C.c_void_p, _f64p, _f64p, _f64p, C.c_double]
         L.swe_ref_step.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.POINTER(Info)]
         L.swe_ref_get_state.argtypes = [C.c_void_p, _f64p, _f64p, _f64p]
+        L.swe_ref_set_scalars.argtypes = [C.c_void_p, C.c_int, _f64p]
+        L.swe_ref_get_scalars.argtypes = [C.c_void_p, _f64p]
+        L.swe_ref_set_boundary_scalar.argtypes = [C.c_void_p, C.c_int, _f64p, C.c_int]
         L.swe_ref_destroy.argtypes = [C.c_void_p]
         L.swe_ref_destroy.restype = None
         L.swe_ref_last_error.argtypes = [C.c_void_p]
@@ -123,6 +126,21 @@ class RefSolver:
         assert all(x.shape == (self.n_cells,) for x in a)
         rc = lib().swe_ref_set_state(self._h, _p(a[0], _f64p), _p(a[1], _f64p), _p(a[2], _f64p), float(t0))
         assert rc == 0
+
+    def set_scalars(self, qc):
+        """qc: [n_species, n_cells] specific masses q_c = h * phi_c."""
+        a = np.ascontiguousarray(qc, np.float64).reshape(-1, self.n_cells)
+        self.n_species = a.shape[0]
+        assert lib().swe_ref_set_scalars(self._h, int(a.shape[0]), _p(a, _f64p)) == 0
+
+    def get_scalars(self):
+        out = np.empty((getattr(self, "n_species", 0), self.n_cells))
+        assert lib().swe_ref_get_scalars(self._h, _p(out, _f64p)) == 0
+        return out
+
+    def set_boundary_scalar(self, string_id, phi):
+        a = np.ascontiguousarray(phi, np.float64)
+        assert lib().swe_ref_set_boundary_scalar(self._h, int(string_id), _p(a, _f64p), int(a.size)) == 0
 
     def step(self, n_steps=-1, t_end=float("inf"), cfl=0.9):
         info = Info()
