@@ -74,7 +74,8 @@ typedef struct {
                            1: they take DEVICE pointers (e.g. torch tensors), read/written on stream  */
   int steps_per_graph;  /* time steps captured per CUDA graph launch; default 32; 0 = no graph       */
   int variant;          /* SWE_VARIANT_*; default AUTO                                               */
-  int patch_cells;      /* cells per patch of the fused step; 0 = default (512)                      */
+  int patch_cells;      /* cells per patch of the fused step; 0 = default (384)                      */
+  int n_species;        /* passive scalar species advected with the flow (0..5); default 0    */
   void *cuda_stream;    /* cudaStream_t all work is enqueued on; NULL = the legacy default stream    */
   void *workspace;      /* DEVICE memory lent by the caller for the context's lifetime (e.g. a torch
                            uint8 tensor), 256-byte aligned, or NULL: the library then cudaMallocs.
@@ -122,6 +123,15 @@ int swe_set_state(swe_ctx *ctx, const double *h, const double *hu, const double 
  * the stream once per chunk of steps when t_end is finite, and once at the end if info != NULL.
  * info may be NULL.  Returns SWE_ENONFINITE if info was requested and the state holds NaN/inf. */
 int swe_step(swe_ctx *ctx, int64_t n_steps, double t_end, double cfl, swe_step_info *info);
+
+/* Passive scalars (section 3.3, Eq. 8, advective part; update Eq. 20 P:298-304 with A_ij = limited mass flux
+ * x concentration on the upwind side of the contact wave; R-19).  qc = [n_species][n_cells] specific masses
+ * q_c = h * phi_c in the CALLER's cell numbering (host or device pointers as for swe_set_state).  They are advanced by
+ * every step of swe_step; swe_set_state does not touch them (new contexts hold q_c = 0). */
+int swe_set_scalars(swe_ctx *ctx, const double *qc);
+int swe_get_scalars(swe_ctx *ctx, double *qc);
+/* concentrations phi[0..n) of the water entering through SWE_BC_INFLOW_Q string string_id (default 0) */
+int swe_set_boundary_scalar(swe_ctx *ctx, int string_id, const double *phi, int n);
 
 /* Reads the state in the caller's cell numbering (host or device pointers as for swe_set_state). */
 int swe_get_state(swe_ctx *ctx, double *h, double *hu, double *hv);

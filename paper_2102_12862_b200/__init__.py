@@ -37,6 +37,7 @@ EXPORTS = (
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
     "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_get_patch_stats",
+    "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar",
 )
 
 
@@ -49,7 +50,7 @@ class SweMesh(C.Structure):
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("h_dry", C.c_double), ("dt_max", C.c_double), ("renumber", C.c_int),
                 ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("variant", C.c_int), ("patch_cells", C.c_int),
-                ("cuda_stream", C.c_void_p),
+                ("n_species", C.c_int), ("cuda_stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -107,6 +108,9 @@ def lib():
         L.swe_algorithmic_bytes.argtypes = [C.c_void_p, C.c_int]
         L.swe_algorithmic_bytes.restype = C.c_int64
         L.swe_get_patch_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int]
+        L.swe_set_scalars.argtypes = [C.c_void_p, C.c_void_p]
+        L.swe_get_scalars.argtypes = [C.c_void_p, C.c_void_p]
+        L.swe_set_boundary_scalar.argtypes = [C.c_void_p, C.c_int, _f64p, C.c_int]
         _lib = L
     return _lib
 
@@ -121,7 +125,7 @@ class Solver:
 
     def __init__(self, node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, *, g=9.81, h_dry=1e-3,
                  dt_max=float("inf"), renumber=RENUMBER_MORTON, state_on_device=False, steps_per_graph=32,
-                 device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0):
+                 device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0, n_species=0):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -145,7 +149,8 @@ class Solver:
         L.swe_params_default(C.byref(prm))
         prm.g, prm.h_dry, prm.dt_max = float(g), float(h_dry), float(dt_max)
         prm.renumber, prm.state_on_device, prm.steps_per_graph = int(renumber), int(bool(state_on_device)), int(steps_per_graph)
-        prm.variant, prm.patch_cells = int(variant), int(patch_cells)
+        prm.variant, prm.patch_cells, prm.n_species = int(variant), int(patch_cells), int(n_species)
+        self.n_species = int(n_species)
         self.stream = torch.cuda.current_stream(self.device)
         prm.cuda_stream = self.stream.cuda_stream
         self.workspace = None
@@ -200,6 +205,32 @@ class Solver:
                 out = tuple(np.empty(self.n_cells) for _ in range(3))
         self._check(lib().swe_get_state(self._h, *self._ptrs(out)))
         return out
+
+    def set_scalars(self, qc):
+        """qc: [n_species, n_cells] specific masses q_c = h * phi_c (numpy, or a torch CUDA tensor with
+        state_on_device=True)."""
+        if self.state_on_device:
+            assert qc.is_cuda and qc.dtype == self._torch.float64 and qc.is_contiguous()
+            assert qc.numel() == self.n_species * self.n_cells
+            ptr = C.c_void_p(qc.data_ptr())
+        else:
+            qc = np.ascontiguousarray(qc, np.float64).reshape(self.n_species, self.n_cells)
+            ptr = C.c_void_p(qc.ctypes.data)
+        self._check(lib().swe_set_scalars(self._h, ptr))
+
+    def get_scalars(self):
+        if self.state_on_device:
+            out = self._torch.empty((self.n_species, self.n_cells), dtype=self._torch.float64, device=self.device)
+            ptr = C.c_void_p(out.data_ptr())
+        else:
+            out = np.empty((self.n_species, self.n_cells))
+            ptr = C.c_void_p(out.ctypes.data)
+        self._check(lib().swe_get_scalars(self._h, ptr))
+        return out
+
+    def set_boundary_scalar(self, string_id, phi):
+        a = np.ascontiguousarray(phi, np.float64)
+        self._check(lib().swe_set_boundary_scalar(self._h, int(string_id), _p(a, _f64p), int(a.size)))
 
     def close(self):
         if getattr(self, "_h", None):

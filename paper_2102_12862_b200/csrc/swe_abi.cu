@@ -76,6 +76,8 @@ struct swe_ctx {
   PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
   PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
+  Scalars sc{};                      // passive scalars: device arrays owned by the library (cudaMalloc)
+  double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
   int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
   int n_patches = 0; size_t patch_smem = 0;
   void (*patch_kernel)(Control *, PatchArgs) = nullptr;
@@ -113,6 +115,7 @@ PatchArgs patch_args(const swe_ctx *c) {
   a.rec_a = c->rec; a.rec_b = c->rec_b; a.area = c->area; a.inv_area = c->inv_area; a.gn2 = c->gn2; a.kst = c->kst;
   a.strings = c->d_strings; a.slot_string = c->d_slot_string; a.string_M = c->d_string_M;
   a.patch_nbr = c->d_patch_nbr; a.dry_a = c->d_dry; a.dry_b = c->d_dry + c->n_patches;
+  a.sc = c->sc;
   a.max_loc = c->pt.max_loc; a.max_c1 = c->pt.max_c1; a.max_e = c->pt.max_e; a.max_eown = c->pt.max_eown;
   return a;
 }
@@ -132,13 +135,13 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
-  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0);
+  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
   if (ev) cudaEventRecord(ev[2], s);
   k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                              (int)c->nc, 0);
   if (ev) cudaEventRecord(ev[3], s);
   k_cell_update<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
-                                                   c->inv_area, c->gn2, c->rec, (int)c->nc);
+                                                   c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   if (ev) cudaEventRecord(ev[4], s);
 }
 
@@ -180,6 +183,12 @@ void release(swe_ctx *c) {
   if (c->d_string_M) cudaFree(c->d_string_M);
   if (c->d_info_part) cudaFree(c->d_info_part);
   if (c->d_info_ticket) cudaFree(c->d_info_ticket);
+  for (int sp = 0; sp < kMaxSpecies; ++sp) {
+    if (c->sc.qa[sp]) cudaFree(c->sc.qa[sp]);
+    if (c->sc.qb[sp]) cudaFree(c->sc.qb[sp]);
+    if (c->sc.phi_up[sp]) cudaFree(c->sc.phi_up[sp]);
+  }
+  if (c->d_scalar_stage) cudaFree(c->d_scalar_stage);
   if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
   if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -339,6 +348,19 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
   }
 
+  // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
+  if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
+  c->sc.n = p.n_species;
+  for (int sp = 0; sp < c->sc.n; ++sp) {
+    SWE_CUDA(c, cudaMalloc((void **)&c->sc.qa[sp], 8 * nc));
+    SWE_CUDA(c, cudaMalloc((void **)&c->sc.qb[sp], 8 * nc));
+    SWE_CUDA(c, cudaMalloc((void **)&c->sc.phi_up[sp], 8 * ne));
+    SWE_CUDA(c, cudaMemset(c->sc.qa[sp], 0, 8 * nc));
+    SWE_CUDA(c, cudaMemset(c->sc.qb[sp], 0, 8 * nc));
+    SWE_CUDA(c, cudaMemset(c->sc.phi_up[sp], 0, 8 * ne));
+  }
+  if (c->sc.n > 0) SWE_CUDA(c, cudaMalloc((void **)&c->d_scalar_stage, 8 * nc));
+
   // ---- fused patch step: patch tables (host build, upload), shared-memory size
   c->variant = (p.variant == SWE_VARIANT_THREE_PASS) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
   if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) {
@@ -354,7 +376,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     PatchTables &pt = c->pt;
     if (!build_patches(nc, ne, geom, ce4, area, string_pos, pc, pt, c->err)) return SWE_EINVAL;
     c->n_patches = (int)pt.hdr.size();
-    c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown).total;
+    c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown, c->sc.n).total;
     // 3 blocks per SM need <= 75 KB each; a numbering that is not spatially compact (renumber = NONE on a
     // scattered input order) blows the halos up: AUTO then falls back to the three-pass step
     if (c->patch_smem > 227 * 1024 || (p.variant == SWE_VARIANT_AUTO && c->patch_smem > 75 * 1024)) {
@@ -370,7 +392,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     // default patch size on a compact numbering: shared-memory arrays with compile-time capacities; anything else
     // (other patch sizes, fatter halos) runs the same kernel with run-time capacities
     constexpr int kCapLoc = 640, kCapC1 = 544, kCapE = 864, kCapEown = 704;
-    if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown &&
+    if (c->sc.n > 0) {               // scalar module: run-time capacities (the concentrations enlarge the block)
+      c->patch_kernel = c->patch_smem <= 75 * 1024 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0, true>
+                                                   : k_patch_step<kPatchThreads, 2, 0, 0, 0, 0, true>;
+    } else if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown &&
         !std::getenv("SWE_PATCH_DYNAMIC")) {
       c->patch_kernel = k_patch_step<kPatchThreads, 3, kCapLoc, kCapC1, kCapE, kCapEown>;
       c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown).total;
@@ -400,7 +425,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
     // state in 32 + state out 32 + pce 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
     c->alg_bytes[0] = 0;
-    c->alg_bytes[1] = 104 * nc + 32 * ne;
+    c->alg_bytes[1] = 104 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;        // + q_c in and out per species
     pt.halo_ids = {}; pt.halo_area = {}; pt.pedge = {}; pt.pce = {}; pt.patch_nbr = {};   // host copies no longer needed
   }
   if (c->variant != SWE_VARIANT_PATCH) {
@@ -411,6 +436,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->alg_bytes[2] = (16 + 32 + 8 + 8) * nc + 64 * ne;
     // cell_edge, 1/area, g/k^2, theta read, CellRec read + written per cell; every EdgeGeom and EdgeFlux gathered once
     c->alg_bytes[3] = (16 + 8 + 8 + 8 + 64) * nc + 64 * ne;
+    c->alg_bytes[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
+    c->alg_bytes[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
   }
 
   // ---- control block
@@ -440,6 +467,7 @@ void swe_params_default(swe_params *p) {
   p->steps_per_graph = 32;
   p->variant = SWE_VARIANT_AUTO;
   p->patch_cells = 0;
+  p->n_species = 0;
 }
 
 size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges) {
@@ -510,7 +538,7 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
   k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
   if (c->variant == SWE_VARIANT_PATCH) {
     k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
-                                                                             c->d_dry + c->n_patches);
+                                                                             c->d_dry + c->n_patches, c->sc);
     c->launches += 1;
   }
   k_reset<<<1, 1, 0, c->stream>>>(c->d_ctl, t0);
@@ -574,6 +602,56 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
   return SWE_OK;
 }
 
+int swe_set_scalars(swe_ctx *c, const double *qc) {
+  if (!c) return SWE_EINVAL;
+  if (c->sc.n == 0) { c->err = "the context was created with n_species = 0"; return SWE_EINVAL; }
+  if (!qc) { c->err = "null scalar pointer"; return SWE_EINVAL; }
+  const int64_t nc = c->nc;
+  for (int sp = 0; sp < c->sc.n; ++sp) {
+    const double *src = qc + (size_t)sp * nc;
+    if (!c->prm.state_on_device) {
+      SWE_CUDA(c, cudaMemcpyAsync(c->d_scalar_stage, src, 8 * nc, cudaMemcpyHostToDevice, c->stream));
+      src = c->d_scalar_stage;
+    }
+    k_pack_scalar<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, src, c->sc.qa[sp], c->sc.qb[sp], (int)nc);
+    c->launches += 1;
+  }
+  if (c->variant == SWE_VARIANT_PATCH) {
+    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
+                                                                             c->d_dry + c->n_patches, c->sc);
+    c->launches += 1;
+  }
+  SWE_CUDA(c, cudaGetLastError());
+  return SWE_OK;
+}
+
+int swe_get_scalars(swe_ctx *c, double *qc) {
+  if (!c) return SWE_EINVAL;
+  if (c->sc.n == 0) { c->err = "the context was created with n_species = 0"; return SWE_EINVAL; }
+  if (!qc) { c->err = "null scalar pointer"; return SWE_EINVAL; }
+  const int64_t nc = c->nc;
+  for (int sp = 0; sp < c->sc.n; ++sp) {
+    double *dst = c->prm.state_on_device ? qc + (size_t)sp * nc : c->d_scalar_stage;
+    k_unpack_scalar<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->sc.qa[sp], c->sc.qb[sp], dst, (int)nc);
+    c->launches += 1;
+    if (!c->prm.state_on_device) {
+      SWE_CUDA(c, cudaMemcpyAsync(qc + (size_t)sp * nc, c->d_scalar_stage, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
+      SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+  }
+  SWE_CUDA(c, cudaGetLastError());
+  return SWE_OK;
+}
+
+int swe_set_boundary_scalar(swe_ctx *c, int string_id, const double *phi, int n) {
+  if (!c) return SWE_EINVAL;
+  if (string_id < 0 || string_id >= (int)c->strings.size() || c->strings[string_id].n_edges == 0) { c->err = "no edge of the mesh belongs to this boundary string"; return SWE_EINVAL; }
+  if (n < 0 || n > kMaxSpecies || (n > 0 && !phi)) { c->err = "bad concentration list"; return SWE_EINVAL; }
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int sp = 0; sp < kMaxSpecies; ++sp) c->strings[string_id].phi_in[sp] = sp < n ? phi[sp] : 0.0;
+  return upload_strings(c);
+}
+
 int swe_get_state(swe_ctx *c, double *h, double *hu, double *hv) {
   if (!c) return SWE_EINVAL;
   if (!h || !hu || !hv) { c->err = "null state pointer"; return SWE_EINVAL; }
@@ -628,7 +706,7 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
-    k_edge_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1);
+    k_edge_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{});
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }

@@ -137,7 +137,7 @@ __device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const Boun
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
-            EdgeFlux *__restrict__ flux, int n_edges, int force) {
+            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc) {
   if (!ctl->active && !force) return;
   const int e = blockIdx.x * kBlock + threadIdx.x;
   if (e >= n_edges) return;
@@ -159,6 +159,18 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     o = boundary_flux(g, eg.R, bs, kst, eg.L, eg.nx, eg.ny, eg.len, a.h, a.z, uL, vL);
   }
   flux[e] = o;
+  // passive scalars (Eq. 8 / Eq. 20 advective part, R-19): concentration on the upwind side of the contact wave
+  for (int sp = 0; sp < sc.n; ++sp) {
+    const double phiL = a.h > 0.0 ? sc.qa[sp][eg.L] / a.h : 0.0;
+    double phiR = phiL;
+    if (eg.R >= 0) {
+      const double hR = rec[eg.R].h;
+      phiR = hR > 0.0 ? sc.qa[sp][eg.R] / hR : 0.0;
+    } else if (eg.R <= -3 && (-3 - eg.R) < ctl->n_strings && strings[-3 - eg.R].type == kBcInflowQ) {
+      phiR = strings[-3 - eg.R].phi_in[sp];
+    }
+    sc.phi_up[sp][e] = o.F1 >= 0.0 ? phiL : phiR;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -232,7 +244,7 @@ __global__ void __launch_bounds__(kBlock)
 k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
               const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
               const double *__restrict__ area, const double *__restrict__ inv_area,
-              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells) {
+              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells, const Scalars sc) {
   if (!ctl->active) return;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   double rate = 0.0;
@@ -241,7 +253,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
     const int4 ce = cell_edge[i];
     const int es[3] = {ce.x, ce.y, ce.z};
     double nx[3], ny[3], len[3];
-    double dHk[3], dXk[3], dYk[3];
+    double dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const EdgeGeom eg = geom[es[k]];
@@ -255,6 +267,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
       const double s = isL ? 1.0 : -1.0;
       nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
+      sgn[k] = s; F1lim[k] = f.F1;
       dHk[k] = s * (eg.len * f.F1);
       dXk[k] = s * (eg.len * (G * eg.nx - f.F3 * eg.ny));
       dYk[k] = s * (eg.len * (G * eg.ny + f.F3 * eg.nx));
@@ -284,6 +297,13 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
     rec[i] = c;
+    for (int sp = 0; sp < sc.n; ++sp) {              // Eq. 20, advective part: same gather, same slot order (R-19)
+      double Ck[3];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) Ck[k] = sgn[k] * (len[k] * (F1lim[k] * sc.phi_up[sp][es[k]]));
+      const double dC = ((Ck[0] + Ck[1]) + Ck[2]);
+      sc.qa[sp][i] = sc.qa[sp][i] - a * dC;
+    }
   }
   block_max_to_global(rate, &ctl->rate_bits);
 }
@@ -530,6 +550,21 @@ k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_per
   const int o = cell_perm[i];
   const CellRec c = rec[i];
   h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
+}
+
+// one scalar species, caller numbering <-> internal numbering, newest state buffer
+__global__ void __launch_bounds__(kBlock)
+k_pack_scalar(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *__restrict__ src,
+              double *qa, double *qb, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i < n_cells) (ctl->cur ? qb : qa)[i] = src[cell_perm[i]];
+}
+
+__global__ void __launch_bounds__(kBlock)
+k_unpack_scalar(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *qa, const double *qb,
+                double *__restrict__ dst, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i < n_cells) dst[cell_perm[i]] = (ctl->cur ? qb : qa)[i];
 }
 
 // inspection (swe_device_cbrt): the cube root of R-14 as the kernels evaluate it

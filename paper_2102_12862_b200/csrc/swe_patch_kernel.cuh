@@ -15,10 +15,11 @@
 namespace swe {
 
 struct PatchSmem {          // offsets (in doubles) into the dynamic shared memory; the same for every block
-  int h, u, v, z, theta, F1, len, F3, GL, GR, nx, ny, total;
+  int h, u, v, z, theta, F1, len, F3, GL, GR, nx, ny, phi, total;
 };
 
-__host__ __device__ inline PatchSmem patch_smem_layout(int max_loc, int max_c1, int max_e, int max_eown) {
+__host__ __device__ inline PatchSmem patch_smem_layout(int max_loc, int max_c1, int max_e, int max_eown,
+                                                       int n_species = 0) {
   PatchSmem s;
   int o = 0;
   s.h = o; o += max_loc; s.u = o; o += max_loc; s.v = o; o += max_loc; s.z = o; o += max_loc;
@@ -26,6 +27,7 @@ __host__ __device__ inline PatchSmem patch_smem_layout(int max_loc, int max_c1, 
   s.F1 = o; o += max_e; s.len = o; o += max_e;
   s.F3 = o; o += max_eown; s.GL = o; o += max_eown; s.GR = o; o += max_eown;
   s.nx = o; o += max_eown; s.ny = o; o += max_eown;
+  s.phi = o; o += n_species * max_loc;          // concentrations of the local cells, species-major
   s.total = o;
   return s;
 }
@@ -44,19 +46,25 @@ struct PatchArgs {
   const int32_t *patch_nbr;       // PatchHeader::nbr_off / n_nbr
   uint8_t *dry_a, *dry_b;         // per state buffer and patch: 1 = every own cell of the patch is exactly (0, 0, 0)
   int max_loc, max_c1, max_e, max_eown;
+  Scalars sc;                     // passive scalars (kScalars instantiation only)
 };
 
 // Loads are software-pipelined: the record an iteration needs is loaded one iteration (or one phase) ahead, so that
 // the global-memory latency overlaps the arithmetic of the current item instead of stalling its first use.
 // kCap* != 0: the shared-memory arrays have these compile-time capacities (every offset becomes an immediate of the
 // LDS / STS instructions); kCap* == 0: capacities come from PatchArgs at run time (any patch size).
-template <int kThreads, int kMinBlocks, int kCapLoc, int kCapC1, int kCapE, int kCapEown>
+// kScalars: the passive-scalar module (R-19) is on: concentrations of the local cells in shared memory, one more
+// gather per species in phase 4 (always with run-time capacities).
+template <int kThreads, int kMinBlocks, int kCapLoc, int kCapC1, int kCapE, int kCapEown, bool kScalars = false>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
   if (!ctl->active) return;
   extern __shared__ double sm[];
+  const int n_sp = kScalars ? A.sc.n : 0;
+  const int cap_loc = kCapLoc ? kCapLoc : A.max_loc;
   const PatchSmem S = kCapLoc ? patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown)
-                              : patch_smem_layout(A.max_loc, A.max_c1, A.max_e, A.max_eown);
+                              : patch_smem_layout(A.max_loc, A.max_c1, A.max_e, A.max_eown, n_sp);
+  double *sh_phi = sm + S.phi;
   double *sh_h = sm + S.h, *sh_u = sm + S.u, *sh_v = sm + S.v, *sh_z = sm + S.z, *sh_th = sm + S.theta;
   double *sh_F1 = sm + S.F1, *sh_len = sm + S.len, *sh_F3 = sm + S.F3, *sh_GL = sm + S.GL, *sh_GR = sm + S.GR;
   double *sh_nx = sm + S.nx, *sh_ny = sm + S.ny;
@@ -90,6 +98,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           CellRec c = in[H.cell0 + l];
           c.h = 0.0; c.qx = 0.0; c.qy = 0.0;
           out[H.cell0 + l] = c;
+          for (int sp = 0; sp < n_sp; ++sp) (src ? A.sc.qa : A.sc.qb)[sp][H.cell0 + l] = 0.0;   // flag: all q_c are 0 too
         }
         __syncthreads();
         if (tid == 0) dry_out[blockIdx.x] = 1;
@@ -140,17 +149,27 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           if (c[j].h > h_dry) { u = c[j].qx / c[j].h; v = c[j].qy / c[j].h; }
           sh_h[l] = c[j].h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c[j].z;
           water |= (c[j].h != 0.0);
+          if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
+            for (int sp = 0; sp < n_sp; ++sp)
+              sh_phi[sp * cap_loc + l] = c[j].h > 0.0 ? (src ? A.sc.qb : A.sc.qa)[sp][gid[j]] / c[j].h : 0.0;
         }
       }
     }
     // second, exact test on the local cells themselves (the flags above are per whole patch): no water in any
     // local cell and no boundary string -> same result (+0, 0, 0)
     if (!__syncthreads_or(water) && H.n_string_edges == 0) {
+      int scalar_mass = 0;
       for (l = tid; l < H.n_own; l += kThreads) {
         CellRec c; c.h = 0.0; c.qx = 0.0; c.qy = 0.0; c.z = sh_z[l];
         out[H.cell0 + l] = c;
+        for (int sp = 0; sp < n_sp; ++sp) {          // no flux: scalar mass parked in dry cells stays where it is
+          const double q = (src ? A.sc.qb : A.sc.qa)[sp][H.cell0 + l];
+          (src ? A.sc.qa : A.sc.qb)[sp][H.cell0 + l] = q;
+          scalar_mass |= (q != 0.0);
+        }
       }
-      if (tid == 0) { dry_out[blockIdx.x] = 1; atomicAdd(&ctl->patches_skipped, 1ull); }
+      scalar_mass = kScalars ? __syncthreads_or(scalar_mass) : 0;
+      if (tid == 0) { dry_out[blockIdx.x] = scalar_mass ? 0 : 1; atomicAdd(&ctl->patches_skipped, 1ull); }
       return;
     }
   }
@@ -223,6 +242,8 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     if (ln < H.n_own) { pc4 = pce[ln]; c4_next = in[i + kThreads]; invA_next = A.inv_area[i + kThreads]; gn2_next = A.gn2[i + kThreads]; }
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
     double dH = 0.0, dX = 0.0, dY = 0.0;             // ((d0 + d1) + d2), accumulated in slot order
+    double F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,
+    int up[3];                                       // local id of the upwind cell, or -1 - slot of an inflow-string edge
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const int e = w[k] & 0x7FFFu;
@@ -241,9 +262,18 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
       const double dXk = s * (lenk * (G * nxk - F3 * nyk));
       const double dYk = s * (lenk * (G * nyk + F3 * nxk));
       if (k == 0) { dH = dHk; dX = dXk; dY = dYk; } else { dH = dH + dHk; dX = dX + dXk; dY = dY + dYk; }
+      if (kScalars) {
+        F1k[k] = F1; slk[k] = lenk;
+        const uint32_t Lc = isL ? (uint32_t)l : nb, Rc = isL ? nb : (uint32_t)l;
+        up[k] = (int)((F1 >= 0.0 || Rc == kPceNoNeighbour) ? Lc : Rc);   // ghost concentration = the interior cell's
+        if (!isL) slk[k] = -lenk;
+      }
       if (nb == kPceNoNeighbour) {                  // boundary-string edge: volume bookkeeping of k_step_control
         const int aux = pedge[e].aux;
-        if (aux <= -3) A.string_M[-3 - aux] = lenk * F1;
+        if (aux <= -3) {
+          A.string_M[-3 - aux] = lenk * F1;
+          if (kScalars && !(F1 >= 0.0) && A.strings[A.slot_string[-3 - aux]].type == kBcInflowQ) up[k] = -1 - (-3 - aux);
+        }
       }
     }
     const double a = dt * invA;
@@ -275,6 +305,21 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     c.h = hn; c.qx = qxn; c.qy = qyn;
     out[i] = c;
     nonzero |= (hn != 0.0) | (qxn != 0.0) | (qyn != 0.0);
+    if (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
+      for (int sp = 0; sp < n_sp; ++sp) {
+        double dC = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const double phi = up[k] >= 0 ? sh_phi[sp * cap_loc + up[k]] : A.strings[A.slot_string[-1 - up[k]]].phi_in[sp];
+          const double lC = fabs(slk[k]) * (F1k[k] * phi);
+          const double Ck = slk[k] < 0.0 ? -lC : lC;
+          dC = k == 0 ? Ck : dC + Ck;
+        }
+        const double qn = (src ? A.sc.qb : A.sc.qa)[sp][i] - a * dC;
+        (src ? A.sc.qa : A.sc.qb)[sp][i] = qn;
+        nonzero |= (qn != 0.0);
+      }
+    }
   }
   nonzero = __syncthreads_or(nonzero);
   if (tid == 0) dry_out[blockIdx.x] = nonzero ? 0 : 1;
@@ -285,13 +330,14 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
 template <int kThreads>
 __global__ void __launch_bounds__(kThreads)
 k_patch_flags(const Control *__restrict__ ctl, const PatchHeader *__restrict__ hdr, const CellRec *rec_a,
-              const CellRec *rec_b, uint8_t *dry_a, uint8_t *dry_b) {
+              const CellRec *rec_b, uint8_t *dry_a, uint8_t *dry_b, const Scalars sc) {
   const PatchHeader H = hdr[blockIdx.x];
   const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   int nonzero = 0;
   for (int l = threadIdx.x; l < H.n_own; l += kThreads) {
     const CellRec c = rec[H.cell0 + l];
     nonzero |= !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
+    for (int sp = 0; sp < sc.n; ++sp) nonzero |= ((ctl->cur ? sc.qb : sc.qa)[sp][H.cell0 + l] != 0.0);
   }
   nonzero = __syncthreads_or(nonzero);
   if (threadIdx.x == 0) {

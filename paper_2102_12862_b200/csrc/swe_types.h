@@ -57,6 +57,16 @@ struct BoundaryString {          // one boundary string (R-11, R-12); lives in d
   double sumL;                   // tree sum of the member lengths (constant)
   double Q, sumK;                // INFLOW_Q: values at t^n, written by k_step_control
   double S0;                     // OUTFLOW_UNIFORM
+  double phi_in[5];              // INFLOW_Q: concentration of every scalar species in the entering water (R-19)
+};
+
+constexpr int kMaxSpecies = 5;   // "up to a maximum of 5"
+
+struct Scalars {                 // passive scalars q_c = h phi_c (section 3.3, Eq. 8; R-19), SoA per species
+  int n;                         // species in use (0: the module is off)
+  double *qa[kMaxSpecies];       // [n_cells] state buffer a (the only one of the three-pass step)
+  double *qb[kMaxSpecies];       // [n_cells] state buffer b (fused patch step)
+  double *phi_up[kMaxSpecies];   // [n_edges] three-pass step: concentration on the upwind side of every edge
 };
 
 struct Control {                 // device-side step-loop state: nothing of it is read by the host per step
