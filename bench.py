@@ -53,6 +53,7 @@ def parse():
     ap.add_argument("--patch-cells", type=int, default=0, help="cells per patch of the fused step (0 = default)")
     ap.add_argument("--renumber", type=int, default=1, help="SWE_RENUMBER_*: 0 input order, 1 Morton, 2 RCM")
     ap.add_argument("--shuffle-input", action="store_true", help="randomly renumber the input mesh first (A/B runs)")
+    ap.add_argument("--species", type=int, default=0, help="passive scalar species advected with the flow (0..5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-wet", action="store_true", help="skip the second (all-wet mesh) line")
@@ -257,7 +258,17 @@ def main():
     N, E, T = w.n_cells, w.n_edges, args.time_steps
     t_create = time.perf_counter()
     s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells,
-                        renumber=args.renumber)
+                        renumber=args.renumber, n_species=args.species)
+    if args.species:
+        from workloads import mesh as WM
+        ctr = WM.centroids(w.node_xy, w.tri)
+        span = np.ptp(ctr, axis=0) + 1e-300
+        phi = [0.5 + 0.5 * np.sin((k + 1) * 6.283185307179586 * (ctr[:, 0] / span[0] + ctr[:, 1] / span[1]))
+               for k in range(args.species)]
+        s.set_scalars(np.stack([p_ * w.h for p_ in phi]))
+        for sid, typ, _ in w.strings:
+            if typ == 1:
+                s.set_boundary_scalar(sid, [1.0] * args.species)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     stream = torch.cuda.current_stream(dev)
@@ -313,6 +324,7 @@ def main():
     if not args.no_e2e:
         host = [torch.empty(N, dtype=torch.float64, pin_memory=True).numpy() for _ in range(3)]
         s.get_state(tuple(host))
+        host_q = s.get_scalars() if args.species else None      # (pageable; the scalar copies are in the region too)
         t_now = info["t"]
         for _ in range(min(2, args.warmup)):
             s.set_state(*host, t0=t_now)
@@ -323,20 +335,24 @@ def main():
         t0 = time.perf_counter()
         for _ in range(args.steps):
             s.set_state(*host, t0=t_now)                               # H2D: 3 x 8 x N bytes
+            if args.species:
+                s.set_scalars(host_q)                                  # H2D: species x 8 x N bytes
             t_now = s.step(T, float("inf"), w.cfl, info=True)["t"]    # info: the step's result scalars come back
             s.get_state(tuple(host))                                   # D2H: 3 x 8 x N bytes
+            if args.species:
+                host_q = s.get_scalars()
         torch.cuda.synchronize()
         dt_e2e = time.perf_counter() - t0
         dt_e2e = max_over_ranks(dt_e2e, world, dev)
-        e2e = {"value": aggregate_value(N, T, args.steps, world, dt_e2e), "unit": UNIT, "h2d_bytes_per_step": 24 * N,
-               "d2h_bytes_per_step": 24 * N + 72}
+        e2e = {"value": aggregate_value(N, T, args.steps, world, dt_e2e), "unit": UNIT, "h2d_bytes_per_step": (24 + 8 * args.species) * N,
+               "d2h_bytes_per_step": (24 + 8 * args.species) * N + 72}
     s.close()
 
     # ---- the other step variant on the same workload (rank 0, N = 1): the default is the fused patch step, which
     # moves a third of the bytes; the three-pass step (edge flux -> theta -> CSR gather/update, the design the
     # north_star names) is the bandwidth-bound one, so its per-kernel HBM fractions are reported beside the default's
     other = None
-    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0:
+    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0:
         ov = P.VARIANT_THREE_PASS if s_kernels[-1] == "k_patch_step" else P.VARIANT_PATCH
         s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber)
         for _ in range(2):
@@ -362,7 +378,7 @@ def main():
     # ---- second line (rank 0, N = 1): an ALL-WET mesh of the same size, where no patch can be skipped -- the
     # BASELINE.json configs[4] construction (circular dam break, every cell wet, friction everywhere) at 4M cells
     all_wet = None
-    if rank == 0 and world == 1 and not args.no_all_wet:
+    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0:
         from workloads import configs as C
         w2 = C.config5(target_cells=N)
         s2 = P.from_workload(w2, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
@@ -401,7 +417,7 @@ def main():
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
-                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "step_kernels": s_kernels, "patch": patch_stats},
+                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet, "other_variant": other,

@@ -135,13 +135,20 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
-  k_edge_flux<<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
+  if (c->sc.n > 0)
+    k_edge_flux<true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
+  else
+    k_edge_flux<false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
   if (ev) cudaEventRecord(ev[2], s);
   k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                              (int)c->nc, 0);
   if (ev) cudaEventRecord(ev[3], s);
-  k_cell_update<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
-                                                   c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
+  if (c->sc.n > 0)
+    k_cell_update<true><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
+                                                           c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
+  else
+    k_cell_update<false><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
+                                                            c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   if (ev) cudaEventRecord(ev[4], s);
 }
 
@@ -379,7 +386,9 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown, c->sc.n).total;
     // 3 blocks per SM need <= 75 KB each; a numbering that is not spatially compact (renumber = NONE on a
     // scattered input order) blows the halos up: AUTO then falls back to the three-pass step
-    if (c->patch_smem > 227 * 1024 || (p.variant == SWE_VARIANT_AUTO && c->patch_smem > 75 * 1024)) {
+    // (with scalar species the block is fatter anyway: 2 blocks per SM, <= 113 KB, still beat the three-pass step)
+    const size_t auto_limit = (c->sc.n > 0 ? 113 : 75) * 1024;
+    if (c->patch_smem > 227 * 1024 || (p.variant == SWE_VARIANT_AUTO && c->patch_smem > auto_limit)) {
       if (p.variant == SWE_VARIANT_AUTO) { c->variant = SWE_VARIANT_THREE_PASS; c->pt = PatchTables{}; c->n_patches = 0; c->patch_smem = 0; }
       else { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
     }
@@ -706,7 +715,7 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
-    k_edge_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{});
+    k_edge_flux<false><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{});
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }

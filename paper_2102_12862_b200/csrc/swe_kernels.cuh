@@ -134,6 +134,7 @@ __device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const Boun
 // S1: one thread per edge.  Reads one EdgeGeom record (coalesced 256-bit), gathers the two CellRec records
 // (one sector each), writes one EdgeFlux record (coalesced 256-bit).
 // ---------------------------------------------------------------------------------------------------------
+template <bool kScalars>
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
@@ -160,7 +161,8 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
   }
   flux[e] = o;
   // passive scalars (Eq. 8 / Eq. 20 advective part, R-19): concentration on the upwind side of the contact wave
-  for (int sp = 0; sp < sc.n; ++sp) {
+  if (kScalars)
+  _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
     const double phiL = a.h > 0.0 ? sc.qa[sp][eg.L] / a.h : 0.0;
     double phiR = phiL;
     if (eg.R >= 0) {
@@ -240,6 +242,7 @@ __device__ __forceinline__ double cell_rate(double g, double h, double qx, doubl
 // ---------------------------------------------------------------------------------------------------------
 // S2 + S3, and S0 of the NEXT step fused in: one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
+template <bool kScalars>
 __global__ void __launch_bounds__(kBlock)
 k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
               const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
@@ -267,7 +270,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
       const double s = isL ? 1.0 : -1.0;
       nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
-      sgn[k] = s; F1lim[k] = f.F1;
+      if (kScalars) { sgn[k] = s; F1lim[k] = f.F1; }
       dHk[k] = s * (eg.len * f.F1);
       dXk[k] = s * (eg.len * (G * eg.nx - f.F3 * eg.ny));
       dYk[k] = s * (eg.len * (G * eg.ny + f.F3 * eg.nx));
@@ -297,7 +300,8 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
     rec[i] = c;
-    for (int sp = 0; sp < sc.n; ++sp) {              // Eq. 20, advective part: same gather, same slot order (R-19)
+    if (kScalars)                                    // Eq. 20, advective part: same gather, same slot order (R-19)
+    _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
       double Ck[3];
 #pragma unroll
       for (int k = 0; k < 3; ++k) Ck[k] = sgn[k] * (len[k] * (F1lim[k] * sc.phi_up[sp][es[k]]));

@@ -98,7 +98,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           CellRec c = in[H.cell0 + l];
           c.h = 0.0; c.qx = 0.0; c.qy = 0.0;
           out[H.cell0 + l] = c;
-          for (int sp = 0; sp < n_sp; ++sp) (src ? A.sc.qa : A.sc.qb)[sp][H.cell0 + l] = 0.0;   // flag: all q_c are 0 too
+          _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) (src ? A.sc.qa[sp] : A.sc.qb[sp])[H.cell0 + l] = 0.0;   // flag: all q_c are 0 too
         }
         __syncthreads();
         if (tid == 0) dry_out[blockIdx.x] = 1;
@@ -150,8 +150,8 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           sh_h[l] = c[j].h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c[j].z;
           water |= (c[j].h != 0.0);
           if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
-            for (int sp = 0; sp < n_sp; ++sp)
-              sh_phi[sp * cap_loc + l] = c[j].h > 0.0 ? (src ? A.sc.qb : A.sc.qa)[sp][gid[j]] / c[j].h : 0.0;
+            _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
+              sh_phi[sp * cap_loc + l] = c[j].h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[gid[j]] / c[j].h : 0.0;
         }
       }
     }
@@ -162,9 +162,9 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
       for (l = tid; l < H.n_own; l += kThreads) {
         CellRec c; c.h = 0.0; c.qx = 0.0; c.qy = 0.0; c.z = sh_z[l];
         out[H.cell0 + l] = c;
-        for (int sp = 0; sp < n_sp; ++sp) {          // no flux: scalar mass parked in dry cells stays where it is
-          const double q = (src ? A.sc.qb : A.sc.qa)[sp][H.cell0 + l];
-          (src ? A.sc.qa : A.sc.qb)[sp][H.cell0 + l] = q;
+        _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {          // no flux: scalar mass parked in dry cells stays where it is
+          const double q = (src ? A.sc.qb[sp] : A.sc.qa[sp])[H.cell0 + l];
+          (src ? A.sc.qa[sp] : A.sc.qb[sp])[H.cell0 + l] = q;
           scalar_mass |= (q != 0.0);
         }
       }
@@ -306,7 +306,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     out[i] = c;
     nonzero |= (hn != 0.0) | (qxn != 0.0) | (qyn != 0.0);
     if (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
-      for (int sp = 0; sp < n_sp; ++sp) {
+      _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {
         double dC = 0.0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -315,8 +315,8 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           const double Ck = slk[k] < 0.0 ? -lC : lC;
           dC = k == 0 ? Ck : dC + Ck;
         }
-        const double qn = (src ? A.sc.qb : A.sc.qa)[sp][i] - a * dC;
-        (src ? A.sc.qa : A.sc.qb)[sp][i] = qn;
+        const double qn = (src ? A.sc.qb[sp] : A.sc.qa[sp])[i] - a * dC;
+        (src ? A.sc.qa[sp] : A.sc.qb[sp])[i] = qn;
         nonzero |= (qn != 0.0);
       }
     }
@@ -337,7 +337,7 @@ k_patch_flags(const Control *__restrict__ ctl, const PatchHeader *__restrict__ h
   for (int l = threadIdx.x; l < H.n_own; l += kThreads) {
     const CellRec c = rec[H.cell0 + l];
     nonzero |= !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
-    for (int sp = 0; sp < sc.n; ++sp) nonzero |= ((ctl->cur ? sc.qb : sc.qa)[sp][H.cell0 + l] != 0.0);
+    _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) nonzero |= ((ctl->cur ? sc.qb[sp] : sc.qa[sp])[H.cell0 + l] != 0.0);
   }
   nonzero = __syncthreads_or(nonzero);
   if (threadIdx.x == 0) {

@@ -67,13 +67,22 @@ def test_config4_full_size_windows(gpu, ref):
 
 
 def test_config3_full_size_window(gpu, ref):
+    """configs[2] at full size, with two passive scalar species riding along (R-19)."""
     w = C.config3()
     assert 0.95e6 < w.n_cells < 1.05e6
-    s = make(gpu, w)
+    rng = np.random.default_rng(3)
+    qc0 = np.stack([rng.random(w.n_cells) * w.h, w.h])
+    s = make(gpu, w, n_species=2)
     o = ref.RefSolver(w)
-    ig, io, _ = window(s, o, w, 40, "config3 full size, steps 0-40")
+    s.set_scalars(qc0)
+    o.set_scalars(qc0)
+    ig, io, sg = window(s, o, w, 40, "config3 full size, steps 0-40")
     check_info(ig, io)
     assert ig["vol_clipped"] == 0.0
+    qg, qo = s.get_scalars(), o.get_scalars()
+    for sp in range(2):
+        assert np.all(np.abs(qg[sp] - qo[sp]) <= 1e-10 * np.abs(qo[sp]) + 1e-14 * np.max(np.abs(qo[sp])))
+    assert np.array_equal(qg[1], sg[0])                  # phi = 1: q_c == h bit for bit
     s.close()
     o.close()
 
