@@ -76,6 +76,7 @@ struct swe_ctx {
   PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
   PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
+  uint8_t *d_drain_flag = nullptr;   // three-pass step: cells flagged as possible drainers (lazy theta)
   Scalars sc{};                      // passive scalars: device arrays owned by the library (cudaMalloc)
   double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
   int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
@@ -104,7 +105,7 @@ namespace {
 // the kernels of one time step, in stream order; ev (nullable) = n_step_kernels + 1 events recorded around them
 constexpr int kMaxStepKernels = 4;
 constexpr int kPatchThreads = 256;
-const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta", "k_cell_update"};
+const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"};
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
 
 inline int n_step_kernels(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH ? 2 : 4; }
@@ -122,7 +123,7 @@ PatchArgs patch_args(const swe_ctx *c) {
 
 void launch_control(swe_ctx *c, cudaStream_t s, int mode) {
   k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
-                                           c->theta, c->rec, c->rec_b, c->kst,
+                                           nullptr /* records are limited in place */, c->rec, c->rec_b, c->kst,
                                            c->variant == SWE_VARIANT_PATCH ? c->d_string_M : nullptr, mode);
 }
 
@@ -136,18 +137,20 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     return;
   }
   if (c->sc.n > 0)
-    k_edge_flux<true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
+    k_edge_flux<true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+                                                         c->area, c->d_drain_flag);
   else
-    k_edge_flux<false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc);
+    k_edge_flux<false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+                                                          c->area, c->d_drain_flag);
   if (ev) cudaEventRecord(ev[2], s);
-  k_theta<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
-                                             (int)c->nc, 0);
+  k_theta_lazy<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
+                                                  c->d_drain_flag, (int)c->nc);
   if (ev) cudaEventRecord(ev[3], s);
   if (c->sc.n > 0)
-    k_cell_update<true><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
+    k_cell_update<true><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
                                                            c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   else
-    k_cell_update<false><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->theta, c->area,
+    k_cell_update<false><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
                                                             c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   if (ev) cudaEventRecord(ev[4], s);
 }
@@ -196,6 +199,7 @@ void release(swe_ctx *c) {
     if (c->sc.phi_up[sp]) cudaFree(c->sc.phi_up[sp]);
   }
   if (c->d_scalar_stage) cudaFree(c->d_scalar_stage);
+  if (c->d_drain_flag) cudaFree(c->d_drain_flag);
   if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
   if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -355,6 +359,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
   }
 
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_drain_flag, std::max<size_t>(nc, 16)));
+  SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, std::max<size_t>(nc, 16)));
   // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
   c->sc.n = p.n_species;
@@ -442,9 +448,9 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->alg_bytes[0] = 0;
     c->alg_bytes[1] = 64 * ne + 32 * nc;
     // cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
-    c->alg_bytes[2] = (16 + 32 + 8 + 8) * nc + 64 * ne;
+    c->alg_bytes[2] = 1 * nc;                                      // k_theta_lazy: one flag byte per cell
     // cell_edge, 1/area, g/k^2, theta read, CellRec read + written per cell; every EdgeGeom and EdgeFlux gathered once
-    c->alg_bytes[3] = (16 + 8 + 8 + 8 + 64) * nc + 64 * ne;
+    c->alg_bytes[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
     c->alg_bytes[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
     c->alg_bytes[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
   }
@@ -715,13 +721,14 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
-    k_edge_flux<false><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{});
+    k_edge_flux<false><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{}, c->area, nullptr);
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }
   double *d = nullptr;
   SWE_CUDA(c, cudaMalloc((void **)&d, 8 * 4 * ne));
-  k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, c->theta, d, d + ne, d + 2 * ne,
+  const double *th_apply = (c->variant == SWE_VARIANT_PATCH) ? c->theta : nullptr;   // three-pass: limited in place
+  k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, th_apply, d, d + ne, d + 2 * ne,
                                                         d + 3 * ne, (int)ne);
   c->launches += 1;
   cudaError_t e1 = cudaStreamSynchronize(c->stream);

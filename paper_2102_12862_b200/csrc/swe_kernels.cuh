@@ -138,7 +138,8 @@ template <bool kScalars>
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
-            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc) {
+            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,
+            const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
   if (!ctl->active && !force) return;
   const int e = blockIdx.x * kBlock + threadIdx.x;
   if (e >= n_edges) return;
@@ -160,6 +161,16 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     o = boundary_flux(g, eg.R, bs, kst, eg.L, eg.nx, eg.ny, eg.len, a.h, a.z, uL, vL);
   }
   flux[e] = o;
+  // S1c, lazily (R-8b): theta_i < 1 needs dt * (o_0 + o_1 + o_2) > h_i |Omega_i|, hence at least one outgoing edge with
+  // dt * o_k > 0.3 h_i |Omega_i| (0.3 * 3 * (1 + rounding) < 1).  Only such donor cells are flagged; k_theta_lazy evaluates
+  // theta exactly for them and every other cell keeps theta = 1 without being visited.
+  if (drain_flag) {
+    const int d = o.F1 > 0.0 ? eg.L : ((o.F1 < 0.0 && eg.R >= 0) ? eg.R : -1);
+    if (d >= 0) {
+      const double hd = (d == eg.L) ? a.h : rec[d].h;
+      if (ctl->dt * (eg.len * fabs(o.F1)) > 0.3 * (hd * area[d])) drain_flag[d] = 1;
+    }
+  }
   // passive scalars (Eq. 8 / Eq. 20 advective part, R-19): concentration on the upwind side of the contact wave
   if (kScalars)
   _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
@@ -199,6 +210,50 @@ k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
   const double out = ((o[0] + o[1]) + o[2]);
   const double avail = rec[i].h * area[i];
   theta[i] = (dt * out > avail) ? avail / (dt * out) : 1.0;
+}
+
+// S1c for the flagged cells only (see k_edge_flux): theta_i exactly as in k_theta; when theta_i < 1 the cell scales the
+// records of its own outgoing edges in place -- every edge has exactly one donor, so no two cells touch one record,
+// and a neighbour that reads the same record for its own theta sees it as an inflow (o_k = 0) before and after.
+// flag bits: 1 = flagged by k_edge_flux in this step, 2 = theta[i] holds a value < 1 from an earlier step.
+__global__ void __launch_bounds__(kBlock)
+k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
+             EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
+             double *__restrict__ theta, uint8_t *__restrict__ drain_flag, int n_cells) {
+  if (!ctl->active) return;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  const uint8_t fl = drain_flag[i];
+  if (fl == 0) return;
+  double th = 1.0;
+  if (fl & 1) {
+    const double dt = ctl->dt;
+    const int4 ce = cell_edge[i];
+    const int es[3] = {ce.x, ce.y, ce.z};
+    double o[3];
+    bool isL[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const EdgeGeom eg = geom[es[k]];
+      isL[k] = (eg.L == i);
+      const double sM = (isL[k] ? 1.0 : -1.0) * (eg.len * flux[es[k]].F1);
+      o[k] = dmax0(sM);
+    }
+    const double out = ((o[0] + o[1]) + o[2]);
+    const double avail = rec[i].h * area[i];
+    if (dt * out > avail) th = avail / (dt * out);
+    if (th < 1.0) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k)
+        if (o[k] > 0.0) {
+          EdgeFlux f = flux[es[k]];
+          f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR;
+          flux[es[k]] = f;
+        }
+    }
+  }
+  theta[i] = th;
+  drain_flag[i] = th < 1.0 ? 2 : 0;
 }
 
 // block-wide max of non-negative doubles -> one atomicMax on the bit pattern (order-preserving for x >= 0)
@@ -263,11 +318,13 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       EdgeFlux f = flux[es[k]];
       const bool isL = (eg.L == i);
       // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
-      double th = 1.0;
-      if (f.F1 > 0.0) th = theta[eg.L];
-      else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
       double G = isL ? f.GL : f.GR;
-      if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
+      if (theta) {                                   // eager variant; nullptr: k_theta_lazy has limited the records
+        double th = 1.0;
+        if (f.F1 > 0.0) th = theta[eg.L];
+        else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
+        if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
+      }
       const double s = isL ? 1.0 : -1.0;
       nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
       if (kScalars) { sgn[k] = s; F1lim[k] = f.F1; }
@@ -390,7 +447,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
               const int e = string_edges[bs.first + j];
               const EdgeGeom eg = geom[e];
               double F1 = flux[e].F1;
-              if (F1 > 0.0) {
+              if (theta && F1 > 0.0) {              // nullptr: the records are limited already (k_theta_lazy)
                 const double th = theta[eg.L];
                 if (th < 1.0) F1 = th * F1;
               }
@@ -587,10 +644,12 @@ k_export_flux(const int *__restrict__ edge_perm, const EdgeGeom *__restrict__ ge
   if (e >= n_edges) return;
   const EdgeGeom eg = geom[e];
   EdgeFlux f = flux[e];
-  double th = 1.0;
-  if (f.F1 > 0.0) th = theta[eg.L];
-  else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
-  if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR; }
+  if (theta) {                                       // nullptr: the records are limited already (k_theta_lazy)
+    double th = 1.0;
+    if (f.F1 > 0.0) th = theta[eg.L];
+    else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
+    if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR; }
+  }
   const int o = edge_perm[e];
   F1[o] = f.F1; F3[o] = f.F3; GL[o] = f.GL; GR[o] = f.GR;
 }
