@@ -143,7 +143,7 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     k_edge_flux<false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                           c->area, c->d_drain_flag);
   if (ev) cudaEventRecord(ev[2], s);
-  k_theta_lazy<<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
+  k_theta_lazy<<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                                   c->d_drain_flag, (int)c->nc);
   if (ev) cudaEventRecord(ev[3], s);
   if (c->sc.n > 0)
@@ -359,8 +359,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
   }
 
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_drain_flag, std::max<size_t>(nc, 16)));
-  SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, std::max<size_t>(nc, 16)));
+  SWE_CUDA(c, cudaMalloc((void **)&c->d_drain_flag, (size_t)nc + 16));           // read four bytes at a time
+  SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, (size_t)nc + 16));
   // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
   c->sc.n = p.n_species;

@@ -221,10 +221,15 @@ k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge
              EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
              double *__restrict__ theta, uint8_t *__restrict__ drain_flag, int n_cells) {
   if (!ctl->active) return;
-  const int i = blockIdx.x * kBlock + threadIdx.x;
-  if (i >= n_cells) return;
-  const uint8_t fl = drain_flag[i];
-  if (fl == 0) return;
+  // four flag bytes per thread: almost every word is 0 and the thread leaves after one 4-byte load
+  const int i4 = (blockIdx.x * kBlock + threadIdx.x) * 4;
+  if (i4 >= n_cells) return;
+  const uint32_t f4 = *reinterpret_cast<const uint32_t *>(drain_flag + i4);     // the array is padded to 4 bytes
+  if (f4 == 0u) return;
+  for (int j = 0; j < 4; ++j) {
+  const int i = i4 + j;
+  const uint8_t fl = (uint8_t)(f4 >> (8 * j));
+  if (fl == 0 || i >= n_cells) continue;
   double th = 1.0;
   if (fl & 1) {
     const double dt = ctl->dt;
@@ -254,6 +259,7 @@ k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge
   }
   theta[i] = th;
   drain_flag[i] = th < 1.0 ? 2 : 0;
+  }
 }
 
 // block-wide max of non-negative doubles -> one atomicMax on the bit pattern (order-preserving for x >= 0)
@@ -298,7 +304,7 @@ __device__ __forceinline__ double cell_rate(double g, double h, double qx, doubl
 // S2 + S3, and S0 of the NEXT step fused in: one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
 template <bool kScalars>
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(kBlock, kScalars ? 3 : 4)      // 4 blocks/SM = 64 registers: measured faster than 3
 k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
               const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
               const double *__restrict__ area, const double *__restrict__ inv_area,
