@@ -82,9 +82,10 @@ struct swe_ctx {
   int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
   int n_patches = 0; size_t patch_smem = 0;
   void (*patch_kernel)(Control *, PatchArgs) = nullptr;
-  int64_t alg_bytes[4] = {0, 0, 0, 0};   // algorithmic DRAM bytes per launch of the kernels of one step
+  int64_t alg_bytes_v[3][4] = {};        // [variant][kernel]: algorithmic DRAM bytes per launch of the kernels of a step
+  bool auto_mode = false;                // AUTO with both variants available: chosen at swe_set_state (wet fraction)
   cudaGraph_t graph = nullptr;
-  cudaGraphExec_t graph_exec = nullptr;
+  cudaGraphExec_t graph_exec_v[3] = {nullptr, nullptr, nullptr};   // by variant
   int steps_per_graph = 0;
   int64_t launches = 0;
   double t_host = 0.0;               // t as of the last synchronisation
@@ -161,8 +162,10 @@ int capture_graph(swe_ctx *c) {
   SWE_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
   SWE_CUDA(c, cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
   for (int k = 0; k < c->steps_per_graph; ++k) enqueue_step(c, cap);
-  SWE_CUDA(c, cudaStreamEndCapture(cap, &c->graph));
-  SWE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+  cudaGraph_t g = nullptr;
+  SWE_CUDA(c, cudaStreamEndCapture(cap, &g));
+  SWE_CUDA(c, cudaGraphInstantiate(&c->graph_exec_v[c->variant], g, 0));
+  cudaGraphDestroy(g);
   SWE_CUDA(c, cudaStreamDestroy(cap));
   return SWE_OK;
 }
@@ -176,7 +179,7 @@ int read_control(swe_ctx *c) {   // device -> pinned host, synchronises the stre
 
 void release(swe_ctx *c) {
   if (!c) return;
-  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  for (auto &ge : c->graph_exec_v) if (ge) cudaGraphExecDestroy(ge);
   if (c->graph) cudaGraphDestroy(c->graph);
   for (double *p : c->d_params) if (p) cudaFree(p);
   if (c->d_ctl) cudaFree(c->d_ctl);
@@ -439,20 +442,22 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 8 * std::max<size_t>(1, flat.size())));
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
     // state in 32 + state out 32 + pce 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
-    c->alg_bytes[0] = 0;
-    c->alg_bytes[1] = 104 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;        // + q_c in and out per species
+    int64_t *ab = c->alg_bytes_v[SWE_VARIANT_PATCH];
+    ab[0] = 0;
+    ab[1] = 104 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;        // + q_c in and out per species
     pt.halo_ids = {}; pt.halo_area = {}; pt.pedge = {}; pt.pce = {}; pt.patch_nbr = {};   // host copies no longer needed
   }
-  if (c->variant != SWE_VARIANT_PATCH) {
+  {
     // EdgeGeom read + EdgeFlux written per edge, every CellRec gathered once
-    c->alg_bytes[0] = 0;
-    c->alg_bytes[1] = 64 * ne + 32 * nc;
+    int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
+    ab[0] = 0;
+    ab[1] = 64 * ne + 32 * nc;
     // cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
-    c->alg_bytes[2] = 1 * nc;                                      // k_theta_lazy: one flag byte per cell
+    ab[2] = 1 * nc;                                      // k_theta_lazy: one flag byte per cell
     // cell_edge, 1/area, g/k^2, theta read, CellRec read + written per cell; every EdgeGeom and EdgeFlux gathered once
-    c->alg_bytes[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
-    c->alg_bytes[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
-    c->alg_bytes[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
+    ab[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
+    ab[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
+    ab[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
   }
 
   // ---- control block
@@ -463,6 +468,15 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   h.ping_pong = (c->variant == SWE_VARIANT_PATCH) ? 1 : 0;
   SWE_CUDA(c, cudaMemcpy(c->d_ctl, &h, sizeof(Control), cudaMemcpyHostToDevice));
   *c->h_ctl = h;
+  // AUTO with a compact numbering: both variants stay available (their graphs are captured now) and swe_set_state
+  // picks one from the wet fraction of the state -- they compute bit-identical results
+  c->auto_mode = (p.variant == SWE_VARIANT_AUTO && c->variant == SWE_VARIANT_PATCH && !std::getenv("SWE_NO_AUTO_SWITCH"));
+  if (c->auto_mode) {
+    c->variant = SWE_VARIANT_THREE_PASS;
+    int rc = capture_graph(c);
+    c->variant = SWE_VARIANT_PATCH;
+    if (rc != SWE_OK) return rc;
+  }
   return capture_graph(c);
 }
 
@@ -550,6 +564,24 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     SWE_CUDA(c, cudaMemcpyAsync(c->stage + 2 * nc, hv, 8 * nc, cudaMemcpyHostToDevice, c->stream));
     dh = c->stage; dhu = c->stage + nc; dhv = c->stage + 2 * nc;
   }
+  if (c->auto_mode) {
+    // the fused patch step wins where part of the domain is dry (it skips dry patches), the three-pass step on
+    // (almost) all-wet states: count the wet cells of the new state and pick
+    k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, 0, 1);
+    k_count_wet<<<std::min(grid_for(nc), kInfoMaxBlocks), kBlock, 0, c->stream>>>(c->d_ctl, dh, (int)nc);
+    c->launches += 2;
+    int rc = read_control(c);
+    if (rc != SWE_OK) return rc;
+    const int want = (double)c->h_ctl->n_wet > 0.9 * (double)nc ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+    if (want != c->variant) {
+      if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
+        for (int sp = 0; sp < c->sc.n; ++sp)
+          SWE_CUDA(c, cudaMemcpyAsync(c->sc.qa[sp], c->sc.qb[sp], 8 * nc, cudaMemcpyDeviceToDevice, c->stream));
+      c->variant = want;
+    }
+    k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, want == SWE_VARIANT_PATCH ? 1 : 0, 0);
+    c->launches += 1;
+  }
   k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
   if (c->variant == SWE_VARIANT_PATCH) {
     k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
@@ -580,7 +612,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (K > 0 && remaining >= K) {
       int64_t n_graphs = remaining / K;
       if (finite_end) n_graphs = std::min(n_graphs, poll_every);
-      for (int64_t j = 0; j < n_graphs; ++j) SWE_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+      for (int64_t j = 0; j < n_graphs; ++j) SWE_CUDA(c, cudaGraphLaunch(c->graph_exec_v[c->variant], c->stream));
       batch_steps = n_graphs * K;
     } else {
       batch_steps = std::min<int64_t>(remaining, 64);   // tail shorter than a graph, or graphs switched off
@@ -800,7 +832,7 @@ const char *swe_step_kernel_name(const swe_ctx *c, int k) {
   return c->variant == SWE_VARIANT_PATCH ? kPatchNames[k] : kThreePassNames[k];
 }
 
-int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes[k] : 0; }
+int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes_v[c->variant][k] : 0; }
 
 int swe_get_patch_stats(swe_ctx *c, int64_t *out, int n_out) {
   if (!c || !out || n_out < 1) return SWE_EINVAL;

@@ -528,6 +528,24 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   }
 }
 
+// AUTO variant choice at swe_set_state: number of cells with h > h_dry in the caller's array
+__global__ void __launch_bounds__(kBlock)
+k_count_wet(Control *__restrict__ ctl, const double *__restrict__ h, int n_cells) {
+  long long wet = 0;
+  const double h_dry = ctl->h_dry;
+  for (int i = blockIdx.x * kBlock + threadIdx.x; i < n_cells; i += gridDim.x * kBlock) wet += (h[i] > h_dry);
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) wet += __shfl_xor_sync(0xffffffffu, wet, off);
+  if ((threadIdx.x & 31) == 0 && wet) atomicAdd((unsigned long long *)&ctl->n_wet, (unsigned long long)wet);
+}
+
+// switches the step variant (both compute bit-identical states): the three-pass step works in place in buffer a
+__global__ void k_set_variant(Control *ctl, int ping_pong, int zero_wet) {
+  if (zero_wet) { ctl->n_wet = 0; return; }
+  ctl->ping_pong = ping_pong;
+  if (!ping_pong) { ctl->cur = 0; ctl->src = 0; }
+}
+
 // start of an swe_step call: the stop conditions of this call
 __global__ void k_call_begin(Control *ctl, long long n_steps, double t_end, double cfl) {
   ctl->steps_left = n_steps;

@@ -93,13 +93,13 @@ def test_config5_8m_window_and_variants(gpu, ref):
     update path) stay bit-identical over 300 steps -- and the volume balance of the transmissive domain."""
     w = C.config5()
     assert 7.8e6 < w.n_cells < 8.2e6
-    s = gpu.from_workload(w)                                           # default variant, as bench.py runs it
-    assert s.patch_stats()["variant"] == gpu.VARIANT_PATCH
+    s = gpu.from_workload(w)                                           # AUTO, as bench.py runs it: all wet -> three-pass
+    assert s.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS
     o = ref.RefSolver(w)
     ig, io, _ = window(s, o, w, 10, "config5 8M, steps 0-10")
     check_info(ig, io)
     o.close()
-    t = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    t = gpu.from_workload(w, variant=gpu.VARIANT_PATCH)
     t.step(10, float("inf"), w.cfl, info=False)
     i1, i2 = s.step(300, float("inf"), w.cfl), t.step(300, float("inf"), w.cfl)
     assert i1 == i2 and i1["flags"] == 0 and i1["steps_done"] == 310

@@ -417,3 +417,35 @@ def test_dry_patches_are_skipped_and_rewetted(gpu, ref):
     s3.step(20, float("inf"), w3.cfl)
     assert s3.patch_stats()["patch_steps_skipped"] == 0
     s3.close()
+
+
+def test_auto_picks_the_variant_from_the_wet_fraction(gpu, ref):
+    """AUTO keeps both step variants ready and picks one at every swe_set_state: the fused patch step while part of
+    the domain is dry, the three-pass step on (almost) all-wet states.  Switching is invisible in the results."""
+    w4, w3 = CASES["config4-small"](), CASES["config3-small"]()
+    a = gpu.from_workload(w4, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_step_control", "k_patch_step"]
+    b = gpu.from_workload(w3, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    assert b.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS and len(b.step_kernels()) == 4
+    # odd number of steps (the patch step ping-pongs), then flood the river reach: AUTO switches to three-pass
+    o = ref.RefSolver(w4)
+    a.step(33, float("inf"), w4.cfl)
+    o.step(33, float("inf"), w4.cfl)
+    assert_state_close(a.get_state(), o.get_state(), "river, patch step")
+    h, hu, hv = a.get_state()
+    h2 = h + 0.5
+    a.set_state(h2, hu, hv, t0=1.0)
+    o.set_state(h2, hu, hv, t0=1.0)
+    assert a.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS
+    ia, io = a.step(40, float("inf"), w4.cfl), o.step(40, float("inf"), w4.cfl)
+    assert_state_close(a.get_state(), o.get_state(), "flooded river, three-pass step")
+    check_info(ia, io)
+    # and back: the original state again -> patch step
+    a.set_state(w4.h, w4.hu, w4.hv, t0=0.0)
+    o.set_state(w4.h, w4.hu, w4.hv, t0=0.0)
+    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH
+    ia, io = a.step(25, float("inf"), w4.cfl), o.step(25, float("inf"), w4.cfl)
+    assert_state_close(a.get_state(), o.get_state(), "river again, patch step")
+    check_info(ia, io)
+    a.close()
+    b.close()
