@@ -383,7 +383,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->err = "unknown variant"; return SWE_EINVAL;
   }
   if (c->variant == SWE_VARIANT_PATCH) {
-    const int pc = p.patch_cells > 0 ? p.patch_cells : 384;   // 384 cells, 3 blocks/SM: fastest in the round-1 sweep
+    // default: 384 cells (3 blocks/SM: fastest in the round-1 sweep); small meshes get smaller patches, so that the
+    // launch-latency-bound step still spreads over ~256 blocks (4k cells: 9.3 us/step at 64 cells vs 14.5 at 384)
+    int pc = p.patch_cells > 0 ? p.patch_cells : 384;
+    if (p.patch_cells <= 0 && nc < 256 * 384) pc = std::max<int>(64, (int)((nc / 256 + 31) / 32 * 32));
     if (pc < 32 || pc > 8192) { c->err = "patch_cells must be in [32, 8192]"; return SWE_EINVAL; }
     std::vector<int32_t> string_pos(ne, -1);
     for (size_t j = 0; j < flat.size(); ++j) string_pos[flat[j]] = (int32_t)j;
