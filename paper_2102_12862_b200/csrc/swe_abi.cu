@@ -426,7 +426,18 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       c->patch_kernel = min_blocks <= 2 ? k_patch_step<kPatchThreads, 2, 0, 0, 0, 0> : min_blocks == 3 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0>
                       : k_patch_step<kPatchThreads, 4, 0, 0, 0, 0>;
     }
-    SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->patch_smem));
+    // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
+    // context with smaller patches cannot lower it under an earlier context's launches
+    {
+      int dev = 0, optin = 0;
+      cudaFuncAttributes fa{};
+      SWE_CUDA(c, cudaGetDevice(&dev));
+      SWE_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+      SWE_CUDA(c, cudaFuncGetAttributes(&fa, c->patch_kernel));
+      const int limit = optin - (int)fa.sharedSizeBytes;
+      if ((int)c->patch_smem > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
+      SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
+    }
     auto dup = [&](void **dst, const void *src, size_t bytes) {
       cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
       if (e == cudaSuccess && bytes) e = cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
