@@ -209,6 +209,28 @@ void release(swe_ctx *c) {
   delete c;
 }
 
+// AUTO: makes `want` the active variant for the state as it is now (no step in flight).  cur = Control::cur as last
+// read.  The three-pass step works in place in buffer a; the patch step ping-pongs and needs its dry flags.
+int switch_variant(swe_ctx *c, int want, int cur) {
+  if (want == c->variant) return SWE_OK;
+  const int64_t nc = c->nc;
+  if (want == SWE_VARIANT_THREE_PASS && cur == 1) {
+    SWE_CUDA(c, cudaMemcpyAsync(c->rec, c->rec_b, sizeof(CellRec) * nc, cudaMemcpyDeviceToDevice, c->stream));
+    for (int sp = 0; sp < c->sc.n; ++sp)
+      SWE_CUDA(c, cudaMemcpyAsync(c->sc.qa[sp], c->sc.qb[sp], 8 * nc, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  c->variant = want;
+  k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, want == SWE_VARIANT_PATCH ? 1 : 0, 0);
+  c->launches += 1;
+  if (want == SWE_VARIANT_PATCH) {
+    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
+                                                                             c->d_dry + c->n_patches, c->sc);
+    c->launches += 1;
+  }
+  SWE_CUDA(c, cudaGetLastError());
+  return SWE_OK;
+}
+
 int upload_strings(swe_ctx *c) {
   if (c->strings.empty()) return SWE_OK;
   SWE_CUDA(c, cudaMemcpyAsync(c->d_strings, c->strings.data(), sizeof(BoundaryString) * c->strings.size(),
@@ -657,6 +679,12 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     info->vol = h.vol; info->vol_clipped = h.vol_clipped; info->vol_in = h.vol_in; info->vol_out = h.vol_out;
     info->flags = h.flags | (h.nonfinite ? SWE_FLAG_NONFINITE : 0);
     if (h.nonfinite) { c->err = "non-finite state value"; return SWE_ENONFINITE; }
+    if (c->auto_mode) {   // the wet count is known here: follow a flood that spreads (or recedes), with hysteresis
+      const double wet = (double)h.n_wet / (double)c->nc;
+      const int want = wet > 0.92 ? SWE_VARIANT_THREE_PASS : (wet < 0.85 ? SWE_VARIANT_PATCH : c->variant);
+      rc = switch_variant(c, want, h.cur);
+      if (rc != SWE_OK) return rc;
+    }
   } else if (!finite_end) {
     c->t_host = -std::numeric_limits<double>::infinity();   // unknown until the next read; never blocks stepping
   }
