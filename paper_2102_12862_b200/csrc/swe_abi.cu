@@ -105,6 +105,7 @@ namespace {
 
 // the kernels of one time step, in stream order; ev (nullable) = n_step_kernels + 1 events recorded around them
 constexpr int kMaxStepKernels = 4;
+constexpr int kEdgesPerThread = 1;      // 2 (two gather chains in flight per thread) needs 80 registers: measured slower
 constexpr int kPatchThreads = 256;
 const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"};
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
@@ -138,10 +139,10 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     return;
   }
   if (c->sc.n > 0)
-    k_edge_flux<true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+    k_edge_flux<true, 1><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                          c->area, c->d_drain_flag);
   else
-    k_edge_flux<false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+    k_edge_flux<false, kEdgesPerThread><<<grid_for((c->ne + kEdgesPerThread - 1) / kEdgesPerThread), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                           c->area, c->d_drain_flag);
   if (ev) cudaEventRecord(ev[2], s);
   k_theta_lazy<<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
@@ -795,7 +796,7 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
-    k_edge_flux<false><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{}, c->area, nullptr);
+    k_edge_flux<false, 1><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{}, c->area, nullptr);
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }

@@ -135,22 +135,15 @@ __device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const Boun
 // (one sector each), writes one EdgeFlux record (coalesced 256-bit).
 // ---------------------------------------------------------------------------------------------------------
 template <bool kScalars>
-__global__ void __launch_bounds__(kBlock)
-k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
-            const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
-            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,
-            const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
-  if (!ctl->active && !force) return;
-  const int e = blockIdx.x * kBlock + threadIdx.x;
-  if (e >= n_edges) return;
-  const double g = ctl->g, h_dry = ctl->h_dry;
-  const EdgeGeom eg = geom[e];
-  const CellRec a = rec[eg.L];
+__device__ __forceinline__ void
+edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, const EdgeGeom &eg, const CellRec &a,
+             const CellRec &b, const CellRec *__restrict__ rec, const double *__restrict__ kst,
+             const BoundaryString *__restrict__ strings, EdgeFlux *__restrict__ flux, const Scalars &sc,
+             const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
   double uL = 0.0, vL = 0.0;
   if (a.h > h_dry) { uL = a.qx / a.h; vL = a.qy / a.h; }   // R-8: thin films carry no momentum
   EdgeFlux o;
   if (eg.R >= 0) {
-    const CellRec b = rec[eg.R];
     double uR = 0.0, vR = 0.0;
     if (b.h > h_dry) { uR = b.qx / b.h; vR = b.qy / b.h; }
     const double unL = uL * eg.nx + vL * eg.ny, utL = vL * eg.nx - uL * eg.ny;
@@ -167,7 +160,7 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
   if (drain_flag) {
     const int d = o.F1 > 0.0 ? eg.L : ((o.F1 < 0.0 && eg.R >= 0) ? eg.R : -1);
     if (d >= 0) {
-      const double hd = (d == eg.L) ? a.h : rec[d].h;
+      const double hd = (d == eg.L) ? a.h : b.h;
       if (ctl->dt * (eg.len * fabs(o.F1)) > 0.3 * (hd * area[d])) drain_flag[d] = 1;
     }
   }
@@ -177,13 +170,42 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     const double phiL = a.h > 0.0 ? sc.qa[sp][eg.L] / a.h : 0.0;
     double phiR = phiL;
     if (eg.R >= 0) {
-      const double hR = rec[eg.R].h;
-      phiR = hR > 0.0 ? sc.qa[sp][eg.R] / hR : 0.0;
+      phiR = b.h > 0.0 ? sc.qa[sp][eg.R] / b.h : 0.0;
     } else if (eg.R <= -3 && (-3 - eg.R) < ctl->n_strings && strings[-3 - eg.R].type == kBcInflowQ) {
       phiR = strings[-3 - eg.R].phi_in[sp];
     }
     sc.phi_up[sp][e] = o.F1 >= 0.0 ? phiL : phiR;
   }
+}
+
+// kPerThread edges per thread (block b: edges [b * kBlock * kPerThread, ...), strided by kBlock so that every load
+// is coalesced): the geometry records of all of them are loaded first, then all their cell records, so that
+// kPerThread independent gather chains are in flight per thread (the kernel is bound by the latency of
+// geom -> cell record, profiles/r1f).
+template <bool kScalars, int kPerThread>
+__global__ void __launch_bounds__(kBlock)
+k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
+            const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
+            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,
+            const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
+  if (!ctl->active && !force) return;
+  const double g = ctl->g, h_dry = ctl->h_dry;
+  const int e0 = blockIdx.x * (kBlock * kPerThread) + threadIdx.x;
+  EdgeGeom eg[kPerThread];
+  CellRec a[kPerThread], b[kPerThread];
+#pragma unroll
+  for (int j = 0; j < kPerThread; ++j)
+    if (e0 + j * kBlock < n_edges) eg[j] = geom[e0 + j * kBlock];
+#pragma unroll
+  for (int j = 0; j < kPerThread; ++j)
+    if (e0 + j * kBlock < n_edges) {
+      a[j] = rec[eg[j].L];
+      if (eg[j].R >= 0) b[j] = rec[eg[j].R];
+    }
+#pragma unroll
+  for (int j = 0; j < kPerThread; ++j)
+    if (e0 + j * kBlock < n_edges)
+      edge_process<kScalars>(ctl, g, h_dry, e0 + j * kBlock, eg[j], a[j], b[j], rec, kst, strings, flux, sc, area, drain_flag);
 }
 
 // ---------------------------------------------------------------------------------------------------------
