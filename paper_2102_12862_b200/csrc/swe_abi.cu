@@ -76,6 +76,8 @@ struct swe_ctx {
   PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
   PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
+  int cell_grid = 148 * 4;           // resident blocks of the persistent k_cell_update
+  int edge_grid = 148 * 5;           // resident blocks of the persistent k_edge_flux (set from the occupancy API)
   uint8_t *d_drain_flag = nullptr;   // three-pass step: cells flagged as possible drainers (lazy theta)
   Scalars sc{};                      // passive scalars: device arrays owned by the library (cudaMalloc)
   double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
@@ -105,7 +107,7 @@ namespace {
 
 // the kernels of one time step, in stream order; ev (nullable) = n_step_kernels + 1 events recorded around them
 constexpr int kMaxStepKernels = 4;
-constexpr int kEdgesPerThread = 1;      // 2 (two gather chains in flight per thread) needs 80 registers: measured slower
+// (two edges per thread, i.e. two gather chains in flight, needs 80 registers: measured slower)
 constexpr int kPatchThreads = 256;
 const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"};
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
@@ -139,20 +141,20 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     return;
   }
   if (c->sc.n > 0)
-    k_edge_flux<true, 1><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+    k_edge_flux<true, false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                          c->area, c->d_drain_flag);
   else
-    k_edge_flux<false, kEdgesPerThread><<<grid_for((c->ne + kEdgesPerThread - 1) / kEdgesPerThread), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+    k_edge_flux<false, true><<<std::min(grid_for(c->ne), c->edge_grid), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                           c->area, c->d_drain_flag);
   if (ev) cudaEventRecord(ev[2], s);
   k_theta_lazy<<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                                   c->d_drain_flag, (int)c->nc);
   if (ev) cudaEventRecord(ev[3], s);
   if (c->sc.n > 0)
-    k_cell_update<true><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+    k_cell_update<true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
                                                            c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   else
-    k_cell_update<false><<<grid_for(c->nc), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+    k_cell_update<false><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
                                                             c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   if (ev) cudaEventRecord(ev[4], s);
 }
@@ -387,6 +389,17 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
 
   SWE_CUDA(c, cudaMalloc((void **)&c->d_drain_flag, (size_t)nc + 16));           // read four bytes at a time
   SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, (size_t)nc + 16));
+  {
+    int dev = 0, sms = 148, per_sm = 4;
+    SWE_CUDA(c, cudaGetDevice(&dev));
+    SWE_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_edge_flux<false, true>, kBlock, 0));
+    c->edge_grid = std::max(1, sms * per_sm);
+    if (c->sc.n > 0) SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<true>, kBlock, 0));
+    else SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false>, kBlock, 0));
+    c->cell_grid = std::max(1, sms * per_sm);
+    if (const char *e = std::getenv("SWE_EDGE_GRID_MULT")) c->edge_grid *= std::max(1, std::atoi(e));   // tuning only
+  }
   // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
   c->sc.n = p.n_species;
@@ -796,7 +809,7 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
-    k_edge_flux<false, 1><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{}, c->area, nullptr);
+    k_edge_flux<false, false><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{}, c->area, nullptr);
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }

@@ -178,11 +178,11 @@ edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, con
   }
 }
 
-// kPerThread edges per thread (block b: edges [b * kBlock * kPerThread, ...), strided by kBlock so that every load
-// is coalesced): the geometry records of all of them are loaded first, then all their cell records, so that
-// kPerThread independent gather chains are in flight per thread (the kernel is bound by the latency of
-// geom -> cell record, profiles/r1f).
-template <bool kScalars, int kPerThread>
+// kPersistent = false: one edge per thread.  kPersistent = true: a grid of resident blocks strides over the edges and
+// the (streamed) geometry record of a thread's next edge is loaded while the current edge is worked on, so that the
+// geom -> cell record gather chain of an edge pays one memory latency instead of two (profiles/r1f: the kernel's
+// stalls are exactly these two loads).
+template <bool kScalars, bool kPersistent>
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
@@ -190,22 +190,26 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
             const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
   if (!ctl->active && !force) return;
   const double g = ctl->g, h_dry = ctl->h_dry;
-  const int e0 = blockIdx.x * (kBlock * kPerThread) + threadIdx.x;
-  EdgeGeom eg[kPerThread];
-  CellRec a[kPerThread], b[kPerThread];
-#pragma unroll
-  for (int j = 0; j < kPerThread; ++j)
-    if (e0 + j * kBlock < n_edges) eg[j] = geom[e0 + j * kBlock];
-#pragma unroll
-  for (int j = 0; j < kPerThread; ++j)
-    if (e0 + j * kBlock < n_edges) {
-      a[j] = rec[eg[j].L];
-      if (eg[j].R >= 0) b[j] = rec[eg[j].R];
-    }
-#pragma unroll
-  for (int j = 0; j < kPerThread; ++j)
-    if (e0 + j * kBlock < n_edges)
-      edge_process<kScalars>(ctl, g, h_dry, e0 + j * kBlock, eg[j], a[j], b[j], rec, kst, strings, flux, sc, area, drain_flag);
+  int e = blockIdx.x * kBlock + threadIdx.x;
+  if (e >= n_edges) return;
+  if (!kPersistent) {
+    const EdgeGeom eg = geom[e];
+    const CellRec a = rec[eg.L];
+    CellRec b = a;
+    if (eg.R >= 0) b = rec[eg.R];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
+    return;
+  }
+  const int stride = gridDim.x * kBlock;
+  EdgeGeom eg_next = geom[e];
+  for (; e < n_edges; e += stride) {
+    const EdgeGeom eg = eg_next;
+    const CellRec a = rec[eg.L];
+    CellRec b = a;
+    if (eg.R >= 0) b = rec[eg.R];
+    if (e + stride < n_edges) eg_next = geom[e + stride];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -332,11 +336,17 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
               const double *__restrict__ area, const double *__restrict__ inv_area,
               const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells, const Scalars sc) {
   if (!ctl->active) return;
-  const int i = blockIdx.x * kBlock + threadIdx.x;
+  // a grid of resident blocks strides over the cells; the (streamed) slot record of a thread's next cell is loaded
+  // while the current cell is worked on: its cell_edge -> (geometry, flux) gather chain pays one latency, not two
   double rate = 0.0;
-  if (i < n_cells) {
-    const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
-    const int4 ce = cell_edge[i];
+  const int stride = gridDim.x * kBlock;
+  int i = blockIdx.x * kBlock + threadIdx.x;
+  int4 ce_next = make_int4(0, 0, 0, 0);
+  if (i < n_cells) ce_next = cell_edge[i];
+  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+  for (; i < n_cells; i += stride) {
+    const int4 ce = ce_next;
+    if (i + stride < n_cells) ce_next = cell_edge[i + stride];
     const int es[3] = {ce.x, ce.y, ce.z};
     double nx[3], ny[3], len[3];
     double dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3];
@@ -381,7 +391,8 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
         qxn = qxn / D;
         qyn = qyn / D;
       }
-      rate = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
+      const double r = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
+      if (r > rate) rate = r;
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
     rec[i] = c;
