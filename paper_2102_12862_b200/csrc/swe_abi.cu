@@ -622,7 +622,8 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     c->launches += 2;
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
-    const int want = (double)c->h_ctl->n_wet > 0.9 * (double)nc ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+    // measured crossover on the river reach filled to different stages: ~52 % wet cells (profiles/r1i_auto_threshold.md)
+    const int want = (double)c->h_ctl->n_wet > 0.5 * (double)nc ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
       if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
         for (int sp = 0; sp < c->sc.n; ++sp)
@@ -695,7 +696,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (h.nonfinite) { c->err = "non-finite state value"; return SWE_ENONFINITE; }
     if (c->auto_mode) {   // the wet count is known here: follow a flood that spreads (or recedes), with hysteresis
       const double wet = (double)h.n_wet / (double)c->nc;
-      const int want = wet > 0.92 ? SWE_VARIANT_THREE_PASS : (wet < 0.85 ? SWE_VARIANT_PATCH : c->variant);
+      const int want = wet > 0.55 ? SWE_VARIANT_THREE_PASS : (wet < 0.45 ? SWE_VARIANT_PATCH : c->variant);
       rc = switch_variant(c, want, h.cur);
       if (rc != SWE_OK) return rc;
     }

@@ -454,11 +454,11 @@ def test_auto_picks_the_variant_from_the_wet_fraction(gpu, ref):
 def test_auto_follows_a_spreading_flood(gpu, ref):
     """AUTO re-evaluates its choice whenever swe_step returns info: a dam break that wets the whole (short) channel
     starts on the patch step and ends on the three-pass step, with the state equal to the oracle's throughout."""
-    w = C.dam_break_channel(nx=120, ny=4, lx=24.0, ly=0.8, x_dam=14.0, t_end=20.0)
+    w = C.dam_break_channel(nx=120, ny=4, lx=24.0, ly=0.8, x_dam=8.0, t_end=20.0)
     s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, patch_cells=0)
     o = ref.RefSolver(w)
     seen = [s.patch_stats()["variant"]]
-    for _ in range(12):
+    for _ in range(16):
         ig, io = s.step(35, float("inf"), w.cfl), o.step(35, float("inf"), w.cfl)     # odd chunks: the patch step ping-pongs
         assert_state_close(s.get_state(), o.get_state(), f"after {io['steps_done']} steps")
         check_info(ig, io)

@@ -223,7 +223,7 @@ def river_section(d):
                     np.where(d < 26.0, -3.0 + (d - 20.0) / 2.0, 2.0 * (d - 26.0) / (350.0 - 26.0)))
 
 
-def config4(target_cells=4_000_000, n_steps=5000, length=10000.0) -> Workload:
+def config4(target_cells=4_000_000, n_steps=5000, length=10000.0, stage=-2.0) -> Workload:
     """BASELINE.json configs[3]: river reach flood wave with wetting/drying. length x 500 m,
     centreline y = 100 sin(2 pi x / 1500), mesh 3x finer for d < 40 m (20 m graded transition),
     slope 0.001, fractal bed noise sigma 0.1 m, k = 25 (channel) / 15 (floodplain), channel 1 m deep
@@ -282,7 +282,7 @@ def config4(target_cells=4_000_000, n_steps=5000, length=10000.0) -> Workload:
     ctr = M.centroids(node_xy, tri)
     dc = np.abs(ctr[:, 1] - yc(ctr[:, 0]))
     kst = np.where(dc < 26.0, 25.0, 15.0)
-    h = np.maximum(0.0, (-0.001 * ctr[:, 0] - 2.0) - zb)
+    h = np.maximum(0.0, (-0.001 * ctr[:, 0] + stage) - zb)     # stage = -2: 1 m over the channel bottom (the config)
     w = _finish(f"config4-river-reach-{n}", node_xy, tri, zb, kst, h, n_steps=n_steps, dt_max=10.0)
     _set_boundary_codes(w, lambda mx, my: np.where(mx < 1e-9, M.bc_string(0),
                                                    np.where(mx > length - 1e-9, M.bc_string(1), M.BC_WALL)))
