@@ -159,6 +159,13 @@ int swe_get_tables(swe_ctx *ctx, int64_t *n_edges, int32_t *edge_cell, int32_t *
 /* y[i] = cube root of x[i] rounded to nearest, evaluated on the device by the function the kernels use (R-14);
  * x, y: HOST pointers [n]; uses the current device and the legacy default stream; needs no context */
 int swe_device_cbrt(const double *x, double *y, int64_t n);
+/* The HOST part of swe_create alone (no CUDA call, works without a GPU): validation, edge tables, geometry,
+ * renumbering and -- when patch_cells > 0 -- the patch tables of the fused step.  out[0..9] = edges, patches, sum of
+ * local cells, sum of local edges, largest local cell count, largest local edge count, shared memory per block
+ * [bytes], sum of own cells, distinct own cells, entries of the patch-neighbour lists.  cell_perm / edge_perm (may be
+ * NULL): internal -> caller numbering.  Returns the same error codes as swe_create (swe_last_error(NULL)). */
+int swe_host_preprocess(const swe_mesh *mesh, int renumber, int patch_cells, int64_t *out, int n_out,
+                        int32_t *cell_perm, int32_t *edge_perm);
 /* number of kernel launches enqueued by this context since swe_create (graph nodes count individually) */
 int64_t swe_kernel_launches(const swe_ctx *ctx);
 /* Measurement (bench.py roofline): advances n_steps >= 1 time steps with plain launches, every kernel of the step

@@ -37,7 +37,7 @@ EXPORTS = (
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
     "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_get_patch_stats",
-    "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar",
+    "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar", "swe_host_preprocess",
 )
 
 
@@ -108,6 +108,7 @@ def lib():
         L.swe_algorithmic_bytes.argtypes = [C.c_void_p, C.c_int]
         L.swe_algorithmic_bytes.restype = C.c_int64
         L.swe_get_patch_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int]
+        L.swe_host_preprocess.argtypes = [C.POINTER(SweMesh), C.c_int, C.c_int, C.POINTER(C.c_int64), C.c_int, _i32p, _i32p]
         L.swe_set_scalars.argtypes = [C.c_void_p, C.c_void_p]
         L.swe_get_scalars.argtypes = [C.c_void_p, C.c_void_p]
         L.swe_set_boundary_scalar.argtypes = [C.c_void_p, C.c_int, _f64p, C.c_int]
@@ -300,6 +301,31 @@ class Solver:
     @property
     def kernel_launches(self):
         return int(lib().swe_kernel_launches(self._h))
+
+
+def host_preprocess(node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, renumber=RENUMBER_MORTON,
+                    patch_cells=384):
+    """swe_host_preprocess: the host part of swe_create (validation, tables, geometry, renumbering, patch tables).
+    Needs no GPU.  Returns (stats dict, cell_perm, edge_perm); raises SweError for an invalid mesh."""
+    node_xy = np.ascontiguousarray(node_xy, np.float64)
+    tri = np.ascontiguousarray(tri, np.int32)
+    n = int(tri.shape[0])
+    ec = None if edge_cell is None else np.ascontiguousarray(edge_cell, np.int32)
+    ce = None if cell_edge is None else np.ascontiguousarray(cell_edge, np.int32)
+    zb = np.ascontiguousarray(zb if zb is not None else np.zeros(n), np.float64)
+    kst = np.ascontiguousarray(kst if kst is not None else np.full(n, np.inf), np.float64)
+    mesh = SweMesh(int(node_xy.shape[0]), n, 0 if ec is None else int(ec.shape[0]), _p(node_xy, _f64p), _p(tri, _i32p),
+                   _p(ec, _i32p), _p(ce, _i32p), _p(zb, _f64p), _p(kst, _f64p))
+    out = (C.c_int64 * 10)()
+    cp = np.empty(n, np.int32)
+    ep = np.empty(3 * n, np.int32)
+    rc = lib().swe_host_preprocess(C.byref(mesh), int(renumber), int(patch_cells), out, 10, _p(cp, _i32p), _p(ep, _i32p))
+    if rc != OK:
+        raise SweError(rc, lib().swe_last_error(None).decode())
+    keys = ("n_edges", "patches", "sum_local_cells", "sum_local_edges", "max_local_cells", "max_local_edges",
+            "smem_bytes", "sum_own_cells", "distinct_own_cells", "patch_neighbour_entries")
+    st = dict(zip(keys, (int(v) for v in out)))
+    return st, cp, ep[:st["n_edges"]]
 
 
 def workspace_bytes(n_cells, n_edges=0):

@@ -257,6 +257,48 @@ k_string_lengths(BoundaryString *strings, int n_strings, const int *__restrict__
   }
 }
 
+// Host part of swe_create: edge tables (given or built), validation + geometry of section 4.1, renumbering.
+int host_prepare(const swe_mesh *mesh, int renumber_mode, HostMesh &hm, std::string &err) {
+  const int64_t nc = mesh->n_cells, nn = mesh->n_nodes;
+  hm.nc = nc; hm.nn = nn;
+  if (mesh->edge_cell && mesh->cell_edge) {
+    if (mesh->n_edges <= 0 || mesh->n_edges > 3 * nc) { err = "n_edges out of range"; return SWE_EINVAL; }
+    hm.ne = mesh->n_edges;
+    hm.edge_cell.assign(mesh->edge_cell, mesh->edge_cell + 2 * hm.ne);
+    hm.cell_edge.assign(mesh->cell_edge, mesh->cell_edge + 3 * nc);
+  } else if (!mesh->edge_cell && !mesh->cell_edge) {
+    if (!build_tables(nc, nn, mesh->tri, hm, err)) return SWE_EMESH;
+  } else {
+    err = "edge_cell and cell_edge must be given together or both be NULL";
+    return SWE_EINVAL;
+  }
+  if (!validate_and_measure(nc, nn, mesh->node_xy, mesh->tri, hm, err)) return SWE_EMESH;
+  for (int64_t i = 0; i < nc; ++i) {
+    const double k = mesh->kst[i];
+    if (!(k > 0.0) || !std::isfinite(mesh->zb[i])) { err = "cell " + std::to_string(i) + ": kst must be > 0 (or +inf), zb finite"; return SWE_EINVAL; }
+  }
+  if (renumber_mode < 0 || renumber_mode > 2) { err = "unknown renumbering"; return SWE_EINVAL; }
+  renumber(renumber_mode, nc, mesh->node_xy, mesh->tri, hm);
+  return SWE_OK;
+}
+
+// internal-numbering edge geometry and slot table, as uploaded by swe_create
+void internal_tables(const HostMesh &hm, std::vector<EdgeGeom> &geom, std::vector<int32_t> &ce4, std::vector<double> &area) {
+  const int64_t nc = hm.nc, ne = hm.ne;
+  geom.resize(ne); ce4.resize((size_t)4 * nc); area.resize(nc);
+  for (int64_t i = 0; i < nc; ++i) {
+    const int32_t o = hm.cell_perm[i];
+    for (int k = 0; k < 3; ++k) ce4[4 * i + k] = hm.edge_new[hm.cell_edge[3 * o + k]];
+    ce4[4 * i + 3] = 0;
+    area[i] = hm.area[o];
+  }
+  for (int64_t e = 0; e < ne; ++e) {
+    const int32_t o = hm.edge_perm[e];
+    const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
+    geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
+  }
+}
+
 int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   const int64_t nc = mesh->n_cells, nn = mesh->n_nodes;
   c->nc = nc;
@@ -268,24 +310,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
 
   // ---- tables, validation, geometry, numbering (host)
   HostMesh &hm = c->hm;
-  hm.nc = nc; hm.nn = nn;
-  if (mesh->edge_cell && mesh->cell_edge) {
-    if (mesh->n_edges <= 0 || mesh->n_edges > 3 * nc) { c->err = "n_edges out of range"; return SWE_EINVAL; }
-    hm.ne = mesh->n_edges;
-    hm.edge_cell.assign(mesh->edge_cell, mesh->edge_cell + 2 * hm.ne);
-    hm.cell_edge.assign(mesh->cell_edge, mesh->cell_edge + 3 * nc);
-  } else if (!mesh->edge_cell && !mesh->cell_edge) {
-    if (!build_tables(nc, nn, mesh->tri, hm, c->err)) return SWE_EMESH;
-  } else {
-    c->err = "edge_cell and cell_edge must be given together or both be NULL";
-    return SWE_EINVAL;
+  {
+    int rc = host_prepare(mesh, p.renumber, hm, c->err);
+    if (rc != SWE_OK) return rc;
   }
-  if (!validate_and_measure(nc, nn, mesh->node_xy, mesh->tri, hm, c->err)) return SWE_EMESH;
-  for (int64_t i = 0; i < nc; ++i) {
-    const double k = mesh->kst[i];
-    if (!(k > 0.0) || !std::isfinite(mesh->zb[i])) { c->err = "cell " + std::to_string(i) + ": kst must be > 0 (or +inf), zb finite"; return SWE_EINVAL; }
-  }
-  renumber(p.renumber, nc, mesh->node_xy, mesh->tri, hm);
   const int64_t ne = c->ne = hm.ne;
 
   // ---- workspace
@@ -881,6 +909,45 @@ int swe_device_cbrt(const double *x, double *y, int64_t n) {
 }
 
 int64_t swe_kernel_launches(const swe_ctx *c) { return c ? c->launches : 0; }
+
+int swe_host_preprocess(const swe_mesh *mesh, int renumber_mode, int patch_cells, int64_t *out, int n_out,
+                        int32_t *cell_perm, int32_t *edge_perm) {
+  if (!mesh || !mesh->node_xy || !mesh->tri || !mesh->zb || !mesh->kst || mesh->n_cells <= 0 || mesh->n_nodes <= 0) {
+    g_create_error = "null argument / empty mesh";
+    return SWE_EINVAL;
+  }
+  try {
+    HostMesh hm;
+    int rc = host_prepare(mesh, renumber_mode, hm, g_create_error);
+    if (rc != SWE_OK) return rc;
+    int64_t v[10] = {hm.ne, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    if (patch_cells > 0) {
+      std::vector<EdgeGeom> geom; std::vector<int32_t> ce4; std::vector<double> area;
+      internal_tables(hm, geom, ce4, area);
+      std::vector<int32_t> string_pos(hm.ne, -1);
+      int32_t n_string = 0;
+      for (int64_t e = 0; e < hm.ne; ++e) if (geom[e].R <= -3) string_pos[e] = n_string++;
+      PatchTables pt;
+      if (!build_patches(hm.nc, hm.ne, geom, ce4, area, string_pos, patch_cells, pt, g_create_error)) return SWE_EINVAL;
+      int64_t own = 0, covered = 0;
+      std::vector<uint8_t> seen(hm.nc, 0);
+      for (const PatchHeader &h : pt.hdr) {
+        own += h.n_own;
+        for (int32_t l = 0; l < h.n_own; ++l) if (!seen[h.cell0 + l]) { seen[h.cell0 + l] = 1; ++covered; }
+      }
+      v[1] = (int64_t)pt.hdr.size(); v[2] = pt.sum_loc; v[3] = pt.sum_e; v[4] = pt.max_loc; v[5] = pt.max_e;
+      v[6] = (int64_t)sizeof(double) * patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown).total;
+      v[7] = own; v[8] = covered; v[9] = (int64_t)pt.patch_nbr.size();
+    }
+    for (int k = 0; k < n_out && k < 10; ++k) out[k] = v[k];
+    if (cell_perm) std::memcpy(cell_perm, hm.cell_perm.data(), 4 * hm.nc);
+    if (edge_perm) std::memcpy(edge_perm, hm.edge_perm.data(), 4 * hm.ne);
+  } catch (const std::bad_alloc &) {
+    g_create_error = "out of host memory";
+    return SWE_ENOMEM;
+  }
+  return SWE_OK;
+}
 
 int swe_step_kernel_count(const swe_ctx *c) { return c ? n_step_kernels(c) : 0; }
 
