@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--patch-cells", type=int, default=0, help="cells per patch of the fused step (0 = default)")
     ap.add_argument("--renumber", type=int, default=1, help="SWE_RENUMBER_*: 0 input order, 1 Morton, 2 RCM")
     ap.add_argument("--shuffle-input", action="store_true", help="randomly renumber the input mesh first (A/B runs)")
+    ap.add_argument("--stage", type=float, default=None,
+                    help="config 4 only: initial water level relative to the sloped datum (default -2 = the configuration)")
     ap.add_argument("--species", type=int, default=0, help="passive scalar species advected with the flow (0..5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -73,9 +75,11 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def load_workload(config_id, scale, rank=0, world=1, barrier=None):
+def load_workload(config_id, scale, rank=0, world=1, barrier=None, stage=None):
     """Seeded synthetic workload; rank 0 generates, the others read its cache file (generation is ~50 s at 4M)."""
     from workloads import configs as C
+    if stage is not None and config_id == 4:
+        return C.config4(target_cells=int(4_000_000 * scale), length=10000.0 * scale, stage=stage)
     if world == 1:
         return C.by_id(config_id, scale)
     import pickle
@@ -252,7 +256,7 @@ def main():
         if world > 1:
             dist.barrier()
 
-    w = load_workload(args.config, args.scale, rank, world, barrier)
+    w = load_workload(args.config, args.scale, rank, world, barrier, stage=args.stage)
     if args.shuffle_input:
         w = w.permuted(12862)[0]
     N, E, T = w.n_cells, w.n_edges, args.time_steps
@@ -417,7 +421,7 @@ def main():
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
-                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "step_kernels": s_kernels, "patch": patch_stats},
+                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "stage": args.stage, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet, "other_variant": other,
