@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 # profiles/ (kernel name, n_cells) -> bytes; absent -> "traffic": null
 NCU_TRAFFIC_BYTES = {("k_cell_update", 3964806): 726.9e6, ("k_theta_lazy", 3964806): 4.0e6,
                      ("k_edge_flux", 3964806): 486.2e6,   # profiles/r1i_ncu_full_three_pass.md
-                     ("k_patch_step", 3964806): 407.8e6,  # profiles/r1c_ncu_full_patch_river.md (52 % of patches dry)
+                     ("k_patch_step", 3964806): 502.0e6,  # profiles/r1i_ncu_full_patch_river.md (52 % of patches dry)
                      ("k_patch_step", 3964136): 678.6e6}  # profiles/r1c_ncu_full_patch_allwet.md
 
 METRIC = "cell_updates_per_s"
