@@ -322,6 +322,10 @@ def main():
                     "step_algorithmic_bytes": sum(alg.values()),
                     "step_achieved": sum(alg.values()) / (ms * 1e-3 / (T * args.steps)) / 1e9,
                     "share_of_step": kernel_ms[top] / sum(kernel_ms.values())}
+        if top == "k_patch_step":
+            roofline["note"] = ("the fused patch step moves about a third of the bytes of the bandwidth-bound "
+                                "three-pass step (other_variant: its kernels and whole step against the same HBM "
+                                "peak) and is bound by fp64 issue / latency, not by HBM (DESIGN.md section 7)")
 
     # ---- end-to-end arm: the same K steps through the C-ABI with HOST (pinned) buffers, copies inside the region
     e2e = None

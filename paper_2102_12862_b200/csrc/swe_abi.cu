@@ -426,7 +426,6 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     if (c->sc.n > 0) SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<true>, kBlock, 0));
     else SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false>, kBlock, 0));
     c->cell_grid = std::max(1, sms * per_sm);
-    if (const char *e = std::getenv("SWE_EDGE_GRID_MULT")) c->edge_grid *= std::max(1, std::atoi(e));   // tuning only
   }
   // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
@@ -480,15 +479,12 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     if (c->sc.n > 0) {               // scalar module: run-time capacities (the concentrations enlarge the block)
       c->patch_kernel = c->patch_smem <= 75 * 1024 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0, true>
                                                    : k_patch_step<kPatchThreads, 2, 0, 0, 0, 0, true>;
-    } else if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown &&
-        !std::getenv("SWE_PATCH_DYNAMIC")) {
+    } else if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown) {
       c->patch_kernel = k_patch_step<kPatchThreads, 3, kCapLoc, kCapC1, kCapE, kCapEown>;
       c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown).total;
     } else {
-      int min_blocks = 3;
-      if (const char *e = std::getenv("SWE_PATCH_MINBLOCKS")) min_blocks = std::atoi(e);   // tuning experiments only
-      c->patch_kernel = min_blocks <= 2 ? k_patch_step<kPatchThreads, 2, 0, 0, 0, 0> : min_blocks == 3 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0>
-                      : k_patch_step<kPatchThreads, 4, 0, 0, 0, 0>;
+      // 3 blocks/SM while the patch fits 75 KB (the round-1 sweep: 2 blocks are slower, 4 need 64 registers and spill)
+      c->patch_kernel = c->patch_smem <= 75 * 1024 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0> : k_patch_step<kPatchThreads, 2, 0, 0, 0, 0>;
     }
     // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
     // context with smaller patches cannot lower it under an earlier context's launches
@@ -548,7 +544,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   *c->h_ctl = h;
   // AUTO with a compact numbering: both variants stay available (their graphs are captured now) and swe_set_state
   // picks one from the wet fraction of the state -- they compute bit-identical results
-  c->auto_mode = (p.variant == SWE_VARIANT_AUTO && c->variant == SWE_VARIANT_PATCH && !std::getenv("SWE_NO_AUTO_SWITCH"));
+  c->auto_mode = (p.variant == SWE_VARIANT_AUTO && c->variant == SWE_VARIANT_PATCH);
   if (c->auto_mode) {
     c->variant = SWE_VARIANT_THREE_PASS;
     int rc = capture_graph(c);
