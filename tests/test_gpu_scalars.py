@@ -139,3 +139,24 @@ def test_scalars_do_not_change_the_flow_and_api_errors(gpu):
     assert np.array_equal(b.get_scalars(), c.get_scalars())
     for s in (a, b, c):
         s.close()
+
+
+def test_auto_switches_variant_with_scalars_on_board(gpu, ref):
+    """AUTO moves from the patch step to the three-pass step while a dam break wets a short channel; the scalar
+    masses travel with the state through the switch (buffer b -> buffer a) and stay equal to the oracle's."""
+    w = C.dam_break_channel(nx=120, ny=4, lx=24.0, ly=0.8, x_dam=8.0, t_end=20.0)
+    x = M.centroids(w.node_xy, w.tri)[:, 0]
+    qc0 = np.stack([np.where(x < 4.0, 1.0, 0.0) * w.h, 0.25 * w.h])
+    s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, n_species=2)
+    o = ref.RefSolver(w)
+    s.set_scalars(qc0)
+    o.set_scalars(qc0)
+    seen = [s.patch_stats()["variant"]]
+    for _ in range(10):
+        ig, io = s.step(35, float("inf"), w.cfl), o.step(35, float("inf"), w.cfl)
+        assert_state_close(s.get_state(), o.get_state(), f"after {io['steps_done']} steps")
+        assert_scalars_close(s.get_scalars(), o.get_scalars(), f"after {io['steps_done']} steps")
+        check_info(ig, io)
+        seen.append(s.patch_stats()["variant"])
+    assert seen[0] == gpu.VARIANT_PATCH and seen[-1] == gpu.VARIANT_THREE_PASS, seen
+    s.close()
