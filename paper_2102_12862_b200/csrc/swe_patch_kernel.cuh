@@ -15,7 +15,7 @@
 namespace swe {
 
 struct PatchSmem {          // offsets (in doubles) into the dynamic shared memory; the same for every block
-  int h, u, v, z, theta, F1, len, F3, GL, GR, nx, ny, phi, total;
+  int h, u, v, z, theta, area, F1, len, F3, GL, GR, nx, ny, phi, total;
 };
 
 __host__ __device__ inline PatchSmem patch_smem_layout(int max_loc, int max_c1, int max_e, int max_eown,
@@ -24,6 +24,7 @@ __host__ __device__ inline PatchSmem patch_smem_layout(int max_loc, int max_c1, 
   int o = 0;
   s.h = o; o += max_loc; s.u = o; o += max_loc; s.v = o; o += max_loc; s.z = o; o += max_loc;
   s.theta = o; o += max_c1;
+  s.area = o; o += max_c1;                      // |Omega| of own and ring-1 cells (limiter)
   s.F1 = o; o += max_e; s.len = o; o += max_e;
   s.F3 = o; o += max_eown; s.GL = o; o += max_eown; s.GR = o; o += max_eown;
   s.nx = o; o += max_eown; s.ny = o; o += max_eown;
@@ -67,7 +68,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
   double *sh_phi = sm + S.phi;
   double *sh_h = sm + S.h, *sh_u = sm + S.u, *sh_v = sm + S.v, *sh_z = sm + S.z, *sh_th = sm + S.theta;
   double *sh_F1 = sm + S.F1, *sh_len = sm + S.len, *sh_F3 = sm + S.F3, *sh_GL = sm + S.GL, *sh_GR = sm + S.GR;
-  double *sh_nx = sm + S.nx, *sh_ny = sm + S.ny;
+  double *sh_nx = sm + S.nx, *sh_ny = sm + S.ny, *sh_area = sm + S.area;
 
   const PatchHeader H = A.hdr[blockIdx.x];
   const int src = ctl->src;
@@ -148,6 +149,7 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
           double u = 0.0, v = 0.0;
           if (c[j].h > h_dry) { u = c[j].qx / c[j].h; v = c[j].qy / c[j].h; }
           sh_h[l] = c[j].h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c[j].z;
+          if (l < n_c1) { sh_th[l] = 1.0; sh_area[l] = l < H.n_own ? A.area[gid[j]] : halo_area[l]; }
           water |= (c[j].h != 0.0);
           if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
             _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
@@ -173,9 +175,8 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
       return;
     }
   }
-  uint4 pc_next = make_uint4(0u, 0u, 0u, 0u);          // first record of phase 3 (and of phase 4: same cell)
-  double A_next = 0.0;
-  if (tid < n_c1) { pc_next = pce[tid]; A_next = tid < H.n_own ? A.area[H.cell0 + tid] : halo_area[tid]; }
+  uint4 pc_next = make_uint4(0u, 0u, 0u, 0u);          // slot record of this thread's first own cell (phase 4)
+  if (tid < H.n_own) pc_next = pce[tid];
 
   // ---- phase 2: edge fluxes
   for (int e = tid; e < n_e; e += kThreads) {
@@ -199,6 +200,10 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
     }
     sh_F1[e] = o.F1; sh_len[e] = pe.len;
     if (e < H.n_eown) { sh_F3[e] = o.F3; sh_GL[e] = o.GL; sh_GR[e] = o.GR; sh_nx[e] = pe.nx; sh_ny[e] = pe.ny; }
+    // S1c, lazily (R-8b; as in k_edge_flux): theta_i < 1 needs one outgoing edge with dt * o_k > 0.3 h_i |Omega_i|.  Only
+    // such donor cells are marked (theta = -1); phase 3 evaluates theta for them and every other cell keeps theta = 1.
+    const int d = o.F1 > 0.0 ? L : ((o.F1 < 0.0 && pe.R != 0xFFFF) ? (int)pe.R : n_c1);
+    if (d < n_c1 && dt * (pe.len * fabs(o.F1)) > 0.3 * (sh_h[d] * sh_area[d])) sh_th[d] = -1.0;
   }
   // first own cell of this thread in phase 4: its record and constants, in flight during phase 3
   const uint4 pc4_first = pc_next;
@@ -207,12 +212,11 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
   if (tid < H.n_own) { c4_next = in[H.cell0 + tid]; invA_next = A.inv_area[H.cell0 + tid]; gn2_next = A.gn2[H.cell0 + tid]; }
   __syncthreads();
 
-  // ---- phase 3 (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1)), slots in order
+  // ---- phase 3 (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1)), slots in order -- for the
+  // cells marked in phase 2 only
   for (int l = tid; l < n_c1; l += kThreads) {
-    const uint4 pc = pc_next;
-    const double Ai = A_next;
-    const int ln = l + kThreads;
-    if (ln < n_c1) { pc_next = pce[ln]; A_next = ln < H.n_own ? A.area[H.cell0 + ln] : halo_area[ln]; }
+    if (sh_th[l] >= 0.0) continue;
+    const uint4 pc = pce[l];
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
     double o[3];
 #pragma unroll
@@ -222,9 +226,9 @@ k_patch_step(Control *__restrict__ ctl, const PatchArgs A) {
       o[k] = dmax0(sM);
     }
     const double outflow = ((o[0] + o[1]) + o[2]);
-    const double avail = sh_h[l] * Ai;
+    const double avail = sh_h[l] * sh_area[l];
     double th = 1.0;
-    if (dt * outflow > avail) th = avail / (dt * outflow);       // rare: keep the division off the common path
+    if (dt * outflow > avail) th = avail / (dt * outflow);
     sh_th[l] = th;
   }
   __syncthreads();
