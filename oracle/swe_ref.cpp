@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstring>
 #include <limits>
 #include <map>
 #include <string>
@@ -41,6 +42,10 @@ struct swe_ref_ctx {
   int n_species = 0;
   std::vector<std::vector<double>> qc;  // [species][cell]
   std::vector<std::vector<double>> Ac;  // [species][edge] advective scalar flux of the most recent step
+  // morphodynamics (section 3.2 Eq. 3, section 4.3 Eq. 13-16; R-20): 0 = fixed bed
+  int morph_formula = 0;
+  double morph_alpha = 0.0, morph_theta_cr = 0.047, morph_s = 2.65, morph_dm = 1e-3, morph_p = 0.4;
+  std::vector<double> qB;               // per edge: normal sediment flux q_Bij of the most recent step
   std::map<int, BString> strings;
   double t = 0.0, dt_last = 0.0, vol_clipped = 0.0, vol_in = 0.0, vol_out = 0.0;
   int64_t steps_done = 0;
@@ -308,6 +313,70 @@ void boundary_flux(swe_ref_ctx *c, int64_t e) {
   (void)GR;
 }
 
+}  // namespace
+
+// ---- section 3.2.1 Table 2 + Eq. 16, R-20 ------------------------
+// One cell seen from one interface with unit normal (nx, ny): normal sediment flux q_B.n, the derivative
+// psi = d(q_B,n)/d(q_n) (q_n = h u_n; h and the tangential velocity held fixed) and the two speeds of Eq. 16.
+//   formula 1, Grass-like:  |q_B| = alpha |u|^3 (m = 3, u_cr = 0), along u
+//   formula 2, MPM-like:    |q_B| = alpha (theta - theta_cr)^1.5 sqrt((s-1) g d_m^3) for theta > theta_cr, along u, with the
+//                           Shields parameter theta = tau_B / (rho g (s-1) d_m) and the Strickler bed shear stress of
+//                           Table 1, tau_B / rho = g |u|^2 / (k_st^2 h^(1/3))   (gn2 = g / k_st^2)
+extern "C" void swe_ref_sediment_state(int formula, double alpha, double theta_cr, double sdens, double dm, double g,
+                                       double h, double u, double v, double gn2, double nx, double ny,
+                                       double *qBn, double *psi, double *lam1, double *lam2) {
+  const double un = u * nx + v * ny, ut = v * nx - u * ny;
+  const double sp2 = u * u + v * v;
+  double q = 0.0, ps = 0.0;
+  if (formula == 1) {
+    q = alpha * (sp2 * un);
+    ps = (alpha * (sp2 + 2.0 * (un * un))) / h;
+  } else if (formula == 2) {
+    const double th = (gn2 * sp2) / (swe_ref_cbrt(h) * (g * ((sdens - 1.0) * dm)));
+    const double x = th - theta_cr;
+    if (x > 0.0 && sp2 > 0.0) {
+      const double Gm = alpha * std::sqrt(((sdens - 1.0) * g) * (dm * (dm * dm)));
+      const double rx = std::sqrt(x), spd = std::sqrt(sp2);
+      q = (Gm * (x * rx)) * (un / spd);
+      ps = (Gm * (((3.0 * rx) * th) * (un * un) + (x * rx) * (ut * ut))) / ((sp2 * spd) * h);
+    }
+  }
+  const double cel = std::sqrt(g * h);
+  const double a = un - cel;
+  const double disc = std::sqrt(a * a + 4.0 * (ps * (cel * cel)));
+  *qBn = q; *psi = ps; *lam1 = 0.5 * (a - disc); *lam2 = 0.5 * (a + disc);
+}
+
+// Eq. 14-15: HLL-type sediment flux through the interface between cell i (left) and cell j (right)
+extern "C" double swe_ref_sediment_flux(double qBi, double l1i, double l2i, double zi,
+                                        double qBj, double l1j, double l2j, double zj) {
+  const double sm = std::fmin(l1i, l1j), sp = std::fmax(l2i, l2j);
+  if (!(sp - sm > 0.0)) return 0.0;
+  return ((sp * qBi - sm * qBj) + (sp * sm) * (zj - zi)) / (sp - sm);
+}
+
+namespace {
+
+// S1m: q_Bij of every edge from the state at t^n (synchronous-decoupled).  R-20: no transport where a
+// cell is dry (h <= h_dry), so an interface with a dry side carries none; walls carry none; through every open
+// boundary the interior cell's own flux leaves or enters (equilibrium boundary: q_Bij = q_Bi . n).
+void sediment_fluxes(swe_ref_ctx *c) {
+  for (int64_t e = 0; e < c->ne; ++e) {
+    const int64_t L = c->eL[e], R = c->eR[e];
+    c->qB[e] = 0.0;
+    if (!is_wet(c, L) || R == -1) continue;
+    double qi, psi, l1i, l2i;
+    swe_ref_sediment_state(c->morph_formula, c->morph_alpha, c->morph_theta_cr, c->morph_s, c->morph_dm, c->g, c->h[L],
+                           c->qx[L] / c->h[L], c->qy[L] / c->h[L], c->gn2[L], c->nx[e], c->ny[e], &qi, &psi, &l1i, &l2i);
+    if (R < 0) { c->qB[e] = qi; continue; }
+    if (!is_wet(c, R)) continue;
+    double qj, l1j, l2j;
+    swe_ref_sediment_state(c->morph_formula, c->morph_alpha, c->morph_theta_cr, c->morph_s, c->morph_dm, c->g, c->h[R],
+                           c->qx[R] / c->h[R], c->qy[R] / c->h[R], c->gn2[R], c->nx[e], c->ny[e], &qj, &psi, &l1j, &l2j);
+    c->qB[e] = swe_ref_sediment_flux(qi, l1i, l2i, c->zb[L], qj, l1j, l2j, c->zb[R]);
+  }
+}
+
 void one_step(swe_ref_ctx *c, double dt, double t_new) {
   const double g = c->g;
   eval_strings(c);
@@ -322,6 +391,7 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
     swe_ref_edge_flux(g, heL, uL, vL, c->zb[L], heR, uR, vR, c->zb[R], c->nx[e], c->ny[e],
                       &c->F1[e], &c->F3[e], &c->GL[e], &c->GR[e]);
   }
+  if (c->morph_formula) sediment_fluxes(c);
   // ---- S1c draining-time limiter (R-8b): a cell may not lose more water than it holds.
   //      theta_i = min(1, h_i |Omega_i| / (dt * sum of its outgoing l F1)); every flux component of
   //      an edge is scaled by theta of the edge's donor cell (the cell the mass flux leaves).
@@ -399,6 +469,20 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
       for (int k = 0; k < 3; ++k) { const int32_t e = c->ce[3 * i + k]; C[k] = c->len[e] * c->Ac[sp][e]; }
       const double dC = ((s[0] * C[0] + s[1] * C[1]) + s[2] * C[2]);
       c->qc[sp][i] = c->qc[sp][i] - a * dC;
+    }
+  }
+  // ---- Eq. 13, S_b = 0: z_B <- z_B - 1/(1-p) * dt/|Omega| * sum_j l_ij q_Bij, slots in order
+  if (c->morph_formula) {
+    const double inv1mp = 1.0 / (1.0 - c->morph_p);
+    for (int64_t i = 0; i < c->nc; ++i) {
+      double B[3], s[3];
+      for (int k = 0; k < 3; ++k) {
+        const int32_t e = c->ce[3 * i + k];
+        s[k] = (c->eL[e] == i) ? 1.0 : -1.0;
+        B[k] = c->len[e] * c->qB[e];
+      }
+      const double dB = ((s[0] * B[0] + s[1] * B[1]) + s[2] * B[2]);
+      c->zb[i] = c->zb[i] - inv1mp * ((dt * c->invA[i]) * dB);
     }
   }
   for (auto &kv : c->strings) {      // bookkeeping from the (limited) fluxes actually applied
@@ -517,6 +601,28 @@ extern "C" int swe_ref_get_scalars(swe_ref_ctx *c, double *qc) {
 extern "C" int swe_ref_set_boundary_scalar(swe_ref_ctx *c, int string_id, const double *phi, int n) {
   if (!c || string_id < 0 || n < 0 || (n > 0 && !phi)) return -1;
   c->strings[string_id].phi_in.assign(phi, phi + n);
+  return 0;
+}
+
+extern "C" int swe_ref_set_morphology(swe_ref_ctx *c, int formula, double alpha, double theta_cr, double sdens,
+                                      double dm, double porosity) {
+  if (formula < 0 || formula > 2) { c->err = "formula must be 0 (fixed bed), 1 (Grass-like) or 2 (MPM-like)"; return 1; }
+  if (!(porosity >= 0.0 && porosity < 1.0)) { c->err = "porosity must be in [0, 1)"; return 1; }
+  if (formula == 2 && !(sdens > 1.0 && dm > 0.0)) { c->err = "MPM-like formula needs s > 1 and d_m > 0"; return 1; }
+  c->morph_formula = formula; c->morph_alpha = alpha; c->morph_theta_cr = theta_cr; c->morph_s = sdens; c->morph_dm = dm;
+  c->morph_p = porosity;
+  c->qB.assign(c->ne, 0.0);
+  return 0;
+}
+
+extern "C" int swe_ref_get_bed(swe_ref_ctx *c, double *zb) {
+  std::memcpy(zb, c->zb.data(), sizeof(double) * c->nc);
+  return 0;
+}
+
+extern "C" int swe_ref_get_sediment_flux(swe_ref_ctx *c, double *qB) {
+  if (c->qB.empty()) { c->err = "morphodynamics is off"; return 1; }
+  std::memcpy(qB, c->qB.data(), sizeof(double) * c->ne);
   return 0;
 }
 

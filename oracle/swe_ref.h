@@ -19,6 +19,9 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): hand-computed fluxes, literal Eq. 10/11 H-form
  * identity, geometry closed forms, Ritter and Stoker dam breaks, lake at rest, mass conservation,
  * uniform-flow normal depth, permutation invariance, restart, T6 rest level 0.364 m.
+ * Morphodynamics (tests/test_oracle_morph.py): Table 2 by hand, psi of Eq. 16 by finite differences, Vieta's relations
+ * of Eq. 16, HLL special cases of Eq. 14-15, Eq. 13 re-assembled with numpy, porosity factor, sediment volume in a closed
+ * box, flat bed under a uniform stream, bed-hump celerity under the Grass-like law.
  * "parity unpinned" items: none of the functions; but the *choice* of readings R-2 (HLLC form) and
  * R-11 (inflow distribution) cannot be pinned against BASEMENT itself (closed source).
  */
@@ -62,6 +65,18 @@ int swe_ref_set_scalars(swe_ref_ctx *c, int n_species, const double *qc);
 int swe_ref_get_scalars(swe_ref_ctx *c, double *qc);
 /* concentrations phi[0..n) carried by the water that enters through INFLOW_Q string string_id (default 0) */
 int swe_ref_set_boundary_scalar(swe_ref_ctx *c, int string_id, const double *phi, int n);
+/* Morphodynamics (Eq. 3; Eq. 13-16; Table 2; R-20):
+ * formula 0 = fixed bed, 1 = Grass-like alpha |u|^3, 2 = MPM-like alpha (theta - theta_cr)^1.5 sqrt((s-1) g d_m^3).
+ * From the next step on the bed z_B of every cell moves by Eq. 13 with the HLL-type sediment flux of Eq. 14-16. */
+int swe_ref_set_morphology(swe_ref_ctx *c, int formula, double alpha, double theta_cr, double sdens, double dm,
+                           double porosity);
+int swe_ref_get_bed(swe_ref_ctx *c, double *zb);
+int swe_ref_get_sediment_flux(swe_ref_ctx *c, double *qB);   /* q_Bij [n_edges] of the most recent step */
+/* inspection: one cell seen from one interface (Table 2 + Eq. 16), and Eq. 14-15 for one interface */
+void swe_ref_sediment_state(int formula, double alpha, double theta_cr, double sdens, double dm, double g,
+                            double h, double u, double v, double gn2, double nx, double ny,
+                            double *qBn, double *psi, double *lam1, double *lam2);
+double swe_ref_sediment_flux(double qBi, double l1i, double l2i, double zi, double qBj, double l1j, double l2j, double zj);
 int swe_ref_step(swe_ref_ctx *c, int64_t n_steps, double t_end, double cfl, swe_ref_info *info);
 int swe_ref_get_state(swe_ref_ctx *c, double *h, double *hu, double *hv);
 void swe_ref_destroy(swe_ref_ctx *c);

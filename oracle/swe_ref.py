@@ -52,6 +52,13 @@ def lib():
         L.swe_ref_set_scalars.argtypes = [C.c_void_p, C.c_int, _f64p]
         L.swe_ref_get_scalars.argtypes = [C.c_void_p, _f64p]
         L.swe_ref_set_boundary_scalar.argtypes = [C.c_void_p, C.c_int, _f64p, C.c_int]
+        L.swe_ref_set_morphology.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 5
+        L.swe_ref_get_bed.argtypes = [C.c_void_p, _f64p]
+        L.swe_ref_get_sediment_flux.argtypes = [C.c_void_p, _f64p]
+        L.swe_ref_sediment_state.argtypes = [C.c_int] + [C.c_double] * 11 + [_f64p] * 4
+        L.swe_ref_sediment_state.restype = None
+        L.swe_ref_sediment_flux.argtypes = [C.c_double] * 8
+        L.swe_ref_sediment_flux.restype = C.c_double
         L.swe_ref_destroy.argtypes = [C.c_void_p]
         L.swe_ref_destroy.restype = None
         L.swe_ref_last_error.argtypes = [C.c_void_p]
@@ -84,6 +91,21 @@ def edge_flux(g, heL, uL, vL, zL, heR, uR, vR, zR, nx, ny):
 def cbrt(x):
     """Cube root rounded to nearest (R-14)."""
     return lib().swe_ref_cbrt(float(x))
+
+
+GRASS, MPM = 1, 2
+
+
+def sediment_state(formula, alpha, theta_cr, s, dm, g, h, u, v, gn2, nx, ny):
+    """(q_B.n, psi = d q_Bn / d q_n, lambda_1, lambda_2) of one cell seen from one interface (Table 2, Eq. 16)."""
+    o = [C.c_double() for _ in range(4)]
+    lib().swe_ref_sediment_state(int(formula), alpha, theta_cr, s, dm, g, h, u, v, gn2, nx, ny, *[C.byref(x) for x in o])
+    return tuple(x.value for x in o)
+
+
+def sediment_flux(qBi, l1i, l2i, zi, qBj, l1j, l2j, zj):
+    """q_Bij of Eq. 14-15."""
+    return lib().swe_ref_sediment_flux(qBi, l1i, l2i, zi, qBj, l1j, l2j, zj)
 
 
 def wall_flux_via_ghost(g, he, un, ut):
@@ -141,6 +163,23 @@ class RefSolver:
     def set_boundary_scalar(self, string_id, phi):
         a = np.ascontiguousarray(phi, np.float64)
         assert lib().swe_ref_set_boundary_scalar(self._h, int(string_id), _p(a, _f64p), int(a.size)) == 0
+
+    def set_morphology(self, formula, alpha, theta_cr=0.047, s=2.65, dm=1e-3, porosity=0.4):
+        """Eq. 3 / Eq. 13-16: 0 fixed bed, 1 Grass-like, 2 MPM-like (R-20)."""
+        rc = lib().swe_ref_set_morphology(self._h, int(formula), float(alpha), float(theta_cr), float(s), float(dm),
+                                          float(porosity))
+        if rc != 0:
+            raise ValueError(lib().swe_ref_last_error(self._h).decode())
+
+    def get_bed(self):
+        out = np.empty(self.n_cells)
+        assert lib().swe_ref_get_bed(self._h, _p(out, _f64p)) == 0
+        return out
+
+    def sediment_fluxes(self):
+        out = np.empty(self.n_edges)
+        assert lib().swe_ref_get_sediment_flux(self._h, _p(out, _f64p)) == 0
+        return out
 
     def step(self, n_steps=-1, t_end=float("inf"), cfl=0.9):
         info = Info()
