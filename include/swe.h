@@ -135,6 +135,23 @@ int swe_get_scalars(swe_ctx *ctx, double *qc);
 /* concentrations phi[0..n) of the water entering through SWE_BC_INFLOW_Q string string_id (default 0) */
 int swe_set_boundary_scalar(swe_ctx *ctx, int string_id, const double *phi, int n);
 
+/* Morphodynamics (section 3.2, Eq. 3; section 4.3, Eq. 13-16; Table 2; R-20).
+ * From the next step on the bed elevation of every cell moves, with the hydrodynamic time step ("synchronous-decoupled",
+ * P:256), by Eq. 13 with S_b = 0 and the HLL-type sediment flux of Eq. 14-16 evaluated from the state at t^n:
+ *   formula 0  fixed bed (switches the module off again)
+ *   formula 1  Grass-like   |q_B| = alpha |u|^3                              (m = 3, u_cr = 0)
+ *   formula 2  MPM-like     |q_B| = alpha (theta - theta_cr)^1.5 sqrt((s-1) g d_m^3), theta = |u|^2 / (k_st^2 h^(1/3) (s-1) d_m)
+ * theta_cr, s, d_m are read by formula 2 only; porosity p in [0, 1).  No transport through walls or where a side of an
+ * interface is dry (h <= h_dry); through every open boundary the interior cell's own flux passes (equilibrium).
+ * The step becomes the three-pass one (its edge kernel also writes q_Bij, 8 B per edge; its cell kernel gathers it and
+ * writes z_B with the record it writes anyway): SWE_EINVAL on a context created with SWE_VARIANT_PATCH or with
+ * n_species > 0.  Synchronises the stream and captures the CUDA graph of the step again (once per call). */
+int swe_set_morphology(swe_ctx *ctx, int formula, double alpha, double theta_cr, double s, double d_m, double porosity);
+/* bed elevation z_B [n_cells] in the caller's cell numbering (host or device pointer as for swe_get_state) */
+int swe_get_bed(swe_ctx *ctx, double *zb);
+/* inspection: q_Bij [n_edges] of the most recent step, caller edge numbering, positive from L to R */
+int swe_get_sediment_flux(swe_ctx *ctx, double *qB);
+
 /* Reads the state in the caller's cell numbering (host or device pointers as for swe_set_state). */
 int swe_get_state(swe_ctx *ctx, double *h, double *hu, double *hv);
 

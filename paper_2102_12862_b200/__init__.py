@@ -38,6 +38,7 @@ EXPORTS = (
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
     "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_get_patch_stats",
     "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar", "swe_host_preprocess",
+    "swe_set_morphology", "swe_get_bed", "swe_get_sediment_flux",
 )
 
 
@@ -112,6 +113,9 @@ def lib():
         L.swe_set_scalars.argtypes = [C.c_void_p, C.c_void_p]
         L.swe_get_scalars.argtypes = [C.c_void_p, C.c_void_p]
         L.swe_set_boundary_scalar.argtypes = [C.c_void_p, C.c_int, _f64p, C.c_int]
+        L.swe_set_morphology.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 5
+        L.swe_get_bed.argtypes = [C.c_void_p, C.c_void_p]
+        L.swe_get_sediment_flux.argtypes = [C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -228,6 +232,29 @@ class Solver:
             ptr = C.c_void_p(out.ctypes.data)
         self._check(lib().swe_get_scalars(self._h, ptr))
         return out
+
+    def set_morphology(self, formula, alpha, theta_cr=0.047, s=2.65, dm=1e-3, porosity=0.4):
+        """swe_set_morphology: 0 fixed bed, 1 Grass-like, 2 MPM-like (Eq. 3, Eq. 13-16, Table 2; R-20)."""
+        self._check(lib().swe_set_morphology(self._h, int(formula), float(alpha), float(theta_cr), float(s), float(dm),
+                                             float(porosity)))
+
+    def _get_vector(self, fn, n):
+        if self.state_on_device:
+            out = self._torch.empty(n, dtype=self._torch.float64, device=self.device)
+            ptr = C.c_void_p(out.data_ptr())
+        else:
+            out = np.empty(n)
+            ptr = C.c_void_p(out.ctypes.data)
+        self._check(fn(self._h, ptr))
+        return out
+
+    def get_bed(self):
+        """z_B per cell, caller numbering."""
+        return self._get_vector(lib().swe_get_bed, self.n_cells)
+
+    def sediment_fluxes(self):
+        """q_Bij per edge of the most recent step (inspection)."""
+        return self._get_vector(lib().swe_get_sediment_flux, self.n_edges)
 
     def set_boundary_scalar(self, string_id, phi):
         a = np.ascontiguousarray(phi, np.float64)

@@ -78,12 +78,15 @@ struct swe_ctx {
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
   int cell_grid = 148 * 4;           // resident blocks of the persistent k_cell_update
   int edge_grid = 148 * 5;           // resident blocks of the persistent k_edge_flux (set from the occupancy API)
+  int base_edge_grid = 0, base_cell_grid = 0, sms = 148;
+  Morph mp{};                        // morphodynamics (swe_set_morphology); formula 0 = fixed bed
   uint8_t *d_drain_flag = nullptr;   // three-pass step: cells flagged as possible drainers (lazy theta)
   Scalars sc{};                      // passive scalars: device arrays owned by the library (cudaMalloc)
   double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
   int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
   int n_patches = 0; size_t patch_smem = 0;
   void (*patch_kernel)(Control *, PatchArgs) = nullptr;
+  int64_t alg_bytes_base[2] = {};        // three-pass k_edge_flux / k_cell_update without the mobile bed
   int64_t alg_bytes_v[3][4] = {};        // [variant][kernel]: algorithmic DRAM bytes per launch of the kernels of a step
   bool auto_mode = false;                // AUTO with both variants available: chosen at swe_set_state (wet fraction)
   cudaGraph_t graph = nullptr;
@@ -140,7 +143,10 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
-  if (c->sc.n > 0)
+  if (c->mp.formula)
+    k_edge_flux<false, true, true><<<std::min(grid_for(c->ne), c->edge_grid), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+                                                          c->area, c->d_drain_flag, c->mp);
+  else if (c->sc.n > 0)
     k_edge_flux<true, false><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                          c->area, c->d_drain_flag);
   else
@@ -150,7 +156,10 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
   k_theta_lazy<<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                                   c->d_drain_flag, (int)c->nc);
   if (ev) cudaEventRecord(ev[3], s);
-  if (c->sc.n > 0)
+  if (c->mp.formula)
+    k_cell_update<false, true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+                                                                  c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc, c->mp);
+  else if (c->sc.n > 0)
     k_cell_update<true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
                                                            c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   else
@@ -206,6 +215,7 @@ void release(swe_ctx *c) {
   }
   if (c->d_scalar_stage) cudaFree(c->d_scalar_stage);
   if (c->d_drain_flag) cudaFree(c->d_drain_flag);
+  if (c->mp.qB) cudaFree(c->mp.qB);
   if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
   if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -426,6 +436,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     if (c->sc.n > 0) SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<true>, kBlock, 0));
     else SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false>, kBlock, 0));
     c->cell_grid = std::max(1, sms * per_sm);
+    c->base_edge_grid = c->edge_grid; c->base_cell_grid = c->cell_grid; c->sms = sms;
   }
   // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
@@ -532,6 +543,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     ab[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
     ab[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
     ab[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
+    c->alg_bytes_base[0] = ab[1]; c->alg_bytes_base[1] = ab[3];
   }
 
   // ---- control block
@@ -768,6 +780,98 @@ int swe_get_scalars(swe_ctx *c, double *qc) {
     }
   }
   SWE_CUDA(c, cudaGetLastError());
+  return SWE_OK;
+}
+
+// Morphodynamics (include/swe.h): the bed moves from the next step on.  The step becomes the three-pass one with the
+// <kMorph> instances of its edge and cell kernels (the fused patch step keeps the bed of its halo cells in tables built
+// for a fixed bed); the CUDA graph of the three-pass step is captured again.
+int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, double s, double d_m, double porosity) {
+  if (!c) return SWE_EINVAL;
+  if (formula < 0 || formula > 2) { c->err = "formula must be 0 (fixed bed), 1 (Grass-like) or 2 (MPM-like)"; return SWE_EINVAL; }
+  if (!(porosity >= 0.0 && porosity < 1.0)) { c->err = "porosity must be in [0, 1)"; return SWE_EINVAL; }
+  if (!std::isfinite(alpha) || alpha < 0.0) { c->err = "alpha must be finite and >= 0"; return SWE_EINVAL; }
+  if (formula == 2 && !(s > 1.0 && d_m > 0.0 && std::isfinite(s) && std::isfinite(d_m) && std::isfinite(theta_cr))) {
+    c->err = "the MPM-like formula needs s > 1, d_m > 0 and a finite theta_cr"; return SWE_EINVAL;
+  }
+  if (formula && c->sc.n > 0) { c->err = "passive scalars and a mobile bed in one context are not built"; return SWE_EINVAL; }
+  if (formula && !c->auto_mode && c->variant == SWE_VARIANT_PATCH) {
+    c->err = "the fused patch step has no mobile bed: create the context with SWE_VARIANT_AUTO or SWE_VARIANT_THREE_PASS";
+    return SWE_EINVAL;
+  }
+  int rc = read_control(c);          // synchronises: no step in flight
+  if (rc != SWE_OK) return rc;
+  if (formula) {
+    if (c->variant == SWE_VARIANT_PATCH) {
+      rc = switch_variant(c, SWE_VARIANT_THREE_PASS, c->h_ctl->cur);
+      if (rc != SWE_OK) return rc;
+    }
+    c->auto_mode = false;            // stays three-pass from here on
+    if (!c->mp.qB) {
+      SWE_CUDA(c, cudaMalloc((void **)&c->mp.qB, 8 * (size_t)c->ne));
+      SWE_CUDA(c, cudaMemsetAsync(c->mp.qB, 0, 8 * (size_t)c->ne, c->stream));
+    }
+  }
+  const double g = c->prm.g;
+  c->mp.formula = formula; c->mp.alpha = alpha; c->mp.theta_cr = theta_cr;
+  c->mp.shields_den = g * ((s - 1.0) * d_m);
+  c->mp.Gm = alpha * std::sqrt(((s - 1.0) * g) * (d_m * (d_m * d_m)));
+  c->mp.inv1mp = 1.0 / (1.0 - porosity);
+  c->mp.gn2 = c->gn2;
+  {                                   // algorithmic bytes of the two kernels that carry the extra work
+    int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
+    ab[1] = c->alg_bytes_base[0] + (formula ? 8 * c->ne + (formula == 2 ? 8 * c->nc : 0) : 0);
+    ab[3] = c->alg_bytes_base[1] + (formula ? 8 * c->ne : 0);
+  }
+  c->edge_grid = c->base_edge_grid; c->cell_grid = c->base_cell_grid;
+  if (formula) {                      // resident grids of the <kMorph> instances
+    int per_sm = 3;
+    SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_edge_flux<false, true, true>, kBlock, 0));
+    c->edge_grid = std::max(1, c->sms * per_sm);
+    SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false, true>, kBlock, 0));
+    c->cell_grid = std::max(1, c->sms * per_sm);
+  }
+  if (c->graph_exec_v[SWE_VARIANT_THREE_PASS]) {
+    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaGraphExecDestroy(c->graph_exec_v[SWE_VARIANT_THREE_PASS]);
+    c->graph_exec_v[SWE_VARIANT_THREE_PASS] = nullptr;
+  }
+  if (c->variant == SWE_VARIANT_THREE_PASS) return capture_graph(c);
+  const int keep = c->variant;        // fixed bed again on a context that steps with the patch kernel
+  c->variant = SWE_VARIANT_THREE_PASS;
+  rc = capture_graph(c);
+  c->variant = keep;
+  return rc;
+}
+
+int swe_get_bed(swe_ctx *c, double *zb) {
+  if (!c) return SWE_EINVAL;
+  if (!zb) { c->err = "null bed pointer"; return SWE_EINVAL; }
+  const int64_t nc = c->nc;
+  double *dst = c->prm.state_on_device ? zb : c->stage;
+  k_unpack_bed<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, dst, (int)nc);
+  c->launches += 1;
+  SWE_CUDA(c, cudaGetLastError());
+  if (!c->prm.state_on_device) {
+    SWE_CUDA(c, cudaMemcpyAsync(zb, c->stage, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
+    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return SWE_OK;
+}
+
+int swe_get_sediment_flux(swe_ctx *c, double *qB) {
+  if (!c) return SWE_EINVAL;
+  if (!qB) { c->err = "null flux pointer"; return SWE_EINVAL; }
+  if (!c->mp.qB) { c->err = "morphodynamics was never switched on"; return SWE_EINVAL; }
+  const int64_t ne = c->ne;
+  double *dst = c->prm.state_on_device ? qB : c->stage;       // stage holds 3 n_cells >= n_edges doubles
+  k_export_sediment<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->mp.qB, dst, (int)ne);
+  c->launches += 1;
+  SWE_CUDA(c, cudaGetLastError());
+  if (!c->prm.state_on_device) {
+    SWE_CUDA(c, cudaMemcpyAsync(qB, c->stage, 8 * ne, cudaMemcpyDeviceToHost, c->stream));
+    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
   return SWE_OK;
 }
 

@@ -178,16 +178,63 @@ edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, con
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Morphodynamics, S1m (section 4.3; R-20): Table 2's transport law and the two speeds of Eq. 16 for one
+// cell seen from one interface, then Eq. 14-15.
+// ---------------------------------------------------------------------------------------------------------
+struct SedState { double q, l1, l2; };
+
+__device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double h, double u, double v, double f2,
+                                              double nx, double ny) {
+  const double un = u * nx + v * ny, ut = v * nx - u * ny;
+  const double sp2 = u * u + v * v;
+  double q = 0.0, ps = 0.0;
+  if (mp.formula == 1) {                       // Grass-like, m = 3, u_cr = 0 (Table 2)
+    q = mp.alpha * (sp2 * un);
+    ps = (mp.alpha * (sp2 + 2.0 * (un * un))) / h;
+  } else {                                     // MPM-like, m = 1.5 (Table 2); Shields parameter from Table 1's
+    const double th = (f2 * sp2) / (cbrt_rn(h) * mp.shields_den);          // Strickler shear stress
+    const double x = th - mp.theta_cr;
+    if (x > 0.0 && sp2 > 0.0) {
+      const double rx = sqrt(x), spd = sqrt(sp2);
+      q = (mp.Gm * (x * rx)) * (un / spd);
+      ps = (mp.Gm * (((3.0 * rx) * th) * (un * un) + (x * rx) * (ut * ut))) / ((sp2 * spd) * h);
+    }
+  }
+  const double cel = sqrt(g * h);
+  const double a = un - cel;                   // Eq. 16 as printed: (u_n - c) in both roots
+  const double disc = sqrt(a * a + 4.0 * (ps * (cel * cel)));
+  SedState o;
+  o.q = q; o.l1 = 0.5 * (a - disc); o.l2 = 0.5 * (a + disc);
+  return o;
+}
+
+// q_Bij of edge e from the two cell records of t^n: nothing where a side is dry or at a wall; through open boundaries
+// the interior cell's own flux (equilibrium boundary)
+__device__ __forceinline__ double sediment_edge(const Morph &mp, double g, double h_dry, const EdgeGeom &eg,
+                                                const CellRec &a, const CellRec &b) {
+  if (!(a.h > h_dry) || eg.R == -1) return 0.0;
+  const double f2L = mp.formula == 2 ? mp.gn2[eg.L] : 0.0;
+  const SedState si = sed_state(mp, g, a.h, a.qx / a.h, a.qy / a.h, f2L, eg.nx, eg.ny);
+  if (eg.R < 0) return si.q;
+  if (!(b.h > h_dry)) return 0.0;
+  const double f2R = mp.formula == 2 ? mp.gn2[eg.R] : 0.0;
+  const SedState sj = sed_state(mp, g, b.h, b.qx / b.h, b.qy / b.h, f2R, eg.nx, eg.ny);
+  const double sm = dmin2(si.l1, sj.l1), sp = dmax2(si.l2, sj.l2);        // Eq. 15
+  if (!(sp - sm > 0.0)) return 0.0;
+  return ((sp * si.q - sm * sj.q) + (sp * sm) * (b.z - a.z)) / (sp - sm);  // Eq. 14
+}
+
 // kPersistent = false: one edge per thread.  kPersistent = true: a grid of resident blocks strides over the edges and
 // the (streamed) geometry record of a thread's next edge is loaded while the current edge is worked on, so that the
 // geom -> cell record gather chain of an edge pays one memory latency instead of two (profiles/r1f: the kernel's
 // stalls are exactly these two loads).
-template <bool kScalars, bool kPersistent>
+template <bool kScalars, bool kPersistent, bool kMorph = false>
 __global__ void __launch_bounds__(kBlock)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
             EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,
-            const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
+            const double *__restrict__ area, uint8_t *__restrict__ drain_flag, const Morph mp = Morph{}) {
   if (!ctl->active && !force) return;
   const double g = ctl->g, h_dry = ctl->h_dry;
   int e = blockIdx.x * kBlock + threadIdx.x;
@@ -198,6 +245,7 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     CellRec b = a;
     if (eg.R >= 0) b = rec[eg.R];
     edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
+    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b);
     return;
   }
   const int stride = gridDim.x * kBlock;
@@ -209,6 +257,7 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     if (eg.R >= 0) b = rec[eg.R];
     if (e + stride < n_edges) eg_next = geom[e + stride];
     edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
+    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b);
   }
 }
 
@@ -329,12 +378,13 @@ __device__ __forceinline__ double cell_rate(double g, double h, double qx, doubl
 // ---------------------------------------------------------------------------------------------------------
 // S2 + S3, and S0 of the NEXT step fused in: one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
-template <bool kScalars>
-__global__ void __launch_bounds__(kBlock, kScalars ? 3 : 4)      // 4 blocks/SM = 64 registers: measured faster than 3
+template <bool kScalars, bool kMorph = false>
+__global__ void __launch_bounds__(kBlock, (kScalars || kMorph) ? 3 : 4)      // 4 blocks/SM = 64 registers: measured faster than 3
 k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
               const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
               const double *__restrict__ area, const double *__restrict__ inv_area,
-              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells, const Scalars sc) {
+              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells, const Scalars sc,
+              const Morph mp = Morph{}) {
   if (!ctl->active) return;
   // a grid of resident blocks strides over the cells; the (streamed) slot record of a thread's next cell is loaded
   // while the current cell is worked on: its cell_edge -> (geometry, flux) gather chain pays one latency, not two
@@ -349,7 +399,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
     if (i + stride < n_cells) ce_next = cell_edge[i + stride];
     const int es[3] = {ce.x, ce.y, ce.z};
     double nx[3], ny[3], len[3];
-    double dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3];
+    double dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3], dBk[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const EdgeGeom eg = geom[es[k]];
@@ -366,6 +416,7 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       const double s = isL ? 1.0 : -1.0;
       nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
       if (kScalars) { sgn[k] = s; F1lim[k] = f.F1; }
+      if (kMorph) dBk[k] = s * (eg.len * mp.qB[es[k]]);
       dHk[k] = s * (eg.len * f.F1);
       dXk[k] = s * (eg.len * (G * eg.nx - f.F3 * eg.ny));
       dYk[k] = s * (eg.len * (G * eg.ny + f.F3 * eg.nx));
@@ -395,6 +446,8 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       if (r > rate) rate = r;
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
+    if (kMorph)                                      // Eq. 13, S_b = 0: the bed rides in the same record
+      c.z = c.z - mp.inv1mp * (a * ((dBk[0] + dBk[1]) + dBk[2]));
     rec[i] = c;
     if (kScalars)                                    // Eq. 20, advective part: same gather, same slot order (R-19)
     _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
@@ -668,6 +721,22 @@ k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_per
   const int o = cell_perm[i];
   const CellRec c = rec[i];
   h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
+}
+
+// bed elevation z_B (swe_get_bed), newest state buffer, caller numbering
+__global__ void __launch_bounds__(kBlock)
+k_unpack_bed(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const CellRec *rec_a,
+             const CellRec *rec_b, double *__restrict__ zb, int n_cells) {
+  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i < n_cells) zb[cell_perm[i]] = rec[i].z;
+}
+
+// q_Bij of the most recent step in caller edge numbering (swe_get_sediment_flux); the sign follows the caller's L -> R
+__global__ void __launch_bounds__(kBlock)
+k_export_sediment(const int *__restrict__ edge_perm, const double *__restrict__ qB, double *__restrict__ out, int n_edges) {
+  const int e = blockIdx.x * kBlock + threadIdx.x;
+  if (e < n_edges) out[edge_perm[e]] = qB[e];
 }
 
 // one scalar species, caller numbering <-> internal numbering, newest state buffer

@@ -69,6 +69,16 @@ struct Scalars {                 // passive scalars q_c = h phi_c (section 3.3, 
   double *phi_up[kMaxSpecies];   // [n_edges] three-pass step: concentration on the upwind side of every edge
 };
 
+struct Morph {                   // morphodynamics (section 3.2 Eq. 3, section 4.3 Eq. 13-16; R-20); formula 0: fixed bed
+  int formula;                   // 1 Grass-like alpha |u|^3, 2 MPM-like alpha (theta - theta_cr)^1.5 sqrt((s-1) g d_m^3)
+  double alpha, theta_cr;
+  double shields_den;            // g (s-1) d_m: theta = (g/k_st^2) |u|^2 / (h^(1/3) * shields_den)
+  double Gm;                     // alpha sqrt((s-1) g d_m^3)
+  double inv1mp;                 // 1 / (1 - p)
+  const double *gn2;             // [n_cells] g / k_st^2 (0: no friction law, no bed shear stress)
+  double *qB;                    // [n_edges] normal sediment flux q_Bij of the step in flight
+};
+
 struct Control {                 // device-side step-loop state: nothing of it is read by the host per step
   double t, dt, t_end, cfl, dt_max, g, h_dry;
   double dt_last, vol_in, vol_out, vol_clipped;

@@ -1,0 +1,166 @@
+"""GPU parity of the morphodynamic module (R-20; Eq. 3, Eq. 13-16, Table 2
+PAPER.md:152-161) against the oracle, through the C-ABI (swe_set_morphology / swe_get_bed / swe_get_sediment_flux).
+Bar: the hydrodynamic state as in test_gpu_parity.py; bed elevation and per-edge sediment flux <= 1e-10 relative
+(expected and asserted where stated: bit-identical)."""
+import numpy as np
+import pytest
+
+from workloads import configs as C
+from workloads import mesh as M
+
+from test_gpu_parity import assert_state_close, check_info
+from test_gpu_fuzz import random_workload
+
+pytestmark = pytest.mark.gpu
+
+GRASS, MPM = 1, 2
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box")
+    import paper_2102_12862_b200 as P
+    P.lib()
+    return P
+
+
+def assert_close(got, want, what):
+    scale = np.max(np.abs(want)) if want.size else 0.0
+    tol = 1e-10 * np.abs(want) + 1e-14 * scale
+    bad = np.nonzero(~(np.abs(got - want) <= tol))[0]
+    assert bad.size == 0, f"{what}: {bad.size} entries out of tolerance, e.g. {bad[:5]}, got {got[bad[:3]]} want {want[bad[:3]]}"
+
+
+def both(gpu, ref, w, morph, chunks, **kw):
+    s = gpu.from_workload(w, **kw)
+    o = ref.RefSolver(w)
+    s.set_morphology(*morph)
+    o.set_morphology(*morph)
+    identical = True
+    for n in chunks:
+        ig, io = s.step(n, float("inf"), w.cfl), o.step(n, float("inf"), w.cfl)
+        sg, so = s.get_state(), o.get_state()
+        assert np.array_equal(sg[0] > w.h_dry, so[0] > w.h_dry)
+        assert_state_close(sg, so, f"{w.name} after {io['steps_done']} steps")
+        check_info(ig, io)
+        zg, zo = s.get_bed(), o.get_bed()
+        assert_close(zg - w.zb, zo - w.zb, f"{w.name}: bed change after {io['steps_done']} steps")
+        qg, qo = s.sediment_fluxes(), o.sediment_fluxes()
+        assert_close(qg, qo, f"{w.name}: q_Bij of step {io['steps_done']}")
+        identical &= np.array_equal(zg, zo) and np.array_equal(qg, qo) and all(np.array_equal(a, b) for a, b in zip(sg, so))
+    names = s.step_kernels()
+    s.close()
+    o.close()
+    return identical, zg, names
+
+
+def mobile_dam_break():
+    w = C.dam_break_channel(nx=120, ny=6, lx=30.0, ly=1.5, h_left=1.0, h_right=0.2, x_dam=15.0, t_end=float("inf"))
+    w.kst[:] = 35.0
+    return w
+
+
+@pytest.mark.parametrize("morph", [(GRASS, 0.02, 0.0, 2.65, 1e-3, 0.4), (MPM, 8.0, 0.047, 2.65, 0.002, 0.4),
+                                   (MPM, 4.93, 0.047, 2.6, 0.0005, 0.35)])
+@pytest.mark.parametrize("renumber", [0, 1])
+def test_dam_break_over_a_mobile_bed(gpu, ref, morph, renumber):
+    w = mobile_dam_break()
+    ident, zg, names = both(gpu, ref, w, morph, (1, 31, 68, 100), renumber=renumber)
+    assert ident
+    assert np.abs(zg - w.zb).max() > 1e-5                     # the bed did move
+    assert names == ["k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"]
+
+
+@pytest.mark.parametrize("morph", [(GRASS, 0.005, 0.0, 2.65, 1e-3, 0.4), (MPM, 8.0, 0.047, 2.65, 0.01, 0.4)])
+def test_river_reach_with_wet_dry_fronts_and_strings(gpu, ref, morph):
+    """A shrunken configs[3]: wet/dry fronts, limiter, friction, hydrograph inflow and normal-depth outflow (both open
+    boundaries pass the interior cell's q_B).  Created as AUTO: the context is on the patch step until
+    swe_set_morphology moves it to the three-pass one."""
+    w = C.by_id(4, 0.01)
+    ident, zg, names = both(gpu, ref, w, morph, (1, 40, 59, 100))
+    assert ident
+    assert np.abs(zg - w.zb).max() > 1e-7
+    assert names[1] == "k_edge_flux"
+
+
+def test_switching_the_module_on_mid_run_and_off_again(gpu, ref):
+    w = C.by_id(4, 0.01)
+    s, o = gpu.from_workload(w), ref.RefSolver(w)
+    assert s.step_kernels()[1] == "k_patch_step"             # AUTO picked the patch step for this half-dry reach
+    for sol in (s, o):
+        sol.step(45, float("inf"), w.cfl)
+        sol.set_morphology(GRASS, 0.01)
+        sol.step(70, float("inf"), w.cfl)
+    assert s.step_kernels()[1] == "k_edge_flux"
+    assert all(np.array_equal(a, b) for a, b in zip(s.get_state(), o.get_state()))
+    assert np.array_equal(s.get_bed(), o.get_bed())
+    z1 = s.get_bed()
+    for sol in (s, o):
+        sol.set_morphology(0, 0.0)
+        sol.step(40, float("inf"), w.cfl)
+    assert np.array_equal(s.get_bed(), z1)                    # fixed bed again: the moved bed stays where it is
+    assert all(np.array_equal(a, b) for a, b in zip(s.get_state(), o.get_state()))
+    s.close()
+    o.close()
+
+
+def test_zero_alpha_is_the_fixed_bed_scheme(gpu):
+    w = mobile_dam_break()
+    a, b = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS), gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    b.set_morphology(GRASS, 0.0)
+    a.step(64, float("inf"), w.cfl)
+    b.step(64, float("inf"), w.cfl)
+    assert all(np.array_equal(x, y) for x, y in zip(a.get_state(), b.get_state()))
+    assert np.array_equal(b.get_bed(), w.zb) and np.array_equal(a.get_bed(), w.zb)
+    a.close()
+    b.close()
+
+
+def test_invalid_combinations_are_refused(gpu):
+    w = mobile_dam_break()
+    s = gpu.from_workload(w, n_species=1)
+    with pytest.raises(RuntimeError, match="scalars"):
+        s.set_morphology(GRASS, 0.01)
+    s.close()
+    s = gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=96)
+    with pytest.raises(RuntimeError, match="patch"):
+        s.set_morphology(GRASS, 0.01)
+    s.close()
+    s = gpu.from_workload(w)
+    for bad in [(3, 0.01), (GRASS, -1.0), (GRASS, 0.01, 0.047, 2.65, 1e-3, 1.0), (MPM, 8.0, 0.047, 1.0, 1e-3, 0.4),
+                (MPM, 8.0, 0.047, 2.65, 0.0, 0.4)]:
+        with pytest.raises(RuntimeError):
+            s.set_morphology(*bad)
+    with pytest.raises(RuntimeError, match="never switched on"):
+        s.sediment_fluxes()
+    s.close()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_case_with_a_mobile_bed(gpu, ref, seed):
+    """The fuzz workloads of test_gpu_fuzz.py (random Delaunay meshes, bumps, thin films, mixed boundaries and friction,
+    frictionless cells included) with a random transport law."""
+    w, rng = random_workload(100 + seed)
+    morph = (GRASS, float(rng.uniform(0.0005, 0.01)), 0.0, 2.65, 1e-3, float(rng.uniform(0.2, 0.5))) if seed % 2 == 0 else \
+            (MPM, float(rng.uniform(3.0, 9.0)), 0.047, float(rng.uniform(2.0, 2.7)), float(10.0 ** rng.uniform(-4, -2)), 0.4)
+    both(gpu, ref, w, morph, (1, int(rng.integers(2, 40)), int(rng.integers(2, 60))),
+         steps_per_graph=int(rng.choice([0, 4, 32])), renumber=int(rng.choice([0, 1, 2])))
+
+
+def test_state_on_device_get_bed(gpu):
+    import torch
+    w = mobile_dam_break()
+    s = gpu.from_workload(w, state_on_device=True)
+    s.set_morphology(GRASS, 0.02)
+    s.step(10, float("inf"), w.cfl)
+    zb = s.get_bed()
+    assert zb.is_cuda and zb.shape == (w.n_cells,)
+    t = gpu.from_workload(w)
+    t.set_morphology(GRASS, 0.02)
+    t.step(10, float("inf"), w.cfl)
+    assert np.array_equal(zb.cpu().numpy(), t.get_bed())
+    assert np.array_equal(s.sediment_fluxes().cpu().numpy(), t.sediment_fluxes())
+    s.close()
+    t.close()
