@@ -36,6 +36,8 @@ NCU_TRAFFIC_BYTES = {("k_cell_update", 3964806): 726.9e6, ("k_theta_lazy", 39648
                      ("k_patch_step", 3964806): 502.0e6,  # profiles/r1i_ncu_full_patch_river.md (52 % of patches dry)
                      ("k_patch_step", 3964136): 678.6e6}  # profiles/r1c_ncu_full_patch_allwet.md
 
+# --morph: parameter sets of swe_set_morphology (formula, alpha, theta_cr, s, d_m, porosity)
+MORPH_PARAMS = {1: (1, 0.001, 0.0, 2.65, 1e-3, 0.4), 2: (2, 8.0, 0.047, 2.65, 0.005, 0.4)}
 METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
 
@@ -56,6 +58,8 @@ def parse():
     ap.add_argument("--stage", type=float, default=None,
                     help="config 4 only: initial water level relative to the sloped datum (default -2 = the configuration)")
     ap.add_argument("--species", type=int, default=0, help="passive scalar species advected with the flow (0..5)")
+    ap.add_argument("--morph", type=int, default=0, choices=[0, 1, 2],
+                    help="mobile bed (swe_set_morphology): 1 Grass-like alpha = 0.001, 2 MPM-like alpha = 8, d_m = 5 mm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-wet", action="store_true", help="skip the second (all-wet mesh) line")
@@ -186,10 +190,12 @@ def physical_gpu_index(local_rank):
     return local_rank
 
 
-def oracle_time(w, n_warm, max_steps, min_seconds, cfl):
+def oracle_time(w, n_warm, max_steps, min_seconds, cfl, morph=0):
     """The oracle as it stands on this box's host cores (single thread): (cell-updates/s, time steps timed, s)."""
     from oracle import swe_ref
     o = swe_ref.RefSolver(w)
+    if morph:
+        o.set_morphology(*MORPH_PARAMS[morph])
     if n_warm:
         o.step(n_warm, float("inf"), cfl)
     done, t0 = 0, time.perf_counter()
@@ -210,6 +216,8 @@ def run_reference(args, rank):
     from oracle import swe_ref
     w = load_workload(args.config, args.scale)
     o = swe_ref.RefSolver(w)
+    if args.morph:
+        o.set_morphology(*MORPH_PARAMS[args.morph])
     for _ in range(args.warmup):
         o.step(1, float("inf"), w.cfl)
     t0 = time.perf_counter()
@@ -273,6 +281,8 @@ def main():
         for sid, typ, _ in w.strings:
             if typ == 1:
                 s.set_boundary_scalar(sid, [1.0] * args.species)
+    if args.morph:
+        s.set_morphology(*MORPH_PARAMS[args.morph])
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     stream = torch.cuda.current_stream(dev)
@@ -360,7 +370,7 @@ def main():
     # moves a third of the bytes; the three-pass step (edge flux -> theta -> CSR gather/update, the design the
     # north_star names) is the bandwidth-bound one, so its per-kernel HBM fractions are reported beside the default's
     other = None
-    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0:
+    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0 and not args.morph:
         ov = P.VARIANT_THREE_PASS if s_kernels[-1] == "k_patch_step" else P.VARIANT_PATCH
         s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber)
         for _ in range(2):
@@ -386,7 +396,7 @@ def main():
     # ---- second line (rank 0, N = 1): an ALL-WET mesh of the same size, where no patch can be skipped -- the
     # BASELINE.json configs[4] construction (circular dam break, every cell wet, friction everywhere) at 4M cells
     all_wet = None
-    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0:
+    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0 and not args.morph:
         from workloads import configs as C
         w2 = C.config5(target_cells=N)
         s2 = P.from_workload(w2, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
@@ -413,7 +423,7 @@ def main():
     # ---- CPU baseline: the oracle, single thread, bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl)
+        v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl, args.morph)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"all {N} cells x {n_done} time steps from the initial state ({secs:.1f} s, 1 thread)"}
 
@@ -425,7 +435,7 @@ def main():
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
-                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "stage": args.stage, "step_kernels": s_kernels, "patch": patch_stats},
+                       "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "morph": args.morph, "stage": args.stage, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet, "other_variant": other,

@@ -230,7 +230,7 @@ __device__ __forceinline__ double sediment_edge(const Morph &mp, double g, doubl
 // geom -> cell record gather chain of an edge pays one memory latency instead of two (profiles/r1f: the kernel's
 // stalls are exactly these two loads).
 template <bool kScalars, bool kPersistent, bool kMorph = false>
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(kBlock, kMorph ? 3 : 0)
 k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
             const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
             EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,

@@ -108,3 +108,26 @@ def test_config5_8m_window_and_variants(gpu, ref):
     assert i1["n_wet"] == w.n_cells and i1["vol_clipped"] == 0.0
     s.close()
     t.close()
+
+
+def test_config4_full_size_mobile_bed(gpu, ref):
+    """configs[3] at full size with the morphodynamic module on (R-20; MPM-like law, d_m = 5 mm): every cell's state and
+    bed elevation and every edge's q_Bij against the oracle over a short window; a cell no water ever reached keeps its
+    bed (property that holds at any size)."""
+    w = C.config4()
+    s = make(gpu, w)
+    o = ref.RefSolver(w)
+    morph = (2, 8.0, 0.047, 2.65, 0.005, 0.4)
+    s.set_morphology(*morph)
+    o.set_morphology(*morph)
+    assert s.step_kernels() == ["k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"]
+    window(s, o, w, 12, "config4 full size, mobile bed, steps 0-12")
+    zg, zo = s.get_bed(), o.get_bed()
+    assert np.array_equal(zg, zo)
+    assert np.array_equal(s.sediment_fluxes(), o.sediment_fluxes())
+    moved = zg != w.zb
+    assert moved.any() and not moved[(w.h <= w.h_dry) & (s.get_state()[0] == 0.0)].any()
+    ig = s.step(500, float("inf"), w.cfl)
+    assert ig["flags"] == 0 and np.all(np.isfinite(s.get_bed()))
+    s.close()
+    o.close()
