@@ -336,6 +336,11 @@ def main():
             roofline["note"] = ("the fused patch step moves about a third of the bytes of the bandwidth-bound "
                                 "three-pass step (other_variant: its kernels and whole step against the same HBM "
                                 "peak) and is bound by fp64 issue / latency, not by HBM (DESIGN.md section 7)")
+        if args.morph and top == "k_edge_flux":
+            roofline["traffic"] = None
+            roofline["note"] = ("mobile bed: the <kMorph> edge kernel is bound by fp64 instruction issue (Table 2 + Eq. 16 "
+                                "per side on top of the HLLC flux; ncu: fp64 pipe 47 %, issue slots 58 % at 24 warps/SM), "
+                                "not by HBM (profiles/r1j_morph.md)")
 
     # ---- end-to-end arm: the same K steps through the C-ABI with HOST (pinned) buffers, copies inside the region
     e2e = None
