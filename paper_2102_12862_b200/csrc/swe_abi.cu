@@ -216,6 +216,7 @@ void release(swe_ctx *c) {
   if (c->d_scalar_stage) cudaFree(c->d_scalar_stage);
   if (c->d_drain_flag) cudaFree(c->d_drain_flag);
   if (c->mp.qB) cudaFree(c->mp.qB);
+  if (c->mp.cell) cudaFree(c->mp.cell);
   if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
   if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -675,6 +676,10 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
                                                                              c->d_dry + c->n_patches, c->sc);
     c->launches += 1;
   }
+  if (c->mp.formula == 2) {           // mobile bed, MPM-like law: the per-cell cube roots of the new state
+    k_sed_cell_init<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)nc);
+    c->launches += 1;
+  }
   k_reset<<<1, 1, 0, c->stream>>>(c->d_ctl, t0);
   k_rate<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, c->rec_b, (int)nc);
   c->launches += 3;
@@ -817,11 +822,16 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
   c->mp.shields_den = g * ((s - 1.0) * d_m);
   c->mp.Gm = alpha * std::sqrt(((s - 1.0) * g) * (d_m * (d_m * d_m)));
   c->mp.inv1mp = 1.0 / (1.0 - porosity);
-  c->mp.gn2 = c->gn2;
+  if (formula == 2) {                 // (g/k^2, cbrt(h)) of the state as it stands; k_cell_update keeps it current
+    if (!c->mp.cell) SWE_CUDA(c, cudaMalloc((void **)&c->mp.cell, 16 * (size_t)c->nc));
+    k_sed_cell_init<<<grid_for(c->nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)c->nc);
+    c->launches += 1;
+    SWE_CUDA(c, cudaGetLastError());
+  }
   {                                   // algorithmic bytes of the two kernels that carry the extra work
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
-    ab[1] = c->alg_bytes_base[0] + (formula ? 8 * c->ne + (formula == 2 ? 8 * c->nc : 0) : 0);
-    ab[3] = c->alg_bytes_base[1] + (formula ? 8 * c->ne : 0);
+    ab[1] = c->alg_bytes_base[0] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
+    ab[3] = c->alg_bytes_base[1] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
   }
   c->edge_grid = c->base_edge_grid; c->cell_grid = c->base_cell_grid;
   if (formula) {                      // resident grids of the <kMorph> instances

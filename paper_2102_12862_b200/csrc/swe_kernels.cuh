@@ -139,13 +139,15 @@ __device__ __forceinline__ void
 edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, const EdgeGeom &eg, const CellRec &a,
              const CellRec &b, const CellRec *__restrict__ rec, const double *__restrict__ kst,
              const BoundaryString *__restrict__ strings, EdgeFlux *__restrict__ flux, const Scalars &sc,
-             const double *__restrict__ area, uint8_t *__restrict__ drain_flag) {
+             const double *__restrict__ area, uint8_t *__restrict__ drain_flag, double (&vel)[4]) {
   double uL = 0.0, vL = 0.0;
   if (a.h > h_dry) { uL = a.qx / a.h; vL = a.qy / a.h; }   // R-8: thin films carry no momentum
+  vel[0] = uL; vel[1] = vL; vel[2] = 0.0; vel[3] = 0.0;    // handed to the sediment flux of the <kMorph> instance
   EdgeFlux o;
   if (eg.R >= 0) {
     double uR = 0.0, vR = 0.0;
     if (b.h > h_dry) { uR = b.qx / b.h; vR = b.qy / b.h; }
+    vel[2] = uR; vel[3] = vR;
     const double unL = uL * eg.nx + vL * eg.ny, utL = vL * eg.nx - uL * eg.ny;
     const double unR = uR * eg.nx + vR * eg.ny, utR = vR * eg.nx - uR * eg.ny;
     o = riemann_nt(g, a.h, unL, utL, a.z, b.h, unR, utR, b.z);
@@ -184,7 +186,7 @@ edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, con
 // ---------------------------------------------------------------------------------------------------------
 struct SedState { double q, l1, l2; };
 
-__device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double h, double u, double v, double f2,
+__device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double h, double u, double v, double2 fc,
                                               double nx, double ny) {
   const double un = u * nx + v * ny, ut = v * nx - u * ny;
   const double sp2 = u * u + v * v;
@@ -193,7 +195,8 @@ __device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double 
     q = mp.alpha * (sp2 * un);
     ps = (mp.alpha * (sp2 + 2.0 * (un * un))) / h;
   } else {                                     // MPM-like, m = 1.5 (Table 2); Shields parameter from Table 1's
-    const double th = (f2 * sp2) / (cbrt_rn(h) * mp.shields_den);          // Strickler shear stress
+    // Strickler shear stress; fc = (g / k_st^2, cbrt_rn(h)) from Morph::cell; no friction law: theta = 0 / (..) = 0
+    const double th = fc.x > 0.0 ? (fc.x * sp2) / (fc.y * mp.shields_den) : 0.0;
     const double x = th - mp.theta_cr;
     if (x > 0.0 && sp2 > 0.0) {
       const double rx = sqrt(x), spd = sqrt(sp2);
@@ -211,15 +214,16 @@ __device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double 
 
 // q_Bij of edge e from the two cell records of t^n: nothing where a side is dry or at a wall; through open boundaries
 // the interior cell's own flux (equilibrium boundary)
+// vel = (u, v) of L and R as edge_process formed them (q / h where h > h_dry): the same quotients the oracle forms
 __device__ __forceinline__ double sediment_edge(const Morph &mp, double g, double h_dry, const EdgeGeom &eg,
-                                                const CellRec &a, const CellRec &b) {
+                                                const CellRec &a, const CellRec &b, const double (&vel)[4]) {
   if (!(a.h > h_dry) || eg.R == -1) return 0.0;
-  const double f2L = mp.formula == 2 ? mp.gn2[eg.L] : 0.0;
-  const SedState si = sed_state(mp, g, a.h, a.qx / a.h, a.qy / a.h, f2L, eg.nx, eg.ny);
+  const double2 fcL = mp.formula == 2 ? mp.cell[eg.L] : make_double2(0.0, 0.0);
+  const SedState si = sed_state(mp, g, a.h, vel[0], vel[1], fcL, eg.nx, eg.ny);
   if (eg.R < 0) return si.q;
   if (!(b.h > h_dry)) return 0.0;
-  const double f2R = mp.formula == 2 ? mp.gn2[eg.R] : 0.0;
-  const SedState sj = sed_state(mp, g, b.h, b.qx / b.h, b.qy / b.h, f2R, eg.nx, eg.ny);
+  const double2 fcR = mp.formula == 2 ? mp.cell[eg.R] : make_double2(0.0, 0.0);
+  const SedState sj = sed_state(mp, g, b.h, vel[2], vel[3], fcR, eg.nx, eg.ny);
   const double sm = dmin2(si.l1, sj.l1), sp = dmax2(si.l2, sj.l2);        // Eq. 15
   if (!(sp - sm > 0.0)) return 0.0;
   return ((sp * si.q - sm * sj.q) + (sp * sm) * (b.z - a.z)) / (sp - sm);  // Eq. 14
@@ -244,8 +248,9 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     const CellRec a = rec[eg.L];
     CellRec b = a;
     if (eg.R >= 0) b = rec[eg.R];
-    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
-    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b);
+    double vel[4];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
+    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
     return;
   }
   const int stride = gridDim.x * kBlock;
@@ -256,8 +261,9 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, 
     CellRec b = a;
     if (eg.R >= 0) b = rec[eg.R];
     if (e + stride < n_edges) eg_next = geom[e + stride];
-    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag);
-    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b);
+    double vel[4];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
+    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
   }
 }
 
@@ -433,21 +439,26 @@ k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
       hn = 0.0;
     }
     double qxn = 0.0, qyn = 0.0;
+    double2 fc = make_double2(0.0, 0.0);             // <kMorph>, MPM-like law: (g/k^2, cbrt(h^{n+1})) for the next step's edges
     if (hn > h_dry) {
       qxn = c.qx - a * dX;
       qyn = c.qy - a * dY;
       const double f2 = gn2[i];
       if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
-        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_rn(hn));
+        const double cb = cbrt_rn(hn);
+        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cb);
         qxn = qxn / D;
         qyn = qyn / D;
+        fc = make_double2(f2, cb);
       }
       const double r = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
       if (r > rate) rate = r;
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
-    if (kMorph)                                      // Eq. 13, S_b = 0: the bed rides in the same record
+    if (kMorph) {                                    // Eq. 13, S_b = 0: the bed rides in the same record
       c.z = c.z - mp.inv1mp * (a * ((dBk[0] + dBk[1]) + dBk[2]));
+      if (mp.formula == 2) mp.cell[i] = fc;
+    }
     rec[i] = c;
     if (kScalars)                                    // Eq. 20, advective part: same gather, same slot order (R-19)
     _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
@@ -721,6 +732,16 @@ k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_per
   const int o = cell_perm[i];
   const CellRec c = rec[i];
   h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
+}
+
+// Morph::cell of the state as it stands (after swe_set_morphology / swe_set_state): what k_cell_update leaves behind
+__global__ void __launch_bounds__(kBlock)
+k_sed_cell_init(const Control *__restrict__ ctl, const CellRec *__restrict__ rec, const double *__restrict__ gn2,
+                double2 *__restrict__ cell, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  const double h = rec[i].h, f2 = gn2[i];
+  cell[i] = (h > ctl->h_dry && f2 > 0.0) ? make_double2(f2, cbrt_rn(h)) : make_double2(0.0, 0.0);
 }
 
 // bed elevation z_B (swe_get_bed), newest state buffer, caller numbering

@@ -75,7 +75,9 @@ struct Morph {                   // morphodynamics (section 3.2 Eq. 3, section 4
   double shields_den;            // g (s-1) d_m: theta = (g/k_st^2) |u|^2 / (h^(1/3) * shields_den)
   double Gm;                     // alpha sqrt((s-1) g d_m^3)
   double inv1mp;                 // 1 / (1 - p)
-  const double *gn2;             // [n_cells] g / k_st^2 (0: no friction law, no bed shear stress)
+  double2 *cell;                 // [n_cells] MPM-like law: (g / k_st^2, cbrt(h)) of the CURRENT state -- the cube root
+                                 // k_cell_update takes for the friction term anyway, kept for the next step's edges
+                                 // (0 where the cell is dry or has no friction law: not used there)
   double *qB;                    // [n_edges] normal sediment flux q_Bij of the step in flight
 };
 
