@@ -232,7 +232,7 @@ def run_reference(args, rank):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "baseline_config": args.config, "n_cells": w.n_cells, "n_edges": w.n_edges,
-                   "time_steps_per_step": 1, "cfl": w.cfl},
+                   "time_steps_per_step": 1, "cfl": w.cfl, "morph": args.morph},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,

@@ -164,3 +164,33 @@ def test_state_on_device_get_bed(gpu):
     assert np.array_equal(s.sediment_fluxes().cpu().numpy(), t.sediment_fluxes())
     s.close()
     t.close()
+
+
+def test_bed_hump_celerity_on_a_fine_mesh(gpu):
+    """Property that needs no oracle and holds at any size: the bed hump of tests/test_oracle_morph.py on a mesh four
+    times finer (12,800 cells, 27,000 time steps, GPU only) travels with the bed-wave speed of the coupled system
+    (27.5 m in 300 s); the finer mesh must come closer to it and keep more of the crest than the 800-cell mesh the
+    oracle is pinned on (28.51 m, crest 0.107 m).  CFL 0.5: with 8 rows of regular right triangles the hydrodynamic
+    scheme is unstable at 0.7 over this many steps (oracle and GPU alike; R-7)."""
+    from test_oracle_morph import bed_wave_celerity
+    lx, H, q, alpha, p, T = 400.0, 10.0, 10.0, 0.2, 0.4, 300.0
+    w = C.dam_break_channel(nx=800, ny=8, lx=lx, ly=4.0, h_left=H, h_right=H, transmissive_ends=True,
+                            q_left=q, q_right=q, t_end=float("inf"))
+    x = M.centroids(w.node_xy, w.tri)[:, 0]
+    w.zb = 0.2 * np.exp(-((x - 200.0) / 20.0) ** 2)
+    w.h = H - w.zb
+    s = gpu.from_workload(w)
+    s.set_morphology(GRASS, alpha, porosity=p)
+    area = s.geometry()[0]
+    info = s.step(-1, T, 0.5)
+    assert info["t"] == T and info["flags"] == 0
+    zb = s.get_bed()
+    xc0 = (w.zb * x * area).sum() / (w.zb * area).sum()
+    xc1 = (zb * x * area).sum() / (zb * area).sum()
+    cb = bed_wave_celerity(q / H, H, alpha, p)
+    print("fine-mesh hump displacement", xc1 - xc0, "expected", cb * T, "crest", zb.max(), "steps", info["steps_done"])
+    assert abs((xc1 - xc0) - cb * T) < abs(28.5084 - cb * T)
+    assert xc1 - xc0 == pytest.approx(cb * T, rel=0.04)
+    assert zb.max() > 0.15
+    assert np.abs(s.get_state()[2]).max() < 1e-2                 # no transverse flow has grown
+    s.close()

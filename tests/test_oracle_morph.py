@@ -3,7 +3,7 @@ DESIGN.md R-20) against what the paper and the mathematics fix: Table 2 evaluate
 finite differences, Eq. 16's two speeds through Vieta's relations of the quadratic they solve, the textbook special cases
 of an HLL flux (consistency, one-sided upwinding, Rusanov), Eq. 13 re-assembled with numpy from the per-edge fluxes, the
 porosity factor, conservation of sediment volume in a closed box, a fixed bed when the module is off, and the celerity
-of a small bed hump under a Grass-like law (the classical quasi-steady result 3 alpha u^3 / ((1-p) h (1-Fr^2))).
+of a small bed hump under a Grass-like law (the bed-wave eigenvalue of the coupled shallow-water / Exner system).
 CPU only."""
 import numpy as np
 import pytest
@@ -166,11 +166,30 @@ def test_uniform_stream_leaves_a_flat_bed_flat(ref):
     assert np.abs(s.get_state()[0] - 2.0).max() < 1e-12
 
 
+def bed_wave_celerity(u, h, alpha, p, g=G):
+    """Exact speed of the bed wave of the coupled shallow-water / Exner system with q_B = alpha u^3 (linearised about a
+    uniform stream): the smallest root in modulus of the characteristic polynomial
+    lambda^3 - 2u lambda^2 + (u^2 - g(h + d)) lambda + g u d = 0,  d = 3 alpha u^2 / (1 - p)
+    of the matrix [[u, h, 0], [g, u, g], [0, d, 0]] acting on (h, u, z_B).  For weak transport it tends to the
+    quasi-steady value 3 alpha u^3 / ((1-p) h (1 - Fr^2))."""
+    d = 3.0 * alpha * u * u / (1.0 - p)
+    r = np.roots([1.0, -2.0 * u, u * u - g * (h + d), g * u * d])
+    r = r[np.abs(r.imag) < 1e-12].real
+    return r[np.argmin(np.abs(r))]
+
+
+def test_bed_wave_celerity_limits():
+    assert bed_wave_celerity(1.0, 10.0, 1e-6, 0.4) == pytest.approx(3e-6 / (0.6 * 10.0 * (1.0 - 1.0 / 98.1)), rel=1e-5)
+    assert bed_wave_celerity(1.0, 10.0, 0.2, 0.4) == pytest.approx(0.09167, rel=1e-3)
+    assert bed_wave_celerity(-1.0, 10.0, 0.2, 0.4) == pytest.approx(-0.09167, rel=1e-3)
+
+
 @pytest.mark.parametrize("direction", [1.0, -1.0])
-def test_bed_hump_travels_with_the_grass_celerity(ref, direction):
-    """A low hump on the bed of a slow deep stream (Fr = 0.1) under q_B = alpha u^3 moves downstream with
-    c_b = 3 alpha u^3 / ((1-p) h (1 - Fr^2)) (quasi-steady flow over a slowly moving bed; e.g. Hudson & Sweby's test).
-    Checked on the centroid of the hump, in both flow directions (Eq. 16 is not symmetric in u_n)."""
+def test_bed_hump_travels_with_the_bed_wave_celerity(ref, direction):
+    """A low hump on the bed of a slow deep stream (Fr = 0.1) under q_B = alpha u^3 moves downstream with the bed-wave
+    speed of the coupled system (27.5 m in 300 s here; the scheme gives 28.5 m on this mesh, 28.3 m on finer ones: the
+    crest, where the water is shallower, runs a little faster than the linearised speed).  Checked on the centroid of
+    the hump, in both flow directions (Eq. 16 is not symmetric in u_n)."""
     lx, H, q, alpha, p = 400.0, 10.0, 10.0, 0.2, 0.4
     w = C.dam_break_channel(nx=200, ny=2, lx=lx, ly=4.0, h_left=H, h_right=H, transmissive_ends=True,
                             q_left=direction * q, q_right=direction * q, t_end=float("inf"))
@@ -185,10 +204,9 @@ def test_bed_hump_travels_with_the_grass_celerity(ref, direction):
     zb = s.get_bed()
     xc0 = (w.zb * x * area).sum() / (w.zb * area).sum()
     xc1 = (zb * x * area).sum() / (zb * area).sum()
-    u = q / H
-    cb = 3.0 * alpha * u ** 3 / ((1.0 - p) * H * (1.0 - u * u / (G * H)))
-    assert cb * T > 25.0
-    print("hump displacement", xc1 - xc0, "expected", direction * cb * T, "crest", zb.max())
-    assert (xc1 - xc0) * direction == pytest.approx(cb * T, rel=0.15)
+    cb = bed_wave_celerity(direction * q / H, H, alpha, p)
+    print("hump displacement", xc1 - xc0, "expected", cb * T, "crest", zb.max())
+    assert abs(cb * T) > 25.0
+    assert xc1 - xc0 == pytest.approx(cb * T, rel=0.05)
     assert (zb * area).sum() == pytest.approx((w.zb * area).sum(), rel=2e-3)     # what left through the ends is tiny
     assert zb.max() > 0.08                                                      # still a hump, not smeared away
