@@ -524,17 +524,127 @@ __device__ __forceinline__ double hydrograph(const double *p, int n_params, doub
 
 // mode 0: start of a step.  mode 1: end of an swe_step call (bookkeeping of the last step only; zeroes the
 // accumulators of k_info).
-__global__ void __launch_bounds__(kCtlThreads)
+constexpr int kCtlPre = 4;            // boundary strings whose members k_step_control gathers up front (one per thread)
+
+__global__ void __launch_bounds__(kCtlThreads, 1)
 k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ string_edges, double *scratch,
                const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
                const double *__restrict__ theta, const CellRec *rec_a, const CellRec *rec_b,
                const double *__restrict__ kst, const double *__restrict__ string_M, int mode) {
   // the pairwise trees run in shared memory when the string fits (same pairs, same order as in global scratch)
   __shared__ double s_tree[kTreeCap];
-  const int ns = ctl->n_strings;
+  __shared__ double s_Q[kCtlPre];
+  __shared__ int s_active;
+  __shared__ double s_t_old;
+  // This block sits on the critical path between two steps, and what it does is a chain of dependent global loads
+  // (control word -> string descriptor -> member list -> geometry -> cell record).  Everything that depends only on
+  // what is in memory when the kernel starts is therefore loaded NOW, by all threads at once: the control fields
+  // (thread 0), every string member's term of both sums (thread j: member j of each string; the conveyance weights
+  // use the state the step will read, buffer `cur` before the flip), the hydrographs (one thread per string).
+  const int ns = ctl->n_strings, pending = ctl->pending, cur = ctl->cur;
+  const double dt_prev = ctl->dt_last, t_now = ctl->t;
+  double c_tend = 0.0, c_cfl = 0.0, c_dtmax = 0.0;
+  long long c_left = 0, c_done = 0;
+  int c_flags = 0, c_pp = 0;
+  unsigned long long c_rate = 0ull;
+  if (threadIdx.x == 0) {
+    c_tend = ctl->t_end; c_cfl = ctl->cfl; c_dtmax = ctl->dt_max; c_left = ctl->steps_left; c_done = ctl->steps_done;
+    c_flags = ctl->flags; c_pp = ctl->ping_pong; c_rate = ctl->rate_bits;
+  }
+  const CellRec *__restrict__ rec = cur ? rec_b : rec_a;
+  auto term_out = [&](const BoundaryString &bs, int j) -> double {   // l * (limited F1) of member j (bookkeeping)
+    if (string_M) return string_M[bs.first + j];         // fused patch step: written by the owning patch
+    const int e = string_edges[bs.first + j];
+    const EdgeGeom eg = geom[e];
+    double F1 = flux[e].F1;
+    if (theta && F1 > 0.0) {                              // nullptr: the records are limited already (k_theta_lazy)
+      const double th = theta[eg.L];
+      if (th < 1.0) F1 = th * F1;
+    }
+    return eg.len * F1;
+  };
+  auto term_in = [&](const BoundaryString &bs, int j) -> double {    // conveyance weight of member j (R-11)
+    const int e = string_edges[bs.first + j];
+    const EdgeGeom eg = geom[e];
+    return (eg.len * k_weight(kst[eg.L])) * pow53(rec[eg.L].h);
+  };
+  bool fast = ns <= kCtlPre;                             // block-uniform: every thread reads the same descriptors
+  double pre[kCtlPre];
+#pragma unroll
+  for (int s = 0; s < kCtlPre; ++s) {
+    pre[s] = 0.0;
+    if (s < ns) {
+      const BoundaryString &bs = strings[s];
+      if (bs.pow2 > (int)blockDim.x) fast = false;
+      else if ((int)threadIdx.x < bs.n_edges) {
+        if (bs.type == kBcOutflowUniform) { if (pending) pre[s] = term_out(bs, threadIdx.x); }
+        else if (bs.type == kBcInflowQ && mode == 0) pre[s] = term_in(bs, threadIdx.x);
+      }
+      if (bs.type == kBcInflowQ && mode == 0 && threadIdx.x == blockDim.x - 1 - s)
+        s_Q[s] = hydrograph(bs.params, bs.n_params, t_now);
+    }
+  }
+  if (fast) {
+    // every string's pairwise tree at once, out of registers: xor-free shuffle tree inside each warp (lane 0 ends up
+    // with v[i] + v[i+1], then + (v[i+2] + v[i+3]), ...: the same pairs in the same order as block_tree_sum; the
+    // padding zeros beyond pow2 add nothing), the warp sums to shared memory, warp s finishes string s.
+    __shared__ double s_part[kCtlPre][32];
+    __shared__ double s_sum[kCtlPre];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int s = 0; s < kCtlPre; ++s) {
+      double x = pre[s];
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) x = x + __shfl_down_sync(0xffffffffu, x, off);
+      if (lane == 0) s_part[s][wid] = x;
+    }
+    __syncthreads();
+    if (wid < kCtlPre) {
+      double x = (lane < (int)(blockDim.x >> 5)) ? s_part[wid][lane] : 0.0;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) x = x + __shfl_down_sync(0xffffffffu, x, off);
+      if (lane == 0) s_sum[wid] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    if (pending)
+      for (int s = 0; s < ns; ++s) {
+        if (strings[s].type == kBcInflowQ) ctl->vol_in += dt_prev * strings[s].Q;
+        else if (strings[s].type == kBcOutflowUniform) ctl->vol_out += dt_prev * s_sum[s & (kCtlPre - 1)];
+      }
+    if (mode == 1) { ctl->pending = 0; ctl->vol = 0.0; ctl->n_wet = 0; ctl->nonfinite = 0; return; }
+    int active = 0, new_pending = 0;
+    const double t = t_now, t_end = c_tend;
+    if (c_left != 0 && t < t_end && !(c_flags & kFlagUnbounded)) {
+      const double r = __longlong_as_double((long long)c_rate);
+      double dt = (r > 0.0) ? c_cfl / r : c_dtmax;
+      dt = fmin(dt, c_dtmax);
+      const double rem = t_end - t;
+      double t_new;
+      if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = t + dt; }
+      if (!isfinite(dt)) {
+        ctl->flags = c_flags | kFlagUnbounded;
+      } else {
+        active = 1;
+        ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
+        ctl->rate_bits = 0ull;
+        ctl->src = cur;                      // the step reads the newest state ...
+        ctl->cur = cur ^ c_pp;               // ... and, when it ping-pongs, writes the other buffer
+        ctl->steps_done = c_done + 1;
+        if (c_left > 0) ctl->steps_left = c_left - 1;
+        new_pending = 1;
+      }
+    }
+    ctl->pending = new_pending;
+    ctl->active = active;
+    if (active)                              // boundary strings at t^n (R-11): Q(t^n) and the conveyance sum
+      for (int s = 0; s < ns; ++s)
+        if (strings[s].type == kBcInflowQ) { strings[s].sumK = s_sum[s & (kCtlPre - 1)]; strings[s].Q = s_Q[s & (kCtlPre - 1)]; }
+    return;
+  }
+  // ---- general path (more than kCtlPre strings, or a string with more members than the block has threads)
   // ---- volume bookkeeping of the previous step, from the (limited) fluxes actually applied
-  if (ctl->pending) {
-    const double dt_prev = ctl->dt_last;
+  if (pending) {
     for (int s = 0; s < ns; ++s) {
       BoundaryString &bs = strings[s];
       if (bs.type == kBcInflowQ) {
@@ -543,20 +653,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
         double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
         for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
           double a = 0.0;
-          if (j < bs.n_edges) {
-            if (string_M) {                      // fused patch step: l * (limited F1), written by the owning patch
-              a = string_M[bs.first + j];
-            } else {
-              const int e = string_edges[bs.first + j];
-              const EdgeGeom eg = geom[e];
-              double F1 = flux[e].F1;
-              if (theta && F1 > 0.0) {              // nullptr: the records are limited already (k_theta_lazy)
-                const double th = theta[eg.L];
-                if (th < 1.0) F1 = th * F1;
-              }
-              a = eg.len * F1;
-            }
-          }
+          if (j < bs.n_edges) a = term_out(bs, j);
           v[j] = a;
         }
         const double sum = block_tree_sum(v, bs.pow2);
@@ -570,32 +667,30 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
     return;
   }
   // ---- S0: dt from the rate of U^n; S4: t += dt (t_end is hit exactly)
-  __shared__ int s_active;
-  __shared__ double s_t_old;
   if (threadIdx.x == 0) {
-    int active = 0;
-    ctl->pending = 0;
-    const double t = ctl->t, t_end = ctl->t_end;
-    if (ctl->steps_left != 0 && t < t_end && !(ctl->flags & kFlagUnbounded)) {
-      const double r = __longlong_as_double((long long)ctl->rate_bits);
-      double dt = (r > 0.0) ? ctl->cfl / r : ctl->dt_max;
-      dt = fmin(dt, ctl->dt_max);
+    int active = 0, new_pending = 0;
+    const double t = t_now, t_end = c_tend;
+    if (c_left != 0 && t < t_end && !(c_flags & kFlagUnbounded)) {
+      const double r = __longlong_as_double((long long)c_rate);
+      double dt = (r > 0.0) ? c_cfl / r : c_dtmax;
+      dt = fmin(dt, c_dtmax);
       const double rem = t_end - t;
       double t_new;
       if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = t + dt; }
       if (!isfinite(dt)) {
-        ctl->flags |= kFlagUnbounded;
+        ctl->flags = c_flags | kFlagUnbounded;
       } else {
         active = 1;
         ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
         ctl->rate_bits = 0ull;
-        ctl->src = ctl->cur;                 // the step reads the newest state ...
-        ctl->cur ^= ctl->ping_pong;          // ... and, when it ping-pongs, writes the other buffer
-        ctl->steps_done += 1;
-        if (ctl->steps_left > 0) ctl->steps_left -= 1;
-        ctl->pending = 1;
+        ctl->src = cur;                      // the step reads the newest state ...
+        ctl->cur = cur ^ c_pp;               // ... and, when it ping-pongs, writes the other buffer
+        ctl->steps_done = c_done + 1;
+        if (c_left > 0) ctl->steps_left = c_left - 1;
+        new_pending = 1;
       }
     }
+    ctl->pending = new_pending;
     ctl->active = active;
     s_active = active;
     s_t_old = t;
@@ -603,18 +698,13 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   __syncthreads();
   if (!s_active) return;
   // ---- boundary strings at t^n (R-11): Q(t^n) and the conveyance sum over the string
-  const CellRec *__restrict__ rec = ctl->src ? rec_b : rec_a;
   for (int s = 0; s < ns; ++s) {
     BoundaryString &bs = strings[s];
     if (bs.type != kBcInflowQ) continue;
     double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
     for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
       double a = 0.0;
-      if (j < bs.n_edges) {
-        const int e = string_edges[bs.first + j];
-        const EdgeGeom eg = geom[e];
-        a = (eg.len * k_weight(kst[eg.L])) * pow53(rec[eg.L].h);
-      }
+      if (j < bs.n_edges) a = term_in(bs, j);
       v[j] = a;
     }
     const double sum = block_tree_sum(v, bs.pow2);

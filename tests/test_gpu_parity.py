@@ -9,6 +9,7 @@ import numpy as np
 import pytest
 
 from workloads import configs as C
+from workloads import mesh as M
 
 pytestmark = pytest.mark.gpu
 
@@ -466,3 +467,52 @@ def test_auto_follows_a_spreading_flood(gpu, ref):
     assert seen[0] == gpu.VARIANT_PATCH and seen[-1] == gpu.VARIANT_THREE_PASS, seen
     assert ig["n_wet"] == w.n_cells
     s.close()
+
+
+def _many_strings_workload(nx, ny, n_in, n_out):
+    """A wide basin with the west side cut into n_in INFLOW_Q strings and the east side into n_out OUTFLOW_UNIFORM
+    strings (string ids interleaved), walls north and south."""
+    lx, ly = 4.0 * nx, 2.0 * ny
+    node_xy, tri = M.structured_tri_mesh(nx, ny, lx, ly, alternate=True)
+    n = tri.shape[0]
+    ctr = M.centroids(node_xy, tri)
+    rng = np.random.default_rng(77)
+    zb = -0.002 * ctr[:, 0] + 0.01 * rng.standard_normal(n)
+    w = C._finish(f"many-strings-{nx}x{ny}-{n_in}+{n_out}", node_xy, tri, zb, np.full(n, 30.0),
+                  np.full(n, 0.8) + 0.05 * rng.random(n), cfl=0.7, dt_max=2.0)
+    w.hu = 0.5 * w.h
+    def code(mx, my):
+        out = np.full(mx.shape, M.BC_WALL)
+        west, east = mx < 1e-9, mx > lx - 1e-9
+        seg_w = np.minimum((my / ly * n_in).astype(int), n_in - 1)
+        seg_e = np.minimum((my / ly * n_out).astype(int), n_out - 1)
+        out[west] = [M.bc_string(2 * k) for k in seg_w[west]]
+        out[east] = [M.bc_string(2 * k + 1) for k in seg_e[east]]
+        return out
+    C._set_boundary_codes(w, code)
+    for k in range(n_in):
+        q = (0.4 + 0.1 * k) * ly / n_in
+        w.strings.append((2 * k, C.BC_INFLOW_Q, np.array([0.0, q, 5.0, 2.0 * q])))
+    for k in range(n_out):
+        w.strings.append((2 * k + 1, C.BC_OUTFLOW_UNIFORM, np.array([0.002])))
+    return w
+
+
+@pytest.mark.parametrize("nx,ny,n_in,n_out", [(6, 40, 3, 3),        # six strings: general path of k_step_control
+                                               (4, 1500, 1, 1),     # 1500 members: more than the control block's threads
+                                               (3, 4500, 1, 1),     # 4500 members: pairwise tree in global scratch
+                                               (8, 64, 2, 2)])      # four short strings: the up-front path
+def test_boundary_string_sums_many_and_long_strings(gpu, ref, nx, ny, n_in, n_out):
+    """R-11: the fixed-shape pairwise sums over boundary strings (conveyance weights, outflow volume) and the volume
+    bookkeeping, for string counts and sizes on both sides of the limits of k_step_control's up-front path."""
+    w = _many_strings_workload(nx, ny, n_in, n_out)
+    s, o = make(gpu, w), ref.RefSolver(w)
+    for n in (1, 7, 40):
+        ig, io = s.step(n, float("inf"), w.cfl), o.step(n, float("inf"), w.cfl)
+        assert_state_close(s.get_state(), o.get_state(), w.name)
+        check_info(ig, io)
+        assert ig["vol_in"] > 0.0 and ig["vol_out"] > 0.0
+        assert abs(ig["vol_in"] - io["vol_in"]) <= 1e-13 * io["vol_in"]
+        assert abs(ig["vol_out"] - io["vol_out"]) <= 1e-13 * io["vol_out"]
+    s.close()
+    o.close()
