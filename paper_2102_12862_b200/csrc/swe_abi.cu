@@ -311,7 +311,7 @@ void internal_tables(const HostMesh &hm, std::vector<EdgeGeom> &geom, std::vecto
 }
 
 int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
-  const int64_t nc = mesh->n_cells, nn = mesh->n_nodes;
+  const int64_t nc = mesh->n_cells;
   c->nc = nc;
   if (params) c->prm = *params; else swe_params_default(&c->prm);
   const swe_params &p = c->prm;
