@@ -270,7 +270,7 @@ def main():
     N, E, T = w.n_cells, w.n_edges, args.time_steps
     t_create = time.perf_counter()
     s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells,
-                        renumber=args.renumber, n_species=args.species)
+                        renumber=args.renumber, n_species=args.species, morphology=bool(args.morph))
     if args.species:
         from workloads import mesh as WM
         ctr = WM.centroids(w.node_xy, w.tri)
@@ -286,7 +286,7 @@ def main():
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     stream = torch.cuda.current_stream(dev)
-    s_kernels, patch_stats = s.step_kernels(), s.patch_stats()
+    s_kernels, patch_stats, s_workspace_bytes = s.step_kernels(), s.patch_stats(), s.workspace_nbytes
 
     # ---- device-resident arm: W warm-up steps, then exactly K steps between barrier + synchronize on both sides
     for _ in range(args.warmup):
@@ -439,7 +439,7 @@ def main():
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
-                       "l2": "working set (%.0f MB) larger than L2, no flush" % (P.workspace_bytes(N, E) / 1e6),
+                       "l2": "working set (%.0f MB) larger than L2, no flush" % (s_workspace_bytes / 1e6),
                        "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "morph": args.morph, "stage": args.stage, "step_kernels": s_kernels, "patch": patch_stats},
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),

@@ -32,7 +32,7 @@ enum {
   SWE_OK = 0,
   SWE_EINVAL = -1,     /* null / out-of-range argument                                             */
   SWE_EMESH = -2,      /* non-CCW or zero-area cell, non-conforming mesh, inconsistent tables       */
-  SWE_ENOMEM = -3,     /* host allocation failed, or the lent workspace is too small                */
+  SWE_ENOMEM = -3,     /* host or device allocation failed, or the lent workspace is too small      */
   SWE_ECUDA = -4,      /* a CUDA call failed (no device, launch error, ...); see swe_last_error     */
   SWE_ENONFINITE = -5  /* swe_step found a non-finite state value at the end of the call            */
 };
@@ -49,7 +49,9 @@ enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1, SWE_RENUMBER_RCM = 2 /* r
 enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta -> CSR gather + update */,
        SWE_VARIANT_PATCH = 2 /* one fused kernel per step over shared-memory mesh patches */ };
 /* swe_step_info.flags */
-enum { SWE_FLAG_NONFINITE = 1, SWE_FLAG_DT_UNBOUNDED = 2 };
+enum { SWE_FLAG_NONFINITE = 1, SWE_FLAG_DT_UNBOUNDED = 2 /* whole domain dry and dt_max = +inf */,
+       SWE_FLAG_STALLED = 4 /* Eq. 21 gave dt <= 0 or t + dt == t (a rate of +inf from a non-finite state, or dt below
+                               ulp(t)): swe_step stops stepping and returns, with this flag in info */ };
 
 /* The mesh (section 4.1, Fig. 2): conforming triangulation, cell i with neighbours j = 1..3
  * across edges Gamma_ij.  All pointers are HOST pointers; everything is copied during swe_create and
@@ -76,14 +78,16 @@ typedef struct {
                            1: they take DEVICE pointers (e.g. torch tensors), read/written on stream  */
   int steps_per_graph;  /* time steps captured per CUDA graph launch; default 32; 0 = no graph       */
   int variant;          /* SWE_VARIANT_*; default AUTO                                               */
-  int patch_cells;      /* cells per patch of the fused step; 0 = default (384)                      */
+  int patch_cells;      /* cells per patch of the fused step, 32..1024 (one thread per own cell);
+                           0 = default (256; less on meshes that would not fill the SMs)             */
   int n_species;        /* passive scalar species advected with the flow (0..5); default 0    */
+  int morphology;       /* 1: reserve room for the mobile-bed module (swe_set_morphology); default 0 */
   void *cuda_stream;    /* cudaStream_t all work is enqueued on; NULL = the legacy default stream    */
   void *workspace;      /* DEVICE memory lent by the caller for the context's lifetime (e.g. a torch
-                           uint8 tensor), 256-byte aligned, or NULL: the library then cudaMallocs.
-                           (The patch tables of the fused step, whose size is known only once they are
-                           built, are always allocated by the library.)                             */
-  size_t workspace_bytes; /* size of workspace; must be >= swe_workspace_bytes(n_cells, n_edges)     */
+                           uint8 tensor), 256-byte aligned: EVERY device array of the context is carved
+                           from it (state, tables, patch blobs, scalars, mobile bed, control block).
+                           NULL: the library makes one cudaMalloc of the same size instead.          */
+  size_t workspace_bytes; /* size of workspace; must be >= swe_workspace_bytes(mesh, params)         */
 } swe_params;
 
 typedef struct {
@@ -98,9 +102,10 @@ typedef struct {
 /* Fills *p with the defaults named above. */
 void swe_params_default(swe_params *p);
 
-/* Device bytes a context for a mesh of this size needs (an upper bound that also covers tables the
- * library builds itself).  n_edges <= 0: assume the worst case 3 * n_cells. */
-size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges);
+/* Device bytes a context for this mesh and these parameters needs (params == NULL: defaults; workspace / stream
+ * fields are ignored).  Runs the host part of swe_create (validation, renumbering, patch tables) to size every
+ * array, with no CUDA call; returns 0 when swe_create would reject the arguments (swe_last_error(NULL)). */
+size_t swe_workspace_bytes(const swe_mesh *mesh, const swe_params *params);
 
 /* Validates the mesh (CCW, positive area, both tables consistent and conforming), computes the geometry
  * of section 4.1 (areas, edge lengths, unit normals L->R), renumbers cells and edges (Morton order of the
@@ -196,9 +201,11 @@ const char *swe_step_kernel_name(const swe_ctx *ctx, int k);
 /* algorithmic DRAM bytes per launch of kernel k of the step: every datum the kernel needs counted once at the size
  * of the record that carries it; re-reads of halo cells / duplicated records are NOT counted */
 int64_t swe_algorithmic_bytes(const swe_ctx *ctx, int k);
-/* out[0..8] = variant, patches, cells per patch, dynamic shared memory per block [bytes], sum over patches of local
- * cells, sum over patches of local edges, largest local cell count, largest local edge count, and the number of
- * patch-steps since swe_create in which a block found its whole patch dry and skipped the flux work.  It synchronises. */
+/* out[0..11] = variant, patches, cells per patch, dynamic shared memory per block [bytes], sum over patches of local
+ * cells, sum over patches of local edges, largest local cell count, largest local edge count, the number of
+ * patch-steps since swe_create in which a block found its whole patch dry and skipped the flux work, the
+ * __launch_bounds__ minimum blocks per SM of the kernel instance, bytes per patch blob, bytes of a blob that are
+ * staged into shared memory.  It synchronises. */
 int swe_get_patch_stats(swe_ctx *ctx, int64_t *out, int n_out);
 
 #ifdef __cplusplus

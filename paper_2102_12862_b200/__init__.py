@@ -26,7 +26,7 @@ OK, EINVAL, EMESH, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4, -5
 EDGE_WALL, EDGE_TRANSMISSIVE = -1, -2
 BC_NONE, BC_INFLOW_Q, BC_OUTFLOW_UNIFORM = 0, 1, 2
 RENUMBER_NONE, RENUMBER_MORTON, RENUMBER_RCM = 0, 1, 2
-FLAG_NONFINITE, FLAG_DT_UNBOUNDED = 1, 2
+FLAG_NONFINITE, FLAG_DT_UNBOUNDED, FLAG_STALLED = 1, 2, 4
 VARIANT_AUTO, VARIANT_THREE_PASS, VARIANT_PATCH = 0, 1, 2
 
 _f64p = C.POINTER(C.c_double)
@@ -51,7 +51,7 @@ class SweMesh(C.Structure):
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("h_dry", C.c_double), ("dt_max", C.c_double), ("renumber", C.c_int),
                 ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("variant", C.c_int), ("patch_cells", C.c_int),
-                ("n_species", C.c_int), ("cuda_stream", C.c_void_p),
+                ("n_species", C.c_int), ("morphology", C.c_int), ("cuda_stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -83,7 +83,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.swe_params_default.argtypes = [C.POINTER(SweParams)]
         L.swe_params_default.restype = None
-        L.swe_workspace_bytes.argtypes = [C.c_int64, C.c_int64]
+        L.swe_workspace_bytes.argtypes = [C.POINTER(SweMesh), C.POINTER(SweParams)]
         L.swe_workspace_bytes.restype = C.c_size_t
         L.swe_create.argtypes = [C.POINTER(SweMesh), C.POINTER(SweParams), C.POINTER(C.c_void_p)]
         L.swe_set_boundary.argtypes = [C.c_void_p, C.c_int, C.c_int, _f64p, C.c_int]
@@ -130,7 +130,8 @@ class Solver:
 
     def __init__(self, node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, *, g=9.81, h_dry=1e-3,
                  dt_max=float("inf"), renumber=RENUMBER_MORTON, state_on_device=False, steps_per_graph=32,
-                 device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0, n_species=0):
+                 device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0, n_species=0,
+                 morphology=False, workspace_bytes=None):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -155,14 +156,19 @@ class Solver:
         prm.g, prm.h_dry, prm.dt_max = float(g), float(h_dry), float(dt_max)
         prm.renumber, prm.state_on_device, prm.steps_per_graph = int(renumber), int(bool(state_on_device)), int(steps_per_graph)
         prm.variant, prm.patch_cells, prm.n_species = int(variant), int(patch_cells), int(n_species)
+        prm.morphology = int(bool(morphology))
         self.n_species = int(n_species)
         self.stream = torch.cuda.current_stream(self.device)
         prm.cuda_stream = self.stream.cuda_stream
         self.workspace = None
         if not own_workspace:
-            nbytes = int(L.swe_workspace_bytes(self.n_cells, n_edges))
+            # every device array of the context lives in this torch tensor (workspace_bytes: tests lend too little)
+            nbytes = int(L.swe_workspace_bytes(C.byref(mesh), C.byref(prm))) if workspace_bytes is None else int(workspace_bytes)
+            if nbytes == 0:
+                raise SweError(EINVAL, L.swe_last_error(None).decode())
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             prm.workspace, prm.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.workspace_nbytes = 0 if self.workspace is None else int(self.workspace.numel())
         self.state_on_device = bool(state_on_device)
         h = C.c_void_p()
         rc = L.swe_create(C.byref(mesh), C.byref(prm), C.byref(h))
@@ -319,10 +325,11 @@ class Solver:
         return {nm: int(lib().swe_algorithmic_bytes(self._h, k)) for k, nm in enumerate(self.step_kernels())}
 
     def patch_stats(self):
-        out = (C.c_int64 * 9)()
-        self._check(lib().swe_get_patch_stats(self._h, out, 9))
+        out = (C.c_int64 * 12)()
+        self._check(lib().swe_get_patch_stats(self._h, out, 12))
         keys = ("variant", "patches", "patch_cells", "smem_bytes", "sum_local_cells", "sum_local_edges",
-                "max_local_cells", "max_local_edges", "patch_steps_skipped")
+                "max_local_cells", "max_local_edges", "patch_steps_skipped", "min_blocks_per_sm", "blob_stride",
+                "blob_staged_bytes")
         return dict(zip(keys, (int(v) for v in out)))
 
     @property
@@ -355,9 +362,23 @@ def host_preprocess(node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=N
     return st, cp, ep[:st["n_edges"]]
 
 
-def workspace_bytes(n_cells, n_edges=0):
-    """swe_workspace_bytes: device bytes of a context of this size."""
-    return int(lib().swe_workspace_bytes(int(n_cells), int(n_edges)))
+def workspace_bytes(node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, **params):
+    """swe_workspace_bytes: device bytes of a context for this mesh and these swe_params fields (renumber, variant,
+    patch_cells, n_species, morphology); 0 if swe_create would reject them.  Needs no GPU."""
+    node_xy = np.ascontiguousarray(node_xy, np.float64)
+    tri = np.ascontiguousarray(tri, np.int32)
+    n = int(tri.shape[0])
+    ec = None if edge_cell is None else np.ascontiguousarray(edge_cell, np.int32)
+    ce = None if cell_edge is None else np.ascontiguousarray(cell_edge, np.int32)
+    zb = np.ascontiguousarray(zb if zb is not None else np.zeros(n), np.float64)
+    kst = np.ascontiguousarray(kst if kst is not None else np.full(n, np.inf), np.float64)
+    mesh = SweMesh(int(node_xy.shape[0]), n, 0 if ec is None else int(ec.shape[0]), _p(node_xy, _f64p), _p(tri, _i32p),
+                   _p(ec, _i32p), _p(ce, _i32p), _p(zb, _f64p), _p(kst, _f64p))
+    prm = SweParams()
+    lib().swe_params_default(C.byref(prm))
+    for k, v in params.items():
+        setattr(prm, k, int(v))
+    return int(lib().swe_workspace_bytes(C.byref(mesh), C.byref(prm)))
 
 
 def device_cbrt(x):

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswe_b200.so")
 SRC = [os.path.join(CSRC, "swe_abi.cu")]
-DEPS = SRC + [os.path.join(CSRC, f) for f in ("swe_kernels.cuh", "swe_patch_kernel.cuh", "swe_cbrt.cuh", "swe_types.h", "mesh_prep.hpp", "patch_prep.hpp")] + [
+DEPS = SRC + [os.path.join(CSRC, f) for f in ("swe_kernels.cuh", "swe_patch2_kernel.cuh", "swe_cbrt.cuh", "swe_types.h", "mesh_prep.hpp", "patch_blob.hpp")] + [
     os.path.join(os.path.dirname(HERE), "include", "swe.h")]
 
 NVCC_FLAGS = [

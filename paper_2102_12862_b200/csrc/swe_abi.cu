@@ -1,5 +1,9 @@
 // C-ABI of include/swe.h: context, workspace carving, upload, CUDA-graph step loop.  Host logic only;
-// every step of the numerical path runs in the kernels of swe_kernels.cuh.
+// every step of the numerical path runs in the kernels of swe_kernels.cuh / swe_patch2_kernel.cuh.
+//
+// Device memory: ONE block, laid out by `Layout` from the sizes a host-only planning pass (`make_plan`) finds --
+// the caller's workspace (swe_params.workspace, sized by swe_workspace_bytes, which runs the same planning pass), or,
+// when none is lent, one cudaMalloc of that size.  Nothing else is allocated on the device while a context lives.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -14,9 +18,9 @@
 
 #include "../../include/swe.h"
 #include "mesh_prep.hpp"
-#include "patch_prep.hpp"
+#include "patch_blob.hpp"
 #include "swe_kernels.cuh"
-#include "swe_patch_kernel.cuh"
+#include "swe_patch2_kernel.cuh"
 #include "swe_types.h"
 
 using namespace swe;
@@ -27,13 +31,30 @@ thread_local std::string g_create_error;
 
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+constexpr int kParamsPool = 16384;        // doubles reserved for the boundary strings' parameter tables (hydrographs)
+constexpr size_t kSmemPerSM = 228 * 1024, kSmemPerBlockMax = 227 * 1024, kSmemBlockReserve = 1024;
 
-// Sizes of the O(N) device arrays carved out of the workspace, in carving order.
+// What the planning pass finds out about a context: every size that decides the device layout.
+struct Sizes {
+  int64_t nc = 0, ne = 0;
+  int n_species = 0;
+  bool morph = false;                     // room for the mobile-bed module (swe_params.morphology)
+  int64_t n_strings = 0, n_string_edges = 0, scratch = 0;
+  int64_t n_patches = 0, blob_bytes = 0;  // fused patch step (0: the context has no patch step)
+};
+
+// Offsets of the device arrays inside the workspace, in carving order.
 struct Layout {
-  size_t rec, rec_b, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, total;
-  Layout(int64_t nc, int64_t ne) {
+  size_t rec, rec_b, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, drain_flag;
+  size_t ctl, info_part, info_ticket, strings, string_edges, scratch, params, slot_string, string_M;
+  size_t qa[kMaxSpecies], qb[kMaxSpecies], phi_up[kMaxSpecies], scalar_stage;
+  size_t blob, pflag;
+  size_t qB, mcell;
+  size_t total;
+  explicit Layout(const Sizes &z) {
     size_t o = 0;
-    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(std::max<size_t>(bytes, 16)); return at; };
+    const size_t nc = (size_t)z.nc, ne = (size_t)z.ne, nse = (size_t)std::max<int64_t>(1, z.n_string_edges);
     rec = take(sizeof(CellRec) * nc);
     rec_b = take(sizeof(CellRec) * nc);     // second state buffer of the fused patch step
     geom = take(sizeof(EdgeGeom) * ne);
@@ -41,12 +62,82 @@ struct Layout {
     cell_edge = take(sizeof(int4) * nc);
     area = take(8 * nc); inv_area = take(8 * nc); gn2 = take(8 * nc); kst = take(8 * nc); theta = take(8 * nc);
     cell_perm = take(4 * nc); edge_perm = take(4 * ne);
-    stage = take(24 * nc);
+    stage = take(std::max(24 * nc, 16 * ne));           // host <-> device staging of set / get calls
+    drain_flag = take(nc + 16);                         // read four bytes at a time
+    ctl = take(sizeof(Control));
+    info_part = take(sizeof(InfoPartial) * kInfoMaxBlocks);
+    info_ticket = take(sizeof(unsigned int));
+    strings = take(sizeof(BoundaryString) * (size_t)std::max<int64_t>(1, z.n_strings));
+    string_edges = take(4 * nse);
+    scratch = take(8 * (size_t)std::max<int64_t>(1, z.scratch));
+    params = take(8 * (size_t)kParamsPool);
+    slot_string = take(4 * nse);
+    string_M = take(8 * nse);
+    for (int sp = 0; sp < kMaxSpecies; ++sp) {
+      qa[sp] = qb[sp] = phi_up[sp] = 0;
+      if (sp < z.n_species) { qa[sp] = take(8 * nc); qb[sp] = take(8 * nc); phi_up[sp] = take(8 * ne); }
+    }
+    scalar_stage = z.n_species > 0 ? take(8 * nc) : 0;
+    blob = z.n_patches > 0 ? take((size_t)z.blob_bytes) : 0;
+    pflag = z.n_patches > 0 ? take(2 * (size_t)kPflagBytes * (size_t)z.n_patches) : 0;
+    qB = z.morph ? take(8 * ne) : 0;
+    mcell = z.morph ? take(16 * nc) : 0;
     total = o;
   }
 };
 
 inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
+
+// ---- the fused patch kernel's instantiations: one thread per own cell (P = threads), __launch_bounds__ minimum
+// blocks per SM chosen from what the shared memory admits (it only caps the registers)
+typedef void (*PatchKernel)(Control *, Patch2Args);
+struct PatchInst { int T, min_blocks; bool scalars; PatchKernel fn; };   // T threads per block >= cells per patch
+#define SWE_PI(P, B) {P, B, false, k_patch2<P, B, false>}
+#define SWE_PIS(P, B) {P, B, true, k_patch2<P, B, true>}
+const PatchInst kPatchInst[] = {
+    SWE_PI(128, 8), SWE_PI(128, 6), SWE_PI(128, 4), SWE_PI(192, 5), SWE_PI(192, 4), SWE_PI(192, 3), SWE_PI(256, 4), SWE_PI(256, 3),
+    SWE_PI(256, 2), SWE_PI(384, 2), SWE_PI(384, 1), SWE_PI(512, 2), SWE_PI(512, 1), SWE_PI(1024, 1), SWE_PI(64, 8), SWE_PI(32, 8),
+    SWE_PIS(128, 4), SWE_PIS(128, 2), SWE_PIS(192, 3), SWE_PIS(192, 2), SWE_PIS(256, 3), SWE_PIS(256, 2), SWE_PIS(256, 1), SWE_PIS(384, 1), SWE_PIS(512, 1),
+    SWE_PIS(1024, 1), SWE_PIS(64, 4), SWE_PIS(32, 4)};
+#undef SWE_PI
+#undef SWE_PIS
+
+inline int patch_threads(int P) {           // the smallest block size of an instance that gives every own cell a thread
+  int T = 1 << 30;
+  for (const PatchInst &pi : kPatchInst) if (pi.T >= P && pi.T < T) T = pi.T;
+  return T;
+}
+
+// the instantiation with the most blocks per SM that the shared memory of one block admits (force_blocks > 0: that one)
+inline const PatchInst *pick_patch_kernel(int T, bool scalars, size_t smem, int force_blocks) {
+  const int fit = (int)(kSmemPerSM / (smem + kSmemBlockReserve));
+  const PatchInst *best = nullptr;
+  for (const PatchInst &pi : kPatchInst) {
+    if (pi.T != T || pi.scalars != scalars) continue;
+    if (force_blocks > 0) { if (pi.min_blocks == force_blocks) return &pi; continue; }
+    if (pi.min_blocks <= std::max(1, fit) && (!best || pi.min_blocks > best->min_blocks)) best = &pi;
+  }
+  if (!best)
+    for (const PatchInst &pi : kPatchInst)
+      if (pi.T == T && pi.scalars == scalars && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
+  return best;
+}
+
+// Everything the host works out before the first CUDA call (shared by swe_workspace_bytes and swe_create)
+struct Plan {
+  HostMesh hm;
+  Sizes z;
+  std::vector<BoundaryString> strings;
+  std::vector<int32_t> flat;             // string_edges[]: members of all strings, internal edge ids
+  std::vector<int32_t> slot_string;      // string id of every position of flat[]
+  std::vector<EdgeGeom> geom;            // internal numbering
+  std::vector<int32_t> ce4;
+  std::vector<double> area, inv_area, gn2, kst;
+  int variant = SWE_VARIANT_THREE_PASS;  // the variant the context starts with
+  bool has_patch = false, auto_mode = false;
+  PatchBlobs pb;
+  size_t patch_smem = 0;
+};
 
 }  // namespace
 
@@ -62,34 +153,37 @@ struct swe_ctx {
   double *area = nullptr, *inv_area = nullptr, *gn2 = nullptr, *kst = nullptr, *theta = nullptr;
   int *cell_perm = nullptr, *edge_perm = nullptr;
   double *stage = nullptr;
-  // small device allocations owned by the library
   Control *d_ctl = nullptr;
-  Control *h_ctl = nullptr;          // pinned
+  Control *h_ctl = nullptr;          // pinned host memory
   BoundaryString *d_strings = nullptr;
   int *d_string_edges = nullptr;
   double *d_scratch = nullptr;
+  double *d_params = nullptr;        // pool of kParamsPool doubles; bump-allocated by swe_set_boundary
+  int64_t params_used = 0;
   std::vector<BoundaryString> strings;
-  std::vector<double *> d_params;
-  // fused patch step (variant SWE_VARIANT_PATCH): tables built by patch_prep.hpp, allocated by the library
+  std::vector<int64_t> param_off, param_cap;     // per string: its slice of the pool
+  // fused patch step (variant SWE_VARIANT_PATCH)
   int variant = 0;
-  PatchTables pt;                    // host copy (headers kept for statistics; the big vectors are released)
-  PatchHeader *d_hdr = nullptr; int32_t *d_halo_ids = nullptr; double *d_halo_area = nullptr;
-  PatchEdge *d_pedge = nullptr; uint4 *d_pce = nullptr; int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
+  bool has_patch = false;
+  BlobLayout blay{};
+  unsigned char *d_blob = nullptr, *d_pflag = nullptr;
+  int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
+  int n_patches = 0, patch_threads = 0; size_t patch_smem = 0;
+  int64_t patch_sum_loc = 0, patch_sum_e = 0; int patch_max_loc = 0, patch_max_e = 0, patch_min_blocks = 0;
+  PatchKernel patch_kernel = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
   int cell_grid = 148 * 4;           // resident blocks of the persistent k_cell_update
   int edge_grid = 148 * 5;           // resident blocks of the persistent k_edge_flux (set from the occupancy API)
   int base_edge_grid = 0, base_cell_grid = 0, sms = 148;
   Morph mp{};                        // morphodynamics (swe_set_morphology); formula 0 = fixed bed
+  bool morph_reserved = false;
   uint8_t *d_drain_flag = nullptr;   // three-pass step: cells flagged as possible drainers (lazy theta)
-  Scalars sc{};                      // passive scalars: device arrays owned by the library (cudaMalloc)
+  Scalars sc{};                      // passive scalars
   double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
-  int32_t *d_patch_nbr = nullptr; uint8_t *d_dry = nullptr;   // d_dry: [2][n_patches]
-  int n_patches = 0; size_t patch_smem = 0;
-  void (*patch_kernel)(Control *, PatchArgs) = nullptr;
   int64_t alg_bytes_base[2] = {};        // three-pass k_edge_flux / k_cell_update without the mobile bed
   int64_t alg_bytes_v[3][4] = {};        // [variant][kernel]: algorithmic DRAM bytes per launch of the kernels of a step
+  int64_t survey_bytes_v[3][4] = {};     // the same on SURVEY.md section 8(d)'s per-cell figures
   bool auto_mode = false;                // AUTO with both variants available: chosen at swe_set_state (wet fraction)
-  cudaGraph_t graph = nullptr;
   cudaGraphExec_t graph_exec_v[3] = {nullptr, nullptr, nullptr};   // by variant
   int steps_per_graph = 0;
   int64_t launches = 0;
@@ -110,22 +204,28 @@ namespace {
 
 // the kernels of one time step, in stream order; ev (nullable) = n_step_kernels + 1 events recorded around them
 constexpr int kMaxStepKernels = 4;
-// (two edges per thread, i.e. two gather chains in flight, needs 80 registers: measured slower)
-constexpr int kPatchThreads = 256;
 const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"};
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
 
 inline int n_step_kernels(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH ? 2 : 4; }
 
-PatchArgs patch_args(const swe_ctx *c) {
-  PatchArgs a;
-  a.hdr = c->d_hdr; a.halo_ids = c->d_halo_ids; a.halo_area = c->d_halo_area; a.pedge = c->d_pedge; a.pce = c->d_pce;
-  a.rec_a = c->rec; a.rec_b = c->rec_b; a.area = c->area; a.inv_area = c->inv_area; a.gn2 = c->gn2; a.kst = c->kst;
+Patch2Args patch_args(const swe_ctx *c) {
+  Patch2Args a;
+  a.blob = c->d_blob; a.L = c->blay;
+  a.rec_a = c->rec; a.rec_b = c->rec_b; a.kst = c->kst;
   a.strings = c->d_strings; a.slot_string = c->d_slot_string; a.string_M = c->d_string_M;
-  a.patch_nbr = c->d_patch_nbr; a.dry_a = c->d_dry; a.dry_b = c->d_dry + c->n_patches;
+  a.pflag_a = c->d_pflag; a.pflag_b = c->d_pflag + (size_t)kPflagBytes * (size_t)c->n_patches;
+  a.n_cells = (int32_t)c->nc;
   a.sc = c->sc;
-  a.max_loc = c->pt.max_loc; a.max_c1 = c->pt.max_c1; a.max_e = c->pt.max_e; a.max_eown = c->pt.max_eown;
   return a;
+}
+
+// dry flags of the patches from the state as it stands (after swe_set_state / swe_set_scalars / a variant switch)
+void launch_patch_flags(swe_ctx *c) {
+  const Patch2Args a = patch_args(c);
+  k_patch2_own_flags<256><<<c->n_patches, 256, 0, c->stream>>>(c->d_ctl, a);
+  k_patch2_nbr_flags<<<grid_for(c->n_patches), kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
+  c->launches += 2;
 }
 
 void launch_control(swe_ctx *c, cudaStream_t s, int mode) {
@@ -139,7 +239,7 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
   launch_control(c, s, 0);
   if (ev) cudaEventRecord(ev[1], s);
   if (c->variant == SWE_VARIANT_PATCH) {
-    c->patch_kernel<<<c->n_patches, kPatchThreads, c->patch_smem, s>>>(c->d_ctl, patch_args(c));
+    c->patch_kernel<<<c->n_patches, c->patch_threads, c->patch_smem, s>>>(c->d_ctl, patch_args(c));
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
@@ -192,33 +292,7 @@ int read_control(swe_ctx *c) {   // device -> pinned host, synchronises the stre
 void release(swe_ctx *c) {
   if (!c) return;
   for (auto &ge : c->graph_exec_v) if (ge) cudaGraphExecDestroy(ge);
-  if (c->graph) cudaGraphDestroy(c->graph);
-  for (double *p : c->d_params) if (p) cudaFree(p);
-  if (c->d_ctl) cudaFree(c->d_ctl);
   if (c->h_ctl) cudaFreeHost(c->h_ctl);
-  if (c->d_strings) cudaFree(c->d_strings);
-  if (c->d_string_edges) cudaFree(c->d_string_edges);
-  if (c->d_scratch) cudaFree(c->d_scratch);
-  if (c->d_hdr) cudaFree(c->d_hdr);
-  if (c->d_halo_ids) cudaFree(c->d_halo_ids);
-  if (c->d_halo_area) cudaFree(c->d_halo_area);
-  if (c->d_pedge) cudaFree(c->d_pedge);
-  if (c->d_pce) cudaFree(c->d_pce);
-  if (c->d_slot_string) cudaFree(c->d_slot_string);
-  if (c->d_string_M) cudaFree(c->d_string_M);
-  if (c->d_info_part) cudaFree(c->d_info_part);
-  if (c->d_info_ticket) cudaFree(c->d_info_ticket);
-  for (int sp = 0; sp < kMaxSpecies; ++sp) {
-    if (c->sc.qa[sp]) cudaFree(c->sc.qa[sp]);
-    if (c->sc.qb[sp]) cudaFree(c->sc.qb[sp]);
-    if (c->sc.phi_up[sp]) cudaFree(c->sc.phi_up[sp]);
-  }
-  if (c->d_scalar_stage) cudaFree(c->d_scalar_stage);
-  if (c->d_drain_flag) cudaFree(c->d_drain_flag);
-  if (c->mp.qB) cudaFree(c->mp.qB);
-  if (c->mp.cell) cudaFree(c->mp.cell);
-  if (c->d_patch_nbr) cudaFree(c->d_patch_nbr);
-  if (c->d_dry) cudaFree(c->d_dry);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
 }
@@ -236,11 +310,7 @@ int switch_variant(swe_ctx *c, int want, int cur) {
   c->variant = want;
   k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, want == SWE_VARIANT_PATCH ? 1 : 0, 0);
   c->launches += 1;
-  if (want == SWE_VARIANT_PATCH) {
-    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
-                                                                             c->d_dry + c->n_patches, c->sc);
-    c->launches += 1;
-  }
+  if (want == SWE_VARIANT_PATCH) launch_patch_flags(c);
   SWE_CUDA(c, cudaGetLastError());
   return SWE_OK;
 }
@@ -293,93 +363,50 @@ int host_prepare(const swe_mesh *mesh, int renumber_mode, HostMesh &hm, std::str
   return SWE_OK;
 }
 
-// internal-numbering edge geometry and slot table, as uploaded by swe_create
-void internal_tables(const HostMesh &hm, std::vector<EdgeGeom> &geom, std::vector<int32_t> &ce4, std::vector<double> &area) {
+int check_args(const swe_mesh *mesh, std::string &err) {
+  if (!mesh || !mesh->node_xy || !mesh->tri || !mesh->zb || !mesh->kst) { err = "null argument"; return SWE_EINVAL; }
+  if (mesh->n_cells <= 0 || mesh->n_nodes <= 0 || mesh->n_cells > (int64_t)0x7fffffff / 3) { err = "n_cells / n_nodes out of range"; return SWE_EINVAL; }
+  return SWE_OK;
+}
+
+int check_params(const swe_params &p, std::string &err) {
+  if (!(p.g > 0.0) || !(p.h_dry >= 0.0) || !(p.dt_max > 0.0)) { err = "g, h_dry, dt_max out of range"; return SWE_EINVAL; }
+  if (p.n_species < 0 || p.n_species > kMaxSpecies) { err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
+  if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) { err = "unknown variant"; return SWE_EINVAL; }
+  if (p.patch_cells != 0 && (p.patch_cells < 32 || p.patch_cells > 1024)) { err = "patch_cells must be 0 (default) or in [32, 1024]"; return SWE_EINVAL; }
+  return SWE_OK;
+}
+
+// The planning pass: host preprocessing, boundary strings, internal-numbering tables, patch blobs (emit: with their
+// bytes; else capacities only) and from those every size of the device layout.  No CUDA call.
+int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, std::string &err) {
+  int rc = check_args(mesh, err);
+  if (rc != SWE_OK) return rc;
+  rc = check_params(p, err);
+  if (rc != SWE_OK) return rc;
+  HostMesh &hm = pl.hm;
+  rc = host_prepare(mesh, p.renumber, hm, err);
+  if (rc != SWE_OK) return rc;
   const int64_t nc = hm.nc, ne = hm.ne;
-  geom.resize(ne); ce4.resize((size_t)4 * nc); area.resize(nc);
+  pl.z.nc = nc; pl.z.ne = ne; pl.z.n_species = p.n_species; pl.z.morph = p.morphology != 0;
+
+  // ---- arrays in internal numbering
+  pl.geom.resize(ne); pl.ce4.resize((size_t)4 * nc);
+  pl.area.resize(nc); pl.inv_area.resize(nc); pl.gn2.resize(nc); pl.kst.resize(nc);
   for (int64_t i = 0; i < nc; ++i) {
     const int32_t o = hm.cell_perm[i];
-    for (int k = 0; k < 3; ++k) ce4[4 * i + k] = hm.edge_new[hm.cell_edge[3 * o + k]];
-    ce4[4 * i + 3] = 0;
-    area[i] = hm.area[o];
+    for (int k = 0; k < 3; ++k) pl.ce4[4 * i + k] = hm.edge_new[hm.cell_edge[3 * o + k]];
+    pl.ce4[4 * i + 3] = 0;
+    const double A = hm.area[o], k = mesh->kst[o];
+    pl.area[i] = A;
+    pl.inv_area[i] = 1.0 / A;
+    pl.gn2[i] = std::isfinite(k) ? p.g / (k * k) : 0.0;    // g / k_str^2 (Eq. 2 P:106-111 with Table 1, R-6)
+    pl.kst[i] = k;
   }
   for (int64_t e = 0; e < ne; ++e) {
     const int32_t o = hm.edge_perm[e];
     const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
-    geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
-  }
-}
-
-int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
-  const int64_t nc = mesh->n_cells;
-  c->nc = nc;
-  if (params) c->prm = *params; else swe_params_default(&c->prm);
-  const swe_params &p = c->prm;
-  if (!(p.g > 0.0) || !(p.h_dry >= 0.0) || !(p.dt_max > 0.0)) { c->err = "g, h_dry, dt_max out of range"; return SWE_EINVAL; }
-  c->stream = (cudaStream_t)p.cuda_stream;
-  c->steps_per_graph = p.steps_per_graph;
-
-  // ---- tables, validation, geometry, numbering (host)
-  HostMesh &hm = c->hm;
-  {
-    int rc = host_prepare(mesh, p.renumber, hm, c->err);
-    if (rc != SWE_OK) return rc;
-  }
-  const int64_t ne = c->ne = hm.ne;
-
-  // ---- workspace
-  const Layout lay(nc, ne);
-  if (p.workspace) {
-    if (p.workspace_bytes < lay.total) { c->err = "workspace too small: need " + std::to_string(lay.total) + " bytes"; return SWE_ENOMEM; }
-    if (((uintptr_t)p.workspace) % kAlign != 0) { c->err = "workspace must be 256-byte aligned"; return SWE_EINVAL; }
-    c->ws = (char *)p.workspace;
-  } else {
-    SWE_CUDA(c, cudaMalloc((void **)&c->ws, lay.total));
-    c->own_ws = true;
-  }
-  c->rec = (CellRec *)(c->ws + lay.rec); c->rec_b = (CellRec *)(c->ws + lay.rec_b); c->geom = (EdgeGeom *)(c->ws + lay.geom); c->flux = (EdgeFlux *)(c->ws + lay.flux);
-  c->cell_edge = (int4 *)(c->ws + lay.cell_edge);
-  c->area = (double *)(c->ws + lay.area); c->inv_area = (double *)(c->ws + lay.inv_area);
-  c->gn2 = (double *)(c->ws + lay.gn2); c->kst = (double *)(c->ws + lay.kst); c->theta = (double *)(c->ws + lay.theta);
-  c->cell_perm = (int *)(c->ws + lay.cell_perm); c->edge_perm = (int *)(c->ws + lay.edge_perm);
-  c->stage = (double *)(c->ws + lay.stage);
-
-  // ---- arrays in internal numbering
-  std::vector<int4> ce(nc);
-  std::vector<double> area(nc);
-  std::vector<EdgeGeom> geom(ne);
-  {
-    std::vector<CellRec> rec(nc);
-    std::vector<double> inv_area(nc), gn2(nc), kst(nc), theta(nc, 1.0);
-    for (int64_t i = 0; i < nc; ++i) {
-      const int32_t o = hm.cell_perm[i];
-      rec[i] = {0.0, 0.0, 0.0, mesh->zb[o]};
-      ce[i] = make_int4(hm.edge_new[hm.cell_edge[3 * o]], hm.edge_new[hm.cell_edge[3 * o + 1]],
-                        hm.edge_new[hm.cell_edge[3 * o + 2]], 0);
-      const double A = hm.area[o], k = mesh->kst[o];
-      area[i] = A;
-      inv_area[i] = 1.0 / A;
-      gn2[i] = std::isfinite(k) ? p.g / (k * k) : 0.0;    // g / k_str^2 (Eq. 2 P:106-111 with Table 1, R-6)
-      kst[i] = k;
-    }
-    for (int64_t e = 0; e < ne; ++e) {
-      const int32_t o = hm.edge_perm[e];
-      const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
-      geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
-    }
-    auto up = [&](void *dst, const void *src, size_t bytes) { return cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice); };
-    SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
-    SWE_CUDA(c, up(c->rec_b, rec.data(), sizeof(CellRec) * nc));     // z_B must be valid in both state buffers
-    SWE_CUDA(c, up(c->cell_edge, ce.data(), sizeof(int4) * nc));
-    SWE_CUDA(c, up(c->area, area.data(), 8 * nc));
-    SWE_CUDA(c, up(c->inv_area, inv_area.data(), 8 * nc));
-    SWE_CUDA(c, up(c->gn2, gn2.data(), 8 * nc));
-    SWE_CUDA(c, up(c->kst, kst.data(), 8 * nc));
-    SWE_CUDA(c, up(c->theta, theta.data(), 8 * nc));
-    SWE_CUDA(c, up(c->geom, geom.data(), sizeof(EdgeGeom) * ne));
-    SWE_CUDA(c, up(c->cell_perm, hm.cell_perm.data(), 4 * nc));
-    SWE_CUDA(c, up(c->edge_perm, hm.edge_perm.data(), 4 * ne));
-    SWE_CUDA(c, cudaMemset(c->flux, 0, sizeof(EdgeFlux) * ne));
+    pl.geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
   }
 
   // ---- boundary strings: members in ascending caller edge id ("string order", R-11)
@@ -388,36 +415,137 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     const int32_t R = hm.edge_cell[2 * e + 1];
     if (R <= -3) max_id = std::max(max_id, -3 - R);
   }
-  if (max_id > 65535) { c->err = "boundary string id too large"; return SWE_EINVAL; }
-  c->strings.assign(max_id + 1, BoundaryString{});
-  c->d_params.assign(max_id + 1, nullptr);
+  if (max_id > 65535) { err = "boundary string id too large"; return SWE_EINVAL; }
+  pl.strings.assign(max_id + 1, BoundaryString{});
   std::vector<std::vector<int32_t>> members(max_id + 1);
   for (int64_t e = 0; e < ne; ++e) {
     const int32_t R = hm.edge_cell[2 * e + 1];
     if (R <= -3) members[-3 - R].push_back(hm.edge_new[e]);
   }
-  std::vector<int32_t> flat;
   size_t scratch = 0;
   for (int s = 0; s <= max_id; ++s) {
-    BoundaryString &bs = c->strings[s];
+    BoundaryString &bs = pl.strings[s];
     bs.n_edges = (int32_t)members[s].size();
-    bs.first = (int32_t)flat.size();
-    int32_t P = 1;
-    while (P < bs.n_edges) P <<= 1;
-    bs.pow2 = P;
+    bs.first = (int32_t)pl.flat.size();
+    int32_t P2 = 1;
+    while (P2 < bs.n_edges) P2 <<= 1;
+    bs.pow2 = P2;
     bs.scratch = (int32_t)scratch;
-    scratch += P;
-    flat.insert(flat.end(), members[s].begin(), members[s].end());
+    scratch += P2;
+    pl.flat.insert(pl.flat.end(), members[s].begin(), members[s].end());
   }
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_ctl, sizeof(Control)));
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_info_part, sizeof(InfoPartial) * kInfoMaxBlocks));
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_info_ticket, sizeof(unsigned int)));
-  SWE_CUDA(c, cudaMemset(c->d_info_ticket, 0, sizeof(unsigned int)));
+  pl.slot_string.assign(std::max<size_t>(1, pl.flat.size()), 0);
+  for (int s = 0; s <= max_id; ++s)
+    for (int32_t j = 0; j < pl.strings[s].n_edges; ++j) pl.slot_string[pl.strings[s].first + j] = s;
+  pl.z.n_strings = max_id + 1; pl.z.n_string_edges = (int64_t)pl.flat.size(); pl.z.scratch = (int64_t)scratch;
+
+  // ---- fused patch step: patch blobs, shared-memory size
+  pl.variant = (p.variant == SWE_VARIANT_THREE_PASS) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+  if (pl.variant == SWE_VARIANT_PATCH) {
+    // default: 256 cells = 256 threads (profiles/r2*_patch_sweep.md); small meshes get smaller patches, so that the
+    // launch-latency-bound step still spreads over the SMs
+    int P = p.patch_cells > 0 ? p.patch_cells : 256;
+    if (p.patch_cells <= 0 && nc < 148 * 256) P = nc < 148 * 64 ? 32 : (nc < 148 * 128 ? 64 : 128);
+    std::vector<int32_t> string_pos(ne, -1);
+    for (size_t j = 0; j < pl.flat.size(); ++j) string_pos[pl.flat[j]] = (int32_t)j;
+    if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, emit, pl.pb, err)) return SWE_EINVAL;
+    pl.patch_smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species).total;
+    // a numbering that is not spatially compact (renumber = NONE on a scattered input order) blows the halos up:
+    // more than 2.2 local cells per own cell, or a block that no longer fits an SM twice -> AUTO falls back to the
+    // three-pass step (round 1: such patches were 2-3x slower than the three-pass step)
+    const bool bloated = (double)pl.pb.sum_loc > 2.2 * (double)nc || pl.patch_smem + kSmemBlockReserve > kSmemPerSM / 2;
+    if (pl.patch_smem > kSmemPerBlockMax || (p.variant == SWE_VARIANT_AUTO && bloated)) {
+      if (p.variant == SWE_VARIANT_AUTO) { pl.variant = SWE_VARIANT_THREE_PASS; pl.pb = PatchBlobs{}; pl.patch_smem = 0; }
+      else { err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
+    }
+  }
+  pl.has_patch = (pl.variant == SWE_VARIANT_PATCH);
+  pl.auto_mode = (p.variant == SWE_VARIANT_AUTO && pl.has_patch);
+  if (pl.has_patch) { pl.z.n_patches = pl.pb.n_patches; pl.z.blob_bytes = (int64_t)pl.pb.lay.stride * pl.pb.n_patches; }
+  return SWE_OK;
+}
+
+int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
+  if (params) c->prm = *params; else swe_params_default(&c->prm);
+  const swe_params &p = c->prm;
+  c->stream = (cudaStream_t)p.cuda_stream;
+  c->steps_per_graph = p.steps_per_graph;
+
+  // ---- host: tables, validation, geometry, numbering, boundary strings, patch blobs, device layout
+  Plan pl;
+  {
+    int rc = make_plan(mesh, p, true, pl, c->err);
+    if (rc != SWE_OK) return rc;
+  }
+  c->hm = std::move(pl.hm);
+  const int64_t nc = c->nc = pl.z.nc, ne = c->ne = pl.z.ne;
+  const Layout lay(pl.z);
+
+  // ---- workspace: the caller's, or one allocation of the same size
+  if (p.workspace) {
+    if (p.workspace_bytes < lay.total) { c->err = "workspace too small: need " + std::to_string(lay.total) + " bytes (swe_workspace_bytes)"; return SWE_ENOMEM; }
+    if (((uintptr_t)p.workspace) % kAlign != 0) { c->err = "workspace must be 256-byte aligned"; return SWE_EINVAL; }
+    c->ws = (char *)p.workspace;
+  } else {
+    cudaError_t e = cudaMalloc((void **)&c->ws, lay.total);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); c->ws = nullptr; c->err = "out of device memory (" + std::to_string(lay.total) + " bytes)"; return SWE_ENOMEM; }
+    SWE_CUDA(c, e);
+    c->own_ws = true;
+  }
+  char *ws = c->ws;
+  c->rec = (CellRec *)(ws + lay.rec); c->rec_b = (CellRec *)(ws + lay.rec_b); c->geom = (EdgeGeom *)(ws + lay.geom); c->flux = (EdgeFlux *)(ws + lay.flux);
+  c->cell_edge = (int4 *)(ws + lay.cell_edge);
+  c->area = (double *)(ws + lay.area); c->inv_area = (double *)(ws + lay.inv_area);
+  c->gn2 = (double *)(ws + lay.gn2); c->kst = (double *)(ws + lay.kst); c->theta = (double *)(ws + lay.theta);
+  c->cell_perm = (int *)(ws + lay.cell_perm); c->edge_perm = (int *)(ws + lay.edge_perm);
+  c->stage = (double *)(ws + lay.stage);
+  c->d_drain_flag = (uint8_t *)(ws + lay.drain_flag);
+  c->d_ctl = (Control *)(ws + lay.ctl);
+  c->d_info_part = (InfoPartial *)(ws + lay.info_part); c->d_info_ticket = (unsigned int *)(ws + lay.info_ticket);
+  c->d_strings = (BoundaryString *)(ws + lay.strings); c->d_string_edges = (int *)(ws + lay.string_edges);
+  c->d_scratch = (double *)(ws + lay.scratch); c->d_params = (double *)(ws + lay.params);
+  c->d_slot_string = (int32_t *)(ws + lay.slot_string); c->d_string_M = (double *)(ws + lay.string_M);
+  c->sc.n = p.n_species;
+  for (int sp = 0; sp < c->sc.n; ++sp) {
+    c->sc.qa[sp] = (double *)(ws + lay.qa[sp]); c->sc.qb[sp] = (double *)(ws + lay.qb[sp]); c->sc.phi_up[sp] = (double *)(ws + lay.phi_up[sp]);
+  }
+  if (c->sc.n > 0) c->d_scalar_stage = (double *)(ws + lay.scalar_stage);
+  c->morph_reserved = pl.z.morph;
+  if (pl.z.morph) { c->mp.qB = (double *)(ws + lay.qB); c->mp.cell = (double2 *)(ws + lay.mcell); }
   SWE_CUDA(c, cudaMallocHost((void **)&c->h_ctl, sizeof(Control)));
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_strings, sizeof(BoundaryString) * std::max<size_t>(1, c->strings.size())));
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_string_edges, 4 * std::max<size_t>(1, flat.size())));
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_scratch, 8 * std::max<size_t>(1, scratch)));
-  if (!flat.empty()) SWE_CUDA(c, cudaMemcpy(c->d_string_edges, flat.data(), 4 * flat.size(), cudaMemcpyHostToDevice));
+
+  // ---- upload
+  {
+    std::vector<CellRec> rec(nc);
+    for (int64_t i = 0; i < nc; ++i) rec[i] = {0.0, 0.0, 0.0, mesh->zb[c->hm.cell_perm[i]]};
+    std::vector<double> theta(nc, 1.0);
+    auto up = [&](void *dst, const void *src, size_t bytes) { return bytes ? cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) : cudaSuccess; };
+    SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
+    SWE_CUDA(c, up(c->rec_b, rec.data(), sizeof(CellRec) * nc));     // z_B must be valid in both state buffers
+    SWE_CUDA(c, up(c->cell_edge, pl.ce4.data(), sizeof(int4) * nc));
+    SWE_CUDA(c, up(c->area, pl.area.data(), 8 * nc));
+    SWE_CUDA(c, up(c->inv_area, pl.inv_area.data(), 8 * nc));
+    SWE_CUDA(c, up(c->gn2, pl.gn2.data(), 8 * nc));
+    SWE_CUDA(c, up(c->kst, pl.kst.data(), 8 * nc));
+    SWE_CUDA(c, up(c->theta, theta.data(), 8 * nc));
+    SWE_CUDA(c, up(c->geom, pl.geom.data(), sizeof(EdgeGeom) * ne));
+    SWE_CUDA(c, up(c->cell_perm, c->hm.cell_perm.data(), 4 * nc));
+    SWE_CUDA(c, up(c->edge_perm, c->hm.edge_perm.data(), 4 * ne));
+    SWE_CUDA(c, cudaMemset(c->flux, 0, sizeof(EdgeFlux) * ne));
+    SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, (size_t)nc + 16));
+    SWE_CUDA(c, cudaMemset(c->d_info_ticket, 0, sizeof(unsigned int)));
+    SWE_CUDA(c, up(c->d_string_edges, pl.flat.data(), 4 * pl.flat.size()));
+    SWE_CUDA(c, up(c->d_slot_string, pl.slot_string.data(), 4 * pl.slot_string.size()));
+    SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 8 * std::max<size_t>(1, pl.flat.size())));
+    for (int sp = 0; sp < c->sc.n; ++sp) {
+      SWE_CUDA(c, cudaMemset(c->sc.qa[sp], 0, 8 * nc));
+      SWE_CUDA(c, cudaMemset(c->sc.qb[sp], 0, 8 * nc));
+      SWE_CUDA(c, cudaMemset(c->sc.phi_up[sp], 0, 8 * ne));
+    }
+    if (pl.z.morph) SWE_CUDA(c, cudaMemset(c->mp.qB, 0, 8 * ne));
+  }
+  c->strings = std::move(pl.strings);
+  c->param_off.assign(c->strings.size(), 0); c->param_cap.assign(c->strings.size(), 0);
   if (!c->strings.empty()) {
     SWE_CUDA(c, cudaMemcpy(c->d_strings, c->strings.data(), sizeof(BoundaryString) * c->strings.size(), cudaMemcpyHostToDevice));
     k_string_lengths<<<1, kCtlThreads, 0, c->stream>>>(c->d_strings, (int)c->strings.size(), c->d_string_edges, c->d_scratch, c->geom);
@@ -426,8 +554,6 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
   }
 
-  SWE_CUDA(c, cudaMalloc((void **)&c->d_drain_flag, (size_t)nc + 16));           // read four bytes at a time
-  SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, (size_t)nc + 16));
   {
     int dev = 0, sms = 148, per_sm = 4;
     SWE_CUDA(c, cudaGetDevice(&dev));
@@ -439,65 +565,25 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->cell_grid = std::max(1, sms * per_sm);
     c->base_edge_grid = c->edge_grid; c->base_cell_grid = c->cell_grid; c->sms = sms;
   }
-  // ---- passive scalars (R-19): state per species (both buffers), per-edge upwind concentrations of the three-pass step
-  if (p.n_species < 0 || p.n_species > kMaxSpecies) { c->err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
-  c->sc.n = p.n_species;
-  for (int sp = 0; sp < c->sc.n; ++sp) {
-    SWE_CUDA(c, cudaMalloc((void **)&c->sc.qa[sp], 8 * nc));
-    SWE_CUDA(c, cudaMalloc((void **)&c->sc.qb[sp], 8 * nc));
-    SWE_CUDA(c, cudaMalloc((void **)&c->sc.phi_up[sp], 8 * ne));
-    SWE_CUDA(c, cudaMemset(c->sc.qa[sp], 0, 8 * nc));
-    SWE_CUDA(c, cudaMemset(c->sc.qb[sp], 0, 8 * nc));
-    SWE_CUDA(c, cudaMemset(c->sc.phi_up[sp], 0, 8 * ne));
-  }
-  if (c->sc.n > 0) SWE_CUDA(c, cudaMalloc((void **)&c->d_scalar_stage, 8 * nc));
 
-  // ---- fused patch step: patch tables (host build, upload), shared-memory size
-  c->variant = (p.variant == SWE_VARIANT_THREE_PASS) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
-  if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) {
-    c->err = "unknown variant"; return SWE_EINVAL;
-  }
-  if (c->variant == SWE_VARIANT_PATCH) {
-    // default: 384 cells (3 blocks/SM: fastest in the round-1 sweep); small meshes get smaller patches, so that the
-    // launch-latency-bound step still spreads over ~256 blocks (4k cells: 9.3 us/step at 64 cells vs 14.5 at 384)
-    int pc = p.patch_cells > 0 ? p.patch_cells : 384;
-    if (p.patch_cells <= 0 && nc < 256 * 384) pc = std::max<int>(64, (int)((nc / 256 + 31) / 32 * 32));
-    if (pc < 32 || pc > 8192) { c->err = "patch_cells must be in [32, 8192]"; return SWE_EINVAL; }
-    std::vector<int32_t> string_pos(ne, -1);
-    for (size_t j = 0; j < flat.size(); ++j) string_pos[flat[j]] = (int32_t)j;
-    std::vector<int32_t> ce4((size_t)4 * nc);
-    for (int64_t i = 0; i < nc; ++i) { ce4[4 * i] = ce[i].x; ce4[4 * i + 1] = ce[i].y; ce4[4 * i + 2] = ce[i].z; ce4[4 * i + 3] = 0; }
-    PatchTables &pt = c->pt;
-    if (!build_patches(nc, ne, geom, ce4, area, string_pos, pc, pt, c->err)) return SWE_EINVAL;
-    c->n_patches = (int)pt.hdr.size();
-    c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown, c->sc.n).total;
-    // 3 blocks per SM need <= 75 KB each; a numbering that is not spatially compact (renumber = NONE on a
-    // scattered input order) blows the halos up: AUTO then falls back to the three-pass step
-    // (with scalar species the block is fatter anyway: 2 blocks per SM, <= 113 KB, still beat the three-pass step)
-    const size_t auto_limit = (c->sc.n > 0 ? 113 : 75) * 1024;
-    if (c->patch_smem > 227 * 1024 || (p.variant == SWE_VARIANT_AUTO && c->patch_smem > auto_limit)) {
-      if (p.variant == SWE_VARIANT_AUTO) { c->variant = SWE_VARIANT_THREE_PASS; c->pt = PatchTables{}; c->n_patches = 0; c->patch_smem = 0; }
-      else { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
-    }
-  }
-  if (c->variant == SWE_VARIANT_PATCH) {
-    PatchTables &pt = c->pt;
-    std::vector<int32_t> slot_string(std::max<size_t>(1, flat.size()), 0);
-    for (int s = 0; s <= max_id; ++s)
-      for (int32_t j = 0; j < c->strings[s].n_edges; ++j) slot_string[c->strings[s].first + j] = s;
-    // default patch size on a compact numbering: shared-memory arrays with compile-time capacities; anything else
-    // (other patch sizes, fatter halos) runs the same kernel with run-time capacities
-    constexpr int kCapLoc = 640, kCapC1 = 544, kCapE = 864, kCapEown = 704;
-    if (c->sc.n > 0) {               // scalar module: run-time capacities (the concentrations enlarge the block)
-      c->patch_kernel = c->patch_smem <= 75 * 1024 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0, true>
-                                                   : k_patch_step<kPatchThreads, 2, 0, 0, 0, 0, true>;
-    } else if (pt.max_loc <= kCapLoc && pt.max_c1 <= kCapC1 && pt.max_e <= kCapE && pt.max_eown <= kCapEown) {
-      c->patch_kernel = k_patch_step<kPatchThreads, 3, kCapLoc, kCapC1, kCapE, kCapEown>;
-      c->patch_smem = sizeof(double) * (size_t)patch_smem_layout(kCapLoc, kCapC1, kCapE, kCapEown).total;
-    } else {
-      // 3 blocks/SM while the patch fits 75 KB (the round-1 sweep: 2 blocks are slower, 4 need 64 registers and spill)
-      c->patch_kernel = c->patch_smem <= 75 * 1024 ? k_patch_step<kPatchThreads, 3, 0, 0, 0, 0> : k_patch_step<kPatchThreads, 2, 0, 0, 0, 0>;
-    }
+  // ---- fused patch step: blobs, flag words, kernel instance
+  c->variant = pl.variant;
+  c->has_patch = pl.has_patch;
+  if (pl.has_patch) {
+    const PatchBlobs &pb = pl.pb;
+    c->blay = pb.lay;
+    c->n_patches = (int)pb.n_patches;
+    c->patch_smem = pl.patch_smem;
+    c->patch_sum_loc = pb.sum_loc; c->patch_sum_e = pb.sum_e; c->patch_max_loc = pb.max_loc; c->patch_max_e = pb.max_e;
+    c->d_blob = (unsigned char *)(ws + lay.blob); c->d_pflag = (unsigned char *)(ws + lay.pflag);
+    SWE_CUDA(c, cudaMemcpy(c->d_blob, pb.bytes.data(), pb.bytes.size(), cudaMemcpyHostToDevice));
+    SWE_CUDA(c, cudaMemset(c->d_pflag, 0, 2 * (size_t)kPflagBytes * (size_t)c->n_patches));
+    int force = 0;
+    if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) force = std::atoi(s);
+    c->patch_threads = patch_threads(pb.lay.P);
+    const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force);
+    if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
+    c->patch_kernel = pi->fn; c->patch_min_blocks = pi->min_blocks;
     // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
     // context with smaller patches cannot lower it under an earlier context's launches
     {
@@ -510,41 +596,30 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       if ((int)c->patch_smem > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
       SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
     }
-    auto dup = [&](void **dst, const void *src, size_t bytes) {
-      cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
-      if (e == cudaSuccess && bytes) e = cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
-      return e;
-    };
-    SWE_CUDA(c, dup((void **)&c->d_hdr, pt.hdr.data(), sizeof(PatchHeader) * pt.hdr.size()));
-    SWE_CUDA(c, dup((void **)&c->d_halo_ids, pt.halo_ids.data(), 4 * pt.halo_ids.size()));
-    SWE_CUDA(c, dup((void **)&c->d_halo_area, pt.halo_area.data(), 8 * pt.halo_area.size()));
-    SWE_CUDA(c, dup((void **)&c->d_pedge, pt.pedge.data(), sizeof(PatchEdge) * pt.pedge.size()));
-    SWE_CUDA(c, dup((void **)&c->d_pce, pt.pce.data(), 4 * pt.pce.size()));
-    SWE_CUDA(c, dup((void **)&c->d_slot_string, slot_string.data(), 4 * slot_string.size()));
-    SWE_CUDA(c, dup((void **)&c->d_patch_nbr, pt.patch_nbr.data(), 4 * pt.patch_nbr.size()));
-    SWE_CUDA(c, cudaMalloc((void **)&c->d_dry, 2 * (size_t)c->n_patches));
-    SWE_CUDA(c, cudaMemset(c->d_dry, 0, 2 * (size_t)c->n_patches));
-    SWE_CUDA(c, cudaMalloc((void **)&c->d_string_M, 8 * std::max<size_t>(1, flat.size())));
-    SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 8 * std::max<size_t>(1, flat.size())));
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
-    // state in 32 + state out 32 + pce 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
+    // state in 32 + state out 32 + slot words 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_PATCH];
     ab[0] = 0;
     ab[1] = 104 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;        // + q_c in and out per species
-    pt.halo_ids = {}; pt.halo_area = {}; pt.pedge = {}; pt.pce = {}; pt.patch_nbr = {};   // host copies no longer needed
+    // SURVEY.md section 8(d), one-pass column: 132 B per cell-step (+ 16 per species: q_c in and out)
+    c->survey_bytes_v[SWE_VARIANT_PATCH][1] = (132 + 16 * (int64_t)c->sc.n) * nc;
   }
   {
     // EdgeGeom read + EdgeFlux written per edge, every CellRec gathered once
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
     ab[0] = 0;
     ab[1] = 64 * ne + 32 * nc;
-    // cell_edge, CellRec, area read + theta written per cell; every EdgeGeom and EdgeFlux gathered once
     ab[2] = 1 * nc;                                      // k_theta_lazy: one flag byte per cell
     // cell_edge, 1/area, g/k^2, theta read, CellRec read + written per cell; every EdgeGeom and EdgeFlux gathered once
     ab[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
     ab[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
     ab[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
     c->alg_bytes_base[0] = ab[1]; c->alg_bytes_base[1] = ab[3];
+    // SURVEY.md section 8(d), two-kernel column (284 B per cell-step with 1/A read in the edge pass), split as the
+    // survey's rows split: edge pass = state 24 + z 8 + 1/A 8 + geometry 36 + edge->cell 12 + flux written 60 = 148;
+    // cell pass = state 24 r + 24 w + g/k^2, 1/A 16 + cell->edge 12 + flux read 60 = 136
+    int64_t *sb = c->survey_bytes_v[SWE_VARIANT_THREE_PASS];
+    sb[1] = 148 * nc; sb[2] = 0; sb[3] = 136 * nc;
   }
 
   // ---- control block
@@ -557,7 +632,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   *c->h_ctl = h;
   // AUTO with a compact numbering: both variants stay available (their graphs are captured now) and swe_set_state
   // picks one from the wet fraction of the state -- they compute bit-identical results
-  c->auto_mode = (p.variant == SWE_VARIANT_AUTO && c->variant == SWE_VARIANT_PATCH);
+  c->auto_mode = pl.auto_mode;
   if (c->auto_mode) {
     c->variant = SWE_VARIANT_THREE_PASS;
     int rc = capture_graph(c);
@@ -584,18 +659,25 @@ void swe_params_default(swe_params *p) {
   p->variant = SWE_VARIANT_AUTO;
   p->patch_cells = 0;
   p->n_species = 0;
+  p->morphology = 0;
 }
 
-size_t swe_workspace_bytes(int64_t n_cells, int64_t n_edges) {
-  if (n_cells < 0) return 0;
-  if (n_edges <= 0) n_edges = 3 * n_cells;
-  return Layout(n_cells, n_edges).total;
+size_t swe_workspace_bytes(const swe_mesh *mesh, const swe_params *params) {
+  swe_params p;
+  if (params) p = *params; else swe_params_default(&p);
+  try {
+    Plan pl;
+    if (make_plan(mesh, p, false, pl, g_create_error) != SWE_OK) return 0;
+    return Layout(pl.z).total;
+  } catch (const std::bad_alloc &) {
+    g_create_error = "out of host memory";
+    return 0;
+  }
 }
 
 int swe_create(const swe_mesh *mesh, const swe_params *params, swe_ctx **out) {
   if (out) *out = nullptr;
-  if (!mesh || !out || !mesh->node_xy || !mesh->tri || !mesh->zb || !mesh->kst) { g_create_error = "null argument"; return SWE_EINVAL; }
-  if (mesh->n_cells <= 0 || mesh->n_nodes <= 0 || mesh->n_cells > (int64_t)0x7fffffff / 3) { g_create_error = "n_cells / n_nodes out of range"; return SWE_EINVAL; }
+  if (!out) { g_create_error = "null argument"; return SWE_EINVAL; }
   swe_ctx *c = new (std::nothrow) swe_ctx;
   if (!c) { g_create_error = "out of host memory"; return SWE_ENOMEM; }
   int rc;
@@ -620,6 +702,7 @@ int swe_set_boundary(swe_ctx *c, int string_id, int type, const double *params, 
   if (n_params < 0 || (n_params > 0 && !params)) { c->err = "bad params"; return SWE_EINVAL; }
   if (type == SWE_BC_INFLOW_Q) {
     if (n_params < 2 || n_params % 2) { c->err = "INFLOW_Q needs a (t, Q) table"; return SWE_EINVAL; }
+    for (int k = 0; k < n_params; ++k) if (!std::isfinite(params[k])) { c->err = "hydrograph entries must be finite"; return SWE_EINVAL; }
     for (int k = 2; k < n_params; k += 2) if (!(params[k] > params[k - 2])) { c->err = "hydrograph times must ascend"; return SWE_EINVAL; }
   } else if (type == SWE_BC_OUTFLOW_UNIFORM) {
     if (n_params < 1 || !(params[0] >= 0.0)) { c->err = "OUTFLOW_UNIFORM needs S0 >= 0"; return SWE_EINVAL; }
@@ -627,15 +710,20 @@ int swe_set_boundary(swe_ctx *c, int string_id, int type, const double *params, 
     c->err = "unknown boundary type";
     return SWE_EINVAL;
   }
+  // the table goes into the string's slice of the parameter pool (a new slice when it has grown)
+  if (n_params > c->param_cap[string_id]) {
+    if (c->params_used + n_params > kParamsPool) { c->err = "boundary parameter pool exhausted (16384 doubles per context)"; return SWE_ENOMEM; }
+    c->param_off[string_id] = c->params_used; c->param_cap[string_id] = n_params;
+    c->params_used += n_params;
+  }
   SWE_CUDA(c, cudaStreamSynchronize(c->stream));
   BoundaryString &bs = c->strings[string_id];
-  if (c->d_params[string_id]) { cudaFree(c->d_params[string_id]); c->d_params[string_id] = nullptr; }
   bs.type = type; bs.n_params = n_params; bs.params = nullptr; bs.Q = 0.0; bs.sumK = 0.0;
   bs.S0 = (type == SWE_BC_OUTFLOW_UNIFORM) ? params[0] : 0.0;
   if (n_params > 0) {
-    SWE_CUDA(c, cudaMalloc((void **)&c->d_params[string_id], 8 * (size_t)n_params));
-    SWE_CUDA(c, cudaMemcpy(c->d_params[string_id], params, 8 * (size_t)n_params, cudaMemcpyHostToDevice));
-    bs.params = c->d_params[string_id];
+    double *dst = c->d_params + c->param_off[string_id];
+    SWE_CUDA(c, cudaMemcpy(dst, params, 8 * (size_t)n_params, cudaMemcpyHostToDevice));
+    bs.params = dst;
   }
   return upload_strings(c);
 }
@@ -671,11 +759,7 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     c->launches += 1;
   }
   k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
-  if (c->variant == SWE_VARIANT_PATCH) {
-    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
-                                                                             c->d_dry + c->n_patches, c->sc);
-    c->launches += 1;
-  }
+  if (c->variant == SWE_VARIANT_PATCH) launch_patch_flags(c);
   if (c->mp.formula == 2) {           // mobile bed, MPM-like law: the per-cell cube roots of the new state
     k_sed_cell_init<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)nc);
     c->launches += 1;
@@ -716,7 +800,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (finite_end) {                // the only host synchronisation inside the loop: once per batch
       int rc = read_control(c);
       if (rc != SWE_OK) return rc;
-      if (!(c->h_ctl->t < t_end) || (c->h_ctl->flags & SWE_FLAG_DT_UNBOUNDED)) done = true;
+      if (!(c->h_ctl->t < t_end) || (c->h_ctl->flags & (SWE_FLAG_DT_UNBOUNDED | SWE_FLAG_STALLED))) done = true;
       poll_every = std::min<int64_t>(poll_every * 2, 64);
     }
   }
@@ -761,11 +845,7 @@ int swe_set_scalars(swe_ctx *c, const double *qc) {
     k_pack_scalar<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, src, c->sc.qa[sp], c->sc.qb[sp], (int)nc);
     c->launches += 1;
   }
-  if (c->variant == SWE_VARIANT_PATCH) {
-    k_patch_flags<kPatchThreads><<<c->n_patches, kPatchThreads, 0, c->stream>>>(c->d_ctl, c->d_hdr, c->rec, c->rec_b, c->d_dry,
-                                                                             c->d_dry + c->n_patches, c->sc);
-    c->launches += 1;
-  }
+  if (c->variant == SWE_VARIANT_PATCH) launch_patch_flags(c);
   SWE_CUDA(c, cudaGetLastError());
   return SWE_OK;
 }
@@ -799,6 +879,7 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
   if (formula == 2 && !(s > 1.0 && d_m > 0.0 && std::isfinite(s) && std::isfinite(d_m) && std::isfinite(theta_cr))) {
     c->err = "the MPM-like formula needs s > 1, d_m > 0 and a finite theta_cr"; return SWE_EINVAL;
   }
+  if (formula && !c->morph_reserved) { c->err = "the context was created without room for the mobile-bed module: set swe_params.morphology = 1"; return SWE_EINVAL; }
   if (formula && c->sc.n > 0) { c->err = "passive scalars and a mobile bed in one context are not built"; return SWE_EINVAL; }
   if (formula && !c->auto_mode && c->variant == SWE_VARIANT_PATCH) {
     c->err = "the fused patch step has no mobile bed: create the context with SWE_VARIANT_AUTO or SWE_VARIANT_THREE_PASS";
@@ -812,10 +893,6 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
       if (rc != SWE_OK) return rc;
     }
     c->auto_mode = false;            // stays three-pass from here on
-    if (!c->mp.qB) {
-      SWE_CUDA(c, cudaMalloc((void **)&c->mp.qB, 8 * (size_t)c->ne));
-      SWE_CUDA(c, cudaMemsetAsync(c->mp.qB, 0, 8 * (size_t)c->ne, c->stream));
-    }
   }
   const double g = c->prm.g;
   c->mp.formula = formula; c->mp.alpha = alpha; c->mp.theta_cr = theta_cr;
@@ -823,7 +900,6 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
   c->mp.Gm = alpha * std::sqrt(((s - 1.0) * g) * (d_m * (d_m * d_m)));
   c->mp.inv1mp = 1.0 / (1.0 - porosity);
   if (formula == 2) {                 // (g/k^2, cbrt(h)) of the state as it stands; k_cell_update keeps it current
-    if (!c->mp.cell) SWE_CUDA(c, cudaMalloc((void **)&c->mp.cell, 16 * (size_t)c->nc));
     k_sed_cell_init<<<grid_for(c->nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)c->nc);
     c->launches += 1;
     SWE_CUDA(c, cudaGetLastError());
@@ -872,7 +948,7 @@ int swe_get_bed(swe_ctx *c, double *zb) {
 int swe_get_sediment_flux(swe_ctx *c, double *qB) {
   if (!c) return SWE_EINVAL;
   if (!qB) { c->err = "null flux pointer"; return SWE_EINVAL; }
-  if (!c->mp.qB) { c->err = "morphodynamics was never switched on"; return SWE_EINVAL; }
+  if (!c->morph_reserved) { c->err = "the context has no mobile-bed module (swe_params.morphology)"; return SWE_EINVAL; }
   const int64_t ne = c->ne;
   double *dst = c->prm.state_on_device ? qB : c->stage;       // stage holds 3 n_cells >= n_edges doubles
   k_export_sediment<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->mp.qB, dst, (int)ne);
@@ -952,19 +1028,17 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
     k_theta<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, in, c->area, c->theta, (int)nc, 1);
     c->launches += 2;
   }
-  double *d = nullptr;
-  SWE_CUDA(c, cudaMalloc((void **)&d, 8 * 4 * ne));
   const double *th_apply = (c->variant == SWE_VARIANT_PATCH) ? c->theta : nullptr;   // three-pass: limited in place
-  k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, th_apply, d, d + ne, d + 2 * ne,
-                                                        d + 3 * ne, (int)ne);
-  c->launches += 1;
-  cudaError_t e1 = cudaStreamSynchronize(c->stream);
-  if (e1 == cudaSuccess) e1 = cudaMemcpy(F1, d, 8 * ne, cudaMemcpyDeviceToHost);
-  if (e1 == cudaSuccess) e1 = cudaMemcpy(F3, d + ne, 8 * ne, cudaMemcpyDeviceToHost);
-  if (e1 == cudaSuccess) e1 = cudaMemcpy(GL, d + 2 * ne, 8 * ne, cudaMemcpyDeviceToHost);
-  if (e1 == cudaSuccess) e1 = cudaMemcpy(GR, d + 3 * ne, 8 * ne, cudaMemcpyDeviceToHost);
-  cudaFree(d);
-  SWE_CUDA(c, e1);
+  double *d = c->stage;                                // holds 2 n_edges doubles: export in two halves
+  for (int half = 0; half < 2; ++half) {
+    k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, th_apply, half ? nullptr : d, half ? nullptr : d + ne,
+                                                          half ? d : nullptr, half ? d + ne : nullptr, (int)ne);
+    c->launches += 1;
+    SWE_CUDA(c, cudaGetLastError());
+    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+    SWE_CUDA(c, cudaMemcpy(half ? GL : F1, d, 8 * ne, cudaMemcpyDeviceToHost));
+    SWE_CUDA(c, cudaMemcpy(half ? GR : F3, d + ne, 8 * ne, cudaMemcpyDeviceToHost));
+  }
   if (theta) {
     std::vector<double> th(nc);
     SWE_CUDA(c, cudaMemcpy(th.data(), c->theta, 8 * nc, cudaMemcpyDeviceToHost));
@@ -1032,22 +1106,56 @@ int swe_host_preprocess(const swe_mesh *mesh, int renumber_mode, int patch_cells
     if (rc != SWE_OK) return rc;
     int64_t v[10] = {hm.ne, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     if (patch_cells > 0) {
-      std::vector<EdgeGeom> geom; std::vector<int32_t> ce4; std::vector<double> area;
-      internal_tables(hm, geom, ce4, area);
-      std::vector<int32_t> string_pos(hm.ne, -1);
-      int32_t n_string = 0;
-      for (int64_t e = 0; e < hm.ne; ++e) if (geom[e].R <= -3) string_pos[e] = n_string++;
-      PatchTables pt;
-      if (!build_patches(hm.nc, hm.ne, geom, ce4, area, string_pos, patch_cells, pt, g_create_error)) return SWE_EINVAL;
-      int64_t own = 0, covered = 0;
-      std::vector<uint8_t> seen(hm.nc, 0);
-      for (const PatchHeader &h : pt.hdr) {
-        own += h.n_own;
-        for (int32_t l = 0; l < h.n_own; ++l) if (!seen[h.cell0 + l]) { seen[h.cell0 + l] = 1; ++covered; }
+      const int64_t nc = hm.nc, ne = hm.ne;
+      std::vector<EdgeGeom> geom(ne); std::vector<int32_t> ce4((size_t)4 * nc); std::vector<double> area(nc), inv_area(nc), gn2(nc, 0.0);
+      for (int64_t i = 0; i < nc; ++i) {
+        const int32_t o = hm.cell_perm[i];
+        for (int k = 0; k < 3; ++k) ce4[4 * i + k] = hm.edge_new[hm.cell_edge[3 * o + k]];
+        ce4[4 * i + 3] = 0;
+        area[i] = hm.area[o]; inv_area[i] = 1.0 / hm.area[o];
       }
-      v[1] = (int64_t)pt.hdr.size(); v[2] = pt.sum_loc; v[3] = pt.sum_e; v[4] = pt.max_loc; v[5] = pt.max_e;
-      v[6] = (int64_t)sizeof(double) * patch_smem_layout(pt.max_loc, pt.max_c1, pt.max_e, pt.max_eown).total;
-      v[7] = own; v[8] = covered; v[9] = (int64_t)pt.patch_nbr.size();
+      for (int64_t e = 0; e < ne; ++e) {
+        const int32_t o = hm.edge_perm[e];
+        const int32_t L = hm.edge_cell[2 * o], R = hm.edge_cell[2 * o + 1];
+        geom[e] = {hm.nx[o], hm.ny[o], hm.len[o], hm.cell_new[L], R >= 0 ? hm.cell_new[R] : R};
+      }
+      std::vector<int32_t> string_pos(ne, -1);
+      int32_t n_string = 0;
+      for (int64_t e = 0; e < ne; ++e) if (geom[e].R <= -3) string_pos[e] = n_string++;
+      PatchBlobs pb;
+      if (!build_blobs(nc, ne, geom, ce4, area, inv_area, gn2, string_pos, patch_cells, true, pb, g_create_error)) return SWE_EINVAL;
+      // every cell must be an own cell of exactly one patch
+      // ... and the emitted blobs must describe what the capacity pass counted: local cells / edges of every header,
+      // local indices inside the patch, every slot word pointing at an edge that joins the two cells it names
+      int64_t own = 0, covered = 0, hdr_loc = 0, hdr_e = 0;
+      std::vector<uint8_t> seen(nc, 0);
+      const BlobLayout &BL = pb.lay;
+      for (int64_t p = 0; p < pb.n_patches; ++p) {
+        const unsigned char *B = pb.bytes.data() + (size_t)BL.stride * (size_t)p;
+        const BlobHeader *h = (const BlobHeader *)B;
+        own += h->n_own;
+        for (int32_t l = 0; l < h->n_own; ++l) { const int64_t cidx = p * patch_cells + l; if (!seen[cidx]) { seen[cidx] = 1; ++covered; } }
+        const int32_t n_loc = h->n_own + h->n_r1 + h->n_r2, n_e = h->n_eown + h->n_er1;
+        hdr_loc += n_loc; hdr_e += n_e;
+        const uint32_t *lr = (const uint32_t *)(B + BL.off_stage + BL.s_lr);
+        const uint32_t *pce = (const uint32_t *)(B + BL.off_stage + BL.s_pce);
+        for (int32_t j = 0; j < n_e; ++j) {
+          const uint32_t Ll = lr[j] & 0xFFFFu, Rl = lr[j] >> 16;
+          if ((int32_t)Ll >= n_loc || (Rl != 0xFFFFu && (int32_t)Rl >= n_loc)) { g_create_error = "patch blob: local cell index out of range"; return SWE_EINVAL; }
+        }
+        for (int32_t l = 0; l < h->n_own + h->n_r1; ++l)
+          for (int k = 0; k < 3; ++k) {
+            const uint32_t wd = pce[4 * l + k], e = wd & 0x7FFFu, nb = wd >> 16;
+            const bool isL = (wd & 0x8000u) != 0u;
+            if ((int32_t)e >= n_e) { g_create_error = "patch blob: slot word names an edge outside the patch"; return SWE_EINVAL; }
+            const uint32_t Ll = lr[e] & 0xFFFFu, Rl = lr[e] >> 16;
+            if ((isL ? Ll : Rl) != (uint32_t)l || (isL ? Rl : Ll) != nb) { g_create_error = "patch blob: slot word and edge record disagree"; return SWE_EINVAL; }
+          }
+      }
+      if (hdr_loc != pb.sum_loc || hdr_e != pb.sum_e) { g_create_error = "patch blob: headers disagree with the capacity pass"; return SWE_EINVAL; }
+      v[1] = pb.n_patches; v[2] = pb.sum_loc; v[3] = pb.sum_e; v[4] = pb.max_loc; v[5] = pb.max_e;
+      v[6] = (int64_t)patch2_smem_layout(pb.lay, 0).total;
+      v[7] = own; v[8] = covered; v[9] = pb.sum_nbr;
     }
     for (int k = 0; k < n_out && k < 10; ++k) out[k] = v[k];
     if (cell_perm) std::memcpy(cell_perm, hm.cell_perm.data(), 4 * hm.nc);
@@ -1072,9 +1180,10 @@ int swe_get_patch_stats(swe_ctx *c, int64_t *out, int n_out) {
   if (!c || !out || n_out < 1) return SWE_EINVAL;
   int rc = read_control(c);
   if (rc != SWE_OK) return rc;
-  const int64_t v[9] = {c->variant, c->n_patches, c->pt.patch_cells, (int64_t)c->patch_smem, c->pt.sum_loc, c->pt.sum_e,
-                        c->pt.max_loc, c->pt.max_e, (int64_t)c->h_ctl->patches_skipped};
-  for (int k = 0; k < n_out && k < 9; ++k) out[k] = v[k];
+  const int64_t v[12] = {c->variant, c->n_patches, c->blay.P, (int64_t)c->patch_smem, c->patch_sum_loc, c->patch_sum_e,
+                         c->patch_max_loc, c->patch_max_e, (int64_t)c->h_ctl->patches_skipped, c->patch_min_blocks,
+                         c->blay.stride, c->blay.stage_bytes};
+  for (int k = 0; k < n_out && k < 12; ++k) out[k] = v[k];
   return SWE_OK;
 }
 

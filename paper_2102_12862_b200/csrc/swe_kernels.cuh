@@ -23,7 +23,7 @@ constexpr int kTreeCap = 4096;        // boundary-string members whose pairwise 
 // boundary codes / string types (values of include/swe.h, restated so that device code needs no host header)
 constexpr int kEdgeTransmissive = -2;
 constexpr int kBcInflowQ = 1, kBcOutflowUniform = 2;
-constexpr int kFlagUnbounded = 2;
+constexpr int kFlagUnbounded = 2, kFlagStalled = 4;
 
 // ---------------------------------------------------------------------------------------------------------
 // S1, one edge in the (normal, tangential) frame.  P:252 HLLC ("Chapter 10 of [18]"): HLL for mass and normal
@@ -358,7 +358,7 @@ __device__ __forceinline__ void block_max_to_global(double r, unsigned long long
   if (wid == 0) {
     r = (lane < kThreads / 32) ? warp_max[lane] : 0.0;
 #pragma unroll
-    for (int off = (kThreads / 32) / 2; off > 0; off >>= 1) {
+    for (int off = 16; off > 0; off >>= 1) {          // all 32 lanes: the warp count need not be a power of two
       const double other = __shfl_xor_sync(0xffffffffu, r, off);
       r = (other > r) ? other : r;
     }
@@ -517,7 +517,7 @@ __device__ __forceinline__ double hydrograph(const double *p, int n_params, doub
   if (t <= p[0]) return p[1];
   if (t >= p[2 * (m - 1)]) return p[2 * (m - 1) + 1];
   int k = 0;
-  while (!(p[2 * k] <= t && t < p[2 * (k + 1)])) ++k;
+  while (k < m - 2 && !(p[2 * k] <= t && t < p[2 * (k + 1)])) ++k;   // bounded: entries are finite and ascending (swe_set_boundary)
   const double tk = p[2 * k], Qk = p[2 * k + 1], tk1 = p[2 * k + 2], Qk1 = p[2 * k + 3];
   return Qk + (Qk1 - Qk) * ((t - tk) / (tk1 - tk));
 }
@@ -615,7 +615,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
     if (mode == 1) { ctl->pending = 0; ctl->vol = 0.0; ctl->n_wet = 0; ctl->nonfinite = 0; return; }
     int active = 0, new_pending = 0;
     const double t = t_now, t_end = c_tend;
-    if (c_left != 0 && t < t_end && !(c_flags & kFlagUnbounded)) {
+    if (c_left != 0 && t < t_end && !(c_flags & (kFlagUnbounded | kFlagStalled))) {
       const double r = __longlong_as_double((long long)c_rate);
       double dt = (r > 0.0) ? c_cfl / r : c_dtmax;
       dt = fmin(dt, c_dtmax);
@@ -624,6 +624,8 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
       if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = t + dt; }
       if (!isfinite(dt)) {
         ctl->flags = c_flags | kFlagUnbounded;
+      } else if (!(dt > 0.0) || !(t_new > t)) {   // the clock cannot advance (a rate of +inf, or dt below ulp(t)):
+        ctl->flags = c_flags | kFlagStalled;      // stop instead of stepping in place for ever
       } else {
         active = 1;
         ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
@@ -670,7 +672,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   if (threadIdx.x == 0) {
     int active = 0, new_pending = 0;
     const double t = t_now, t_end = c_tend;
-    if (c_left != 0 && t < t_end && !(c_flags & kFlagUnbounded)) {
+    if (c_left != 0 && t < t_end && !(c_flags & (kFlagUnbounded | kFlagStalled))) {
       const double r = __longlong_as_double((long long)c_rate);
       double dt = (r > 0.0) ? c_cfl / r : c_dtmax;
       dt = fmin(dt, c_dtmax);
@@ -679,6 +681,8 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
       if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = t + dt; }
       if (!isfinite(dt)) {
         ctl->flags = c_flags | kFlagUnbounded;
+      } else if (!(dt > 0.0) || !(t_new > t)) {   // the clock cannot advance (a rate of +inf, or dt below ulp(t)):
+        ctl->flags = c_flags | kFlagStalled;      // stop instead of stepping in place for ever
       } else {
         active = 1;
         ctl->dt = dt; ctl->dt_last = dt; ctl->t = t_new;
@@ -738,7 +742,7 @@ __global__ void k_call_begin(Control *ctl, long long n_steps, double t_end, doub
   ctl->steps_left = n_steps;
   ctl->t_end = t_end;
   ctl->cfl = cfl;
-  ctl->flags &= ~kFlagUnbounded;
+  ctl->flags &= ~(kFlagUnbounded | kFlagStalled);
 }
 
 __global__ void k_reset(Control *ctl, double t0) {
@@ -888,7 +892,8 @@ k_export_flux(const int *__restrict__ edge_perm, const EdgeGeom *__restrict__ ge
     if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR; }
   }
   const int o = edge_perm[e];
-  F1[o] = f.F1; F3[o] = f.F3; GL[o] = f.GL; GR[o] = f.GR;
+  if (F1) { F1[o] = f.F1; F3[o] = f.F3; }             // the caller exports in two halves (staging holds 2 n_edges doubles)
+  if (GL) { GL[o] = f.GL; GR[o] = f.GR; }
 }
 
 }  // namespace swe

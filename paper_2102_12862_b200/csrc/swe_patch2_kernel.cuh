@@ -1,0 +1,426 @@
+// Fused patch step (sm_100a), second design: one thread block advances one patch of P consecutive (Morton-ordered)
+// cells by a whole time step -- S1 edge fluxes, S1c limiter, S2 gather, S3 update + friction, and Eq. 21 of the new
+// state for the next dt -- out of shared memory, one thread per own cell.  Edge fluxes never go to DRAM; the state
+// ping-pongs between two buffers because neighbouring patches read the old state of this patch's cells.
+// Arithmetic and parenthesisation are those of the three-pass kernels in swe_kernels.cuh (R-14), so
+// both variants give bit-identical states.
+//
+// Data movement (what differs from the first design, profiles/r1j: long-scoreboard stalls 5.3 cycles per issue):
+//   * everything a patch streams sits in ONE fixed-stride blob (patch_blob.hpp); the block knows every address from
+//     blockIdx alone, there is no header -> table -> record chain of dependent loads;
+//   * the blob's staged part and the patch's own cell records arrive in shared memory by two bulk asynchronous
+//     copies (cp.async.bulk.shared.global + mbarrier complete_tx; SASS: UBLKCP) issued by one thread right after
+//     the skip test; no thread holds a register for a load in flight, and phases 2-4 read shared memory only;
+//   * the halo records (ring 1 / ring 2: a gather) are fetched by the other threads while the bulk copies fly, and
+//     their velocities are formed at once;
+//   * the skip test is ONE 32-byte load: every patch owns a word of flag bytes {neighbours..., own, skippable} per
+//     state buffer, and a block that finishes publishes its flag into its neighbours' words (byte stores).
+//
+// Phases (separated by __syncthreads):
+//   1  states of the local cells (own, ring 1, ring 2) -> shared memory as (h, u, v, z)
+//   2  every local edge: hydrostatic reconstruction + HLLC, boundary edges
+//   3  theta of own and ring-1 cells (R-8b)
+//   4  own cells: limited fluxes in slot order (Eq. 12), update, friction (Eq. 2), Eq. 21 rate
+#pragma once
+#include "swe_kernels.cuh"
+
+namespace swe {
+
+struct Patch2Args {
+  const unsigned char *blob;
+  BlobLayout L;
+  CellRec *rec_a, *rec_b;
+  const double *kst;
+  const BoundaryString *strings;
+  const int32_t *slot_string;     // string id of every position of string_edges[]
+  double *string_M;               // l * (limited F1) of every boundary-string edge, by position in string_edges[]
+  unsigned char *pflag_a, *pflag_b;   // [n_patches][kPflagBytes], one array per state buffer
+  int32_t n_cells;
+  Scalars sc;                     // passive scalars (kScalars instantiation only)
+};
+
+// ---- shared-memory carving (bytes), the same for every block of a context
+struct Patch2Smem {
+  int32_t stage, crec, h, u, v, z, theta, F1, F3, GL, GR, phi, total;
+};
+
+__host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species) {
+  Patch2Smem s;
+  int32_t o = 128;                                  // [0, 8): the mbarrier
+  s.stage = o; o += blob_align(L.stage_bytes, 128);
+  s.crec = o; o += 32 * L.P;                        // own CellRec records as they are in global memory
+  s.h = o; o += 8 * L.cap_loc; s.u = o; o += 8 * L.cap_loc; s.v = o; o += 8 * L.cap_loc; s.z = o; o += 8 * L.cap_loc;
+  s.theta = o; o += 8 * L.cap_c1;
+  s.F1 = o; o += 8 * L.cap_e;
+  s.F3 = o; o += 8 * L.cap_eown; s.GL = o; o += 8 * L.cap_eown; s.GR = o; o += 8 * L.cap_eown;
+  s.phi = o; o += 8 * n_species * L.cap_loc;        // concentrations of the local cells, species-major
+  s.total = o;
+  return s;
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// own flag + the byte this patch has in each neighbour's flag word (nbr / nbr_slot: cap_nbr entries, -1 padded)
+template <int kThreads>
+__device__ __forceinline__ void publish_flag(unsigned char *pf_out_base, int b, const int32_t *nbr, const int32_t *nbr_slot,
+                                             int cap_nbr, unsigned char flag) {
+  if (threadIdx.x == 0) pf_out_base[(size_t)b * kPflagBytes + kPflagOwn] = flag;
+  for (int j = threadIdx.x; j < cap_nbr; j += kThreads) {
+    const int q = nbr[j], sl = nbr_slot[j];
+    if (q >= 0 && sl >= 0) pf_out_base[(size_t)q * kPflagBytes + sl] = flag;
+  }
+}
+
+// kThreads >= BlobLayout::P (one thread per own cell; the host picks the smallest instance that covers P).  kScalars: the passive-scalar module (R-19) is on:
+// concentrations of the local cells in shared memory, one more gather per species in phase 4.
+template <int kThreads, int kMinBlocks, bool kScalars = false>
+__global__ void __launch_bounds__(kThreads, kMinBlocks)
+k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
+  if (!ctl->active) return;
+  extern __shared__ __align__(128) unsigned char smraw[];
+  const BlobLayout &L = A.L;
+  const int tid = threadIdx.x, b = blockIdx.x;
+  const int n_sp = kScalars ? A.sc.n : 0;
+  const int src = ctl->src;
+  const CellRec *__restrict__ in = src ? A.rec_b : A.rec_a;
+  CellRec *__restrict__ out = src ? A.rec_a : A.rec_b;
+  unsigned char *pf_out_base = src ? A.pflag_a : A.pflag_b;
+  const unsigned char *blob = A.blob + (size_t)b * (size_t)L.stride;
+  const int cell0 = b * L.P;                       // L.P <= kThreads: one thread per own cell
+  const int n_own = min(L.P, A.n_cells - cell0);
+
+  // ---- skip test (section 5b): when the own cells of this patch and of every patch that owns one of its halo cells
+  // are exactly (0, 0, 0) in the state being read, and no boundary string can feed the patch, every flux of S1 is
+  // exactly 0, theta = 1 and S3 returns (+0, 0, 0) for every own cell: write that (unless the target holds it already).
+  {
+    const ulonglong2 *pf = reinterpret_cast<const ulonglong2 *>((src ? A.pflag_b : A.pflag_a) + (size_t)b * kPflagBytes);
+    const ulonglong2 w0 = pf[0], w1 = pf[1];
+    const unsigned long long ones = 0x0101010101010101ull;
+    if (w0.x == ones && w0.y == ones && w1.x == ones && w1.y == ones) {
+      const unsigned char had = pf_out_base[(size_t)b * kPflagBytes + kPflagOwn];
+      if (!had) {
+        if (tid < n_own) {
+          CellRec c = in[cell0 + tid];
+          c.h = 0.0; c.qx = 0.0; c.qy = 0.0;
+          out[cell0 + tid] = c;
+          _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) (src ? A.sc.qa[sp] : A.sc.qb[sp])[cell0 + tid] = 0.0;   // flag: all q_c are 0 too
+        }
+        __syncthreads();            // every thread has read `had` before the flag changes
+        publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(blob + L.off_nbr), (const int32_t *)(blob + L.off_nbr_slot), L.cap_nbr, 1);
+      }
+      if (tid == 0) atomicAdd(&ctl->patches_skipped, 1ull);
+      return;
+    }
+  }
+
+  const Patch2Smem S = patch2_smem_layout(L, n_sp);
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smraw);
+  unsigned char *stage = smraw + S.stage;
+  CellRec *crec = reinterpret_cast<CellRec *>(smraw + S.crec);
+  double *sh_h = (double *)(smraw + S.h), *sh_u = (double *)(smraw + S.u), *sh_v = (double *)(smraw + S.v), *sh_z = (double *)(smraw + S.z);
+  double *sh_th = (double *)(smraw + S.theta), *sh_F1 = (double *)(smraw + S.F1), *sh_F3 = (double *)(smraw + S.F3);
+  double *sh_GL = (double *)(smraw + S.GL), *sh_GR = (double *)(smraw + S.GR), *sh_phi = (double *)(smraw + S.phi);
+  const int cap_loc = L.cap_loc;
+
+  // ---- the two bulk copies: staged part of the blob, own cell records
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    mbar_expect_tx(bar, (uint32_t)L.stage_bytes + 32u * (uint32_t)n_own);
+    bulk_g2s(stage, blob + L.off_stage, (uint32_t)L.stage_bytes, bar);
+    bulk_g2s(crec, in + cell0, 32u * (uint32_t)n_own, bar);
+  }
+  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+
+  // ---- phase 1a: halo cells (a gather: id -> record), while the bulk copies are in flight; velocities once per cell
+  // (R-8: thin films carry no momentum)
+  const int32_t *__restrict__ halo_ids = (const int32_t *)(blob + L.off_halo_ids);
+  int water = 0;
+  for (int j0 = tid; j0 < L.cap_halo; j0 += 2 * kThreads) {
+    const int j1 = j0 + kThreads;
+    const int id0 = halo_ids[j0];
+    const int id1 = j1 < L.cap_halo ? halo_ids[j1] : -1;
+    CellRec c0, c1;
+    if (id0 >= 0) c0 = in[id0];
+    if (id1 >= 0) c1 = in[id1];
+    if (id0 >= 0) {
+      const int l = n_own + j0;
+      double u = 0.0, v = 0.0;
+      if (c0.h > h_dry) { u = c0.qx / c0.h; v = c0.qy / c0.h; }
+      sh_h[l] = c0.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c0.z;
+      if (l < L.cap_c1) sh_th[l] = 1.0;
+      water |= (c0.h != 0.0);
+      if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
+        _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
+          sh_phi[sp * cap_loc + l] = c0.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[id0] / c0.h : 0.0;
+    }
+    if (id1 >= 0) {
+      const int l = n_own + j1;
+      double u = 0.0, v = 0.0;
+      if (c1.h > h_dry) { u = c1.qx / c1.h; v = c1.qy / c1.h; }
+      sh_h[l] = c1.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c1.z;
+      if (l < L.cap_c1) sh_th[l] = 1.0;
+      water |= (c1.h != 0.0);
+      if (kScalars)
+        _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
+          sh_phi[sp * cap_loc + l] = c1.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[id1] / c1.h : 0.0;
+    }
+  }
+  __syncthreads();                 // the mbarrier is initialised for every thread
+  mbar_wait(bar, 0);               // both bulk copies have landed
+
+  const BlobHeader H = *reinterpret_cast<const BlobHeader *>(stage + L.s_hdr);
+  const int n_c1 = H.n_own + H.n_r1, n_e = H.n_eown + H.n_er1;
+  const double *__restrict__ b_halo_area = (const double *)(stage + L.s_halo_area);
+  const uint4 *__restrict__ b_pce = (const uint4 *)(stage + L.s_pce);
+  const double *__restrict__ b_nx = (const double *)(stage + L.s_nx), *__restrict__ b_ny = (const double *)(stage + L.s_ny);
+  const double *__restrict__ b_len = (const double *)(stage + L.s_len);
+  const uint32_t *__restrict__ b_lr = (const uint32_t *)(stage + L.s_lr);
+  const int32_t *__restrict__ b_aux = (const int32_t *)(stage + L.s_aux);
+  const double *__restrict__ b_area = (const double *)(stage + L.s_area), *__restrict__ b_inv_area = (const double *)(stage + L.s_inv_area);
+  const double *__restrict__ b_gn2 = (const double *)(stage + L.s_gn2);
+
+  // ---- phase 1b: own cells, from the records the bulk copy delivered
+  if (tid < n_own) {
+    const CellRec c_own = crec[tid];
+    double u = 0.0, v = 0.0;
+    if (c_own.h > h_dry) { u = c_own.qx / c_own.h; v = c_own.qy / c_own.h; }
+    sh_h[tid] = c_own.h; sh_u[tid] = u; sh_v[tid] = v; sh_z[tid] = c_own.z; sh_th[tid] = 1.0;
+    water |= (c_own.h != 0.0);
+    if (kScalars)
+      _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
+        sh_phi[sp * cap_loc + tid] = c_own.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + tid] / c_own.h : 0.0;
+  }
+  // second, exact test on the local cells themselves (the flags above are per whole patch): no water in any
+  // local cell and no boundary string -> same result (+0, 0, 0)
+  if (!__syncthreads_or(water) && H.n_string_edges == 0) {
+    int scalar_mass = 0;
+    if (tid < n_own) {
+      CellRec c; c.h = 0.0; c.qx = 0.0; c.qy = 0.0; c.z = sh_z[tid];
+      out[cell0 + tid] = c;
+      _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {          // no flux: scalar mass parked in dry cells stays where it is
+        const double q = (src ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + tid];
+        (src ? A.sc.qa[sp] : A.sc.qb[sp])[cell0 + tid] = q;
+        scalar_mass |= (q != 0.0);
+      }
+    }
+    scalar_mass = kScalars ? __syncthreads_or(scalar_mass) : 0;
+    publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(blob + L.off_nbr), (const int32_t *)(blob + L.off_nbr_slot), L.cap_nbr,
+                           scalar_mass ? 0 : 1);
+    if (tid == 0) atomicAdd(&ctl->patches_skipped, 1ull);
+    return;
+  }
+
+  // ---- phase 2: edge fluxes
+  for (int e = tid; e < n_e; e += kThreads) {
+    const uint32_t lr = b_lr[e];
+    const int Lc = (int)(lr & 0xFFFFu), Rc = (int)(lr >> 16);
+    const double nx = b_nx[e], ny = b_ny[e], len = b_len[e];
+    const double hL = sh_h[Lc], uL = sh_u[Lc], vL = sh_v[Lc], zL = sh_z[Lc];
+    EdgeFlux o;
+    if (Rc != 0xFFFF) {
+      const double hR = sh_h[Rc], uR = sh_u[Rc], vR = sh_v[Rc], zR = sh_z[Rc];
+      const double unL = uL * nx + vL * ny, utL = vL * nx - uL * ny;
+      const double unR = uR * nx + vR * ny, utR = vR * nx - uR * ny;
+      o = riemann_nt(g, hL, unL, utL, zL, hR, unR, utR, zR);
+    } else {
+      const BoundaryString *bs = nullptr;
+      int code = b_aux[e];
+      if (code <= -3) { bs = A.strings + A.slot_string[-3 - code]; code = -3; }
+      const int gidL = Lc < n_own ? cell0 + Lc : halo_ids[Lc - n_own];
+      o = boundary_flux(g, code, bs, A.kst, gidL, nx, ny, len, hL, zL, uL, vL);
+    }
+    sh_F1[e] = o.F1;
+    if (e < H.n_eown) { sh_F3[e] = o.F3; sh_GL[e] = o.GL; sh_GR[e] = o.GR; }
+    // S1c, lazily (R-8b; as in k_edge_flux): theta_i < 1 needs one outgoing edge with dt * o_k > 0.3 h_i |Omega_i|.  Only
+    // such donor cells are marked (theta = -1); phase 3 evaluates theta for them and every other cell keeps theta = 1.
+    const int d = o.F1 > 0.0 ? Lc : ((o.F1 < 0.0 && Rc != 0xFFFF) ? Rc : n_c1);
+    if (d < n_c1) {
+      const double ad = d < n_own ? b_area[d] : b_halo_area[d - n_own];
+      if (dt * (len * fabs(o.F1)) > 0.3 * (sh_h[d] * ad)) sh_th[d] = -1.0;
+    }
+  }
+  __syncthreads();
+
+  // ---- phase 3 (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1)), slots in order -- for the
+  // cells marked in phase 2 only
+  for (int l = tid; l < n_c1; l += kThreads) {
+    if (sh_th[l] >= 0.0) continue;
+    const uint4 pc = b_pce[l];
+    const uint32_t w[3] = {pc.x, pc.y, pc.z};
+    double o[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const int e = w[k] & 0x7FFFu;
+      const double sM = ((w[k] & 0x8000u) ? 1.0 : -1.0) * (b_len[e] * sh_F1[e]);
+      o[k] = dmax0(sM);
+    }
+    const double outflow = ((o[0] + o[1]) + o[2]);
+    const double avail = sh_h[l] * (l < n_own ? b_area[l] : b_halo_area[l - n_own]);
+    double th = 1.0;
+    if (dt * outflow > avail) th = avail / (dt * outflow);
+    sh_th[l] = th;
+  }
+  __syncthreads();
+
+  // ---- phase 4: own cells, one per thread
+  double rate = 0.0;
+  int nonzero = 0;
+  if (tid < n_own) {
+    const int l = tid, i = cell0 + tid;
+    const uint4 pc = b_pce[l];
+    const CellRec c_own = crec[l];
+    const double invA = b_inv_area[l], f2 = b_gn2[l];
+    const uint32_t w[3] = {pc.x, pc.y, pc.z};
+    double dH = 0.0, dX = 0.0, dY = 0.0;             // ((d0 + d1) + d2), accumulated in slot order
+    double F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,
+    int up[3];                                       // local id of the upwind cell, or -1 - slot of an inflow-string edge
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const int e = w[k] & 0x7FFFu;
+      const bool isL = (w[k] & 0x8000u) != 0u;
+      const uint32_t nb = w[k] >> 16;
+      double F1 = sh_F1[e], F3 = sh_F3[e];
+      double G = isL ? sh_GL[e] : sh_GR[e];
+      // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
+      double th = 1.0;
+      if (F1 > 0.0) th = sh_th[isL ? (uint32_t)l : nb];
+      else if (F1 < 0.0 && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
+      if (th < 1.0) { F1 = th * F1; F3 = th * F3; G = th * G; }
+      const double s = isL ? 1.0 : -1.0;
+      const double nxk = b_nx[e], nyk = b_ny[e], lenk = b_len[e];
+      const double dHk = s * (lenk * F1);
+      const double dXk = s * (lenk * (G * nxk - F3 * nyk));
+      const double dYk = s * (lenk * (G * nyk + F3 * nxk));
+      if (k == 0) { dH = dHk; dX = dXk; dY = dYk; } else { dH = dH + dHk; dX = dX + dXk; dY = dY + dYk; }
+      if (kScalars) {
+        F1k[k] = F1; slk[k] = lenk;
+        const uint32_t Lc = isL ? (uint32_t)l : nb, Rc = isL ? nb : (uint32_t)l;
+        up[k] = (int)((F1 >= 0.0 || Rc == kPceNoNeighbour) ? Lc : Rc);   // ghost concentration = the interior cell's
+        if (!isL) slk[k] = -lenk;
+      }
+      if (nb == kPceNoNeighbour) {                  // boundary-string edge: volume bookkeeping of k_step_control
+        const int aux = b_aux[e];
+        if (aux <= -3) {
+          A.string_M[-3 - aux] = lenk * F1;
+          if (kScalars && !(F1 >= 0.0) && A.strings[A.slot_string[-3 - aux]].type == kBcInflowQ) up[k] = -1 - (-3 - aux);
+        }
+      }
+    }
+    const double a = dt * invA;
+    double hn = c_own.h - a * dH;
+    if (hn < 0.0) {                                  // residual negatives (R-8b): clip and count
+      atomicAdd(&ctl->vol_clipped, -hn * b_area[l]);
+      hn = 0.0;
+    }
+    double qxn = 0.0, qyn = 0.0;
+    if (hn > h_dry) {
+      qxn = c_own.qx - a * dX;
+      qyn = c_own.qy - a * dY;
+      if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
+        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_rn(hn));
+        qxn = qxn / D;
+        qyn = qyn / D;
+      }
+      // Eq. 21 (R-7) of the new state, for the next dt: max_j lambda_ij / rho_ij
+      const double u = qxn / hn, v = qyn / hn;
+      const double cel = sqrt(g * hn);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        const int e = w[k] & 0x7FFFu;
+        const double lam = fabs(u * b_nx[e] + v * b_ny[e]) + cel;
+        const double val = lam * ((0.75 * b_len[e]) * invA);
+        if (val > rate) rate = val;
+      }
+    }
+    CellRec c = c_own;
+    c.h = hn; c.qx = qxn; c.qy = qyn;
+    out[i] = c;
+    nonzero |= (hn != 0.0) | (qxn != 0.0) | (qyn != 0.0);
+    if (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
+      _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {
+        double dC = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const double phi = up[k] >= 0 ? sh_phi[sp * cap_loc + up[k]] : A.strings[A.slot_string[-1 - up[k]]].phi_in[sp];
+          const double lC = fabs(slk[k]) * (F1k[k] * phi);
+          const double Ck = slk[k] < 0.0 ? -lC : lC;
+          dC = k == 0 ? Ck : dC + Ck;
+        }
+        const double qn = (src ? A.sc.qb[sp] : A.sc.qa[sp])[i] - a * dC;
+        (src ? A.sc.qa[sp] : A.sc.qb[sp])[i] = qn;
+        nonzero |= (qn != 0.0);
+      }
+    }
+  }
+  nonzero = __syncthreads_or(nonzero);
+  publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(stage + L.s_nbr), (const int32_t *)(stage + L.s_nbr_slot), L.cap_nbr,
+                         nonzero ? 0 : 1);
+  block_max_to_global<kThreads>(rate, &ctl->rate_bits);
+}
+
+// flags after swe_set_state, two launches: (1) own flag of the buffer that holds the newest state from the records
+// (the other buffer: unknown = 0); (2) every patch collects its neighbours' own flags into its word
+template <int kThreads>
+__global__ void __launch_bounds__(kThreads)
+k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
+  const int b = blockIdx.x, cell0 = b * A.L.P, n_own = min(A.L.P, A.n_cells - cell0);
+  const CellRec *__restrict__ rec = ctl->cur ? A.rec_b : A.rec_a;
+  int nonzero = 0;
+  for (int l = threadIdx.x; l < n_own; l += kThreads) {
+    const CellRec c = rec[cell0 + l];
+    nonzero |= !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
+    _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < A.sc.n) nonzero |= ((ctl->cur ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + l] != 0.0);
+  }
+  nonzero = __syncthreads_or(nonzero);
+  if (threadIdx.x == 0) {
+    (ctl->cur ? A.pflag_b : A.pflag_a)[(size_t)b * kPflagBytes + kPflagOwn] = nonzero ? 0 : 1;
+    (ctl->cur ? A.pflag_a : A.pflag_b)[(size_t)b * kPflagBytes + kPflagOwn] = 0;
+  }
+}
+
+__global__ void __launch_bounds__(kBlock)
+k_patch2_nbr_flags(const Control *__restrict__ ctl, const Patch2Args A, int n_patches) {
+  const int p = blockIdx.x * kBlock + threadIdx.x;
+  if (p >= n_patches) return;
+  const unsigned char *blob = A.blob + (size_t)p * (size_t)A.L.stride;
+  const BlobHeader H = *reinterpret_cast<const BlobHeader *>(blob);
+  const int32_t *nbr = (const int32_t *)(blob + A.L.off_nbr);
+  unsigned char *cur = (ctl->cur ? A.pflag_b : A.pflag_a), *oth = (ctl->cur ? A.pflag_a : A.pflag_b);
+  for (int j = 0; j < kPflagSlots; ++j) {
+    unsigned char f = 1, fo = 1;                  // unused slots never veto
+    if (j < H.n_nbr) { f = cur[(size_t)nbr[j] * kPflagBytes + kPflagOwn]; fo = 0; }
+    cur[(size_t)p * kPflagBytes + j] = f;
+    oth[(size_t)p * kPflagBytes + j] = fo;
+  }
+  const unsigned char skippable = (H.n_string_edges == 0 && H.n_nbr <= kPflagSlots) ? 1 : 0;
+  cur[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
+  oth[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
+}
+
+}  // namespace swe

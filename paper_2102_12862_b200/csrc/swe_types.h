@@ -21,30 +21,70 @@ struct __align__(32) EdgeFlux {  // S1 outputs: F1 mass, F3 tangential momentum,
   double F1, F3, GL, GR;
 };
 
-// ---- fused patch step: the mesh is cut into patches of consecutive (Morton-ordered) cells;
-// one thread block advances one patch by a whole time step out of shared memory.
-//   local cells : [0, n_own) the patch's own cells, then ring 1 (cells sharing an edge with an own cell), then
-//                 ring 2 (cells sharing an edge with a ring-1 cell; needed because the limiter factor theta of a
-//                 ring-1 cell depends on all three of its edges)
-//   local edges : [0, n_eown) every edge of an own cell, then [n_eown, n_eown + n_er1) the other edges of ring 1
-struct __align__(16) PatchHeader {
-  int32_t cell0, n_own, n_r1, n_r2;
-  int32_t n_eown, n_er1;
-  int32_t halo_off;              // first entry of this patch in halo_ids[] / halo_area[]  (n_r1 + n_r2 entries)
-  int32_t edge_off;              // first record of this patch in pedge[]
-  int32_t pce_off;               // first record of this patch in pce[]  (n_own + n_r1 records)
-  int32_t n_string_edges;        // boundary-string edges among the local edges (such a patch is never skipped)
-  int32_t nbr_off, n_nbr;        // the patches that own this patch's ring-1 / ring-2 cells: entries of patch_nbr[]
-};
-
-struct __align__(32) PatchEdge { // geometry of section 4.1 + the two cells in patch-local numbering
-  double nx, ny, len;
-  uint16_t L, R;                 // R == 0xFFFF: boundary edge
-  int32_t aux;                   // boundary: -1 wall, -2 transmissive, <= -3: -3 - (position in string_edges[])
-};
-
 // pce[] record = uint4 {slot0, slot1, slot2, unused}; slot = edge (bits 0-14) | isL (bit 15) | neighbour cell (bits 16-31)
 constexpr uint32_t kPceNoNeighbour = 0xFFFFu;
+
+// ---- patch blobs: everything a patch streams lives in ONE contiguous, fixed-stride block of
+// device memory ("blob"), so that a thread block knows every address from blockIdx alone and pulls the part it
+// computes from into shared memory with one bulk asynchronous copy (cp.async.bulk + mbarrier).  All offsets are in
+// bytes from the start of the blob and are the same for every patch (capacities = maxima over the patches).
+//   [0, off_stage)          "cold" part, read straight from global memory when needed:
+//                             BlobHeader | nbr[cap_nbr] int32 | nbr_slot[cap_nbr] int32 | halo_ids[cap_halo] int32
+//   [off_stage, off_stage + stage_bytes)   staged into shared memory by the bulk copy, SoA (bank-conflict-free):
+//                             BlobHeader copy | nbr, nbr_slot copies | halo_area[cap_r1] | pce[cap_c1] uint4 | nx, ny, len [cap_e] double |
+//                             lr[cap_e] uint32 (L | R << 16; R = 0xFFFF boundary) | aux[cap_e] int32 |
+//                             area, inv_area, gn2 [P] double
+struct BlobHeader {              // 32 bytes
+  int32_t n_own, n_r1, n_r2, n_eown, n_er1, n_string_edges, n_nbr, pad_;
+};
+
+struct BlobLayout {
+  int32_t P;                     // own cells per patch (= threads per block)
+  int32_t cap_nbr, cap_halo, cap_r1, cap_c1, cap_loc, cap_e, cap_eown;
+  int32_t off_nbr, off_nbr_slot, off_halo_ids, off_stage;
+  // offsets RELATIVE TO off_stage (= offsets inside the staged copy in shared memory)
+  int32_t s_hdr, s_nbr, s_nbr_slot, s_halo_area, s_pce, s_nx, s_ny, s_len, s_lr, s_aux, s_area, s_inv_area, s_gn2;
+  int32_t stage_bytes;           // multiple of 16
+  int32_t stride;                // bytes per blob, multiple of 128
+};
+
+// per patch and state buffer: 32 flag bytes {neighbour 0..29 | own | skippable}; a byte is 1 when every own cell of
+// that patch is exactly (0, 0, 0) in that buffer (byte 31: 1 when the patch has no boundary-string edge and at most
+// kPflagSlots neighbours -- constant).  All 32 bytes == 1  <=>  the block may skip the patch (section 5b).
+constexpr int kPflagBytes = 32, kPflagSlots = 30, kPflagOwn = 30, kPflagSkippable = 31;
+
+__host__ __device__ inline int32_t blob_align(int32_t x, int32_t a) { return (x + a - 1) / a * a; }
+
+__host__ __device__ inline BlobLayout blob_layout(int P, int cap_nbr, int cap_halo, int cap_r1, int cap_e, int cap_eown) {
+  BlobLayout L;
+  L.P = P; L.cap_nbr = cap_nbr; L.cap_halo = cap_halo; L.cap_r1 = cap_r1; L.cap_c1 = P + cap_r1; L.cap_loc = P + cap_halo;
+  L.cap_e = cap_e; L.cap_eown = cap_eown;
+  int32_t o = (int32_t)sizeof(BlobHeader);
+  L.off_nbr = o; o += 4 * cap_nbr;
+  L.off_nbr_slot = o; o += 4 * cap_nbr;
+  L.off_halo_ids = o; o += 4 * cap_halo;
+  L.off_stage = blob_align(o, 128);
+  int32_t s = 0;
+  L.s_hdr = s; s += (int32_t)sizeof(BlobHeader);
+  L.s_nbr = s; s += 4 * cap_nbr;
+  L.s_nbr_slot = s; s += 4 * cap_nbr;
+  s = blob_align(s, 8);
+  L.s_halo_area = s; s += 8 * cap_r1;
+  s = blob_align(s, 16);
+  L.s_pce = s; s += 16 * L.cap_c1;
+  L.s_nx = s; s += 8 * cap_e;
+  L.s_ny = s; s += 8 * cap_e;
+  L.s_len = s; s += 8 * cap_e;
+  L.s_lr = s; s += 4 * cap_e;
+  L.s_aux = s; s += 4 * cap_e;
+  s = blob_align(s, 8);
+  L.s_area = s; s += 8 * P;
+  L.s_inv_area = s; s += 8 * P;
+  L.s_gn2 = s; s += 8 * P;
+  L.stage_bytes = blob_align(s, 16);
+  L.stride = blob_align(L.off_stage + L.stage_bytes, 128);
+  return L;
+}
 
 struct BoundaryString {          // one boundary string (R-11, R-12); lives in device memory
   int32_t type;                  // SWE_BC_*

@@ -47,13 +47,36 @@ def test_host_only_entry_points():
     L.swe_params_default(ctypes.byref(prm))
     assert prm.g == 9.81 and prm.h_dry == 1e-3 and prm.dt_max == float("inf")
     assert prm.renumber == P.RENUMBER_MORTON and prm.state_on_device == 0
-    a = L.swe_workspace_bytes(1000, 1600)
-    b = L.swe_workspace_bytes(1000, 0)           # n_edges unknown: worst case 3 N
-    c = L.swe_workspace_bytes(4_000_000, 6_010_000)
-    assert 0 < a <= b and a % 256 == 0
-    assert c >= 4_000_000 * 32 + 6_010_000 * 64   # at least the state records, edge geometry and edge fluxes
-    assert c < 4_000_000 * 400                    # a 4M-cell context stays well below 2 GB of the 180 GB
-    assert L.swe_workspace_bytes(-1, 0) == 0
+    assert prm.morphology == 0 and prm.n_species == 0 and prm.patch_cells == 0
+
+
+def test_workspace_bytes_sizes_every_array_on_the_host():
+    """swe_workspace_bytes(mesh, params) runs the host part of swe_create (no CUDA call, works here): the size covers
+    the base arrays, the patch blobs of the fused step, the scalar species and the mobile-bed arrays, and a mesh that
+    swe_create would reject gives 0 with a message."""
+    import numpy as np
+    import paper_2102_12862_b200 as P
+    from workloads import configs as C
+    w = C.by_id(4, 0.01)
+    N, E = w.n_cells, w.n_edges
+    args = (w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
+    three = P.workspace_bytes(*args, variant=P.VARIANT_THREE_PASS)
+    auto = P.workspace_bytes(*args)
+    assert three % 256 == 0 and three >= 64 * N + 64 * E          # both state buffers, edge geometry and edge fluxes
+    assert three < 400 * N + (1 << 20)                             # a 4M-cell context stays well below 2 GB of the 180 GB
+    st, _, _ = P.host_preprocess(*args, patch_cells=256)
+    assert auto - three >= st["patches"] * 64                      # + patch blobs and flag words
+    assert auto > three + 100 * N                                  # blobs: > 100 bytes per cell (edge records + slot words)
+    assert P.workspace_bytes(*args, n_species=2) - auto >= 2 * (16 * N + 8 * E)
+    assert P.workspace_bytes(*args, morphology=1) - auto >= 8 * E + 16 * N
+    assert P.workspace_bytes(*args, patch_cells=128, variant=P.VARIANT_PATCH) != P.workspace_bytes(*args, patch_cells=512, variant=P.VARIANT_PATCH)
+    # rejected arguments -> 0 and a reason
+    bad = w.tri.copy()
+    bad[0] = bad[0][::-1]                                          # a clockwise triangle
+    assert P.workspace_bytes(w.node_xy, bad, None, None, w.zb, w.kst) == 0
+    assert b"counter-clockwise" in P.lib().swe_last_error(None)
+    assert P.workspace_bytes(*args, n_species=6) == 0
+    assert P.workspace_bytes(*args, patch_cells=7) == 0
 
 
 def test_product_fails_loudly_without_gpu():

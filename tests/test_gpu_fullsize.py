@@ -115,7 +115,7 @@ def test_config4_full_size_mobile_bed(gpu, ref):
     bed elevation and every edge's q_Bij against the oracle over a short window; a cell no water ever reached keeps its
     bed (property that holds at any size)."""
     w = C.config4()
-    s = make(gpu, w)
+    s = make(gpu, w, morphology=True)
     o = ref.RefSolver(w)
     morph = (2, 8.0, 0.047, 2.65, 0.005, 0.4)
     s.set_morphology(*morph)

@@ -34,7 +34,7 @@ def assert_close(got, want, what):
 
 
 def both(gpu, ref, w, morph, chunks, **kw):
-    s = gpu.from_workload(w, **kw)
+    s = gpu.from_workload(w, morphology=True, **kw)
     o = ref.RefSolver(w)
     s.set_morphology(*morph)
     o.set_morphology(*morph)
@@ -87,7 +87,7 @@ def test_river_reach_with_wet_dry_fronts_and_strings(gpu, ref, morph):
 
 def test_switching_the_module_on_mid_run_and_off_again(gpu, ref):
     w = C.by_id(4, 0.01)
-    s, o = gpu.from_workload(w), ref.RefSolver(w)
+    s, o = gpu.from_workload(w, morphology=True), ref.RefSolver(w)
     assert s.step_kernels()[1] == "k_patch_step"             # AUTO picked the patch step for this half-dry reach
     for sol in (s, o):
         sol.step(45, float("inf"), w.cfl)
@@ -108,7 +108,7 @@ def test_switching_the_module_on_mid_run_and_off_again(gpu, ref):
 
 def test_zero_alpha_is_the_fixed_bed_scheme(gpu):
     w = mobile_dam_break()
-    a, b = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS), gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    a, b = gpu.from_workload(w, morphology=True, variant=gpu.VARIANT_THREE_PASS), gpu.from_workload(w, morphology=True, variant=gpu.VARIANT_THREE_PASS)
     b.set_morphology(GRASS, 0.0)
     a.step(64, float("inf"), w.cfl)
     b.step(64, float("inf"), w.cfl)
@@ -120,20 +120,25 @@ def test_zero_alpha_is_the_fixed_bed_scheme(gpu):
 
 def test_invalid_combinations_are_refused(gpu):
     w = mobile_dam_break()
-    s = gpu.from_workload(w, n_species=1)
+    s = gpu.from_workload(w, morphology=True, n_species=1)
     with pytest.raises(RuntimeError, match="scalars"):
         s.set_morphology(GRASS, 0.01)
     s.close()
-    s = gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=96)
+    s = gpu.from_workload(w, morphology=True, variant=gpu.VARIANT_PATCH, patch_cells=96)
     with pytest.raises(RuntimeError, match="patch"):
         s.set_morphology(GRASS, 0.01)
     s.close()
-    s = gpu.from_workload(w)
+    s = gpu.from_workload(w, morphology=True)
     for bad in [(3, 0.01), (GRASS, -1.0), (GRASS, 0.01, 0.047, 2.65, 1e-3, 1.0), (MPM, 8.0, 0.047, 1.0, 1e-3, 0.4),
                 (MPM, 8.0, 0.047, 2.65, 0.0, 0.4)]:
         with pytest.raises(RuntimeError):
             s.set_morphology(*bad)
-    with pytest.raises(RuntimeError, match="never switched on"):
+    assert np.all(s.sediment_fluxes() == 0.0)            # module reserved but never switched on: no transport yet
+    s.close()
+    s = gpu.from_workload(w)                             # a context created without room for the module (swe_params.morphology = 0)
+    with pytest.raises(RuntimeError, match="morphology"):
+        s.set_morphology(GRASS, 0.01)
+    with pytest.raises(RuntimeError, match="morphology"):
         s.sediment_fluxes()
     s.close()
 
@@ -152,12 +157,12 @@ def test_random_case_with_a_mobile_bed(gpu, ref, seed):
 def test_state_on_device_get_bed(gpu):
     import torch
     w = mobile_dam_break()
-    s = gpu.from_workload(w, state_on_device=True)
+    s = gpu.from_workload(w, morphology=True, state_on_device=True)
     s.set_morphology(GRASS, 0.02)
     s.step(10, float("inf"), w.cfl)
     zb = s.get_bed()
     assert zb.is_cuda and zb.shape == (w.n_cells,)
-    t = gpu.from_workload(w)
+    t = gpu.from_workload(w, morphology=True)
     t.set_morphology(GRASS, 0.02)
     t.step(10, float("inf"), w.cfl)
     assert np.array_equal(zb.cpu().numpy(), t.get_bed())
@@ -179,7 +184,7 @@ def test_bed_hump_celerity_on_a_fine_mesh(gpu):
     x = M.centroids(w.node_xy, w.tri)[:, 0]
     w.zb = 0.2 * np.exp(-((x - 200.0) / 20.0) ** 2)
     w.h = H - w.zb
-    s = gpu.from_workload(w)
+    s = gpu.from_workload(w, morphology=True)
     s.set_morphology(GRASS, alpha, porosity=p)
     area = s.geometry()[0]
     info = s.step(-1, T, 0.5)

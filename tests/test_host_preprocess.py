@@ -58,17 +58,17 @@ def test_tables_built_by_the_library_match_the_harness(P):
     assert a["n_edges"] == b["n_edges"] == w.n_edges
 
 
-@pytest.mark.parametrize("pc", [32, 384, 1000])
+@pytest.mark.parametrize("pc", [32, 256, 1000])
 def test_patch_tables(P, pc):
     w = C.by_id(4, 0.01)
     st, _, _ = P.host_preprocess(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst, patch_cells=pc)
     assert st["patches"] == -(-w.n_cells // pc)
     assert st["sum_own_cells"] == st["distinct_own_cells"] == w.n_cells      # the patches partition the cells
     assert st["sum_local_cells"] > w.n_cells and st["sum_local_edges"] > w.n_edges
-    if pc == 384:       # two halo rings of a compact 384-cell blob: 30-60 % more cells, < 45 % more edges; 3 blocks/SM fit
-        assert 1.2 < st["sum_local_cells"] / w.n_cells < 1.7
-        assert st["sum_local_edges"] / w.n_edges < 1.45
-        assert st["smem_bytes"] <= 75 * 1024
+    if pc == 256:       # two halo rings of a compact 256-cell blob: 30-70 % more cells, < 50 % more edges; 3 blocks/SM fit
+        assert 1.3 < st["sum_local_cells"] / w.n_cells < 1.7
+        assert st["sum_local_edges"] / w.n_edges < 1.5
+        assert 3 * (st["smem_bytes"] + 1024) <= 228 * 1024
     # on a random numbering the "patches" are not compact: the halos explode (AUTO then takes the three-pass step)
     wp, _ = w.permuted(3)
     bad, _, _ = P.host_preprocess(wp.node_xy, wp.tri, wp.edge_cell, wp.cell_edge, wp.zb, wp.kst, renumber=P.RENUMBER_NONE,

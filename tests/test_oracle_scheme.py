@@ -1,5 +1,7 @@
 """Pins for the oracle's geometry, time step (Eq. 21), friction source, limiter and bookkeeping.
 CPU only; every expected value is a closed form or a brute-force numpy evaluation written here."""
+import os
+
 import numpy as np
 import pytest
 
@@ -198,6 +200,39 @@ def test_draining_limiter_positivity_and_mass(ref):
     ln = s.geometry()[3]
     per = ln[w.cell_edge[i0]].sum()
     assert abs((1.0 - h2[i0]) - dt * per * (2.0 / 3.0) * np.sqrt(G) / area[i0]) < 1e-14
+
+
+def test_limiter_scales_every_flux_component_moving_water(ref):
+    """DESIGN R-8b with moving water, against values computed by hand (tests/golden/limiter_moving_water.txt): a fast
+    thin cell drains into a dry neighbour with theta = 0.8986; F1, F3, GL and GR of the edge are all scaled by theta,
+    the donor ends empty and the receiver gets exactly (dt/A) theta = 1/4 of every component.  Leaving G or F3
+    unscaled changes q_x by 11 % and q_y by 11 %."""
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "limiter_moving_water.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()
+            gold[k] = float(v)
+    w = C.tiny_mesh("two-cells-x")
+    e = int(np.nonzero((w.edge_cell[:, 0] == 0) & (w.edge_cell[:, 1] == 1))[0][0])      # the shared edge, L = cell 0
+    w.h[:] = [0.01, 0.0]
+    w.hu[:] = [0.04, 0.0]
+    w.hv[:] = [0.01, 0.0]
+    s = ref.RefSolver(w)
+    area, nx, ny, ln = s.geometry()
+    assert np.allclose(area, 0.5, rtol=0, atol=1e-16) and (nx[e], ny[e], ln[e]) == (1.0, 0.0, 1.0)
+    assert abs(s.peek_dt(0.9) - gold["dt"]) <= 1e-15
+    info = s.step(n_steps=1, cfl=0.9)
+    assert abs(info["dt_last"] - gold["dt"]) <= 1e-15
+    F1, F3, GL, GR = s.edge_fluxes()                                  # after the limiter
+    for name, got in (("F1", F1[e]), ("F3", F3[e]), ("GL", GL[e]), ("GR", GR[e])):
+        assert abs(got - gold[name]) <= 1e-15 * max(1.0, abs(gold[name])) * 4, (name, got, gold[name])
+    walls = np.arange(w.n_edges) != e
+    assert np.all(F1[walls] == 0.0) and np.all(F3[walls] == 0.0)     # reflective walls carry no mass
+    h, hu, hv = s.get_state()
+    assert abs(h[0] - gold["h0_new"]) <= 2e-18 and hu[0] == 0.0 and hv[0] == 0.0     # emptied: below h_dry, no momentum
+    assert abs(h[1] - gold["h1_new"]) <= 1e-17
+    assert abs(hu[1] - gold["qx1_new"]) <= 1e-16 and abs(hv[1] - gold["qy1_new"]) <= 1e-17
+    assert info["vol_clipped"] <= 1e-18 and abs((h * area).sum() - 0.005) <= 1e-18     # mass conserved, nothing clipped
 
 
 def test_restart_and_stop_conditions(ref):
