@@ -29,12 +29,38 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures under
-# profiles/ (kernel name, n_cells) -> bytes; absent -> "traffic": null
-NCU_TRAFFIC_BYTES = {("k_cell_update", 3964806): 726.9e6, ("k_theta_lazy", 3964806): 4.0e6,
-                     ("k_edge_flux", 3964806): 486.2e6,   # profiles/r1i_ncu_full_three_pass.md
-                     ("k_patch_step", 3964806): 502.0e6,  # profiles/r1i_ncu_full_patch_river.md (52 % of patches dry)
-                     ("k_patch_step", 3964136): 678.6e6}  # profiles/r1c_ncu_full_patch_allwet.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel come from profiles/ncu_traffic.csv: one row per
+# committed `ncu --set full` capture, keyed by kernel name, cell count AND the git blob hash of the source file the
+# kernel was compiled from at capture time -- a row whose hash is not the hash of that file as it stands is ignored
+# ("traffic": null), so the figure can never describe another kernel than the one being timed
+KERNEL_SOURCE = {"k_patch_step": "paper_2102_12862_b200/csrc/swe_patch2_kernel.cuh",
+                 "k_edge_flux": "paper_2102_12862_b200/csrc/swe_kernels.cuh",
+                 "k_theta_lazy": "paper_2102_12862_b200/csrc/swe_kernels.cuh",
+                 "k_cell_update": "paper_2102_12862_b200/csrc/swe_kernels.cuh",
+                 "k_step_control": "paper_2102_12862_b200/csrc/swe_kernels.cuh"}
+
+
+def git_blob_hash(path):
+    """sha1 of `blob <size>\0<content>`: what `git hash-object` prints, computed without git."""
+    import hashlib
+    data = open(os.path.join(ROOT, path), "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_traffic(kernel, n_cells):
+    """(bytes per launch, capture name) of the newest matching row of profiles/ncu_traffic.csv, else (None, None)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    src = KERNEL_SOURCE.get(kernel)
+    if not os.path.exists(path) or src is None:
+        return None, None
+    want = git_blob_hash(src)
+    hit = (None, None)
+    for row in csv.DictReader(line for line in open(path) if not line.startswith("#")):
+        if row["kernel"] == kernel and int(row["n_cells"]) == int(n_cells) and row["source_blob"] == want:
+            hit = (float(row["dram_bytes_per_launch"]), row["capture"])
+    return hit
+
 
 # --morph: parameter sets of swe_set_morphology (formula, alpha, theta_cr, s, d_m, porosity)
 MORPH_PARAMS = {1: (1, 0.001, 0.0, 2.65, 1e-3, 0.4), 2: (2, 8.0, 0.047, 2.65, 0.005, 0.4)}
@@ -61,6 +87,9 @@ def parse():
     ap.add_argument("--morph", type=int, default=0, choices=[0, 1, 2],
                     help="mobile bed (swe_set_morphology): 1 Grass-like alpha = 0.001, 2 MPM-like alpha = 8, d_m = 5 mm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-omp", action="store_true", help="also time the oracle source built with OpenMP on all host cores")
+    ap.add_argument("--parity-steps", type=int, default=5,
+                    help="time steps of the oracle window started from the state after the timed region (0 = off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-wet", action="store_true", help="skip the second (all-wet mesh) line")
     ap.add_argument("--no-other-variant", action="store_true", help="skip the other step variant's line")
@@ -190,10 +219,31 @@ def physical_gpu_index(local_rank):
     return local_rank
 
 
-def oracle_time(w, n_warm, max_steps, min_seconds, cfl, morph=0):
-    """The oracle as it stands on this box's host cores (single thread): (cell-updates/s, time steps timed, s)."""
+def pin_to_one_core():
+    """Pins this process to one of the cores it may run on (the oracle is timed single-threaded on a
+    pinned core); returns (core, previous affinity) or (None, None) where the platform has no such call."""
+    try:
+        prev = os.sched_getaffinity(0)
+        core = sorted(prev)[-1]
+        os.sched_setaffinity(0, {core})
+        return core, prev
+    except (AttributeError, OSError):
+        return None, None
+
+
+def unpin(prev):
+    if prev:
+        try:
+            os.sched_setaffinity(0, prev)
+        except OSError:
+            pass
+
+
+def oracle_time(w, n_warm, max_steps, min_seconds, cfl, morph=0, omp=False):
+    """The oracle as it stands on this box's host cores: (cell-updates/s, time steps timed, s).  omp=False: single
+    thread (the caller pins the process to one core); omp=True: the same source built with OpenMP, all cores."""
     from oracle import swe_ref
-    o = swe_ref.RefSolver(w)
+    o = swe_ref.RefSolver(w, omp=omp)
     if morph:
         o.set_morphology(*MORPH_PARAMS[morph])
     if n_warm:
@@ -215,6 +265,7 @@ def run_reference(args, rank):
         return
     from oracle import swe_ref
     w = load_workload(args.config, args.scale)
+    core, prev_aff = pin_to_one_core()
     o = swe_ref.RefSolver(w)
     if args.morph:
         o.set_morphology(*MORPH_PARAMS[args.morph])
@@ -225,8 +276,10 @@ def run_reference(args, rank):
         o.step(1, float("inf"), w.cfl)
     dt = time.perf_counter() - t0
     o.close()
+    unpin(prev_aff)
     value = w.n_cells * args.steps / dt
-    sample = f"all {w.n_cells} cells x 1 time step per step (the GPU arm's step is {args.time_steps} time steps)"
+    sample = (f"all {w.n_cells} cells x 1 time step per step (the GPU arm's step is {args.time_steps} time steps); "
+              f"single thread pinned to core {core}")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
@@ -238,6 +291,33 @@ def run_reference(args, rank):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def parity_window(s, w, info, n_steps):
+    """State after the timed region -> oracle (get_state -> set_state at the same t), then n_steps on both sides;
+    every cell compared at the north_star tolerances (|d| <= 1e-10 |ref| + 1e-14 max|ref|; dt <= 1e-12 relative;
+    identical wet/dry masks).  The oracle runs here as the checker of the timed state, outside every timed region."""
+    from oracle import swe_ref
+    st = s.get_state()
+    o = swe_ref.RefSolver(w)
+    o.set_state(*st, t0=info["t"])
+    s.set_state(*st, t0=info["t"])
+    ig, io = s.step(n_steps, float("inf"), w.cfl), o.step(n_steps, float("inf"), w.cfl)
+    got, want = s.get_state(), o.get_state()
+    o.close()
+    ok = bool(np.array_equal(got[0] > w.h_dry, want[0] > w.h_dry))
+    max_rel = 0.0
+    for a, b in zip(got, want):
+        scale = float(np.max(np.abs(b))) if b.size else 0.0
+        err = np.abs(a - b)
+        ok = ok and bool(np.all(err <= 1e-10 * np.abs(b) + 1e-14 * scale))
+        big = np.abs(b) > 1e-8 * scale
+        if np.any(big):
+            max_rel = max(max_rel, float(np.max(err[big] / np.abs(b[big]))))
+    dt_rel = abs(ig["dt_last"] - io["dt_last"]) / io["dt_last"] if io["dt_last"] else 0.0
+    ok = ok and dt_rel <= 1e-12 and ig["n_wet"] == io["n_wet"]
+    return {"parity_steps": n_steps, "parity_from_step": info["steps_done"], "parity_ok": ok, "max_rel_err": max_rel,
+            "dt_rel_err": dt_rel, "bit_identical": bool(all(np.array_equal(a, b) for a, b in zip(got, want)))}
 
 
 def main():
@@ -297,17 +377,27 @@ def main():
     sampler.start()
     launches0 = s.kernel_launches
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]    # one chunk = one bench step
     torch.cuda.synchronize()
     ev0.record(stream)
-    for _ in range(args.steps):
+    marks[0].record(stream)
+    for k in range(args.steps):
         s.step(T, float("inf"), w.cfl, info=False)
+        marks[k + 1].record(stream)
     ev1.record(stream)
     torch.cuda.synchronize()
     clocks = sampler.stop()
     barrier()
     ms = ev0.elapsed_time(ev1)
+    chunk_ms = [marks[k].elapsed_time(marks[k + 1]) for k in range(args.steps)]
+    ms_median = float(np.median(chunk_ms)) if chunk_ms else None
     launches = s.kernel_launches - launches0
     info = s.step(0, float("inf"), w.cfl, info=True)       # state check after the timed region: finite, mass balance
+    # ... and parity: the oracle continues from the GPU's state for a short window (rank 0, N = 1), all cells compared
+    parity = None
+    if rank == 0 and world == 1 and args.parity_steps > 0 and not args.species and not args.morph:
+        parity = parity_window(s, w, info, args.parity_steps)
+        info = s.step(0, float("inf"), w.cfl, info=True)
     ms = max_over_ranks(ms, world, dev)
     value = aggregate_value(N, T, args.steps, world, ms * 1e-3)
 
@@ -322,15 +412,24 @@ def main():
         # taken OUT of the algorithmic bytes (never counted as achieved bandwidth)
         f_skip = (st["patch_steps_skipped"] - skipped0) / max(1, args.profile_steps * max(1, st["patches"]))
         alg = {k: v * (1.0 - f_skip) if k == "k_patch_step" else v for k, v in s.algorithmic_bytes().items()}
+        # SURVEY.md section 8(d) "Algorithmic bytes per cell-step" (132 B one-pass, 284 B = 148 + 136 two-kernel) x the cells
+        # the launch actually processes: the basis of `achieved` / `frac`; the library's own count (32-byte records,
+        # DESIGN.md section 6) gives `frac_own_count`
+        surv = {k: v * (1.0 - f_skip) if k == "k_patch_step" else v for k, v in s.survey_bytes().items()}
         top = max(kernel_ms, key=kernel_ms.get)
         peak, how = peaks()
-        achieved = alg[top] / (kernel_ms[top] * 1e-3) / 1e9
+        achieved = surv[top] / (kernel_ms[top] * 1e-3) / 1e9
+        achieved_own = alg[top] / (kernel_ms[top] * 1e-3) / 1e9
+        traffic, capture = ncu_traffic(top, N)
         roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((top, N)), "peak_source": how,
-                    "algorithmic_bytes_per_launch": alg[top], "kernel_ms": kernel_ms[top],
+                    "frac": achieved / peak, "traffic": traffic, "traffic_capture": capture, "peak_source": how,
+                    "bytes_basis": "SURVEY.md 8(d): %d B per cell-step x cells processed" % round(surv[top] / max(1.0, N * (1.0 - (f_skip if top == "k_patch_step" else 0.0)))),
+                    "algorithmic_bytes_per_launch": surv[top], "kernel_ms": kernel_ms[top],
+                    "frac_own_count": achieved_own / peak, "achieved_own_count": achieved_own,
+                    "own_count_bytes_per_launch": alg[top],
                     "dry_patch_fraction_skipped": f_skip,
-                    "step_algorithmic_bytes": sum(alg.values()),
-                    "step_achieved": sum(alg.values()) / (ms * 1e-3 / (T * args.steps)) / 1e9,
+                    "step_algorithmic_bytes": sum(surv.values()),
+                    "step_achieved": sum(surv.values()) / (ms * 1e-3 / (T * args.steps)) / 1e9,
                     "share_of_step": kernel_ms[top] / sum(kernel_ms.values())}
         if top == "k_patch_step":
             roofline["note"] = ("the fused patch step moves about a third of the bytes of the bandwidth-bound "
@@ -388,7 +487,7 @@ def main():
         torch.cuda.synchronize()
         ms3 = ev0.elapsed_time(ev1)
         km3 = s3.profile_step(16, w.cfl)
-        alg3 = s3.algorithmic_bytes()
+        alg3 = s3.survey_bytes()
         pk = peaks()[0]
         other = {"step_kernels": s3.step_kernels(), "value": N * T * 5 / (ms3 * 1e-3), "unit": UNIT,
                  "ms_per_time_step": ms3 / (5 * T), "kernel_ms": km3,
@@ -416,7 +515,7 @@ def main():
         ms2 = ev0.elapsed_time(ev1)
         km2 = s2.profile_step(16, w2.cfl)
         i2 = s2.step(0, float("inf"), w2.cfl, info=True)
-        alg2 = s2.algorithmic_bytes()
+        alg2 = s2.survey_bytes()
         top2 = max(km2, key=km2.get)
         all_wet = {"workload": w2.name, "n_cells": w2.n_cells, "value": w2.n_cells * T * 5 / (ms2 * 1e-3), "unit": UNIT,
                    "ms_per_time_step": ms2 / (5 * T), "kernel_ms": km2, "n_wet": i2["n_wet"],
@@ -428,14 +527,21 @@ def main():
     # ---- CPU baseline: the oracle, single thread, bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        core, prev_aff = pin_to_one_core()
         v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl, args.morph)
+        unpin(prev_aff)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"all {N} cells x {n_done} time steps from the initial state ({secs:.1f} s, 1 thread)"}
+               "sample": f"all {N} cells x {n_done} time steps from the initial state ({secs:.1f} s, 1 thread pinned to core {core})"}
+        if args.cpu_omp:        # PAPER.md:427 (the `omp` backend): the same oracle source, OpenMP on every host core
+            v2, n2, secs2 = oracle_time(w, 1, 40, 8.0, w.cfl, args.morph, omp=True)
+            cpu["omp"] = {"value": v2, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle, OpenMP build",
+                          "sample": f"all {N} cells x {n2} time steps ({secs2:.1f} s)"}
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "ms_per_step_median": ms_median,
+            "ms_per_step_chunks": chunk_ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
@@ -444,8 +550,8 @@ def main():
             "ms_per_time_step": ms / (args.steps * T),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "kernel_ms": kernel_ms, "cpu_baseline": cpu, "all_wet": all_wet, "other_variant": other,
-            "state_check": {"t": info["t"], "steps_done": info["steps_done"], "n_wet": info["n_wet"],
-                            "vol_clipped": info["vol_clipped"], "flags": info["flags"]},
+            "state_check": dict({"t": info["t"], "steps_done": info["steps_done"], "n_wet": info["n_wet"],
+                                 "vol_clipped": info["vol_clipped"], "flags": info["flags"]}, **(parity or {})),
         }
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -201,6 +201,10 @@ const char *swe_step_kernel_name(const swe_ctx *ctx, int k);
 /* algorithmic DRAM bytes per launch of kernel k of the step: every datum the kernel needs counted once at the size
  * of the record that carries it; re-reads of halo cells / duplicated records are NOT counted */
 int64_t swe_algorithmic_bytes(const swe_ctx *ctx, int k);
+/* the same on the per-cell figures of SURVEY.md section 8(d) ("Algorithmic bytes per cell-step"): 132 B x n_cells for
+ * the one-pass fused step; 284 B x n_cells for the edge-flux -> gather design, split 148 (edge pass) + 136 (cell pass);
+ * + 16 B per cell and scalar species.  bench.py reports the roofline fraction on both counts. */
+int64_t swe_survey_bytes(const swe_ctx *ctx, int k);
 /* out[0..11] = variant, patches, cells per patch, dynamic shared memory per block [bytes], sum over patches of local
  * cells, sum over patches of local edges, largest local cell count, largest local edge count, the number of
  * patch-steps since swe_create in which a block found its whole patch dry and skipped the flux work, the

@@ -19,5 +19,32 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+LIB_F32 = os.path.join(HERE, "libswe_ref_f32.so")
+
+
+def build_f32(force: bool = False) -> str:
+    """The same source with -DSWE_REF_REAL=float: the single-precision oracle."""
+    if not force and os.path.exists(LIB_F32) and all(os.path.getmtime(LIB_F32) >= os.path.getmtime(d) for d in DEPS):
+        return LIB_F32
+    cmd = ["g++", "-std=c++17", "-O2", "-DSWE_REF_REAL=float", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+           "-Wall", "-Wextra", "-Wdouble-promotion", "-o", LIB_F32] + SRC
+    subprocess.run(cmd, check=True)
+    return LIB_F32
+
+
+LIB_OMP = os.path.join(HERE, "libswe_ref_omp.so")
+
+
+def build_omp(force: bool = False) -> str:
+    """The same source with -fopenmp -DSWE_REF_OMP: bench.py's optional cpu_baseline_omp line (the
+    paper's `omp` backend).  No test uses it."""
+    if not force and os.path.exists(LIB_OMP) and all(os.path.getmtime(LIB_OMP) >= os.path.getmtime(d) for d in DEPS):
+        return LIB_OMP
+    cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-DSWE_REF_OMP", "-ffp-contract=off", "-fno-fast-math", "-fPIC",
+           "-shared", "-Wall", "-Wextra", "-o", LIB_OMP] + SRC
+    subprocess.run(cmd, check=True)
+    return LIB_OMP
+
+
 if __name__ == "__main__":
     print(build(force=True))

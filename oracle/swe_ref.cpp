@@ -14,6 +14,32 @@
 #include <string>
 #include <vector>
 
+// Optional OpenMP build (oracle/build.py build_omp(): -fopenmp -DSWE_REF_OMP), the analogue of the paper's `omp`
+// backend (Table 3) for bench.py's cpu_baseline_omp line ONLY: the loops below are race-free as written
+// (per-edge outputs in the edge loops, per-cell outputs in the cell loops, gather in slot order), so the same source
+// runs them in parallel with identical results.  The default build, which every test uses, is single-threaded.
+#if defined(SWE_REF_OMP)
+#define SWE_REF_PARALLEL_FOR _Pragma("omp parallel for schedule(static)")
+#define SWE_REF_PARALLEL_MAX(r) _Pragma("omp parallel for schedule(static) reduction(max : r)")
+#define SWE_REF_ATOMIC _Pragma("omp atomic")
+#else
+#define SWE_REF_PARALLEL_FOR
+#define SWE_REF_PARALLEL_MAX(r)
+#define SWE_REF_ATOMIC
+#endif
+
+// Precision switch ("single or double"): the SAME source builds the fp64
+// oracle (default) and, with -DSWE_REF_REAL=float (oracle/build.py build_f32()), the single-precision oracle.  `real`
+// is the type of the state, the geometry and every flux / update operation; RL(x) is the literal x in that type.  What
+// stays fp64 in both builds: time and the time step (t, dt = cfl / rate, t_end), the hydrograph lookup, the volume
+// bookkeeping, and the mesh geometry as computed from the node coordinates (rounded once to `real` when stored).
+// The cube root of a `real` is the correctly rounded fp64 cube root rounded to `real` (R-14, R-21).
+#ifndef SWE_REF_REAL
+#define SWE_REF_REAL double
+#endif
+typedef SWE_REF_REAL real;
+#define RL(x) (static_cast<real>(x))
+
 namespace {
 
 struct BString {
@@ -22,7 +48,7 @@ struct BString {
   std::vector<int32_t> edges;  // members in ascending (caller) edge id = "string order"
   std::vector<double> phi_in;  // scalar concentrations carried by an INFLOW_Q string, one per species (default 0)
   // values fixed at t^n by eval_strings():
-  double Q = 0.0, sumK = 0.0, sumL = 0.0;
+  real Q = 0, sumK = 0, sumL = 0;
 };
 
 thread_local std::string g_create_error;
@@ -31,21 +57,22 @@ thread_local std::string g_create_error;
 
 struct swe_ref_ctx {
   int64_t nc = 0, ne = 0;
-  double g = 9.81, h_dry = 1e-3, dt_max = std::numeric_limits<double>::infinity();
-  std::vector<double> area, invA, gn2, zb, kst;
+  real g = RL(9.81), h_dry = RL(1e-3);
+  double dt_max = std::numeric_limits<double>::infinity();
+  std::vector<real> area, invA, gn2, zb, kst;
   std::vector<int32_t> eL, eR, ce;      // ce[3*i+k]
-  std::vector<double> nx, ny, len;      // per edge, normal from L to R  [PAPER.md:228]
-  std::vector<double> h, qx, qy;
-  std::vector<double> F1, F3, GL, GR;   // per edge, most recent step (after the limiter)
-  std::vector<double> theta;            // per cell, most recent step
+  std::vector<real> nx, ny, len;        // per edge, normal from L to R  [PAPER.md:228]
+  std::vector<real> h, qx, qy;
+  std::vector<real> F1, F3, GL, GR;     // per edge, most recent step (after the limiter)
+  std::vector<real> theta;              // per cell, most recent step
   // passive scalars (section 3.3, Eq. 8 advective part; Eq. 20 with A_ij only): specific mass q_c = h phi_c
   int n_species = 0;
-  std::vector<std::vector<double>> qc;  // [species][cell]
-  std::vector<std::vector<double>> Ac;  // [species][edge] advective scalar flux of the most recent step
+  std::vector<std::vector<real>> qc;    // [species][cell]
+  std::vector<std::vector<real>> Ac;    // [species][edge] advective scalar flux of the most recent step
   // morphodynamics (section 3.2 Eq. 3, section 4.3 Eq. 13-16; R-20): 0 = fixed bed
   int morph_formula = 0;
   double morph_alpha = 0.0, morph_theta_cr = 0.047, morph_s = 2.65, morph_dm = 1e-3, morph_p = 0.4;
-  std::vector<double> qB;               // per edge: normal sediment flux q_Bij of the most recent step
+  std::vector<real> qB;                 // per edge: normal sediment flux q_Bij of the most recent step
   std::map<int, BString> strings;
   double t = 0.0, dt_last = 0.0, vol_clipped = 0.0, vol_in = 0.0, vol_out = 0.0;
   int64_t steps_done = 0;
@@ -57,65 +84,74 @@ struct swe_ref_ctx {
 // S1, interior edge. PAPER.md:252 (HLLC, "Chapter 10 of [18]"), PAPER.md:254 (modified-state bed
 // slope of ref [69]); arithmetic exactly as SURVEY.md 8(c) S1 / DESIGN.md R-1, R-2, R-3.
 // ------------------------------------------------------------------------------------------------
-static void riemann_nt(double g, double heL, double unL, double utL, double zL,
-                       double heR, double unR, double utR, double zR,
-                       double *F1o, double *F3o, double *GLo, double *GRo) {
-  const double dz = zR - zL;
-  const double hsL = std::fmax(0.0, heL - std::fmax(0.0, dz));    // face depths over z* = max(zL, zR)
-  const double hsR = std::fmax(0.0, heR - std::fmax(0.0, -dz));
-  if (hsL == 0.0 && hsR == 0.0) {
-    *F1o = 0.0; *F3o = 0.0; *GLo = 0.0; *GRo = 0.0;
+static void riemann_nt(real g, real heL, real unL, real utL, real zL,
+                       real heR, real unR, real utR, real zR,
+                       real *F1o, real *F3o, real *GLo, real *GRo) {
+  const real dz = zR - zL;
+  const real hsL = std::fmax(RL(0.0), heL - std::fmax(RL(0.0), dz));    // face depths over z* = max(zL, zR)
+  const real hsR = std::fmax(RL(0.0), heR - std::fmax(RL(0.0), -dz));
+  if (hsL == RL(0.0) && hsR == RL(0.0)) {
+    *F1o = RL(0.0); *F3o = RL(0.0); *GLo = RL(0.0); *GRo = RL(0.0);
     return;
   }
-  const double cL = std::sqrt(g * hsL), cR = std::sqrt(g * hsR);
-  double SL, SR;
-  if (hsL > 0.0 && hsR > 0.0) {                  // two-rarefaction estimates
-    const double us = 0.5 * (unL + unR) + (cL - cR);
-    const double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
+  const real cL = std::sqrt(g * hsL), cR = std::sqrt(g * hsR);
+  real SL, SR;
+  if (hsL > RL(0.0) && hsR > RL(0.0)) {                  // two-rarefaction estimates
+    const real us = RL(0.5) * (unL + unR) + (cL - cR);
+    const real cs = RL(0.5) * (cL + cR) + RL(0.25) * (unL - unR);
     SL = std::fmin(unL - cL, us - cs);
     SR = std::fmax(unR + cR, us + cs);
-  } else if (hsR == 0.0) {                       // dry bed on the right
+  } else if (hsR == RL(0.0)) {                       // dry bed on the right
     SL = unL - cL;
-    SR = unL + 2.0 * cL;
+    SR = unL + RL(2.0) * cL;
   } else {                                       // dry bed on the left
-    SL = unR - 2.0 * cR;
+    SL = unR - RL(2.0) * cR;
     SR = unR + cR;
   }
-  const double qsL = hsL * unL, qsR = hsR * unR;
-  const double pL = (0.5 * g) * (hsL * hsL), pR = (0.5 * g) * (hsR * hsR);
-  const double FL1 = qsL, FL2 = qsL * unL + pL;
-  const double FR1 = qsR, FR2 = qsR * unR + pR;
-  double F1, F2;
-  if (SL >= 0.0) {
+  const real qsL = hsL * unL, qsR = hsR * unR;
+  const real pL = (RL(0.5) * g) * (hsL * hsL), pR = (RL(0.5) * g) * (hsR * hsR);
+  const real FL1 = qsL, FL2 = qsL * unL + pL;
+  const real FR1 = qsR, FR2 = qsR * unR + pR;
+  real F1, F2;
+  if (SL >= RL(0.0)) {
     F1 = FL1; F2 = FL2;
-  } else if (SR <= 0.0) {
+  } else if (SR <= RL(0.0)) {
     F1 = FR1; F2 = FR2;
   } else {                                       // HLL written as F_L + increment
-    const double inv = 1.0 / (SR - SL);
+    const real inv = RL(1.0) / (SR - SL);
     F1 = FL1 + (SL * (SR * (hsR - hsL) - (FR1 - FL1))) * inv;
     F2 = FL2 + (SL * (SR * (qsR - qsL) - (FR2 - FL2))) * inv;
   }
-  const double F3 = F1 * (F1 >= 0.0 ? utL : utR);  // contact wave: upwind tangential velocity
+  const real F3 = F1 * (F1 >= RL(0.0) ? utL : utR);  // contact wave: upwind tangential velocity
   *F1o = F1;
   *F3o = F3;
   *GLo = F2 - pL;                                  // per-side hydrostatic (bed-slope) correction
   *GRo = F2 - pR;
 }
 
+// one interior edge from the cell states: rotation into the (normal, tangential) frame of the edge, then riemann_nt
+static void edge_flux(real g, real heL, real uL, real vL, real zL, real heR, real uR, real vR, real zR, real nx, real ny,
+                      real *F1o, real *F3o, real *GLo, real *GRo) {
+  const real unL = uL * nx + vL * ny, utL = vL * nx - uL * ny;
+  const real unR = uR * nx + vR * ny, utR = vR * nx - uR * ny;
+  riemann_nt(g, heL, unL, utL, zL, heR, unR, utR, zR, F1o, F3o, GLo, GRo);
+}
+
 extern "C" void swe_ref_edge_flux(double g, double heL, double uL, double vL, double zL,
                                   double heR, double uR, double vR, double zR, double nx, double ny,
                                   double *F1o, double *F3o, double *GLo, double *GRo) {
-  const double unL = uL * nx + vL * ny, utL = vL * nx - uL * ny;
-  const double unR = uR * nx + vR * ny, utR = vR * nx - uR * ny;
-  riemann_nt(g, heL, unL, utL, zL, heR, unR, utR, zR, F1o, F3o, GLo, GRo);
+  real F1, F3, GL, GR;
+  edge_flux(RL(g), RL(heL), RL(uL), RL(vL), RL(zL), RL(heR), RL(uR), RL(vR), RL(zR), RL(nx), RL(ny), &F1, &F3, &GL, &GR);
+  *F1o = F1; *F3o = F3; *GLo = GL; *GRo = GR;
 }
 
 // wall evaluated through the solver with a mirror ghost (u_n -> -u_n): used only by the pin that
 // checks the closed form in boundary_flux() against it.
 extern "C" void swe_ref_wall_flux_via_ghost(double g, double he, double un, double ut,
                                             double *F1o, double *F3o, double *Go) {
-  double GR;
-  riemann_nt(g, he, un, ut, 0.0, he, -un, ut, 0.0, F1o, F3o, Go, &GR);
+  real F1, F3, G, GR;
+  riemann_nt(RL(g), RL(he), RL(un), RL(ut), RL(0.0), RL(he), -RL(un), RL(ut), RL(0.0), &F1, &F3, &G, &GR);
+  *F1o = F1; *F3o = F3; *Go = G;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -181,22 +217,24 @@ namespace {
 
 // fixed-shape pairwise tree in string order (R-11): pad to a power of two with zeros,
 // then add neighbours at stride 1, 2, 4, ...
-double tree_sum(std::vector<double> v) {
-  if (v.empty()) return 0.0;
+real tree_sum(std::vector<real> v) {
+  if (v.empty()) return RL(0.0);
   size_t P = 1;
   while (P < v.size()) P <<= 1;
-  v.resize(P, 0.0);
+  v.resize(P, RL(0.0));
   for (size_t s = 1; s < P; s <<= 1)
     for (size_t i = 0; i + s < P; i += 2 * s) v[i] = v[i] + v[i + s];
   return v[0];
 }
 
-inline double pow53(double he) {       // he^(5/3)
-  const double c3 = swe_ref_cbrt(he);
+inline real cbrt_real(real x) { return RL(swe_ref_cbrt((double)x)); }   // fp64: swe_ref_cbrt itself
+
+inline real pow53(real he) {           // he^(5/3)
+  const real c3 = cbrt_real(he);
   return (he * c3) * c3;
 }
 
-inline double kweight(double k) { return std::isfinite(k) ? k : 1.0; }
+inline real kweight(real k) { return std::isfinite(k) ? k : RL(1.0); }
 
 double hydrograph(const std::vector<double> &p, double t) {  // piecewise linear, clamped
   const size_t m = p.size() / 2;
@@ -214,16 +252,17 @@ double hydrograph(const std::vector<double> &p, double t) {  // piecewise linear
 inline bool is_wet(const swe_ref_ctx *c, int64_t i) { return c->h[i] > c->h_dry; }
 
 // S0 -- Eq. 21: rho_ij = 2 * dist(centroid, edge j) = 4|Omega_i| / (3 l_ij)
-double max_rate(const swe_ref_ctx *c) {
-  double r = 0.0;
+real max_rate(const swe_ref_ctx *c) {
+  real r = RL(0.0);
+  SWE_REF_PARALLEL_MAX(r)
   for (int64_t i = 0; i < c->nc; ++i) {
     if (!(c->h[i] > c->h_dry)) continue;
-    const double u = c->qx[i] / c->h[i], v = c->qy[i] / c->h[i];
-    const double cel = std::sqrt(c->g * c->h[i]);
+    const real u = c->qx[i] / c->h[i], v = c->qy[i] / c->h[i];
+    const real cel = std::sqrt(c->g * c->h[i]);
     for (int k = 0; k < 3; ++k) {
       const int32_t e = c->ce[3 * i + k];
-      const double lam = std::fabs(u * c->nx[e] + v * c->ny[e]) + cel;
-      const double val = lam * ((0.75 * c->len[e]) * c->invA[i]);
+      const real lam = std::fabs(u * c->nx[e] + v * c->ny[e]) + cel;
+      const real val = lam * ((RL(0.75) * c->len[e]) * c->invA[i]);
       if (val > r) r = val;
     }
   }
@@ -233,7 +272,7 @@ double max_rate(const swe_ref_ctx *c) {
 struct DtChoice { double dt, t_new; bool unbounded; };
 
 DtChoice choose_dt(const swe_ref_ctx *c, double cfl, double t_end) {
-  const double r = max_rate(c);
+  const double r = (double)max_rate(c);
   double dt = (r > 0.0) ? cfl / r : c->dt_max;
   dt = std::fmin(dt, c->dt_max);
   const double rem = t_end - c->t;
@@ -248,10 +287,10 @@ DtChoice choose_dt(const swe_ref_ctx *c, double cfl, double t_end) {
 void eval_strings(swe_ref_ctx *c) {
   for (auto &kv : c->strings) {
     BString &s = kv.second;
-    s.Q = s.sumK = s.sumL = 0.0;
-    std::vector<double> a, b;
+    s.Q = s.sumK = s.sumL = RL(0.0);
+    std::vector<real> a, b;
     if (s.type == SWE_REF_BC_INFLOW_Q) {
-      s.Q = hydrograph(s.params, c->t);
+      s.Q = RL(hydrograph(s.params, c->t));
       for (int32_t e : s.edges) {
         const int64_t L = c->eL[e];
         a.push_back((c->len[e] * kweight(c->kst[L])) * pow53(c->h[L]));
@@ -266,11 +305,11 @@ void eval_strings(swe_ref_ctx *c) {
 void boundary_flux(swe_ref_ctx *c, int64_t e) {
   const int64_t L = c->eL[e];
   const int code = c->eR[e];
-  const double nx = c->nx[e], ny = c->ny[e];
-  const double he = c->h[L];
-  double u = 0.0, v = 0.0;
+  const real nx = c->nx[e], ny = c->ny[e];
+  const real he = c->h[L];
+  real u = RL(0.0), v = RL(0.0);
   if (is_wet(c, L)) { u = c->qx[L] / c->h[L]; v = c->qy[L] / c->h[L]; }
-  double F1 = 0.0, F3 = 0.0, GL = 0.0, GR = 0.0;
+  real F1 = RL(0.0), F3 = RL(0.0), GL = RL(0.0), GR = RL(0.0);
   const BString *s = nullptr;
   if (code <= -3) {
     auto it = c->strings.find(-3 - code);
@@ -278,23 +317,23 @@ void boundary_flux(swe_ref_ctx *c, int64_t e) {
   }
   if (code == -2) {
     // transmissive: ghost = copy of the interior state (R-10)
-    swe_ref_edge_flux(c->g, he, u, v, c->zb[L], he, u, v, c->zb[L], nx, ny, &F1, &F3, &GL, &GR);
+    edge_flux(c->g, he, u, v, c->zb[L], he, u, v, c->zb[L], nx, ny, &F1, &F3, &GL, &GR);
   } else if (s && s->type == SWE_REF_BC_INFLOW_Q) {
-    double qe;
-    if (s->sumK > 0.0) {
-      const double Ke = (c->len[e] * kweight(c->kst[L])) * pow53(he);
+    real qe;
+    if (s->sumK > RL(0.0)) {
+      const real Ke = (c->len[e] * kweight(c->kst[L])) * pow53(he);
       qe = ((s->Q * Ke) / s->sumK) / c->len[e];
     } else {
       qe = s->Q / s->sumL;
     }
     F1 = -qe;
-    GL = (he > 0.0) ? (qe * qe) / he : 0.0;
-    F3 = 0.0;
+    GL = (he > RL(0.0)) ? (qe * qe) / he : RL(0.0);
+    F3 = RL(0.0);
   } else if (s && s->type == SWE_REF_BC_OUTFLOW_UNIFORM) {
-    if (he > 0.0) {
-      const double sqrtS0 = std::sqrt(s->params.empty() ? 0.0 : s->params[0]);
-      const double qn = (kweight(c->kst[L]) * pow53(he)) * sqrtS0;
-      const double ut = v * nx - u * ny;
+    if (he > RL(0.0)) {
+      const real sqrtS0 = std::sqrt(s->params.empty() ? RL(0.0) : RL(s->params[0]));
+      const real qn = (kweight(c->kst[L]) * pow53(he)) * sqrtS0;
+      const real ut = v * nx - u * ny;
       F1 = qn;
       GL = (qn * qn) / he;
       F3 = qn * ut;
@@ -302,14 +341,14 @@ void boundary_flux(swe_ref_ctx *c, int64_t e) {
   } else {
     // wall (default): reflective; closed form of the mirror-ghost Riemann problem (R-9):
     // F1 = 0, F3 = 0, G = h u_n (u_n + S), S = max(c - u_n, c + u_n/2)
-    if (he > 0.0) {
-      const double un = u * nx + v * ny;
-      const double cel = std::sqrt(c->g * he);
-      const double S = std::fmax(cel - un, cel + 0.5 * un);
+    if (he > RL(0.0)) {
+      const real un = u * nx + v * ny;
+      const real cel = std::sqrt(c->g * he);
+      const real S = std::fmax(cel - un, cel + RL(0.5) * un);
       GL = (he * un) * (un + S);
     }
   }
-  c->F1[e] = F1; c->F3[e] = F3; c->GL[e] = GL; c->GR[e] = 0.0;
+  c->F1[e] = F1; c->F3[e] = F3; c->GL[e] = GL; c->GR[e] = RL(0.0);
   (void)GR;
 }
 
@@ -361,57 +400,62 @@ namespace {
 // cell is dry (h <= h_dry), so an interface with a dry side carries none; walls carry none; through every open
 // boundary the interior cell's own flux leaves or enters (equilibrium boundary: q_Bij = q_Bi . n).
 void sediment_fluxes(swe_ref_ctx *c) {
+  SWE_REF_PARALLEL_FOR
   for (int64_t e = 0; e < c->ne; ++e) {
     const int64_t L = c->eL[e], R = c->eR[e];
-    c->qB[e] = 0.0;
+    c->qB[e] = RL(0.0);
     if (!is_wet(c, L) || R == -1) continue;
     double qi, psi, l1i, l2i;
     swe_ref_sediment_state(c->morph_formula, c->morph_alpha, c->morph_theta_cr, c->morph_s, c->morph_dm, c->g, c->h[L],
                            c->qx[L] / c->h[L], c->qy[L] / c->h[L], c->gn2[L], c->nx[e], c->ny[e], &qi, &psi, &l1i, &l2i);
-    if (R < 0) { c->qB[e] = qi; continue; }
+    if (R < 0) { c->qB[e] = RL(qi); continue; }
     if (!is_wet(c, R)) continue;
     double qj, l1j, l2j;
     swe_ref_sediment_state(c->morph_formula, c->morph_alpha, c->morph_theta_cr, c->morph_s, c->morph_dm, c->g, c->h[R],
                            c->qx[R] / c->h[R], c->qy[R] / c->h[R], c->gn2[R], c->nx[e], c->ny[e], &qj, &psi, &l1j, &l2j);
-    c->qB[e] = swe_ref_sediment_flux(qi, l1i, l2i, c->zb[L], qj, l1j, l2j, c->zb[R]);
+    c->qB[e] = RL(swe_ref_sediment_flux(qi, l1i, l2i, c->zb[L], qj, l1j, l2j, c->zb[R]));
   }
 }
 
-void one_step(swe_ref_ctx *c, double dt, double t_new) {
-  const double g = c->g;
+void one_step(swe_ref_ctx *c, const double dt_, const double t_new) {
+  const real g = c->g;
+  const real dt = RL(dt_);          // the step in the precision of the state (fp64: dt_ itself)
   eval_strings(c);
   // ---- S1 / S1b
+  SWE_REF_PARALLEL_FOR
   for (int64_t e = 0; e < c->ne; ++e) {
     const int64_t L = c->eL[e], R = c->eR[e];
     if (R < 0) { boundary_flux(c, e); continue; }
-    const double heL = c->h[L], heR = c->h[R];
-    double uL = 0, vL = 0, uR = 0, vR = 0;
+    const real heL = c->h[L], heR = c->h[R];
+    real uL = 0, vL = 0, uR = 0, vR = 0;
     if (is_wet(c, L)) { uL = c->qx[L] / c->h[L]; vL = c->qy[L] / c->h[L]; }
     if (is_wet(c, R)) { uR = c->qx[R] / c->h[R]; vR = c->qy[R] / c->h[R]; }
-    swe_ref_edge_flux(g, heL, uL, vL, c->zb[L], heR, uR, vR, c->zb[R], c->nx[e], c->ny[e],
-                      &c->F1[e], &c->F3[e], &c->GL[e], &c->GR[e]);
+    edge_flux(g, heL, uL, vL, c->zb[L], heR, uR, vR, c->zb[R], c->nx[e], c->ny[e],
+              &c->F1[e], &c->F3[e], &c->GL[e], &c->GR[e]);
   }
   if (c->morph_formula) sediment_fluxes(c);
   // ---- S1c draining-time limiter (R-8b): a cell may not lose more water than it holds.
   //      theta_i = min(1, h_i |Omega_i| / (dt * sum of its outgoing l F1)); every flux component of
   //      an edge is scaled by theta of the edge's donor cell (the cell the mass flux leaves).
+  SWE_REF_PARALLEL_FOR
   for (int64_t i = 0; i < c->nc; ++i) {
-    double o[3];
+    real o[3];
     for (int k = 0; k < 3; ++k) {
       const int32_t e = c->ce[3 * i + k];
-      const double sM = (c->eL[e] == i ? 1.0 : -1.0) * (c->len[e] * c->F1[e]);
-      o[k] = std::fmax(0.0, sM);
+      const real sM = (c->eL[e] == i ? RL(1.0) : -RL(1.0)) * (c->len[e] * c->F1[e]);
+      o[k] = std::fmax(RL(0.0), sM);
     }
-    const double out = ((o[0] + o[1]) + o[2]);
-    const double avail = c->h[i] * c->area[i];
-    c->theta[i] = (dt * out > avail) ? avail / (dt * out) : 1.0;
+    const real out = ((o[0] + o[1]) + o[2]);
+    const real avail = c->h[i] * c->area[i];
+    c->theta[i] = (dt * out > avail) ? avail / (dt * out) : RL(1.0);
   }
+  SWE_REF_PARALLEL_FOR
   for (int64_t e = 0; e < c->ne; ++e) {
     const int64_t L = c->eL[e], R = c->eR[e];
-    double th = 1.0;
-    if (c->F1[e] > 0.0) th = c->theta[L];
-    else if (c->F1[e] < 0.0 && R >= 0) th = c->theta[R];
-    if (th < 1.0) { c->F1[e] = th * c->F1[e]; c->F3[e] = th * c->F3[e]; c->GL[e] = th * c->GL[e]; c->GR[e] = th * c->GR[e]; }
+    real th = RL(1.0);
+    if (c->F1[e] > RL(0.0)) th = c->theta[L];
+    else if (c->F1[e] < RL(0.0) && R >= 0) th = c->theta[R];
+    if (th < RL(1.0)) { c->F1[e] = th * c->F1[e]; c->F3[e] = th * c->F3[e]; c->GL[e] = th * c->GL[e]; c->GR[e] = th * c->GR[e]; }
   }
   // ---- scalar advection, PAPER.md:204-208 (Eq. 8), PAPER.md:298-304 (Eq. 20, advective part A_ij): "the HLLC solver
   //      ... provides the advective component of the scalar fluxes" = the mass flux times the concentration on the
@@ -420,83 +464,89 @@ void one_step(swe_ref_ctx *c, double dt, double t_new) {
   //      mass than it holds.  Ghost concentrations: transmissive, wall, outflow = phi of the interior cell; an
   //      INFLOW_Q string carries the concentrations set with swe_ref_set_boundary_scalar.
   for (int sp = 0; sp < c->n_species; ++sp) {
-    const std::vector<double> &q = c->qc[sp];
+    const std::vector<real> &q = c->qc[sp];
     for (int64_t e = 0; e < c->ne; ++e) {
       const int64_t L = c->eL[e], R = c->eR[e];
-      const double phiL = c->h[L] > 0.0 ? q[L] / c->h[L] : 0.0;
-      double phiR = phiL;
-      if (R >= 0) phiR = c->h[R] > 0.0 ? q[R] / c->h[R] : 0.0;
+      const real phiL = c->h[L] > RL(0.0) ? q[L] / c->h[L] : RL(0.0);
+      real phiR = phiL;
+      if (R >= 0) phiR = c->h[R] > RL(0.0) ? q[R] / c->h[R] : RL(0.0);
       else if (R <= -3) {
         auto it = c->strings.find(-3 - (int)R);
         if (it != c->strings.end() && it->second.type == SWE_REF_BC_INFLOW_Q)
-          phiR = sp < (int)it->second.phi_in.size() ? it->second.phi_in[sp] : 0.0;
+          phiR = sp < (int)it->second.phi_in.size() ? RL(it->second.phi_in[sp]) : RL(0.0);
       }
-      c->Ac[sp][e] = c->F1[e] * (c->F1[e] >= 0.0 ? phiL : phiR);
+      c->Ac[sp][e] = c->F1[e] * (c->F1[e] >= RL(0.0) ? phiL : phiR);
     }
   }
   // ---- S2 + S3 (in place: the fluxes of step n are already stored per edge)
+  SWE_REF_PARALLEL_FOR
   for (int64_t i = 0; i < c->nc; ++i) {
-    double M[3], X[3], Y[3], s[3];
+    real M[3], X[3], Y[3], s[3];
     for (int k = 0; k < 3; ++k) {
       const int32_t e = c->ce[3 * i + k];
       const bool isL = (c->eL[e] == i);
-      const double G = isL ? c->GL[e] : c->GR[e];
-      const double l = c->len[e], nx = c->nx[e], ny = c->ny[e];
-      s[k] = isL ? 1.0 : -1.0;
+      const real G = isL ? c->GL[e] : c->GR[e];
+      const real l = c->len[e], nx = c->nx[e], ny = c->ny[e];
+      s[k] = isL ? RL(1.0) : -RL(1.0);
       M[k] = l * c->F1[e];
       X[k] = l * (G * nx - c->F3[e] * ny);
       Y[k] = l * (G * ny + c->F3[e] * nx);
     }
-    const double dH = ((s[0] * M[0] + s[1] * M[1]) + s[2] * M[2]);
-    const double dX = ((s[0] * X[0] + s[1] * X[1]) + s[2] * X[2]);
-    const double dY = ((s[0] * Y[0] + s[1] * Y[1]) + s[2] * Y[2]);
-    const double a = dt * c->invA[i];
-    double hn = c->h[i] - a * dH;
-    if (hn < 0.0) { c->vol_clipped += -hn * c->area[i]; hn = 0.0; }
-    double qxn = 0.0, qyn = 0.0;
+    const real dH = ((s[0] * M[0] + s[1] * M[1]) + s[2] * M[2]);
+    const real dX = ((s[0] * X[0] + s[1] * X[1]) + s[2] * X[2]);
+    const real dY = ((s[0] * Y[0] + s[1] * Y[1]) + s[2] * Y[2]);
+    const real a = dt * c->invA[i];
+    real hn = c->h[i] - a * dH;
+    if (hn < RL(0.0)) {
+      SWE_REF_ATOMIC
+      c->vol_clipped += (double)(-hn * c->area[i]);
+      hn = RL(0.0);
+    }
+    real qxn = RL(0.0), qyn = RL(0.0);
     if (hn > c->h_dry) {
       qxn = c->qx[i] - a * dX;
       qyn = c->qy[i] - a * dY;
-      if (c->gn2[i] > 0.0) {   // split friction, exact integral of dq/dt = -gamma |q| q (R-5, R-6)
-        const double D = 1.0 + ((dt * c->gn2[i]) * std::sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * swe_ref_cbrt(hn));
+      if (c->gn2[i] > RL(0.0)) {   // split friction, exact integral of dq/dt = -gamma |q| q (R-5, R-6)
+        const real D = RL(1.0) + ((dt * c->gn2[i]) * std::sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_real(hn));
         qxn = qxn / D;
         qyn = qyn / D;
       }
     }
     c->h[i] = hn; c->qx[i] = qxn; c->qy[i] = qyn;
     for (int sp = 0; sp < c->n_species; ++sp) {     // Eq. 20, advective part: same gather, same slot order
-      double C[3];
+      real C[3];
       for (int k = 0; k < 3; ++k) { const int32_t e = c->ce[3 * i + k]; C[k] = c->len[e] * c->Ac[sp][e]; }
-      const double dC = ((s[0] * C[0] + s[1] * C[1]) + s[2] * C[2]);
+      const real dC = ((s[0] * C[0] + s[1] * C[1]) + s[2] * C[2]);
       c->qc[sp][i] = c->qc[sp][i] - a * dC;
     }
   }
   // ---- Eq. 13, S_b = 0: z_B <- z_B - 1/(1-p) * dt/|Omega| * sum_j l_ij q_Bij, slots in order
   if (c->morph_formula) {
-    const double inv1mp = 1.0 / (1.0 - c->morph_p);
+    const real inv1mp = RL(1.0 / (1.0 - c->morph_p));
+    SWE_REF_PARALLEL_FOR
     for (int64_t i = 0; i < c->nc; ++i) {
-      double B[3], s[3];
+      real B[3], s[3];
       for (int k = 0; k < 3; ++k) {
         const int32_t e = c->ce[3 * i + k];
-        s[k] = (c->eL[e] == i) ? 1.0 : -1.0;
+        s[k] = (c->eL[e] == i) ? RL(1.0) : -RL(1.0);
         B[k] = c->len[e] * c->qB[e];
       }
-      const double dB = ((s[0] * B[0] + s[1] * B[1]) + s[2] * B[2]);
+      const real dB = ((s[0] * B[0] + s[1] * B[1]) + s[2] * B[2]);
       c->zb[i] = c->zb[i] - inv1mp * ((dt * c->invA[i]) * dB);
     }
   }
   for (auto &kv : c->strings) {      // bookkeeping from the (limited) fluxes actually applied
     BString &s = kv.second;
-    if (s.type == SWE_REF_BC_INFLOW_Q) c->vol_in += dt * s.Q;
+    if (s.type == SWE_REF_BC_INFLOW_Q) c->vol_in += dt_ * (double)s.Q;
     if (s.type == SWE_REF_BC_OUTFLOW_UNIFORM) {
-      std::vector<double> a;
+      std::vector<real> a;
       for (int32_t e : s.edges) a.push_back(c->len[e] * c->F1[e]);
-      c->vol_out += dt * tree_sum(a);
+      c->vol_out += dt_ * (double)tree_sum(a);
     }
   }
   // ---- S4
   c->t = t_new;
-  c->dt_last = dt;
+  c->dt_last = dt_;
   c->steps_done += 1;
 }
 
@@ -506,7 +556,7 @@ void fill_info(swe_ref_ctx *c, swe_ref_info *info) {
   int64_t nwet = 0;
   bool bad = false;
   for (int64_t i = 0; i < c->nc; ++i) {
-    vol += c->h[i] * c->area[i];
+    vol += (double)c->h[i] * (double)c->area[i];
     if (c->h[i] > c->h_dry) ++nwet;
     if (!std::isfinite(c->h[i]) || !std::isfinite(c->qx[i]) || !std::isfinite(c->qy[i])) bad = true;
   }
@@ -525,15 +575,17 @@ extern "C" int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, sw
   }
   swe_ref_ctx *c = new swe_ref_ctx;
   c->nc = m->n_cells; c->ne = m->n_edges;
-  if (p) { c->g = p->g; c->h_dry = p->h_dry; c->dt_max = p->dt_max; }
+  const double g64 = p ? p->g : 9.81;
+  if (p) { c->g = RL(p->g); c->h_dry = RL(p->h_dry); c->dt_max = p->dt_max; }
   const int64_t nc = c->nc, ne = c->ne;
   c->area.resize(nc); c->invA.resize(nc); c->gn2.resize(nc);
-  c->zb.assign(m->zb, m->zb + nc); c->kst.assign(m->kst, m->kst + nc);
+  c->zb.resize(nc); c->kst.resize(nc);
+  for (int64_t i = 0; i < nc; ++i) { c->zb[i] = RL(m->zb[i]); c->kst[i] = RL(m->kst[i]); }
   c->ce.assign(m->cell_edge, m->cell_edge + 3 * nc);
   c->eL.resize(ne); c->eR.resize(ne); c->nx.resize(ne); c->ny.resize(ne); c->len.resize(ne);
-  c->h.assign(nc, 0.0); c->qx.assign(nc, 0.0); c->qy.assign(nc, 0.0);
-  c->theta.assign(nc, 1.0);
-  c->F1.assign(ne, 0.0); c->F3.assign(ne, 0.0); c->GL.assign(ne, 0.0); c->GR.assign(ne, 0.0);
+  c->h.assign(nc, RL(0.0)); c->qx.assign(nc, RL(0.0)); c->qy.assign(nc, RL(0.0));
+  c->theta.assign(nc, RL(1.0));
+  c->F1.assign(ne, RL(0.0)); c->F3.assign(ne, RL(0.0)); c->GL.assign(ne, RL(0.0)); c->GR.assign(ne, RL(0.0));
   for (int64_t e = 0; e < ne; ++e) { c->eL[e] = m->edge_cell[2 * e]; c->eR[e] = m->edge_cell[2 * e + 1]; }
   // geometry, PAPER.md:226-228 (section 4.1, Fig. 2)
   for (int64_t i = 0; i < nc; ++i) {
@@ -543,10 +595,10 @@ extern "C" int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, sw
     const double x2 = m->node_xy[2 * t[2]], y2 = m->node_xy[2 * t[2] + 1];
     const double A = 0.5 * ((x1 - x0) * (y2 - y0) - (x2 - x0) * (y1 - y0));
     if (!(A > 0.0)) { g_create_error = "cell " + std::to_string(i) + " is not counter-clockwise / has no area"; delete c; return -2; }
-    c->area[i] = A;
-    c->invA[i] = 1.0 / A;
+    c->area[i] = RL(A);                  // geometry and constants: computed in fp64, rounded once to `real`
+    c->invA[i] = RL(1.0 / A);
     const double k = m->kst[i];
-    c->gn2[i] = std::isfinite(k) ? c->g / (k * k) : 0.0;
+    c->gn2[i] = std::isfinite(k) ? RL(g64 / (k * k)) : RL(0.0);
     for (int s = 0; s < 3; ++s) {
       const int32_t e = c->ce[3 * i + s];
       if (e < 0 || e >= ne) { g_create_error = "cell_edge out of range"; delete c; return -2; }
@@ -554,7 +606,7 @@ extern "C" int swe_ref_create(const swe_ref_mesh *m, const swe_ref_params *p, sw
         const int32_t a = t[s], b = t[(s + 1) % 3];
         const double dx = m->node_xy[2 * b] - m->node_xy[2 * a], dy = m->node_xy[2 * b + 1] - m->node_xy[2 * a + 1];
         const double l = std::sqrt(dx * dx + dy * dy);
-        c->len[e] = l; c->nx[e] = dy / l; c->ny[e] = -dx / l;
+        c->len[e] = RL(l); c->nx[e] = RL(dy / l); c->ny[e] = RL(-dx / l);
       } else if (c->eR[e] != i) {
         g_create_error = "edge_cell / cell_edge tables are inconsistent at cell " + std::to_string(i);
         delete c; return -2;
@@ -577,7 +629,7 @@ extern "C" int swe_ref_set_boundary(swe_ref_ctx *c, int string_id, int type, con
 
 extern "C" int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *hu, const double *hv, double t0) {
   if (!c || !h || !hu || !hv) return -1;
-  c->h.assign(h, h + c->nc); c->qx.assign(hu, hu + c->nc); c->qy.assign(hv, hv + c->nc);
+  for (int64_t i = 0; i < c->nc; ++i) { c->h[i] = RL(h[i]); c->qx[i] = RL(hu[i]); c->qy[i] = RL(hv[i]); }
   c->t = t0; c->dt_last = 0.0; c->steps_done = 0; c->vol_clipped = c->vol_in = c->vol_out = 0.0; c->flags = 0;
   return 0;
 }
@@ -585,9 +637,10 @@ extern "C" int swe_ref_set_state(swe_ref_ctx *c, const double *h, const double *
 extern "C" int swe_ref_set_scalars(swe_ref_ctx *c, int n_species, const double *qc) {
   if (!c || n_species < 0 || n_species > 5 || (n_species > 0 && !qc)) return -1;   // "up to a maximum of 5"
   c->n_species = n_species;
-  c->qc.assign(n_species, std::vector<double>(c->nc, 0.0));
-  c->Ac.assign(n_species, std::vector<double>(c->ne, 0.0));
-  for (int sp = 0; sp < n_species; ++sp) c->qc[sp].assign(qc + (size_t)sp * c->nc, qc + (size_t)(sp + 1) * c->nc);
+  c->qc.assign(n_species, std::vector<real>(c->nc, RL(0.0)));
+  c->Ac.assign(n_species, std::vector<real>(c->ne, RL(0.0)));
+  for (int sp = 0; sp < n_species; ++sp)
+    for (int64_t i = 0; i < c->nc; ++i) c->qc[sp][i] = RL(qc[(size_t)sp * c->nc + i]);
   return 0;
 }
 
@@ -611,18 +664,18 @@ extern "C" int swe_ref_set_morphology(swe_ref_ctx *c, int formula, double alpha,
   if (formula == 2 && !(sdens > 1.0 && dm > 0.0)) { c->err = "MPM-like formula needs s > 1 and d_m > 0"; return 1; }
   c->morph_formula = formula; c->morph_alpha = alpha; c->morph_theta_cr = theta_cr; c->morph_s = sdens; c->morph_dm = dm;
   c->morph_p = porosity;
-  c->qB.assign(c->ne, 0.0);
+  c->qB.assign(c->ne, RL(0.0));
   return 0;
 }
 
 extern "C" int swe_ref_get_bed(swe_ref_ctx *c, double *zb) {
-  std::memcpy(zb, c->zb.data(), sizeof(double) * c->nc);
+  for (int64_t i = 0; i < c->nc; ++i) zb[i] = c->zb[i];
   return 0;
 }
 
 extern "C" int swe_ref_get_sediment_flux(swe_ref_ctx *c, double *qB) {
   if (c->qB.empty()) { c->err = "morphodynamics is off"; return 1; }
-  std::memcpy(qB, c->qB.data(), sizeof(double) * c->ne);
+  for (int64_t e = 0; e < c->ne; ++e) qB[e] = c->qB[e];
   return 0;
 }
 

@@ -22,6 +22,11 @@
  * Morphodynamics (tests/test_oracle_morph.py): Table 2 by hand, psi of Eq. 16 by finite differences, Vieta's relations
  * of Eq. 16, HLL special cases of Eq. 14-15, Eq. 13 re-assembled with numpy, porosity factor, sediment volume in a closed
  * box, flat bed under a uniform stream, bed-hump celerity under the Grass-like law.
+ * Draining-time limiter with moving water: tests/golden/limiter_moving_water.txt (hand-computed: F1, F3, GL, GR all scaled).
+ * Builds of this one source (oracle/build.py): fp64 single-threaded (the default; every parity test), single precision
+ * (-DSWE_REF_REAL=float; R-21; pinned by tests/test_oracle_f32.py: golden values to fp32 round-off, mass, lake
+ * at rest, dam-break errors against the fp64 build), and an OpenMP build of the fp64 source for bench.py's optional
+ * cpu_baseline omp line (bit-identical results; no test depends on it).
  * "parity unpinned" items: none of the functions; but the *choice* of readings R-2 (HLLC form) and
  * R-11 (inflow distribution) cannot be pinned against BASEMENT itself (closed source).
  */

@@ -35,13 +35,16 @@ class Info(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        path = _build.build()
+def lib(omp=False, single=False):
+    """The oracle library: the single-threaded fp64 build (the default), the same source built for single precision
+    (single=True: -DSWE_REF_REAL=float), or -- omp=True, bench.py's cpu_baseline_omp line only --
+    the fp64 source built with OpenMP."""
+    omp = (bool(omp), bool(single))
+    if omp not in _libs:
+        path = _build.build_f32() if single else (_build.build_omp() if omp[0] else _build.build())
         L = C.CDLL(path)
         L.swe_ref_create.argtypes = [C.POINTER(_Mesh), C.POINTER(_Params), C.POINTER(C.c_void_p)]
         L.swe_ref_create.restype = C.c_int
@@ -73,8 +76,8 @@ def lib():
         L.swe_ref_peek_dt.restype = C.c_double
         L.swe_ref_cbrt.argtypes = [C.c_double]
         L.swe_ref_cbrt.restype = C.c_double
-        _lib = L
-    return _lib
+        _libs[omp] = L
+    return _libs[omp]
 
 
 def _p(a, typ):
@@ -117,8 +120,9 @@ def wall_flux_via_ghost(g, he, un, ut):
 class RefSolver:
     """Oracle context built from a workloads.configs.Workload (or the same arrays)."""
 
-    def __init__(self, w, g=None, h_dry=None, dt_max=None):
-        L = lib()
+    def __init__(self, w, g=None, h_dry=None, dt_max=None, omp=False, precision="double"):
+        assert precision in ("double", "single")
+        L = self._L = lib(omp, precision == "single")
         self._keep = dict(
             node_xy=np.ascontiguousarray(w.node_xy, np.float64), tri=np.ascontiguousarray(w.tri, np.int32),
             edge_cell=np.ascontiguousarray(w.edge_cell, np.int32), cell_edge=np.ascontiguousarray(w.cell_edge, np.int32),
@@ -140,77 +144,77 @@ class RefSolver:
 
     def set_boundary(self, string_id, typ, params):
         a = np.ascontiguousarray(params, np.float64)
-        rc = lib().swe_ref_set_boundary(self._h, int(string_id), int(typ), _p(a, _f64p), int(a.size))
+        rc = self._L.swe_ref_set_boundary(self._h, int(string_id), int(typ), _p(a, _f64p), int(a.size))
         assert rc == 0
 
     def set_state(self, h, hu, hv, t0=0.0):
         a = [np.ascontiguousarray(x, np.float64) for x in (h, hu, hv)]
         assert all(x.shape == (self.n_cells,) for x in a)
-        rc = lib().swe_ref_set_state(self._h, _p(a[0], _f64p), _p(a[1], _f64p), _p(a[2], _f64p), float(t0))
+        rc = self._L.swe_ref_set_state(self._h, _p(a[0], _f64p), _p(a[1], _f64p), _p(a[2], _f64p), float(t0))
         assert rc == 0
 
     def set_scalars(self, qc):
         """qc: [n_species, n_cells] specific masses q_c = h * phi_c."""
         a = np.ascontiguousarray(qc, np.float64).reshape(-1, self.n_cells)
         self.n_species = a.shape[0]
-        assert lib().swe_ref_set_scalars(self._h, int(a.shape[0]), _p(a, _f64p)) == 0
+        assert self._L.swe_ref_set_scalars(self._h, int(a.shape[0]), _p(a, _f64p)) == 0
 
     def get_scalars(self):
         out = np.empty((getattr(self, "n_species", 0), self.n_cells))
-        assert lib().swe_ref_get_scalars(self._h, _p(out, _f64p)) == 0
+        assert self._L.swe_ref_get_scalars(self._h, _p(out, _f64p)) == 0
         return out
 
     def set_boundary_scalar(self, string_id, phi):
         a = np.ascontiguousarray(phi, np.float64)
-        assert lib().swe_ref_set_boundary_scalar(self._h, int(string_id), _p(a, _f64p), int(a.size)) == 0
+        assert self._L.swe_ref_set_boundary_scalar(self._h, int(string_id), _p(a, _f64p), int(a.size)) == 0
 
     def set_morphology(self, formula, alpha, theta_cr=0.047, s=2.65, dm=1e-3, porosity=0.4):
         """Eq. 3 / Eq. 13-16: 0 fixed bed, 1 Grass-like, 2 MPM-like (R-20)."""
-        rc = lib().swe_ref_set_morphology(self._h, int(formula), float(alpha), float(theta_cr), float(s), float(dm),
+        rc = self._L.swe_ref_set_morphology(self._h, int(formula), float(alpha), float(theta_cr), float(s), float(dm),
                                           float(porosity))
         if rc != 0:
-            raise ValueError(lib().swe_ref_last_error(self._h).decode())
+            raise ValueError(self._L.swe_ref_last_error(self._h).decode())
 
     def get_bed(self):
         out = np.empty(self.n_cells)
-        assert lib().swe_ref_get_bed(self._h, _p(out, _f64p)) == 0
+        assert self._L.swe_ref_get_bed(self._h, _p(out, _f64p)) == 0
         return out
 
     def sediment_fluxes(self):
         out = np.empty(self.n_edges)
-        assert lib().swe_ref_get_sediment_flux(self._h, _p(out, _f64p)) == 0
+        assert self._L.swe_ref_get_sediment_flux(self._h, _p(out, _f64p)) == 0
         return out
 
     def step(self, n_steps=-1, t_end=float("inf"), cfl=0.9):
         info = Info()
-        rc = lib().swe_ref_step(self._h, int(n_steps), float(t_end), float(cfl), C.byref(info))
+        rc = self._L.swe_ref_step(self._h, int(n_steps), float(t_end), float(cfl), C.byref(info))
         if rc != 0:
             raise RuntimeError(f"swe_ref_step failed ({rc})")
         return info.as_dict()
 
     def get_state(self):
         out = [np.empty(self.n_cells) for _ in range(3)]
-        rc = lib().swe_ref_get_state(self._h, *[_p(x, _f64p) for x in out])
+        rc = self._L.swe_ref_get_state(self._h, *[_p(x, _f64p) for x in out])
         assert rc == 0
         return tuple(out)
 
     def geometry(self):
         area = np.empty(self.n_cells)
         nx, ny, ln = (np.empty(self.n_edges) for _ in range(3))
-        lib().swe_ref_get_geometry(self._h, _p(area, _f64p), _p(nx, _f64p), _p(ny, _f64p), _p(ln, _f64p))
+        self._L.swe_ref_get_geometry(self._h, _p(area, _f64p), _p(nx, _f64p), _p(ny, _f64p), _p(ln, _f64p))
         return area, nx, ny, ln
 
     def edge_fluxes(self):
         out = [np.empty(self.n_edges) for _ in range(4)]
-        lib().swe_ref_get_edge_flux(self._h, *[_p(x, _f64p) for x in out])
+        self._L.swe_ref_get_edge_flux(self._h, *[_p(x, _f64p) for x in out])
         return tuple(out)
 
     def peek_dt(self, cfl=0.9, t_end=float("inf")):
-        return lib().swe_ref_peek_dt(self._h, float(cfl), float(t_end))
+        return self._L.swe_ref_peek_dt(self._h, float(cfl), float(t_end))
 
     def close(self):
         if self._h:
-            lib().swe_ref_destroy(self._h)
+            self._L.swe_ref_destroy(self._h)
             self._h = None
 
     def __del__(self):

@@ -36,7 +36,7 @@ EXPORTS = (
     "swe_params_default", "swe_workspace_bytes", "swe_create", "swe_set_boundary", "swe_set_state", "swe_step",
     "swe_get_state", "swe_destroy", "swe_last_error", "swe_get_geometry", "swe_get_edge_flux", "swe_peek_dt",
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
-    "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_get_patch_stats",
+    "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_survey_bytes", "swe_get_patch_stats",
     "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar", "swe_host_preprocess",
     "swe_set_morphology", "swe_get_bed", "swe_get_sediment_flux",
 )
@@ -108,6 +108,8 @@ def lib():
         L.swe_step_kernel_name.restype = C.c_char_p
         L.swe_algorithmic_bytes.argtypes = [C.c_void_p, C.c_int]
         L.swe_algorithmic_bytes.restype = C.c_int64
+        L.swe_survey_bytes.argtypes = [C.c_void_p, C.c_int]
+        L.swe_survey_bytes.restype = C.c_int64
         L.swe_get_patch_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int]
         L.swe_host_preprocess.argtypes = [C.POINTER(SweMesh), C.c_int, C.c_int, C.POINTER(C.c_int64), C.c_int, _i32p, _i32p]
         L.swe_set_scalars.argtypes = [C.c_void_p, C.c_void_p]
@@ -164,10 +166,9 @@ class Solver:
         if not own_workspace:
             # every device array of the context lives in this torch tensor (workspace_bytes: tests lend too little)
             nbytes = int(L.swe_workspace_bytes(C.byref(mesh), C.byref(prm))) if workspace_bytes is None else int(workspace_bytes)
-            if nbytes == 0:
-                raise SweError(EINVAL, L.swe_last_error(None).decode())
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            prm.workspace, prm.workspace_bytes = self.workspace.data_ptr(), nbytes
+            if nbytes > 0:       # 0: the arguments are invalid -- swe_create below reports why, with its error code
+                self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+                prm.workspace, prm.workspace_bytes = self.workspace.data_ptr(), nbytes
         self.workspace_nbytes = 0 if self.workspace is None else int(self.workspace.numel())
         self.state_on_device = bool(state_on_device)
         h = C.c_void_p()
@@ -323,6 +324,10 @@ class Solver:
     def algorithmic_bytes(self):
         """{kernel name: algorithmic DRAM bytes per launch} (swe_algorithmic_bytes)."""
         return {nm: int(lib().swe_algorithmic_bytes(self._h, k)) for k, nm in enumerate(self.step_kernels())}
+
+    def survey_bytes(self):
+        """{kernel name: bytes per launch on SURVEY.md section 8(d)'s per-cell figures} (swe_survey_bytes)."""
+        return {nm: int(lib().swe_survey_bytes(self._h, k)) for k, nm in enumerate(self.step_kernels())}
 
     def patch_stats(self):
         out = (C.c_int64 * 12)()

@@ -91,35 +91,38 @@ inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
 // ---- the fused patch kernel's instantiations: one thread per own cell (P = threads), __launch_bounds__ minimum
 // blocks per SM chosen from what the shared memory admits (it only caps the registers)
 typedef void (*PatchKernel)(Control *, Patch2Args);
-struct PatchInst { int T, min_blocks; bool scalars; PatchKernel fn; };   // T threads per block >= cells per patch
-#define SWE_PI(P, B) {P, B, false, k_patch2<P, B, false>}
-#define SWE_PIS(P, B) {P, B, true, k_patch2<P, B, true>}
+struct PatchInst { int T, min_blocks; bool scalars; PatchKernel fn; bool pair; };   // T threads per block >= cells per patch
+#define SWE_PI(P, B) {P, B, false, k_patch2<P, B, false>, false}
+#define SWE_PIS(P, B) {P, B, true, k_patch2<P, B, true>, false}
+#define SWE_PIP(P, B) {P, B, false, k_patch2<P, B, false, true>, true}
 const PatchInst kPatchInst[] = {
     SWE_PI(128, 8), SWE_PI(128, 6), SWE_PI(128, 4), SWE_PI(192, 5), SWE_PI(192, 4), SWE_PI(192, 3), SWE_PI(256, 4), SWE_PI(256, 3),
     SWE_PI(256, 2), SWE_PI(384, 2), SWE_PI(384, 1), SWE_PI(512, 2), SWE_PI(512, 1), SWE_PI(1024, 1), SWE_PI(64, 8), SWE_PI(32, 8),
     SWE_PIS(128, 4), SWE_PIS(128, 2), SWE_PIS(192, 3), SWE_PIS(192, 2), SWE_PIS(256, 3), SWE_PIS(256, 2), SWE_PIS(256, 1), SWE_PIS(384, 1), SWE_PIS(512, 1),
-    SWE_PIS(1024, 1), SWE_PIS(64, 4), SWE_PIS(32, 4)};
+    SWE_PIS(1024, 1), SWE_PIS(64, 4), SWE_PIS(32, 4),
+    SWE_PIP(256, 3), SWE_PIP(256, 2), SWE_PIP(192, 4), SWE_PIP(128, 4)};
 #undef SWE_PI
 #undef SWE_PIS
+#undef SWE_PIP
 
 inline int patch_threads(int P) {           // the smallest block size of an instance that gives every own cell a thread
   int T = 1 << 30;
-  for (const PatchInst &pi : kPatchInst) if (pi.T >= P && pi.T < T) T = pi.T;
+  for (const PatchInst &pi : kPatchInst) if (!pi.pair && pi.T >= P && pi.T < T) T = pi.T;
   return T;
 }
 
 // the instantiation with the most blocks per SM that the shared memory of one block admits (force_blocks > 0: that one)
-inline const PatchInst *pick_patch_kernel(int T, bool scalars, size_t smem, int force_blocks) {
+inline const PatchInst *pick_patch_kernel(int T, bool scalars, size_t smem, int force_blocks, bool pair) {
   const int fit = (int)(kSmemPerSM / (smem + kSmemBlockReserve));
   const PatchInst *best = nullptr;
   for (const PatchInst &pi : kPatchInst) {
-    if (pi.T != T || pi.scalars != scalars) continue;
+    if (pi.T != T || pi.scalars != scalars || pi.pair != pair) continue;
     if (force_blocks > 0) { if (pi.min_blocks == force_blocks) return &pi; continue; }
     if (pi.min_blocks <= std::max(1, fit) && (!best || pi.min_blocks > best->min_blocks)) best = &pi;
   }
   if (!best)
     for (const PatchInst &pi : kPatchInst)
-      if (pi.T == T && pi.scalars == scalars && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
+      if (pi.T == T && pi.scalars == scalars && pi.pair == pair && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
   return best;
 }
 
@@ -168,7 +171,7 @@ struct swe_ctx {
   BlobLayout blay{};
   unsigned char *d_blob = nullptr, *d_pflag = nullptr;
   int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
-  int n_patches = 0, patch_threads = 0; size_t patch_smem = 0;
+  int n_patches = 0, patch_threads = 0, patch_prefetch = 0; size_t patch_smem = 0;
   int64_t patch_sum_loc = 0, patch_sum_e = 0; int patch_max_loc = 0, patch_max_e = 0, patch_min_blocks = 0;
   PatchKernel patch_kernel = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
@@ -216,6 +219,7 @@ Patch2Args patch_args(const swe_ctx *c) {
   a.strings = c->d_strings; a.slot_string = c->d_slot_string; a.string_M = c->d_string_M;
   a.pflag_a = c->d_pflag; a.pflag_b = c->d_pflag + (size_t)kPflagBytes * (size_t)c->n_patches;
   a.n_cells = (int32_t)c->nc;
+  a.prefetch_dist = c->patch_prefetch;
   a.sc = c->sc;
   return a;
 }
@@ -581,7 +585,12 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     int force = 0;
     if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) force = std::atoi(s);
     c->patch_threads = patch_threads(pb.lay.P);
-    const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force);
+    bool pair = false;
+    if (const char *s = std::getenv("SWE_PATCH_PAIR")) pair = std::atoi(s) != 0 && c->sc.n == 0;
+    c->patch_prefetch = 3 * 148;
+    if (const char *s = std::getenv("SWE_PATCH_PREFETCH")) c->patch_prefetch = std::atoi(s);
+    const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force, pair);
+    if (!pi && pair) pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force, false);
     if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
     c->patch_kernel = pi->fn; c->patch_min_blocks = pi->min_blocks;
     // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
@@ -1175,6 +1184,8 @@ const char *swe_step_kernel_name(const swe_ctx *c, int k) {
 }
 
 int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes_v[c->variant][k] : 0; }
+
+int64_t swe_survey_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->survey_bytes_v[c->variant][k] : 0; }
 
 int swe_get_patch_stats(swe_ctx *c, int64_t *out, int n_out) {
   if (!c || !out || n_out < 1) return SWE_EINVAL;

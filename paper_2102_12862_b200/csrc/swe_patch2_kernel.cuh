@@ -36,6 +36,8 @@ struct Patch2Args {
   double *string_M;               // l * (limited F1) of every boundary-string edge, by position in string_edges[]
   unsigned char *pflag_a, *pflag_b;   // [n_patches][kPflagBytes], one array per state buffer
   int32_t n_cells;
+  int32_t prefetch_dist;          // > 0: block b pulls the tables of patch b + prefetch_dist into L2 (about the blocks
+                                  // resident at a time, so that it is the patch that takes over this block's slot)
   Scalars sc;                     // passive scalars (kScalars instantiation only)
 };
 
@@ -72,6 +74,9 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes) {   // bytes: a multiple of 16
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   asm volatile(
       "{\n"
@@ -99,29 +104,47 @@ __device__ __forceinline__ void publish_flag(unsigned char *pf_out_base, int b, 
 
 // kThreads >= BlobLayout::P (one thread per own cell; the host picks the smallest instance that covers P).  kScalars: the passive-scalar module (R-19) is on:
 // concentrations of the local cells in shared memory, one more gather per species in phase 4.
-template <int kThreads, int kMinBlocks, bool kScalars = false>
+template <int kThreads, int kMinBlocks, bool kScalars = false, bool kPair = false>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
-  if (!ctl->active) return;
   extern __shared__ __align__(128) unsigned char smraw[];
   const BlobLayout &L = A.L;
   const int tid = threadIdx.x, b = blockIdx.x;
   const int n_sp = kScalars ? A.sc.n : 0;
-  const int src = ctl->src;
-  const CellRec *__restrict__ in = src ? A.rec_b : A.rec_a;
-  CellRec *__restrict__ out = src ? A.rec_a : A.rec_b;
-  unsigned char *pf_out_base = src ? A.pflag_a : A.pflag_b;
   const unsigned char *blob = A.blob + (size_t)b * (size_t)L.stride;
   const int cell0 = b * L.P;                       // L.P <= kThreads: one thread per own cell
   const int n_own = min(L.P, A.n_cells - cell0);
+  const int32_t *__restrict__ halo_ids = (const int32_t *)(blob + L.off_halo_ids);
+
+  // ---- everything whose address depends on blockIdx alone is requested at once (one memory latency for all of it):
+  // the control block, this patch's flag word in BOTH state buffers (which one is read depends on Control::src), the
+  // first halo ids of every thread, and the flag words of the patch whose tables this block pulls into L2 (below)
+  const ulonglong2 *pfa = reinterpret_cast<const ulonglong2 *>(A.pflag_a + (size_t)b * kPflagBytes);
+  const ulonglong2 *pfb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b * kPflagBytes);
+  const int active = ctl->active, src = ctl->src;
+  const ulonglong2 fa0 = pfa[0], fa1 = pfa[1], fb0 = pfb[0], fb1 = pfb[1];
+  const int hid0 = tid < L.cap_halo ? halo_ids[tid] : -1;
+  const int hid1 = tid + kThreads < L.cap_halo ? halo_ids[tid + kThreads] : -1;
+  const int b_pf = b + A.prefetch_dist;            // the block that will run in this block's slot next (about)
+  const bool do_pf = A.prefetch_dist > 0 && b_pf < (int)gridDim.x && tid == 0;
+  ulonglong2 ga0, ga1, gb0, gb1;
+  if (do_pf) {
+    const ulonglong2 *qa = reinterpret_cast<const ulonglong2 *>(A.pflag_a + (size_t)b_pf * kPflagBytes);
+    const ulonglong2 *qb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b_pf * kPflagBytes);
+    ga0 = qa[0]; ga1 = qa[1]; gb0 = qb[0]; gb1 = qb[1];
+  }
+  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+  if (!active) return;
+  const CellRec *__restrict__ in = src ? A.rec_b : A.rec_a;
+  CellRec *__restrict__ out = src ? A.rec_a : A.rec_b;
+  unsigned char *pf_out_base = src ? A.pflag_a : A.pflag_b;
+  const unsigned long long ones = 0x0101010101010101ull;
 
   // ---- skip test (section 5b): when the own cells of this patch and of every patch that owns one of its halo cells
   // are exactly (0, 0, 0) in the state being read, and no boundary string can feed the patch, every flux of S1 is
   // exactly 0, theta = 1 and S3 returns (+0, 0, 0) for every own cell: write that (unless the target holds it already).
   {
-    const ulonglong2 *pf = reinterpret_cast<const ulonglong2 *>((src ? A.pflag_b : A.pflag_a) + (size_t)b * kPflagBytes);
-    const ulonglong2 w0 = pf[0], w1 = pf[1];
-    const unsigned long long ones = 0x0101010101010101ull;
+    const ulonglong2 w0 = src ? fb0 : fa0, w1 = src ? fb1 : fa1;
     if (w0.x == ones && w0.y == ones && w1.x == ones && w1.y == ones) {
       const unsigned char had = pf_out_base[(size_t)b * kPflagBytes + kPflagOwn];
       if (!had) {
@@ -154,17 +177,25 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     mbar_expect_tx(bar, (uint32_t)L.stage_bytes + 32u * (uint32_t)n_own);
     bulk_g2s(stage, blob + L.off_stage, (uint32_t)L.stage_bytes, bar);
     bulk_g2s(crec, in + cell0, 32u * (uint32_t)n_own, bar);
+    // the tables and own records of the patch that will run in this slot next go to L2 now (unless that patch will
+    // be skipped): its block then pays L2 latency, not DRAM latency, in the chain flag word -> bulk copy -> phase 1
+    if (do_pf) {
+      const ulonglong2 v0 = src ? gb0 : ga0, v1 = src ? gb1 : ga1;
+      if (!(v0.x == ones && v0.y == ones && v1.x == ones && v1.y == ones)) {
+        const int c0n = b_pf * L.P, n_next = min(L.P, A.n_cells - c0n);
+        bulk_prefetch_l2(A.blob + (size_t)b_pf * (size_t)L.stride, (uint32_t)(L.off_stage + L.stage_bytes));
+        bulk_prefetch_l2(in + c0n, 32u * (uint32_t)n_next);
+      }
+    }
   }
-  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
 
   // ---- phase 1a: halo cells (a gather: id -> record), while the bulk copies are in flight; velocities once per cell
   // (R-8: thin films carry no momentum)
-  const int32_t *__restrict__ halo_ids = (const int32_t *)(blob + L.off_halo_ids);
   int water = 0;
   for (int j0 = tid; j0 < L.cap_halo; j0 += 2 * kThreads) {
     const int j1 = j0 + kThreads;
-    const int id0 = halo_ids[j0];
-    const int id1 = j1 < L.cap_halo ? halo_ids[j1] : -1;
+    const int id0 = j0 == tid ? hid0 : halo_ids[j0];
+    const int id1 = j0 == tid ? hid1 : (j1 < L.cap_halo ? halo_ids[j1] : -1);
     CellRec c0, c1;
     if (id0 >= 0) c0 = in[id0];
     if (id1 >= 0) c1 = in[id1];
@@ -236,33 +267,68 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     return;
   }
 
-  // ---- phase 2: edge fluxes
-  for (int e = tid; e < n_e; e += kThreads) {
+  // ---- phase 2: edge fluxes.  kPair: two edges per thread and iteration, so that their instruction streams interleave
+  // (the flux of one edge is a long chain of dependent fp64 operations: sqrt -> wave speeds -> division -> fluxes)
+  struct EdgeIn { double nx, ny, len, hL, uL, vL, zL, hR, uR, vR, zR; int Lc, Rc; };
+  auto load_edge = [&](int e) {
+    EdgeIn q;
     const uint32_t lr = b_lr[e];
-    const int Lc = (int)(lr & 0xFFFFu), Rc = (int)(lr >> 16);
-    const double nx = b_nx[e], ny = b_ny[e], len = b_len[e];
-    const double hL = sh_h[Lc], uL = sh_u[Lc], vL = sh_v[Lc], zL = sh_z[Lc];
+    q.Lc = (int)(lr & 0xFFFFu); q.Rc = (int)(lr >> 16);
+    q.nx = b_nx[e]; q.ny = b_ny[e]; q.len = b_len[e];
+    q.hL = sh_h[q.Lc]; q.uL = sh_u[q.Lc]; q.vL = sh_v[q.Lc]; q.zL = sh_z[q.Lc];
+    const int Rs = q.Rc != 0xFFFF ? q.Rc : q.Lc;
+    q.hR = sh_h[Rs]; q.uR = sh_u[Rs]; q.vR = sh_v[Rs]; q.zR = sh_z[Rs];
+    return q;
+  };
+  auto flux_edge = [&](const EdgeIn &q, int e) {
     EdgeFlux o;
-    if (Rc != 0xFFFF) {
-      const double hR = sh_h[Rc], uR = sh_u[Rc], vR = sh_v[Rc], zR = sh_z[Rc];
-      const double unL = uL * nx + vL * ny, utL = vL * nx - uL * ny;
-      const double unR = uR * nx + vR * ny, utR = vR * nx - uR * ny;
-      o = riemann_nt(g, hL, unL, utL, zL, hR, unR, utR, zR);
+    if (q.Rc != 0xFFFF) {
+      const double unL = q.uL * q.nx + q.vL * q.ny, utL = q.vL * q.nx - q.uL * q.ny;
+      const double unR = q.uR * q.nx + q.vR * q.ny, utR = q.vR * q.nx - q.uR * q.ny;
+      o = riemann_nt(g, q.hL, unL, utL, q.zL, q.hR, unR, utR, q.zR);
     } else {
       const BoundaryString *bs = nullptr;
       int code = b_aux[e];
       if (code <= -3) { bs = A.strings + A.slot_string[-3 - code]; code = -3; }
-      const int gidL = Lc < n_own ? cell0 + Lc : halo_ids[Lc - n_own];
-      o = boundary_flux(g, code, bs, A.kst, gidL, nx, ny, len, hL, zL, uL, vL);
+      const int gidL = q.Lc < n_own ? cell0 + q.Lc : halo_ids[q.Lc - n_own];
+      o = boundary_flux(g, code, bs, A.kst, gidL, q.nx, q.ny, q.len, q.hL, q.zL, q.uL, q.vL);
     }
+    return o;
+  };
+  auto store_edge = [&](const EdgeIn &q, int e, const EdgeFlux &o) {
     sh_F1[e] = o.F1;
     if (e < H.n_eown) { sh_F3[e] = o.F3; sh_GL[e] = o.GL; sh_GR[e] = o.GR; }
     // S1c, lazily (R-8b; as in k_edge_flux): theta_i < 1 needs one outgoing edge with dt * o_k > 0.3 h_i |Omega_i|.  Only
     // such donor cells are marked (theta = -1); phase 3 evaluates theta for them and every other cell keeps theta = 1.
-    const int d = o.F1 > 0.0 ? Lc : ((o.F1 < 0.0 && Rc != 0xFFFF) ? Rc : n_c1);
+    const int d = o.F1 > 0.0 ? q.Lc : ((o.F1 < 0.0 && q.Rc != 0xFFFF) ? q.Rc : n_c1);
     if (d < n_c1) {
       const double ad = d < n_own ? b_area[d] : b_halo_area[d - n_own];
-      if (dt * (len * fabs(o.F1)) > 0.3 * (sh_h[d] * ad)) sh_th[d] = -1.0;
+      const double hd = d == q.Lc ? q.hL : q.hR;
+      if (dt * (q.len * fabs(o.F1)) > 0.3 * (hd * ad)) sh_th[d] = -1.0;
+    }
+  };
+  if (!kPair) {
+    for (int e = tid; e < n_e; e += kThreads) {
+      const EdgeIn q = load_edge(e);
+      const EdgeFlux o = flux_edge(q, e);
+      store_edge(q, e, o);
+    }
+  } else {
+    // (trip count and the choice pair / single are warp-uniform: eb is the first edge of the warp's chunk)
+    for (int eb = tid - (tid & 31); eb < n_e; eb += 2 * kThreads) {
+      const int e0 = eb + (tid & 31), e1 = e0 + kThreads;
+      const bool has0 = e0 < n_e, has1 = e1 < n_e;
+      if (eb + kThreads < n_e) {                       // the warp's second chunk has at least one edge
+        const int e0s = has0 ? e0 : eb, e1s = has1 ? e1 : e0s;
+        const EdgeIn q0 = load_edge(e0s), q1 = load_edge(e1s);
+        const EdgeFlux o0 = flux_edge(q0, e0s), o1 = flux_edge(q1, e1s);
+        if (has0) store_edge(q0, e0, o0);
+        if (has1) store_edge(q1, e1, o1);
+      } else if (has0) {
+        const EdgeIn q = load_edge(e0);
+        const EdgeFlux o = flux_edge(q, e0);
+        store_edge(q, e0, o);
+      }
     }
   }
   __syncthreads();

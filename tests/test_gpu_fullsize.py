@@ -1,9 +1,10 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default renumbering,
 default CUDA-graph step loop, one swe_step call per window): configs[3] (river reach, ~4M cells, wetting/drying,
 hydrograph inflow, normal-depth outflow) and configs[2] (circular dam break, ~1M cells).  The oracle steps the
-whole mesh too (about 1 s per step at 4M cells), so the windows are short: one from the initial state and one
-re-started from the GPU's own state deep into the run (get_state -> oracle set_state), where the flood wave has
-wetted part of the floodplain.  All cells are compared; mass balance and wet counts are checked as well."""
+whole mesh too (about 0.6 s per step at 4M cells); the configs[3] windows follow SURVEY section 8(d): 100 steps from
+the initial state and from the GPU's own states at steps 1000 and 4000 (get_state -> oracle set_state), where the
+flood wave has wetted part of the floodplain; configs[4] is checked at 8M and at 16M cells.  All cells are compared;
+mass balance and wet counts are checked as well."""
 import numpy as np
 import pytest
 
@@ -42,28 +43,62 @@ def window(s, o, w, n, what):
 
 
 def test_config4_full_size_windows(gpu, ref):
+    """SURVEY section 8(d) parity windows on configs[3] at full size, all cells: 100 steps from the initial state, and
+    100-step windows started from the GPU's own states at steps 1000 and 4000 (get_state -> oracle set_state), where
+    the flood wave has wetted part of the floodplain."""
     w = C.config4()
     assert 3.8e6 < w.n_cells < 4.2e6
     s = make(gpu, w)
     o = ref.RefSolver(w)
     area = s.geometry()[0]
     vol0 = float(np.sum(w.h * area))
-    ig, io, _ = window(s, o, w, 20, "config4 full size, steps 0-20")
+    ig, io, _ = window(s, o, w, 100, "config4 full size, steps 0-100")
     check_info(ig, io)
-    # deep into the run: 1500 more steps on the GPU only, then both sides continue from the GPU's state
-    ig = s.step(1500, float("inf"), w.cfl)
-    assert ig["flags"] == 0
-    # mass balance over the whole run so far (property that holds at any size)
-    bal = ig["vol"] - vol0 - ig["vol_in"] + ig["vol_out"] - ig["vol_clipped"]
-    assert abs(bal) <= 1e-11 * vol0, bal
-    assert ig["vol_in"] > 0.0 and ig["vol_out"] > 0.0
-    st = s.get_state()
-    assert ig["n_wet"] == int(np.sum(st[0] > w.h_dry)) and ig["n_wet"] != int(np.sum(w.h > w.h_dry))
-    o.set_state(*st, t0=ig["t"])
-    s.set_state(*st, t0=ig["t"])
-    window(s, o, w, 20, "config4 full size, 20 steps from the GPU state at step 1520")
+    wet0 = int(np.sum(w.h > w.h_dry))
+    for start in (1000, 4000):
+        # GPU only up to `start` steps, then both sides continue from the GPU's state
+        ig = s.step(start - ig["steps_done"], float("inf"), w.cfl)
+        assert ig["flags"] == 0 and ig["steps_done"] == start
+        # mass balance over the whole run so far (property that holds at any size)
+        bal = ig["vol"] - vol0 - ig["vol_in"] + ig["vol_out"] - ig["vol_clipped"]
+        assert abs(bal) <= 1e-11 * vol0, bal
+        assert ig["vol_in"] > 0.0 and ig["vol_out"] > 0.0
+        st = s.get_state()
+        assert ig["n_wet"] == int(np.sum(st[0] > w.h_dry)) and ig["n_wet"] != wet0
+        o.set_state(*st, t0=ig["t"])
+        # (the GPU keeps stepping from its own state: no swe_set_state, so steps_done and the volume counters run on)
+        io = o.step(100, float("inf"), w.cfl)
+        ig = s.step(100, float("inf"), w.cfl)
+        sg, so = s.get_state(), o.get_state()
+        what = f"config4 full size, 100 steps from the GPU state at step {start}"
+        assert np.array_equal(sg[0] > w.h_dry, so[0] > w.h_dry), f"{what}: wet/dry masks differ"
+        assert_state_close(sg, so, what)
+        assert ig["n_wet"] == io["n_wet"] and ig["steps_done"] == start + 100
+        assert abs(ig["dt_last"] - io["dt_last"]) <= DT_RTOL * io["dt_last"]
+        assert abs(ig["t"] - io["t"]) <= DT_RTOL * abs(io["t"])
+        assert abs(ig["vol"] - io["vol"]) <= 1e-12 * io["vol"]
     s.close()
     o.close()
+
+
+def test_config5_16m_window(gpu, ref):
+    """BASELINE.json configs[4], second size (16M triangles): every cell against the oracle over the first 6 steps, in
+    the launch configuration bench.py times, then the fused patch step against the three-pass step over 40 more."""
+    w = C.by_id(5, 2.0)
+    assert 15.5e6 < w.n_cells < 16.5e6
+    s = make(gpu, w)
+    o = ref.RefSolver(w)
+    ig, io, _ = window(s, o, w, 6, "config5 16M, steps 0-6")
+    check_info(ig, io)
+    o.close()
+    t = gpu.from_workload(w, variant=gpu.VARIANT_PATCH)
+    t.step(6, float("inf"), w.cfl, info=False)
+    i1, i2 = s.step(40, float("inf"), w.cfl), t.step(40, float("inf"), w.cfl)
+    assert i1 == i2 and i1["flags"] == 0 and i1["n_wet"] == w.n_cells
+    for x, y in zip(s.get_state(), t.get_state()):
+        assert np.array_equal(x, y)
+    s.close()
+    t.close()
 
 
 def test_config3_full_size_window(gpu, ref):
