@@ -86,6 +86,8 @@ def parse():
     ap.add_argument("--species", type=int, default=0, help="passive scalar species advected with the flow (0..5)")
     ap.add_argument("--morph", type=int, default=0, choices=[0, 1, 2],
                     help="mobile bed (swe_set_morphology): 1 Grass-like alpha = 0.001, 2 MPM-like alpha = 8, d_m = 5 mm")
+    ap.add_argument("--precision", default="double", choices=["double", "single"],
+                    help="arithmetic of the step (include/swe.h SWE_PRECISION_*; single: fp32 three-pass step, DESIGN.md R-21)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-omp", action="store_true", help="also time the oracle source built with OpenMP on all host cores")
     ap.add_argument("--parity-steps", type=int, default=5,
@@ -239,11 +241,11 @@ def unpin(prev):
             pass
 
 
-def oracle_time(w, n_warm, max_steps, min_seconds, cfl, morph=0, omp=False):
+def oracle_time(w, n_warm, max_steps, min_seconds, cfl, morph=0, omp=False, precision="double"):
     """The oracle as it stands on this box's host cores: (cell-updates/s, time steps timed, s).  omp=False: single
     thread (the caller pins the process to one core); omp=True: the same source built with OpenMP, all cores."""
     from oracle import swe_ref
-    o = swe_ref.RefSolver(w, omp=omp)
+    o = swe_ref.RefSolver(w, omp=omp, precision=precision)
     if morph:
         o.set_morphology(*MORPH_PARAMS[morph])
     if n_warm:
@@ -266,7 +268,7 @@ def run_reference(args, rank):
     from oracle import swe_ref
     w = load_workload(args.config, args.scale)
     core, prev_aff = pin_to_one_core()
-    o = swe_ref.RefSolver(w)
+    o = swe_ref.RefSolver(w, precision=args.precision)
     if args.morph:
         o.set_morphology(*MORPH_PARAMS[args.morph])
     for _ in range(args.warmup):
@@ -283,9 +285,9 @@ def run_reference(args, rank):
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == "double" else "f32", "data": "synthetic",
         "config": {"workload": w.name, "baseline_config": args.config, "n_cells": w.n_cells, "n_edges": w.n_edges,
-                   "time_steps_per_step": 1, "cfl": w.cfl, "morph": args.morph},
+                   "time_steps_per_step": 1, "cfl": w.cfl, "morph": args.morph, "precision": args.precision},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -293,13 +295,13 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
-def parity_window(s, w, info, n_steps):
+def parity_window(s, w, info, n_steps, precision="double"):
     """State after the timed region -> oracle (get_state -> set_state at the same t), then n_steps on both sides;
     every cell compared at the north_star tolerances (|d| <= 1e-10 |ref| + 1e-14 max|ref|; dt <= 1e-12 relative;
     identical wet/dry masks).  The oracle runs here as the checker of the timed state, outside every timed region."""
     from oracle import swe_ref
     st = s.get_state()
-    o = swe_ref.RefSolver(w)
+    o = swe_ref.RefSolver(w, precision=precision)
     o.set_state(*st, t0=info["t"])
     s.set_state(*st, t0=info["t"])
     ig, io = s.step(n_steps, float("inf"), w.cfl), o.step(n_steps, float("inf"), w.cfl)
@@ -350,7 +352,8 @@ def main():
     N, E, T = w.n_cells, w.n_edges, args.time_steps
     t_create = time.perf_counter()
     s = P.from_workload(w, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells,
-                        renumber=args.renumber, n_species=args.species, morphology=bool(args.morph))
+                        renumber=args.renumber, n_species=args.species, morphology=bool(args.morph),
+                        precision=P.PRECISION_SINGLE if args.precision == "single" else P.PRECISION_DOUBLE)
     if args.species:
         from workloads import mesh as WM
         ctr = WM.centroids(w.node_xy, w.tri)
@@ -396,7 +399,7 @@ def main():
     # ... and parity: the oracle continues from the GPU's state for a short window (rank 0, N = 1), all cells compared
     parity = None
     if rank == 0 and world == 1 and args.parity_steps > 0 and not args.species and not args.morph:
-        parity = parity_window(s, w, info, args.parity_steps)
+        parity = parity_window(s, w, info, args.parity_steps, args.precision)
         info = s.step(0, float("inf"), w.cfl, info=True)
     ms = max_over_ranks(ms, world, dev)
     value = aggregate_value(N, T, args.steps, world, ms * 1e-3)
@@ -474,7 +477,7 @@ def main():
     # moves a third of the bytes; the three-pass step (edge flux -> theta -> CSR gather/update, the design the
     # north_star names) is the bandwidth-bound one, so its per-kernel HBM fractions are reported beside the default's
     other = None
-    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0 and not args.morph:
+    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0 and not args.morph and args.precision == "double":
         ov = P.VARIANT_THREE_PASS if s_kernels[-1] == "k_patch_step" else P.VARIANT_PATCH
         s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber)
         for _ in range(2):
@@ -500,7 +503,7 @@ def main():
     # ---- second line (rank 0, N = 1): an ALL-WET mesh of the same size, where no patch can be skipped -- the
     # BASELINE.json configs[4] construction (circular dam break, every cell wet, friction everywhere) at 4M cells
     all_wet = None
-    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0 and not args.morph:
+    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0 and not args.morph and args.precision == "double":
         from workloads import configs as C
         w2 = C.config5(target_cells=N)
         s2 = P.from_workload(w2, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
@@ -528,7 +531,7 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         core, prev_aff = pin_to_one_core()
-        v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl, args.morph)
+        v, n_done, secs = oracle_time(w, 1, 40, 12.0, w.cfl, args.morph, precision=args.precision)
         unpin(prev_aff)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"all {N} cells x {n_done} time steps from the initial state ({secs:.1f} s, 1 thread pinned to core {core})"}
@@ -542,8 +545,8 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "ms_per_step_median": ms_median,
             "ms_per_step_chunks": chunk_ms, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "baseline_config": args.config, "n_cells": N, "n_edges": E,
+            "vs_baseline": None, "dtype": "f64" if args.precision == "double" else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "precision": args.precision, "baseline_config": args.config, "n_cells": N, "n_edges": E,
                        "time_steps_per_step": T, "cfl": w.cfl, "parallelism": f"replicas x{world}",
                        "l2": "working set (%.0f MB) larger than L2, no flush" % (s_workspace_bytes / 1e6),
                        "create_s": round(t_create, 2), "renumber": args.renumber, "shuffled_input": args.shuffle_input, "n_species": args.species, "morph": args.morph, "stage": args.stage, "step_kernels": s_kernels, "patch": patch_stats},

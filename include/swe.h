@@ -48,6 +48,11 @@ enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1, SWE_RENUMBER_RCM = 2 /* r
  * step on all-wet states); on a numbering that is not spatially compact it is the three-pass step. */
 enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta -> CSR gather + update */,
        SWE_VARIANT_PATCH = 2 /* one fused kernel per step over shared-memory mesh patches */ };
+/* Arithmetic ("single or double"; R-21).  SINGLE: state, geometry and every flux / update operation in
+ * fp32 (16-byte records); time, dt = CFL / rate, the hydrograph lookup and the volume bookkeeping stay fp64; built for the
+ * three-pass hydrodynamic step only (SWE_EINVAL with scalars, mobile bed or SWE_VARIANT_PATCH; AUTO = three-pass).  The
+ * arrays at this boundary stay fp64 in both cases (rounded once on the way in, exact on the way out). */
+enum { SWE_PRECISION_DOUBLE = 0, SWE_PRECISION_SINGLE = 1 };
 /* swe_step_info.flags */
 enum { SWE_FLAG_NONFINITE = 1, SWE_FLAG_DT_UNBOUNDED = 2 /* whole domain dry and dt_max = +inf */,
        SWE_FLAG_STALLED = 4 /* Eq. 21 gave dt <= 0 or t + dt == t (a rate of +inf from a non-finite state, or dt below
@@ -82,6 +87,7 @@ typedef struct {
                            0 = default (256; less on meshes that would not fill the SMs)             */
   int n_species;        /* passive scalar species advected with the flow (0..5); default 0    */
   int morphology;       /* 1: reserve room for the mobile-bed module (swe_set_morphology); default 0 */
+  int precision;        /* SWE_PRECISION_*; default DOUBLE                                           */
   void *cuda_stream;    /* cudaStream_t all work is enqueued on; NULL = the legacy default stream    */
   void *workspace;      /* DEVICE memory lent by the caller for the context's lifetime (e.g. a torch
                            uint8 tensor), 256-byte aligned: EVERY device array of the context is carved
@@ -148,9 +154,12 @@ int swe_set_boundary_scalar(swe_ctx *ctx, int string_id, const double *phi, int 
  *   formula 2  MPM-like     |q_B| = alpha (theta - theta_cr)^1.5 sqrt((s-1) g d_m^3), theta = |u|^2 / (k_st^2 h^(1/3) (s-1) d_m)
  * theta_cr, s, d_m are read by formula 2 only; porosity p in [0, 1).  No transport through walls or where a side of an
  * interface is dry (h <= h_dry); through every open boundary the interior cell's own flux passes (equilibrium).
- * The step becomes the three-pass one (its edge kernel also writes q_Bij, 8 B per edge; its cell kernel gathers it and
- * writes z_B with the record it writes anyway): SWE_EINVAL on a context created with SWE_VARIANT_PATCH or with
- * n_species > 0.  Synchronises the stream and captures the CUDA graph of the step again (once per call). */
+ * Both step variants carry the module (three-pass: the edge kernel also writes q_Bij, 8 B per edge, the cell kernel gathers it
+ * and writes z_B with the record it writes anyway; fused patch step: q_Bij of the patch's own edges in shared memory), with
+ * or without scalar species, bit-identical to each other; AUTO keeps choosing between them.  The context must have been
+ * created with swe_params.morphology = 1 (room for q_Bij and the per-cell record of the MPM-like law), else SWE_EINVAL; not
+ * built for single precision.  The bed persists across swe_set_state (there is no call that resets it; create a new
+ * context for the initial bed).  Synchronises the stream and captures the CUDA graphs of the step again (once per call). */
 int swe_set_morphology(swe_ctx *ctx, int formula, double alpha, double theta_cr, double s, double d_m, double porosity);
 /* bed elevation z_B [n_cells] in the caller's cell numbering (host or device pointer as for swe_get_state) */
 int swe_get_bed(swe_ctx *ctx, double *zb);

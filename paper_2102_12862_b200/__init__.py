@@ -28,6 +28,7 @@ BC_NONE, BC_INFLOW_Q, BC_OUTFLOW_UNIFORM = 0, 1, 2
 RENUMBER_NONE, RENUMBER_MORTON, RENUMBER_RCM = 0, 1, 2
 FLAG_NONFINITE, FLAG_DT_UNBOUNDED, FLAG_STALLED = 1, 2, 4
 VARIANT_AUTO, VARIANT_THREE_PASS, VARIANT_PATCH = 0, 1, 2
+PRECISION_DOUBLE, PRECISION_SINGLE = 0, 1
 
 _f64p = C.POINTER(C.c_double)
 _i32p = C.POINTER(C.c_int32)
@@ -51,7 +52,7 @@ class SweMesh(C.Structure):
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("h_dry", C.c_double), ("dt_max", C.c_double), ("renumber", C.c_int),
                 ("state_on_device", C.c_int), ("steps_per_graph", C.c_int), ("variant", C.c_int), ("patch_cells", C.c_int),
-                ("n_species", C.c_int), ("morphology", C.c_int), ("cuda_stream", C.c_void_p),
+                ("n_species", C.c_int), ("morphology", C.c_int), ("precision", C.c_int), ("cuda_stream", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
@@ -133,7 +134,7 @@ class Solver:
     def __init__(self, node_xy, tri, edge_cell=None, cell_edge=None, zb=None, kst=None, *, g=9.81, h_dry=1e-3,
                  dt_max=float("inf"), renumber=RENUMBER_MORTON, state_on_device=False, steps_per_graph=32,
                  device="cuda:0", own_workspace=False, variant=VARIANT_AUTO, patch_cells=0, n_species=0,
-                 morphology=False, workspace_bytes=None):
+                 morphology=False, workspace_bytes=None, precision=PRECISION_DOUBLE):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -159,6 +160,7 @@ class Solver:
         prm.renumber, prm.state_on_device, prm.steps_per_graph = int(renumber), int(bool(state_on_device)), int(steps_per_graph)
         prm.variant, prm.patch_cells, prm.n_species = int(variant), int(patch_cells), int(n_species)
         prm.morphology = int(bool(morphology))
+        prm.precision = int(precision)
         self.n_species = int(n_species)
         self.stream = torch.cuda.current_stream(self.device)
         prm.cuda_stream = self.stream.cuda_stream

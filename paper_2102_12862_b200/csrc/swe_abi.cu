@@ -39,14 +39,15 @@ struct Sizes {
   int64_t nc = 0, ne = 0;
   int n_species = 0;
   bool morph = false;                     // room for the mobile-bed module (swe_params.morphology)
+  bool single = false;                    // swe_params.precision = SWE_PRECISION_SINGLE: 4-byte reals, 16-byte records
   int64_t n_strings = 0, n_string_edges = 0, scratch = 0;
   int64_t n_patches = 0, blob_bytes = 0;  // fused patch step (0: the context has no patch step)
 };
 
 // Offsets of the device arrays inside the workspace, in carving order.
 struct Layout {
-  size_t rec, rec_b, geom, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, drain_flag;
-  size_t ctl, info_part, info_ticket, strings, string_edges, scratch, params, slot_string, string_M;
+  size_t rec, rec_b, geom, geomR, flux, cell_edge, area, inv_area, gn2, kst, theta, cell_perm, edge_perm, stage, drain_flag;
+  size_t ctl, info_part, info_ticket, strings, string_edges, scratch, params, slot_string, string_M, string_lk, string_cell;
   size_t qa[kMaxSpecies], qb[kMaxSpecies], phi_up[kMaxSpecies], scalar_stage;
   size_t blob, pflag;
   size_t qB, mcell;
@@ -55,12 +56,14 @@ struct Layout {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += align_up(std::max<size_t>(bytes, 16)); return at; };
     const size_t nc = (size_t)z.nc, ne = (size_t)z.ne, nse = (size_t)std::max<int64_t>(1, z.n_string_edges);
-    rec = take(sizeof(CellRec) * nc);
-    rec_b = take(sizeof(CellRec) * nc);     // second state buffer of the fused patch step
-    geom = take(sizeof(EdgeGeom) * ne);
-    flux = take(sizeof(EdgeFlux) * ne);
+    const size_t r = z.single ? 4 : 8;      // bytes of a real; records are 4 reals
+    rec = take(4 * r * nc);
+    rec_b = z.single ? 0 : take(4 * r * nc);   // second state buffer of the fused patch step (fp64 only)
+    geom = take(4 * r * ne);
+    geomR = z.single ? take(4 * ne) : 0;    // fp32: R of every edge beside the 16-byte geometry record
+    flux = take(4 * r * ne);
     cell_edge = take(sizeof(int4) * nc);
-    area = take(8 * nc); inv_area = take(8 * nc); gn2 = take(8 * nc); kst = take(8 * nc); theta = take(8 * nc);
+    area = take(r * nc); inv_area = take(r * nc); gn2 = take(r * nc); kst = take(r * nc); theta = take(r * nc);
     cell_perm = take(4 * nc); edge_perm = take(4 * ne);
     stage = take(std::max(24 * nc, 16 * ne));           // host <-> device staging of set / get calls
     drain_flag = take(nc + 16);                         // read four bytes at a time
@@ -72,7 +75,8 @@ struct Layout {
     scratch = take(8 * (size_t)std::max<int64_t>(1, z.scratch));
     params = take(8 * (size_t)kParamsPool);
     slot_string = take(4 * nse);
-    string_M = take(8 * nse);
+    string_M = take(2 * 8 * nse);                       // two buffers: the self-controlled patch step alternates
+    string_lk = take(8 * nse); string_cell = take(4 * nse);
     for (int sp = 0; sp < kMaxSpecies; ++sp) {
       qa[sp] = qb[sp] = phi_up[sp] = 0;
       if (sp < z.n_species) { qa[sp] = take(8 * nc); qb[sp] = take(8 * nc); phi_up[sp] = take(8 * ne); }
@@ -91,38 +95,34 @@ inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
 // ---- the fused patch kernel's instantiations: one thread per own cell (P = threads), __launch_bounds__ minimum
 // blocks per SM chosen from what the shared memory admits (it only caps the registers)
 typedef void (*PatchKernel)(Control *, Patch2Args);
-struct PatchInst { int T, min_blocks; bool scalars; PatchKernel fn; bool pair; };   // T threads per block >= cells per patch
-#define SWE_PI(P, B) {P, B, false, k_patch2<P, B, false>, false}
-#define SWE_PIS(P, B) {P, B, true, k_patch2<P, B, true>, false}
-#define SWE_PIP(P, B) {P, B, false, k_patch2<P, B, false, true>, true}
-const PatchInst kPatchInst[] = {
-    SWE_PI(128, 8), SWE_PI(128, 6), SWE_PI(128, 4), SWE_PI(192, 5), SWE_PI(192, 4), SWE_PI(192, 3), SWE_PI(256, 4), SWE_PI(256, 3),
-    SWE_PI(256, 2), SWE_PI(384, 2), SWE_PI(384, 1), SWE_PI(512, 2), SWE_PI(512, 1), SWE_PI(1024, 1), SWE_PI(64, 8), SWE_PI(32, 8),
-    SWE_PIS(128, 4), SWE_PIS(128, 2), SWE_PIS(192, 3), SWE_PIS(192, 2), SWE_PIS(256, 3), SWE_PIS(256, 2), SWE_PIS(256, 1), SWE_PIS(384, 1), SWE_PIS(512, 1),
-    SWE_PIS(1024, 1), SWE_PIS(64, 4), SWE_PIS(32, 4),
-    SWE_PIP(256, 3), SWE_PIP(256, 2), SWE_PIP(192, 4), SWE_PIP(128, 4)};
+struct PatchInst { int T, min_blocks; PatchKernel fn[2][2][2]; };   // T threads per block >= cells per patch; [scalars][self][morph]
+// self = 0: dt / stop rules from k_step_control; 1: every block derives them itself (no control kernel between steps)
+#define SWE_PK(P, B, S) {{k_patch2<P, B, S, false, false>, k_patch2<P, B, S, false, true>}, {k_patch2<P, B, S, true, false>, k_patch2<P, B, S, true, true>}}
+#define SWE_PI(P, B) {P, B, {SWE_PK(P, B, false), SWE_PK(P, B, true)}}
+const PatchInst kPatchInst[] = {SWE_PI(32, 8), SWE_PI(64, 8), SWE_PI(128, 6), SWE_PI(128, 4), SWE_PI(192, 4), SWE_PI(192, 3),
+                                SWE_PI(256, 4), SWE_PI(256, 3), SWE_PI(256, 2), SWE_PI(384, 2), SWE_PI(384, 1), SWE_PI(512, 1),
+                                SWE_PI(1024, 1)};
 #undef SWE_PI
-#undef SWE_PIS
-#undef SWE_PIP
+#undef SWE_PK
 
 inline int patch_threads(int P) {           // the smallest block size of an instance that gives every own cell a thread
   int T = 1 << 30;
-  for (const PatchInst &pi : kPatchInst) if (!pi.pair && pi.T >= P && pi.T < T) T = pi.T;
+  for (const PatchInst &pi : kPatchInst) if (pi.T >= P && pi.T < T) T = pi.T;
   return T;
 }
 
 // the instantiation with the most blocks per SM that the shared memory of one block admits (force_blocks > 0: that one)
-inline const PatchInst *pick_patch_kernel(int T, bool scalars, size_t smem, int force_blocks, bool pair) {
+inline const PatchInst *pick_patch_kernel(int T, size_t smem, int force_blocks) {
   const int fit = (int)(kSmemPerSM / (smem + kSmemBlockReserve));
   const PatchInst *best = nullptr;
   for (const PatchInst &pi : kPatchInst) {
-    if (pi.T != T || pi.scalars != scalars || pi.pair != pair) continue;
+    if (pi.T != T) continue;
     if (force_blocks > 0) { if (pi.min_blocks == force_blocks) return &pi; continue; }
     if (pi.min_blocks <= std::max(1, fit) && (!best || pi.min_blocks > best->min_blocks)) best = &pi;
   }
   if (!best)
     for (const PatchInst &pi : kPatchInst)
-      if (pi.T == T && pi.scalars == scalars && pi.pair == pair && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
+      if (pi.T == T && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
   return best;
 }
 
@@ -133,6 +133,8 @@ struct Plan {
   std::vector<BoundaryString> strings;
   std::vector<int32_t> flat;             // string_edges[]: members of all strings, internal edge ids
   std::vector<int32_t> slot_string;      // string id of every position of flat[]
+  std::vector<double> string_lk;         // l_e * k_weight(k_st of cell L) of every position of flat[] (R-11)
+  std::vector<int32_t> string_cell;      // cell L of every position of flat[]
   std::vector<EdgeGeom> geom;            // internal numbering
   std::vector<int32_t> ce4;
   std::vector<double> area, inv_area, gn2, kst;
@@ -171,15 +173,21 @@ struct swe_ctx {
   BlobLayout blay{};
   unsigned char *d_blob = nullptr, *d_pflag = nullptr;
   int32_t *d_slot_string = nullptr; double *d_string_M = nullptr;
+  double *d_string_lk = nullptr; int32_t *d_string_cell = nullptr;
+  bool self_ctl = false;             // fused patch step without k_step_control (every block derives dt itself)
+  int64_t step_idx = 0;              // step launches enqueued so far (self_ctl: launch n reads Control::slot[n % 4])
+  int64_t n_string_edges = 0;
+  const PatchInst *patch_inst = nullptr;
   int n_patches = 0, patch_threads = 0, patch_prefetch = 0; size_t patch_smem = 0;
   int64_t patch_sum_loc = 0, patch_sum_e = 0; int patch_max_loc = 0, patch_max_e = 0, patch_min_blocks = 0;
-  PatchKernel patch_kernel = nullptr;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
   int cell_grid = 148 * 4;           // resident blocks of the persistent k_cell_update
   int edge_grid = 148 * 5;           // resident blocks of the persistent k_edge_flux (set from the occupancy API)
   int base_edge_grid = 0, base_cell_grid = 0, sms = 148;
   Morph mp{};                        // morphodynamics (swe_set_morphology); formula 0 = fixed bed
   bool morph_reserved = false;
+  bool single = false;               // single precision: the typed pointers above hold CellRecT<float> etc. (view<T>())
+  int32_t *geomR = nullptr;          // fp32: R of every edge
   uint8_t *d_drain_flag = nullptr;   // three-pass step: cells flagged as possible drainers (lazy theta)
   Scalars sc{};                      // passive scalars
   double *d_scalar_stage = nullptr;  // [n_cells] staging of one species for host-pointer set / get
@@ -196,6 +204,19 @@ struct swe_ctx {
 
 namespace {
 
+// the precision-dependent device arrays of a context, typed (fp64: the members themselves)
+template <typename T> struct View {
+  CellRecT<T> *rec, *rec_b; EdgeGeomT<T> *geom; EdgeFluxT<T> *flux; T *area, *inv_area, *gn2, *kst, *theta;
+};
+template <typename T> View<T> view(const swe_ctx *c) {
+  View<T> v;
+  v.rec = reinterpret_cast<CellRecT<T> *>(c->rec); v.rec_b = reinterpret_cast<CellRecT<T> *>(c->rec_b);
+  v.geom = reinterpret_cast<EdgeGeomT<T> *>(c->geom); v.flux = reinterpret_cast<EdgeFluxT<T> *>(c->flux);
+  v.area = reinterpret_cast<T *>(c->area); v.inv_area = reinterpret_cast<T *>(c->inv_area); v.gn2 = reinterpret_cast<T *>(c->gn2);
+  v.kst = reinterpret_cast<T *>(c->kst); v.theta = reinterpret_cast<T *>(c->theta);
+  return v;
+}
+
 #define SWE_CUDA(ctx, call)                                                                       \
   do {                                                                                            \
     cudaError_t e_ = (call);                                                                      \
@@ -209,8 +230,10 @@ namespace {
 constexpr int kMaxStepKernels = 4;
 const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"};
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
+const char *const kSelfNames[1] = {"k_patch_step"};
 
-inline int n_step_kernels(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH ? 2 : 4; }
+inline bool self_mode(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH && c->self_ctl && !c->single; }
+inline int n_step_kernels(const swe_ctx *c) { return self_mode(c) ? 1 : (c->variant == SWE_VARIANT_PATCH ? 2 : 4); }
 
 Patch2Args patch_args(const swe_ctx *c) {
   Patch2Args a;
@@ -219,8 +242,11 @@ Patch2Args patch_args(const swe_ctx *c) {
   a.strings = c->d_strings; a.slot_string = c->d_slot_string; a.string_M = c->d_string_M;
   a.pflag_a = c->d_pflag; a.pflag_b = c->d_pflag + (size_t)kPflagBytes * (size_t)c->n_patches;
   a.n_cells = (int32_t)c->nc;
+  a.step_k = (int32_t)(c->step_idx & 3); a.n_strings = (int32_t)c->strings.size(); a.n_string_edges = (int32_t)c->n_string_edges;
+  a.string_lk = c->d_string_lk; a.string_cell = c->d_string_cell;
   a.prefetch_dist = c->patch_prefetch;
   a.sc = c->sc;
+  a.mp = c->mp; a.gn2 = c->gn2;
   return a;
 }
 
@@ -232,22 +258,63 @@ void launch_patch_flags(swe_ctx *c) {
   c->launches += 2;
 }
 
+template <typename T>
+void launch_control_t(swe_ctx *c, cudaStream_t s, int mode) {
+  const View<T> v = view<T>(c);
+  k_step_control<T><<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, v.geom, v.flux,
+                                              (const T *)nullptr /* records are limited in place */, v.rec, v.rec_b, v.kst,
+                                              c->variant == SWE_VARIANT_PATCH ? c->d_string_M : nullptr, mode);
+}
 void launch_control(swe_ctx *c, cudaStream_t s, int mode) {
-  k_step_control<<<1, kCtlThreads, 0, s>>>(c->d_ctl, c->d_strings, c->d_string_edges, c->d_scratch, c->geom, c->flux,
-                                           nullptr /* records are limited in place */, c->rec, c->rec_b, c->kst,
-                                           c->variant == SWE_VARIANT_PATCH ? c->d_string_M : nullptr, mode);
+  if (c->single) launch_control_t<float>(c, s, mode); else launch_control_t<double>(c, s, mode);
 }
 
+// single precision: the three-pass step in fp32 (16-byte records); no scalars / mobile bed / patch step
+void enqueue_three_pass_f32(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev) {
+  const View<float> v = view<float>(c);
+  k_edge_flux<false, true, false, float><<<std::min(grid_for(c->ne), c->edge_grid), kBlock, 0, s>>>(
+      c->d_ctl, v.geom, v.rec, v.kst, c->d_strings, v.flux, (int)c->ne, 0, c->sc, v.area, c->d_drain_flag, Morph{}, c->geomR);
+  if (ev) cudaEventRecord(ev[2], s);
+  k_theta_lazy<float><<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, v.geom, v.flux, v.rec, v.area, v.theta,
+                                                                   c->d_drain_flag, (int)c->nc);
+  if (ev) cudaEventRecord(ev[3], s);
+  k_cell_update<false, false, float><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(
+      c->d_ctl, c->cell_edge, v.geom, v.flux, (const float *)nullptr, v.area, v.inv_area, v.gn2, v.rec, (int)c->nc, c->sc);
+  if (ev) cudaEventRecord(ev[4], s);
+}
+
+// the fused patch kernel of this context: instance by (scalars, self-controlled, mobile bed); the shared memory of a
+// block grows with the scalar species and the mobile-bed law
+void launch_patch(swe_ctx *c, cudaStream_t s, int self) {
+  const int morph = c->mp.formula;
+  const size_t smem = (size_t)patch2_smem_layout(c->blay, c->sc.n, morph).total;
+  c->patch_inst->fn[c->sc.n > 0][self][morph != 0]<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
+}
+
+// one time step, in stream order.  Self-controlled patch step: the launch number decides the control slot it reads
 void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
+  if (self_mode(c)) {
+    if (ev) cudaEventRecord(ev[0], s);
+    launch_patch(c, s, 1);
+    if (ev) cudaEventRecord(ev[1], s);
+    c->step_idx += 1;
+    return;
+  }
+  c->step_idx += 1;
   if (ev) cudaEventRecord(ev[0], s);
   launch_control(c, s, 0);
   if (ev) cudaEventRecord(ev[1], s);
+  if (c->single) { enqueue_three_pass_f32(c, s, ev); return; }
   if (c->variant == SWE_VARIANT_PATCH) {
-    c->patch_kernel<<<c->n_patches, c->patch_threads, c->patch_smem, s>>>(c->d_ctl, patch_args(c));
+    launch_patch(c, s, 0);
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
-  if (c->mp.formula)
+  const double *no_theta = nullptr;         // the records are limited in place by k_theta_lazy
+  if (c->mp.formula && c->sc.n > 0)
+    k_edge_flux<true, false, true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
+                                                               c->area, c->d_drain_flag, c->mp);
+  else if (c->mp.formula)
     k_edge_flux<false, true, true><<<std::min(grid_for(c->ne), c->edge_grid), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
                                                           c->area, c->d_drain_flag, c->mp);
   else if (c->sc.n > 0)
@@ -260,14 +327,17 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
   k_theta_lazy<<<grid_for((c->nc + 3) / 4), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, c->rec, c->area, c->theta,
                                                   c->d_drain_flag, (int)c->nc);
   if (ev) cudaEventRecord(ev[3], s);
-  if (c->mp.formula)
-    k_cell_update<false, true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+  if (c->mp.formula && c->sc.n > 0)
+    k_cell_update<true, true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, no_theta, c->area,
+                                                                 c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc, c->mp);
+  else if (c->mp.formula)
+    k_cell_update<false, true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, no_theta, c->area,
                                                                   c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc, c->mp);
   else if (c->sc.n > 0)
-    k_cell_update<true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+    k_cell_update<true><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, no_theta, c->area,
                                                            c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   else
-    k_cell_update<false><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, nullptr, c->area,
+    k_cell_update<false><<<std::min(grid_for(c->nc), c->cell_grid), kBlock, 0, s>>>(c->d_ctl, c->cell_edge, c->geom, c->flux, no_theta, c->area,
                                                             c->inv_area, c->gn2, c->rec, (int)c->nc, c->sc);
   if (ev) cudaEventRecord(ev[4], s);
 }
@@ -277,7 +347,10 @@ int capture_graph(swe_ctx *c) {
   cudaStream_t cap;
   SWE_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
   SWE_CUDA(c, cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
+  const int64_t idx = c->step_idx;     // a graph launch always starts at a launch number that is a multiple of 4
+  c->step_idx = 0;
   for (int k = 0; k < c->steps_per_graph; ++k) enqueue_step(c, cap);
+  c->step_idx = idx;
   cudaGraph_t g = nullptr;
   SWE_CUDA(c, cudaStreamEndCapture(cap, &g));
   SWE_CUDA(c, cudaGraphInstantiate(&c->graph_exec_v[c->variant], g, 0));
@@ -291,6 +364,21 @@ int read_control(swe_ctx *c) {   // device -> pinned host, synchronises the stre
   SWE_CUDA(c, cudaStreamSynchronize(c->stream));
   c->t_host = c->h_ctl->t;
   return SWE_OK;
+}
+
+// start / end of a run of steps (swe_step, swe_profile_step): stop conditions in; bookkeeping of the last step out
+void begin_call(swe_ctx *c, long long n_steps, double t_end, double cfl) {
+  if (self_mode(c)) k_self_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, n_steps, t_end, cfl, (int)(c->step_idx & 3));
+  else k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, n_steps, t_end, cfl);
+  c->launches += 1;
+}
+void end_call(swe_ctx *c, int final) {
+  if (self_mode(c))
+    k_self_finish<256><<<1, 256, 0, c->stream>>>(c->d_ctl, c->d_strings, (int)c->strings.size(), c->d_string_M, (int)c->n_string_edges,
+                                                  (int)(c->step_idx & 3), final);
+  else if (final) launch_control(c, c->stream, 1);
+  else return;
+  c->launches += 1;
 }
 
 void release(swe_ctx *c) {
@@ -315,6 +403,10 @@ int switch_variant(swe_ctx *c, int want, int cur) {
   k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, want == SWE_VARIANT_PATCH ? 1 : 0, 0);
   c->launches += 1;
   if (want == SWE_VARIANT_PATCH) launch_patch_flags(c);
+  if (want == SWE_VARIANT_THREE_PASS && c->mp.formula == 2) {     // the patch step does not keep Morph::cell
+    k_sed_cell_init<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)nc);
+    c->launches += 1;
+  }
   SWE_CUDA(c, cudaGetLastError());
   return SWE_OK;
 }
@@ -328,16 +420,18 @@ int upload_strings(swe_ctx *c) {
 }
 
 // sum of the member lengths of every string, by the same pairwise tree as the per-step sums
+template <typename T>
 __global__ void __launch_bounds__(kCtlThreads)
-k_string_lengths(BoundaryString *strings, int n_strings, const int *__restrict__ string_edges, double *scratch,
-                 const EdgeGeom *__restrict__ geom) {
+k_string_lengths(BoundaryString *strings, int n_strings, const int *__restrict__ string_edges, double *scratch_,
+                 const EdgeGeomT<T> *__restrict__ geom) {
+  T *scratch = reinterpret_cast<T *>(scratch_);
   for (int s = 0; s < n_strings; ++s) {
     BoundaryString &bs = strings[s];
     if (bs.n_edges == 0) continue;
-    double *v = scratch + bs.scratch;
-    for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) v[j] = j < bs.n_edges ? geom[string_edges[bs.first + j]].len : 0.0;
-    const double sum = block_tree_sum(v, bs.pow2);
-    if (threadIdx.x == 0) bs.sumL = sum;
+    T *v = scratch + bs.scratch;
+    for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) v[j] = j < bs.n_edges ? geom[string_edges[bs.first + j]].len : T(0.0);
+    const T sum = block_tree_sum(v, bs.pow2);
+    if (threadIdx.x == 0) bs.sumL = (double)sum;
     __syncthreads();
   }
 }
@@ -377,6 +471,10 @@ int check_params(const swe_params &p, std::string &err) {
   if (!(p.g > 0.0) || !(p.h_dry >= 0.0) || !(p.dt_max > 0.0)) { err = "g, h_dry, dt_max out of range"; return SWE_EINVAL; }
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
   if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) { err = "unknown variant"; return SWE_EINVAL; }
+  if (p.precision != SWE_PRECISION_DOUBLE && p.precision != SWE_PRECISION_SINGLE) { err = "unknown precision"; return SWE_EINVAL; }
+  if (p.precision == SWE_PRECISION_SINGLE && (p.n_species > 0 || p.morphology || p.variant == SWE_VARIANT_PATCH)) {
+    err = "single precision is built for the three-pass hydrodynamic step only (no scalars, mobile bed or patch step)"; return SWE_EINVAL;
+  }
   if (p.patch_cells != 0 && (p.patch_cells < 32 || p.patch_cells > 1024)) { err = "patch_cells must be 0 (default) or in [32, 1024]"; return SWE_EINVAL; }
   return SWE_OK;
 }
@@ -393,6 +491,7 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
   if (rc != SWE_OK) return rc;
   const int64_t nc = hm.nc, ne = hm.ne;
   pl.z.nc = nc; pl.z.ne = ne; pl.z.n_species = p.n_species; pl.z.morph = p.morphology != 0;
+  pl.z.single = p.precision == SWE_PRECISION_SINGLE;
 
   // ---- arrays in internal numbering
   pl.geom.resize(ne); pl.ce4.resize((size_t)4 * nc);
@@ -442,9 +541,16 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
   for (int s = 0; s <= max_id; ++s)
     for (int32_t j = 0; j < pl.strings[s].n_edges; ++j) pl.slot_string[pl.strings[s].first + j] = s;
   pl.z.n_strings = max_id + 1; pl.z.n_string_edges = (int64_t)pl.flat.size(); pl.z.scratch = (int64_t)scratch;
+  pl.string_lk.assign(std::max<size_t>(1, pl.flat.size()), 0.0); pl.string_cell.assign(std::max<size_t>(1, pl.flat.size()), 0);
+  for (size_t j = 0; j < pl.flat.size(); ++j) {
+    const EdgeGeom &eg = pl.geom[pl.flat[j]];
+    const double k = pl.kst[eg.L];
+    pl.string_lk[j] = eg.len * (std::isfinite(k) ? k : 1.0);
+    pl.string_cell[j] = eg.L;
+  }
 
   // ---- fused patch step: patch blobs, shared-memory size
-  pl.variant = (p.variant == SWE_VARIANT_THREE_PASS) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+  pl.variant = (p.variant == SWE_VARIANT_THREE_PASS || pl.z.single) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
   if (pl.variant == SWE_VARIANT_PATCH) {
     // default: 256 cells = 256 threads (profiles/r2*_patch_sweep.md); small meshes get smaller patches, so that the
     // launch-latency-bound step still spreads over the SMs
@@ -497,7 +603,9 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->own_ws = true;
   }
   char *ws = c->ws;
-  c->rec = (CellRec *)(ws + lay.rec); c->rec_b = (CellRec *)(ws + lay.rec_b); c->geom = (EdgeGeom *)(ws + lay.geom); c->flux = (EdgeFlux *)(ws + lay.flux);
+  c->single = pl.z.single;
+  if (c->single) c->geomR = (int32_t *)(ws + lay.geomR);
+  c->rec = (CellRec *)(ws + lay.rec); c->rec_b = (CellRec *)(ws + (c->single ? lay.rec : lay.rec_b)); c->geom = (EdgeGeom *)(ws + lay.geom); c->flux = (EdgeFlux *)(ws + lay.flux);
   c->cell_edge = (int4 *)(ws + lay.cell_edge);
   c->area = (double *)(ws + lay.area); c->inv_area = (double *)(ws + lay.inv_area);
   c->gn2 = (double *)(ws + lay.gn2); c->kst = (double *)(ws + lay.kst); c->theta = (double *)(ws + lay.theta);
@@ -509,6 +617,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   c->d_strings = (BoundaryString *)(ws + lay.strings); c->d_string_edges = (int *)(ws + lay.string_edges);
   c->d_scratch = (double *)(ws + lay.scratch); c->d_params = (double *)(ws + lay.params);
   c->d_slot_string = (int32_t *)(ws + lay.slot_string); c->d_string_M = (double *)(ws + lay.string_M);
+  c->d_string_lk = (double *)(ws + lay.string_lk); c->d_string_cell = (int32_t *)(ws + lay.string_cell);
+  c->n_string_edges = (int64_t)std::max<size_t>(1, pl.flat.size());
   c->sc.n = p.n_species;
   for (int sp = 0; sp < c->sc.n; ++sp) {
     c->sc.qa[sp] = (double *)(ws + lay.qa[sp]); c->sc.qb[sp] = (double *)(ws + lay.qb[sp]); c->sc.phi_up[sp] = (double *)(ws + lay.phi_up[sp]);
@@ -520,27 +630,51 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
 
   // ---- upload
   {
-    std::vector<CellRec> rec(nc);
-    for (int64_t i = 0; i < nc; ++i) rec[i] = {0.0, 0.0, 0.0, mesh->zb[c->hm.cell_perm[i]]};
-    std::vector<double> theta(nc, 1.0);
     auto up = [&](void *dst, const void *src, size_t bytes) { return bytes ? cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) : cudaSuccess; };
-    SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
-    SWE_CUDA(c, up(c->rec_b, rec.data(), sizeof(CellRec) * nc));     // z_B must be valid in both state buffers
+    if (!c->single) {
+      std::vector<CellRec> rec(nc);
+      for (int64_t i = 0; i < nc; ++i) rec[i] = {0.0, 0.0, 0.0, mesh->zb[c->hm.cell_perm[i]]};
+      std::vector<double> theta(nc, 1.0);
+      SWE_CUDA(c, up(c->rec, rec.data(), sizeof(CellRec) * nc));
+      SWE_CUDA(c, up(c->rec_b, rec.data(), sizeof(CellRec) * nc));     // z_B must be valid in both state buffers
+      SWE_CUDA(c, up(c->area, pl.area.data(), 8 * nc));
+      SWE_CUDA(c, up(c->inv_area, pl.inv_area.data(), 8 * nc));
+      SWE_CUDA(c, up(c->gn2, pl.gn2.data(), 8 * nc));
+      SWE_CUDA(c, up(c->kst, pl.kst.data(), 8 * nc));
+      SWE_CUDA(c, up(c->theta, theta.data(), 8 * nc));
+      SWE_CUDA(c, up(c->geom, pl.geom.data(), sizeof(EdgeGeom) * ne));
+    } else {
+      // single precision (R-21): geometry and constants are the fp64 values rounded ONCE to fp32
+      const View<float> v = view<float>(c);
+      std::vector<CellRecT<float>> rec(nc);
+      std::vector<float> f(nc);
+      for (int64_t i = 0; i < nc; ++i) rec[i] = {0.f, 0.f, 0.f, (float)mesh->zb[c->hm.cell_perm[i]]};
+      SWE_CUDA(c, up(v.rec, rec.data(), sizeof(CellRecT<float>) * nc));
+      const std::vector<double> *srcs[4] = {&pl.area, &pl.inv_area, &pl.gn2, &pl.kst};
+      float *dsts[4] = {v.area, v.inv_area, v.gn2, v.kst};
+      for (int a = 0; a < 4; ++a) {
+        for (int64_t i = 0; i < nc; ++i) f[i] = (float)(*srcs[a])[i];
+        SWE_CUDA(c, up(dsts[a], f.data(), 4 * nc));
+      }
+      for (int64_t i = 0; i < nc; ++i) f[i] = 1.f;
+      SWE_CUDA(c, up(v.theta, f.data(), 4 * nc));
+      std::vector<EdgeGeomT<float>> g32(ne);
+      std::vector<int32_t> gR(ne);
+      for (int64_t e = 0; e < ne; ++e) { g32[e] = {(float)pl.geom[e].nx, (float)pl.geom[e].ny, (float)pl.geom[e].len, pl.geom[e].L}; gR[e] = pl.geom[e].R; }
+      SWE_CUDA(c, up(v.geom, g32.data(), sizeof(EdgeGeomT<float>) * ne));
+      SWE_CUDA(c, up(c->geomR, gR.data(), 4 * ne));
+    }
     SWE_CUDA(c, up(c->cell_edge, pl.ce4.data(), sizeof(int4) * nc));
-    SWE_CUDA(c, up(c->area, pl.area.data(), 8 * nc));
-    SWE_CUDA(c, up(c->inv_area, pl.inv_area.data(), 8 * nc));
-    SWE_CUDA(c, up(c->gn2, pl.gn2.data(), 8 * nc));
-    SWE_CUDA(c, up(c->kst, pl.kst.data(), 8 * nc));
-    SWE_CUDA(c, up(c->theta, theta.data(), 8 * nc));
-    SWE_CUDA(c, up(c->geom, pl.geom.data(), sizeof(EdgeGeom) * ne));
     SWE_CUDA(c, up(c->cell_perm, c->hm.cell_perm.data(), 4 * nc));
     SWE_CUDA(c, up(c->edge_perm, c->hm.edge_perm.data(), 4 * ne));
-    SWE_CUDA(c, cudaMemset(c->flux, 0, sizeof(EdgeFlux) * ne));
+    SWE_CUDA(c, cudaMemset(c->flux, 0, (c->single ? sizeof(EdgeFluxT<float>) : sizeof(EdgeFlux)) * ne));
     SWE_CUDA(c, cudaMemset(c->d_drain_flag, 0, (size_t)nc + 16));
     SWE_CUDA(c, cudaMemset(c->d_info_ticket, 0, sizeof(unsigned int)));
     SWE_CUDA(c, up(c->d_string_edges, pl.flat.data(), 4 * pl.flat.size()));
     SWE_CUDA(c, up(c->d_slot_string, pl.slot_string.data(), 4 * pl.slot_string.size()));
-    SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 8 * std::max<size_t>(1, pl.flat.size())));
+    SWE_CUDA(c, cudaMemset(c->d_string_M, 0, 2 * 8 * std::max<size_t>(1, pl.flat.size())));
+    SWE_CUDA(c, up(c->d_string_lk, pl.string_lk.data(), 8 * pl.string_lk.size()));
+    SWE_CUDA(c, up(c->d_string_cell, pl.string_cell.data(), 4 * pl.string_cell.size()));
     for (int sp = 0; sp < c->sc.n; ++sp) {
       SWE_CUDA(c, cudaMemset(c->sc.qa[sp], 0, 8 * nc));
       SWE_CUDA(c, cudaMemset(c->sc.qb[sp], 0, 8 * nc));
@@ -552,7 +686,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   c->param_off.assign(c->strings.size(), 0); c->param_cap.assign(c->strings.size(), 0);
   if (!c->strings.empty()) {
     SWE_CUDA(c, cudaMemcpy(c->d_strings, c->strings.data(), sizeof(BoundaryString) * c->strings.size(), cudaMemcpyHostToDevice));
-    k_string_lengths<<<1, kCtlThreads, 0, c->stream>>>(c->d_strings, (int)c->strings.size(), c->d_string_edges, c->d_scratch, c->geom);
+    if (c->single) k_string_lengths<float><<<1, kCtlThreads, 0, c->stream>>>(c->d_strings, (int)c->strings.size(), c->d_string_edges, c->d_scratch, view<float>(c).geom);
+    else k_string_lengths<double><<<1, kCtlThreads, 0, c->stream>>>(c->d_strings, (int)c->strings.size(), c->d_string_edges, c->d_scratch, c->geom);
     SWE_CUDA(c, cudaGetLastError());
     SWE_CUDA(c, cudaStreamSynchronize(c->stream));
     SWE_CUDA(c, cudaMemcpy(c->strings.data(), c->d_strings, sizeof(BoundaryString) * c->strings.size(), cudaMemcpyDeviceToHost));
@@ -567,6 +702,12 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     if (c->sc.n > 0) SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<true>, kBlock, 0));
     else SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false>, kBlock, 0));
     c->cell_grid = std::max(1, sms * per_sm);
+    if (c->single) {
+      SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_edge_flux<false, true, false, float>, kBlock, 0));
+      c->edge_grid = std::max(1, sms * per_sm);
+      SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false, false, float>, kBlock, 0));
+      c->cell_grid = std::max(1, sms * per_sm);
+    }
     c->base_edge_grid = c->edge_grid; c->base_cell_grid = c->cell_grid; c->sms = sms;
   }
 
@@ -585,14 +726,24 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     int force = 0;
     if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) force = std::atoi(s);
     c->patch_threads = patch_threads(pb.lay.P);
-    bool pair = false;
-    if (const char *s = std::getenv("SWE_PATCH_PAIR")) pair = std::atoi(s) != 0 && c->sc.n == 0;
     c->patch_prefetch = 3 * 148;
     if (const char *s = std::getenv("SWE_PATCH_PREFETCH")) c->patch_prefetch = std::atoi(s);
-    const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force, pair);
-    if (!pi && pair) pi = pick_patch_kernel(c->patch_threads, c->sc.n > 0, c->patch_smem, force, false);
+    // (sized for the fattest block the context can ask for: the mobile bed with the MPM-like law, when reserved)
+    const size_t smem_max = (size_t)patch2_smem_layout(pb.lay, c->sc.n, pl.z.morph ? 2 : 0).total;
+    const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem_max, force);
     if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
-    c->patch_kernel = pi->fn; c->patch_min_blocks = pi->min_blocks;
+    c->patch_inst = pi; c->patch_min_blocks = pi->min_blocks;
+    // self-controlled steps: at most kCtlPre strings, each string's pairwise tree inside the block's scratch (the
+    // flux arrays of the patch, and the 1024 doubles of k_self_finish), graphs a multiple of 4 steps long
+    {
+      const int64_t cap = std::min<int64_t>(1024, (int64_t)pb.lay.cap_e + 3 * (int64_t)pb.lay.cap_eown);
+      // (it saves the control kernel's graph node, 2.3-2.6 us per step: + 20-30 % on meshes up to ~100k cells, nothing
+      // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2_self_ctl.md)
+      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= 8192;
+      for (const BoundaryString &bs : c->strings) ok = ok && bs.pow2 <= cap;
+      if (const char *s = std::getenv("SWE_PATCH_SELF")) ok = ok && std::atoi(s) != 0;
+      c->self_ctl = ok;
+    }
     // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
     // context with smaller patches cannot lower it under an earlier context's launches
     {
@@ -600,10 +751,13 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       cudaFuncAttributes fa{};
       SWE_CUDA(c, cudaGetDevice(&dev));
       SWE_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-      SWE_CUDA(c, cudaFuncGetAttributes(&fa, c->patch_kernel));
-      const int limit = optin - (int)fa.sharedSizeBytes;
-      if ((int)c->patch_smem > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
-      SWE_CUDA(c, cudaFuncSetAttribute(c->patch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
+      for (int a = 0; a < 8; ++a) {
+        PatchKernel fn = pi->fn[a & 1][(a >> 1) & 1][(a >> 2) & 1];
+        SWE_CUDA(c, cudaFuncGetAttributes(&fa, fn));
+        const int limit = optin - (int)fa.sharedSizeBytes;
+        if ((int)smem_max > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
+        SWE_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
+      }
     }
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
     // state in 32 + state out 32 + slot words 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
@@ -623,12 +777,17 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     ab[3] = (16 + 8 + 8 + 64) * nc + 64 * ne;
     ab[1] += (int64_t)c->sc.n * (8 * nc + 8 * ne);       // q_c gathered once, upwind concentration written
     ab[3] += (int64_t)c->sc.n * (16 * nc + 8 * ne);      // q_c read + written, upwind concentration gathered
+    if (c->single) {      // 16-byte records, 4-byte reals, R of an edge in its own int32 array
+      ab[1] = (16 + 4 + 16) * ne + 16 * nc;
+      ab[3] = (16 + 4 + 4 + 32) * nc + 32 * ne;
+    }
     c->alg_bytes_base[0] = ab[1]; c->alg_bytes_base[1] = ab[3];
     // SURVEY.md section 8(d), two-kernel column (284 B per cell-step with 1/A read in the edge pass), split as the
     // survey's rows split: edge pass = state 24 + z 8 + 1/A 8 + geometry 36 + edge->cell 12 + flux written 60 = 148;
     // cell pass = state 24 r + 24 w + g/k^2, 1/A 16 + cell->edge 12 + flux read 60 = 136
     int64_t *sb = c->survey_bytes_v[SWE_VARIANT_THREE_PASS];
     sb[1] = 148 * nc; sb[2] = 0; sb[3] = 136 * nc;
+    if (c->single) { sb[1] = (148 - 12 - 12) / 2 * nc + 24 * nc; sb[3] = (136 - 12) / 2 * nc + 12 * nc; }   // reals halve, int32 tables stay
   }
 
   // ---- control block
@@ -669,6 +828,7 @@ void swe_params_default(swe_params *p) {
   p->patch_cells = 0;
   p->n_species = 0;
   p->morphology = 0;
+  p->precision = SWE_PRECISION_DOUBLE;
 }
 
 size_t swe_workspace_bytes(const swe_mesh *mesh, const swe_params *params) {
@@ -767,14 +927,16 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     k_set_variant<<<1, 1, 0, c->stream>>>(c->d_ctl, want == SWE_VARIANT_PATCH ? 1 : 0, 0);
     c->launches += 1;
   }
-  k_pack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
+  if (c->single) { const View<float> v = view<float>(c); k_pack_state<float><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, v.rec, v.rec_b, (int)nc); }
+  else k_pack_state<double><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, dh, dhu, dhv, c->rec, c->rec_b, (int)nc);
   if (c->variant == SWE_VARIANT_PATCH) launch_patch_flags(c);
-  if (c->mp.formula == 2) {           // mobile bed, MPM-like law: the per-cell cube roots of the new state
+  if (c->mp.formula == 2 && c->variant == SWE_VARIANT_THREE_PASS) {   // mobile bed, MPM-like law: the per-cell cube roots of the new state
     k_sed_cell_init<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)nc);
     c->launches += 1;
   }
   k_reset<<<1, 1, 0, c->stream>>>(c->d_ctl, t0);
-  k_rate<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, c->rec_b, (int)nc);
+  if (c->single) { const View<float> v = view<float>(c); k_rate<float><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, v.geom, v.inv_area, v.rec, v.rec_b, (int)nc); }
+  else k_rate<double><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_edge, c->geom, c->inv_area, c->rec, c->rec_b, (int)nc);
   c->launches += 3;
   SWE_CUDA(c, cudaGetLastError());
   c->t_host = t0;
@@ -786,19 +948,23 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
   if (!(cfl > 0.0) || std::isnan(t_end)) { c->err = "cfl must be > 0 and t_end a number"; return SWE_EINVAL; }
   const bool finite_end = std::isfinite(t_end);
   if (n_steps < 0 && !finite_end) { c->err = "either n_steps >= 0 or a finite t_end is needed"; return SWE_EINVAL; }
-  k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, (long long)n_steps, t_end, cfl);
-  c->launches += 1;
+  begin_call(c, (long long)n_steps, t_end, cfl);
   const int K = c->steps_per_graph;
   int64_t remaining = n_steps < 0 ? std::numeric_limits<int64_t>::max() : n_steps;
   int64_t poll_every = 4;            // graph launches between two reads of t (only when t_end is finite)
   bool done = !(c->t_host < t_end);  // t_end already reached: nothing to do
   while (!done && remaining > 0) {
     int64_t batch_steps = 0;
-    if (K > 0 && remaining >= K) {
+    if (K > 0 && remaining >= K && self_mode(c) && (c->step_idx & 3) != 0) {
+      batch_steps = std::min<int64_t>(remaining, 4 - (c->step_idx & 3));   // plain launches up to a multiple of 4
+      for (int64_t j = 0; j < batch_steps; ++j) enqueue_step(c, c->stream);
+      SWE_CUDA(c, cudaGetLastError());
+    } else if (K > 0 && remaining >= K) {
       int64_t n_graphs = remaining / K;
       if (finite_end) n_graphs = std::min(n_graphs, poll_every);
       for (int64_t j = 0; j < n_graphs; ++j) SWE_CUDA(c, cudaGraphLaunch(c->graph_exec_v[c->variant], c->stream));
       batch_steps = n_graphs * K;
+      c->step_idx += batch_steps;
     } else {
       batch_steps = std::min<int64_t>(remaining, 64);   // tail shorter than a graph, or graphs switched off
       for (int64_t j = 0; j < batch_steps; ++j) enqueue_step(c, c->stream);
@@ -807,6 +973,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     c->launches += batch_steps * n_step_kernels(c);
     remaining -= batch_steps;
     if (finite_end) {                // the only host synchronisation inside the loop: once per batch
+      end_call(c, 0);                // (self-controlled steps: snapshot of the newest slot into the fields read here)
       int rc = read_control(c);
       if (rc != SWE_OK) return rc;
       if (!(c->h_ctl->t < t_end) || (c->h_ctl->flags & (SWE_FLAG_DT_UNBOUNDED | SWE_FLAG_STALLED))) done = true;
@@ -814,12 +981,11 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     }
   }
   // volume bookkeeping of the last step; then the reductions of swe_step_info
-  launch_control(c, c->stream, 1);
-  c->launches += 1;
+  end_call(c, 1);
   SWE_CUDA(c, cudaGetLastError());
   if (info) {
-    k_info<<<std::min(grid_for(c->nc), kInfoMaxBlocks), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, c->area, (int)c->nc,
-                                                                               c->d_info_part, c->d_info_ticket);
+    if (c->single) { const View<float> v = view<float>(c); k_info<float><<<std::min(grid_for(c->nc), kInfoMaxBlocks), kBlock, 0, c->stream>>>(c->d_ctl, v.rec, v.rec_b, v.area, (int)c->nc, c->d_info_part, c->d_info_ticket); }
+    else k_info<double><<<std::min(grid_for(c->nc), kInfoMaxBlocks), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, c->area, (int)c->nc, c->d_info_part, c->d_info_ticket);
     c->launches += 1;
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
@@ -889,58 +1055,59 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
     c->err = "the MPM-like formula needs s > 1, d_m > 0 and a finite theta_cr"; return SWE_EINVAL;
   }
   if (formula && !c->morph_reserved) { c->err = "the context was created without room for the mobile-bed module: set swe_params.morphology = 1"; return SWE_EINVAL; }
-  if (formula && c->sc.n > 0) { c->err = "passive scalars and a mobile bed in one context are not built"; return SWE_EINVAL; }
-  if (formula && !c->auto_mode && c->variant == SWE_VARIANT_PATCH) {
-    c->err = "the fused patch step has no mobile bed: create the context with SWE_VARIANT_AUTO or SWE_VARIANT_THREE_PASS";
-    return SWE_EINVAL;
-  }
   int rc = read_control(c);          // synchronises: no step in flight
   if (rc != SWE_OK) return rc;
-  if (formula) {
-    if (c->variant == SWE_VARIANT_PATCH) {
-      rc = switch_variant(c, SWE_VARIANT_THREE_PASS, c->h_ctl->cur);
-      if (rc != SWE_OK) return rc;
-    }
-    c->auto_mode = false;            // stays three-pass from here on
-  }
   const double g = c->prm.g;
   c->mp.formula = formula; c->mp.alpha = alpha; c->mp.theta_cr = theta_cr;
   c->mp.shields_den = g * ((s - 1.0) * d_m);
   c->mp.Gm = alpha * std::sqrt(((s - 1.0) * g) * (d_m * (d_m * d_m)));
   c->mp.inv1mp = 1.0 / (1.0 - porosity);
-  if (formula == 2) {                 // (g/k^2, cbrt(h)) of the state as it stands; k_cell_update keeps it current
+  // the fused patch step ping-pongs between two record buffers and leaves the records of skipped (dry) patches alone:
+  // both buffers must hold the bed as it is now (afterwards a patch's bed only moves in steps that rewrite its records)
+  if (c->has_patch) {
+    k_sync_bed<<<grid_for(c->nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->rec_b, (int)c->nc);
+    c->launches += 1;
+  }
+  if (formula == 2 && c->variant == SWE_VARIANT_THREE_PASS) {   // (g/k^2, cbrt(h)) of the state as it stands; k_cell_update keeps it current
     k_sed_cell_init<<<grid_for(c->nc), kBlock, 0, c->stream>>>(c->d_ctl, c->rec, c->gn2, c->mp.cell, (int)c->nc);
     c->launches += 1;
-    SWE_CUDA(c, cudaGetLastError());
   }
-  {                                   // algorithmic bytes of the two kernels that carry the extra work
+  SWE_CUDA(c, cudaGetLastError());
+  {                                   // algorithmic bytes of the kernels that carry the extra work
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
     ab[1] = c->alg_bytes_base[0] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
     ab[3] = c->alg_bytes_base[1] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
+    if (c->has_patch) c->alg_bytes_v[SWE_VARIANT_PATCH][1] = 104 * c->nc + 32 * c->ne + (int64_t)c->sc.n * 16 * c->nc + (formula == 2 ? 8 * c->nc : 0);
   }
   c->edge_grid = c->base_edge_grid; c->cell_grid = c->base_cell_grid;
   if (formula) {                      // resident grids of the <kMorph> instances
     int per_sm = 3;
-    SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_edge_flux<false, true, true>, kBlock, 0));
-    c->edge_grid = std::max(1, c->sms * per_sm);
-    SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false, true>, kBlock, 0));
+    if (c->sc.n > 0) SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<true, true>, kBlock, 0));
+    else {
+      SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_edge_flux<false, true, true>, kBlock, 0));
+      c->edge_grid = std::max(1, c->sms * per_sm);
+      SWE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_update<false, true>, kBlock, 0));
+    }
     c->cell_grid = std::max(1, c->sms * per_sm);
   }
-  if (c->graph_exec_v[SWE_VARIANT_THREE_PASS]) {
-    SWE_CUDA(c, cudaStreamSynchronize(c->stream));
-    cudaGraphExecDestroy(c->graph_exec_v[SWE_VARIANT_THREE_PASS]);
-    c->graph_exec_v[SWE_VARIANT_THREE_PASS] = nullptr;
+  // the graphs of both variants launch other kernel instances now: capture them again
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  const int keep = c->variant;
+  for (int v : {SWE_VARIANT_THREE_PASS, SWE_VARIANT_PATCH}) {
+    if (!c->graph_exec_v[v]) continue;
+    cudaGraphExecDestroy(c->graph_exec_v[v]);
+    c->graph_exec_v[v] = nullptr;
+    c->variant = v;
+    rc = capture_graph(c);
+    if (rc != SWE_OK) { c->variant = keep; return rc; }
   }
-  if (c->variant == SWE_VARIANT_THREE_PASS) return capture_graph(c);
-  const int keep = c->variant;        // fixed bed again on a context that steps with the patch kernel
-  c->variant = SWE_VARIANT_THREE_PASS;
-  rc = capture_graph(c);
   c->variant = keep;
-  return rc;
+  return SWE_OK;
 }
 
 int swe_get_bed(swe_ctx *c, double *zb) {
   if (!c) return SWE_EINVAL;
+  if (c->single) { c->err = "swe_get_bed: not built for single precision (the bed is fixed there: it is the caller's zb rounded to fp32)"; return SWE_EINVAL; }
   if (!zb) { c->err = "null bed pointer"; return SWE_EINVAL; }
   const int64_t nc = c->nc;
   double *dst = c->prm.state_on_device ? zb : c->stage;
@@ -959,6 +1126,17 @@ int swe_get_sediment_flux(swe_ctx *c, double *qB) {
   if (!qB) { c->err = "null flux pointer"; return SWE_EINVAL; }
   if (!c->morph_reserved) { c->err = "the context has no mobile-bed module (swe_params.morphology)"; return SWE_EINVAL; }
   const int64_t ne = c->ne;
+  if (c->variant == SWE_VARIANT_PATCH && c->mp.formula) {
+    // the fused step keeps q_Bij in shared memory: re-evaluate the most recent step's with the stand-alone edge kernel,
+    // from the state that step read (still intact in the other buffer)
+    int rc = read_control(c);
+    if (rc != SWE_OK) return rc;
+    const CellRec *in = c->h_ctl->src ? c->rec_b : c->rec;
+    if (c->mp.formula == 2) k_sed_cell_init<<<grid_for(c->nc), kBlock, 0, c->stream>>>(c->d_ctl, in, c->gn2, c->mp.cell, (int)c->nc);
+    k_edge_flux<false, false, true><<<grid_for(ne), kBlock, 0, c->stream>>>(c->d_ctl, c->geom, in, c->kst, c->d_strings, c->flux, (int)ne, 1, Scalars{},
+                                                                          c->area, nullptr, c->mp);
+    c->launches += 2;
+  }
   double *dst = c->prm.state_on_device ? qB : c->stage;       // stage holds 3 n_cells >= n_edges doubles
   k_export_sediment<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->mp.qB, dst, (int)ne);
   c->launches += 1;
@@ -984,13 +1162,14 @@ int swe_get_state(swe_ctx *c, double *h, double *hu, double *hv) {
   if (!h || !hu || !hv) { c->err = "null state pointer"; return SWE_EINVAL; }
   const int64_t nc = c->nc;
   if (c->prm.state_on_device) {
-    k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, h, hu, hv, (int)nc);
+    if (c->single) { const View<float> v = view<float>(c); k_unpack_state<float><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, v.rec, v.rec_b, h, hu, hv, (int)nc); }
+    else k_unpack_state<double><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, h, hu, hv, (int)nc);
     c->launches += 1;
     SWE_CUDA(c, cudaGetLastError());
     return SWE_OK;
   }
-  k_unpack_state<<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, c->stage, c->stage + nc,
-                                                         c->stage + 2 * nc, (int)nc);
+  if (c->single) { const View<float> v = view<float>(c); k_unpack_state<float><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, v.rec, v.rec_b, c->stage, c->stage + nc, c->stage + 2 * nc, (int)nc); }
+  else k_unpack_state<double><<<grid_for(nc), kBlock, 0, c->stream>>>(c->d_ctl, c->cell_perm, c->rec, c->rec_b, c->stage, c->stage + nc, c->stage + 2 * nc, (int)nc);
   c->launches += 1;
   SWE_CUDA(c, cudaMemcpyAsync(h, c->stage, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
   SWE_CUDA(c, cudaMemcpyAsync(hu, c->stage + nc, 8 * nc, cudaMemcpyDeviceToHost, c->stream));
@@ -1011,9 +1190,21 @@ const char *swe_last_error(const swe_ctx *c) { return c ? c->err.c_str() : g_cre
 int swe_get_geometry(swe_ctx *c, double *area, double *nx, double *ny, double *len) {
   if (!c || !area || !nx || !ny || !len) return SWE_EINVAL;
   // read back what the kernels use (device arrays, internal numbering) and undo the renumbering
+  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (c->single) {
+    std::vector<float> a(c->nc);
+    std::vector<EdgeGeomT<float>> g(c->ne);
+    SWE_CUDA(c, cudaMemcpy(a.data(), c->area, 4 * c->nc, cudaMemcpyDeviceToHost));
+    SWE_CUDA(c, cudaMemcpy(g.data(), c->geom, sizeof(EdgeGeomT<float>) * c->ne, cudaMemcpyDeviceToHost));
+    for (int64_t i = 0; i < c->nc; ++i) area[c->hm.cell_perm[i]] = a[i];
+    for (int64_t e = 0; e < c->ne; ++e) {
+      const int32_t o = c->hm.edge_perm[e];
+      nx[o] = g[e].nx; ny[o] = g[e].ny; len[o] = g[e].len;
+    }
+    return SWE_OK;
+  }
   std::vector<double> a(c->nc);
   std::vector<EdgeGeom> g(c->ne);
-  SWE_CUDA(c, cudaStreamSynchronize(c->stream));
   SWE_CUDA(c, cudaMemcpy(a.data(), c->area, 8 * c->nc, cudaMemcpyDeviceToHost));
   SWE_CUDA(c, cudaMemcpy(g.data(), c->geom, sizeof(EdgeGeom) * c->ne, cudaMemcpyDeviceToHost));
   for (int64_t i = 0; i < c->nc; ++i) area[c->hm.cell_perm[i]] = a[i];
@@ -1040,15 +1231,20 @@ int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR
   const double *th_apply = (c->variant == SWE_VARIANT_PATCH) ? c->theta : nullptr;   // three-pass: limited in place
   double *d = c->stage;                                // holds 2 n_edges doubles: export in two halves
   for (int half = 0; half < 2; ++half) {
-    k_export_flux<<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, th_apply, half ? nullptr : d, half ? nullptr : d + ne,
-                                                          half ? d : nullptr, half ? d + ne : nullptr, (int)ne);
+    double *o1 = half ? nullptr : d, *o2 = half ? nullptr : d + ne, *o3 = half ? d : nullptr, *o4 = half ? d + ne : nullptr;
+    if (c->single) { const View<float> v = view<float>(c); k_export_flux<float><<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, v.geom, v.flux, (const float *)nullptr, o1, o2, o3, o4, (int)ne); }
+    else k_export_flux<double><<<grid_for(ne), kBlock, 0, c->stream>>>(c->edge_perm, c->geom, c->flux, th_apply, o1, o2, o3, o4, (int)ne);
     c->launches += 1;
     SWE_CUDA(c, cudaGetLastError());
     SWE_CUDA(c, cudaStreamSynchronize(c->stream));
     SWE_CUDA(c, cudaMemcpy(half ? GL : F1, d, 8 * ne, cudaMemcpyDeviceToHost));
     SWE_CUDA(c, cudaMemcpy(half ? GR : F3, d + ne, 8 * ne, cudaMemcpyDeviceToHost));
   }
-  if (theta) {
+  if (theta && c->single) {
+    std::vector<float> th(nc);
+    SWE_CUDA(c, cudaMemcpy(th.data(), c->theta, 4 * nc, cudaMemcpyDeviceToHost));
+    for (int64_t i = 0; i < nc; ++i) theta[c->hm.cell_perm[i]] = th[i];
+  } else if (theta) {
     std::vector<double> th(nc);
     SWE_CUDA(c, cudaMemcpy(th.data(), c->theta, 8 * nc, cudaMemcpyDeviceToHost));
     for (int64_t i = 0; i < nc; ++i) theta[c->hm.cell_perm[i]] = th[i];
@@ -1180,12 +1376,12 @@ int swe_step_kernel_count(const swe_ctx *c) { return c ? n_step_kernels(c) : 0; 
 
 const char *swe_step_kernel_name(const swe_ctx *c, int k) {
   if (!c || k < 0 || k >= n_step_kernels(c)) return nullptr;
-  return c->variant == SWE_VARIANT_PATCH ? kPatchNames[k] : kThreePassNames[k];
+  return self_mode(c) ? kSelfNames[k] : (c->variant == SWE_VARIANT_PATCH ? kPatchNames[k] : kThreePassNames[k]);
 }
 
-int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes_v[c->variant][k] : 0; }
+int64_t swe_algorithmic_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->alg_bytes_v[c->variant][self_mode(c) ? k + 1 : k] : 0; }
 
-int64_t swe_survey_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->survey_bytes_v[c->variant][k] : 0; }
+int64_t swe_survey_bytes(const swe_ctx *c, int k) { return (c && k >= 0 && k < n_step_kernels(c)) ? c->survey_bytes_v[c->variant][self_mode(c) ? k + 1 : k] : 0; }
 
 int swe_get_patch_stats(swe_ctx *c, int64_t *out, int n_out) {
   if (!c || !out || n_out < 1) return SWE_EINVAL;
@@ -1207,8 +1403,7 @@ int swe_profile_step(swe_ctx *c, int64_t n_steps, double cfl, double *ms, int n_
   std::vector<cudaEvent_t> ev((size_t)kBatch * kEv, nullptr);
   for (auto &e : ev) SWE_CUDA(c, cudaEventCreate(&e));
   double sum[kMaxStepKernels] = {0.0};
-  k_call_begin<<<1, 1, 0, c->stream>>>(c->d_ctl, (long long)n_steps, std::numeric_limits<double>::infinity(), cfl);
-  c->launches += 1;
+  begin_call(c, (long long)n_steps, std::numeric_limits<double>::infinity(), cfl);
   cudaError_t rc = cudaSuccess;
   for (int64_t done = 0; done < n_steps && rc == cudaSuccess; done += kBatch) {
     const int nb = (int)std::min<int64_t>(kBatch, n_steps - done);
@@ -1224,8 +1419,7 @@ int swe_profile_step(swe_ctx *c, int64_t n_steps, double cfl, double *ms, int n_
   }
   for (auto &e : ev) cudaEventDestroy(e);
   SWE_CUDA(c, rc);
-  launch_control(c, c->stream, 1);
-  c->launches += 1;
+  end_call(c, 1);
   SWE_CUDA(c, cudaGetLastError());
   for (int k = 0; k < n_ms; ++k) ms[k] = k < nk ? sum[k] / (double)n_steps : 0.0;
   c->t_host = -std::numeric_limits<double>::infinity();

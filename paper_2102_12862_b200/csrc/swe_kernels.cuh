@@ -33,97 +33,100 @@ constexpr int kFlagUnbounded = 2, kFlagStalled = 4;
 // ---------------------------------------------------------------------------------------------------------
 // min / max of finite doubles as one compare + select (fmin / fmax also order NaNs and signed zeros, which costs
 // several more instructions; here a zero of either sign leads to the same branch and the same values)
-__device__ __forceinline__ double dmax0(double x) { return x > 0.0 ? x : 0.0; }
-__device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
-__device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
+template <typename T> __device__ __forceinline__ T dmax0(T x) { return x > T(0.0) ? x : T(0.0); }
+template <typename T> __device__ __forceinline__ T dmin2(T a, T b) { return a < b ? a : b; }
+template <typename T> __device__ __forceinline__ T dmax2(T a, T b) { return a > b ? a : b; }
 
-__device__ __forceinline__ EdgeFlux riemann_nt(double g, double hL, double unL, double utL, double zL,
-                                               double hR, double unR, double utR, double zR) {
-  EdgeFlux o;
-  const double dz = zR - zL;
-  const double hsL = dmax0(hL - dmax0(dz));
-  const double hsR = dmax0(hR - dmax0(-dz));
-  if (hsL == 0.0 && hsR == 0.0) {
-    o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
+template <typename T>
+__device__ __forceinline__ EdgeFluxT<T> riemann_nt(T g, T hL, T unL, T utL, T zL,
+                                               T hR, T unR, T utR, T zR) {
+  EdgeFluxT<T> o;
+  const T dz = zR - zL;
+  const T hsL = dmax0(hL - dmax0(dz));
+  const T hsR = dmax0(hR - dmax0(-dz));
+  if (hsL == T(0.0) && hsR == T(0.0)) {
+    o.F1 = T(0.0); o.F3 = T(0.0); o.GL = T(0.0); o.GR = T(0.0);
     return o;
   }
-  const double cL = sqrt(g * hsL), cR = sqrt(g * hsR);
-  double SL, SR;
-  if (hsL > 0.0 && hsR > 0.0) {
-    const double us = 0.5 * (unL + unR) + (cL - cR);
-    const double cs = 0.5 * (cL + cR) + 0.25 * (unL - unR);
+  const T cL = sqrt(g * hsL), cR = sqrt(g * hsR);
+  T SL, SR;
+  if (hsL > T(0.0) && hsR > T(0.0)) {
+    const T us = T(0.5) * (unL + unR) + (cL - cR);
+    const T cs = T(0.5) * (cL + cR) + T(0.25) * (unL - unR);
     SL = dmin2(unL - cL, us - cs);
     SR = dmax2(unR + cR, us + cs);
-  } else if (hsR == 0.0) {
+  } else if (hsR == T(0.0)) {
     SL = unL - cL;
-    SR = unL + 2.0 * cL;
+    SR = unL + T(2.0) * cL;
   } else {
-    SL = unR - 2.0 * cR;
+    SL = unR - T(2.0) * cR;
     SR = unR + cR;
   }
-  const double qsL = hsL * unL, qsR = hsR * unR;
-  const double pL = (0.5 * g) * (hsL * hsL), pR = (0.5 * g) * (hsR * hsR);
-  const double FL2 = qsL * unL + pL, FR2 = qsR * unR + pR;
-  double F1, F2;
-  if (SL >= 0.0) {
+  const T qsL = hsL * unL, qsR = hsR * unR;
+  const T pL = (T(0.5) * g) * (hsL * hsL), pR = (T(0.5) * g) * (hsR * hsR);
+  const T FL2 = qsL * unL + pL, FR2 = qsR * unR + pR;
+  T F1, F2;
+  if (SL >= T(0.0)) {
     F1 = qsL; F2 = FL2;
-  } else if (SR <= 0.0) {
+  } else if (SR <= T(0.0)) {
     F1 = qsR; F2 = FR2;
   } else {
-    const double inv = 1.0 / (SR - SL);
+    const T inv = T(1.0) / (SR - SL);
     F1 = qsL + (SL * (SR * (hsR - hsL) - (qsR - qsL))) * inv;
     F2 = FL2 + (SL * (SR * (qsR - qsL) - (FR2 - FL2))) * inv;
   }
   o.F1 = F1;
-  o.F3 = F1 * (F1 >= 0.0 ? utL : utR);
+  o.F3 = F1 * (F1 >= T(0.0) ? utL : utR);
   o.GL = F2 - pL;
   o.GR = F2 - pR;
   return o;
 }
 
-__device__ __forceinline__ double pow53(double h) {  // h^(5/3), Strickler conveyance (Table 1)
-  const double c3 = cbrt_rn(h);
+template <typename T>
+__device__ __forceinline__ T pow53(T h) {  // h^(5/3), Strickler conveyance (Table 1)
+  const T c3 = cbrt_rn(h);
   return (h * c3) * c3;
 }
 
-__device__ __forceinline__ double k_weight(double k) { return isfinite(k) ? k : 1.0; }
+template <typename T> __device__ __forceinline__ T k_weight(T k) { return isfinite(k) ? k : T(1.0); }
 
 // S1b, boundary edge (only the L side exists).  P:332 wall; P:342 zero-gradient, inflow hydrograph, uniform outflow.
 // code: -1 wall, -2 transmissive; s: the boundary string the edge belongs to (nullptr if none); kL = k_str of cell L
 // is read only for string edges.
-__device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const BoundaryString *__restrict__ s,
-                                                  const double *__restrict__ kst, int L, double nx, double ny,
-                                                  double len, double he, double z, double u, double v) {
-  EdgeFlux o;
-  o.F1 = 0.0; o.F3 = 0.0; o.GL = 0.0; o.GR = 0.0;
+template <typename T>
+__device__ __forceinline__ EdgeFluxT<T> boundary_flux(T g, int code, const BoundaryString *__restrict__ s,
+                                                  const T *__restrict__ kst, int L, T nx, T ny,
+                                                  T len, T he, T z, T u, T v) {
+  EdgeFluxT<T> o;
+  o.F1 = T(0.0); o.F3 = T(0.0); o.GL = T(0.0); o.GR = T(0.0);
   const int type = s ? s->type : 0;
   if (code == kEdgeTransmissive) {            // R-10: ghost = copy of the interior state
-    const double un = u * nx + v * ny, ut = v * nx - u * ny;
+    const T un = u * nx + v * ny, ut = v * nx - u * ny;
     o = riemann_nt(g, he, un, ut, z, he, un, ut, z);
-    o.GR = 0.0;
+    o.GR = T(0.0);
   } else if (type == kBcInflowQ) {            // R-11: Q(t) distributed by conveyance l k h^(5/3)
-    double qe;
-    if (s->sumK > 0.0) {
-      const double Ke = (len * k_weight(kst[L])) * pow53(he);
-      qe = ((s->Q * Ke) / s->sumK) / len;
+    T qe;
+    if ((T)s->sumK > T(0.0)) {
+      const T Ke = (len * k_weight(kst[L])) * pow53(he);
+      qe = (((T)s->Q * Ke) / (T)s->sumK) / len;
     } else {
-      qe = s->Q / s->sumL;
+      qe = (T)s->Q / (T)s->sumL;
     }
     o.F1 = -qe;
-    o.GL = (he > 0.0) ? (qe * qe) / he : 0.0;
+    o.GL = (he > T(0.0)) ? (qe * qe) / he : T(0.0);
   } else if (type == kBcOutflowUniform) {     // R-12: normal depth, q_n = k h^(5/3) sqrt(S0)
-    if (he > 0.0) {
-      const double qn = (k_weight(kst[L]) * pow53(he)) * sqrt(s->S0);
-      const double ut = v * nx - u * ny;
+    if (he > T(0.0)) {
+      const T qn = (k_weight(kst[L]) * pow53(he)) * sqrt((T)s->S0);
+      const T ut = v * nx - u * ny;
       o.F1 = qn;
       o.GL = (qn * qn) / he;
       o.F3 = qn * ut;
     }
   } else {                                    // R-9: reflective wall, closed form of the mirror-ghost problem
-    if (he > 0.0) {
-      const double un = u * nx + v * ny;
-      const double cel = sqrt(g * he);
-      const double S = dmax2(cel - un, cel + 0.5 * un);
+    if (he > T(0.0)) {
+      const T un = u * nx + v * ny;
+      const T cel = sqrt(g * he);
+      const T S = dmax2(cel - un, cel + T(0.5) * un);
       o.GL = (he * un) * (un + S);
     }
   }
@@ -134,49 +137,53 @@ __device__ __forceinline__ EdgeFlux boundary_flux(double g, int code, const Boun
 // S1: one thread per edge.  Reads one EdgeGeom record (coalesced 256-bit), gathers the two CellRec records
 // (one sector each), writes one EdgeFlux record (coalesced 256-bit).
 // ---------------------------------------------------------------------------------------------------------
-template <bool kScalars>
+// R of an edge: inside the fp64 geometry record; a separate array beside the 16-byte fp32 record
+__device__ __forceinline__ int edge_R(const EdgeGeomT<double> &eg, const int32_t *, int) { return eg.R; }
+__device__ __forceinline__ int edge_R(const EdgeGeomT<float> &, const int32_t *__restrict__ geomR, int e) { return geomR[e]; }
+
+template <bool kScalars, typename T>
 __device__ __forceinline__ void
-edge_process(const Control *__restrict__ ctl, double g, double h_dry, int e, const EdgeGeom &eg, const CellRec &a,
-             const CellRec &b, const CellRec *__restrict__ rec, const double *__restrict__ kst,
-             const BoundaryString *__restrict__ strings, EdgeFlux *__restrict__ flux, const Scalars &sc,
-             const double *__restrict__ area, uint8_t *__restrict__ drain_flag, double (&vel)[4]) {
-  double uL = 0.0, vL = 0.0;
+edge_process(const Control *__restrict__ ctl, T g, T h_dry, int e, const EdgeGeomT<T> &eg, const int egR, const CellRecT<T> &a,
+             const CellRecT<T> &b, const CellRecT<T> *__restrict__ rec, const T *__restrict__ kst,
+             const BoundaryString *__restrict__ strings, EdgeFluxT<T> *__restrict__ flux, const Scalars &sc,
+             const T *__restrict__ area, uint8_t *__restrict__ drain_flag, T (&vel)[4]) {
+  T uL = T(0.0), vL = T(0.0);
   if (a.h > h_dry) { uL = a.qx / a.h; vL = a.qy / a.h; }   // R-8: thin films carry no momentum
-  vel[0] = uL; vel[1] = vL; vel[2] = 0.0; vel[3] = 0.0;    // handed to the sediment flux of the <kMorph> instance
-  EdgeFlux o;
-  if (eg.R >= 0) {
-    double uR = 0.0, vR = 0.0;
+  vel[0] = uL; vel[1] = vL; vel[2] = T(0.0); vel[3] = T(0.0);    // handed to the sediment flux of the <kMorph> instance
+  EdgeFluxT<T> o;
+  if (egR >= 0) {
+    T uR = T(0.0), vR = T(0.0);
     if (b.h > h_dry) { uR = b.qx / b.h; vR = b.qy / b.h; }
     vel[2] = uR; vel[3] = vR;
-    const double unL = uL * eg.nx + vL * eg.ny, utL = vL * eg.nx - uL * eg.ny;
-    const double unR = uR * eg.nx + vR * eg.ny, utR = vR * eg.nx - uR * eg.ny;
+    const T unL = uL * eg.nx + vL * eg.ny, utL = vL * eg.nx - uL * eg.ny;
+    const T unR = uR * eg.nx + vR * eg.ny, utR = vR * eg.nx - uR * eg.ny;
     o = riemann_nt(g, a.h, unL, utL, a.z, b.h, unR, utR, b.z);
   } else {
-    const BoundaryString *bs = (eg.R <= -3 && (-3 - eg.R) < ctl->n_strings) ? strings + (-3 - eg.R) : nullptr;
-    o = boundary_flux(g, eg.R, bs, kst, eg.L, eg.nx, eg.ny, eg.len, a.h, a.z, uL, vL);
+    const BoundaryString *bs = (egR <= -3 && (-3 - egR) < ctl->n_strings) ? strings + (-3 - egR) : nullptr;
+    o = boundary_flux(g, egR, bs, kst, eg.L, eg.nx, eg.ny, eg.len, a.h, a.z, uL, vL);
   }
   flux[e] = o;
   // S1c, lazily (R-8b): theta_i < 1 needs dt * (o_0 + o_1 + o_2) > h_i |Omega_i|, hence at least one outgoing edge with
   // dt * o_k > 0.3 h_i |Omega_i| (0.3 * 3 * (1 + rounding) < 1).  Only such donor cells are flagged; k_theta_lazy evaluates
   // theta exactly for them and every other cell keeps theta = 1 without being visited.
   if (drain_flag) {
-    const int d = o.F1 > 0.0 ? eg.L : ((o.F1 < 0.0 && eg.R >= 0) ? eg.R : -1);
+    const int d = o.F1 > T(0.0) ? eg.L : ((o.F1 < T(0.0) && egR >= 0) ? egR : -1);
     if (d >= 0) {
-      const double hd = (d == eg.L) ? a.h : b.h;
-      if (ctl->dt * (eg.len * fabs(o.F1)) > 0.3 * (hd * area[d])) drain_flag[d] = 1;
+      const T hd = (d == eg.L) ? a.h : b.h;
+      if ((T)ctl->dt * (eg.len * fabs(o.F1)) > T(0.3) * (hd * area[d])) drain_flag[d] = 1;
     }
   }
   // passive scalars (Eq. 8 / Eq. 20 advective part, R-19): concentration on the upwind side of the contact wave
   if (kScalars)
   _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
-    const double phiL = a.h > 0.0 ? sc.qa[sp][eg.L] / a.h : 0.0;
-    double phiR = phiL;
-    if (eg.R >= 0) {
-      phiR = b.h > 0.0 ? sc.qa[sp][eg.R] / b.h : 0.0;
-    } else if (eg.R <= -3 && (-3 - eg.R) < ctl->n_strings && strings[-3 - eg.R].type == kBcInflowQ) {
-      phiR = strings[-3 - eg.R].phi_in[sp];
+    const T phiL = a.h > T(0.0) ? sc.qa[sp][eg.L] / a.h : T(0.0);
+    T phiR = phiL;
+    if (egR >= 0) {
+      phiR = b.h > T(0.0) ? sc.qa[sp][egR] / b.h : T(0.0);
+    } else if (egR <= -3 && (-3 - egR) < ctl->n_strings && strings[-3 - egR].type == kBcInflowQ) {
+      phiR = strings[-3 - egR].phi_in[sp];
     }
-    sc.phi_up[sp][e] = o.F1 >= 0.0 ? phiL : phiR;
+    sc.phi_up[sp][e] = o.F1 >= T(0.0) ? phiL : phiR;
   }
 }
 
@@ -215,55 +222,67 @@ __device__ __forceinline__ SedState sed_state(const Morph &mp, double g, double 
 // q_Bij of edge e from the two cell records of t^n: nothing where a side is dry or at a wall; through open boundaries
 // the interior cell's own flux (equilibrium boundary)
 // vel = (u, v) of L and R as edge_process formed them (q / h where h > h_dry): the same quotients the oracle forms
-__device__ __forceinline__ double sediment_edge(const Morph &mp, double g, double h_dry, const EdgeGeom &eg,
-                                                const CellRec &a, const CellRec &b, const double (&vel)[4]) {
-  if (!(a.h > h_dry) || eg.R == -1) return 0.0;
-  const double2 fcL = mp.formula == 2 ? mp.cell[eg.L] : make_double2(0.0, 0.0);
-  const SedState si = sed_state(mp, g, a.h, vel[0], vel[1], fcL, eg.nx, eg.ny);
-  if (eg.R < 0) return si.q;
-  if (!(b.h > h_dry)) return 0.0;
-  const double2 fcR = mp.formula == 2 ? mp.cell[eg.R] : make_double2(0.0, 0.0);
-  const SedState sj = sed_state(mp, g, b.h, vel[2], vel[3], fcR, eg.nx, eg.ny);
+// (R: >= 0 interior edge, < 0 boundary code; fcL / fcR: (g / k_st^2, cbrt(h)) of the two cells, MPM-like law only)
+__device__ __forceinline__ double sediment_flux_core(const Morph &mp, double g, double h_dry, int R, double nx, double ny,
+                                                     double hL, double uL, double vL, double zL, double2 fcL,
+                                                     double hR, double uR, double vR, double zR, double2 fcR) {
+  if (!(hL > h_dry) || R == -1) return 0.0;
+  const SedState si = sed_state(mp, g, hL, uL, vL, fcL, nx, ny);
+  if (R < 0) return si.q;
+  if (!(hR > h_dry)) return 0.0;
+  const SedState sj = sed_state(mp, g, hR, uR, vR, fcR, nx, ny);
   const double sm = dmin2(si.l1, sj.l1), sp = dmax2(si.l2, sj.l2);        // Eq. 15
   if (!(sp - sm > 0.0)) return 0.0;
-  return ((sp * si.q - sm * sj.q) + (sp * sm) * (b.z - a.z)) / (sp - sm);  // Eq. 14
+  return ((sp * si.q - sm * sj.q) + (sp * sm) * (zR - zL)) / (sp - sm);    // Eq. 14
+}
+
+__device__ __forceinline__ double sediment_edge(const Morph &mp, double g, double h_dry, const EdgeGeom &eg,
+                                                const CellRec &a, const CellRec &b, const double (&vel)[4]) {
+  const double2 zero = make_double2(0.0, 0.0);
+  const double2 fcL = (mp.formula == 2 && a.h > h_dry && eg.R != -1) ? mp.cell[eg.L] : zero;
+  const double2 fcR = (mp.formula == 2 && a.h > h_dry && eg.R >= 0 && b.h > h_dry) ? mp.cell[eg.R] : zero;
+  return sediment_flux_core(mp, g, h_dry, eg.R, eg.nx, eg.ny, a.h, vel[0], vel[1], a.z, fcL, b.h, vel[2], vel[3], b.z, fcR);
 }
 
 // kPersistent = false: one edge per thread.  kPersistent = true: a grid of resident blocks strides over the edges and
 // the (streamed) geometry record of a thread's next edge is loaded while the current edge is worked on, so that the
 // geom -> cell record gather chain of an edge pays one memory latency instead of two (profiles/r1f: the kernel's
 // stalls are exactly these two loads).
-template <bool kScalars, bool kPersistent, bool kMorph = false>
+template <bool kScalars, bool kPersistent, bool kMorph = false, typename T = double>
 __global__ void __launch_bounds__(kBlock, kMorph ? 3 : 0)
-k_edge_flux(const Control *__restrict__ ctl, const EdgeGeom *__restrict__ geom, const CellRec *__restrict__ rec,
-            const double *__restrict__ kst, const BoundaryString *__restrict__ strings,
-            EdgeFlux *__restrict__ flux, int n_edges, int force, const Scalars sc,
-            const double *__restrict__ area, uint8_t *__restrict__ drain_flag, const Morph mp = Morph{}) {
+k_edge_flux(const Control *__restrict__ ctl, const EdgeGeomT<T> *__restrict__ geom, const CellRecT<T> *__restrict__ rec,
+            const T *__restrict__ kst, const BoundaryString *__restrict__ strings,
+            EdgeFluxT<T> *__restrict__ flux, int n_edges, int force, const Scalars sc,
+            const T *__restrict__ area, uint8_t *__restrict__ drain_flag, const Morph mp = Morph{},
+            const int32_t *__restrict__ geomR = nullptr) {
   if (!ctl->active && !force) return;
-  const double g = ctl->g, h_dry = ctl->h_dry;
+  const T g = (T)ctl->g, h_dry = (T)ctl->h_dry;
   int e = blockIdx.x * kBlock + threadIdx.x;
   if (e >= n_edges) return;
   if (!kPersistent) {
-    const EdgeGeom eg = geom[e];
-    const CellRec a = rec[eg.L];
-    CellRec b = a;
-    if (eg.R >= 0) b = rec[eg.R];
-    double vel[4];
-    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
-    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
+    const EdgeGeomT<T> eg = geom[e];
+    const int R = edge_R(eg, geomR, e);
+    const CellRecT<T> a = rec[eg.L];
+    CellRecT<T> b = a;
+    if (R >= 0) b = rec[R];
+    T vel[4];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, R, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
+    if constexpr (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
     return;
   }
   const int stride = gridDim.x * kBlock;
-  EdgeGeom eg_next = geom[e];
+  EdgeGeomT<T> eg_next = geom[e];
+  int R_next = edge_R(eg_next, geomR, e);
   for (; e < n_edges; e += stride) {
-    const EdgeGeom eg = eg_next;
-    const CellRec a = rec[eg.L];
-    CellRec b = a;
-    if (eg.R >= 0) b = rec[eg.R];
-    if (e + stride < n_edges) eg_next = geom[e + stride];
-    double vel[4];
-    edge_process<kScalars>(ctl, g, h_dry, e, eg, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
-    if (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
+    const EdgeGeomT<T> eg = eg_next;
+    const int R = R_next;
+    const CellRecT<T> a = rec[eg.L];
+    CellRecT<T> b = a;
+    if (R >= 0) b = rec[R];
+    if (e + stride < n_edges) { eg_next = geom[e + stride]; R_next = edge_R(eg_next, geomR, e + stride); }
+    T vel[4];
+    edge_process<kScalars>(ctl, g, h_dry, e, eg, R, a, b, rec, kst, strings, flux, sc, area, drain_flag, vel);
+    if constexpr (kMorph) mp.qB[e] = sediment_edge(mp, g, h_dry, eg, a, b, vel);
   }
 }
 
@@ -297,10 +316,11 @@ k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, con
 // records of its own outgoing edges in place -- every edge has exactly one donor, so no two cells touch one record,
 // and a neighbour that reads the same record for its own theta sees it as an inflow (o_k = 0) before and after.
 // flag bits: 1 = flagged by k_edge_flux in this step, 2 = theta[i] holds a value < 1 from an earlier step.
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
-k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
-             EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
-             double *__restrict__ theta, uint8_t *__restrict__ drain_flag, int n_cells) {
+k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeomT<T> *__restrict__ geom,
+             EdgeFluxT<T> *__restrict__ flux, const CellRecT<T> *__restrict__ rec, const T *__restrict__ area,
+             T *__restrict__ theta, uint8_t *__restrict__ drain_flag, int n_cells) {
   if (!ctl->active) return;
   // four flag bytes per thread: almost every word is 0 and the thread leaves after one 4-byte load
   const int i4 = (blockIdx.x * kBlock + threadIdx.x) * 4;
@@ -311,35 +331,35 @@ k_theta_lazy(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge
   const int i = i4 + j;
   const uint8_t fl = (uint8_t)(f4 >> (8 * j));
   if (fl == 0 || i >= n_cells) continue;
-  double th = 1.0;
+  T th = T(1.0);
   if (fl & 1) {
-    const double dt = ctl->dt;
+    const T dt = (T)ctl->dt;
     const int4 ce = cell_edge[i];
     const int es[3] = {ce.x, ce.y, ce.z};
-    double o[3];
+    T o[3];
     bool isL[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      const EdgeGeom eg = geom[es[k]];
+      const EdgeGeomT<T> eg = geom[es[k]];
       isL[k] = (eg.L == i);
-      const double sM = (isL[k] ? 1.0 : -1.0) * (eg.len * flux[es[k]].F1);
+      const T sM = (isL[k] ? T(1.0) : -T(1.0)) * (eg.len * flux[es[k]].F1);
       o[k] = dmax0(sM);
     }
-    const double out = ((o[0] + o[1]) + o[2]);
-    const double avail = rec[i].h * area[i];
+    const T out = ((o[0] + o[1]) + o[2]);
+    const T avail = rec[i].h * area[i];
     if (dt * out > avail) th = avail / (dt * out);
-    if (th < 1.0) {
+    if (th < T(1.0)) {
 #pragma unroll
       for (int k = 0; k < 3; ++k)
-        if (o[k] > 0.0) {
-          EdgeFlux f = flux[es[k]];
+        if (o[k] > T(0.0)) {
+          EdgeFluxT<T> f = flux[es[k]];
           f.F1 = th * f.F1; f.F3 = th * f.F3; f.GL = th * f.GL; f.GR = th * f.GR;
           flux[es[k]] = f;
         }
     }
   }
   theta[i] = th;
-  drain_flag[i] = th < 1.0 ? 2 : 0;
+  drain_flag[i] = th < T(1.0) ? 2 : 0;
   }
 }
 
@@ -367,15 +387,16 @@ __device__ __forceinline__ void block_max_to_global(double r, unsigned long long
 }
 
 // Eq. 21 (R-7) for one cell: max_j lambda_ij / rho_ij with rho_ij = 4|Omega_i| / (3 l_ij)
-__device__ __forceinline__ double cell_rate(double g, double h, double qx, double qy, double invA,
-                                            const double nx[3], const double ny[3], const double len[3]) {
-  const double u = qx / h, v = qy / h;
-  const double cel = sqrt(g * h);
-  double r = 0.0;
+template <typename T>
+__device__ __forceinline__ T cell_rate(T g, T h, T qx, T qy, T invA,
+                                            const T nx[3], const T ny[3], const T len[3]) {
+  const T u = qx / h, v = qy / h;
+  const T cel = sqrt(g * h);
+  T r = T(0.0);
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    const double lam = fabs(u * nx[k] + v * ny[k]) + cel;
-    const double val = lam * ((0.75 * len[k]) * invA);
+    const T lam = fabs(u * nx[k] + v * ny[k]) + cel;
+    const T val = lam * ((T(0.75) * len[k]) * invA);
     if (val > r) r = val;
   }
   return r;
@@ -384,129 +405,131 @@ __device__ __forceinline__ double cell_rate(double g, double h, double qx, doubl
 // ---------------------------------------------------------------------------------------------------------
 // S2 + S3, and S0 of the NEXT step fused in: one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
-template <bool kScalars, bool kMorph = false>
+template <bool kScalars, bool kMorph = false, typename T = double>
 __global__ void __launch_bounds__(kBlock, (kScalars || kMorph) ? 3 : 4)      // 4 blocks/SM = 64 registers: measured faster than 3
-k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
-              const EdgeFlux *__restrict__ flux, const double *__restrict__ theta,
-              const double *__restrict__ area, const double *__restrict__ inv_area,
-              const double *__restrict__ gn2, CellRec *__restrict__ rec, int n_cells, const Scalars sc,
+k_cell_update(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeomT<T> *__restrict__ geom,
+              const EdgeFluxT<T> *__restrict__ flux, const T *__restrict__ theta,
+              const T *__restrict__ area, const T *__restrict__ inv_area,
+              const T *__restrict__ gn2, CellRecT<T> *__restrict__ rec, int n_cells, const Scalars sc,
               const Morph mp = Morph{}) {
   if (!ctl->active) return;
   // a grid of resident blocks strides over the cells; the (streamed) slot record of a thread's next cell is loaded
   // while the current cell is worked on: its cell_edge -> (geometry, flux) gather chain pays one latency, not two
-  double rate = 0.0;
+  T rate = T(0.0);
   const int stride = gridDim.x * kBlock;
   int i = blockIdx.x * kBlock + threadIdx.x;
   int4 ce_next = make_int4(0, 0, 0, 0);
   if (i < n_cells) ce_next = cell_edge[i];
-  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+  const T dt = (T)ctl->dt, g = (T)ctl->g, h_dry = (T)ctl->h_dry;
   for (; i < n_cells; i += stride) {
     const int4 ce = ce_next;
     if (i + stride < n_cells) ce_next = cell_edge[i + stride];
     const int es[3] = {ce.x, ce.y, ce.z};
-    double nx[3], ny[3], len[3];
-    double dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3], dBk[3];
+    T nx[3], ny[3], len[3];
+    T dHk[3], dXk[3], dYk[3], sgn[3], F1lim[3], dBk[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      const EdgeGeom eg = geom[es[k]];
-      EdgeFlux f = flux[es[k]];
+      const EdgeGeomT<T> eg = geom[es[k]];
+      EdgeFluxT<T> f = flux[es[k]];
       const bool isL = (eg.L == i);
       // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
-      double G = isL ? f.GL : f.GR;
-      if (theta) {                                   // eager variant; nullptr: k_theta_lazy has limited the records
-        double th = 1.0;
-        if (f.F1 > 0.0) th = theta[eg.L];
-        else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];
-        if (th < 1.0) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
+      T G = isL ? f.GL : f.GR;
+      if constexpr (sizeof(T) == 8) if (theta) {     // eager variant (fp64 inspection only); nullptr: k_theta_lazy has limited the records
+        T th = T(1.0);
+        if (f.F1 > T(0.0)) th = theta[eg.L];
+        else if (f.F1 < T(0.0) && eg.R >= 0) th = theta[eg.R];
+        if (th < T(1.0)) { f.F1 = th * f.F1; f.F3 = th * f.F3; G = th * G; }
       }
-      const double s = isL ? 1.0 : -1.0;
+      const T s = isL ? T(1.0) : -T(1.0);
       nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
       if (kScalars) { sgn[k] = s; F1lim[k] = f.F1; }
-      if (kMorph) dBk[k] = s * (eg.len * mp.qB[es[k]]);
+      if constexpr (kMorph) dBk[k] = s * (eg.len * mp.qB[es[k]]);
       dHk[k] = s * (eg.len * f.F1);
       dXk[k] = s * (eg.len * (G * eg.nx - f.F3 * eg.ny));
       dYk[k] = s * (eg.len * (G * eg.ny + f.F3 * eg.nx));
     }
-    const double dH = ((dHk[0] + dHk[1]) + dHk[2]);
-    const double dX = ((dXk[0] + dXk[1]) + dXk[2]);
-    const double dY = ((dYk[0] + dYk[1]) + dYk[2]);
-    CellRec c = rec[i];
-    const double invA = inv_area[i];
-    const double a = dt * invA;
-    double hn = c.h - a * dH;
-    if (hn < 0.0) {                                  // residual negatives (R-8b): clip and count
-      atomicAdd(&ctl->vol_clipped, -hn * area[i]);
-      hn = 0.0;
+    const T dH = ((dHk[0] + dHk[1]) + dHk[2]);
+    const T dX = ((dXk[0] + dXk[1]) + dXk[2]);
+    const T dY = ((dYk[0] + dYk[1]) + dYk[2]);
+    CellRecT<T> c = rec[i];
+    const T invA = inv_area[i];
+    const T a = dt * invA;
+    T hn = c.h - a * dH;
+    if (hn < T(0.0)) {                                  // residual negatives (R-8b): clip and count
+      atomicAdd(&ctl->vol_clipped, (double)(-hn * area[i]));
+      hn = T(0.0);
     }
-    double qxn = 0.0, qyn = 0.0;
-    double2 fc = make_double2(0.0, 0.0);             // <kMorph>, MPM-like law: (g/k^2, cbrt(h^{n+1})) for the next step's edges
+    T qxn = T(0.0), qyn = T(0.0);
+    double2 fc = make_double2(T(0.0), T(0.0));             // <kMorph>, MPM-like law: (g/k^2, cbrt(h^{n+1})) for the next step's edges
     if (hn > h_dry) {
       qxn = c.qx - a * dX;
       qyn = c.qy - a * dY;
-      const double f2 = gn2[i];
-      if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
-        const double cb = cbrt_rn(hn);
-        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cb);
+      const T f2 = gn2[i];
+      if (f2 > T(0.0)) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
+        const T cb = cbrt_rn(hn);
+        const T D = T(1.0) + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cb);
         qxn = qxn / D;
         qyn = qyn / D;
         fc = make_double2(f2, cb);
       }
-      const double r = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
+      const T r = cell_rate(g, hn, qxn, qyn, invA, nx, ny, len);
       if (r > rate) rate = r;
     }
     c.h = hn; c.qx = qxn; c.qy = qyn;
-    if (kMorph) {                                    // Eq. 13, S_b = 0: the bed rides in the same record
+    if constexpr (kMorph) {                          // Eq. 13, S_b = 0: the bed rides in the same record
       c.z = c.z - mp.inv1mp * (a * ((dBk[0] + dBk[1]) + dBk[2]));
       if (mp.formula == 2) mp.cell[i] = fc;
     }
     rec[i] = c;
     if (kScalars)                                    // Eq. 20, advective part: same gather, same slot order (R-19)
     _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < sc.n) {
-      double Ck[3];
+      T Ck[3];
 #pragma unroll
       for (int k = 0; k < 3; ++k) Ck[k] = sgn[k] * (len[k] * (F1lim[k] * sc.phi_up[sp][es[k]]));
-      const double dC = ((Ck[0] + Ck[1]) + Ck[2]);
+      const T dC = ((Ck[0] + Ck[1]) + Ck[2]);
       sc.qa[sp][i] = sc.qa[sp][i] - a * dC;
     }
   }
-  block_max_to_global(rate, &ctl->rate_bits);
+  block_max_to_global((double)rate, &ctl->rate_bits);
 }
 
 // Eq. 21 on the current state (after swe_set_state): same arithmetic as the fused part of k_cell_update
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
-k_rate(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
-       const double *__restrict__ inv_area, const CellRec *rec_a, const CellRec *rec_b, int n_cells) {
-  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
+k_rate(Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeomT<T> *__restrict__ geom,
+       const T *__restrict__ inv_area, const CellRecT<T> *rec_a, const CellRecT<T> *rec_b, int n_cells) {
+  const CellRecT<T> *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
-  double rate = 0.0;
+  T rate = T(0.0);
   if (i < n_cells) {
-    const CellRec c = rec[i];
-    if (c.h > ctl->h_dry) {
+    const CellRecT<T> c = rec[i];
+    if (c.h > (T)ctl->h_dry) {
       const int4 ce = cell_edge[i];
       const int es[3] = {ce.x, ce.y, ce.z};
-      double nx[3], ny[3], len[3];
+      T nx[3], ny[3], len[3];
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
-        const EdgeGeom eg = geom[es[k]];
+        const EdgeGeomT<T> eg = geom[es[k]];
         nx[k] = eg.nx; ny[k] = eg.ny; len[k] = eg.len;
       }
-      rate = cell_rate(ctl->g, c.h, c.qx, c.qy, inv_area[i], nx, ny, len);
+      rate = cell_rate((T)ctl->g, c.h, c.qx, c.qy, inv_area[i], nx, ny, len);
     }
   }
-  block_max_to_global(rate, &ctl->rate_bits);
+  block_max_to_global((double)rate, &ctl->rate_bits);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // Step control: one block.  Fixed-shape pairwise tree in string order (R-11): pad to a power of two with zeros,
 // add neighbours at stride 1, 2, 4, ... -- the same pairs whatever the thread count, hence bit-reproducible.
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double block_tree_sum(double *v, int pow2) {
+template <typename T>
+__device__ __forceinline__ T block_tree_sum(T *v, int pow2) {
   for (int s = 1; s < pow2; s <<= 1) {
     __syncthreads();
     for (int j = threadIdx.x; 2 * s * j + s < pow2; j += blockDim.x) v[2 * s * j] = v[2 * s * j] + v[2 * s * j + s];
   }
   __syncthreads();
-  const double sum = v[0];
+  const T sum = v[0];
   __syncthreads();                    // v may be refilled by the caller right away
   return sum;
 }
@@ -526,13 +549,16 @@ __device__ __forceinline__ double hydrograph(const double *p, int n_params, doub
 // accumulators of k_info).
 constexpr int kCtlPre = 4;            // boundary strings whose members k_step_control gathers up front (one per thread)
 
+template <typename T = double>
 __global__ void __launch_bounds__(kCtlThreads, 1)
-k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ string_edges, double *scratch,
-               const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
-               const double *__restrict__ theta, const CellRec *rec_a, const CellRec *rec_b,
-               const double *__restrict__ kst, const double *__restrict__ string_M, int mode) {
+k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ string_edges, double *scratch_,
+               const EdgeGeomT<T> *__restrict__ geom, const EdgeFluxT<T> *__restrict__ flux,
+               const T *__restrict__ theta, const CellRecT<T> *rec_a, const CellRecT<T> *rec_b,
+               const T *__restrict__ kst, const double *__restrict__ string_M, int mode) {
+  // T: the precision of the state; the string sums run in T (fixed-shape trees, R-11), time / dt / volumes in fp64
+  T *scratch = reinterpret_cast<T *>(scratch_);
   // the pairwise trees run in shared memory when the string fits (same pairs, same order as in global scratch)
-  __shared__ double s_tree[kTreeCap];
+  __shared__ T s_tree[kTreeCap];
   __shared__ double s_Q[kCtlPre];
   __shared__ int s_active;
   __shared__ double s_t_old;
@@ -551,28 +577,28 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
     c_tend = ctl->t_end; c_cfl = ctl->cfl; c_dtmax = ctl->dt_max; c_left = ctl->steps_left; c_done = ctl->steps_done;
     c_flags = ctl->flags; c_pp = ctl->ping_pong; c_rate = ctl->rate_bits;
   }
-  const CellRec *__restrict__ rec = cur ? rec_b : rec_a;
-  auto term_out = [&](const BoundaryString &bs, int j) -> double {   // l * (limited F1) of member j (bookkeeping)
-    if (string_M) return string_M[bs.first + j];         // fused patch step: written by the owning patch
+  const CellRecT<T> *__restrict__ rec = cur ? rec_b : rec_a;
+  auto term_out = [&](const BoundaryString &bs, int j) -> T {   // l * (limited F1) of member j (bookkeeping)
+    if (string_M) return (T)string_M[bs.first + j];         // fused patch step: written by the owning patch
     const int e = string_edges[bs.first + j];
-    const EdgeGeom eg = geom[e];
-    double F1 = flux[e].F1;
-    if (theta && F1 > 0.0) {                              // nullptr: the records are limited already (k_theta_lazy)
-      const double th = theta[eg.L];
-      if (th < 1.0) F1 = th * F1;
+    const EdgeGeomT<T> eg = geom[e];
+    T F1 = flux[e].F1;
+    if (theta && F1 > T(0.0)) {                              // nullptr: the records are limited already (k_theta_lazy)
+      const T th = theta[eg.L];
+      if (th < T(1.0)) F1 = th * F1;
     }
     return eg.len * F1;
   };
-  auto term_in = [&](const BoundaryString &bs, int j) -> double {    // conveyance weight of member j (R-11)
+  auto term_in = [&](const BoundaryString &bs, int j) -> T {    // conveyance weight of member j (R-11)
     const int e = string_edges[bs.first + j];
-    const EdgeGeom eg = geom[e];
+    const EdgeGeomT<T> eg = geom[e];
     return (eg.len * k_weight(kst[eg.L])) * pow53(rec[eg.L].h);
   };
   bool fast = ns <= kCtlPre;                             // block-uniform: every thread reads the same descriptors
-  double pre[kCtlPre];
+  T pre[kCtlPre];
 #pragma unroll
   for (int s = 0; s < kCtlPre; ++s) {
-    pre[s] = 0.0;
+    pre[s] = T(0.0);
     if (s < ns) {
       const BoundaryString &bs = strings[s];
       if (bs.pow2 > (int)blockDim.x) fast = false;
@@ -581,26 +607,26 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
         else if (bs.type == kBcInflowQ && mode == 0) pre[s] = term_in(bs, threadIdx.x);
       }
       if (bs.type == kBcInflowQ && mode == 0 && threadIdx.x == blockDim.x - 1 - s)
-        s_Q[s] = hydrograph(bs.params, bs.n_params, t_now);
+        s_Q[s] = (double)(T)hydrograph(bs.params, bs.n_params, t_now);   // Q(t^n) in the precision of the state
     }
   }
   if (fast) {
     // every string's pairwise tree at once, out of registers: xor-free shuffle tree inside each warp (lane 0 ends up
     // with v[i] + v[i+1], then + (v[i+2] + v[i+3]), ...: the same pairs in the same order as block_tree_sum; the
     // padding zeros beyond pow2 add nothing), the warp sums to shared memory, warp s finishes string s.
-    __shared__ double s_part[kCtlPre][32];
-    __shared__ double s_sum[kCtlPre];
+    __shared__ T s_part[kCtlPre][32];
+    __shared__ T s_sum[kCtlPre];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
     for (int s = 0; s < kCtlPre; ++s) {
-      double x = pre[s];
+      T x = pre[s];
 #pragma unroll
       for (int off = 1; off < 32; off <<= 1) x = x + __shfl_down_sync(0xffffffffu, x, off);
       if (lane == 0) s_part[s][wid] = x;
     }
     __syncthreads();
     if (wid < kCtlPre) {
-      double x = (lane < (int)(blockDim.x >> 5)) ? s_part[wid][lane] : 0.0;
+      T x = (lane < (int)(blockDim.x >> 5)) ? s_part[wid][lane] : T(0.0);
 #pragma unroll
       for (int off = 1; off < 32; off <<= 1) x = x + __shfl_down_sync(0xffffffffu, x, off);
       if (lane == 0) s_sum[wid] = x;
@@ -610,7 +636,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
     if (pending)
       for (int s = 0; s < ns; ++s) {
         if (strings[s].type == kBcInflowQ) ctl->vol_in += dt_prev * strings[s].Q;
-        else if (strings[s].type == kBcOutflowUniform) ctl->vol_out += dt_prev * s_sum[s & (kCtlPre - 1)];
+        else if (strings[s].type == kBcOutflowUniform) ctl->vol_out += dt_prev * (double)s_sum[s & (kCtlPre - 1)];
       }
     if (mode == 1) { ctl->pending = 0; ctl->vol = 0.0; ctl->n_wet = 0; ctl->nonfinite = 0; return; }
     int active = 0, new_pending = 0;
@@ -641,7 +667,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
     ctl->active = active;
     if (active)                              // boundary strings at t^n (R-11): Q(t^n) and the conveyance sum
       for (int s = 0; s < ns; ++s)
-        if (strings[s].type == kBcInflowQ) { strings[s].sumK = s_sum[s & (kCtlPre - 1)]; strings[s].Q = s_Q[s & (kCtlPre - 1)]; }
+        if (strings[s].type == kBcInflowQ) { strings[s].sumK = (double)s_sum[s & (kCtlPre - 1)]; strings[s].Q = s_Q[s & (kCtlPre - 1)]; }
     return;
   }
   // ---- general path (more than kCtlPre strings, or a string with more members than the block has threads)
@@ -652,14 +678,14 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
       if (bs.type == kBcInflowQ) {
         if (threadIdx.x == 0) ctl->vol_in += dt_prev * bs.Q;
       } else if (bs.type == kBcOutflowUniform) {
-        double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
+        T *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
         for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
-          double a = 0.0;
+          T a = T(0.0);
           if (j < bs.n_edges) a = term_out(bs, j);
           v[j] = a;
         }
-        const double sum = block_tree_sum(v, bs.pow2);
-        if (threadIdx.x == 0) ctl->vol_out += dt_prev * sum;
+        const T sum = block_tree_sum(v, bs.pow2);
+        if (threadIdx.x == 0) ctl->vol_out += dt_prev * (double)sum;
       }
     }
   }
@@ -705,16 +731,16 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
   for (int s = 0; s < ns; ++s) {
     BoundaryString &bs = strings[s];
     if (bs.type != kBcInflowQ) continue;
-    double *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
+    T *v = bs.pow2 <= kTreeCap ? s_tree : scratch + bs.scratch;
     for (int j = threadIdx.x; j < bs.pow2; j += blockDim.x) {
-      double a = 0.0;
+      T a = T(0.0);
       if (j < bs.n_edges) a = term_in(bs, j);
       v[j] = a;
     }
-    const double sum = block_tree_sum(v, bs.pow2);
+    const T sum = block_tree_sum(v, bs.pow2);
     if (threadIdx.x == 0) {
-      bs.sumK = sum;
-      bs.Q = hydrograph(bs.params, bs.n_params, s_t_old);
+      bs.sumK = (double)sum;
+      bs.Q = (double)(T)hydrograph(bs.params, bs.n_params, s_t_old);
     }
   }
 }
@@ -759,18 +785,19 @@ __global__ void k_reset(Control *ctl, double t0) {
 constexpr int kInfoMaxBlocks = 148 * 8;
 struct InfoPartial { double vol; long long wet; int bad; int pad_; };
 
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
-k_info(Control *__restrict__ ctl, const CellRec *rec_a, const CellRec *rec_b, const double *__restrict__ area,
+k_info(Control *__restrict__ ctl, const CellRecT<T> *rec_a, const CellRecT<T> *rec_b, const T *__restrict__ area,
        int n_cells, InfoPartial *__restrict__ part, unsigned int *__restrict__ ticket) {
-  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
+  const CellRecT<T> *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   double vol = 0.0;
   long long wet = 0;
   int bad = 0;
   const double h_dry = ctl->h_dry;
   for (int i = blockIdx.x * kBlock + threadIdx.x; i < n_cells; i += gridDim.x * kBlock) {
-    const CellRec c = rec[i];
-    vol += c.h * area[i];
-    wet += (c.h > h_dry);
+    const CellRecT<T> c = rec[i];
+    vol += (double)c.h * (double)area[i];
+    wet += (c.h > (T)h_dry);
     bad |= !(isfinite(c.h) && isfinite(c.qx) && isfinite(c.qy));
   }
 #pragma unroll
@@ -804,27 +831,29 @@ k_info(Control *__restrict__ ctl, const CellRec *rec_a, const CellRec *rec_b, co
 }
 
 // caller numbering <-> internal numbering (cell_perm[new] = caller id)
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
 k_pack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *__restrict__ h,
-             const double *__restrict__ hu, const double *__restrict__ hv, CellRec *rec_a, CellRec *rec_b, int n_cells) {
-  CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
+             const double *__restrict__ hu, const double *__restrict__ hv, CellRecT<T> *rec_a, CellRecT<T> *rec_b, int n_cells) {
+  CellRecT<T> *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
   const int o = cell_perm[i];
-  CellRec c = rec[i];
-  c.h = h[o]; c.qx = hu[o]; c.qy = hv[o];
+  CellRecT<T> c = rec[i];
+  c.h = (T)h[o]; c.qx = (T)hu[o]; c.qy = (T)hv[o];      // the caller's arrays are fp64; rounded once when T = float
   rec[i] = c;
 }
 
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
-k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const CellRec *rec_a,
-               const CellRec *rec_b, double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv,
+k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const CellRecT<T> *rec_a,
+               const CellRecT<T> *rec_b, double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv,
                int n_cells) {
-  const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
+  const CellRecT<T> *__restrict__ rec = ctl->cur ? rec_b : rec_a;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
   const int o = cell_perm[i];
-  const CellRec c = rec[i];
+  const CellRecT<T> c = rec[i];
   h[o] = c.h; hu[o] = c.qx; hv[o] = c.qy;
 }
 
@@ -836,6 +865,14 @@ k_sed_cell_init(const Control *__restrict__ ctl, const CellRec *__restrict__ rec
   if (i >= n_cells) return;
   const double h = rec[i].h, f2 = gn2[i];
   cell[i] = (h > ctl->h_dry && f2 > 0.0) ? make_double2(f2, cbrt_rn(h)) : make_double2(0.0, 0.0);
+}
+
+// both record buffers of the fused patch step hold the bed of the newest state (swe_set_morphology)
+__global__ void __launch_bounds__(kBlock)
+k_sync_bed(const Control *__restrict__ ctl, CellRec *rec_a, CellRec *rec_b, int n_cells) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n_cells) return;
+  if (ctl->cur) rec_a[i].z = rec_b[i].z; else rec_b[i].z = rec_a[i].z;
 }
 
 // bed elevation z_B (swe_get_bed), newest state buffer, caller numbering
@@ -877,15 +914,16 @@ k_cbrt(const double *__restrict__ x, double *__restrict__ y, long long n) {
 }
 
 // inspection (swe_get_edge_flux): per-edge records after the limiter, in caller edge numbering
+template <typename T = double>
 __global__ void __launch_bounds__(kBlock)
-k_export_flux(const int *__restrict__ edge_perm, const EdgeGeom *__restrict__ geom, const EdgeFlux *__restrict__ flux,
-              const double *__restrict__ theta, double *__restrict__ F1, double *__restrict__ F3,
+k_export_flux(const int *__restrict__ edge_perm, const EdgeGeomT<T> *__restrict__ geom, const EdgeFluxT<T> *__restrict__ flux,
+              const T *__restrict__ theta, double *__restrict__ F1, double *__restrict__ F3,
               double *__restrict__ GL, double *__restrict__ GR, int n_edges) {
   const int e = blockIdx.x * kBlock + threadIdx.x;
   if (e >= n_edges) return;
-  const EdgeGeom eg = geom[e];
-  EdgeFlux f = flux[e];
-  if (theta) {                                       // nullptr: the records are limited already (k_theta_lazy)
+  const EdgeGeomT<T> eg = geom[e];
+  EdgeFluxT<T> f = flux[e];
+  if constexpr (sizeof(T) == 8) if (theta) {                                       // nullptr: the records are limited already (k_theta_lazy)
     double th = 1.0;
     if (f.F1 > 0.0) th = theta[eg.L];
     else if (f.F1 < 0.0 && eg.R >= 0) th = theta[eg.R];

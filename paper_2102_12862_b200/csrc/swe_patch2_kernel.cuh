@@ -36,19 +36,28 @@ struct Patch2Args {
   double *string_M;               // l * (limited F1) of every boundary-string edge, by position in string_edges[]
   unsigned char *pflag_a, *pflag_b;   // [n_patches][kPflagBytes], one array per state buffer
   int32_t n_cells;
+  // self-controlled step (kSelf): no control kernel runs between two steps
+  int32_t step_k;                 // this launch reads Control::slot[step_k] and writes slot[(step_k + 1) % 4]
+  int32_t n_strings, n_string_edges;
+  const double *string_lk;        // l_e * k_weight(k_st of cell L) of every boundary-string edge (R-11), by position
+  const int32_t *string_cell;     // cell L of every boundary-string edge, by position
   int32_t prefetch_dist;          // > 0: block b pulls the tables of patch b + prefetch_dist into L2 (about the blocks
                                   // resident at a time, so that it is the patch that takes over this block's slot)
   Scalars sc;                     // passive scalars (kScalars instantiation only)
+  Morph mp;                       // mobile bed (kMorph instantiation only; mp.cell / mp.qB are not used here)
+  const double *gn2;              // g / k_st^2 per cell (kMorph, MPM-like law: the halo cells' values)
 };
 
 // ---- shared-memory carving (bytes), the same for every block of a context
 struct Patch2Smem {
-  int32_t stage, crec, h, u, v, z, theta, F1, F3, GL, GR, phi, total;
+  int32_t strs, stage, crec, h, u, v, z, theta, F1, F3, GL, GR, phi, qB, fcx, fcy, total;
 };
 
-__host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species) {
+// morph: 0 fixed bed, 1 Grass-like law (q_B per own edge), 2 MPM-like law (+ (g/k^2, cbrt h) of every local cell)
+__host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species, int morph = 0) {
   Patch2Smem s;
   int32_t o = 128;                                  // [0, 8): the mbarrier
+  s.strs = o; o += blob_align(kCtlPre * (int32_t)sizeof(BoundaryString), 128);   // kSelf: the strings with Q, sumK of t^n
   s.stage = o; o += blob_align(L.stage_bytes, 128);
   s.crec = o; o += 32 * L.P;                        // own CellRec records as they are in global memory
   s.h = o; o += 8 * L.cap_loc; s.u = o; o += 8 * L.cap_loc; s.v = o; o += 8 * L.cap_loc; s.z = o; o += 8 * L.cap_loc;
@@ -56,6 +65,8 @@ __host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, in
   s.F1 = o; o += 8 * L.cap_e;
   s.F3 = o; o += 8 * L.cap_eown; s.GL = o; o += 8 * L.cap_eown; s.GR = o; o += 8 * L.cap_eown;
   s.phi = o; o += 8 * n_species * L.cap_loc;        // concentrations of the local cells, species-major
+  s.qB = o; o += morph ? 8 * L.cap_eown : 0;        // normal sediment flux of the own edges (R-20)
+  s.fcx = o; o += morph == 2 ? 8 * L.cap_loc : 0; s.fcy = o; o += morph == 2 ? 8 * L.cap_loc : 0;
   s.total = o;
   return s;
 }
@@ -102,9 +113,80 @@ __device__ __forceinline__ void publish_flag(unsigned char *pf_out_base, int b, 
   }
 }
 
+// S0 / S4 for a step that reads slot S (the arithmetic of k_step_control): dt from the rate of the state, the stop rules
+struct StepChoice { int active, flags; double dt, t_new; };
+__device__ __forceinline__ StepChoice choose_step(const StepSlot &S, double t_end, double cfl, double dt_max) {
+  StepChoice c;
+  c.active = 0; c.flags = S.flags; c.dt = 0.0; c.t_new = S.t;
+  if (S.steps_left != 0 && S.t < t_end && !(S.flags & (kFlagUnbounded | kFlagStalled))) {
+    const double r = __longlong_as_double((long long)S.rate_bits);
+    double dt = (r > 0.0) ? cfl / r : dt_max;
+    dt = fmin(dt, dt_max);
+    const double rem = t_end - S.t;
+    double t_new;
+    if (dt >= rem) { dt = rem; t_new = t_end; } else { t_new = S.t + dt; }
+    if (!isfinite(dt)) c.flags |= kFlagUnbounded;
+    else if (!(dt > 0.0) || !(t_new > S.t)) c.flags |= kFlagStalled;
+    else { c.active = 1; c.dt = dt; c.t_new = t_new; }
+  }
+  return c;
+}
+
+// outflow volume of the step that produced slot S: dt_last * tree sum of the string's l * (limited F1), by the whole
+// block (v: scratch of pow2 doubles in shared memory).  Returns vol_out with it added (every thread gets the value).
+template <int kThreads>
+__device__ __forceinline__ double book_outflow(const StepSlot &S, const BoundaryString *__restrict__ strings, int n_strings,
+                                               const double *__restrict__ M_prev, double *v) {
+  double vol_out = S.vol_out;
+  if (!S.pending) return vol_out;
+  for (int s = 0; s < n_strings; ++s) {
+    const int type = strings[s].type;
+    if (type != kBcOutflowUniform) continue;
+    const int n = strings[s].n_edges, first = strings[s].first, pow2 = strings[s].pow2;
+    for (int j = threadIdx.x; j < pow2; j += kThreads) v[j] = j < n ? M_prev[first + j] : 0.0;
+    const double sum = block_tree_sum(v, pow2);
+    vol_out += S.dt_last * sum;
+  }
+  return vol_out;
+}
+
+// start of an swe_step call in self-controlled mode: the classic fields -> slot[k0]
+__global__ void k_self_begin(Control *ctl, long long n_steps, double t_end, double cfl, int k0) {
+  ctl->steps_left = n_steps; ctl->t_end = t_end; ctl->cfl = cfl;
+  ctl->flags &= ~(kFlagUnbounded | kFlagStalled);
+  StepSlot S;
+  S.t = ctl->t; S.dt_last = ctl->dt_last; S.vol_in = ctl->vol_in; S.vol_out = ctl->vol_out; S.rate_bits = ctl->rate_bits;
+  S.steps_left = n_steps; S.steps_done = ctl->steps_done; S.src = ctl->cur; S.flags = ctl->flags; S.pending = 0; S.pad_ = 0;
+  ctl->slot[k0 & 3] = S;
+  ctl->slot[(k0 + 1) & 3].rate_bits = 0ull;
+  ctl->slot[(k0 + 2) & 3].rate_bits = 0ull;
+}
+
+// slot[k] -> the classic fields (final: with the outflow bookkeeping of the last step; else a snapshot for polling t)
+template <int kThreads>
+__global__ void __launch_bounds__(kThreads)
+k_self_finish(Control *ctl, const BoundaryString *__restrict__ strings, int n_strings, const double *__restrict__ string_M,
+              int n_string_edges, int k, int final) {
+  __shared__ double v[1024];
+  const StepSlot S = ctl->slot[k & 3];
+  double vol_out = S.vol_out;
+  if (final) vol_out = book_outflow<kThreads>(S, strings, n_strings, string_M + (size_t)((k & 1) ^ 1) * n_string_edges, v);
+  if (threadIdx.x != 0) return;
+  ctl->t = S.t; ctl->dt_last = S.dt_last; ctl->dt = S.dt_last; ctl->vol_in = S.vol_in; ctl->vol_out = vol_out;
+  ctl->rate_bits = S.rate_bits; ctl->steps_left = S.steps_left; ctl->steps_done = S.steps_done;
+  ctl->flags = S.flags; ctl->cur = S.src; ctl->src = S.pending ? (S.src ^ 1) : S.src;
+  ctl->active = 0; ctl->pending = 0;
+  if (final) { ctl->slot[k & 3].vol_out = vol_out; ctl->slot[k & 3].pending = 0; ctl->vol = 0.0; ctl->n_wet = 0; ctl->nonfinite = 0; }
+}
+
 // kThreads >= BlobLayout::P (one thread per own cell; the host picks the smallest instance that covers P).  kScalars: the passive-scalar module (R-19) is on:
 // concentrations of the local cells in shared memory, one more gather per species in phase 4.
-template <int kThreads, int kMinBlocks, bool kScalars = false, bool kPair = false>
+// kSelf: no k_step_control between the steps -- every block derives dt / t / stop rules from Control::slot[step_k], block 0
+// writes the next slot and books the volumes, the blocks that own boundary-string edges evaluate Q(t^n) and the
+// conveyance sums themselves (same fixed-shape trees, R-11).
+// kMorph: the mobile bed (R-20): q_Bij of every own edge in phase 2 (Table 2, Eq. 14-16), Eq. 13 in phase 4 -- the bed
+// rides in the state record.  A skipped patch keeps its bed: no transport where a side is dry.
+template <int kThreads, int kMinBlocks, bool kScalars = false, bool kSelf = false, bool kMorph = false>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   extern __shared__ __align__(128) unsigned char smraw[];
@@ -121,7 +203,11 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   // first halo ids of every thread, and the flag words of the patch whose tables this block pulls into L2 (below)
   const ulonglong2 *pfa = reinterpret_cast<const ulonglong2 *>(A.pflag_a + (size_t)b * kPflagBytes);
   const ulonglong2 *pfb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b * kPflagBytes);
-  const int active = ctl->active, src = ctl->src;
+  StepSlot S0;
+  int active, src;
+  double dt;
+  if (kSelf) { S0 = ctl->slot[A.step_k]; active = 0; src = S0.src; dt = 0.0; }
+  else { active = ctl->active; src = ctl->src; dt = ctl->dt; }
   const ulonglong2 fa0 = pfa[0], fa1 = pfa[1], fb0 = pfb[0], fb1 = pfb[1];
   const int hid0 = tid < L.cap_halo ? halo_ids[tid] : -1;
   const int hid1 = tid + kThreads < L.cap_halo ? halo_ids[tid + kThreads] : -1;
@@ -133,7 +219,29 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const ulonglong2 *qb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b_pf * kPflagBytes);
     ga0 = qa[0]; ga1 = qa[1]; gb0 = qb[0]; gb1 = qb[1];
   }
-  const double dt = ctl->dt, g = ctl->g, h_dry = ctl->h_dry;
+  const double g = ctl->g, h_dry = ctl->h_dry;
+  if (kSelf) {
+    const StepChoice ch = choose_step(S0, ctl->t_end, ctl->cfl, ctl->dt_max);
+    active = ch.active; dt = ch.dt;
+    if (b == 0) {                // the control duty: next slot, volume bookkeeping (before anything can return)
+      const int k1 = (A.step_k + 1) & 3, k2 = (A.step_k + 2) & 3;
+      const double vol_out = book_outflow<kThreads>(S0, A.strings, A.n_strings, A.string_M + (size_t)((A.step_k & 1) ^ 1) * A.n_string_edges,
+                                                    reinterpret_cast<double *>(smraw + 128));
+      if (tid == 0) {
+        double vol_in = S0.vol_in;
+        if (active)
+          for (int s = 0; s < A.n_strings; ++s)
+            if (A.strings[s].type == kBcInflowQ) vol_in += ch.dt * hydrograph(A.strings[s].params, A.strings[s].n_params, S0.t);
+        StepSlot *N = &ctl->slot[k1];
+        N->t = ch.t_new; N->dt_last = active ? ch.dt : S0.dt_last; N->vol_in = vol_in; N->vol_out = vol_out;
+        N->steps_left = (active && S0.steps_left > 0) ? S0.steps_left - 1 : S0.steps_left;
+        N->steps_done = S0.steps_done + active; N->src = active ? (src ^ 1) : src; N->flags = ch.flags; N->pending = active;
+        if (!active) N->rate_bits = S0.rate_bits;       // nothing accumulates into it when the step does no work
+        ctl->slot[k2].rate_bits = 0ull;
+      }
+      __syncthreads();             // the scratch is reused below
+    }
+  }
   if (!active) return;
   const CellRec *__restrict__ in = src ? A.rec_b : A.rec_a;
   CellRec *__restrict__ out = src ? A.rec_a : A.rec_b;
@@ -162,7 +270,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     }
   }
 
-  const Patch2Smem S = patch2_smem_layout(L, n_sp);
+  const int morph = kMorph ? A.mp.formula : 0;
+  const Patch2Smem S = patch2_smem_layout(L, n_sp, morph);
+  double *sh_qB = (double *)(smraw + S.qB), *sh_fcx = (double *)(smraw + S.fcx), *sh_fcy = (double *)(smraw + S.fcy);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smraw);
   unsigned char *stage = smraw + S.stage;
   CellRec *crec = reinterpret_cast<CellRec *>(smraw + S.crec);
@@ -204,6 +314,11 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       double u = 0.0, v = 0.0;
       if (c0.h > h_dry) { u = c0.qx / c0.h; v = c0.qy / c0.h; }
       sh_h[l] = c0.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c0.z;
+      if (kMorph && morph == 2) {                // MPM-like law: (g / k^2, cbrt h) as k_cell_update leaves it in Morph::cell
+        const double f2 = A.gn2[id0];
+        const bool on = c0.h > h_dry && f2 > 0.0;
+        sh_fcx[l] = on ? f2 : 0.0; sh_fcy[l] = on ? cbrt_rn(c0.h) : 0.0;
+      }
       if (l < L.cap_c1) sh_th[l] = 1.0;
       water |= (c0.h != 0.0);
       if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
@@ -215,6 +330,11 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       double u = 0.0, v = 0.0;
       if (c1.h > h_dry) { u = c1.qx / c1.h; v = c1.qy / c1.h; }
       sh_h[l] = c1.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c1.z;
+      if (kMorph && morph == 2) {
+        const double f2 = A.gn2[id1];
+        const bool on = c1.h > h_dry && f2 > 0.0;
+        sh_fcx[l] = on ? f2 : 0.0; sh_fcy[l] = on ? cbrt_rn(c1.h) : 0.0;
+      }
       if (l < L.cap_c1) sh_th[l] = 1.0;
       water |= (c1.h != 0.0);
       if (kScalars)
@@ -236,12 +356,44 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   const double *__restrict__ b_area = (const double *)(stage + L.s_area), *__restrict__ b_inv_area = (const double *)(stage + L.s_inv_area);
   const double *__restrict__ b_gn2 = (const double *)(stage + L.s_gn2);
 
+  // ---- kSelf: this block owns boundary-string edges -> Q(t^n) and the conveyance sum of every inflow string (R-11),
+  // as k_step_control evaluates them: weights from the state being read, fixed-shape pairwise tree in string order
+  const BoundaryString *sm_strings = reinterpret_cast<const BoundaryString *>(smraw + S.strs);
+  if (kSelf && H.n_string_edges > 0) {
+    BoundaryString *st = reinterpret_cast<BoundaryString *>(smraw + S.strs);
+    double *v = sh_F1;                               // scratch: the flux arrays are not in use before phase 2
+    for (int j = tid; j < A.n_strings * (int)(sizeof(BoundaryString) / 8); j += kThreads)
+      reinterpret_cast<unsigned long long *>(st)[j] = reinterpret_cast<const unsigned long long *>(A.strings)[j];
+    __syncthreads();
+    for (int s = 0; s < A.n_strings; ++s) {
+      if (st[s].type != kBcInflowQ) continue;
+      const int n = st[s].n_edges, first = st[s].first, pow2 = st[s].pow2;
+      for (int j = tid; j < pow2; j += kThreads)
+        v[j] = j < n ? A.string_lk[first + j] * pow53(in[A.string_cell[first + j]].h) : 0.0;
+      const double sum = block_tree_sum(v, pow2);
+      if (tid == 0) {
+        const double Q = hydrograph(st[s].params, st[s].n_params, S0.t);
+        st[s].sumK = sum; st[s].Q = Q;
+        // also where k_step_control would leave them (inspection: swe_get_edge_flux re-evaluates this step from them);
+        // every block that owns a string edge writes the same two values
+        BoundaryString *gs = const_cast<BoundaryString *>(A.strings) + s;
+        gs->sumK = sum; gs->Q = Q;
+      }
+    }
+    __syncthreads();
+  }
+
   // ---- phase 1b: own cells, from the records the bulk copy delivered
   if (tid < n_own) {
     const CellRec c_own = crec[tid];
     double u = 0.0, v = 0.0;
     if (c_own.h > h_dry) { u = c_own.qx / c_own.h; v = c_own.qy / c_own.h; }
     sh_h[tid] = c_own.h; sh_u[tid] = u; sh_v[tid] = v; sh_z[tid] = c_own.z; sh_th[tid] = 1.0;
+    if (kMorph && morph == 2) {
+      const double f2 = b_gn2[tid];
+      const bool on = c_own.h > h_dry && f2 > 0.0;
+      sh_fcx[tid] = on ? f2 : 0.0; sh_fcy[tid] = on ? cbrt_rn(c_own.h) : 0.0;
+    }
     water |= (c_own.h != 0.0);
     if (kScalars)
       _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
@@ -267,8 +419,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     return;
   }
 
-  // ---- phase 2: edge fluxes.  kPair: two edges per thread and iteration, so that their instruction streams interleave
-  // (the flux of one edge is a long chain of dependent fp64 operations: sqrt -> wave speeds -> division -> fluxes)
+  // ---- phase 2: edge fluxes (two edges per thread and iteration, to interleave their dependent fp64 chains, was
+  // measured and is slower: 80 registers with spills, branches keep the streams apart)
   struct EdgeIn { double nx, ny, len, hL, uL, vL, zL, hR, uR, vR, zR; int Lc, Rc; };
   auto load_edge = [&](int e) {
     EdgeIn q;
@@ -289,7 +441,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     } else {
       const BoundaryString *bs = nullptr;
       int code = b_aux[e];
-      if (code <= -3) { bs = A.strings + A.slot_string[-3 - code]; code = -3; }
+      if (code <= -3) { bs = (kSelf ? sm_strings : A.strings) + A.slot_string[-3 - code]; code = -3; }
       const int gidL = q.Lc < n_own ? cell0 + q.Lc : halo_ids[q.Lc - n_own];
       o = boundary_flux(g, code, bs, A.kst, gidL, q.nx, q.ny, q.len, q.hL, q.zL, q.uL, q.vL);
     }
@@ -298,6 +450,13 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   auto store_edge = [&](const EdgeIn &q, int e, const EdgeFlux &o) {
     sh_F1[e] = o.F1;
     if (e < H.n_eown) { sh_F3[e] = o.F3; sh_GL[e] = o.GL; sh_GR[e] = o.GR; }
+    if (kMorph && e < H.n_eown) {                     // S1m: q_Bij from the state at t^n (Eq. 14-16; R-20)
+      const int Rcode = q.Rc != 0xFFFF ? 0 : (b_aux[e] <= -3 ? -3 : b_aux[e]);
+      const double2 zero = make_double2(0.0, 0.0);
+      const double2 fcL = morph == 2 ? make_double2(sh_fcx[q.Lc], sh_fcy[q.Lc]) : zero;
+      const double2 fcR = (morph == 2 && q.Rc != 0xFFFF) ? make_double2(sh_fcx[q.Rc], sh_fcy[q.Rc]) : zero;
+      sh_qB[e] = sediment_flux_core(A.mp, g, h_dry, Rcode, q.nx, q.ny, q.hL, q.uL, q.vL, q.zL, fcL, q.hR, q.uR, q.vR, q.zR, fcR);
+    }
     // S1c, lazily (R-8b; as in k_edge_flux): theta_i < 1 needs one outgoing edge with dt * o_k > 0.3 h_i |Omega_i|.  Only
     // such donor cells are marked (theta = -1); phase 3 evaluates theta for them and every other cell keeps theta = 1.
     const int d = o.F1 > 0.0 ? q.Lc : ((o.F1 < 0.0 && q.Rc != 0xFFFF) ? q.Rc : n_c1);
@@ -307,29 +466,10 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       if (dt * (q.len * fabs(o.F1)) > 0.3 * (hd * ad)) sh_th[d] = -1.0;
     }
   };
-  if (!kPair) {
-    for (int e = tid; e < n_e; e += kThreads) {
-      const EdgeIn q = load_edge(e);
-      const EdgeFlux o = flux_edge(q, e);
-      store_edge(q, e, o);
-    }
-  } else {
-    // (trip count and the choice pair / single are warp-uniform: eb is the first edge of the warp's chunk)
-    for (int eb = tid - (tid & 31); eb < n_e; eb += 2 * kThreads) {
-      const int e0 = eb + (tid & 31), e1 = e0 + kThreads;
-      const bool has0 = e0 < n_e, has1 = e1 < n_e;
-      if (eb + kThreads < n_e) {                       // the warp's second chunk has at least one edge
-        const int e0s = has0 ? e0 : eb, e1s = has1 ? e1 : e0s;
-        const EdgeIn q0 = load_edge(e0s), q1 = load_edge(e1s);
-        const EdgeFlux o0 = flux_edge(q0, e0s), o1 = flux_edge(q1, e1s);
-        if (has0) store_edge(q0, e0, o0);
-        if (has1) store_edge(q1, e1, o1);
-      } else if (has0) {
-        const EdgeIn q = load_edge(e0);
-        const EdgeFlux o = flux_edge(q, e0);
-        store_edge(q, e0, o);
-      }
-    }
+  for (int e = tid; e < n_e; e += kThreads) {
+    const EdgeIn q = load_edge(e);
+    const EdgeFlux o = flux_edge(q, e);
+    store_edge(q, e, o);
   }
   __syncthreads();
 
@@ -363,7 +503,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const CellRec c_own = crec[l];
     const double invA = b_inv_area[l], f2 = b_gn2[l];
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
-    double dH = 0.0, dX = 0.0, dY = 0.0;             // ((d0 + d1) + d2), accumulated in slot order
+    double dH = 0.0, dX = 0.0, dY = 0.0, dB = 0.0;   // ((d0 + d1) + d2), accumulated in slot order
     double F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,
     int up[3];                                       // local id of the upwind cell, or -1 - slot of an inflow-string edge
 #pragma unroll
@@ -384,6 +524,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       const double dXk = s * (lenk * (G * nxk - F3 * nyk));
       const double dYk = s * (lenk * (G * nyk + F3 * nxk));
       if (k == 0) { dH = dHk; dX = dXk; dY = dYk; } else { dH = dH + dHk; dX = dX + dXk; dY = dY + dYk; }
+      if (kMorph) { const double dBk = s * (lenk * sh_qB[e]); dB = k == 0 ? dBk : dB + dBk; }
       if (kScalars) {
         F1k[k] = F1; slk[k] = lenk;
         const uint32_t Lc = isL ? (uint32_t)l : nb, Rc = isL ? nb : (uint32_t)l;
@@ -393,7 +534,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       if (nb == kPceNoNeighbour) {                  // boundary-string edge: volume bookkeeping of k_step_control
         const int aux = b_aux[e];
         if (aux <= -3) {
-          A.string_M[-3 - aux] = lenk * F1;
+          A.string_M[(kSelf ? (size_t)(A.step_k & 1) * A.n_string_edges : (size_t)0) + (-3 - aux)] = lenk * F1;
           if (kScalars && !(F1 >= 0.0) && A.strings[A.slot_string[-3 - aux]].type == kBcInflowQ) up[k] = -1 - (-3 - aux);
         }
       }
@@ -426,6 +567,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     }
     CellRec c = c_own;
     c.h = hn; c.qx = qxn; c.qy = qyn;
+    if (kMorph) c.z = c.z - A.mp.inv1mp * (a * dB);   // Eq. 13, S_b = 0
     out[i] = c;
     nonzero |= (hn != 0.0) | (qxn != 0.0) | (qyn != 0.0);
     if (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
@@ -447,7 +589,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   nonzero = __syncthreads_or(nonzero);
   publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(stage + L.s_nbr), (const int32_t *)(stage + L.s_nbr_slot), L.cap_nbr,
                          nonzero ? 0 : 1);
-  block_max_to_global<kThreads>(rate, &ctl->rate_bits);
+  block_max_to_global<kThreads>(rate, kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits);
 }
 
 // flags after swe_set_state, two launches: (1) own flag of the buffer that holds the newest state from the records

@@ -8,18 +8,29 @@
 
 namespace swe {
 
-struct __align__(32) CellRec {   // state U = (h, q_x, q_y) + cell-mean bed z_B (R-13)
-  double h, qx, qy, z;
-};
+// T = double (the default arithmetic) or float (single precision, swe_params.precision; R-21): a record
+// is 32 bytes = one sector in fp64 and 16 bytes in fp32.
+template <typename T> struct CellRecT;     // state U = (h, q_x, q_y) + cell-mean bed z_B (R-13)
+template <> struct __align__(32) CellRecT<double> { double h, qx, qy, z; };
+template <> struct __align__(16) CellRecT<float> { float h, qx, qy, z; };
 
-struct __align__(32) EdgeGeom {  // section 4.1: unit normal from L to R, edge length, the two cells
+template <typename T> struct EdgeGeomT;    // section 4.1: unit normal from L to R, edge length, the two cells
+template <> struct __align__(32) EdgeGeomT<double> {
   double nx, ny, len;
   int32_t L, R;                  // R < 0: boundary code (include/swe.h)
 };
-
-struct __align__(32) EdgeFlux {  // S1 outputs: F1 mass, F3 tangential momentum, G_K = F2 - 1/2 g hs_K^2
-  double F1, F3, GL, GR;
+template <> struct __align__(16) EdgeGeomT<float> {   // R lives in a separate int32 array (only the edge kernel reads it)
+  float nx, ny, len;
+  int32_t L;
 };
+
+template <typename T> struct EdgeFluxT;    // S1 outputs: F1 mass, F3 tangential momentum, G_K = F2 - 1/2 g hs_K^2
+template <> struct __align__(32) EdgeFluxT<double> { double F1, F3, GL, GR; };
+template <> struct __align__(16) EdgeFluxT<float> { float F1, F3, GL, GR; };
+
+typedef CellRecT<double> CellRec;
+typedef EdgeGeomT<double> EdgeGeom;
+typedef EdgeFluxT<double> EdgeFlux;
 
 // pce[] record = uint4 {slot0, slot1, slot2, unused}; slot = edge (bits 0-14) | isL (bit 15) | neighbour cell (bits 16-31)
 constexpr uint32_t kPceNoNeighbour = 0xFFFFu;
@@ -121,6 +132,16 @@ struct Morph {                   // morphodynamics (section 3.2 Eq. 3, section 4
   double *qB;                    // [n_edges] normal sediment flux q_Bij of the step in flight
 };
 
+struct StepSlot {
+  double t, dt_last, vol_in, vol_out;
+  unsigned long long rate_bits;  // max rate of the state this slot describes
+  long long steps_left, steps_done;
+  int32_t src;                   // state buffer that holds this state
+  int32_t flags;
+  int32_t pending;               // 1: the step that produced this state wrote outflow terms not yet booked in vol_out
+  int32_t pad_;
+};
+
 struct Control {                 // device-side step-loop state: nothing of it is read by the host per step
   double t, dt, t_end, cfl, dt_max, g, h_dry;
   double dt_last, vol_in, vol_out, vol_clipped;
@@ -142,6 +163,11 @@ struct Control {                 // device-side step-loop state: nothing of it i
   long long n_wet;
   int32_t nonfinite;
   int32_t pad_;
+  // fused patch step without a control kernel: step number n reads slot[n % 4] -- every block
+  // derives dt, t and the stop rules from it by itself --, block 0 writes slot[(n + 1) % 4], the rate of the new state
+  // is collected in slot[(n + 1) % 4].rate_bits and slot[(n + 2) % 4].rate_bits is cleared for the step after.
+  // swe_step copies the classic fields above into a slot when it starts and back when it ends.
+  StepSlot slot[4];
 };
 
 }  // namespace swe

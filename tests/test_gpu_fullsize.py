@@ -155,7 +155,7 @@ def test_config4_full_size_mobile_bed(gpu, ref):
     morph = (2, 8.0, 0.047, 2.65, 0.005, 0.4)
     s.set_morphology(*morph)
     o.set_morphology(*morph)
-    assert s.step_kernels() == ["k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"]
+    assert s.step_kernels()[-1] == "k_patch_step"          # AUTO stays on the fused patch step with the mobile bed
     window(s, o, w, 12, "config4 full size, mobile bed, steps 0-12")
     zg, zo = s.get_bed(), o.get_bed()
     assert np.array_equal(zg, zo)

@@ -425,7 +425,7 @@ def test_auto_picks_the_variant_from_the_wet_fraction(gpu, ref):
     the domain is dry, the three-pass step on (almost) all-wet states.  Switching is invisible in the results."""
     w4, w3 = CASES["config4-small"](), CASES["config3-small"]()
     a = gpu.from_workload(w4, variant=gpu.VARIANT_AUTO, patch_cells=0)
-    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_step_control", "k_patch_step"]
+    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_patch_step"]   # self-controlled: one kernel per step
     b = gpu.from_workload(w3, variant=gpu.VARIANT_AUTO, patch_cells=0)
     assert b.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS and len(b.step_kernels()) == 4
     # odd number of steps (the patch step ping-pongs), then flood the river reach: AUTO switches to three-pass
@@ -501,7 +501,8 @@ def _many_strings_workload(nx, ny, n_in, n_out):
 @pytest.mark.parametrize("nx,ny,n_in,n_out", [(6, 40, 3, 3),        # six strings: general path of k_step_control
                                                (4, 1500, 1, 1),     # 1500 members: more than the control block's threads
                                                (3, 4500, 1, 1),     # 4500 members: pairwise tree in global scratch
-                                               (8, 64, 2, 2)])      # four short strings: the up-front path
+                                               (8, 64, 2, 2),       # four short strings: the up-front path
+                                               (4, 300, 1, 1)])     # 300 members: a 512-leaf tree, more leaves than threads
 def test_boundary_string_sums_many_and_long_strings(gpu, ref, nx, ny, n_in, n_out):
     """R-11: the fixed-shape pairwise sums over boundary strings (conveyance weights, outflow volume) and the volume
     bookkeeping, for string counts and sizes on both sides of the limits of k_step_control's up-front path."""

@@ -210,3 +210,31 @@ def test_bed_hump_travels_with_the_bed_wave_celerity(ref, direction):
     assert xc1 - xc0 == pytest.approx(cb * T, rel=0.05)
     assert (zb * area).sum() == pytest.approx((w.zb * area).sum(), rel=2e-3)     # what left through the ends is tiny
     assert zb.max() > 0.08                                                      # still a hump, not smeared away
+
+
+def test_scalars_ride_on_a_moving_bed(ref):
+    """Modules active together ("synchronous-decoupled ... same integration timestep"):
+    scalars and the mobile bed in one run.  The scalar update of Eq. 20 uses the hydrodynamic mass flux only, so a uniform
+    concentration stays uniform while the bed moves under it (q_c == phi0 * h bit for bit with phi0 = 1, to round-off for
+    phi0 = 0.37), the hydrodynamic state and the bed are exactly those of the run without scalars, and scalar mass is
+    conserved in the closed box."""
+    w = C.dam_break_channel(nx=80, ny=4, lx=20.0, ly=1.0, h_left=1.0, h_right=0.2, x_dam=10.0, t_end=float("inf"))
+    w.kst[:] = 35.0
+    morph = (ref.GRASS, 0.02, 0.0, 2.65, 1e-3, 0.4)
+    a = ref.RefSolver(w)                       # mobile bed, no scalars
+    a.set_morphology(*morph)
+    b = ref.RefSolver(w)                       # mobile bed + two species: phi = 1 and phi = 0.37
+    b.set_scalars(np.stack([w.h.copy(), 0.37 * w.h]))
+    b.set_morphology(*morph)
+    area = a.geometry()[0]
+    m0 = float(np.sum(0.37 * w.h * area))
+    ia, ib = a.step(150, float("inf"), 0.7), b.step(150, float("inf"), 0.7)
+    assert ia == ib
+    for x, y in zip(a.get_state(), b.get_state()):
+        assert np.array_equal(x, y)
+    assert np.array_equal(a.get_bed(), b.get_bed()) and np.abs(a.get_bed() - w.zb).max() > 1e-5      # the bed did move
+    h = b.get_state()[0]
+    qc = b.get_scalars()
+    assert np.array_equal(qc[0], h)                                     # phi = 1: q_c is h, bit for bit
+    assert np.max(np.abs(qc[1] - 0.37 * h)) <= 1e-14                    # phi = 0.37 stays uniform to round-off
+    assert abs(float(np.sum(qc[1] * area)) - m0) <= 1e-13 * m0          # scalar mass conserved in the closed box
