@@ -154,8 +154,9 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
       if (g.R >= 0) { lr[j] = Ll | ((uint32_t)cloc[g.R] << 16); aux[j] = 0; }
       else { lr[j] = Ll | (0xFFFFu << 16); aux[j] = (g.R <= -3) ? -3 - string_pos[s.edges[j]] : g.R; }
     }
-    double *a = (double *)(S + L.s_area), *ia = (double *)(S + L.s_inv_area), *g2 = (double *)(S + L.s_gn2);
-    for (int32_t l = 0; l < s.n_own; ++l) { a[l] = area[c0 + l]; ia[l] = inv_area[c0 + l]; g2[l] = gn2[c0 + l]; }
+    double *a = (double *)(S + L.s_area), *g2 = (double *)(S + L.s_gn2);
+    for (int32_t l = 0; l < s.n_own; ++l) { a[l] = area[c0 + l]; g2[l] = gn2[c0 + l]; }
+    (void)inv_area;
   }
   return true;
 }

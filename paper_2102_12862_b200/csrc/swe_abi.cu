@@ -177,7 +177,7 @@ struct swe_ctx {
   bool self_ctl = false;             // fused patch step without k_step_control (every block derives dt itself)
   int64_t step_idx = 0;              // step launches enqueued so far (self_ctl: launch n reads Control::slot[n % 4])
   int64_t n_string_edges = 0;
-  const PatchInst *patch_inst = nullptr;
+  int patch_force_blocks = 0;        // SWE_PATCH_MIN_BLOCKS (measurement runs): pin the __launch_bounds__ instance
   int n_patches = 0, patch_threads = 0, patch_prefetch = 0; size_t patch_smem = 0;
   int64_t patch_sum_loc = 0, patch_sum_e = 0; int patch_max_loc = 0, patch_max_e = 0, patch_min_blocks = 0;
   InfoPartial *d_info_part = nullptr; unsigned int *d_info_ticket = nullptr;
@@ -287,8 +287,9 @@ void enqueue_three_pass_f32(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev) {
 // block grows with the scalar species and the mobile-bed law
 void launch_patch(swe_ctx *c, cudaStream_t s, int self) {
   const int morph = c->mp.formula;
-  const size_t smem = (size_t)patch2_smem_layout(c->blay, c->sc.n, morph).total;
-  c->patch_inst->fn[c->sc.n > 0][self][morph != 0]<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
+  const size_t smem = (size_t)patch2_smem_layout(c->blay, c->sc.n, morph, self != 0).total;
+  const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, c->patch_force_blocks);   // most blocks per SM that fit
+  pi->fn[c->sc.n > 0][self][morph != 0]<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
 }
 
 // one time step, in stream order.  Self-controlled patch step: the launch number decides the control slot it reads
@@ -552,12 +553,23 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
   // ---- fused patch step: patch blobs, shared-memory size
   pl.variant = (p.variant == SWE_VARIANT_THREE_PASS || pl.z.single) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
   if (pl.variant == SWE_VARIANT_PATCH) {
-    // default: 256 cells = 256 threads (profiles/r2*_patch_sweep.md); small meshes get smaller patches, so that the
-    // launch-latency-bound step still spreads over the SMs
-    int P = p.patch_cells > 0 ? p.patch_cells : 256;
-    if (p.patch_cells <= 0 && nc < 148 * 256) P = nc < 148 * 64 ? 32 : (nc < 148 * 128 ? 64 : 128);
+    // default: the largest patch of 240, 232, 224, 208, 192 cells (256 threads each) whose block still fits an SM four
+    // times -- 32 warps per SM; the kernel is latency-bound and 4 x 8 warps beat 3 x 8 by 10-13 %, larger patches beat
+    // smaller ones by 1-2 % per step of 8 cells (profiles/r2_patch_sweep.md); small meshes get smaller patches, so that
+    // the launch-latency-bound step still spreads over the SMs
     std::vector<int32_t> string_pos(ne, -1);
     for (size_t j = 0; j < pl.flat.size(); ++j) string_pos[pl.flat[j]] = (int32_t)j;
+    int P = p.patch_cells;
+    if (P <= 0 && nc < 148 * 256) P = nc < 148 * 64 ? 32 : (nc < 148 * 128 ? 64 : 128);
+    if (P <= 0) {
+      const bool self = false;               // (meshes of this size do not run the self-controlled step)
+      for (int cand : {240, 232, 224, 208, 192}) {
+        P = cand;
+        if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, false, pl.pb, err)) return SWE_EINVAL;
+        const size_t smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species, 0, self && nc / P <= 8192).total;
+        if (4 * (smem + kSmemBlockReserve) <= kSmemPerSM) break;
+      }
+    }
     if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, emit, pl.pb, err)) return SWE_EINVAL;
     pl.patch_smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species).total;
     // a numbering that is not spatially compact (renumber = NONE on a scattered input order) blows the halos up:
@@ -723,16 +735,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     c->d_blob = (unsigned char *)(ws + lay.blob); c->d_pflag = (unsigned char *)(ws + lay.pflag);
     SWE_CUDA(c, cudaMemcpy(c->d_blob, pb.bytes.data(), pb.bytes.size(), cudaMemcpyHostToDevice));
     SWE_CUDA(c, cudaMemset(c->d_pflag, 0, 2 * (size_t)kPflagBytes * (size_t)c->n_patches));
-    int force = 0;
-    if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) force = std::atoi(s);
+    if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) c->patch_force_blocks = std::atoi(s);
     c->patch_threads = patch_threads(pb.lay.P);
-    c->patch_prefetch = 3 * 148;
+    c->patch_prefetch = 4 * 148;              // about the blocks resident at a time
     if (const char *s = std::getenv("SWE_PATCH_PREFETCH")) c->patch_prefetch = std::atoi(s);
-    // (sized for the fattest block the context can ask for: the mobile bed with the MPM-like law, when reserved)
-    const size_t smem_max = (size_t)patch2_smem_layout(pb.lay, c->sc.n, pl.z.morph ? 2 : 0).total;
-    const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem_max, force);
-    if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
-    c->patch_inst = pi; c->patch_min_blocks = pi->min_blocks;
     // self-controlled steps: at most kCtlPre strings, each string's pairwise tree inside the block's scratch (the
     // flux arrays of the patch, and the 1024 doubles of k_self_finish), graphs a multiple of 4 steps long
     {
@@ -744,19 +750,29 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       if (const char *s = std::getenv("SWE_PATCH_SELF")) ok = ok && std::atoi(s) != 0;
       c->self_ctl = ok;
     }
+    c->patch_smem = (size_t)patch2_smem_layout(pb.lay, c->sc.n, 0, c->self_ctl).total;
+    {
+      const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->patch_smem, c->patch_force_blocks);
+      if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
+      c->patch_min_blocks = pi->min_blocks;
+    }
     // the attribute belongs to the kernel, not to the context: always raise it to the hardware limit, so that a later
     // context with smaller patches cannot lower it under an earlier context's launches
     {
+      const size_t smem_max = (size_t)patch2_smem_layout(pb.lay, c->sc.n, pl.z.morph ? 2 : 0, true).total;
       int dev = 0, optin = 0;
       cudaFuncAttributes fa{};
       SWE_CUDA(c, cudaGetDevice(&dev));
       SWE_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-      for (int a = 0; a < 8; ++a) {
-        PatchKernel fn = pi->fn[a & 1][(a >> 1) & 1][(a >> 2) & 1];
-        SWE_CUDA(c, cudaFuncGetAttributes(&fa, fn));
-        const int limit = optin - (int)fa.sharedSizeBytes;
-        if ((int)smem_max > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
-        SWE_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
+      for (const PatchInst &pi : kPatchInst) {
+        if (pi.T != c->patch_threads) continue;
+        for (int a = 0; a < 8; ++a) {
+          PatchKernel fn = pi.fn[a & 1][(a >> 1) & 1][(a >> 2) & 1];
+          SWE_CUDA(c, cudaFuncGetAttributes(&fa, fn));
+          const int limit = optin - (int)fa.sharedSizeBytes;
+          if ((int)smem_max > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
+          SWE_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, limit));
+        }
       }
     }
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
@@ -916,8 +932,10 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     c->launches += 2;
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
-    // measured crossover on the river reach filled to different stages: ~52 % wet cells (profiles/r1i_auto_threshold.md)
-    const int want = (double)c->h_ctl->n_wet > 0.5 * (double)nc ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+    // with four blocks of the patch kernel per SM it is the faster step at any wet fraction (all-wet 4M: 259.6 vs 266.1 us,
+    // 8M: 508 vs 521 us; profiles/r2_patch_sweep.md); with fewer (fat halos, scalar species, large patch_cells) the
+    // round-1 crossover holds: three-pass from ~50 % wet cells on (profiles/r1i_auto_threshold.md)
+    const int want = (c->patch_min_blocks < 4 && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
       if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
         for (int sp = 0; sp < c->sc.n; ++sp)
@@ -996,7 +1014,8 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (h.nonfinite) { c->err = "non-finite state value"; return SWE_ENONFINITE; }
     if (c->auto_mode) {   // the wet count is known here: follow a flood that spreads (or recedes), with hysteresis
       const double wet = (double)h.n_wet / (double)c->nc;
-      const int want = wet > 0.55 ? SWE_VARIANT_THREE_PASS : (wet < 0.45 ? SWE_VARIANT_PATCH : c->variant);
+      const int want = c->patch_min_blocks >= 4 ? SWE_VARIANT_PATCH
+                                                : (wet > 0.55 ? SWE_VARIANT_THREE_PASS : (wet < 0.45 ? SWE_VARIANT_PATCH : c->variant));
       rc = switch_variant(c, want, h.cur);
       if (rc != SWE_OK) return rc;
     }

@@ -54,16 +54,20 @@ struct Patch2Smem {
 };
 
 // morph: 0 fixed bed, 1 Grass-like law (q_B per own edge), 2 MPM-like law (+ (g/k^2, cbrt h) of every local cell)
-__host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species, int morph = 0) {
+__host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species, int morph = 0, bool self = true) {
   Patch2Smem s;
   int32_t o = 128;                                  // [0, 8): the mbarrier
-  s.strs = o; o += blob_align(kCtlPre * (int32_t)sizeof(BoundaryString), 128);   // kSelf: the strings with Q, sumK of t^n
+  s.strs = o; o += self ? blob_align(kCtlPre * (int32_t)sizeof(BoundaryString), 128) : 0;   // kSelf: the strings with Q, sumK of t^n
   s.stage = o; o += blob_align(L.stage_bytes, 128);
-  s.crec = o; o += 32 * L.P;                        // own CellRec records as they are in global memory
   s.h = o; o += 8 * L.cap_loc; s.u = o; o += 8 * L.cap_loc; s.v = o; o += 8 * L.cap_loc; s.z = o; o += 8 * L.cap_loc;
   s.theta = o; o += 8 * L.cap_c1;
   s.F1 = o; o += 8 * L.cap_e;
-  s.F3 = o; o += 8 * L.cap_eown; s.GL = o; o += 8 * L.cap_eown; s.GR = o; o += 8 * L.cap_eown;
+  o = blob_align(o, 32);
+  // the own CellRec records as the bulk copy delivers them are consumed in phase 1 (the momenta stay in registers),
+  // the fluxes F3 / GL / GR of the own edges are written from phase 2 on: the two share their shared memory
+  s.crec = o;
+  s.F3 = o; s.GL = o + 8 * L.cap_eown; s.GR = o + 16 * L.cap_eown;
+  o += (24 * L.cap_eown > 32 * L.P) ? 24 * L.cap_eown : 32 * L.P;
   s.phi = o; o += 8 * n_species * L.cap_loc;        // concentrations of the local cells, species-major
   s.qB = o; o += morph ? 8 * L.cap_eown : 0;        // normal sediment flux of the own edges (R-20)
   s.fcx = o; o += morph == 2 ? 8 * L.cap_loc : 0; s.fcy = o; o += morph == 2 ? 8 * L.cap_loc : 0;
@@ -271,7 +275,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   }
 
   const int morph = kMorph ? A.mp.formula : 0;
-  const Patch2Smem S = patch2_smem_layout(L, n_sp, morph);
+  const Patch2Smem S = patch2_smem_layout(L, n_sp, morph, kSelf);
   double *sh_qB = (double *)(smraw + S.qB), *sh_fcx = (double *)(smraw + S.fcx), *sh_fcy = (double *)(smraw + S.fcy);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smraw);
   unsigned char *stage = smraw + S.stage;
@@ -353,39 +357,14 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   const double *__restrict__ b_len = (const double *)(stage + L.s_len);
   const uint32_t *__restrict__ b_lr = (const uint32_t *)(stage + L.s_lr);
   const int32_t *__restrict__ b_aux = (const int32_t *)(stage + L.s_aux);
-  const double *__restrict__ b_area = (const double *)(stage + L.s_area), *__restrict__ b_inv_area = (const double *)(stage + L.s_inv_area);
+  const double *__restrict__ b_area = (const double *)(stage + L.s_area);
   const double *__restrict__ b_gn2 = (const double *)(stage + L.s_gn2);
 
-  // ---- kSelf: this block owns boundary-string edges -> Q(t^n) and the conveyance sum of every inflow string (R-11),
-  // as k_step_control evaluates them: weights from the state being read, fixed-shape pairwise tree in string order
-  const BoundaryString *sm_strings = reinterpret_cast<const BoundaryString *>(smraw + S.strs);
-  if (kSelf && H.n_string_edges > 0) {
-    BoundaryString *st = reinterpret_cast<BoundaryString *>(smraw + S.strs);
-    double *v = sh_F1;                               // scratch: the flux arrays are not in use before phase 2
-    for (int j = tid; j < A.n_strings * (int)(sizeof(BoundaryString) / 8); j += kThreads)
-      reinterpret_cast<unsigned long long *>(st)[j] = reinterpret_cast<const unsigned long long *>(A.strings)[j];
-    __syncthreads();
-    for (int s = 0; s < A.n_strings; ++s) {
-      if (st[s].type != kBcInflowQ) continue;
-      const int n = st[s].n_edges, first = st[s].first, pow2 = st[s].pow2;
-      for (int j = tid; j < pow2; j += kThreads)
-        v[j] = j < n ? A.string_lk[first + j] * pow53(in[A.string_cell[first + j]].h) : 0.0;
-      const double sum = block_tree_sum(v, pow2);
-      if (tid == 0) {
-        const double Q = hydrograph(st[s].params, st[s].n_params, S0.t);
-        st[s].sumK = sum; st[s].Q = Q;
-        // also where k_step_control would leave them (inspection: swe_get_edge_flux re-evaluates this step from them);
-        // every block that owns a string edge writes the same two values
-        BoundaryString *gs = const_cast<BoundaryString *>(A.strings) + s;
-        gs->sumK = sum; gs->Q = Q;
-      }
-    }
-    __syncthreads();
-  }
-
   // ---- phase 1b: own cells, from the records the bulk copy delivered
+  double qx_own = 0.0, qy_own = 0.0;               // the momenta of this thread's own cell, kept for phase 4
   if (tid < n_own) {
     const CellRec c_own = crec[tid];
+    qx_own = c_own.qx; qy_own = c_own.qy;
     double u = 0.0, v = 0.0;
     if (c_own.h > h_dry) { u = c_own.qx / c_own.h; v = c_own.qy / c_own.h; }
     sh_h[tid] = c_own.h; sh_u[tid] = u; sh_v[tid] = v; sh_z[tid] = c_own.z; sh_th[tid] = 1.0;
@@ -417,6 +396,34 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
                            scalar_mass ? 0 : 1);
     if (tid == 0) atomicAdd(&ctl->patches_skipped, 1ull);
     return;
+  }
+
+  // ---- kSelf: this block owns boundary-string edges -> Q(t^n) and the conveyance sum of every inflow string (R-11),
+  // as k_step_control evaluates them: weights from the state being read, fixed-shape pairwise tree in string order
+  const BoundaryString *sm_strings = reinterpret_cast<const BoundaryString *>(smraw + S.strs);
+  if (kSelf && H.n_string_edges > 0) {
+    BoundaryString *st = reinterpret_cast<BoundaryString *>(smraw + S.strs);
+    double *v = sh_F1;                               // scratch: the flux arrays (and the own records aliased with them,
+                                                     // consumed in phase 1) are not in use before phase 2
+    for (int j = tid; j < A.n_strings * (int)(sizeof(BoundaryString) / 8); j += kThreads)
+      reinterpret_cast<unsigned long long *>(st)[j] = reinterpret_cast<const unsigned long long *>(A.strings)[j];
+    __syncthreads();
+    for (int s = 0; s < A.n_strings; ++s) {
+      if (st[s].type != kBcInflowQ) continue;
+      const int n = st[s].n_edges, first = st[s].first, pow2 = st[s].pow2;
+      for (int j = tid; j < pow2; j += kThreads)
+        v[j] = j < n ? A.string_lk[first + j] * pow53(in[A.string_cell[first + j]].h) : 0.0;
+      const double sum = block_tree_sum(v, pow2);
+      if (tid == 0) {
+        const double Q = hydrograph(st[s].params, st[s].n_params, S0.t);
+        st[s].sumK = sum; st[s].Q = Q;
+        // also where k_step_control would leave them (inspection: swe_get_edge_flux re-evaluates this step from them);
+        // every block that owns a string edge writes the same two values
+        BoundaryString *gs = const_cast<BoundaryString *>(A.strings) + s;
+        gs->sumK = sum; gs->Q = Q;
+      }
+    }
+    __syncthreads();
   }
 
   // ---- phase 2: edge fluxes (two edges per thread and iteration, to interleave their dependent fp64 chains, was
@@ -500,8 +507,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   if (tid < n_own) {
     const int l = tid, i = cell0 + tid;
     const uint4 pc = b_pce[l];
-    const CellRec c_own = crec[l];
-    const double invA = b_inv_area[l], f2 = b_gn2[l];
+    CellRec c_own;
+    c_own.h = sh_h[l]; c_own.qx = qx_own; c_own.qy = qy_own; c_own.z = sh_z[l];
+    const double invA = 1.0 / b_area[l], f2 = b_gn2[l];      // 1 / |Omega| as the host forms it for the three-pass step
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
     double dH = 0.0, dX = 0.0, dY = 0.0, dB = 0.0;   // ((d0 + d1) + d2), accumulated in slot order
     double F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,

@@ -44,7 +44,7 @@ constexpr uint32_t kPceNoNeighbour = 0xFFFFu;
 //   [off_stage, off_stage + stage_bytes)   staged into shared memory by the bulk copy, SoA (bank-conflict-free):
 //                             BlobHeader copy | nbr, nbr_slot copies | halo_area[cap_r1] | pce[cap_c1] uint4 | nx, ny, len [cap_e] double |
 //                             lr[cap_e] uint32 (L | R << 16; R = 0xFFFF boundary) | aux[cap_e] int32 |
-//                             area, inv_area, gn2 [P] double
+//                             area, gn2 [P] double  (1 / area is formed in the kernel: the same IEEE quotient)
 struct BlobHeader {              // 32 bytes
   int32_t n_own, n_r1, n_r2, n_eown, n_er1, n_string_edges, n_nbr, pad_;
 };
@@ -54,7 +54,7 @@ struct BlobLayout {
   int32_t cap_nbr, cap_halo, cap_r1, cap_c1, cap_loc, cap_e, cap_eown;
   int32_t off_nbr, off_nbr_slot, off_halo_ids, off_stage;
   // offsets RELATIVE TO off_stage (= offsets inside the staged copy in shared memory)
-  int32_t s_hdr, s_nbr, s_nbr_slot, s_halo_area, s_pce, s_nx, s_ny, s_len, s_lr, s_aux, s_area, s_inv_area, s_gn2;
+  int32_t s_hdr, s_nbr, s_nbr_slot, s_halo_area, s_pce, s_nx, s_ny, s_len, s_lr, s_aux, s_area, s_gn2;
   int32_t stage_bytes;           // multiple of 16
   int32_t stride;                // bytes per blob, multiple of 128
 };
@@ -90,7 +90,6 @@ __host__ __device__ inline BlobLayout blob_layout(int P, int cap_nbr, int cap_ha
   L.s_aux = s; s += 4 * cap_e;
   s = blob_align(s, 8);
   L.s_area = s; s += 8 * P;
-  L.s_inv_area = s; s += 8 * P;
   L.s_gn2 = s; s += 8 * P;
   L.stage_bytes = blob_align(s, 16);
   L.stride = blob_align(L.off_stage + L.stage_bytes, 128);

@@ -83,7 +83,7 @@ def test_config4_full_size_windows(gpu, ref):
 
 def test_config5_16m_window(gpu, ref):
     """BASELINE.json configs[4], second size (16M triangles): every cell against the oracle over the first 6 steps, in
-    the launch configuration bench.py times, then the fused patch step against the three-pass step over 40 more."""
+    the launch configuration bench.py times, then the three-pass step against the fused patch step (AUTO's choice) over 40 more."""
     w = C.by_id(5, 2.0)
     assert 15.5e6 < w.n_cells < 16.5e6
     s = make(gpu, w)
@@ -91,7 +91,7 @@ def test_config5_16m_window(gpu, ref):
     ig, io, _ = window(s, o, w, 6, "config5 16M, steps 0-6")
     check_info(ig, io)
     o.close()
-    t = gpu.from_workload(w, variant=gpu.VARIANT_PATCH)
+    t = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
     t.step(6, float("inf"), w.cfl, info=False)
     i1, i2 = s.step(40, float("inf"), w.cfl), t.step(40, float("inf"), w.cfl)
     assert i1 == i2 and i1["flags"] == 0 and i1["n_wet"] == w.n_cells
@@ -124,17 +124,17 @@ def test_config3_full_size_window(gpu, ref):
 
 def test_config5_8m_window_and_variants(gpu, ref):
     """BASELINE.json configs[4] at 8M cells: a 10-step window against the oracle on all cells, then a property that
-    holds at any size -- the two step variants (three-pass and fused patch, which share no kernel on the flux /
+    holds at any size -- the two step variants (fused patch = AUTO's choice, and three-pass, which share no kernel on the flux /
     update path) stay bit-identical over 300 steps -- and the volume balance of the transmissive domain."""
     w = C.config5()
     assert 7.8e6 < w.n_cells < 8.2e6
-    s = gpu.from_workload(w)                                           # AUTO, as bench.py runs it: all wet -> three-pass
-    assert s.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS
+    s = gpu.from_workload(w)                                           # AUTO, as bench.py runs it: the fused patch step
+    assert s.patch_stats()["variant"] == gpu.VARIANT_PATCH and s.patch_stats()["min_blocks_per_sm"] == 4
     o = ref.RefSolver(w)
     ig, io, _ = window(s, o, w, 10, "config5 8M, steps 0-10")
     check_info(ig, io)
     o.close()
-    t = gpu.from_workload(w, variant=gpu.VARIANT_PATCH)
+    t = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
     t.step(10, float("inf"), w.cfl, info=False)
     i1, i2 = s.step(300, float("inf"), w.cfl), t.step(300, float("inf"), w.cfl)
     assert i1 == i2 and i1["flags"] == 0 and i1["steps_done"] == 310

@@ -43,6 +43,11 @@ def both(gpu, ref, w, morph, chunks, n_species=0, **kw):
         qc0 = np.stack([w.h.copy()] + [rng.random(w.n_cells) * w.h for _ in range(n_species - 1)])
         s.set_scalars(qc0)
         o.set_scalars(qc0)
+        for sid, typ, _ in w.strings:                      # the water that enters carries phi = 1 of species 0 as well
+            if typ == C.BC_INFLOW_Q:
+                phi = [1.0] + [0.3] * (n_species - 1)
+                s.set_boundary_scalar(sid, phi)
+                o.set_boundary_scalar(sid, phi)
     s.set_morphology(*morph)
     o.set_morphology(*morph)
     identical = True

@@ -421,12 +421,19 @@ def test_dry_patches_are_skipped_and_rewetted(gpu, ref):
 
 
 def test_auto_picks_the_variant_from_the_wet_fraction(gpu, ref):
-    """AUTO keeps both step variants ready and picks one at every swe_set_state: the fused patch step while part of
-    the domain is dry, the three-pass step on (almost) all-wet states.  Switching is invisible in the results."""
+    """AUTO keeps both step variants ready and picks one at every swe_set_state.  With the default patch size four blocks
+    of the patch kernel fit an SM and it is the faster step at any wet fraction; with fatter blocks (here: 384-cell
+    patches, two per SM) the fused patch step runs while part of the domain is dry and the three-pass step on (almost)
+    all-wet states.  Switching is invisible in the results."""
     w4, w3 = CASES["config4-small"](), CASES["config3-small"]()
-    a = gpu.from_workload(w4, variant=gpu.VARIANT_AUTO, patch_cells=0)
-    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_patch_step"]   # self-controlled: one kernel per step
-    b = gpu.from_workload(w3, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    d = gpu.from_workload(w3, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    assert d.patch_stats()["variant"] == gpu.VARIANT_PATCH and d.step_kernels() == ["k_patch_step"]   # all wet, default patches; self-controlled: one kernel per step
+    assert d.patch_stats()["min_blocks_per_sm"] >= 4
+    d.close()
+    a = gpu.from_workload(w4, variant=gpu.VARIANT_AUTO, patch_cells=384)
+    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_patch_step"]
+    assert a.patch_stats()["min_blocks_per_sm"] < 4
+    b = gpu.from_workload(w3, variant=gpu.VARIANT_AUTO, patch_cells=384)
     assert b.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS and len(b.step_kernels()) == 4
     # odd number of steps (the patch step ping-pongs), then flood the river reach: AUTO switches to three-pass
     o = ref.RefSolver(w4)
@@ -456,7 +463,7 @@ def test_auto_follows_a_spreading_flood(gpu, ref):
     """AUTO re-evaluates its choice whenever swe_step returns info: a dam break that wets the whole (short) channel
     starts on the patch step and ends on the three-pass step, with the state equal to the oracle's throughout."""
     w = C.dam_break_channel(nx=120, ny=4, lx=24.0, ly=0.8, x_dam=8.0, t_end=20.0)
-    s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, patch_cells=0)
+    s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, patch_cells=384)      # fat patches: the wet-fraction rule applies
     o = ref.RefSolver(w)
     seen = [s.patch_stats()["variant"]]
     for _ in range(16):

@@ -147,7 +147,7 @@ def test_auto_switches_variant_with_scalars_on_board(gpu, ref):
     w = C.dam_break_channel(nx=120, ny=4, lx=24.0, ly=0.8, x_dam=8.0, t_end=20.0)
     x = M.centroids(w.node_xy, w.tri)[:, 0]
     qc0 = np.stack([np.where(x < 4.0, 1.0, 0.0) * w.h, 0.25 * w.h])
-    s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, n_species=2)
+    s = gpu.from_workload(w, variant=gpu.VARIANT_AUTO, n_species=2, patch_cells=384)   # fat patches: AUTO's wet-fraction rule applies
     o = ref.RefSolver(w)
     s.set_scalars(qc0)
     o.set_scalars(qc0)
