@@ -132,7 +132,9 @@ int swe_set_state(swe_ctx *ctx, const double *h, const double *hu, const double 
 
 /* Advances until n_steps steps are done (n_steps < 0: no limit) or t reaches t_end (+inf: no limit),
  * whichever comes first; the last step is shortened to land on t_end exactly.  cfl in (0, 1] (default
- * 0.9 in the paper).  All steps run on the device without host synchronisation per step; the call synchronises
+ * 0.9 in the paper).  With the literal rho_ij of Eq. 21 the first-order scheme is linearly stable only up to
+ * cfl ~ 0.75 on regular right-triangle meshes (bounded transverse noise above that: DESIGN.md R-7,
+ * tests/test_oracle_analytic.py::test_config1_noise_at_cfl_09_and_07); irregular Delaunay meshes run clean at 0.9.  All steps run on the device without host synchronisation per step; the call synchronises
  * the stream once per chunk of steps when t_end is finite, and once at the end if info != NULL.
  * info may be NULL.  Returns SWE_ENONFINITE if info was requested and the state holds NaN/inf. */
 int swe_step(swe_ctx *ctx, int64_t n_steps, double t_end, double cfl, swe_step_info *info);

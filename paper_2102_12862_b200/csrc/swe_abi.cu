@@ -776,10 +776,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       }
     }
     // algorithmic bytes per launch, every datum once (halo re-reads and duplicated edge records NOT counted):
-    // state in 32 + state out 32 + slot words 16 + area, 1/area, g/k^2 24 per cell; one 32-byte edge record per edge
+    // state in 32 + state out 32 + slot words 16 + area, g/k^2 16 per cell; 32 bytes of edge data per edge
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_PATCH];
     ab[0] = 0;
-    ab[1] = 104 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;        // + q_c in and out per species
+    ab[1] = 96 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;         // + q_c in and out per species
     // SURVEY.md section 8(d), one-pass column: 132 B per cell-step (+ 16 per species: q_c in and out)
     c->survey_bytes_v[SWE_VARIANT_PATCH][1] = (132 + 16 * (int64_t)c->sc.n) * nc;
   }
@@ -1096,7 +1096,7 @@ int swe_set_morphology(swe_ctx *c, int formula, double alpha, double theta_cr, d
     int64_t *ab = c->alg_bytes_v[SWE_VARIANT_THREE_PASS];
     ab[1] = c->alg_bytes_base[0] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
     ab[3] = c->alg_bytes_base[1] + (formula ? 8 * c->ne + (formula == 2 ? 16 * c->nc : 0) : 0);
-    if (c->has_patch) c->alg_bytes_v[SWE_VARIANT_PATCH][1] = 104 * c->nc + 32 * c->ne + (int64_t)c->sc.n * 16 * c->nc + (formula == 2 ? 8 * c->nc : 0);
+    if (c->has_patch) c->alg_bytes_v[SWE_VARIANT_PATCH][1] = 96 * c->nc + 32 * c->ne + (int64_t)c->sc.n * 16 * c->nc + (formula == 2 ? 8 * c->nc : 0);
   }
   c->edge_grid = c->base_edge_grid; c->cell_grid = c->base_cell_grid;
   if (formula) {                      // resident grids of the <kMorph> instances
