@@ -13,13 +13,17 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswe_b200.so")
-SRC = [os.path.join(CSRC, "swe_abi.cu")]
-DEPS = SRC + [os.path.join(CSRC, f) for f in ("swe_kernels.cuh", "swe_patch2_kernel.cuh", "swe_cbrt.cuh", "swe_types.h", "mesh_prep.hpp", "patch_blob.hpp")] + [
+OBJ = os.path.join(HERE, "build")
+# swe_abi.cu: the C-ABI and every kernel but the fused patch step; swe_patch_t*.cu: the instances of the fused patch kernel,
+# one translation unit per block size -- compiled in parallel (the kernel is ~5000 SASS instructions, ~50 instances)
+SRC = [os.path.join(CSRC, "swe_abi.cu")] + [os.path.join(CSRC, f"swe_patch_t{t}.cu") for t in (32, 64, 128, 192, 256, 384, 512, 1024)]
+DEPS = SRC + [os.path.join(CSRC, f) for f in ("swe_kernels.cuh", "swe_patch2_kernel.cuh", "swe_patch_inst.cuh", "swe_cbrt.cuh",
+                                              "swe_types.h", "mesh_prep.hpp", "patch_blob.hpp")] + [
     os.path.join(os.path.dirname(HERE), "include", "swe.h")]
 
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
-    "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "-shared",
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall",
 ]
 
 
@@ -31,8 +35,18 @@ def nvcc() -> str:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
-    subprocess.run(cmd, check=True)
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ, exist_ok=True)
+    objs = [os.path.join(OBJ, os.path.basename(s)[:-3] + ".o") for s in SRC]
+
+    def compile_one(pair):
+        src, obj = pair
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+        subprocess.run(cmd, check=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(SRC), os.cpu_count() or 4)) as pool:
+        list(pool.map(compile_one, zip(SRC, objs)))
+    subprocess.run([nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs, check=True)
     return LIB
 
 

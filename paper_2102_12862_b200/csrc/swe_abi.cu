@@ -20,7 +20,7 @@
 #include "mesh_prep.hpp"
 #include "patch_blob.hpp"
 #include "swe_kernels.cuh"
-#include "swe_patch2_kernel.cuh"
+#include "swe_patch_inst.cuh"
 #include "swe_types.h"
 
 using namespace swe;
@@ -94,16 +94,13 @@ inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
 
 // ---- the fused patch kernel's instantiations: one thread per own cell (P = threads), __launch_bounds__ minimum
 // blocks per SM chosen from what the shared memory admits (it only caps the registers)
-typedef void (*PatchKernel)(Control *, Patch2Args);
-struct PatchInst { int T, min_blocks; PatchKernel fn[2][2][2]; };   // T threads per block >= cells per patch; [scalars][self][morph]
-// self = 0: dt / stop rules from k_step_control; 1: every block derives them itself (no control kernel between steps)
-#define SWE_PK(P, B, S) {{k_patch2<P, B, S, false, false>, k_patch2<P, B, S, false, true>}, {k_patch2<P, B, S, true, false>, k_patch2<P, B, S, true, true>}}
-#define SWE_PI(P, B) {P, B, {SWE_PK(P, B, false), SWE_PK(P, B, true)}}
-const PatchInst kPatchInst[] = {SWE_PI(32, 8), SWE_PI(64, 8), SWE_PI(128, 6), SWE_PI(128, 4), SWE_PI(192, 4), SWE_PI(192, 3),
-                                SWE_PI(256, 4), SWE_PI(256, 3), SWE_PI(256, 2), SWE_PI(384, 2), SWE_PI(384, 1), SWE_PI(512, 1),
-                                SWE_PI(1024, 1)};
-#undef SWE_PI
-#undef SWE_PK
+// (T threads per block >= cells per patch, __launch_bounds__ minimum blocks per SM, getter of the instance for
+// [scalars][self-controlled][mobile bed]; the instances live in swe_patch_t*.cu, one translation unit per block size)
+struct PatchInst { int T, min_blocks; PatchKernel (*get)(int B, int scalars, int self, int morph); };
+const PatchInst kPatchInst[] = {{32, 8, patch_kernel_32}, {64, 8, patch_kernel_64}, {128, 6, patch_kernel_128}, {128, 4, patch_kernel_128},
+                                {192, 4, patch_kernel_192}, {192, 3, patch_kernel_192}, {256, 4, patch_kernel_256}, {256, 3, patch_kernel_256},
+                                {256, 2, patch_kernel_256}, {384, 2, patch_kernel_384}, {384, 1, patch_kernel_384}, {512, 1, patch_kernel_512},
+                                {1024, 1, patch_kernel_1024}};
 
 inline int patch_threads(int P) {           // the smallest block size of an instance that gives every own cell a thread
   int T = 1 << 30;
@@ -232,7 +229,7 @@ const char *const kThreePassNames[4] = {"k_step_control", "k_edge_flux", "k_thet
 const char *const kPatchNames[2] = {"k_step_control", "k_patch_step"};
 const char *const kSelfNames[1] = {"k_patch_step"};
 
-inline bool self_mode(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH && c->self_ctl && !c->single; }
+inline bool self_mode(const swe_ctx *c) { return c->variant == SWE_VARIANT_PATCH && c->self_ctl && !c->single && c->mp.formula == 0; }
 inline int n_step_kernels(const swe_ctx *c) { return self_mode(c) ? 1 : (c->variant == SWE_VARIANT_PATCH ? 2 : 4); }
 
 Patch2Args patch_args(const swe_ctx *c) {
@@ -288,8 +285,12 @@ void enqueue_three_pass_f32(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev) {
 void launch_patch(swe_ctx *c, cudaStream_t s, int self) {
   const int morph = c->mp.formula;
   const size_t smem = (size_t)patch2_smem_layout(c->blay, c->sc.n, morph, self != 0).total;
-  const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, c->patch_force_blocks);   // most blocks per SM that fit
-  pi->fn[c->sc.n > 0][self][morph != 0]<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
+  // most blocks per SM that fit -- unless the grid cannot fill them: then the instance with the larger register budget
+  // (76 instead of 64 registers at 256 threads) is the faster one per block (configs[1]: 10.4 vs 11.8 us per step)
+  int force = c->patch_force_blocks;
+  if (!force && c->patch_threads == 256 && c->n_patches <= 3 * c->sms) force = 3;
+  const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, force);
+  pi->get(pi->min_blocks, c->sc.n > 0, self, morph != 0)<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
 }
 
 // one time step, in stream order.  Self-controlled patch step: the launch number decides the control slot it reads
@@ -575,7 +576,8 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
     // a numbering that is not spatially compact (renumber = NONE on a scattered input order) blows the halos up:
     // more than 2.2 local cells per own cell, or a block that no longer fits an SM twice -> AUTO falls back to the
     // three-pass step (round 1: such patches were 2-3x slower than the three-pass step)
-    const bool bloated = (double)pl.pb.sum_loc > 2.2 * (double)nc || pl.patch_smem + kSmemBlockReserve > kSmemPerSM / 2;
+    // (small patches of small meshes have fat halos by geometry: 2.5 local cells per own cell at 32 cells)
+    const bool bloated = (double)pl.pb.sum_loc > (P >= 192 ? 2.2 : 4.5) * (double)nc || pl.patch_smem + kSmemBlockReserve > kSmemPerSM / 2;
     if (pl.patch_smem > kSmemPerBlockMax || (p.variant == SWE_VARIANT_AUTO && bloated)) {
       if (p.variant == SWE_VARIANT_AUTO) { pl.variant = SWE_VARIANT_THREE_PASS; pl.pb = PatchBlobs{}; pl.patch_smem = 0; }
       else { err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }
@@ -745,7 +747,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       const int64_t cap = std::min<int64_t>(1024, (int64_t)pb.lay.cap_e + 3 * (int64_t)pb.lay.cap_eown);
       // (it saves the control kernel's graph node, 2.3-2.6 us per step: + 20-30 % on meshes up to ~100k cells, nothing
       // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2_self_ctl.md)
-      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= 8192;
+      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= 8192 && c->sc.n == 0;
       for (const BoundaryString &bs : c->strings) ok = ok && bs.pow2 <= cap;
       if (const char *s = std::getenv("SWE_PATCH_SELF")) ok = ok && std::atoi(s) != 0;
       c->self_ctl = ok;
@@ -767,7 +769,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       for (const PatchInst &pi : kPatchInst) {
         if (pi.T != c->patch_threads) continue;
         for (int a = 0; a < 8; ++a) {
-          PatchKernel fn = pi.fn[a & 1][(a >> 1) & 1][(a >> 2) & 1];
+          PatchKernel fn = pi.get(pi.min_blocks, a & 1, (a >> 1) & 1, (a >> 2) & 1);
+          if (!fn) continue;
           SWE_CUDA(c, cudaFuncGetAttributes(&fa, fn));
           const int limit = optin - (int)fa.sharedSizeBytes;
           if ((int)smem_max > limit) { c->err = "patch needs more shared memory than an SM has: lower patch_cells or renumber"; return SWE_EINVAL; }

@@ -289,7 +289,7 @@ k_edge_flux(const Control *__restrict__ ctl, const EdgeGeomT<T> *__restrict__ ge
 // ---------------------------------------------------------------------------------------------------------
 // S1c (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1 of cell i)), slots in order.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_theta(const Control *__restrict__ ctl, const int4 *__restrict__ cell_edge, const EdgeGeom *__restrict__ geom,
         const EdgeFlux *__restrict__ flux, const CellRec *__restrict__ rec, const double *__restrict__ area,
         double *__restrict__ theta, int n_cells, int force) {
@@ -746,7 +746,7 @@ k_step_control(Control *ctl, BoundaryString *strings, const int *__restrict__ st
 }
 
 // AUTO variant choice at swe_set_state: number of cells with h > h_dry in the caller's array
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_count_wet(Control *__restrict__ ctl, const double *__restrict__ h, int n_cells) {
   long long wet = 0;
   const double h_dry = ctl->h_dry;
@@ -757,21 +757,21 @@ k_count_wet(Control *__restrict__ ctl, const double *__restrict__ h, int n_cells
 }
 
 // switches the step variant (both compute bit-identical states): the three-pass step works in place in buffer a
-__global__ void k_set_variant(Control *ctl, int ping_pong, int zero_wet) {
+static __global__ void k_set_variant(Control *ctl, int ping_pong, int zero_wet) {
   if (zero_wet) { ctl->n_wet = 0; return; }
   ctl->ping_pong = ping_pong;
   if (!ping_pong) { ctl->cur = 0; ctl->src = 0; }
 }
 
 // start of an swe_step call: the stop conditions of this call
-__global__ void k_call_begin(Control *ctl, long long n_steps, double t_end, double cfl) {
+static __global__ void k_call_begin(Control *ctl, long long n_steps, double t_end, double cfl) {
   ctl->steps_left = n_steps;
   ctl->t_end = t_end;
   ctl->cfl = cfl;
   ctl->flags &= ~(kFlagUnbounded | kFlagStalled);
 }
 
-__global__ void k_reset(Control *ctl, double t0) {
+static __global__ void k_reset(Control *ctl, double t0) {
   ctl->t = t0; ctl->dt = 0.0; ctl->dt_last = 0.0;
   ctl->vol_in = 0.0; ctl->vol_out = 0.0; ctl->vol_clipped = 0.0;
   ctl->rate_bits = 0ull; ctl->steps_left = 0; ctl->steps_done = 0;
@@ -858,7 +858,7 @@ k_unpack_state(const Control *__restrict__ ctl, const int *__restrict__ cell_per
 }
 
 // Morph::cell of the state as it stands (after swe_set_morphology / swe_set_state): what k_cell_update leaves behind
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_sed_cell_init(const Control *__restrict__ ctl, const CellRec *__restrict__ rec, const double *__restrict__ gn2,
                 double2 *__restrict__ cell, int n_cells) {
   const int i = blockIdx.x * kBlock + threadIdx.x;
@@ -868,7 +868,7 @@ k_sed_cell_init(const Control *__restrict__ ctl, const CellRec *__restrict__ rec
 }
 
 // both record buffers of the fused patch step hold the bed of the newest state (swe_set_morphology)
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_sync_bed(const Control *__restrict__ ctl, CellRec *rec_a, CellRec *rec_b, int n_cells) {
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= n_cells) return;
@@ -876,7 +876,7 @@ k_sync_bed(const Control *__restrict__ ctl, CellRec *rec_a, CellRec *rec_b, int 
 }
 
 // bed elevation z_B (swe_get_bed), newest state buffer, caller numbering
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_unpack_bed(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const CellRec *rec_a,
              const CellRec *rec_b, double *__restrict__ zb, int n_cells) {
   const CellRec *__restrict__ rec = ctl->cur ? rec_b : rec_a;
@@ -885,21 +885,21 @@ k_unpack_bed(const Control *__restrict__ ctl, const int *__restrict__ cell_perm,
 }
 
 // q_Bij of the most recent step in caller edge numbering (swe_get_sediment_flux); the sign follows the caller's L -> R
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_export_sediment(const int *__restrict__ edge_perm, const double *__restrict__ qB, double *__restrict__ out, int n_edges) {
   const int e = blockIdx.x * kBlock + threadIdx.x;
   if (e < n_edges) out[edge_perm[e]] = qB[e];
 }
 
 // one scalar species, caller numbering <-> internal numbering, newest state buffer
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_pack_scalar(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *__restrict__ src,
               double *qa, double *qb, int n_cells) {
   const int i = blockIdx.x * kBlock + threadIdx.x;
   if (i < n_cells) (ctl->cur ? qb : qa)[i] = src[cell_perm[i]];
 }
 
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_unpack_scalar(const Control *__restrict__ ctl, const int *__restrict__ cell_perm, const double *qa, const double *qb,
                 double *__restrict__ dst, int n_cells) {
   const int i = blockIdx.x * kBlock + threadIdx.x;
@@ -907,7 +907,7 @@ k_unpack_scalar(const Control *__restrict__ ctl, const int *__restrict__ cell_pe
 }
 
 // inspection (swe_device_cbrt): the cube root of R-14 as the kernels evaluate it
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_cbrt(const double *__restrict__ x, double *__restrict__ y, long long n) {
   const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
   if (i < n) y[i] = cbrt_rn(x[i]);

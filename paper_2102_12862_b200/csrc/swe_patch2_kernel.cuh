@@ -155,7 +155,7 @@ __device__ __forceinline__ double book_outflow(const StepSlot &S, const Boundary
 }
 
 // start of an swe_step call in self-controlled mode: the classic fields -> slot[k0]
-__global__ void k_self_begin(Control *ctl, long long n_steps, double t_end, double cfl, int k0) {
+static __global__ void k_self_begin(Control *ctl, long long n_steps, double t_end, double cfl, int k0) {
   ctl->steps_left = n_steps; ctl->t_end = t_end; ctl->cfl = cfl;
   ctl->flags &= ~(kFlagUnbounded | kFlagStalled);
   StepSlot S;
@@ -620,7 +620,7 @@ k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
   }
 }
 
-__global__ void __launch_bounds__(kBlock)
+static __global__ void __launch_bounds__(kBlock)
 k_patch2_nbr_flags(const Control *__restrict__ ctl, const Patch2Args A, int n_patches) {
   const int p = blockIdx.x * kBlock + threadIdx.x;
   if (p >= n_patches) return;

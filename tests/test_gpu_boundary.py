@@ -62,36 +62,52 @@ def test_too_small_workspace_is_refused_and_nothing_leaks(gpu):
     w = C.by_id(3, 0.02)
     need = gpu.workspace_bytes(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
     gpu.from_workload(w).close()
-    torch.cuda.empty_cache()
-    f0 = free_bytes()
-    for short in (256, need // 2):
-        with pytest.raises(gpu.SweError) as ei:
-            gpu.from_workload(w, workspace_bytes=need - short)
-        assert ei.value.code == gpu.ENOMEM and "workspace too small" in str(ei.value)
-    torch.cuda.empty_cache()
-    assert abs(free_bytes() - f0) < (4 << 20)
+
+    def refused(n):
+        for _ in range(n):
+            for short in (256, need // 2):
+                with pytest.raises(gpu.SweError) as ei:
+                    gpu.from_workload(w, workspace_bytes=need - short)
+                assert ei.value.code == gpu.ENOMEM and "workspace too small" in str(ei.value)
+        torch.cuda.empty_cache()
+        return free_bytes()
+
+    f1 = refused(1)
+    f8 = refused(8)
+    assert abs(f8 - f1) < (1 << 20)                           # eight more refusals: not a byte less free memory
     s = gpu.from_workload(w, workspace_bytes=need)            # exactly enough: fine
     s.step(10, float("inf"), w.cfl)
     s.close()
 
 
 def test_create_that_fails_half_way_leaves_nothing_behind(gpu):
-    """A patch that needs more shared memory than an SM has is only found out after the workspace is carved and
-    the tables are uploaded (own workspace: after the library's one cudaMalloc): SWE_EINVAL, and the memory is back."""
+    """swe_create with its own allocation on a device that has too little memory left: the one cudaMalloc fails after
+    the host planning is done -> SWE_ENOMEM, and repeating it does not eat memory (pinned control block, context).
+    A mesh the host part refuses never reaches the device."""
     import torch
-    w = C.by_id(3, 0.02)
+    w = C.by_id(3, 0.1)                                        # ~100k cells: ~40 MB
+    need = gpu.workspace_bytes(w.node_xy, w.tri, w.edge_cell, w.cell_edge, w.zb, w.kst)
     gpu.from_workload(w).close()
     torch.cuda.empty_cache()
-    f0 = free_bytes()
-    for own in (False, True):
-        with pytest.raises(gpu.SweError) as ei:
-            gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=1024, own_workspace=own)
-        assert ei.value.code == gpu.EINVAL and "shared memory" in str(ei.value)
-    # a mesh the host part refuses (clockwise cell): no workspace is even sized
+    hog = torch.empty(free_bytes() - need // 4, dtype=torch.uint8, device="cuda")     # leave a quarter of what is needed
+
+    def refused(n):
+        for _ in range(n):
+            with pytest.raises(gpu.SweError) as ei:
+                gpu.from_workload(w, own_workspace=True)
+            assert ei.value.code == gpu.ENOMEM and "device memory" in str(ei.value)
+        return free_bytes()
+
+    f1 = refused(1)
+    f6 = refused(6)
+    assert abs(f6 - f1) < (1 << 20)
+    del hog
+    torch.cuda.empty_cache()
+    s = gpu.from_workload(w, own_workspace=True)               # with the memory back the same call succeeds
+    s.step(5, float("inf"), w.cfl)
+    s.close()
     bad = w.tri.copy()
-    bad[5] = bad[5][::-1]
+    bad[5] = bad[5][::-1]                                      # a clockwise cell: refused by the host part
     with pytest.raises(gpu.SweError) as ei:
         gpu.Solver(w.node_xy, bad, None, None, w.zb, w.kst)
     assert ei.value.code == gpu.EMESH
-    torch.cuda.empty_cache()
-    assert abs(free_bytes() - f0) < (4 << 20)
