@@ -34,6 +34,9 @@ constexpr int kFlagUnbounded = 2, kFlagStalled = 4;
 // min / max of finite doubles as one compare + select (fmin / fmax also order NaNs and signed zeros, which costs
 // several more instructions; here a zero of either sign leads to the same branch and the same values)
 template <typename T> __device__ __forceinline__ T dmax0(T x) { return x > T(0.0) ? x : T(0.0); }
+// fp64: the compiler turns the line above into its fmax sequence (DSETP.MAX + NaN quieting, ~7 instructions); a test of
+// the sign bit gives the same value for every x that is not a NaN (-0 and negatives -> +0) in 3
+template <> __device__ __forceinline__ double dmax0<double>(double x) { return __double2hiint(x) < 0 ? 0.0 : x; }
 template <typename T> __device__ __forceinline__ T dmin2(T a, T b) { return a < b ? a : b; }
 template <typename T> __device__ __forceinline__ T dmax2(T a, T b) { return a > b ? a : b; }
 

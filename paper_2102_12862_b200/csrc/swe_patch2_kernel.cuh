@@ -258,7 +258,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   {
     const ulonglong2 w0 = src ? fb0 : fa0, w1 = src ? fb1 : fa1;
     if (w0.x == ones && w0.y == ones && w1.x == ones && w1.y == ones) {
-      const unsigned char had = pf_out_base[(size_t)b * kPflagBytes + kPflagOwn];
+      // the own flag of the word this patch has in the buffer being written: loaded above with everything else
+      const ulonglong2 o1 = src ? fa1 : fb1;
+      const unsigned char had = (unsigned char)((o1.y >> (8 * (kPflagOwn - 24))) & 0xffull);
       if (!had) {
         if (tid < n_own) {
           CellRec c = in[cell0 + tid];
@@ -525,14 +527,13 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       double th = 1.0;
       if (F1 > 0.0) th = sh_th[isL ? (uint32_t)l : nb];
       else if (F1 < 0.0 && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
-      if (th < 1.0) { F1 = th * F1; F3 = th * F3; G = th * G; }
-      const double s = isL ? 1.0 : -1.0;
+      F1 = th * F1; F3 = th * F3; G = th * G;       // theta = 1: the product is the factor itself, bit for bit
       const double nxk = b_nx[e], nyk = b_ny[e], lenk = b_len[e];
-      const double dHk = s * (lenk * F1);
-      const double dXk = s * (lenk * (G * nxk - F3 * nyk));
-      const double dYk = s * (lenk * (G * nyk + F3 * nxk));
+      // s * x with s = +-1 is x or -x exactly: a change of sign instead of a product
+      const double dH0 = lenk * F1, dX0 = lenk * (G * nxk - F3 * nyk), dY0 = lenk * (G * nyk + F3 * nxk);
+      const double dHk = isL ? dH0 : -dH0, dXk = isL ? dX0 : -dX0, dYk = isL ? dY0 : -dY0;
       if (k == 0) { dH = dHk; dX = dXk; dY = dYk; } else { dH = dH + dHk; dX = dX + dXk; dY = dY + dYk; }
-      if (kMorph) { const double dBk = s * (lenk * sh_qB[e]); dB = k == 0 ? dBk : dB + dBk; }
+      if (kMorph) { const double dB0 = lenk * sh_qB[e]; const double dBk = isL ? dB0 : -dB0; dB = k == 0 ? dBk : dB + dBk; }
       if (kScalars) {
         F1k[k] = F1; slk[k] = lenk;
         const uint32_t Lc = isL ? (uint32_t)l : nb, Rc = isL ? nb : (uint32_t)l;
