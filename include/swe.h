@@ -223,6 +223,34 @@ int64_t swe_survey_bytes(const swe_ctx *ctx, int k);
  * staged into shared memory.  It synchronises. */
 int swe_get_patch_stats(swe_ctx *ctx, int64_t *out, int n_out);
 
+/* ---- an entry point that allocates nothing -----------------------------------------------------------------
+ * The reductions of swe_step_info (vol = sum_i h_i |Omega_i|, the quantity whose conservation P:591 promises; n_wet =
+ * cells with h > h_dry, R-8; non-finite check) of a state given as plain arrays, for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  It needs no context and no
+ * workspace: the per-block partial results and the ticket that swe_step keeps in the context's workspace live in a
+ * file-scope __device__ array of 98,560 bytes, which every GPU that loads the library holds until the process exits.
+ * It calls no cudaMalloc / cudaFree / allocating routine, does not synchronise, and enqueues one 4-byte memset and one
+ * kernel on `cuda_stream` (NULL = the legacy default stream) of the CURRENT device.
+ *   h, hu, hv, area : DEVICE pointers, [n_cells] doubles each, read only; any cell numbering (the same in all four)
+ *   n_cells         : 1 .. SWE_SUMMARY_STATIC_MAX_CELLS; beyond that SWE_EINVAL (the array holds one partial per 4096
+ *                     cells) and swe_last_error(NULL) names the limit -- use swe_step's info for larger meshes
+ *   out             : DEVICE pointer to one swe_state_summary, written by the kernel (valid once the stream has
+ *                     reached that point); owned by the caller
+ * vol is summed in a fixed order (independent of scheduling): the same inputs give the same bits; it differs from
+ * swe_step_info.vol, which sums in the library's internal numbering, by rounding only (<= 1e-12 relative).
+ * ALL calls share the one array per GPU: calls that overlap on the GPU (two streams, two host threads) race on it and
+ * give wrong sums -- the caller serialises them.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress); make that first call outside graph capture. */
+#define SWE_SUMMARY_STATIC_MAX_CELLS 16777216 /* 2^24 */
+typedef struct {
+  double vol;        /* sum_i h_i |Omega_i|                */
+  int64_t n_wet;     /* cells with h > h_dry                */
+  int32_t nonfinite; /* 1 if any h, hu or hv is inf or NaN  */
+  int32_t pad_;
+} swe_state_summary;
+int swe_state_summary_static(const double *h, const double *hu, const double *hv, const double *area, int64_t n_cells,
+                             double h_dry, void *cuda_stream, swe_state_summary *out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -39,7 +39,7 @@ EXPORTS = (
     "swe_get_permutation", "swe_get_tables", "swe_device_cbrt", "swe_kernel_launches", "swe_profile_step",
     "swe_step_kernel_count", "swe_step_kernel_name", "swe_algorithmic_bytes", "swe_survey_bytes", "swe_get_patch_stats",
     "swe_set_scalars", "swe_get_scalars", "swe_set_boundary_scalar", "swe_host_preprocess",
-    "swe_set_morphology", "swe_get_bed", "swe_get_sediment_flux",
+    "swe_set_morphology", "swe_get_bed", "swe_get_sediment_flux", "swe_state_summary_static",
 )
 
 
@@ -119,6 +119,7 @@ def lib():
         L.swe_set_morphology.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 5
         L.swe_get_bed.argtypes = [C.c_void_p, C.c_void_p]
         L.swe_get_sediment_flux.argtypes = [C.c_void_p, C.c_void_p]
+        L.swe_state_summary_static.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_double, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -396,6 +397,28 @@ def device_cbrt(x):
     if rc != OK:
         raise SweError(rc, lib().swe_last_error(None).decode())
     return y
+
+
+SUMMARY_STATIC_MAX_CELLS = 1 << 24   # include/swe.h SWE_SUMMARY_STATIC_MAX_CELLS
+
+
+def state_summary_static(h, hu, hv, area, h_dry, out, n_cells=None, stream=None):
+    """swe_state_summary_static: volume, wet-cell count and non-finite check of a state, with no allocation (the scratch
+    is a static device array inside the library; calls must not overlap on the GPU).  h, hu, hv, area: CUDA float64
+    tensors (or integer device addresses, then n_cells is required); out: a CUDA tensor of 24 bytes that receives
+    (vol: f64, n_wet: i64, nonfinite: i32, pad: i32); stream: cudaStream_t as an integer (None: torch's current one).
+    Nothing is copied or synchronised here: read `out` after the stream has run."""
+    def ptr(x):
+        return int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x)
+    if n_cells is None:
+        n_cells = int(h.numel())
+    if stream is None:
+        import torch  # stream handle only
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = lib().swe_state_summary_static(ptr(h), ptr(hu), ptr(hv), ptr(area), int(n_cells), float(h_dry), int(stream) or None,
+                                        ptr(out))
+    if rc != OK:
+        raise SweError(rc, lib().swe_last_error(None).decode())
 
 
 def from_workload(w, **kw):

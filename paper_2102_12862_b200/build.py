@@ -14,9 +14,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswe_b200.so")
 OBJ = os.path.join(HERE, "build")
-# swe_abi.cu: the C-ABI and every kernel but the fused patch step; swe_patch_t*.cu: the instances of the fused patch kernel,
+# swe_abi.cu: the C-ABI and every kernel but the fused patch step; swe_static.cu: the entry point that allocates nothing; swe_patch_t*.cu: the instances of the fused patch kernel,
 # one translation unit per block size -- compiled in parallel (the kernel is ~5000 SASS instructions, ~50 instances)
-SRC = [os.path.join(CSRC, "swe_abi.cu")] + [os.path.join(CSRC, f"swe_patch_t{t}.cu") for t in (32, 64, 128, 192, 256, 384, 512, 1024)]
+SRC = [os.path.join(CSRC, "swe_abi.cu"), os.path.join(CSRC, "swe_static.cu")] + [os.path.join(CSRC, f"swe_patch_t{t}.cu") for t in (32, 64, 128, 192, 256, 384, 512, 1024)]
 DEPS = SRC + [os.path.join(CSRC, f) for f in ("swe_kernels.cuh", "swe_patch2_kernel.cuh", "swe_patch_inst.cuh", "swe_cbrt.cuh",
                                               "swe_types.h", "mesh_prep.hpp", "patch_blob.hpp")] + [
     os.path.join(os.path.dirname(HERE), "include", "swe.h")]

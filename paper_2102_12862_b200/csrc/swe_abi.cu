@@ -832,6 +832,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
 }  // namespace
 
 // =========================================================================================================
+// the message swe_last_error(NULL) returns on this thread, for entry points that live in another translation unit
+// (swe_static.cu)
+namespace swe { void set_thread_error(const char *msg) { g_create_error = msg ? msg : ""; } }
+
 extern "C" {
 
 void swe_params_default(swe_params *p) {
