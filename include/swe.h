@@ -43,9 +43,10 @@ enum { SWE_EDGE_WALL = -1, SWE_EDGE_TRANSMISSIVE = -2 /* , -3 - s = member of bo
 enum { SWE_BC_NONE = 0 /* string behaves as wall */, SWE_BC_INFLOW_Q = 1, SWE_BC_OUTFLOW_UNIFORM = 2 };
 /* Cell / edge renumbering applied inside the library (invisible at this boundary) */
 enum { SWE_RENUMBER_NONE = 0, SWE_RENUMBER_MORTON = 1, SWE_RENUMBER_RCM = 2 /* reverse Cuthill-McKee */ };
-/* Step variant: both compute bit-identical states.  AUTO keeps both ready and chooses at every
- * swe_set_state from the wet fraction of the new state (fused patch step while part of the domain is dry, three-pass
- * step on all-wet states); on a numbering that is not spatially compact it is the three-pass step. */
+/* Step variant: both compute bit-identical states.  AUTO keeps both ready: the fused patch step
+ * whenever four of its blocks fit an SM (the faster variant at every wet fraction then); with
+ * larger patches it chooses at every swe_set_state from the wet fraction of the new state (patch step below 50 % wet
+ * cells, three-pass step above); on a numbering that is not spatially compact it is the three-pass step. */
 enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta -> CSR gather + update */,
        SWE_VARIANT_PATCH = 2 /* one fused kernel per step over shared-memory mesh patches */ };
 /* Arithmetic ("single or double"; R-21).  SINGLE: state, geometry and every flux / update operation in
