@@ -100,6 +100,9 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
   // ---- pass 2: the blobs
   const BlobLayout &L = pb.lay;
   pb.bytes.assign((size_t)L.stride * (size_t)np, 0);
+  // own_mask[c]: bit j is set when cell c (owned by patch p = c / P) is a halo cell of the j-th neighbour patch of p
+  // (j < 32): what p must look at to tell that neighbour "none of MY cells YOU read holds water" (the flag bytes)
+  std::vector<uint32_t> own_mask(nc, 0u);
   for (int64_t p = 0; p < np; ++p) {
     discover(p, (int32_t)(np + p), s);
     unsigned char *B = pb.bytes.data() + (size_t)L.stride * (size_t)p;
@@ -128,6 +131,14 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
     std::memcpy(B + L.off_stage + L.s_nbr_slot, nbr_slot, 4 * (size_t)L.cap_nbr);
     int32_t *halo_ids = (int32_t *)(B + L.off_halo_ids);
     for (int32_t j = 0; j < L.cap_halo; ++j) halo_ids[j] = j < (int32_t)s.ring.size() ? s.ring[j] : -1;
+    for (int32_t c : s.ring) {                    // this patch p reads cell c of patch o: bit (position of p in o's list)
+      const int32_t o = c / P;
+      const int32_t *ob = nbr_all.data() + nbr_off[o], *oe = nbr_all.data() + nbr_off[o + 1];
+      const int32_t *it = std::lower_bound(ob, oe, (int32_t)p);
+      if (it == oe || *it != (int32_t)p) { err = "patch neighbourhood is not symmetric"; return false; }
+      const int32_t j = (int32_t)(it - ob);
+      if (j < 32) own_mask[c] |= 1u << j;
+    }
     unsigned char *S = B + L.off_stage;
     double *halo_area = (double *)(S + L.s_halo_area);
     for (int32_t j = 0; j < s.n_r1; ++j) halo_area[j] = area[s.ring[j]];
@@ -157,6 +168,12 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
     double *a = (double *)(S + L.s_area), *g2 = (double *)(S + L.s_gn2);
     for (int32_t l = 0; l < s.n_own; ++l) { a[l] = area[c0 + l]; g2[l] = gn2[c0 + l]; }
     (void)inv_area;
+  }
+  // the fourth word of an own cell's slot record: its mask (complete only now that every patch has been visited)
+  for (int64_t p = 0; p < np; ++p) {
+    uint32_t *pce = (uint32_t *)(pb.bytes.data() + (size_t)L.stride * (size_t)p + L.off_stage + L.s_pce);
+    const int32_t c0 = (int32_t)(p * P), n_own = (int32_t)std::min<int64_t>(P, nc - c0);
+    for (int32_t l = 0; l < n_own; ++l) pce[4 * l + 3] = own_mask[c0 + l];
   }
   return true;
 }

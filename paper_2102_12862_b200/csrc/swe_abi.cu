@@ -251,7 +251,7 @@ Patch2Args patch_args(const swe_ctx *c) {
 void launch_patch_flags(swe_ctx *c) {
   const Patch2Args a = patch_args(c);
   k_patch2_own_flags<256><<<c->n_patches, 256, 0, c->stream>>>(c->d_ctl, a);
-  k_patch2_nbr_flags<<<grid_for(c->n_patches), kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
+  k_patch2_nbr_flags<<<c->n_patches, kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
   c->launches += 2;
 }
 
@@ -747,7 +747,9 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       const int64_t cap = std::min<int64_t>(1024, (int64_t)pb.lay.cap_e + 3 * (int64_t)pb.lay.cap_eown);
       // (it saves the control kernel's graph node, 2.3-2.6 us per step: + 20-30 % on meshes up to ~100k cells, nothing
       // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2_self_ctl.md)
-      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= 8192 && c->sc.n == 0;
+      const char *self_env = std::getenv("SWE_PATCH_SELF");           // measurement runs: 0 never, 2 on any mesh size
+      const int self_max_patches = (self_env && std::atoi(self_env) == 2) ? (1 << 30) : 8192;
+      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= self_max_patches && c->sc.n == 0;
       for (const BoundaryString &bs : c->strings) ok = ok && bs.pow2 <= cap;
       if (const char *s = std::getenv("SWE_PATCH_SELF")) ok = ok && std::atoi(s) != 0;
       c->self_ctl = ok;

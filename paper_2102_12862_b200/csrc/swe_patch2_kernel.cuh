@@ -107,13 +107,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
 }
 
 // own flag + the byte this patch has in each neighbour's flag word (nbr / nbr_slot: cap_nbr entries, -1 padded)
+// dirty: bit j set = an own cell that the j-th neighbour reads is not (0, 0, 0) (j < 32; beyond: the own flag decides)
 template <int kThreads>
 __device__ __forceinline__ void publish_flag(unsigned char *pf_out_base, int b, const int32_t *nbr, const int32_t *nbr_slot,
-                                             int cap_nbr, unsigned char flag) {
+                                             int cap_nbr, unsigned char flag, uint32_t dirty = 0u) {
   if (threadIdx.x == 0) pf_out_base[(size_t)b * kPflagBytes + kPflagOwn] = flag;
   for (int j = threadIdx.x; j < cap_nbr; j += kThreads) {
     const int q = nbr[j], sl = nbr_slot[j];
-    if (q >= 0 && sl >= 0) pf_out_base[(size_t)q * kPflagBytes + sl] = flag;
+    if (q >= 0 && sl >= 0) pf_out_base[(size_t)q * kPflagBytes + sl] = j < 32 ? (unsigned char)(((dirty >> j) & 1u) ^ 1u) : flag;
   }
 }
 
@@ -288,7 +289,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   const int cap_loc = L.cap_loc;
 
   // ---- the two bulk copies: staged part of the blob, own cell records
+  uint32_t *sm_dirty = reinterpret_cast<uint32_t *>(smraw + 16);   // neighbours that read a wet own cell (phase 4)
   if (tid == 0) {
+    *sm_dirty = 0u;
     mbar_init(bar, 1);
     mbar_expect_tx(bar, (uint32_t)L.stage_bytes + 32u * (uint32_t)n_own);
     bulk_g2s(stage, blob + L.off_stage, (uint32_t)L.stage_bytes, bar);
@@ -595,14 +598,20 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       }
     }
   }
+  // which neighbour patches read an own cell that is not (0, 0, 0): OR of the masks (fourth word of the slot record)
+  {
+    const uint32_t mine = (nonzero && tid < n_own) ? reinterpret_cast<const uint32_t *>(b_pce)[4 * tid + 3] : 0u;
+    const uint32_t warp_dirty = __reduce_or_sync(0xffffffffu, mine);
+    if ((tid & 31) == 0 && warp_dirty) atomicOr(sm_dirty, warp_dirty);
+  }
   nonzero = __syncthreads_or(nonzero);
   publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(stage + L.s_nbr), (const int32_t *)(stage + L.s_nbr_slot), L.cap_nbr,
-                         nonzero ? 0 : 1);
+                         nonzero ? 0 : 1, *sm_dirty);
   block_max_to_global<kThreads>(rate, kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits);
 }
 
 // flags after swe_set_state, two launches: (1) own flag of the buffer that holds the newest state from the records
-// (the other buffer: unknown = 0); (2) every patch collects its neighbours' own flags into its word
+// (the other buffer: unknown = 0); (2) every patch works out its neighbour bytes from its halo cells
 template <int kThreads>
 __global__ void __launch_bounds__(kThreads)
 k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
@@ -621,23 +630,42 @@ k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
   }
 }
 
+// one block per patch: neighbour byte j = 1 when every halo cell of this patch that the j-th neighbour owns is
+// (0, 0, 0) (and carries no scalar mass) in the newest state; the other buffer: unknown = 0
 static __global__ void __launch_bounds__(kBlock)
 k_patch2_nbr_flags(const Control *__restrict__ ctl, const Patch2Args A, int n_patches) {
-  const int p = blockIdx.x * kBlock + threadIdx.x;
+  const int p = blockIdx.x;
   if (p >= n_patches) return;
+  __shared__ uint32_t s_dirty;
   const unsigned char *blob = A.blob + (size_t)p * (size_t)A.L.stride;
   const BlobHeader H = *reinterpret_cast<const BlobHeader *>(blob);
   const int32_t *nbr = (const int32_t *)(blob + A.L.off_nbr);
-  unsigned char *cur = (ctl->cur ? A.pflag_b : A.pflag_a), *oth = (ctl->cur ? A.pflag_a : A.pflag_b);
-  for (int j = 0; j < kPflagSlots; ++j) {
-    unsigned char f = 1, fo = 1;                  // unused slots never veto
-    if (j < H.n_nbr) { f = cur[(size_t)nbr[j] * kPflagBytes + kPflagOwn]; fo = 0; }
-    cur[(size_t)p * kPflagBytes + j] = f;
-    oth[(size_t)p * kPflagBytes + j] = fo;
+  const int32_t *halo_ids = (const int32_t *)(blob + A.L.off_halo_ids);
+  const CellRec *__restrict__ rec = ctl->cur ? A.rec_b : A.rec_a;
+  if (threadIdx.x == 0) s_dirty = 0u;
+  __syncthreads();
+  for (int l = threadIdx.x; l < H.n_r1 + H.n_r2; l += kBlock) {
+    const int id = halo_ids[l];
+    const CellRec c = rec[id];
+    bool nz = !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
+    _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < A.sc.n) nz = nz || ((ctl->cur ? A.sc.qb[sp] : A.sc.qa[sp])[id] != 0.0);
+    if (!nz) continue;
+    const int owner = id / A.L.P;
+    for (int j = 0; j < H.n_nbr && j < kPflagSlots; ++j)
+      if (nbr[j] == owner) { atomicOr(&s_dirty, 1u << j); break; }
   }
-  const unsigned char skippable = (H.n_string_edges == 0 && H.n_nbr <= kPflagSlots) ? 1 : 0;
-  cur[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
-  oth[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
+  __syncthreads();
+  unsigned char *cur = (ctl->cur ? A.pflag_b : A.pflag_a), *oth = (ctl->cur ? A.pflag_a : A.pflag_b);
+  const int j = threadIdx.x;
+  if (j < kPflagSlots) {                          // unused slots never veto
+    cur[(size_t)p * kPflagBytes + j] = j < H.n_nbr ? (unsigned char)(((s_dirty >> j) & 1u) ^ 1u) : 1;
+    oth[(size_t)p * kPflagBytes + j] = j < H.n_nbr ? 0 : 1;
+  }
+  if (j == 0) {
+    const unsigned char skippable = (H.n_string_edges == 0 && H.n_nbr <= kPflagSlots) ? 1 : 0;
+    cur[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
+    oth[(size_t)p * kPflagBytes + kPflagSkippable] = skippable;
+  }
 }
 
 }  // namespace swe

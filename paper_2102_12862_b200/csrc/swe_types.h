@@ -59,9 +59,12 @@ struct BlobLayout {
   int32_t stride;                // bytes per blob, multiple of 128
 };
 
-// per patch and state buffer: 32 flag bytes {neighbour 0..29 | own | skippable}; a byte is 1 when every own cell of
-// that patch is exactly (0, 0, 0) in that buffer (byte 31: 1 when the patch has no boundary-string edge and at most
-// kPflagSlots neighbours -- constant).  All 32 bytes == 1  <=>  the block may skip the patch (section 5b).
+// per patch and state buffer: 32 flag bytes {neighbour 0..29 | own | skippable}.  Own byte: 1 when every own cell of
+// the patch is exactly (0, 0, 0) in that buffer.  Neighbour byte j: 1 when every cell of the j-th neighbour patch that
+// is a halo cell of THIS patch is exactly (0, 0, 0) (the neighbour writes it: the fourth word of an own cell's slot
+// record names the neighbours that read the cell).  Byte 31: 1 when the patch has no boundary-string edge and at most
+// kPflagSlots neighbours -- constant.  All 32 bytes == 1  <=>  every local cell of the patch is dry and nothing can
+// feed it: the block may skip the patch (section 5b).
 constexpr int kPflagBytes = 32, kPflagSlots = 30, kPflagOwn = 30, kPflagSkippable = 31;
 
 __host__ __device__ inline int32_t blob_align(int32_t x, int32_t a) { return (x + a - 1) / a * a; }
