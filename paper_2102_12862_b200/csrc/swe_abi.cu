@@ -98,7 +98,7 @@ inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
 // [scalars][self-controlled][mobile bed]; the instances live in swe_patch_t*.cu, one translation unit per block size)
 struct PatchInst { int T, min_blocks; PatchKernel (*get)(int B, int scalars, int self, int morph); };
 const PatchInst kPatchInst[] = {{32, 8, patch_kernel_32}, {64, 8, patch_kernel_64}, {128, 6, patch_kernel_128}, {128, 4, patch_kernel_128},
-                                {192, 4, patch_kernel_192}, {192, 3, patch_kernel_192}, {256, 4, patch_kernel_256}, {256, 3, patch_kernel_256},
+                                {192, 5, patch_kernel_192}, {192, 4, patch_kernel_192}, {192, 3, patch_kernel_192}, {256, 4, patch_kernel_256}, {256, 3, patch_kernel_256},
                                 {256, 2, patch_kernel_256}, {384, 2, patch_kernel_384}, {384, 1, patch_kernel_384}, {512, 2, patch_kernel_512}, {512, 1, patch_kernel_512},
                                 {1024, 1, patch_kernel_1024}};
 
