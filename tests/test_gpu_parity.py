@@ -420,6 +420,56 @@ def test_dry_patches_are_skipped_and_rewetted(gpu, ref):
     s3.close()
 
 
+def test_skip_flags_are_exact(gpu):
+    """The 32-byte flag test of the fused patch step is exact, not just safe: in every step the number of skipped
+    patches equals the number of patches whose local cells (own cells and everything within two edges of them) are all
+    exactly (0, 0, 0) in the state the step reads and that no boundary-string edge can feed -- counted here on the host
+    from the state and the mesh alone.  First step: flags written after swe_set_state; later steps: flags the blocks
+    publish to their neighbours (one byte per neighbour, from the per-cell reader masks)."""
+    w = CASES["config4-small"]()
+    P = 64
+    s = gpu.from_workload(w, variant=gpu.VARIANT_PATCH, patch_cells=P)
+    perm = s.permutation()[0]                               # perm[internal id] = caller id
+    n = w.n_cells
+    patch_of = np.empty(n, np.int64)
+    patch_of[perm] = np.arange(n) // P
+    n_patches = (n + P - 1) // P
+    L, R = w.edge_cell[:, 0].astype(np.int64), w.edge_cell[:, 1].astype(np.int64)
+    inner = R >= 0
+
+    def dilate(mask):                                       # cells within one edge of a marked cell
+        out = mask.copy()
+        np.logical_or.at(out, L[inner], mask[R[inner]])     # (a cell is L or R of up to three edges: unbuffered)
+        np.logical_or.at(out, R[inner], mask[L[inner]])
+        return out
+
+    fed = np.zeros(n, bool)
+    fed[L[R <= -3]] = True                                  # cells with a boundary-string edge
+    fed_patch = np.zeros(n_patches, bool)
+    np.logical_or.at(fed_patch, patch_of, dilate(fed))      # ... among the own and ring-1 cells of the patch
+
+    def expected_skips(state):
+        nz = (state[0] != 0.0) | (state[1] != 0.0) | (state[2] != 0.0)
+        near = np.zeros(n_patches, bool)
+        np.logical_or.at(near, patch_of, dilate(dilate(nz)))
+        return int(np.count_nonzero(~near & ~fed_patch))
+
+    seen = []
+    done = 0
+    for before in (0, 1, 2, 37, 38, 120):
+        if before > done:
+            s.step(before - done, float("inf"), w.cfl)
+            done = before
+        want = expected_skips(s.get_state())
+        k0 = s.patch_stats()["patch_steps_skipped"]
+        s.step(1, float("inf"), w.cfl)
+        done += 1
+        assert s.patch_stats()["patch_steps_skipped"] - k0 == want, (before, want)
+        seen.append(want)
+    assert 0 < min(seen) and max(seen) < n_patches and len(set(seen)) > 1   # the flood moves the count
+    s.close()
+
+
 def test_auto_picks_the_variant_from_the_wet_fraction(gpu, ref):
     """AUTO keeps both step variants ready and picks one at every swe_set_state.  With the default patch size four blocks
     of the patch kernel fit an SM and it is the faster step at any wet fraction; with fatter blocks (here: 384-cell
