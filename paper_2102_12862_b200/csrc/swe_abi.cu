@@ -556,7 +556,7 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
   if (pl.variant == SWE_VARIANT_PATCH) {
     // default: the largest patch of 240, 232, 224, 208, 192 cells (256 threads each) whose block still fits an SM four
     // times -- 32 warps per SM; the kernel is latency-bound and 4 x 8 warps beat 3 x 8 by 10-13 %, larger patches beat
-    // smaller ones by 1-2 % per step of 8 cells (profiles/r2_patch_sweep.md); small meshes get smaller patches, so that
+    // smaller ones by 1-2 % per step of 8 cells (profiles/r2q_patch_size_sweep.md); small meshes get smaller patches, so that
     // the launch-latency-bound step still spreads over the SMs
     std::vector<int32_t> string_pos(ne, -1);
     for (size_t j = 0; j < pl.flat.size(); ++j) string_pos[pl.flat[j]] = (int32_t)j;
@@ -746,7 +746,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     {
       const int64_t cap = std::min<int64_t>(1024, (int64_t)pb.lay.cap_e + 3 * (int64_t)pb.lay.cap_eown);
       // (it saves the control kernel's graph node, 2.3-2.6 us per step: + 20-30 % on meshes up to ~100k cells, nothing
-      // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2_self_ctl.md)
+      // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2q_patch_size_sweep.md)
       const char *self_env = std::getenv("SWE_PATCH_SELF");           // measurement runs: 0 never, 2 on any mesh size
       const int self_max_patches = (self_env && std::atoi(self_env) == 2) ? (1 << 30) : 8192;
       bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= self_max_patches && c->sc.n == 0;
@@ -942,7 +942,7 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     int rc = read_control(c);
     if (rc != SWE_OK) return rc;
     // with four blocks of the patch kernel per SM it is the faster step at any wet fraction (all-wet 4M: 259.6 vs 266.1 us,
-    // 8M: 508 vs 521 us; profiles/r2_patch_sweep.md); with fewer (fat halos, scalar species, large patch_cells) the
+    // 8M: 508 vs 521 us; profiles/r2q_patch_size_sweep.md); with fewer (fat halos, scalar species, large patch_cells) the
     // round-1 crossover holds: three-pass from ~50 % wet cells on (profiles/r1i_auto_threshold.md)
     const int want = (c->patch_min_blocks < 4 && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
