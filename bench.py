@@ -87,7 +87,7 @@ def parse():
     ap.add_argument("--morph", type=int, default=0, choices=[0, 1, 2],
                     help="mobile bed (swe_set_morphology): 1 Grass-like alpha = 0.001, 2 MPM-like alpha = 8, d_m = 5 mm")
     ap.add_argument("--precision", default="double", choices=["double", "single"],
-                    help="arithmetic of the step (include/swe.h SWE_PRECISION_*; single: fp32 three-pass step, DESIGN.md R-21)")
+                    help="arithmetic of the step (include/swe.h SWE_PRECISION_*; single: fp32 records and arithmetic in both step variants, DESIGN.md R-21)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-omp", action="store_true", help="also time the oracle source built with OpenMP on all host cores")
     ap.add_argument("--parity-steps", type=int, default=5,
@@ -477,9 +477,10 @@ def main():
     # moves a third of the bytes; the three-pass step (edge flux -> theta -> CSR gather/update, the design the
     # north_star names) is the bandwidth-bound one, so its per-kernel HBM fractions are reported beside the default's
     other = None
-    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0 and not args.morph and args.precision == "double":
+    if rank == 0 and world == 1 and not args.no_other_variant and args.variant == 0 and args.species == 0 and not args.morph:
         ov = P.VARIANT_THREE_PASS if s_kernels[-1] == "k_patch_step" else P.VARIANT_PATCH
-        s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber)
+        s3 = P.from_workload(w, device=f"cuda:{local_rank}", variant=ov, renumber=args.renumber,
+                             precision=P.PRECISION_SINGLE if args.precision == "single" else P.PRECISION_DOUBLE)
         for _ in range(2):
             s3.step(T, float("inf"), w.cfl, info=False)
         torch.cuda.synchronize()
@@ -503,10 +504,11 @@ def main():
     # ---- second line (rank 0, N = 1): an ALL-WET mesh of the same size, where no patch can be skipped -- the
     # BASELINE.json configs[4] construction (circular dam break, every cell wet, friction everywhere) at 4M cells
     all_wet = None
-    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0 and not args.morph and args.precision == "double":
+    if rank == 0 and world == 1 and not args.no_all_wet and args.species == 0 and not args.morph:
         from workloads import configs as C
         w2 = C.config5(target_cells=N)
-        s2 = P.from_workload(w2, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells)
+        s2 = P.from_workload(w2, device=f"cuda:{local_rank}", variant=args.variant, patch_cells=args.patch_cells,
+                             precision=P.PRECISION_SINGLE if args.precision == "single" else P.PRECISION_DOUBLE)
         for _ in range(2):
             s2.step(T, float("inf"), w2.cfl, info=False)
         torch.cuda.synchronize()

@@ -36,8 +36,9 @@ struct PatchScratch {                    // what pass 1 finds for one patch (glo
 // (3 internal edge ids); string_pos[e] = position of boundary-string edge e in string_edges[], -1 otherwise.
 inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geom, const std::vector<int32_t> &cell_edge4,
                         const std::vector<double> &area, const std::vector<double> &inv_area, const std::vector<double> &gn2,
-                        const std::vector<int32_t> &string_pos, int P, bool emit, PatchBlobs &pb, std::string &err) {
+                        const std::vector<int32_t> &string_pos, int P, bool emit, PatchBlobs &pb, std::string &err, int rb = 8) {
   pb = PatchBlobs{};
+  // rb: bytes of a real in the staged arrays; 4 = single precision: the fp64 values rounded once to fp32 (R-21)
   if (P < 32 || P > 1024) { err = "patch_cells must be in [32, 1024]"; return false; }
   const int64_t np = (nc + P - 1) / P;
   pb.n_patches = np;
@@ -93,7 +94,7 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
   // round the capacities up a little so that the SoA arrays of the staged part stay 16-byte aligned
   cap_halo = blob_align(cap_halo, 4); cap_r1 = blob_align(cap_r1, 2); cap_e = blob_align(cap_e, 4); cap_eown = blob_align(cap_eown, 2);
   cap_nbr = blob_align(cap_nbr, 4);
-  pb.lay = blob_layout(P, cap_nbr, cap_halo, cap_r1, cap_e, cap_eown);
+  pb.lay = blob_layout(P, cap_nbr, cap_halo, cap_r1, cap_e, cap_eown, rb);
   if ((int64_t)pb.lay.stride * np > (int64_t)1 << 40) { err = "patch blobs exceed 1 TB"; return false; }
   if (!emit) return true;                       // sizing pass (swe_workspace_bytes)
 
@@ -140,8 +141,10 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
       if (j < 32) own_mask[c] |= 1u << j;
     }
     unsigned char *S = B + L.off_stage;
-    double *halo_area = (double *)(S + L.s_halo_area);
-    for (int32_t j = 0; j < s.n_r1; ++j) halo_area[j] = area[s.ring[j]];
+    auto put = [&](int32_t off, int32_t idx, double v) {          // element idx of the staged real array at offset off
+      if (rb == 4) ((float *)(S + off))[idx] = (float)v; else ((double *)(S + off))[idx] = v;
+    };
+    for (int32_t j = 0; j < s.n_r1; ++j) put(L.s_halo_area, j, area[s.ring[j]]);
     uint32_t *pce = (uint32_t *)(S + L.s_pce);
     for (int32_t l = 0; l < s.n_own + s.n_r1; ++l) {
       const int32_t c = l < s.n_own ? c0 + l : s.ring[l - s.n_own];
@@ -155,19 +158,19 @@ inline bool build_blobs(int64_t nc, int64_t ne, const std::vector<EdgeGeom> &geo
       }
       pce[4 * l + 3] = 0u;
     }
-    double *nx = (double *)(S + L.s_nx), *ny = (double *)(S + L.s_ny), *len = (double *)(S + L.s_len);
     uint32_t *lr = (uint32_t *)(S + L.s_lr);
     int32_t *aux = (int32_t *)(S + L.s_aux);
     for (int32_t j = 0; j < n_e; ++j) {
       const EdgeGeom &g = geom[s.edges[j]];
-      nx[j] = g.nx; ny[j] = g.ny; len[j] = g.len;
+      put(L.s_nx, j, g.nx); put(L.s_ny, j, g.ny); put(L.s_len, j, g.len);
       const uint32_t Ll = (uint32_t)cloc[g.L];
       if (g.R >= 0) { lr[j] = Ll | ((uint32_t)cloc[g.R] << 16); aux[j] = 0; }
       else { lr[j] = Ll | (0xFFFFu << 16); aux[j] = (g.R <= -3) ? -3 - string_pos[s.edges[j]] : g.R; }
     }
-    double *a = (double *)(S + L.s_area), *g2 = (double *)(S + L.s_gn2);
-    for (int32_t l = 0; l < s.n_own; ++l) { a[l] = area[c0 + l]; g2[l] = gn2[c0 + l]; }
-    (void)inv_area;
+    for (int32_t l = 0; l < s.n_own; ++l) {
+      put(L.s_area, l, area[c0 + l]); put(L.s_gn2, l, gn2[c0 + l]);
+      if (rb == 4) put(L.s_inv_area, l, inv_area[c0 + l]);
+    }
   }
   // the fourth word of an own cell's slot record: its mask (complete only now that every patch has been visited)
   for (int64_t p = 0; p < np; ++p) {

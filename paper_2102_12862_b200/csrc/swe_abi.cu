@@ -58,7 +58,7 @@ struct Layout {
     const size_t nc = (size_t)z.nc, ne = (size_t)z.ne, nse = (size_t)std::max<int64_t>(1, z.n_string_edges);
     const size_t r = z.single ? 4 : 8;      // bytes of a real; records are 4 reals
     rec = take(4 * r * nc);
-    rec_b = z.single ? 0 : take(4 * r * nc);   // second state buffer of the fused patch step (fp64 only)
+    rec_b = take(4 * r * nc);                  // second state buffer of the fused patch step
     geom = take(4 * r * ne);
     geomR = z.single ? take(4 * ne) : 0;    // fp32: R of every edge beside the 16-byte geometry record
     flux = take(4 * r * ne);
@@ -250,8 +250,13 @@ Patch2Args patch_args(const swe_ctx *c) {
 // dry flags of the patches from the state as it stands (after swe_set_state / swe_set_scalars / a variant switch)
 void launch_patch_flags(swe_ctx *c) {
   const Patch2Args a = patch_args(c);
-  k_patch2_own_flags<256><<<c->n_patches, 256, 0, c->stream>>>(c->d_ctl, a);
-  k_patch2_nbr_flags<<<c->n_patches, kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
+  if (c->single) {
+    k_patch2_own_flags<256, float><<<c->n_patches, 256, 0, c->stream>>>(c->d_ctl, a);
+    k_patch2_nbr_flags<float><<<c->n_patches, kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
+  } else {
+    k_patch2_own_flags<256><<<c->n_patches, 256, 0, c->stream>>>(c->d_ctl, a);
+    k_patch2_nbr_flags<double><<<c->n_patches, kBlock, 0, c->stream>>>(c->d_ctl, a, c->n_patches);
+  }
   c->launches += 2;
 }
 
@@ -290,7 +295,7 @@ void launch_patch(swe_ctx *c, cudaStream_t s, int self) {
   int force = c->patch_force_blocks;
   if (!force && c->patch_threads == 256 && c->n_patches <= 3 * c->sms) force = 3;
   const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, force);
-  pi->get(pi->min_blocks, c->sc.n > 0, self, morph != 0)<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
+  pi->get(pi->min_blocks, c->sc.n > 0, c->single ? 4 : self, morph != 0)<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
 }
 
 // one time step, in stream order.  Self-controlled patch step: the launch number decides the control slot it reads
@@ -306,12 +311,12 @@ void enqueue_step(swe_ctx *c, cudaStream_t s, cudaEvent_t *ev = nullptr) {
   if (ev) cudaEventRecord(ev[0], s);
   launch_control(c, s, 0);
   if (ev) cudaEventRecord(ev[1], s);
-  if (c->single) { enqueue_three_pass_f32(c, s, ev); return; }
   if (c->variant == SWE_VARIANT_PATCH) {
     launch_patch(c, s, 0);
     if (ev) cudaEventRecord(ev[2], s);
     return;
   }
+  if (c->single) { enqueue_three_pass_f32(c, s, ev); return; }
   const double *no_theta = nullptr;         // the records are limited in place by k_theta_lazy
   if (c->mp.formula && c->sc.n > 0)
     k_edge_flux<true, false, true><<<grid_for(c->ne), kBlock, 0, s>>>(c->d_ctl, c->geom, c->rec, c->kst, c->d_strings, c->flux, (int)c->ne, 0, c->sc,
@@ -397,7 +402,7 @@ int switch_variant(swe_ctx *c, int want, int cur) {
   if (want == c->variant) return SWE_OK;
   const int64_t nc = c->nc;
   if (want == SWE_VARIANT_THREE_PASS && cur == 1) {
-    SWE_CUDA(c, cudaMemcpyAsync(c->rec, c->rec_b, sizeof(CellRec) * nc, cudaMemcpyDeviceToDevice, c->stream));
+    SWE_CUDA(c, cudaMemcpyAsync(c->rec, c->rec_b, (c->single ? sizeof(CellRecT<float>) : sizeof(CellRec)) * nc, cudaMemcpyDeviceToDevice, c->stream));
     for (int sp = 0; sp < c->sc.n; ++sp)
       SWE_CUDA(c, cudaMemcpyAsync(c->sc.qa[sp], c->sc.qb[sp], 8 * nc, cudaMemcpyDeviceToDevice, c->stream));
   }
@@ -474,8 +479,8 @@ int check_params(const swe_params &p, std::string &err) {
   if (p.n_species < 0 || p.n_species > kMaxSpecies) { err = "n_species must be in [0, 5] (P:208)"; return SWE_EINVAL; }
   if (p.variant != SWE_VARIANT_AUTO && p.variant != SWE_VARIANT_THREE_PASS && p.variant != SWE_VARIANT_PATCH) { err = "unknown variant"; return SWE_EINVAL; }
   if (p.precision != SWE_PRECISION_DOUBLE && p.precision != SWE_PRECISION_SINGLE) { err = "unknown precision"; return SWE_EINVAL; }
-  if (p.precision == SWE_PRECISION_SINGLE && (p.n_species > 0 || p.morphology || p.variant == SWE_VARIANT_PATCH)) {
-    err = "single precision is built for the three-pass hydrodynamic step only (no scalars, mobile bed or patch step)"; return SWE_EINVAL;
+  if (p.precision == SWE_PRECISION_SINGLE && (p.n_species > 0 || p.morphology)) {
+    err = "single precision is built for the hydrodynamic step only (no scalars, no mobile bed)"; return SWE_EINVAL;
   }
   if (p.patch_cells != 0 && (p.patch_cells < 32 || p.patch_cells > 1024)) { err = "patch_cells must be 0 (default) or in [32, 1024]"; return SWE_EINVAL; }
   return SWE_OK;
@@ -552,7 +557,8 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
   }
 
   // ---- fused patch step: patch blobs, shared-memory size
-  pl.variant = (p.variant == SWE_VARIANT_THREE_PASS || pl.z.single) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+  pl.variant = p.variant == SWE_VARIANT_THREE_PASS ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+  const int rb = pl.z.single ? 4 : 8;      // bytes of a real in the patch blobs
   if (pl.variant == SWE_VARIANT_PATCH) {
     // default: the largest patch of 240, 232, 224, 208, 192 cells (256 threads each) whose block still fits an SM four
     // times -- 32 warps per SM; the kernel is latency-bound and 4 x 8 warps beat 3 x 8 by 10-13 %, larger patches beat
@@ -566,12 +572,12 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
       const bool self = false;               // (meshes of this size do not run the self-controlled step)
       for (int cand : {240, 232, 224, 208, 192}) {
         P = cand;
-        if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, false, pl.pb, err)) return SWE_EINVAL;
+        if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, false, pl.pb, err, rb)) return SWE_EINVAL;
         const size_t smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species, 0, self && nc / P <= 8192).total;
         if (4 * (smem + kSmemBlockReserve) <= kSmemPerSM) break;
       }
     }
-    if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, emit, pl.pb, err)) return SWE_EINVAL;
+    if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, emit, pl.pb, err, rb)) return SWE_EINVAL;
     pl.patch_smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species).total;
     // a numbering that is not spatially compact (renumber = NONE on a scattered input order) blows the halos up:
     // more than 2.2 local cells per own cell, or a block that no longer fits an SM twice -> AUTO falls back to the
@@ -619,7 +625,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
   char *ws = c->ws;
   c->single = pl.z.single;
   if (c->single) c->geomR = (int32_t *)(ws + lay.geomR);
-  c->rec = (CellRec *)(ws + lay.rec); c->rec_b = (CellRec *)(ws + (c->single ? lay.rec : lay.rec_b)); c->geom = (EdgeGeom *)(ws + lay.geom); c->flux = (EdgeFlux *)(ws + lay.flux);
+  c->rec = (CellRec *)(ws + lay.rec); c->rec_b = (CellRec *)(ws + lay.rec_b); c->geom = (EdgeGeom *)(ws + lay.geom); c->flux = (EdgeFlux *)(ws + lay.flux);
   c->cell_edge = (int4 *)(ws + lay.cell_edge);
   c->area = (double *)(ws + lay.area); c->inv_area = (double *)(ws + lay.inv_area);
   c->gn2 = (double *)(ws + lay.gn2); c->kst = (double *)(ws + lay.kst); c->theta = (double *)(ws + lay.theta);
@@ -664,6 +670,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       std::vector<float> f(nc);
       for (int64_t i = 0; i < nc; ++i) rec[i] = {0.f, 0.f, 0.f, (float)mesh->zb[c->hm.cell_perm[i]]};
       SWE_CUDA(c, up(v.rec, rec.data(), sizeof(CellRecT<float>) * nc));
+      SWE_CUDA(c, up(v.rec_b, rec.data(), sizeof(CellRecT<float>) * nc));   // z_B must be valid in both state buffers
       const std::vector<double> *srcs[4] = {&pl.area, &pl.inv_area, &pl.gn2, &pl.kst};
       float *dsts[4] = {v.area, v.inv_area, v.gn2, v.kst};
       for (int a = 0; a < 4; ++a) {
@@ -749,7 +756,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       // measurable from ~2M cells on, where the extra work at the top of 15,000 blocks costs as much: profiles/r2q_patch_size_sweep.md)
       const char *self_env = std::getenv("SWE_PATCH_SELF");           // measurement runs: 0 never, 2 on any mesh size
       const int self_max_patches = (self_env && std::atoi(self_env) == 2) ? (1 << 30) : 8192;
-      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= self_max_patches && c->sc.n == 0;
+      bool ok = (int)c->strings.size() <= kCtlPre && (c->steps_per_graph % 4) == 0 && c->n_patches <= self_max_patches && c->sc.n == 0 && !c->single;
       for (const BoundaryString &bs : c->strings) ok = ok && bs.pow2 <= cap;
       if (const char *s = std::getenv("SWE_PATCH_SELF")) ok = ok && std::atoi(s) != 0;
       c->self_ctl = ok;
@@ -770,8 +777,8 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
       SWE_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
       for (const PatchInst &pi : kPatchInst) {
         if (pi.T != c->patch_threads) continue;
-        for (int a = 0; a < 8; ++a) {
-          PatchKernel fn = pi.get(pi.min_blocks, a & 1, (a >> 1) & 1, (a >> 2) & 1);
+        for (int a = 0; a < 9; ++a) {                  // [scalars][self-controlled][mobile bed], and the single-precision instance
+          PatchKernel fn = a < 8 ? pi.get(pi.min_blocks, a & 1, (a >> 1) & 1, (a >> 2) & 1) : pi.get(pi.min_blocks, 0, 4, 0);
           if (!fn) continue;
           SWE_CUDA(c, cudaFuncGetAttributes(&fa, fn));
           const int limit = optin - (int)fa.sharedSizeBytes;
@@ -787,6 +794,10 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     ab[1] = 96 * nc + 32 * ne + (int64_t)c->sc.n * 16 * nc;         // + q_c in and out per species
     // SURVEY.md section 8(d), one-pass column: 132 B per cell-step (+ 16 per species: q_c in and out)
     c->survey_bytes_v[SWE_VARIANT_PATCH][1] = (132 + 16 * (int64_t)c->sc.n) * nc;
+    if (c->single) {   // 16-byte records, 4-byte reals (abs(Omega), 1/abs(Omega), g/k^2; n_x, n_y, l), int32 tables stay
+      ab[1] = (16 + 16 + 16 + 12) * nc + (12 + 8) * ne;
+      c->survey_bytes_v[SWE_VARIANT_PATCH][1] = (132 - 16) / 2 * nc + 16 * nc;    // reals halve, the slot words stay
+    }
   }
   {
     // EdgeGeom read + EdgeFlux written per edge, every CellRec gathered once
@@ -944,7 +955,9 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     // with four blocks of the patch kernel per SM it is the faster step at any wet fraction (all-wet 4M: 259.6 vs 266.1 us,
     // 8M: 508 vs 521 us; profiles/r2q_patch_size_sweep.md); with fewer (fat halos, scalar species, large patch_cells) the
     // round-1 crossover holds: three-pass from ~50 % wet cells on (profiles/r1i_auto_threshold.md)
-    const int want = (c->patch_min_blocks < 4 && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+    // (single precision: the three-pass step moves half the bytes and wins on all-wet states, 27.5 vs 20.6 G at 8M cells;
+    // the patch step wins while part of the domain is dry, 36.6 vs 29.0 G on the river reach: profiles/r2u_single_precision.md)
+    const int want = ((c->single || c->patch_min_blocks < 4) && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
       if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
         for (int sp = 0; sp < c->sc.n; ++sp)
@@ -1023,7 +1036,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (h.nonfinite) { c->err = "non-finite state value"; return SWE_ENONFINITE; }
     if (c->auto_mode) {   // the wet count is known here: follow a flood that spreads (or recedes), with hysteresis
       const double wet = (double)h.n_wet / (double)c->nc;
-      const int want = c->patch_min_blocks >= 4 ? SWE_VARIANT_PATCH
+      const int want = (c->patch_min_blocks >= 4 && !c->single) ? SWE_VARIANT_PATCH
                                                 : (wet > 0.55 ? SWE_VARIANT_THREE_PASS : (wet < 0.45 ? SWE_VARIANT_PATCH : c->variant));
       rc = switch_variant(c, want, h.cur);
       if (rc != SWE_OK) return rc;
@@ -1246,6 +1259,10 @@ int swe_get_geometry(swe_ctx *c, double *area, double *nx, double *ny, double *l
 int swe_get_edge_flux(swe_ctx *c, double *F1, double *F3, double *GL, double *GR, double *theta) {
   if (!c || !F1 || !F3 || !GL || !GR) return SWE_EINVAL;
   const int64_t ne = c->ne, nc = c->nc;
+  if (c->variant == SWE_VARIANT_PATCH && c->single) {
+    c->err = "swe_get_edge_flux: not built for the single-precision patch step (SWE_VARIANT_THREE_PASS exports its fluxes)";
+    return SWE_EINVAL;
+  }
   if (c->variant == SWE_VARIANT_PATCH) {
     // the fused step keeps edge fluxes in shared memory: re-evaluate S1 and S1c of the most recent step with the
     // stand-alone kernels, from the state that step read (still intact in the other buffer) and its dt

@@ -29,8 +29,8 @@ namespace swe {
 struct Patch2Args {
   const unsigned char *blob;
   BlobLayout L;
-  CellRec *rec_a, *rec_b;
-  const double *kst;
+  void *rec_a, *rec_b;            // CellRecT<T> of the kernel's arithmetic T
+  const void *kst;                // T per cell
   const BoundaryString *strings;
   const int32_t *slot_string;     // string id of every position of string_edges[]
   double *string_M;               // l * (limited F1) of every boundary-string edge, by position in string_edges[]
@@ -56,18 +56,19 @@ struct Patch2Smem {
 // morph: 0 fixed bed, 1 Grass-like law (q_B per own edge), 2 MPM-like law (+ (g/k^2, cbrt h) of every local cell)
 __host__ __device__ inline Patch2Smem patch2_smem_layout(const BlobLayout &L, int n_species, int morph = 0, bool self = true) {
   Patch2Smem s;
+  const int32_t rb = L.rb;                         // bytes of a real (fp64: 8; single precision: 4)
   int32_t o = 128;                                  // [0, 8): the mbarrier
   s.strs = o; o += self ? blob_align(kCtlPre * (int32_t)sizeof(BoundaryString), 128) : 0;   // kSelf: the strings with Q, sumK of t^n
   s.stage = o; o += blob_align(L.stage_bytes, 128);
-  s.h = o; o += 8 * L.cap_loc; s.u = o; o += 8 * L.cap_loc; s.v = o; o += 8 * L.cap_loc; s.z = o; o += 8 * L.cap_loc;
-  s.theta = o; o += 8 * L.cap_c1;
-  s.F1 = o; o += 8 * L.cap_e;
+  s.h = o; o += rb * L.cap_loc; s.u = o; o += rb * L.cap_loc; s.v = o; o += rb * L.cap_loc; s.z = o; o += rb * L.cap_loc;
+  s.theta = o; o += rb * L.cap_c1;
+  s.F1 = o; o += rb * L.cap_e;
   o = blob_align(o, 32);
   // the own CellRec records as the bulk copy delivers them are consumed in phase 1 (the momenta stay in registers),
   // the fluxes F3 / GL / GR of the own edges are written from phase 2 on: the two share their shared memory
   s.crec = o;
-  s.F3 = o; s.GL = o + 8 * L.cap_eown; s.GR = o + 16 * L.cap_eown;
-  o += (24 * L.cap_eown > 32 * L.P) ? 24 * L.cap_eown : 32 * L.P;
+  s.F3 = o; s.GL = o + rb * L.cap_eown; s.GR = o + 2 * rb * L.cap_eown;
+  o += (3 * rb * L.cap_eown > 4 * rb * L.P) ? 3 * rb * L.cap_eown : 4 * rb * L.P;
   s.phi = o; o += 8 * n_species * L.cap_loc;        // concentrations of the local cells, species-major
   s.qB = o; o += morph ? 8 * L.cap_eown : 0;        // normal sediment flux of the own edges (R-20)
   s.fcx = o; o += morph == 2 ? 8 * L.cap_loc : 0; s.fcy = o; o += morph == 2 ? 8 * L.cap_loc : 0;
@@ -191,9 +192,13 @@ k_self_finish(Control *ctl, const BoundaryString *__restrict__ strings, int n_st
 // conveyance sums themselves (same fixed-shape trees, R-11).
 // kMorph: the mobile bed (R-20): q_Bij of every own edge in phase 2 (Table 2, Eq. 14-16), Eq. 13 in phase 4 -- the bed
 // rides in the state record.  A skipped patch keeps its bed: no transport where a side is dry.
-template <int kThreads, int kMinBlocks, bool kScalars = false, bool kSelf = false, bool kMorph = false>
+// T: the arithmetic of the step (double; float = single precision, R-21: plain hydrodynamics behind k_step_control only)
+template <int kThreads, int kMinBlocks, bool kScalars = false, bool kSelf = false, bool kMorph = false, typename T = double>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
+  static_assert(sizeof(T) == 8 || (!kScalars && !kSelf && !kMorph), "single precision: hydrodynamics behind k_step_control only");
+  typedef CellRecT<T> Rec;
+  typedef EdgeFluxT<T> Flux;
   extern __shared__ __align__(128) unsigned char smraw[];
   const BlobLayout &L = A.L;
   const int tid = threadIdx.x, b = blockIdx.x;
@@ -210,9 +215,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   const ulonglong2 *pfb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b * kPflagBytes);
   StepSlot S0;
   int active, src;
-  double dt;
-  if (kSelf) { S0 = ctl->slot[A.step_k]; active = 0; src = S0.src; dt = 0.0; }
-  else { active = ctl->active; src = ctl->src; dt = ctl->dt; }
+  T dt;
+  if (kSelf) { S0 = ctl->slot[A.step_k]; active = 0; src = S0.src; dt = T(0.0); }
+  else { active = ctl->active; src = ctl->src; dt = (T)ctl->dt; }
   const ulonglong2 fa0 = pfa[0], fa1 = pfa[1], fb0 = pfb[0], fb1 = pfb[1];
   const int hid0 = tid < L.cap_halo ? halo_ids[tid] : -1;
   const int hid1 = tid + kThreads < L.cap_halo ? halo_ids[tid + kThreads] : -1;
@@ -224,8 +229,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const ulonglong2 *qb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b_pf * kPflagBytes);
     ga0 = qa[0]; ga1 = qa[1]; gb0 = qb[0]; gb1 = qb[1];
   }
-  const double g = ctl->g, h_dry = ctl->h_dry;
-  if (kSelf) {
+  const T g = (T)ctl->g, h_dry = (T)ctl->h_dry;
+  if constexpr (kSelf) {
     const StepChoice ch = choose_step(S0, ctl->t_end, ctl->cfl, ctl->dt_max);
     active = ch.active; dt = ch.dt;
     if (b == 0) {                // the control duty: next slot, volume bookkeeping (before anything can return)
@@ -248,8 +253,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     }
   }
   if (!active) return;
-  const CellRec *__restrict__ in = src ? A.rec_b : A.rec_a;
-  CellRec *__restrict__ out = src ? A.rec_a : A.rec_b;
+  const Rec *__restrict__ in = reinterpret_cast<const Rec *>(src ? A.rec_b : A.rec_a);      // (the args carry untyped record pointers)
+  Rec *__restrict__ out = reinterpret_cast<Rec *>(src ? A.rec_a : A.rec_b);
   unsigned char *pf_out_base = src ? A.pflag_a : A.pflag_b;
   const unsigned long long ones = 0x0101010101010101ull;
 
@@ -264,8 +269,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       const unsigned char had = (unsigned char)((o1.y >> (8 * (kPflagOwn - 24))) & 0xffull);
       if (!had) {
         if (tid < n_own) {
-          CellRec c = in[cell0 + tid];
-          c.h = 0.0; c.qx = 0.0; c.qy = 0.0;
+          Rec c = in[cell0 + tid];
+          c.h = T(0.0); c.qx = T(0.0); c.qy = T(0.0);
           out[cell0 + tid] = c;
           _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) (src ? A.sc.qa[sp] : A.sc.qb[sp])[cell0 + tid] = 0.0;   // flag: all q_c are 0 too
         }
@@ -279,13 +284,13 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
 
   const int morph = kMorph ? A.mp.formula : 0;
   const Patch2Smem S = patch2_smem_layout(L, n_sp, morph, kSelf);
-  double *sh_qB = (double *)(smraw + S.qB), *sh_fcx = (double *)(smraw + S.fcx), *sh_fcy = (double *)(smraw + S.fcy);
+  T *sh_qB = (T *)(smraw + S.qB), *sh_fcx = (T *)(smraw + S.fcx), *sh_fcy = (T *)(smraw + S.fcy);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smraw);
   unsigned char *stage = smraw + S.stage;
-  CellRec *crec = reinterpret_cast<CellRec *>(smraw + S.crec);
-  double *sh_h = (double *)(smraw + S.h), *sh_u = (double *)(smraw + S.u), *sh_v = (double *)(smraw + S.v), *sh_z = (double *)(smraw + S.z);
-  double *sh_th = (double *)(smraw + S.theta), *sh_F1 = (double *)(smraw + S.F1), *sh_F3 = (double *)(smraw + S.F3);
-  double *sh_GL = (double *)(smraw + S.GL), *sh_GR = (double *)(smraw + S.GR), *sh_phi = (double *)(smraw + S.phi);
+  Rec *crec = reinterpret_cast<Rec *>(smraw + S.crec);
+  T *sh_h = (T *)(smraw + S.h), *sh_u = (T *)(smraw + S.u), *sh_v = (T *)(smraw + S.v), *sh_z = (T *)(smraw + S.z);
+  T *sh_th = (T *)(smraw + S.theta), *sh_F1 = (T *)(smraw + S.F1), *sh_F3 = (T *)(smraw + S.F3);
+  T *sh_GL = (T *)(smraw + S.GL), *sh_GR = (T *)(smraw + S.GR), *sh_phi = (T *)(smraw + S.phi);
   const int cap_loc = L.cap_loc;
 
   // ---- the two bulk copies: staged part of the blob, own cell records
@@ -293,9 +298,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   if (tid == 0) {
     *sm_dirty = 0u;
     mbar_init(bar, 1);
-    mbar_expect_tx(bar, (uint32_t)L.stage_bytes + 32u * (uint32_t)n_own);
+    mbar_expect_tx(bar, (uint32_t)L.stage_bytes + (uint32_t)sizeof(Rec) * (uint32_t)n_own);
     bulk_g2s(stage, blob + L.off_stage, (uint32_t)L.stage_bytes, bar);
-    bulk_g2s(crec, in + cell0, 32u * (uint32_t)n_own, bar);
+    bulk_g2s(crec, in + cell0, (uint32_t)sizeof(Rec) * (uint32_t)n_own, bar);
     // the tables and own records of the patch that will run in this slot next go to L2 now (unless that patch will
     // be skipped): its block then pays L2 latency, not DRAM latency, in the chain flag word -> bulk copy -> phase 1
     if (do_pf) {
@@ -303,7 +308,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       if (!(v0.x == ones && v0.y == ones && v1.x == ones && v1.y == ones)) {
         const int c0n = b_pf * L.P, n_next = min(L.P, A.n_cells - c0n);
         bulk_prefetch_l2(A.blob + (size_t)b_pf * (size_t)L.stride, (uint32_t)(L.off_stage + L.stage_bytes));
-        bulk_prefetch_l2(in + c0n, 32u * (uint32_t)n_next);
+        bulk_prefetch_l2(in + c0n, (uint32_t)sizeof(Rec) * (uint32_t)n_next);
       }
     }
   }
@@ -315,38 +320,38 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const int j1 = j0 + kThreads;
     const int id0 = j0 == tid ? hid0 : halo_ids[j0];
     const int id1 = j0 == tid ? hid1 : (j1 < L.cap_halo ? halo_ids[j1] : -1);
-    CellRec c0, c1;
+    Rec c0, c1;
     if (id0 >= 0) c0 = in[id0];
     if (id1 >= 0) c1 = in[id1];
     if (id0 >= 0) {
       const int l = n_own + j0;
-      double u = 0.0, v = 0.0;
+      T u = T(0.0), v = T(0.0);
       if (c0.h > h_dry) { u = c0.qx / c0.h; v = c0.qy / c0.h; }
       sh_h[l] = c0.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c0.z;
-      if (kMorph && morph == 2) {                // MPM-like law: (g / k^2, cbrt h) as k_cell_update leaves it in Morph::cell
-        const double f2 = A.gn2[id0];
+      if constexpr (kMorph) if (morph == 2) {                // MPM-like law: (g / k^2, cbrt h) as k_cell_update leaves it in Morph::cell
+        const T f2 = A.gn2[id0];
         const bool on = c0.h > h_dry && f2 > 0.0;
         sh_fcx[l] = on ? f2 : 0.0; sh_fcy[l] = on ? cbrt_rn(c0.h) : 0.0;
       }
-      if (l < L.cap_c1) sh_th[l] = 1.0;
-      water |= (c0.h != 0.0);
-      if (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
+      if (l < L.cap_c1) sh_th[l] = T(1.0);
+      water |= (c0.h != T(0.0));
+      if constexpr (kScalars)                              // phi = q_c / h where there is water, else 0 (R-19)
         _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
           sh_phi[sp * cap_loc + l] = c0.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[id0] / c0.h : 0.0;
     }
     if (id1 >= 0) {
       const int l = n_own + j1;
-      double u = 0.0, v = 0.0;
+      T u = T(0.0), v = T(0.0);
       if (c1.h > h_dry) { u = c1.qx / c1.h; v = c1.qy / c1.h; }
       sh_h[l] = c1.h; sh_u[l] = u; sh_v[l] = v; sh_z[l] = c1.z;
-      if (kMorph && morph == 2) {
-        const double f2 = A.gn2[id1];
+      if constexpr (kMorph) if (morph == 2) {
+        const T f2 = A.gn2[id1];
         const bool on = c1.h > h_dry && f2 > 0.0;
         sh_fcx[l] = on ? f2 : 0.0; sh_fcy[l] = on ? cbrt_rn(c1.h) : 0.0;
       }
-      if (l < L.cap_c1) sh_th[l] = 1.0;
-      water |= (c1.h != 0.0);
-      if (kScalars)
+      if (l < L.cap_c1) sh_th[l] = T(1.0);
+      water |= (c1.h != T(0.0));
+      if constexpr (kScalars)
         _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
           sh_phi[sp * cap_loc + l] = c1.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[id1] / c1.h : 0.0;
     }
@@ -356,30 +361,30 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
 
   const BlobHeader H = *reinterpret_cast<const BlobHeader *>(stage + L.s_hdr);
   const int n_c1 = H.n_own + H.n_r1, n_e = H.n_eown + H.n_er1;
-  const double *__restrict__ b_halo_area = (const double *)(stage + L.s_halo_area);
+  const T *__restrict__ b_halo_area = (const T *)(stage + L.s_halo_area);
   const uint4 *__restrict__ b_pce = (const uint4 *)(stage + L.s_pce);
-  const double *__restrict__ b_nx = (const double *)(stage + L.s_nx), *__restrict__ b_ny = (const double *)(stage + L.s_ny);
-  const double *__restrict__ b_len = (const double *)(stage + L.s_len);
+  const T *__restrict__ b_nx = (const T *)(stage + L.s_nx), *__restrict__ b_ny = (const T *)(stage + L.s_ny);
+  const T *__restrict__ b_len = (const T *)(stage + L.s_len);
   const uint32_t *__restrict__ b_lr = (const uint32_t *)(stage + L.s_lr);
   const int32_t *__restrict__ b_aux = (const int32_t *)(stage + L.s_aux);
-  const double *__restrict__ b_area = (const double *)(stage + L.s_area);
-  const double *__restrict__ b_gn2 = (const double *)(stage + L.s_gn2);
+  const T *__restrict__ b_area = (const T *)(stage + L.s_area);
+  const T *__restrict__ b_gn2 = (const T *)(stage + L.s_gn2);
 
   // ---- phase 1b: own cells, from the records the bulk copy delivered
-  double qx_own = 0.0, qy_own = 0.0;               // the momenta of this thread's own cell, kept for phase 4
+  T qx_own = T(0.0), qy_own = T(0.0);               // the momenta of this thread's own cell, kept for phase 4
   if (tid < n_own) {
-    const CellRec c_own = crec[tid];
+    const Rec c_own = crec[tid];
     qx_own = c_own.qx; qy_own = c_own.qy;
-    double u = 0.0, v = 0.0;
+    T u = T(0.0), v = T(0.0);
     if (c_own.h > h_dry) { u = c_own.qx / c_own.h; v = c_own.qy / c_own.h; }
-    sh_h[tid] = c_own.h; sh_u[tid] = u; sh_v[tid] = v; sh_z[tid] = c_own.z; sh_th[tid] = 1.0;
-    if (kMorph && morph == 2) {
-      const double f2 = b_gn2[tid];
+    sh_h[tid] = c_own.h; sh_u[tid] = u; sh_v[tid] = v; sh_z[tid] = c_own.z; sh_th[tid] = T(1.0);
+    if constexpr (kMorph) if (morph == 2) {
+      const T f2 = b_gn2[tid];
       const bool on = c_own.h > h_dry && f2 > 0.0;
       sh_fcx[tid] = on ? f2 : 0.0; sh_fcy[tid] = on ? cbrt_rn(c_own.h) : 0.0;
     }
-    water |= (c_own.h != 0.0);
-    if (kScalars)
+    water |= (c_own.h != T(0.0));
+    if constexpr (kScalars)
       _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp)
         sh_phi[sp * cap_loc + tid] = c_own.h > 0.0 ? (src ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + tid] / c_own.h : 0.0;
   }
@@ -388,10 +393,10 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   if (!__syncthreads_or(water) && H.n_string_edges == 0) {
     int scalar_mass = 0;
     if (tid < n_own) {
-      CellRec c; c.h = 0.0; c.qx = 0.0; c.qy = 0.0; c.z = sh_z[tid];
+      Rec c; c.h = T(0.0); c.qx = T(0.0); c.qy = T(0.0); c.z = sh_z[tid];
       out[cell0 + tid] = c;
-      _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {          // no flux: scalar mass parked in dry cells stays where it is
-        const double q = (src ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + tid];
+      if constexpr (kScalars) _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {          // no flux: scalar mass parked in dry cells stays where it is
+        const T q = (src ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + tid];
         (src ? A.sc.qa[sp] : A.sc.qb[sp])[cell0 + tid] = q;
         scalar_mass |= (q != 0.0);
       }
@@ -406,9 +411,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   // ---- kSelf: this block owns boundary-string edges -> Q(t^n) and the conveyance sum of every inflow string (R-11),
   // as k_step_control evaluates them: weights from the state being read, fixed-shape pairwise tree in string order
   const BoundaryString *sm_strings = reinterpret_cast<const BoundaryString *>(smraw + S.strs);
-  if (kSelf && H.n_string_edges > 0) {
+  if constexpr (kSelf) if (H.n_string_edges > 0) {
     BoundaryString *st = reinterpret_cast<BoundaryString *>(smraw + S.strs);
-    double *v = sh_F1;                               // scratch: the flux arrays (and the own records aliased with them,
+    T *v = sh_F1;                               // scratch: the flux arrays (and the own records aliased with them,
                                                      // consumed in phase 1) are not in use before phase 2
     for (int j = tid; j < A.n_strings * (int)(sizeof(BoundaryString) / 8); j += kThreads)
       reinterpret_cast<unsigned long long *>(st)[j] = reinterpret_cast<const unsigned long long *>(A.strings)[j];
@@ -418,9 +423,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       const int n = st[s].n_edges, first = st[s].first, pow2 = st[s].pow2;
       for (int j = tid; j < pow2; j += kThreads)
         v[j] = j < n ? A.string_lk[first + j] * pow53(in[A.string_cell[first + j]].h) : 0.0;
-      const double sum = block_tree_sum(v, pow2);
+      const T sum = block_tree_sum(v, pow2);
       if (tid == 0) {
-        const double Q = hydrograph(st[s].params, st[s].n_params, S0.t);
+        const T Q = hydrograph(st[s].params, st[s].n_params, S0.t);
         st[s].sumK = sum; st[s].Q = Q;
         // also where k_step_control would leave them (inspection: swe_get_edge_flux re-evaluates this step from them);
         // every block that owns a string edge writes the same two values
@@ -433,7 +438,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
 
   // ---- phase 2: edge fluxes (two edges per thread and iteration, to interleave their dependent fp64 chains, was
   // measured and is slower: 80 registers with spills, branches keep the streams apart)
-  struct EdgeIn { double nx, ny, len, hL, uL, vL, zL, hR, uR, vR, zR; int Lc, Rc; };
+  struct EdgeIn { T nx, ny, len, hL, uL, vL, zL, hR, uR, vR, zR; int Lc, Rc; };
   auto load_edge = [&](int e) {
     EdgeIn q;
     const uint32_t lr = b_lr[e];
@@ -445,24 +450,24 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     return q;
   };
   auto flux_edge = [&](const EdgeIn &q, int e) {
-    EdgeFlux o;
+    Flux o;
     if (q.Rc != 0xFFFF) {
-      const double unL = q.uL * q.nx + q.vL * q.ny, utL = q.vL * q.nx - q.uL * q.ny;
-      const double unR = q.uR * q.nx + q.vR * q.ny, utR = q.vR * q.nx - q.uR * q.ny;
+      const T unL = q.uL * q.nx + q.vL * q.ny, utL = q.vL * q.nx - q.uL * q.ny;
+      const T unR = q.uR * q.nx + q.vR * q.ny, utR = q.vR * q.nx - q.uR * q.ny;
       o = riemann_nt(g, q.hL, unL, utL, q.zL, q.hR, unR, utR, q.zR);
     } else {
       const BoundaryString *bs = nullptr;
       int code = b_aux[e];
       if (code <= -3) { bs = (kSelf ? sm_strings : A.strings) + A.slot_string[-3 - code]; code = -3; }
       const int gidL = q.Lc < n_own ? cell0 + q.Lc : halo_ids[q.Lc - n_own];
-      o = boundary_flux(g, code, bs, A.kst, gidL, q.nx, q.ny, q.len, q.hL, q.zL, q.uL, q.vL);
+      o = boundary_flux(g, code, bs, reinterpret_cast<const T *>(A.kst), gidL, q.nx, q.ny, q.len, q.hL, q.zL, q.uL, q.vL);
     }
     return o;
   };
-  auto store_edge = [&](const EdgeIn &q, int e, const EdgeFlux &o) {
+  auto store_edge = [&](const EdgeIn &q, int e, const Flux &o) {
     sh_F1[e] = o.F1;
     if (e < H.n_eown) { sh_F3[e] = o.F3; sh_GL[e] = o.GL; sh_GR[e] = o.GR; }
-    if (kMorph && e < H.n_eown) {                     // S1m: q_Bij from the state at t^n (Eq. 14-16; R-20)
+    if constexpr (kMorph) if (e < H.n_eown) {                     // S1m: q_Bij from the state at t^n (Eq. 14-16; R-20)
       const int Rcode = q.Rc != 0xFFFF ? 0 : (b_aux[e] <= -3 ? -3 : b_aux[e]);
       const double2 zero = make_double2(0.0, 0.0);
       const double2 fcL = morph == 2 ? make_double2(sh_fcx[q.Lc], sh_fcy[q.Lc]) : zero;
@@ -471,16 +476,16 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     }
     // S1c, lazily (R-8b; as in k_edge_flux): theta_i < 1 needs one outgoing edge with dt * o_k > 0.3 h_i |Omega_i|.  Only
     // such donor cells are marked (theta = -1); phase 3 evaluates theta for them and every other cell keeps theta = 1.
-    const int d = o.F1 > 0.0 ? q.Lc : ((o.F1 < 0.0 && q.Rc != 0xFFFF) ? q.Rc : n_c1);
+    const int d = o.F1 > T(0.0) ? q.Lc : ((o.F1 < T(0.0) && q.Rc != 0xFFFF) ? q.Rc : n_c1);
     if (d < n_c1) {
-      const double ad = d < n_own ? b_area[d] : b_halo_area[d - n_own];
-      const double hd = d == q.Lc ? q.hL : q.hR;
-      if (dt * (q.len * fabs(o.F1)) > 0.3 * (hd * ad)) sh_th[d] = -1.0;
+      const T ad = d < n_own ? b_area[d] : b_halo_area[d - n_own];
+      const T hd = d == q.Lc ? q.hL : q.hR;
+      if (dt * (q.len * fabs(o.F1)) > T(0.3) * (hd * ad)) sh_th[d] = -T(1.0);
     }
   };
   for (int e = tid; e < n_e; e += kThreads) {
     const EdgeIn q = load_edge(e);
-    const EdgeFlux o = flux_edge(q, e);
+    const Flux o = flux_edge(q, e);
     store_edge(q, e, o);
   }
   __syncthreads();
@@ -488,56 +493,59 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   // ---- phase 3 (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1)), slots in order -- for the
   // cells marked in phase 2 only
   for (int l = tid; l < n_c1; l += kThreads) {
-    if (sh_th[l] >= 0.0) continue;
+    if (sh_th[l] >= T(0.0)) continue;
     const uint4 pc = b_pce[l];
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
-    double o[3];
+    T o[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const int e = w[k] & 0x7FFFu;
-      const double sM = ((w[k] & 0x8000u) ? 1.0 : -1.0) * (b_len[e] * sh_F1[e]);
+      const T sM = ((w[k] & 0x8000u) ? T(1.0) : -T(1.0)) * (b_len[e] * sh_F1[e]);
       o[k] = dmax0(sM);
     }
-    const double outflow = ((o[0] + o[1]) + o[2]);
-    const double avail = sh_h[l] * (l < n_own ? b_area[l] : b_halo_area[l - n_own]);
-    double th = 1.0;
+    const T outflow = ((o[0] + o[1]) + o[2]);
+    const T avail = sh_h[l] * (l < n_own ? b_area[l] : b_halo_area[l - n_own]);
+    T th = T(1.0);
     if (dt * outflow > avail) th = avail / (dt * outflow);
     sh_th[l] = th;
   }
   __syncthreads();
 
   // ---- phase 4: own cells, one per thread
-  double rate = 0.0;
+  T rate = T(0.0);
   int nonzero = 0;
   if (tid < n_own) {
     const int l = tid, i = cell0 + tid;
     const uint4 pc = b_pce[l];
-    CellRec c_own;
+    Rec c_own;
     c_own.h = sh_h[l]; c_own.qx = qx_own; c_own.qy = qy_own; c_own.z = sh_z[l];
-    const double invA = 1.0 / b_area[l], f2 = b_gn2[l];      // 1 / |Omega| as the host forms it for the three-pass step
+    T invA;                                          // 1 / |Omega| as the host forms it for the three-pass step
+    if constexpr (sizeof(T) == 8) invA = T(1.0) / b_area[l];
+    else invA = reinterpret_cast<const T *>(stage + L.s_inv_area)[l];   // fp64 quotient rounded once (R-21)
+    const T f2 = b_gn2[l];
     const uint32_t w[3] = {pc.x, pc.y, pc.z};
-    double dH = 0.0, dX = 0.0, dY = 0.0, dB = 0.0;   // ((d0 + d1) + d2), accumulated in slot order
-    double F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,
+    T dH = T(0.0), dX = T(0.0), dY = T(0.0), dB = T(0.0);   // ((d0 + d1) + d2), accumulated in slot order
+    T F1k[3], slk[3];                           // kScalars: limited mass flux and sign * length of every slot,
     int up[3];                                       // local id of the upwind cell, or -1 - slot of an inflow-string edge
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const int e = w[k] & 0x7FFFu;
       const bool isL = (w[k] & 0x8000u) != 0u;
       const uint32_t nb = w[k] >> 16;
-      double F1 = sh_F1[e], F3 = sh_F3[e];
-      double G = isL ? sh_GL[e] : sh_GR[e];
+      T F1 = sh_F1[e], F3 = sh_F3[e];
+      T G = isL ? sh_GL[e] : sh_GR[e];
       // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
-      double th = 1.0;
-      if (F1 > 0.0) th = sh_th[isL ? (uint32_t)l : nb];
-      else if (F1 < 0.0 && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
+      T th = T(1.0);
+      if (F1 > T(0.0)) th = sh_th[isL ? (uint32_t)l : nb];
+      else if (F1 < T(0.0) && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
       F1 = th * F1; F3 = th * F3; G = th * G;       // theta = 1: the product is the factor itself, bit for bit
-      const double nxk = b_nx[e], nyk = b_ny[e], lenk = b_len[e];
+      const T nxk = b_nx[e], nyk = b_ny[e], lenk = b_len[e];
       // s * x with s = +-1 is x or -x exactly: a change of sign instead of a product
-      const double dH0 = lenk * F1, dX0 = lenk * (G * nxk - F3 * nyk), dY0 = lenk * (G * nyk + F3 * nxk);
-      const double dHk = isL ? dH0 : -dH0, dXk = isL ? dX0 : -dX0, dYk = isL ? dY0 : -dY0;
+      const T dH0 = lenk * F1, dX0 = lenk * (G * nxk - F3 * nyk), dY0 = lenk * (G * nyk + F3 * nxk);
+      const T dHk = isL ? dH0 : -dH0, dXk = isL ? dX0 : -dX0, dYk = isL ? dY0 : -dY0;
       if (k == 0) { dH = dHk; dX = dXk; dY = dYk; } else { dH = dH + dHk; dX = dX + dXk; dY = dY + dYk; }
-      if (kMorph) { const double dB0 = lenk * sh_qB[e]; const double dBk = isL ? dB0 : -dB0; dB = k == 0 ? dBk : dB + dBk; }
-      if (kScalars) {
+      if constexpr (kMorph) { const T dB0 = lenk * sh_qB[e]; const T dBk = isL ? dB0 : -dB0; dB = k == 0 ? dBk : dB + dBk; }
+      if constexpr (kScalars) {
         F1k[k] = F1; slk[k] = lenk;
         const uint32_t Lc = isL ? (uint32_t)l : nb, Rc = isL ? nb : (uint32_t)l;
         up[k] = (int)((F1 >= 0.0 || Rc == kPceNoNeighbour) ? Lc : Rc);   // ghost concentration = the interior cell's
@@ -547,52 +555,52 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
         const int aux = b_aux[e];
         if (aux <= -3) {
           A.string_M[(kSelf ? (size_t)(A.step_k & 1) * A.n_string_edges : (size_t)0) + (-3 - aux)] = lenk * F1;
-          if (kScalars && !(F1 >= 0.0) && A.strings[A.slot_string[-3 - aux]].type == kBcInflowQ) up[k] = -1 - (-3 - aux);
+          if (kScalars && !(F1 >= T(0.0)) && A.strings[A.slot_string[-3 - aux]].type == kBcInflowQ) up[k] = -1 - (-3 - aux);
         }
       }
     }
-    const double a = dt * invA;
-    double hn = c_own.h - a * dH;
-    if (hn < 0.0) {                                  // residual negatives (R-8b): clip and count
-      atomicAdd(&ctl->vol_clipped, -hn * b_area[l]);
-      hn = 0.0;
+    const T a = dt * invA;
+    T hn = c_own.h - a * dH;
+    if (hn < T(0.0)) {                                  // residual negatives (R-8b): clip and count
+      atomicAdd(&ctl->vol_clipped, (double)(-hn * b_area[l]));
+      hn = T(0.0);
     }
-    double qxn = 0.0, qyn = 0.0;
+    T qxn = T(0.0), qyn = T(0.0);
     if (hn > h_dry) {
       qxn = c_own.qx - a * dX;
       qyn = c_own.qy - a * dY;
-      if (f2 > 0.0) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
-        const double D = 1.0 + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_rn(hn));
+      if (f2 > T(0.0)) {   // R-5/R-6: exact integral of dq/dt = -(g/(k^2 h^(7/3))) |q| q over dt, h frozen at h^{n+1}
+        const T D = T(1.0) + ((dt * f2) * sqrt(qxn * qxn + qyn * qyn)) / ((hn * hn) * cbrt_rn(hn));
         qxn = qxn / D;
         qyn = qyn / D;
       }
       // Eq. 21 (R-7) of the new state, for the next dt: max_j lambda_ij / rho_ij
-      const double u = qxn / hn, v = qyn / hn;
-      const double cel = sqrt(g * hn);
+      const T u = qxn / hn, v = qyn / hn;
+      const T cel = sqrt(g * hn);
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
         const int e = w[k] & 0x7FFFu;
-        const double lam = fabs(u * b_nx[e] + v * b_ny[e]) + cel;
-        const double val = lam * ((0.75 * b_len[e]) * invA);
+        const T lam = fabs(u * b_nx[e] + v * b_ny[e]) + cel;
+        const T val = lam * ((T(0.75) * b_len[e]) * invA);
         if (val > rate) rate = val;
       }
     }
-    CellRec c = c_own;
+    Rec c = c_own;
     c.h = hn; c.qx = qxn; c.qy = qyn;
-    if (kMorph) c.z = c.z - A.mp.inv1mp * (a * dB);   // Eq. 13, S_b = 0
+    if constexpr (kMorph) c.z = c.z - A.mp.inv1mp * (a * dB);   // Eq. 13, S_b = 0
     out[i] = c;
-    nonzero |= (hn != 0.0) | (qxn != 0.0) | (qyn != 0.0);
-    if (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
+    nonzero |= (hn != T(0.0)) | (qxn != T(0.0)) | (qyn != T(0.0));
+    if constexpr (kScalars) {                                  // Eq. 20, advective part: A_ij = limited F1 x upwind phi (R-19)
       _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < n_sp) {
-        double dC = 0.0;
+        T dC = 0.0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-          const double phi = up[k] >= 0 ? sh_phi[sp * cap_loc + up[k]] : A.strings[A.slot_string[-1 - up[k]]].phi_in[sp];
-          const double lC = fabs(slk[k]) * (F1k[k] * phi);
-          const double Ck = slk[k] < 0.0 ? -lC : lC;
+          const T phi = up[k] >= 0 ? sh_phi[sp * cap_loc + up[k]] : A.strings[A.slot_string[-1 - up[k]]].phi_in[sp];
+          const T lC = fabs(slk[k]) * (F1k[k] * phi);
+          const T Ck = slk[k] < 0.0 ? -lC : lC;
           dC = k == 0 ? Ck : dC + Ck;
         }
-        const double qn = (src ? A.sc.qb[sp] : A.sc.qa[sp])[i] - a * dC;
+        const T qn = (src ? A.sc.qb[sp] : A.sc.qa[sp])[i] - a * dC;
         (src ? A.sc.qa[sp] : A.sc.qb[sp])[i] = qn;
         nonzero |= (qn != 0.0);
       }
@@ -607,20 +615,20 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   nonzero = __syncthreads_or(nonzero);
   publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(stage + L.s_nbr), (const int32_t *)(stage + L.s_nbr_slot), L.cap_nbr,
                          nonzero ? 0 : 1, *sm_dirty);
-  block_max_to_global<kThreads>(rate, kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits);
+  block_max_to_global<kThreads>((double)rate, kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits);
 }
 
 // flags after swe_set_state, two launches: (1) own flag of the buffer that holds the newest state from the records
 // (the other buffer: unknown = 0); (2) every patch works out its neighbour bytes from its halo cells
-template <int kThreads>
+template <int kThreads, typename T = double>
 __global__ void __launch_bounds__(kThreads)
 k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
   const int b = blockIdx.x, cell0 = b * A.L.P, n_own = min(A.L.P, A.n_cells - cell0);
-  const CellRec *__restrict__ rec = ctl->cur ? A.rec_b : A.rec_a;
+  const CellRecT<T> *__restrict__ rec = reinterpret_cast<const CellRecT<T> *>(ctl->cur ? A.rec_b : A.rec_a);
   int nonzero = 0;
   for (int l = threadIdx.x; l < n_own; l += kThreads) {
-    const CellRec c = rec[cell0 + l];
-    nonzero |= !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
+    const CellRecT<T> c = rec[cell0 + l];
+    nonzero |= !(c.h == T(0.0) && c.qx == T(0.0) && c.qy == T(0.0));
     _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < A.sc.n) nonzero |= ((ctl->cur ? A.sc.qb[sp] : A.sc.qa[sp])[cell0 + l] != 0.0);
   }
   nonzero = __syncthreads_or(nonzero);
@@ -632,7 +640,8 @@ k_patch2_own_flags(const Control *__restrict__ ctl, const Patch2Args A) {
 
 // one block per patch: neighbour byte j = 1 when every halo cell of this patch that the j-th neighbour owns is
 // (0, 0, 0) (and carries no scalar mass) in the newest state; the other buffer: unknown = 0
-static __global__ void __launch_bounds__(kBlock)
+template <typename T = double>
+__global__ void __launch_bounds__(kBlock)
 k_patch2_nbr_flags(const Control *__restrict__ ctl, const Patch2Args A, int n_patches) {
   const int p = blockIdx.x;
   if (p >= n_patches) return;
@@ -641,13 +650,13 @@ k_patch2_nbr_flags(const Control *__restrict__ ctl, const Patch2Args A, int n_pa
   const BlobHeader H = *reinterpret_cast<const BlobHeader *>(blob);
   const int32_t *nbr = (const int32_t *)(blob + A.L.off_nbr);
   const int32_t *halo_ids = (const int32_t *)(blob + A.L.off_halo_ids);
-  const CellRec *__restrict__ rec = ctl->cur ? A.rec_b : A.rec_a;
+  const CellRecT<T> *__restrict__ rec = reinterpret_cast<const CellRecT<T> *>(ctl->cur ? A.rec_b : A.rec_a);
   if (threadIdx.x == 0) s_dirty = 0u;
   __syncthreads();
   for (int l = threadIdx.x; l < H.n_r1 + H.n_r2; l += kBlock) {
     const int id = halo_ids[l];
-    const CellRec c = rec[id];
-    bool nz = !(c.h == 0.0 && c.qx == 0.0 && c.qy == 0.0);
+    const CellRecT<T> c = rec[id];
+    bool nz = !(c.h == T(0.0) && c.qx == T(0.0) && c.qy == T(0.0));
     _Pragma("unroll") for (int sp = 0; sp < kMaxSpecies; ++sp) if (sp < A.sc.n) nz = nz || ((ctl->cur ? A.sc.qb[sp] : A.sc.qa[sp])[id] != 0.0);
     if (!nz) continue;
     const int owner = id / A.L.P;

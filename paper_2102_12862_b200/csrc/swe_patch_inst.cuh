@@ -8,9 +8,11 @@ namespace swe {
 typedef void (*PatchKernel)(Control *, Patch2Args);
 
 // the instance of k_patch2<T, B, ...> for (scalar species on board, self-controlled step, mobile bed); the self-controlled
-// step (small meshes) is built for the plain hydrodynamic step only: nullptr otherwise
+// step (small meshes; self = 4 asks for the single-precision instance instead) is built for the plain hydrodynamic step only: nullptr otherwise
 template <int T, int B>
 inline PatchKernel patch_fn(int scalars, int self, int morph) {
+  if (self == 4)    // single precision (R-21): plain hydrodynamics behind k_step_control
+    return (scalars || morph) ? nullptr : (PatchKernel)k_patch2<T, B, false, false, false, float>;
   if (self) return (scalars || morph) ? nullptr : (PatchKernel)k_patch2<T, B, false, true, false>;
   if (scalars) return morph ? (PatchKernel)k_patch2<T, B, true, false, true> : (PatchKernel)k_patch2<T, B, true, false, false>;
   return morph ? (PatchKernel)k_patch2<T, B, false, false, true> : (PatchKernel)k_patch2<T, B, false, false, false>;

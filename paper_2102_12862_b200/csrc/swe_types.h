@@ -54,7 +54,8 @@ struct BlobLayout {
   int32_t cap_nbr, cap_halo, cap_r1, cap_c1, cap_loc, cap_e, cap_eown;
   int32_t off_nbr, off_nbr_slot, off_halo_ids, off_stage;
   // offsets RELATIVE TO off_stage (= offsets inside the staged copy in shared memory)
-  int32_t s_hdr, s_nbr, s_nbr_slot, s_halo_area, s_pce, s_nx, s_ny, s_len, s_lr, s_aux, s_area, s_gn2;
+  int32_t s_hdr, s_nbr, s_nbr_slot, s_halo_area, s_pce, s_nx, s_ny, s_len, s_lr, s_aux, s_area, s_gn2, s_inv_area;
+  int32_t rb;                    // bytes of a real in the staged arrays: 8, or 4 (single precision, R-21)
   int32_t stage_bytes;           // multiple of 16
   int32_t stride;                // bytes per blob, multiple of 128
 };
@@ -69,8 +70,9 @@ constexpr int kPflagBytes = 32, kPflagSlots = 30, kPflagOwn = 30, kPflagSkippabl
 
 __host__ __device__ inline int32_t blob_align(int32_t x, int32_t a) { return (x + a - 1) / a * a; }
 
-__host__ __device__ inline BlobLayout blob_layout(int P, int cap_nbr, int cap_halo, int cap_r1, int cap_e, int cap_eown) {
+__host__ __device__ inline BlobLayout blob_layout(int P, int cap_nbr, int cap_halo, int cap_r1, int cap_e, int cap_eown, int rb = 8) {
   BlobLayout L;
+  L.rb = rb;
   L.P = P; L.cap_nbr = cap_nbr; L.cap_halo = cap_halo; L.cap_r1 = cap_r1; L.cap_c1 = P + cap_r1; L.cap_loc = P + cap_halo;
   L.cap_e = cap_e; L.cap_eown = cap_eown;
   int32_t o = (int32_t)sizeof(BlobHeader);
@@ -83,17 +85,20 @@ __host__ __device__ inline BlobLayout blob_layout(int P, int cap_nbr, int cap_ha
   L.s_nbr = s; s += 4 * cap_nbr;
   L.s_nbr_slot = s; s += 4 * cap_nbr;
   s = blob_align(s, 8);
-  L.s_halo_area = s; s += 8 * cap_r1;
+  L.s_halo_area = s; s += rb * cap_r1;
   s = blob_align(s, 16);
   L.s_pce = s; s += 16 * L.cap_c1;
-  L.s_nx = s; s += 8 * cap_e;
-  L.s_ny = s; s += 8 * cap_e;
-  L.s_len = s; s += 8 * cap_e;
+  L.s_nx = s; s += rb * cap_e;
+  L.s_ny = s; s += rb * cap_e;
+  L.s_len = s; s += rb * cap_e;
   L.s_lr = s; s += 4 * cap_e;
   L.s_aux = s; s += 4 * cap_e;
   s = blob_align(s, 8);
-  L.s_area = s; s += 8 * P;
-  L.s_gn2 = s; s += 8 * P;
+  L.s_area = s; s += rb * P;
+  L.s_gn2 = s; s += rb * P;
+  // single precision: 1 / abs(Omega) is the host's fp64 quotient rounded once (R-21), so it is staged; the fp64 kernel
+  // forms the same IEEE quotient itself
+  L.s_inv_area = s; s += rb == 4 ? 4 * P : 0;
   L.stage_bytes = blob_align(s, 16);
   L.stride = blob_align(L.off_stage + L.stage_bytes, 128);
   return L;

@@ -40,12 +40,16 @@ def f32(x):
     return np.asarray(x, np.float64).astype(np.float32).astype(np.float64)
 
 
+@pytest.mark.parametrize("variant", [1, 2], ids=["three-pass", "patch"])
 @pytest.mark.parametrize("name", list(CASES))
-def test_parity_with_the_fp32_oracle(gpu, ref, name):
+def test_parity_with_the_fp32_oracle(gpu, ref, name, variant):
+    """Both step variants in fp32 (16-byte records; the fused patch step with 4-byte staged geometry) against the fp32
+    build of the oracle: bit-identical."""
     w = CASES[name]()
-    s = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE)
+    s = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, variant=variant, patch_cells=96 if variant == 2 else 0)
     o = ref.RefSolver(w, precision="single")
-    assert s.step_kernels() == ["k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"]
+    assert s.step_kernels() == (["k_step_control", "k_edge_flux", "k_theta_lazy", "k_cell_update"] if variant == 1
+                                else ["k_step_control", "k_patch_step"])
     for a, b in zip(s.geometry(), o.geometry()):
         assert np.array_equal(a, b)                                     # fp64 geometry rounded once to fp32, both sides
     assert s.peek_dt(w.cfl) == o.peek_dt(w.cfl)                         # fp32 rate, dt = cfl / rate in fp64
@@ -63,11 +67,46 @@ def test_parity_with_the_fp32_oracle(gpu, ref, name):
         assert abs(ig["vol"] - io["vol"]) <= 1e-12 * io["vol"]
         assert abs(ig["vol_in"] - io["vol_in"]) <= 1e-12 * max(1.0, io["vol_in"])
         assert abs(ig["vol_out"] - io["vol_out"]) <= 1e-9 * max(1.0, io["vol_out"])
-    F, Fo = s.edge_fluxes(), o.edge_fluxes()
-    for a, b in zip(F[:4], Fo):
-        assert np.array_equal(a, b)
+    if variant == 1:                                                    # (the fp32 patch step does not export its fluxes)
+        F, Fo = s.edge_fluxes(), o.edge_fluxes()
+        for a, b in zip(F[:4], Fo):
+            assert np.array_equal(a, b)
+    else:
+        with pytest.raises(RuntimeError, match="single-precision patch step"):
+            s.edge_fluxes()
     s.close()
     o.close()
+
+
+def test_fp32_variants_agree_and_auto_picks_the_patch_step(gpu, ref):
+    """AUTO in single precision: the fused patch step (default patch size, four blocks per SM) -- bit-identical to the
+    fp32 three-pass step and to the fp32 oracle over 150 steps of the river reach, dry patches skipped."""
+    w = CASES["config4-small"]()
+    a = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE)
+    b = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, variant=gpu.VARIANT_THREE_PASS)
+    o = ref.RefSolver(w, precision="single")
+    assert a.patch_stats()["variant"] == gpu.VARIANT_PATCH and a.step_kernels() == ["k_step_control", "k_patch_step"]
+    for n in (33, 117):
+        ia, ib, io = a.step(n, float("inf"), w.cfl), b.step(n, float("inf"), w.cfl), o.step(n, float("inf"), w.cfl)
+        for x, y, z in zip(a.get_state(), b.get_state(), o.get_state()):
+            assert np.array_equal(x, y) and np.array_equal(x, z)
+        assert ia["t"] == ib["t"] == io["t"] and ia["n_wet"] == ib["n_wet"] == io["n_wet"]
+        assert ia["vol_in"] == ib["vol_in"] and abs(ia["vol_out"] - ib["vol_out"]) <= 1e-12 * max(1.0, ib["vol_out"])
+    assert a.patch_stats()["patch_steps_skipped"] > 0
+    for s in (a, b):
+        s.close()
+    o.close()
+    # an all-wet state: in fp32 the three-pass step moves half the bytes and is the faster one -- AUTO takes it
+    w3 = CASES["config3-small"]()
+    c3 = gpu.from_workload(w3, precision=gpu.PRECISION_SINGLE)
+    o3 = ref.RefSolver(w3, precision="single")
+    assert c3.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS and len(c3.step_kernels()) == 4
+    c3.step(40, float("inf"), w3.cfl)
+    o3.step(40, float("inf"), w3.cfl)
+    for x, z in zip(c3.get_state(), o3.get_state()):
+        assert np.array_equal(x, z)
+    c3.close()
+    o3.close()
 
 
 def test_distance_to_the_fp64_oracle_and_mass(gpu, ref):
@@ -93,12 +132,12 @@ def test_distance_to_the_fp64_oracle_and_mass(gpu, ref):
 
 def test_single_precision_is_hydrodynamics_only(gpu):
     w = CASES["config3-small"]()
-    for kw in (dict(n_species=1), dict(morphology=True), dict(variant=2)):
+    for kw in (dict(n_species=1), dict(morphology=True)):
         with pytest.raises(RuntimeError, match="single precision"):
             gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, **kw)
-    s = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE)           # AUTO -> three-pass
+    s = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, variant=gpu.VARIANT_THREE_PASS)
     assert s.patch_stats()["variant"] == gpu.VARIANT_THREE_PASS
-    d = gpu.from_workload(w)
-    assert s.workspace_nbytes < 0.62 * d.workspace_nbytes              # 16-byte records, no patch tables
+    d = gpu.from_workload(w, variant=gpu.VARIANT_THREE_PASS)
+    assert s.workspace_nbytes < 0.66 * d.workspace_nbytes              # 16-byte records, 4-byte reals; the int32 tables stay
     s.close()
     d.close()
