@@ -746,6 +746,20 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     SWE_CUDA(c, cudaMemset(c->d_pflag, 0, 2 * (size_t)kPflagBytes * (size_t)c->n_patches));
     if (const char *s = std::getenv("SWE_PATCH_MIN_BLOCKS")) c->patch_force_blocks = std::atoi(s);
     c->patch_threads = patch_threads(pb.lay.P);
+    // small meshes whose patches are all resident at once are bound by the latency of one block's chain of phases: one
+    // thread per local EDGE instead of one per own cell makes phase 2 (about two edges per cell, each a dependent chain
+    // of square roots and a division) a single pass -- configs[0]: 8.7 -> 6.4 us per step (profiles/r2w_small_meshes.md)
+    {
+      int dev = 0, sms = 148;
+      SWE_CUDA(c, cudaGetDevice(&dev));
+      SWE_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      const int t_edges = pb.lay.cap_e <= 256 ? patch_threads(pb.lay.cap_e) : 0;   // (blocks of up to 256 threads: the instances with >= 4 blocks per SM)
+      if (t_edges > c->patch_threads && !c->patch_force_blocks) {
+        const size_t smem = (size_t)patch2_smem_layout(pb.lay, c->sc.n, pl.z.morph ? 2 : 0, true).total;
+        const PatchInst *pi = pick_patch_kernel(t_edges, smem, 0);
+        if (pi && (int64_t)c->n_patches <= (int64_t)sms * pi->min_blocks) c->patch_threads = t_edges;
+      }
+    }
     c->patch_prefetch = 4 * 148;              // about the blocks resident at a time
     if (const char *s = std::getenv("SWE_PATCH_PREFETCH")) c->patch_prefetch = std::atoi(s);
     // self-controlled steps: at most kCtlPre strings, each string's pairwise tree inside the block's scratch (the
