@@ -166,3 +166,29 @@ def test_config4_full_size_mobile_bed(gpu, ref):
     assert ig["flags"] == 0 and np.all(np.isfinite(s.get_bed()))
     s.close()
     o.close()
+
+
+def test_config4_full_size_single_precision(gpu, ref):
+    """configs[3] at full size in single precision (R-21), both step variants against the fp32 build of the oracle: all
+    cells bit-identical over a short window from the initial state and over a window started from the GPU's own state
+    after 600 more steps (AUTO: the fused fp32 patch step, 32 % of the cells wet)."""
+    ref.lib(single=True)
+    w = C.config4()
+    a = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE)
+    b = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, variant=gpu.VARIANT_THREE_PASS)
+    o = ref.RefSolver(w, precision="single")
+    assert a.step_kernels() == ["k_step_control", "k_patch_step"] and len(b.step_kernels()) == 4
+    ia, ib, io = a.step(15, float("inf"), w.cfl), b.step(15, float("inf"), w.cfl), o.step(15, float("inf"), w.cfl)
+    for x, y, z in zip(a.get_state(), b.get_state(), o.get_state()):
+        assert np.array_equal(x, z) and np.array_equal(y, z)
+    assert ia["t"] == ib["t"] == io["t"] and ia["n_wet"] == ib["n_wet"] == io["n_wet"]
+    b.close()
+    ia = a.step(600, float("inf"), w.cfl)
+    assert ia["flags"] == 0 and a.patch_stats()["patch_steps_skipped"] > 0
+    o.set_state(*a.get_state(), ia["t"])
+    a.step(10, float("inf"), w.cfl)
+    o.step(10, float("inf"), w.cfl)
+    for x, z in zip(a.get_state(), o.get_state()):
+        assert np.array_equal(x, z)
+    a.close()
+    o.close()
