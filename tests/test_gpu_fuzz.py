@@ -98,3 +98,25 @@ def test_random_case(gpu, ref, seed):
                 assert np.all(np.abs(qg[sp] - qo[sp]) <= 1e-10 * np.abs(qo[sp]) + 1e-14 * scale), f"seed {seed}, species {sp}"
     s.close()
     o.close()
+
+
+@pytest.mark.parametrize("seed", range(100, 110))
+def test_random_case_single_precision(gpu, ref, seed):
+    """The same random cases in single precision (R-21), both step variants with random patch sizes, against the
+    fp32 build of the oracle: bit-identical states (thin films, dry regions, fast flow, strings), fp64 clock."""
+    ref.lib(single=True)
+    w, rng = random_workload(seed)
+    variant = [gpu.VARIANT_THREE_PASS, gpu.VARIANT_PATCH][seed % 2]
+    pc = int(rng.choice([32, 64, 96, 160, 240])) if variant == gpu.VARIANT_PATCH else 0
+    s = gpu.from_workload(w, variant=variant, patch_cells=pc, precision=gpu.PRECISION_SINGLE,
+                          steps_per_graph=int(rng.choice([0, 4, 32])))
+    o = ref.RefSolver(w, precision="single")
+    for n in (1, int(rng.integers(2, 40)), int(rng.integers(2, 60))):
+        ig, io = s.step(n, float("inf"), w.cfl), o.step(n, float("inf"), w.cfl)
+        for nm, a, b in zip(("h", "hu", "hv"), s.get_state(), o.get_state()):
+            assert np.array_equal(a, b), (seed, nm, float(np.max(np.abs(a - b))))
+        assert ig["steps_done"] == io["steps_done"] and ig["n_wet"] == io["n_wet"] and ig["flags"] == io["flags"]
+        assert abs(ig["t"] - io["t"]) <= 1e-12 * abs(io["t"]) and abs(ig["dt_last"] - io["dt_last"]) <= 1e-12 * io["dt_last"]
+        assert abs(ig["vol"] - io["vol"]) <= 1e-12 * abs(io["vol"])
+    s.close()
+    o.close()
