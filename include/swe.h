@@ -86,8 +86,9 @@ typedef struct {
                            1: they take DEVICE pointers (e.g. torch tensors), read/written on stream  */
   int steps_per_graph;  /* time steps captured per CUDA graph launch; default 32; 0 = no graph       */
   int variant;          /* SWE_VARIANT_*; default AUTO                                               */
-  int patch_cells;      /* cells per patch of the fused step, 32..1024 (one thread per own cell);
-                           0 = default (256; less on meshes that would not fill the SMs)             */
+  int patch_cells;      /* cells per patch of the fused step, 32..1024 (at least one thread per own cell);
+                           0 = default (the largest of 240..192 that runs four blocks per SM; less
+                           on meshes that would not fill the SMs)                                    */
   int n_species;        /* passive scalar species advected with the flow (0..5); default 0    */
   int morphology;       /* 1: reserve room for the mobile-bed module (swe_set_morphology); default 0 */
   int precision;        /* SWE_PRECISION_*; default DOUBLE                                           */
