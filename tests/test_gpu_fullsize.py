@@ -29,6 +29,16 @@ def gpu():
     return P
 
 
+_CONFIG4 = []
+
+
+def config4_full():
+    """configs[3] at full size, generated once for the three tests that step it (50 s each time; nobody writes to it)."""
+    if not _CONFIG4:
+        _CONFIG4.append(C.config4())
+    return _CONFIG4[0]
+
+
 def window(s, o, w, n, what):
     ig = s.step(n, float("inf"), w.cfl)
     io = o.step(n, float("inf"), w.cfl)
@@ -46,7 +56,7 @@ def test_config4_full_size_windows(gpu, ref):
     """SURVEY section 8(d) parity windows on configs[3] at full size, all cells: 100 steps from the initial state, and
     100-step windows started from the GPU's own states at steps 1000 and 4000 (get_state -> oracle set_state), where
     the flood wave has wetted part of the floodplain."""
-    w = C.config4()
+    w = config4_full()
     assert 3.8e6 < w.n_cells < 4.2e6
     s = make(gpu, w)
     o = ref.RefSolver(w)
@@ -149,7 +159,7 @@ def test_config4_full_size_mobile_bed(gpu, ref):
     """configs[3] at full size with the morphodynamic module on (R-20; MPM-like law, d_m = 5 mm): every cell's state and
     bed elevation and every edge's q_Bij against the oracle over a short window; a cell no water ever reached keeps its
     bed (property that holds at any size)."""
-    w = C.config4()
+    w = config4_full()
     s = make(gpu, w, morphology=True)
     o = ref.RefSolver(w)
     morph = (2, 8.0, 0.047, 2.65, 0.005, 0.4)
@@ -173,7 +183,7 @@ def test_config4_full_size_single_precision(gpu, ref):
     cells bit-identical over a short window from the initial state and over a window started from the GPU's own state
     after 600 more steps (AUTO: the fused fp32 patch step, 32 % of the cells wet)."""
     ref.lib(single=True)
-    w = C.config4()
+    w = config4_full()
     a = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE)
     b = gpu.from_workload(w, precision=gpu.PRECISION_SINGLE, variant=gpu.VARIANT_THREE_PASS)
     o = ref.RefSolver(w, precision="single")
