@@ -96,9 +96,10 @@ inline int grid_for(int64_t n) { return (int)((n + kBlock - 1) / kBlock); }
 // blocks per SM chosen from what the shared memory admits (it only caps the registers)
 // (T threads per block >= cells per patch, __launch_bounds__ minimum blocks per SM, getter of the instance for
 // [scalars][self-controlled][mobile bed]; the instances live in swe_patch_t*.cu, one translation unit per block size)
-struct PatchInst { int T, min_blocks; PatchKernel (*get)(int B, int scalars, int self, int morph); };
+struct PatchInst { int T, min_blocks; PatchKernel (*get)(int B, int scalars, int self, int morph); bool f32_only = false; };
 const PatchInst kPatchInst[] = {{32, 8, patch_kernel_32}, {64, 8, patch_kernel_64}, {128, 6, patch_kernel_128}, {128, 4, patch_kernel_128},
-                                {192, 5, patch_kernel_192}, {192, 4, patch_kernel_192}, {192, 3, patch_kernel_192}, {256, 4, patch_kernel_256}, {256, 3, patch_kernel_256},
+                                {192, 5, patch_kernel_192}, {192, 4, patch_kernel_192}, {192, 3, patch_kernel_192},
+                                {256, 6, patch_kernel_256, true}, {256, 5, patch_kernel_256, true}, {256, 4, patch_kernel_256}, {256, 3, patch_kernel_256},
                                 {256, 2, patch_kernel_256}, {384, 2, patch_kernel_384}, {384, 1, patch_kernel_384}, {512, 2, patch_kernel_512}, {512, 1, patch_kernel_512},
                                 {1024, 1, patch_kernel_1024}};
 
@@ -109,17 +110,17 @@ inline int patch_threads(int P) {           // the smallest block size of an ins
 }
 
 // the instantiation with the most blocks per SM that the shared memory of one block admits (force_blocks > 0: that one)
-inline const PatchInst *pick_patch_kernel(int T, size_t smem, int force_blocks) {
+inline const PatchInst *pick_patch_kernel(int T, size_t smem, int force_blocks, bool single = false) {
   const int fit = (int)(kSmemPerSM / (smem + kSmemBlockReserve));
   const PatchInst *best = nullptr;
   for (const PatchInst &pi : kPatchInst) {
-    if (pi.T != T) continue;
+    if (pi.T != T || (pi.f32_only && !single)) continue;
     if (force_blocks > 0) { if (pi.min_blocks == force_blocks) return &pi; continue; }
     if (pi.min_blocks <= std::max(1, fit) && (!best || pi.min_blocks > best->min_blocks)) best = &pi;
   }
   if (!best)
     for (const PatchInst &pi : kPatchInst)
-      if (pi.T == T && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
+      if (pi.T == T && !(pi.f32_only && !single) && (!best || pi.min_blocks < best->min_blocks)) best = &pi;
   return best;
 }
 
@@ -294,7 +295,7 @@ void launch_patch(swe_ctx *c, cudaStream_t s, int self) {
   // (76 instead of 64 registers at 256 threads) is the faster one per block (configs[1]: 10.4 vs 11.8 us per step)
   int force = c->patch_force_blocks;
   if (!force && c->patch_threads == 256 && c->n_patches <= 3 * c->sms) force = 3;
-  const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, force);
+  const PatchInst *pi = pick_patch_kernel(c->patch_threads, smem, force, c->single);
   pi->get(pi->min_blocks, c->sc.n > 0, c->single ? 4 : self, morph != 0)<<<c->n_patches, c->patch_threads, smem, s>>>(c->d_ctl, patch_args(c));
 }
 
@@ -570,11 +571,15 @@ int make_plan(const swe_mesh *mesh, const swe_params &p, bool emit, Plan &pl, st
     if (P <= 0 && nc < 148 * 256) P = nc < 148 * 64 ? 32 : (nc < 148 * 128 ? 64 : 128);
     if (P <= 0) {
       const bool self = false;               // (meshes of this size do not run the self-controlled step)
-      for (int cand : {240, 232, 224, 208, 192}) {
+      // (single precision: 34-36 KB per block and 40 registers -- six blocks per SM, patches of up to 256 cells:
+      // 95.5 us per step on the river reach against 107.9 at four blocks of 240 cells, profiles/r2u_single_precision.md)
+      const int blocks_wanted = pl.z.single ? 6 : 4;
+      for (int cand : {256, 248, 240, 232, 224, 208, 192}) {
+        if (cand > 240 && !pl.z.single) continue;
         P = cand;
         if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, false, pl.pb, err, rb)) return SWE_EINVAL;
         const size_t smem = (size_t)patch2_smem_layout(pl.pb.lay, p.n_species, 0, self && nc / P <= 8192).total;
-        if (4 * (smem + kSmemBlockReserve) <= kSmemPerSM) break;
+        if (blocks_wanted * (smem + kSmemBlockReserve) <= kSmemPerSM) break;
       }
     }
     if (!build_blobs(nc, ne, pl.geom, pl.ce4, pl.area, pl.inv_area, pl.gn2, string_pos, P, emit, pl.pb, err, rb)) return SWE_EINVAL;
@@ -777,7 +782,7 @@ int create_impl(const swe_mesh *mesh, const swe_params *params, swe_ctx *c) {
     }
     c->patch_smem = (size_t)patch2_smem_layout(pb.lay, c->sc.n, 0, c->self_ctl).total;
     {
-      const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->patch_smem, c->patch_force_blocks);
+      const PatchInst *pi = pick_patch_kernel(c->patch_threads, c->patch_smem, c->patch_force_blocks, c->single);
       if (!pi) { c->err = "no patch kernel instance for this patch size"; return SWE_EINVAL; }
       c->patch_min_blocks = pi->min_blocks;
     }
@@ -969,8 +974,8 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     // with four blocks of the patch kernel per SM it is the faster step at any wet fraction (all-wet 4M: 259.6 vs 266.1 us,
     // 8M: 508 vs 521 us; profiles/r2q_patch_size_sweep.md); with fewer (fat halos, scalar species, large patch_cells) the
     // round-1 crossover holds: three-pass from ~50 % wet cells on (profiles/r1i_auto_threshold.md)
-    // (single precision: the three-pass step moves half the bytes and wins on all-wet states, 27.5 vs 20.6 G at 8M cells;
-    // the patch step wins while part of the domain is dry, 36.6 vs 29.0 G on the river reach: profiles/r2u_single_precision.md)
+    // (single precision: the three-pass step moves half the bytes and wins on all-wet states, 27.6 vs 23.3 G at 8M cells;
+    // the patch step wins while part of the domain is dry, 41.5 vs 29.2 G on the river reach: profiles/r2u_single_precision.md)
     const int want = ((c->single || c->patch_min_blocks < 4) && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
       if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
