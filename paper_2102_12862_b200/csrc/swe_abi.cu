@@ -1421,6 +1421,30 @@ int swe_host_preprocess(const swe_mesh *mesh, int renumber_mode, int patch_cells
             if ((isL ? Ll : Rl) != (uint32_t)l || (isL ? Rl : Ll) != nb) { g_create_error = "patch blob: slot word and edge record disagree"; return SWE_EINVAL; }
           }
       }
+      // the reader masks (fourth word of an own cell's slot record: bit j = the j-th neighbour patch reads the cell; the exact
+      // skip flags rest on them): every halo entry of every patch has its bit in the owner's mask, and there are no others
+      int64_t halo_entries = 0, mask_bits = 0;
+      for (int64_t p = 0; p < pb.n_patches; ++p) {
+        const unsigned char *B = pb.bytes.data() + (size_t)BL.stride * (size_t)p;
+        const BlobHeader *h = (const BlobHeader *)B;
+        const int32_t *halo = (const int32_t *)(B + BL.off_halo_ids);
+        for (int32_t j = 0; j < h->n_r1 + h->n_r2; ++j) {
+          const int64_t cidx = halo[j], o = cidx / patch_cells;
+          const unsigned char *Bo = pb.bytes.data() + (size_t)BL.stride * (size_t)o;
+          const BlobHeader *ho = (const BlobHeader *)Bo;
+          const int32_t *nbr_o = (const int32_t *)(Bo + BL.off_nbr);
+          int32_t slot = -1;
+          for (int32_t k = 0; k < ho->n_nbr; ++k) if (nbr_o[k] == (int32_t)p) { slot = k; break; }
+          if (slot < 0) { g_create_error = "patch blob: a patch reads a cell of a patch that does not list it as a neighbour"; return SWE_EINVAL; }
+          if (slot >= 32) continue;
+          ++halo_entries;
+          const uint32_t *pce_o = (const uint32_t *)(Bo + BL.off_stage + BL.s_pce);
+          if (!((pce_o[4 * (cidx - o * patch_cells) + 3] >> slot) & 1u)) { g_create_error = "patch blob: reader mask misses a neighbour that reads the cell"; return SWE_EINVAL; }
+        }
+        const uint32_t *pce = (const uint32_t *)(B + BL.off_stage + BL.s_pce);
+        for (int32_t l = 0; l < h->n_own; ++l) mask_bits += __builtin_popcount(pce[4 * l + 3]);
+      }
+      if (mask_bits != halo_entries) { g_create_error = "patch blob: reader masks name neighbours that do not read the cell"; return SWE_EINVAL; }
       if (hdr_loc != pb.sum_loc || hdr_e != pb.sum_e) { g_create_error = "patch blob: headers disagree with the capacity pass"; return SWE_EINVAL; }
       v[1] = pb.n_patches; v[2] = pb.sum_loc; v[3] = pb.sum_e; v[4] = pb.max_loc; v[5] = pb.max_e;
       v[6] = (int64_t)patch2_smem_layout(pb.lay, 0).total;
