@@ -52,7 +52,7 @@ enum { SWE_VARIANT_AUTO = 0, SWE_VARIANT_THREE_PASS = 1 /* edge flux -> theta ->
 /* Arithmetic ("single or double"; R-21).  SINGLE: state, geometry and every flux / update operation in
  * fp32 (16-byte records); time, dt = CFL / rate, the hydrograph lookup and the volume bookkeeping stay fp64; built for the
  * hydrodynamic step only (SWE_EINVAL with scalars or mobile bed), in both step variants; AUTO: fused patch step below
- * 50 % wet cells, three-pass step above (it moves half the bytes in fp32 and wins on all-wet states).  swe_get_edge_flux
+ * 75 % wet cells, three-pass step above (it moves half the bytes in fp32 and wins on all-wet states).  swe_get_edge_flux
  * is not built for the single-precision patch step.  The arrays at this boundary stay fp64 in both cases (rounded once
  * on the way in, exact on the way out). */
 enum { SWE_PRECISION_DOUBLE = 0, SWE_PRECISION_SINGLE = 1 };

@@ -976,7 +976,10 @@ int swe_set_state(swe_ctx *c, const double *h, const double *hu, const double *h
     // round-1 crossover holds: three-pass from ~50 % wet cells on (profiles/r1i_auto_threshold.md)
     // (single precision: the three-pass step moves half the bytes and wins on all-wet states, 27.6 vs 23.3 G at 8M cells;
     // the patch step wins while part of the domain is dry, 41.5 vs 29.2 G on the river reach: profiles/r2u_single_precision.md)
-    const int want = ((c->single || c->patch_min_blocks < 4) && (double)c->h_ctl->n_wet > 0.5 * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
+    // the crossover: 50 % wet cells in fp64 with fat patches (round 1), 75 % in single precision (71 % wet: 78.8 vs 80.3 us,
+    // 85 % wet: 88.0 vs 81.8 us at 2M cells)
+    const double wet_limit = c->single ? 0.75 : 0.5;
+    const int want = ((c->single || c->patch_min_blocks < 4) && (double)c->h_ctl->n_wet > wet_limit * (double)nc) ? SWE_VARIANT_THREE_PASS : SWE_VARIANT_PATCH;
     if (want != c->variant) {
       if (want == SWE_VARIANT_THREE_PASS && c->h_ctl->cur == 1)      // scalars set earlier live in buffer b: move them
         for (int sp = 0; sp < c->sc.n; ++sp)
@@ -1056,7 +1059,7 @@ int swe_step(swe_ctx *c, int64_t n_steps, double t_end, double cfl, swe_step_inf
     if (c->auto_mode) {   // the wet count is known here: follow a flood that spreads (or recedes), with hysteresis
       const double wet = (double)h.n_wet / (double)c->nc;
       const int want = (c->patch_min_blocks >= 4 && !c->single) ? SWE_VARIANT_PATCH
-                                                : (wet > 0.55 ? SWE_VARIANT_THREE_PASS : (wet < 0.45 ? SWE_VARIANT_PATCH : c->variant));
+                                                : (wet > (c->single ? 0.80 : 0.55) ? SWE_VARIANT_THREE_PASS : (wet < (c->single ? 0.70 : 0.45) ? SWE_VARIANT_PATCH : c->variant));
       rc = switch_variant(c, want, h.cur);
       if (rc != SWE_OK) return rc;
     }
