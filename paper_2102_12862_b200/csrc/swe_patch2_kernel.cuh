@@ -209,8 +209,10 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   const int32_t *__restrict__ halo_ids = (const int32_t *)(blob + L.off_halo_ids);
 
   // ---- everything whose address depends on blockIdx alone is requested at once (one memory latency for all of it):
-  // the control block, this patch's flag word in BOTH state buffers (which one is read depends on Control::src), the
-  // first halo ids of every thread, and the flag words of the patch whose tables this block pulls into L2 (below)
+  // the control block, this patch's flag word in BOTH state buffers (which one is read depends on Control::src) and
+  // the flag words of the patch whose tables this block pulls into L2 (below).  The first halo ids of every thread
+  // used to be among them: a block that is skipped then waits for a DRAM access it has no use for before it can
+  // leave (its blob is in nobody's L2), so they are fetched behind the skip test (profiles/r2aa_contention.md)
   const ulonglong2 *pfa = reinterpret_cast<const ulonglong2 *>(A.pflag_a + (size_t)b * kPflagBytes);
   const ulonglong2 *pfb = reinterpret_cast<const ulonglong2 *>(A.pflag_b + (size_t)b * kPflagBytes);
   StepSlot S0;
@@ -219,8 +221,6 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   if (kSelf) { S0 = ctl->slot[A.step_k]; active = 0; src = S0.src; dt = T(0.0); }
   else { active = ctl->active; src = ctl->src; dt = (T)ctl->dt; }
   const ulonglong2 fa0 = pfa[0], fa1 = pfa[1], fb0 = pfb[0], fb1 = pfb[1];
-  const int hid0 = tid < L.cap_halo ? halo_ids[tid] : -1;
-  const int hid1 = tid + kThreads < L.cap_halo ? halo_ids[tid + kThreads] : -1;
   const int b_pf = b + A.prefetch_dist;            // the block that will run in this block's slot next (about)
   const bool do_pf = A.prefetch_dist > 0 && b_pf < (int)gridDim.x && tid == 0;
   ulonglong2 ga0, ga1, gb0, gb1;
@@ -282,6 +282,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     }
   }
 
+  const int hid0 = tid < L.cap_halo ? halo_ids[tid] : -1;
+  const int hid1 = tid + kThreads < L.cap_halo ? halo_ids[tid + kThreads] : -1;
   const int morph = kMorph ? A.mp.formula : 0;
   const Patch2Smem S = patch2_smem_layout(L, n_sp, morph, kSelf);
   T *sh_qB = (T *)(smraw + S.qB), *sh_fcx = (T *)(smraw + S.fcx), *sh_fcy = (T *)(smraw + S.fcy);
@@ -612,10 +614,26 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const uint32_t warp_dirty = __reduce_or_sync(0xffffffffu, mine);
     if ((tid & 31) == 0 && warp_dirty) atomicOr(sm_dirty, warp_dirty);
   }
+  // block maximum of the rate (non-negative doubles order like their bit patterns): per warp two 32-bit REDUX (high
+  // words, then the low words of the lanes that hold the maximal high word) before the barrier that the flag needs
+  // anyway, the warps' results by the first warp after it -- no barrier of its own, no shuffle chain at the block's tail
+  __shared__ unsigned long long warp_rate[kThreads / 32];
+  {
+    const unsigned long long rb = (unsigned long long)__double_as_longlong((double)rate);
+    const uint32_t hi = (uint32_t)(rb >> 32), mhi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? (uint32_t)rb : 0u);
+    if ((tid & 31) == 0) warp_rate[tid >> 5] = ((unsigned long long)mhi << 32) | mlo;
+  }
   nonzero = __syncthreads_or(nonzero);
   publish_flag<kThreads>(pf_out_base, b, (const int32_t *)(stage + L.s_nbr), (const int32_t *)(stage + L.s_nbr_slot), L.cap_nbr,
                          nonzero ? 0 : 1, *sm_dirty);
-  block_max_to_global<kThreads>((double)rate, kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits);
+  if (tid < 32) {
+    const unsigned long long rb = tid < kThreads / 32 ? warp_rate[tid] : 0ull;
+    const uint32_t hi = (uint32_t)(rb >> 32), mhi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? (uint32_t)rb : 0u);
+    const unsigned long long m = ((unsigned long long)mhi << 32) | mlo;
+    if (tid == 0 && m != 0ull) atomicMax(kSelf ? &ctl->slot[(A.step_k + 1) & 3].rate_bits : &ctl->rate_bits, m);
+  }
 }
 
 // flags after swe_set_state, two launches: (1) own flag of the buffer that holds the newest state from the records

@@ -4,6 +4,7 @@
 // cell->edge) is a 32-byte, 32-byte-aligned record = exactly one DRAM/L2 sector, moved by one 256-bit
 // LDG/STG.  Arrays that are only ever streamed by their own index (area, 1/area, g/k^2, theta) are plain SoA.
 #pragma once
+#include <cstddef>
 #include <cstdint>
 
 namespace swe {
@@ -150,9 +151,10 @@ struct StepSlot {
 };
 
 struct Control {                 // device-side step-loop state: nothing of it is read by the host per step
+  // first 128-byte line: what the kernels of a step only read (every block of the fused patch step fetches active, src,
+  // dt, g, h_dry from it when it starts)
   double t, dt, t_end, cfl, dt_max, g, h_dry;
-  double dt_last, vol_in, vol_out, vol_clipped;
-  unsigned long long rate_bits;  // bit pattern of max_i max_j lambda_ij/rho_ij of the CURRENT state (>= 0)
+  double dt_last, vol_in, vol_out;
   long long steps_left;          // < 0: unlimited
   long long steps_done;
   int32_t active;                // 1: the kernels of this step do work; 0: they return at once
@@ -164,7 +166,12 @@ struct Control {                 // device-side step-loop state: nothing of it i
   int32_t src;                   // state buffer the step in flight reads (it writes src ^ ping_pong)
   int32_t ping_pong;             // 1: fused patch step (two state buffers); 0: in-place three-pass step
   int32_t pad2_;
+  // second line: the words the blocks of a step update atomically -- kept off the line above, which every starting
+  // block reads while the finishing ones send their atomics
+  double vol_clipped;
+  unsigned long long rate_bits;  // bit pattern of max_i max_j lambda_ij/rho_ij of the CURRENT state (>= 0)
   unsigned long long patches_skipped;   // fused patch step: blocks that found their whole patch dry, since swe_create
+  unsigned long long pad_line_[13];
   // swe_step_info reductions (k_info)
   double vol;
   long long n_wet;
@@ -176,5 +183,7 @@ struct Control {                 // device-side step-loop state: nothing of it i
   // swe_step copies the classic fields above into a slot when it starts and back when it ends.
   StepSlot slot[4];
 };
+
+static_assert(offsetof(Control, vol_clipped) == 128 && offsetof(Control, vol) == 256, "Control: one line read, one line of atomics");
 
 }  // namespace swe
