@@ -297,8 +297,9 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
 
   // ---- the two bulk copies: staged part of the blob, own cell records
   uint32_t *sm_dirty = reinterpret_cast<uint32_t *>(smraw + 16);   // neighbours that read a wet own cell (phase 4)
+  uint32_t *sm_marked = reinterpret_cast<uint32_t *>(smraw + 20);  // phase 2 marked a donor cell for phase 3
   if (tid == 0) {
-    *sm_dirty = 0u;
+    *sm_dirty = 0u; *sm_marked = 0u;
     mbar_init(bar, 1);
     mbar_expect_tx(bar, (uint32_t)L.stage_bytes + (uint32_t)sizeof(Rec) * (uint32_t)n_own);
     bulk_g2s(stage, blob + L.off_stage, (uint32_t)L.stage_bytes, bar);
@@ -482,7 +483,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     if (d < n_c1) {
       const T ad = d < n_own ? b_area[d] : b_halo_area[d - n_own];
       const T hd = d == q.Lc ? q.hL : q.hR;
-      if (dt * (q.len * fabs(o.F1)) > T(0.3) * (hd * ad)) sh_th[d] = -T(1.0);
+      if (dt * (q.len * fabs(o.F1)) > T(0.3) * (hd * ad)) { sh_th[d] = -T(1.0); *sm_marked = 1u; }
     }
   };
   for (int e = tid; e < n_e; e += kThreads) {
@@ -490,10 +491,12 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     const Flux o = flux_edge(q, e);
     store_edge(q, e, o);
   }
-  __syncthreads();
 
   // ---- phase 3 (R-8b): theta_i = min(1, h_i |Omega_i| / (dt * sum of the outgoing l F1)), slots in order -- for the
-  // cells marked in phase 2 only
+  // cells marked in phase 2 only; a block that marked none (the rule away from wet/dry fronts) goes on to phase 4
+  // without the pass over the cells and its barrier
+  __syncthreads();
+  if (*sm_marked) {
   for (int l = tid; l < n_c1; l += kThreads) {
     if (sh_th[l] >= T(0.0)) continue;
     const uint4 pc = b_pce[l];
@@ -512,6 +515,7 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
     sh_th[l] = th;
   }
   __syncthreads();
+  }
 
   // ---- phase 4: own cells, one per thread
   T rate = T(0.0);
