@@ -140,8 +140,7 @@ struct Morph {                   // morphodynamics (section 3.2 Eq. 3, section 4
   double *qB;                    // [n_edges] normal sediment flux q_Bij of the step in flight
 };
 
-struct alignas(128) StepSlot {    // a line of its own: every block reads slot[n % 4] while the blocks that finish send
-                                  // their rate atomics to slot[(n + 1) % 4]
+struct StepSlot {
   double t, dt_last, vol_in, vol_out;
   unsigned long long rate_bits;  // max rate of the state this slot describes
   long long steps_left, steps_done;
