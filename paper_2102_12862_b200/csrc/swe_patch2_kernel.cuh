@@ -496,7 +496,8 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
   // cells marked in phase 2 only; a block that marked none (the rule away from wet/dry fronts) goes on to phase 4
   // without the pass over the cells and its barrier
   __syncthreads();
-  if (*sm_marked) {
+  const bool any_marked = *sm_marked != 0u;
+  if (any_marked) {
   for (int l = tid; l < n_c1; l += kThreads) {
     if (sh_th[l] >= T(0.0)) continue;
     const uint4 pc = b_pce[l];
@@ -541,10 +542,12 @@ k_patch2(Control *__restrict__ ctl, const Patch2Args A) {
       T F1 = sh_F1[e], F3 = sh_F3[e];
       T G = isL ? sh_GL[e] : sh_GR[e];
       // limiter: every component of the edge is scaled by theta of the donor cell (the one F1 leaves)
-      T th = T(1.0);
-      if (F1 > T(0.0)) th = sh_th[isL ? (uint32_t)l : nb];
-      else if (F1 < T(0.0) && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
-      F1 = th * F1; F3 = th * F3; G = th * G;       // theta = 1: the product is the factor itself, bit for bit
+      if (any_marked) {                             // no donor marked in this block: every theta is 1, x * 1 = x bit for bit
+        T th = T(1.0);
+        if (F1 > T(0.0)) th = sh_th[isL ? (uint32_t)l : nb];
+        else if (F1 < T(0.0) && nb != kPceNoNeighbour) th = sh_th[isL ? nb : (uint32_t)l];
+        F1 = th * F1; F3 = th * F3; G = th * G;     // theta = 1: the product is the factor itself, bit for bit
+      }
       const T nxk = b_nx[e], nyk = b_ny[e], lenk = b_len[e];
       // s * x with s = +-1 is x or -x exactly: a change of sign instead of a product
       const T dH0 = lenk * F1, dX0 = lenk * (G * nxk - F3 * nyk), dY0 = lenk * (G * nyk + F3 * nxk);
